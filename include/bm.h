@@ -1,0 +1,153 @@
+/*
+ * bm.h -- C ABI of the B200-native grouped MoE-layer forward pass (BrownoutMoE full-brownout path).
+ *
+ * The operation (PAPER.md = /root/reference/PAPER.md, "P:NN" = line NN; readings A1..A14 = DESIGN.md):
+ *   P:42   MoE layer with E experts and top-K routing:  h_t = sum_{i<=K} g_i(x_t) * FFN_i(x_t),
+ *          g_i the gating score.
+ *   P:46   united experts / full brownout: every routed expert e is served by the united expert of its
+ *          group, "reducing the number of experts loaded during inference".
+ *   P:118-122 (Eq. 2): the group map g: expert -> group decides which united expert handles the
+ *          tokens originally routed to each expert.
+ *   BASELINE.json north_star: bm_route(x, W_router, k, group_map) and
+ *          bm_moe_forward(x, routing, united W1/W3/W2, out).
+ *
+ * Conventions
+ *   - bf16 values are passed as uint16_t storage (bm_bf16).  Row-major, innermost dimension last.
+ *   - Every pointer is a DEVICE pointer unless its comment says HOST.  The caller owns all memory;
+ *     the library never allocates, frees or synchronises (except bm_moe_layer_host and
+ *     bm_device_status, which say so) and borrows the buffers until the work enqueued on `stream`
+ *     has completed.  All device pointers must be 16-byte aligned.
+ *   - `stream` is a cudaStream_t (0 = the legacy default stream).
+ *   - Return value: BM_OK (0) or a negative bm_status, checked synchronously on the host before
+ *     anything is enqueued.  T == 0 is BM_OK and a no-op.  Data-dependent faults (a group_map entry
+ *     outside [0,G), a non-finite router logit) cannot be seen without a sync: kernels raise a bit in a
+ *     device status word inside the workspace (read it with bm_device_status); the outputs are then
+ *     unspecified but all indices written stay in range.
+ *   - There is no CPU fallback: without a CUDA device of compute capability 10.0 every compute entry
+ *     point returns BM_ERR_CUDA.
+ */
+#ifndef BM_H_
+#define BM_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef uint16_t bm_bf16;
+typedef struct CUstream_st *bm_stream_t;
+
+typedef enum bm_status {
+    BM_OK = 0,
+    BM_ERR_NULL = -1,      /* a required pointer is NULL */
+    BM_ERR_SHAPE = -2,     /* K<1, K>E, K>BM_MAX_K, E>BM_MAX_E, G<1, G>BM_MAX_G, T<0, D%8, F%8, D<8, F<8, S<0 */
+    BM_ERR_ALIGN = -3,     /* a device pointer is not 16-byte aligned */
+    BM_ERR_WORKSPACE = -4, /* workspace_bytes < bm_workspace_bytes(...) */
+    BM_ERR_CUDA = -5,      /* no sm_100 device, driver entry point missing, or a launch failed */
+    BM_ERR_PATH = -6       /* forced path cannot run this shape (bm_moe_forward_path) */
+} bm_status;
+
+enum { BM_MAX_E = 512, BM_MAX_K = 16, BM_MAX_G = 512 };
+
+/* bits of the device status word */
+enum { BM_DEV_BAD_GROUP_MAP = 1, BM_DEV_NONFINITE_LOGIT = 2, BM_DEV_BAD_ROUTING = 4 };
+
+/* execution path of bm_moe_forward_path */
+enum {
+    BM_PATH_AUTO = 0,    /* T <= BM_DECODE_MAX_T -> DECODE, else PREFILL */
+    BM_PATH_DECODE = 1,  /* weight-streaming, weights on the MMA M side (small M; HBM-bound)   */
+    BM_PATH_PREFILL = 2, /* 128-token x 256-column tcgen05 tiles (large M; tensor-pipe-bound)  */
+    BM_PATH_SIMT = 3     /* plain CUDA-core kernels; a debugging cross-check, never picked by AUTO */
+};
+enum { BM_DECODE_MAX_T = 256 };
+
+/*
+ * Routing of one batch: the result of steps R1-R7.  A host struct of device
+ * arrays, every array allocated by the caller at its maximum size.  A = offsets[G] <= T*K is the
+ * number of (token, group) assignments after dedup.
+ */
+typedef struct bm_routing {
+    int32_t T, E, K, G;   /* filled by bm_route (host values) */
+    int32_t *expert_ids;  /* [T,K]  ranked top-K expert indices (rank 0 = largest logit; ties -> lower index) */
+    int32_t *group_ids;   /* [T,K]  distinct groups of the token in first-occurrence (rank) order, -1 padded  */
+    float *gate_w;        /* [T,K]  merged gate weights (softmax over the K selected logits, summed per group), 0 padded */
+    int32_t *n_slots;     /* [T]    number of distinct groups, 1..K */
+    int32_t *counts;      /* [G]    rows per group */
+    int32_t *offsets;     /* [G+1]  exclusive scan of counts; offsets[G] = A */
+    int32_t *row_token;   /* [T*K]  token of permuted row r (rows ordered by group, then token ascending); -1 for r >= A */
+    int32_t *row_slot;    /* [T*K]  slot s of permuted row r; -1 for r >= A */
+    int32_t *slot_row;    /* [T,K]  inverse permutation: row of (token, slot); -1 padded */
+} bm_routing;
+
+/* Bytes of scratch both calls need for shapes up to T_max tokens (independent of the data). HOST call. */
+size_t bm_workspace_bytes(int T_max, int D, int F, int E, int K, int G, int S);
+
+/*
+ * bm_route -- steps R1-R7: router logits in fp32 with the canonical summation order (A1), top-K with
+ * lower-index tie-break (A4), softmax over the selected logits (A2), group remap (Eq. 2), dedup with
+ * summed weights (A5, A6), per-group histogram, exclusive scan and the stable permutation (A7).
+ * Cite: P:42 (gate, top-K), P:118-122 + P:247 (group map).
+ *   x            [T,D]  bf16 tokens
+ *   W_router     [E,D]  bf16
+ *   router_bias  [E]    f32, added once after the reduction; NULL = none
+ *   group_map    [E]    i32, values in [0,G)
+ *   routing      HOST struct of device arrays (see bm_routing); T,E,K,G are written by this call
+ * Every routing array is fully written (pads included).  Integer outputs are deterministic.
+ */
+int bm_route(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, const float *router_bias, int E,
+             int K, const int32_t *group_map, int G, bm_routing *routing, void *workspace,
+             size_t workspace_bytes, bm_stream_t stream);
+
+/*
+ * bm_moe_forward -- steps 9-13: out[t] = sum_s gate_w[t,s] * FFN_{group_ids[t,s]}(x_t) + sum_{j<S} FFN_{G+j}(x_t)
+ * with FFN_u(x) = W2[u] . ( SiLU(W1[u] x) * (W3[u] x) )   (P:42 with united experts P:46; SwiGLU: A3).
+ * bf16 operands, fp32 accumulation (tensor cores), the intermediate h is rounded to bf16 (A12).
+ *   x        [T,D]      bf16
+ *   routing  as produced by bm_route (or any arrays satisfying the same invariants), same T
+ *   W1, W3   [G+S,F,D]  bf16 (united experts 0..G-1, then the S always-on shared experts, A11)
+ *   W2       [G+S,D,F]  bf16
+ *   out      [T,D]      bf16, overwritten
+ * The path (decode / prefill) is picked from T, a host value.
+ */
+int bm_moe_forward(const bm_bf16 *x, int T, int D, const bm_routing *routing, const bm_bf16 *W1,
+                   const bm_bf16 *W3, const bm_bf16 *W2, int F, int S, bm_bf16 *out, void *workspace,
+                   size_t workspace_bytes, bm_stream_t stream);
+
+/* Same as bm_moe_forward with the execution path forced (BM_PATH_*); used by tests and the bench to
+ * exercise every path on any shape.  BM_ERR_PATH if the path cannot run the shape. */
+int bm_moe_forward_path(const bm_bf16 *x, int T, int D, const bm_routing *routing, const bm_bf16 *W1,
+                        const bm_bf16 *W3, const bm_bf16 *W2, int F, int S, bm_bf16 *out,
+                        void *workspace, size_t workspace_bytes, bm_stream_t stream, int path);
+
+/*
+ * bm_moe_layer_host -- the whole layer for one batch held in HOST memory: copies x host->device,
+ * runs bm_route + bm_moe_forward, copies out device->host and SYNCHRONISES `stream`.
+ *   x_host    HOST [T,D] bf16 (pinned memory gives an asynchronous copy)
+ *   out_host  HOST [T,D] bf16
+ *   x_dev, out_dev   device staging buffers [T,D] bf16 owned by the caller
+ * All other arguments as in bm_route / bm_moe_forward (weights, router and group map stay resident on
+ * the device).
+ */
+int bm_moe_layer_host(const bm_bf16 *x_host, int T, int D, const bm_bf16 *W_router,
+                      const float *router_bias, int E, int K, const int32_t *group_map, int G,
+                      const bm_bf16 *W1, const bm_bf16 *W3, const bm_bf16 *W2, int F, int S,
+                      bm_bf16 *out_host, bm_bf16 *x_dev, bm_bf16 *out_dev, bm_routing *routing,
+                      void *workspace, size_t workspace_bytes, bm_stream_t stream);
+
+/* Copies the device status word (OR of BM_DEV_* bits raised since the last call of this function) to
+ * *host_out (HOST), clears it, and SYNCHRONISES `stream`. */
+int bm_device_status(void *workspace, int32_t *host_out, bm_stream_t stream);
+
+/* Number of kernel launches the library has enqueued in this process so far (a HOST counter;
+ * bench.py reports its difference over the timed region as `gpu_launches`). */
+long long bm_launch_count(void);
+
+/* Human-readable name of a bm_status code.  Never NULL. */
+const char *bm_status_string(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BM_H_ */

@@ -1,0 +1,11 @@
+"""B200-native grouped MoE-layer forward pass (BrownoutMoE full-brownout hot path).
+
+The product is the C-ABI library declared in include/bm.h (hand-written sm_100a CUDA kernels under
+csrc/); this package is its thin Python binding.  Importing the package does not load CUDA; the first
+call loads (and if needed builds) libbm.so.
+"""
+from .binding import (  # noqa: F401
+    BM_DEV_BAD_GROUP_MAP, BM_DEV_BAD_ROUTING, BM_DEV_NONFINITE_LOGIT, BM_PATH_AUTO, BM_PATH_DECODE,
+    BM_PATH_PREFILL, BM_PATH_SIMT, BmError, Routing, alloc_workspace, bm_device_status, bm_moe_forward,
+    bm_moe_layer_host, bm_route, launch_count, lib, status_string, workspace_bytes,
+)

@@ -1,0 +1,174 @@
+"""Thin ctypes binding of include/bm.h -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of libbm.so; PyTorch is used for device memory and
+streams.  There is no fallback: if the library is missing it is built with nvcc, and if that fails or
+no sm_100 device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+from ctypes import POINTER, c_float, c_int, c_int32, c_longlong, c_size_t, c_void_p
+
+import torch
+
+from . import build as _build
+
+BM_OK = 0
+BM_PATH_AUTO, BM_PATH_DECODE, BM_PATH_PREFILL, BM_PATH_SIMT = 0, 1, 2, 3
+BM_DEV_BAD_GROUP_MAP, BM_DEV_NONFINITE_LOGIT, BM_DEV_BAD_ROUTING = 1, 2, 4
+BM_MAX_E, BM_MAX_K, BM_MAX_G = 512, 16, 512
+BM_DECODE_MAX_T = 256
+
+EXPORTS = ["bm_workspace_bytes", "bm_route", "bm_moe_forward", "bm_moe_forward_path", "bm_moe_layer_host",
+           "bm_device_status", "bm_launch_count", "bm_status_string"]
+
+
+class BmRouting(ctypes.Structure):
+    _fields_ = [("T", c_int32), ("E", c_int32), ("K", c_int32), ("G", c_int32),
+                ("expert_ids", c_void_p), ("group_ids", c_void_p), ("gate_w", c_void_p),
+                ("n_slots", c_void_p), ("counts", c_void_p), ("offsets", c_void_p),
+                ("row_token", c_void_p), ("row_slot", c_void_p), ("slot_row", c_void_p)]
+
+
+class BmError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: {status_string(code)} ({code})")
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libbm.so (building it in-tree with nvcc if it is missing or stale)."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = ctypes.CDLL(path)
+        L.bm_workspace_bytes.restype = c_size_t
+        L.bm_workspace_bytes.argtypes = [c_int] * 7
+        L.bm_route.restype = c_int
+        L.bm_route.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_int, c_int, c_void_p, c_int,
+                               POINTER(BmRouting), c_void_p, c_size_t, c_void_p]
+        L.bm_moe_forward.restype = c_int
+        L.bm_moe_forward.argtypes = [c_void_p, c_int, c_int, POINTER(BmRouting), c_void_p, c_void_p, c_void_p,
+                                     c_int, c_int, c_void_p, c_void_p, c_size_t, c_void_p]
+        L.bm_moe_forward_path.restype = c_int
+        L.bm_moe_forward_path.argtypes = L.bm_moe_forward.argtypes + [c_int]
+        L.bm_moe_layer_host.restype = c_int
+        L.bm_moe_layer_host.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_int, c_int, c_void_p, c_int,
+                                        c_void_p, c_void_p, c_void_p, c_int, c_int, c_void_p, c_void_p, c_void_p,
+                                        POINTER(BmRouting), c_void_p, c_size_t, c_void_p]
+        L.bm_device_status.restype = c_int
+        L.bm_device_status.argtypes = [c_void_p, POINTER(c_int32), c_void_p]
+        L.bm_launch_count.restype = c_longlong
+        L.bm_launch_count.argtypes = []
+        L.bm_status_string.restype = ctypes.c_char_p
+        L.bm_status_string.argtypes = [c_int]
+        _lib = L
+    return _lib
+
+
+def status_string(code: int) -> str:
+    return lib().bm_status_string(code).decode()
+
+
+def launch_count() -> int:
+    return int(lib().bm_launch_count())
+
+
+def workspace_bytes(T_max: int, D: int, F: int, E: int, K: int, G: int, S: int = 0) -> int:
+    return int(lib().bm_workspace_bytes(T_max, D, F, E, K, G, S))
+
+
+def _ptr(t):
+    return None if t is None else c_void_p(t.data_ptr())
+
+
+def _stream(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return c_void_p(s.cuda_stream)
+
+
+class Routing:
+    """Device arrays of one batch's routing (bm_routing), allocated at their maximum size."""
+
+    def __init__(self, T_max: int, K: int, G: int, device="cuda"):
+        i32 = dict(dtype=torch.int32, device=device)
+        n = max(T_max * K, 1)
+        self.T_max, self.K, self.G = T_max, K, G
+        self.expert_ids = torch.empty(n, **i32)
+        self.group_ids = torch.empty(n, **i32)
+        self.gate_w = torch.empty(n, dtype=torch.float32, device=device)
+        self.n_slots = torch.empty(max(T_max, 1), **i32)
+        self.counts = torch.empty(G, **i32)
+        self.offsets = torch.empty(G + 1, **i32)
+        self.row_token = torch.empty(n, **i32)
+        self.row_slot = torch.empty(n, **i32)
+        self.slot_row = torch.empty(n, **i32)
+        self.c = BmRouting(0, 0, K, G, *[t.data_ptr() for t in (
+            self.expert_ids, self.group_ids, self.gate_w, self.n_slots, self.counts, self.offsets,
+            self.row_token, self.row_slot, self.slot_row)])
+
+    def view(self, T: int):
+        """The routing arrays trimmed/reshaped for a batch of T tokens (no copy)."""
+        K = self.K
+        return dict(expert_ids=self.expert_ids[:T * K].view(T, K), group_ids=self.group_ids[:T * K].view(T, K),
+                    gate_w=self.gate_w[:T * K].view(T, K), n_slots=self.n_slots[:T], counts=self.counts,
+                    offsets=self.offsets, row_token=self.row_token[:T * K], row_slot=self.row_slot[:T * K],
+                    slot_row=self.slot_row[:T * K].view(T, K))
+
+
+def alloc_workspace(T_max: int, D: int, F: int, E: int, K: int, G: int, S: int = 0, device="cuda") -> torch.Tensor:
+    """Workspace for shapes up to T_max; the status word at its start is zeroed."""
+    n = workspace_bytes(T_max, D, F, E, K, G, S)
+    ws = torch.empty(n, dtype=torch.uint8, device=device)
+    ws[:4096].zero_()
+    return ws
+
+
+def bm_route(x, W_router, router_bias, K: int, group_map, G: int, routing: Routing, workspace, stream=None):
+    """R1-R7 (include/bm.h: bm_route).  x [T,D] bf16, W_router [E,D] bf16, router_bias [E] f32 | None,
+    group_map [E] i32; fills `routing` asynchronously on the current stream."""
+    T, D = x.shape
+    E = W_router.shape[0]
+    rc = lib().bm_route(_ptr(x), T, D, _ptr(W_router), _ptr(router_bias), E, K, _ptr(group_map), G,
+                        ctypes.byref(routing.c), _ptr(workspace), workspace.numel(), _stream(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_route")
+    return routing
+
+
+def bm_moe_forward(x, routing: Routing, W1, W3, W2, out, workspace, S: int = 0, path: int = BM_PATH_AUTO,
+                   stream=None):
+    """Steps 9-13 (include/bm.h: bm_moe_forward / bm_moe_forward_path).  W1, W3 [G+S,F,D], W2 [G+S,D,F] bf16;
+    out [T,D] bf16 is overwritten."""
+    T, D = x.shape
+    F = W1.shape[1]
+    rc = lib().bm_moe_forward_path(_ptr(x), T, D, ctypes.byref(routing.c), _ptr(W1), _ptr(W3), _ptr(W2), F, S,
+                                   _ptr(out), _ptr(workspace), workspace.numel(), _stream(stream), path)
+    if rc != BM_OK:
+        raise BmError(rc, "bm_moe_forward")
+    return out
+
+
+def bm_moe_layer_host(x_host, W_router, router_bias, K, group_map, G, W1, W3, W2, S, out_host, x_dev, out_dev,
+                      routing: Routing, workspace, stream=None):
+    """Whole layer for a batch in (pinned) host memory; returns after the device->host copy has finished."""
+    T, D = x_host.shape
+    E = W_router.shape[0]
+    F = W1.shape[1]
+    rc = lib().bm_moe_layer_host(_ptr(x_host), T, D, _ptr(W_router), _ptr(router_bias), E, K, _ptr(group_map), G,
+                                 _ptr(W1), _ptr(W3), _ptr(W2), F, S, _ptr(out_host), _ptr(x_dev), _ptr(out_dev),
+                                 ctypes.byref(routing.c), _ptr(workspace), workspace.numel(), _stream(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_moe_layer_host")
+    return out_host
+
+
+def bm_device_status(workspace, stream=None) -> int:
+    v = c_int32(0)
+    rc = lib().bm_device_status(_ptr(workspace), ctypes.byref(v), _stream(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_device_status")
+    return int(v.value)

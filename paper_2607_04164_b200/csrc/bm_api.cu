@@ -1,0 +1,191 @@
+// bm_api.cu -- the C-ABI entry points of include/bm.h: argument checking, workspace carving, path
+// dispatch.  No compute happens on the host and there is no CPU fallback.
+#include <atomic>
+#include <cstring>
+
+#include "bm_common.cuh"
+
+namespace bm {
+
+static std::atomic<long long> g_launches{0};
+void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+int num_sms() {
+    static int sms = 0;
+    if (sms == 0) {
+        int dev = 0, v = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0)
+            sms = v;
+        else
+            sms = kNumSMsFallback;
+    }
+    return sms;
+}
+
+// 0 = not checked, 1 = sm_100 present, -1 = absent
+static int device_ok() {
+    static int state = 0;
+    if (state == 0) {
+        int dev = 0, major = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) == cudaSuccess && major == 10)
+            state = 1;
+        else
+            state = -1;
+    }
+    return state;
+}
+
+static inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+static int check_shapes(int T, int D, int F, int E, int K, int G, int S, bool with_f) {
+    if (T < 0 || D < 8 || D % 8 != 0) return BM_ERR_SHAPE;
+    if (E < 1 || E > BM_MAX_E || K < 1 || K > E || K > BM_MAX_K) return BM_ERR_SHAPE;
+    if (G < 1 || G > BM_MAX_G) return BM_ERR_SHAPE;
+    if (with_f && (F < 8 || F % 8 != 0 || S < 0 || S > kMaxShared)) return BM_ERR_SHAPE;
+    if ((long long)T * K > 0x3fffffffLL) return BM_ERR_SHAPE;
+    return BM_OK;
+}
+
+}  // namespace bm
+
+using namespace bm;
+
+extern "C" {
+
+size_t bm_workspace_bytes(int T_max, int D, int F, int E, int K, int G, int S) {
+    (void)E;
+    if (T_max < 0 || D < 1 || F < 1 || K < 1 || G < 1 || S < 0) return 0;
+    return workspace_layout(T_max, D, F, K, G, S).total;
+}
+
+int bm_route(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, const float *router_bias, int E, int K,
+             const int32_t *group_map, int G, bm_routing *routing, void *workspace, size_t workspace_bytes,
+             bm_stream_t stream) {
+    if (!routing) return BM_ERR_NULL;
+    int rc = check_shapes(T, D, 8, E, K, G, 0, false);
+    if (rc != BM_OK) return rc;
+    routing->T = T; routing->E = E; routing->K = K; routing->G = G;
+    if (!W_router || !group_map || !workspace || !routing->counts || !routing->offsets) return BM_ERR_NULL;
+    if (T > 0 && (!x || !routing->expert_ids || !routing->group_ids || !routing->gate_w || !routing->n_slots ||
+                  !routing->row_token || !routing->row_slot || !routing->slot_row))
+        return BM_ERR_NULL;
+    if (!aligned16(x) || !aligned16(W_router) || !aligned16(workspace)) return BM_ERR_ALIGN;
+    // only the routing part of the workspace is needed here (F = 8, S = 0 gives its lower bound)
+    const Workspace full = workspace_layout(T, D, 8, K, G, 0);
+    if (workspace_bytes < full.sched) return BM_ERR_WORKSPACE;
+    if (device_ok() != 1) return BM_ERR_CUDA;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    uint8_t *ws = static_cast<uint8_t *>(workspace);
+    int32_t *status = reinterpret_cast<int32_t *>(ws + full.status);
+    if (T == 0) {
+        // empty batch: counts = 0, offsets = 0
+        if (cudaMemsetAsync(routing->counts, 0, sizeof(int32_t) * G, st) != cudaSuccess ||
+            cudaMemsetAsync(routing->offsets, 0, sizeof(int32_t) * (G + 1), st) != cudaSuccess)
+            return BM_ERR_CUDA;
+        return BM_OK;
+    }
+    if (launch_router(x, T, D, W_router, router_bias, E, K, group_map, G, *routing, status, st) != cudaSuccess)
+        return BM_ERR_CUDA;
+    if (launch_permute(T, K, G, *routing, reinterpret_cast<int32_t *>(ws + full.block_hist), status, st) !=
+        cudaSuccess)
+        return BM_ERR_CUDA;
+    return BM_OK;
+}
+
+int bm_moe_forward_path(const bm_bf16 *x, int T, int D, const bm_routing *routing, const bm_bf16 *W1,
+                        const bm_bf16 *W3, const bm_bf16 *W2, int F, int S, bm_bf16 *out, void *workspace,
+                        size_t workspace_bytes, bm_stream_t stream, int path) {
+    if (!routing) return BM_ERR_NULL;
+    const int K = routing->K, G = routing->G;
+    int rc = check_shapes(T, D, F, routing->E, K, G, S, true);
+    if (rc != BM_OK) return rc;
+    if (routing->T != T) return BM_ERR_SHAPE;
+    if (path < BM_PATH_AUTO || path > BM_PATH_SIMT) return BM_ERR_PATH;
+    if (T == 0) return BM_OK;
+    if (!x || !W1 || !W3 || !W2 || !out || !workspace || !routing->group_ids || !routing->gate_w ||
+        !routing->n_slots || !routing->counts || !routing->offsets || !routing->row_token || !routing->row_slot ||
+        !routing->slot_row)
+        return BM_ERR_NULL;
+    if (!aligned16(x) || !aligned16(W1) || !aligned16(W3) || !aligned16(W2) || !aligned16(out) ||
+        !aligned16(workspace))
+        return BM_ERR_ALIGN;
+    const Workspace w = workspace_layout(T, D, F, K, G, S);
+    if (workspace_bytes < w.total) return BM_ERR_WORKSPACE;
+    if (device_ok() != 1) return BM_ERR_CUDA;
+
+    if (path == BM_PATH_AUTO) path = (T <= BM_DECODE_MAX_T) ? BM_PATH_DECODE : BM_PATH_PREFILL;
+
+    uint8_t *ws = static_cast<uint8_t *>(workspace);
+    ForwardArgs a{};
+    a.x = x; a.T = T; a.D = D; a.F = F; a.K = K; a.G = G; a.S = S;
+    a.r = *routing;
+    a.W1 = W1; a.W3 = W3; a.W2 = W2; a.out = out;
+    a.status = reinterpret_cast<int32_t *>(ws + w.status);
+    a.sched = reinterpret_cast<int32_t *>(ws + w.sched);
+    a.xs = reinterpret_cast<bm_bf16 *>(ws + w.xs);
+    a.h = reinterpret_cast<bm_bf16 *>(ws + w.h);
+    a.out_acc = reinterpret_cast<float *>(ws + w.out_acc);
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    cudaError_t e;
+    if (path == BM_PATH_SIMT) e = launch_forward_simt(a, st);
+    else e = launch_forward_tc(a, path == BM_PATH_DECODE, st);
+    return e == cudaSuccess ? BM_OK : BM_ERR_CUDA;
+}
+
+int bm_moe_forward(const bm_bf16 *x, int T, int D, const bm_routing *routing, const bm_bf16 *W1, const bm_bf16 *W3,
+                   const bm_bf16 *W2, int F, int S, bm_bf16 *out, void *workspace, size_t workspace_bytes,
+                   bm_stream_t stream) {
+    return bm_moe_forward_path(x, T, D, routing, W1, W3, W2, F, S, out, workspace, workspace_bytes, stream,
+                               BM_PATH_AUTO);
+}
+
+int bm_moe_layer_host(const bm_bf16 *x_host, int T, int D, const bm_bf16 *W_router, const float *router_bias, int E,
+                      int K, const int32_t *group_map, int G, const bm_bf16 *W1, const bm_bf16 *W3,
+                      const bm_bf16 *W2, int F, int S, bm_bf16 *out_host, bm_bf16 *x_dev, bm_bf16 *out_dev,
+                      bm_routing *routing, void *workspace, size_t workspace_bytes, bm_stream_t stream) {
+    if (T < 0) return BM_ERR_SHAPE;
+    if (T > 0 && (!x_host || !out_host || !x_dev || !out_dev)) return BM_ERR_NULL;
+    if (device_ok() != 1) return BM_ERR_CUDA;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const size_t bytes = (size_t)T * D * sizeof(bm_bf16);
+    if (T > 0 && cudaMemcpyAsync(x_dev, x_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return BM_ERR_CUDA;
+    int rc = bm_route(x_dev, T, D, W_router, router_bias, E, K, group_map, G, routing, workspace, workspace_bytes,
+                      stream);
+    if (rc != BM_OK) return rc;
+    rc = bm_moe_forward(x_dev, T, D, routing, W1, W3, W2, F, S, out_dev, workspace, workspace_bytes, stream);
+    if (rc != BM_OK) return rc;
+    if (T > 0 && cudaMemcpyAsync(out_host, out_dev, bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+        return BM_ERR_CUDA;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return BM_ERR_CUDA;
+    return BM_OK;
+}
+
+int bm_device_status(void *workspace, int32_t *host_out, bm_stream_t stream) {
+    if (!workspace || !host_out) return BM_ERR_NULL;
+    if (device_ok() != 1) return BM_ERR_CUDA;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    if (cudaMemcpyAsync(host_out, workspace, sizeof(int32_t), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaMemsetAsync(workspace, 0, sizeof(int32_t), st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess)
+        return BM_ERR_CUDA;
+    return BM_OK;
+}
+
+long long bm_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+const char *bm_status_string(int code) {
+    switch (code) {
+        case BM_OK: return "BM_OK";
+        case BM_ERR_NULL: return "BM_ERR_NULL: a required pointer is NULL";
+        case BM_ERR_SHAPE: return "BM_ERR_SHAPE: unsupported or inconsistent shape";
+        case BM_ERR_ALIGN: return "BM_ERR_ALIGN: a device pointer is not 16-byte aligned";
+        case BM_ERR_WORKSPACE: return "BM_ERR_WORKSPACE: workspace too small";
+        case BM_ERR_CUDA: return "BM_ERR_CUDA: no sm_100 device or a CUDA call failed";
+        case BM_ERR_PATH: return "BM_ERR_PATH: the forced path cannot run this shape";
+        default: return "unknown bm_status";
+    }
+}
+
+}  // extern "C"

@@ -1,0 +1,101 @@
+// bm_common.cuh -- shared declarations of the CUDA path (internal; the public boundary is include/bm.h).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/bm.h"
+
+namespace bm {
+
+constexpr int kNumSMsFallback = 148;
+constexpr unsigned kFullMask = 0xffffffffu;
+
+// ---------------------------------------------------------------------------------------------
+// Workspace layout (host-computed; all sections 1024-byte aligned).  Shapes only, never data.
+// ---------------------------------------------------------------------------------------------
+constexpr int kPermItemsPerBlock = 2048;   // (token, slot) items per CTA of the permutation kernels
+constexpr int kMaxSchedTiles = 1 << 20;
+
+struct Workspace {
+    // byte offsets from the workspace base
+    size_t status;       // int32[64]: [0] device status bits, [1] A (copy of offsets[G]), [2..] counters
+    size_t block_hist;   // int32[nb * G]   per-block group histograms / bases of the permutation
+    size_t sched;        // int32[kSchedInts] tile-schedule scratch of the forward pass
+    size_t xs;           // bf16[T*K, D]    token rows gathered in permuted order (prefill path)
+    size_t h;            // bf16[T*K + S*T, F]  SwiGLU intermediate
+    size_t out_acc;      // f32[T, D]       fp32 accumulation of the combine
+    size_t total;
+};
+
+constexpr int kMaxShared = 16;                                  // S <= 16 always-on shared experts
+constexpr int kSchedInts = 4 + 2 * (BM_MAX_G + kMaxShared) + 8;
+
+__host__ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+__host__ inline Workspace workspace_layout(int T, int D, int F, int K, int G, int S) {
+    Workspace w{};
+    size_t off = 0;
+    const size_t items = (size_t)T * K;
+    const size_t nb = (items + kPermItemsPerBlock - 1) / kPermItemsPerBlock;
+    w.status = off;      off = align_up(off + 64 * sizeof(int32_t), 1024);
+    w.block_hist = off;  off = align_up(off + (nb > 0 ? nb : 1) * (size_t)G * sizeof(int32_t), 1024);
+    w.sched = off;       off = align_up(off + kSchedInts * sizeof(int32_t), 1024);
+    w.xs = off;          off = align_up(off + items * D * sizeof(bm_bf16), 1024);
+    w.h = off;           off = align_up(off + (items + (size_t)S * T) * F * sizeof(bm_bf16), 1024);
+    w.out_acc = off;     off = align_up(off + (size_t)T * D * sizeof(float), 1024);
+    w.total = off;
+    return w;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Launch bookkeeping (host)
+// ---------------------------------------------------------------------------------------------
+void count_launch(int n = 1);
+int num_sms();
+
+// ---------------------------------------------------------------------------------------------
+// Internal kernel launchers (defined in the .cu files, called from bm_api.cu)
+// ---------------------------------------------------------------------------------------------
+cudaError_t launch_router(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const float *bias, int E,
+                          int K, const int32_t *gmap, int G, const bm_routing &r, int32_t *status,
+                          cudaStream_t stream);
+
+cudaError_t launch_permute(int T, int K, int G, const bm_routing &r, int32_t *block_hist, int32_t *status,
+                           cudaStream_t stream);
+
+struct ForwardArgs {
+    const bm_bf16 *x;
+    int T, D, F, K, G, S;
+    bm_routing r;
+    const bm_bf16 *W1, *W3, *W2;
+    bm_bf16 *out;
+    // workspace sections
+    int32_t *status;
+    int32_t *sched;
+    bm_bf16 *xs;
+    bm_bf16 *h;
+    float *out_acc;
+};
+
+cudaError_t launch_forward_simt(const ForwardArgs &a, cudaStream_t stream);
+cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t stream);
+
+// ---------------------------------------------------------------------------------------------
+// Device helpers
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ float bf16_lo(uint32_t u) { return __uint_as_float(u << 16); }
+__device__ __forceinline__ float bf16_hi(uint32_t u) { return __uint_as_float(u & 0xffff0000u); }
+
+// fp32 -> bf16 bits, round to nearest even (finite inputs; NaN stays NaN)
+__device__ __forceinline__ uint32_t f32_to_bf16_bits(float f) {
+    uint32_t u = __float_as_uint(f);
+    if ((u & 0x7fffffffu) > 0x7f800000u) return (u >> 16) | 0x40u;   // quiet NaN
+    u += 0x7fffu + ((u >> 16) & 1u);
+    return u >> 16;
+}
+__device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
+    return f32_to_bf16_bits(lo) | (f32_to_bf16_bits(hi) << 16);
+}
+
+}  // namespace bm

@@ -1,0 +1,223 @@
+// bm_permute.cu -- steps R6-R8: per-group histogram, exclusive scan and the stable permutation that
+// builds the per-group token lists (BASELINE.json north_star (2): "a warp-level histogram plus
+// prefix-scan permutation kernel"; reading A7: rows ordered by group, then token ascending).
+//
+// The (token, slot) pairs are "items" i = t*K + s.  After dedup a token holds a group at most once,
+// so ordering the items of one group by i is ordering them by token: a STABLE counting sort of the
+// items keyed by group is exactly the required permutation, and it is deterministic -- no atomics
+// whose arrival order could matter.
+//
+//   block b owns items [b*2048, (b+1)*2048); warp w of the block owns a contiguous eighth of them and
+//   walks it 32 items at a time.  __match_any_sync gives every lane the set of lanes holding its key:
+//   rank inside the round = popc(set & lanes below), the round's count = popc(set).
+//
+//   P1  hist    : per-warp counts in shared memory -> per-block counts block_hist[b][u]
+//   P2  scan    : counts[u] = sum_b, offsets = exclusive scan over u, block_hist[b][u] := first row of
+//                 block b in group u
+//   P3  permute : per-warp bases from P2's block bases, replay the walk, write row_token / row_slot /
+//                 slot_row; pads get -1
+//   T*K <= 2048 : one CTA does P1-P3 in a single launch (the decode case).
+#include "bm_common.cuh"
+
+namespace bm {
+
+namespace {
+
+constexpr int kWarps = 8;
+constexpr int kItemsPerWarp = kPermItemsPerBlock / kWarps;   // 256
+
+// Count the items of this warp's slice into whist_w[0..G) (shared memory, zeroed by the caller).
+__device__ __forceinline__ void warp_histogram(const int32_t *__restrict__ group_ids, long long items,
+                                               long long first, int *whist_w, int lane) {
+    for (int r = 0; r < kItemsPerWarp; r += 32) {
+        const long long i = first + r + lane;
+        const int key = (i < items) ? group_ids[i] : -1;
+        const unsigned peers = __match_any_sync(kFullMask, key);
+        if (key >= 0 && lane == __ffs(peers) - 1) whist_w[key] += __popc(peers);
+        __syncwarp();
+    }
+}
+
+// Replay the walk with running bases wbase_w[0..G) (shared memory) and emit the permutation.
+__device__ __forceinline__ void warp_permute(const int32_t *__restrict__ group_ids, long long items,
+                                             long long first, int K, int *wbase_w, int lane, int A,
+                                             int32_t *__restrict__ row_token, int32_t *__restrict__ row_slot,
+                                             int32_t *__restrict__ slot_row) {
+    for (int r = 0; r < kItemsPerWarp; r += 32) {
+        const long long i = first + r + lane;
+        const int key = (i < items) ? group_ids[i] : -1;
+        const unsigned peers = __match_any_sync(kFullMask, key);
+        if (i < items) {
+            if (key >= 0) {
+                const int row = wbase_w[key] + __popc(peers & ((1u << lane) - 1u));
+                row_token[row] = (int32_t)(i / K);
+                row_slot[row] = (int32_t)(i % K);
+                slot_row[i] = row;
+            } else {
+                slot_row[i] = -1;
+            }
+            if (i >= A) {                       // rows past A stay -1 (A <= items)
+                row_token[i] = -1;
+                row_slot[i] = -1;
+            }
+        }
+        __syncwarp();
+        if (key >= 0 && lane == __ffs(peers) - 1) wbase_w[key] += __popc(peers);
+        __syncwarp();
+    }
+}
+
+// Block-wide exclusive scan of v[0..n) (n <= 512) in shared memory; returns the total in *total.
+__device__ void block_exclusive_scan(int *v, int n, int *tmp, int *total) {
+    // Hillis-Steele over 512 slots with 256 threads, two slots per thread
+    for (int i = threadIdx.x; i < 512; i += blockDim.x) tmp[i] = i < n ? v[i] : 0;
+    __syncthreads();
+    for (int d = 1; d < 512; d <<= 1) {
+        int a0 = 0, a1 = 0;
+        const int i0 = threadIdx.x, i1 = threadIdx.x + 256;
+        if (i0 >= d) a0 = tmp[i0 - d];
+        if (i1 >= d) a1 = tmp[i1 - d];
+        __syncthreads();
+        tmp[i0] += a0;
+        tmp[i1] += a1;
+        __syncthreads();
+    }
+    for (int i = threadIdx.x; i < n; i += blockDim.x) v[i] = tmp[i] - v[i];   // inclusive -> exclusive
+    if (threadIdx.x == 0) *total = n > 0 ? tmp[n - 1] : 0;
+    __syncthreads();
+}
+
+// ---- T*K <= 2048: everything in one CTA --------------------------------------------------------
+__global__ void __launch_bounds__(kWarps * 32)
+permute_small_kernel(const int32_t *__restrict__ group_ids, int T, int K, int G,
+                     int32_t *__restrict__ counts, int32_t *__restrict__ offsets,
+                     int32_t *__restrict__ row_token, int32_t *__restrict__ row_slot,
+                     int32_t *__restrict__ slot_row, int32_t *__restrict__ status) {
+    extern __shared__ int s_mem[];
+    int *whist = s_mem;                  // [kWarps][G]
+    int *gsum = whist + kWarps * G;      // [G] -> offsets
+    int *tmp = gsum + G;                 // [512]
+    __shared__ int s_total;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long items = (long long)T * K;
+    for (int i = threadIdx.x; i < kWarps * G; i += blockDim.x) whist[i] = 0;
+    __syncthreads();
+    warp_histogram(group_ids, items, (long long)warp * kItemsPerWarp, whist + warp * G, lane);
+    __syncthreads();
+    for (int u = threadIdx.x; u < G; u += blockDim.x) {
+        int run = 0;
+        for (int w = 0; w < kWarps; ++w) {      // whist[w][u] := rows of group u in warps before w
+            const int c = whist[w * G + u];
+            whist[w * G + u] = run;
+            run += c;
+        }
+        gsum[u] = run;
+        counts[u] = run;
+    }
+    __syncthreads();
+    block_exclusive_scan(gsum, G, tmp, &s_total);
+    for (int u = threadIdx.x; u < G; u += blockDim.x) {
+        offsets[u] = gsum[u];
+        for (int w = 0; w < kWarps; ++w) whist[w * G + u] += gsum[u];
+    }
+    if (threadIdx.x == 0) { offsets[G] = s_total; status[1] = s_total; }
+    __syncthreads();
+    warp_permute(group_ids, items, (long long)warp * kItemsPerWarp, K, whist + warp * G, lane, s_total,
+                 row_token, row_slot, slot_row);
+}
+
+// ---- general case: P1 / P2 / P3 ---------------------------------------------------------------
+__global__ void __launch_bounds__(kWarps * 32)
+permute_hist_kernel(const int32_t *__restrict__ group_ids, int T, int K, int G,
+                    int32_t *__restrict__ block_hist) {
+    extern __shared__ int s_mem[];
+    int *whist = s_mem;                  // [kWarps][G]
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long items = (long long)T * K;
+    for (int i = threadIdx.x; i < kWarps * G; i += blockDim.x) whist[i] = 0;
+    __syncthreads();
+    const long long first = (long long)blockIdx.x * kPermItemsPerBlock + (long long)warp * kItemsPerWarp;
+    warp_histogram(group_ids, items, first, whist + warp * G, lane);
+    __syncthreads();
+    for (int u = threadIdx.x; u < G; u += blockDim.x) {
+        int run = 0;
+        for (int w = 0; w < kWarps; ++w) run += whist[w * G + u];
+        block_hist[(size_t)blockIdx.x * G + u] = run;
+    }
+}
+
+__global__ void __launch_bounds__(256)
+permute_scan_kernel(int nb, int G, int32_t *__restrict__ block_hist, int32_t *__restrict__ counts,
+                    int32_t *__restrict__ offsets, int32_t *__restrict__ status) {
+    __shared__ int gsum[512];
+    __shared__ int tmp[512];
+    __shared__ int s_total;
+    for (int u = threadIdx.x; u < G; u += blockDim.x) {
+        int run = 0;
+        for (int b = 0; b < nb; ++b) {          // block_hist[b][u] := rows of group u in blocks before b
+            const int c = block_hist[(size_t)b * G + u];
+            block_hist[(size_t)b * G + u] = run;
+            run += c;
+        }
+        gsum[u] = run;
+        counts[u] = run;
+    }
+    __syncthreads();
+    block_exclusive_scan(gsum, G, tmp, &s_total);
+    for (int u = threadIdx.x; u < G; u += blockDim.x) {
+        offsets[u] = gsum[u];
+        for (int b = 0; b < nb; ++b) block_hist[(size_t)b * G + u] += gsum[u];
+    }
+    if (threadIdx.x == 0) { offsets[G] = s_total; status[1] = s_total; }
+}
+
+__global__ void __launch_bounds__(kWarps * 32)
+permute_scatter_kernel(const int32_t *__restrict__ group_ids, int T, int K, int G,
+                       const int32_t *__restrict__ block_hist, const int32_t *__restrict__ offsets,
+                       int32_t *__restrict__ row_token, int32_t *__restrict__ row_slot,
+                       int32_t *__restrict__ slot_row) {
+    extern __shared__ int s_mem[];
+    int *whist = s_mem;                  // [kWarps][G]
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long items = (long long)T * K;
+    for (int i = threadIdx.x; i < kWarps * G; i += blockDim.x) whist[i] = 0;
+    __syncthreads();
+    const long long first = (long long)blockIdx.x * kPermItemsPerBlock + (long long)warp * kItemsPerWarp;
+    warp_histogram(group_ids, items, first, whist + warp * G, lane);
+    __syncthreads();
+    for (int u = threadIdx.x; u < G; u += blockDim.x) {
+        int run = block_hist[(size_t)blockIdx.x * G + u];
+        for (int w = 0; w < kWarps; ++w) {
+            const int c = whist[w * G + u];
+            whist[w * G + u] = run;
+            run += c;
+        }
+    }
+    __syncthreads();
+    warp_permute(group_ids, items, first, K, whist + warp * G, lane, offsets[G], row_token, row_slot,
+                 slot_row);
+}
+
+}  // namespace
+
+cudaError_t launch_permute(int T, int K, int G, const bm_routing &r, int32_t *block_hist, int32_t *status,
+                           cudaStream_t stream) {
+    const long long items = (long long)T * K;
+    const int nb = (int)((items + kPermItemsPerBlock - 1) / kPermItemsPerBlock);
+    const size_t smem_w = (size_t)kWarps * G * sizeof(int);
+    if (nb <= 1) {
+        const size_t smem = smem_w + (size_t)(G + 512) * sizeof(int);
+        permute_small_kernel<<<1, kWarps * 32, smem, stream>>>(r.group_ids, T, K, G, r.counts, r.offsets,
+                                                              r.row_token, r.row_slot, r.slot_row, status);
+        count_launch();
+        return cudaGetLastError();
+    }
+    permute_hist_kernel<<<nb, kWarps * 32, smem_w, stream>>>(r.group_ids, T, K, G, block_hist);
+    permute_scan_kernel<<<1, 256, 0, stream>>>(nb, G, block_hist, r.counts, r.offsets, status);
+    permute_scatter_kernel<<<nb, kWarps * 32, smem_w, stream>>>(r.group_ids, T, K, G, block_hist, r.offsets,
+                                                                r.row_token, r.row_slot, r.slot_row);
+    count_launch(3);
+    return cudaGetLastError();
+}
+
+}  // namespace bm

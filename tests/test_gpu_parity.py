@@ -1,0 +1,211 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the CPU oracle on the same
+seeded inputs.  Routing arrays bit-exact; out within max|gpu-oracle| <= 2e-2*(1+|oracle|)
+(BASELINE.json north_star)."""
+import numpy as np
+import pytest
+import torch
+
+from bm_inputs import CONFIGS, LayerConfig, make_layer, identity_variant
+from gpu_helpers import (assert_out_close, assert_routing_equal, gpu_layer, gpu_route, oracle_forward,
+                         oracle_route, routing_to_numpy, to_device)
+from helpers import bf16_tensor, rand_layer
+
+pytestmark = pytest.mark.gpu
+
+PATHS = {"simt": 3, "decode": 1, "prefill": 2}
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_gpu():
+    assert torch.cuda.is_available(), "the -m gpu tests need a CUDA device"
+    import paper_2607_04164_b200 as bm
+    bm.lib()
+
+
+# ---------------------------------------------------------------------------------------------------
+# routing: bit-exact
+# ---------------------------------------------------------------------------------------------------
+ROUTE_SHAPES = [
+    # T, D, E, K, G, zipf_s
+    (1, 256, 8, 2, 4, 0.0),
+    (64, 256, 8, 2, 4, 0.0),
+    (64, 4096, 8, 2, 4, 1.2),
+    (257, 2048, 60, 4, 15, 1.0),
+    (16, 2048, 60, 4, 60, 2.0),
+    (1000, 512, 64, 6, 16, 1.5),       # T*K > 2048: three-kernel permutation
+    (3001, 264, 13, 5, 7, 1.0),        # T >= 2048: throughput router; ragged D (264 = 256 + 8), odd E
+    (4096, 2048, 60, 4, 8, 1.0),
+    (300, 64, 200, 16, 97, 0.0),       # many experts, K = BM_MAX_K
+    (2500, 128, 512, 3, 512, 0.0),     # E = BM_MAX_E, G = BM_MAX_G
+]
+
+
+@pytest.mark.parametrize("T,D,E,K,G,s", ROUTE_SHAPES)
+def test_routing_bit_exact(T, D, E, K, G, s):
+    cfg = LayerConfig("t", T=T, D=D, F=8, E=E, K=K, G=G, zipf_s=s,
+                      gmap_kind="identity" if G == E else "balanced")
+    for seed in range(2):
+        L = make_layer(cfg, seed, weights=False)
+        r, ws, _ = gpu_route(L)
+        import paper_2607_04164_b200 as bm
+        assert bm.bm_device_status(ws) == 0
+        assert_routing_equal(routing_to_numpy(r, T), oracle_route(L))
+
+
+def test_routing_ties_and_degenerate_rows():
+    # coarse integer inputs make exact logit ties frequent: the lower-index rule decides (A4)
+    rng = np.random.default_rng(0)
+    from types import SimpleNamespace
+    for (T, D, E, K, G) in [(500, 16, 6, 3, 3), (2100, 32, 40, 4, 40), (64, 8, 8, 8, 2)]:
+        L = SimpleNamespace(K=K, G=G, S=0)
+        L.x = bf16_tensor(rng.integers(-2, 3, (T, D)))
+        L.W_router = bf16_tensor(rng.integers(-1, 2, (E, D)))
+        L.W_router[E - 1] = L.W_router[0]                      # a guaranteed tie pair
+        L.router_bias = None
+        L.group_map = torch.as_tensor((np.arange(E) % G).astype(np.int32))
+        r, ws, _ = gpu_route(L)
+        o = oracle_route(L, want_logits=True)
+        srt = np.sort(o.logits, axis=1)[:, ::-1]
+        if K < E:
+            assert (srt[:, K - 1] == srt[:, K]).any()          # ties at the selection boundary exist
+        assert_routing_equal(routing_to_numpy(r, T), o)
+    # all-equal logits -> experts 0..K-1
+    L = SimpleNamespace(K=3, G=4, S=0, x=bf16_tensor(np.ones((10, 64))), W_router=bf16_tensor(np.zeros((8, 64))),
+                        router_bias=None, group_map=torch.arange(8, dtype=torch.int32) % 4)
+    r, _, _ = gpu_route(L)
+    g = routing_to_numpy(r, 10)
+    assert (g.expert_ids == np.arange(3)).all()
+    assert_routing_equal(g, oracle_route(L))
+
+
+def test_device_status_flags_bad_group_map_and_nonfinite():
+    import paper_2607_04164_b200 as bm
+    cfg = LayerConfig("t", T=32, D=64, F=8, E=8, K=2, G=4)
+    L = make_layer(cfg, 0, weights=False)
+    L.group_map = L.group_map.clone(); L.group_map[:] = 9      # outside [0, G)
+    r, ws, _ = gpu_route(L)
+    assert bm.bm_device_status(ws) & bm.BM_DEV_BAD_GROUP_MAP
+    g = routing_to_numpy(r, 32)
+    assert ((g.group_ids >= -1) & (g.group_ids < 4)).all()     # indices stay in range
+    L = make_layer(cfg, 0, weights=False)
+    L.router_bias = torch.zeros(8); L.router_bias[3] = float("nan")
+    r, ws, _ = gpu_route(L)
+    assert bm.bm_device_status(ws) & bm.BM_DEV_NONFINITE_LOGIT
+    assert bm.bm_device_status(ws) == 0                        # reading clears the word
+
+
+# ---------------------------------------------------------------------------------------------------
+# forward: every path on shapes spanning several tiles and ragged tails
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("path", ["simt", "decode", "prefill"])
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_tiny_config_all_paths(path, seed):
+    L = make_layer(CONFIGS["tiny"], seed)                      # BJ:configs[0]
+    g, out, status = gpu_layer(L, PATHS[path])
+    o = oracle_route(L)
+    assert status == 0
+    assert_routing_equal(g, o)
+    assert_out_close(out, oracle_forward(L, o))
+
+
+FWD_SHAPES = [
+    # T, D, F, E, K, G, S   -- D, F chosen to leave ragged 64/128/256 tails
+    (300, 512, 1000, 8, 2, 3, 1),
+    (130, 320, 264, 6, 3, 2, 0),
+    (257, 2048, 1408, 60, 4, 15, 0),
+    (700, 256, 640, 16, 4, 5, 2),
+    (5, 64, 64, 4, 2, 4, 0),
+    (1, 256, 512, 8, 2, 4, 1),
+]
+
+
+@pytest.mark.parametrize("path", ["simt", "decode", "prefill"])
+@pytest.mark.parametrize("T,D,F,E,K,G,S", FWD_SHAPES)
+def test_forward_parity_ragged_shapes(path, T, D, F, E, K, G, S):
+    rng = np.random.default_rng(T * 7 + F)
+    L = rand_layer(rng, T=T, D=D, F=F, E=E, K=K, G=G, S=S, bias=True, wstd=0.05)
+    g, out, status = gpu_layer(L, PATHS[path])
+    o = oracle_route(L)
+    assert status == 0
+    assert_routing_equal(g, o)
+    assert_out_close(out, oracle_forward(L, o))
+
+
+def test_empty_groups_and_empty_batch():
+    import paper_2607_04164_b200 as bm
+    rng = np.random.default_rng(5)
+    # half of the groups can never be hit (A10)
+    L = rand_layer(rng, T=96, D=128, F=256, E=8, K=2, G=16, gmap=np.arange(8) * 2)
+    for path in PATHS.values():
+        g, out, status = gpu_layer(L, path)
+        o = oracle_route(L)
+        assert (g.counts[1::2] == 0).all()
+        assert_routing_equal(g, o)
+        assert_out_close(out, oracle_forward(L, o))
+    # T = 0 is a no-op that still defines counts/offsets
+    d = to_device(L)
+    r = bm.Routing(0, 2, 16)
+    ws = bm.alloc_workspace(0, 128, 256, 8, 2, 16)
+    bm.bm_route(d.x[:0], d.W_router, None, 2, d.group_map, 16, r, ws)
+    out = torch.empty((0, 128), dtype=torch.bfloat16, device="cuda")
+    bm.bm_moe_forward(d.x[:0], r, d.W1, d.W3, d.W2, out, ws)
+    torch.cuda.synchronize()
+    assert (r.counts.cpu() == 0).all() and (r.offsets.cpu() == 0).all()
+
+
+def test_grouped_equals_ungrouped_with_replicated_weights_on_gpu():
+    # BJ:north_star check 2, on the device: identity map over E experts that carry their group's weights
+    rng = np.random.default_rng(6)
+    L = rand_layer(rng, T=200, D=256, F=384, E=8, K=3, G=3)
+    g, out, _ = gpu_layer(L, PATHS["prefill"])
+    from types import SimpleNamespace
+    U = SimpleNamespace(**vars(L)); U.G = 8
+    U.group_map = torch.arange(8, dtype=torch.int32)
+    idx = L.group_map.long()
+    U.W1, U.W3, U.W2 = L.W1[idx].contiguous(), L.W3[idx].contiguous(), L.W2[idx].contiguous()
+    gu, outu, _ = gpu_layer(U, PATHS["prefill"])
+    assert (gu.expert_ids == g.expert_ids).all()
+    assert np.abs(out - outu).max() <= 2e-2 * (1 + np.abs(out).max())
+
+
+# ---------------------------------------------------------------------------------------------------
+# full-size configs in the launch configuration bench.py times: sampled tokens vs the oracle
+# ---------------------------------------------------------------------------------------------------
+def _sampled_parity(cfg, n_sample, seed=0):
+    L = make_layer(cfg, seed)
+    g, out, status = gpu_layer(L, 0)                           # BM_PATH_AUTO, as bench.py runs it
+    o = oracle_route(L)
+    assert status == 0
+    assert_routing_equal(g, o)
+    rng = np.random.default_rng(seed)
+    sel = set(rng.choice(cfg.T, size=min(n_sample, cfg.T), replace=False).tolist())
+    u_min = int(np.argmin(np.where(o.counts > 0, o.counts, 1 << 30)))     # least-populated group: all its tokens
+    sel |= set(o.row_token[o.offsets[u_min]:o.offsets[u_min + 1]][:16].tolist())
+    sel = np.array(sorted(sel), np.int32)
+    ref = oracle_forward(L, o, sel_tokens=sel)
+    worst = assert_out_close(out[sel], ref)
+    # properties that hold at any size: finite everywhere, no untouched (NaN-initialised) output
+    assert np.isfinite(out).all()
+    return worst
+
+
+def test_decode_config_full_size_sampled():
+    _sampled_parity(CONFIGS["decode"], 8)                       # BJ:configs[1], grouped G=4
+
+
+def test_decode_config_ungrouped_full_size_sampled():
+    _sampled_parity(identity_variant(CONFIGS["decode"]), 4)     # zero brownout comparison run
+
+
+def test_prefill_config_full_size_sampled():
+    _sampled_parity(CONFIGS["prefill"], 8)                      # BJ:configs[2]
+
+
+def test_finegrained_config_full_size_sampled():
+    _sampled_parity(CONFIGS["finegrained"], 24)                 # BJ:configs[3], shared experts, uneven groups
+
+
+@pytest.mark.parametrize("name", ["sweep_G8_T1_s1", "sweep_G15_T16_s2", "sweep_G60_T256_s0", "sweep_G30_T4096_s1"])
+def test_sweep_points_sampled(name):
+    from bm_inputs import get_config
+    _sampled_parity(get_config(name), 16)                       # BJ:configs[4]
