@@ -1,0 +1,463 @@
+#!/usr/bin/env python
+"""bench.py -- MoE-layer tokens/s of the grouped (and ungrouped) layer on B200, % of roofline.
+
+A "step" is one pass of the whole hot path (bm_route + bm_moe_forward: SURVEY.md 8(a) rows 1-13) over one
+batch of synthetic tokens.  Headline workload at N=1: BASELINE.json configs[1] (Mixtral-8x7B-shaped
+decode layer, T=64, G=4 united groups), the configuration the metric is quoted on; the same layer run
+ungrouped (G=8, identity map) and as a prefill batch (configs[2], T=8192) are reported beside it.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-extras]
+
+For N>1 launch under torchrun (one rank per GPU); tokens are sharded across ranks with no data-path
+collective (weak scaling: every rank runs the same layer on its own batch).
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+import torch
+
+from bm_inputs import CONFIGS, bf16_bits, identity_variant, make_layer
+
+METRIC = "moe_layer_tokens_per_s"
+UNIT = "tokens/s"
+L2_BYTES = 126e6
+
+
+# ---------------------------------------------------------------------------------------------------
+# peaks, roofline arithmetic
+# ---------------------------------------------------------------------------------------------------
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            p = json.load(fh)
+        return dict(hbm_gbs=float(p["hbm_gbs"]), bf16_tflops=float(p["bf16_tflops"]),
+                    bf16_tflops_sustained=float(p.get("bf16_tflops_sustained", p["bf16_tflops"])),
+                    source="measured (MEASURED_PEAKS.json)")
+    # B200_PROFILING.md fallback: an earlier measurement on this pool
+    return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, source="fallback (B200_PROFILING.md)")
+
+
+def layer_work(cfg, A, G_act):
+    """Algorithmic FLOPs and bytes of one layer call; H, xs and split-K partials are
+    implementation traffic and are not counted."""
+    T, D, F, E, S = cfg.T, cfg.D, cfg.F, cfg.E, cfg.S
+    flops = A * 6 * D * F + S * T * 6 * D * F + 2 * T * E * D
+    nbytes = (G_act + S) * 3 * D * F * 2 + T * D * 2 + T * D * 2 + E * D * 2
+    return flops, nbytes
+
+
+def gemm1_work(cfg, A, G_act):
+    """Algorithmic work of the dominant kernel (GEMM1 + SwiGLU): W1, W3 of the active groups once, the
+    gathered rows in, H out (bf16)."""
+    T, D, F, S = cfg.T, cfg.D, cfg.F, cfg.S
+    rows = A + S * T
+    return rows * 4 * D * F, (G_act + S) * 2 * D * F * 2 + rows * D * 2 + rows * F * 2
+
+
+# ---------------------------------------------------------------------------------------------------
+# clocks during the timed region (NVML polling thread)
+# ---------------------------------------------------------------------------------------------------
+class ClockSampler:
+    REASONS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+               0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.ok = [], set(), False
+        self._stop = threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = index
+            if vis:
+                ids = [v for v in vis.split(",") if v.strip()]
+                if index < len(ids) and ids[index].strip().isdigit():
+                    phys = int(ids[index])
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as exc:  # NVML missing: report that clocks were not sampled
+            self.err = repr(exc)
+            self.max_mhz = None
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)) if hasattr(
+                    nv, "nvmlDeviceGetCurrentClocksEventReasons") else int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for bit, name in self.REASONS.items():
+                    if mask & bit and name != "gpu_idle":
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(0.005)
+
+    def __enter__(self):
+        if self.ok:
+            self.t = threading.Thread(target=self._run, daemon=True)
+            self.t.start()
+        return self
+
+    def __exit__(self, *a):
+        if self.ok:
+            self._stop.set()
+            self.t.join()
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "note": "NVML sampling unavailable"}
+        return {"sm_mhz": statistics.median(self.samples), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ---------------------------------------------------------------------------------------------------
+# distributed plumbing
+# ---------------------------------------------------------------------------------------------------
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def barrier(ws):
+    if ws > 1:
+        torch.distributed.barrier()
+
+
+def max_over_ranks(v: float, ws: int, device) -> float:
+    if ws == 1:
+        return v
+    t = torch.tensor([v], dtype=torch.float64, device=device)
+    torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+    return float(t.item())
+
+
+# ---------------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------------
+class DeviceLayer:
+    """One layer resident in HBM: weights, router, group map, workspace, routing arrays."""
+
+    def __init__(self, cfg, seed, x_seed, weights_from=None, keep_host_weights=False):
+        import paper_2607_04164_b200 as bm
+        self.bm, self.cfg = bm, cfg
+        L = make_layer(cfg, seed, weights=weights_from is None)
+        if x_seed != seed:   # ranks share the layer, not the tokens
+            L.x = make_layer(cfg, x_seed, weights=False).x
+        self.host = L
+        self.x = L.x.cuda()
+        self.W_router = L.W_router.cuda()
+        self.bias = None if L.router_bias is None else L.router_bias.cuda()
+        self.gmap = L.group_map.cuda()
+        if weights_from is None:
+            self.W1, self.W3, self.W2 = L.W1.cuda(), L.W3.cuda(), L.W2.cuda()
+            if not keep_host_weights:
+                L.W1 = L.W3 = L.W2 = None      # free the host copies (1.4 - 2.8 GB)
+        else:
+            self.W1, self.W3, self.W2 = weights_from.W1, weights_from.W3, weights_from.W2
+        self.ws = bm.alloc_workspace(cfg.T, cfg.D, cfg.F, cfg.E, cfg.K, cfg.G, cfg.S)
+        self.routing = bm.Routing(cfg.T, cfg.K, cfg.G)
+        self.out = torch.empty((cfg.T, cfg.D), dtype=torch.bfloat16, device="cuda")
+        self.x_pinned = L.x.pin_memory()
+        self.out_pinned = torch.empty((cfg.T, cfg.D), dtype=torch.bfloat16).pin_memory()
+        self.x_stage = torch.empty_like(self.x)
+
+    def step(self):
+        bm, c = self.bm, self.cfg
+        bm.bm_route(self.x, self.W_router, self.bias, c.K, self.gmap, c.G, self.routing, self.ws)
+        bm.bm_moe_forward(self.x, self.routing, self.W1, self.W3, self.W2, self.out, self.ws, S=c.S)
+
+    def step_host(self):
+        bm, c = self.bm, self.cfg
+        bm.bm_moe_layer_host(self.x_pinned, self.W_router, self.bias, c.K, self.gmap, c.G, self.W1, self.W3, self.W2,
+                             c.S, self.out_pinned, self.x_stage, self.out, self.routing, self.ws)
+
+    def realised(self):
+        counts = self.routing.counts.cpu().numpy()
+        return int(counts.sum()), int((counts > 0).sum()), counts.tolist()
+
+
+def timed_loop(fn, steps, warmup, ws, device, sampler=None):
+    """W warm-up steps, then exactly `steps` steps between barrier+synchronize, timed with CUDA events on
+    the launching stream; returns the max over ranks in seconds."""
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    barrier(ws)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ctx = sampler if sampler is not None else _Null()
+    with ctx:
+        e0.record()
+        for _ in range(steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+    barrier(ws)
+    torch.cuda.synchronize()
+    return max_over_ranks(e0.elapsed_time(e1) / 1e3, ws, device)
+
+
+class _Null:
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        return False
+
+
+def kernel_time(layer, kernel, steps, warmup):
+    """Average device time of one kernel kind per step, from CUDA events recorded inside the library on
+    the launching stream (bm_profile_*), over `steps` timed steps after warm-up."""
+    bm = layer.bm
+    for _ in range(warmup):
+        layer.step()
+    torch.cuda.synchronize()
+    bm.profile_enable(kernel, steps + 4)
+    for _ in range(steps):
+        layer.step()
+    torch.cuda.synchronize()
+    ms, n = bm.profile_read()
+    bm.profile_enable(None)
+    return ms / 1e3 / max(n, 1), n
+
+
+def roofline_times(cfg, A, G_act, peaks):
+    flops, nbytes = layer_work(cfg, A, G_act)
+    t_flop = flops / (peaks["bf16_tflops"] * 1e12)
+    t_hbm = nbytes / (peaks["hbm_gbs"] * 1e9)
+    return flops, nbytes, t_flop, t_hbm
+
+
+def measure(layer, steps, warmup, ws, device, peaks, sampler=None, with_e2e=True, prof_steps=None):
+    cfg = layer.cfg
+    bm = layer.bm
+    l0 = bm.launch_count()
+    t = timed_loop(layer.step, steps, warmup, ws, device, sampler)
+    launches_per_step = (bm.launch_count() - l0) // (steps + warmup)
+    status = bm.bm_device_status(layer.ws)
+    A, G_act, counts = layer.realised()
+    flops, nbytes, t_flop, t_hbm = roofline_times(cfg, A, G_act, peaks)
+    t_step = t / steps
+    res = dict(tokens_per_s=ws * cfg.T / t_step, ms_per_step=t_step * 1e3, A=A, G_act=G_act, counts=counts,
+               flops=flops, bytes=nbytes, t_flop_us=t_flop * 1e6, t_hbm_us=t_hbm * 1e6,
+               bound="hbm" if t_hbm >= t_flop else "tensor", roofline_frac=max(t_flop, t_hbm) / t_step,
+               achieved_gbs=nbytes / t_step / 1e9, achieved_tflops=flops / t_step / 1e12,
+               launches_per_step=launches_per_step, gpu_launches=launches_per_step * steps, device_status=status)
+    if with_e2e:
+        te = timed_loop(layer.step_host, max(steps // 2, 3), max(warmup // 2, 3), ws, device)
+        res["e2e_tokens_per_s"] = ws * cfg.T / (te / max(steps // 2, 3))
+    # dominant kernel: GEMM1 + SwiGLU (two thirds of the weight bytes / FLOPs)
+    ps = prof_steps or min(steps, 50)
+    kt, n = kernel_time(layer, "gemm1", ps, 3)
+    kflops, kbytes = gemm1_work(cfg, A, G_act)
+    res["gemm1"] = dict(avg_us=kt * 1e6, launches_timed=n, alg_bytes=kbytes, alg_flops=kflops,
+                        gbs=kbytes / kt / 1e9, tflops=kflops / kt / 1e12)
+    kt2, n2 = kernel_time(layer, "gemm2", ps, 3)
+    res["gemm2"] = dict(avg_us=kt2 * 1e6, launches_timed=n2)
+    return res
+
+
+def load_traffic(kind):
+    """dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/), or None."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(path):
+        try:
+            with open(path) as fh:
+                return json.load(fh).get(kind)
+        except Exception:
+            return None
+    return None
+
+
+def cpu_baseline(L, budget_s=12.0):
+    """The oracle as it stands (never tuned for this), timed on this box's host cores on a bounded sample
+    of the same workload: whole batches of the layer if one takes seconds, else a token prefix."""
+    import oracle
+    cfg = L.cfg
+    xb, wr = bf16_bits(L.x), bf16_bits(L.W_router)
+    bias = None if L.router_bias is None else L.router_bias.numpy()
+    W1, W3, W2 = bf16_bits(L.W1), bf16_bits(L.W3), bf16_bits(L.W2)
+    gm = L.group_map.numpy()
+    cores = oracle.num_threads()
+
+    def run(n):
+        t0 = time.perf_counter()
+        r = oracle.route(xb[:n], wr, bias, cfg.K, gm, cfg.G)
+        oracle.moe_forward(xb[:n], r, W1, W3, W2, cfg.S)
+        return time.perf_counter() - t0
+
+    n0 = min(cfg.T, max(2, cores // max(cfg.K, 1)))
+    t_probe = run(n0)                                   # also warms the page cache
+    n = int(min(cfg.T, max(n0, n0 * budget_s / max(t_probe, 1e-3))))
+    reps = max(1, int(budget_s / max(t_probe * n / n0, 1e-3))) if n == cfg.T else 1
+    t = sum(run(n) for _ in range(reps))
+    return dict(value=n * reps / t, unit=UNIT, cores=cores, kind="oracle",
+                sample=f"{reps} x the first {n} of {cfg.T} tokens of '{cfg.name}' (oracle route + forward), {t:.1f} s")
+
+
+def run_ours(args):
+    rank, local_rank, ws = dist_env()
+    torch.cuda.set_device(local_rank)
+    device = torch.device("cuda", local_rank)
+    if ws > 1:
+        torch.distributed.init_process_group("nccl", device_id=device)
+    import paper_2607_04164_b200 as bm
+    bm.lib()
+    peaks = load_peaks()
+    cfg = CONFIGS[args.config]
+    steps, warmup = args.steps, max(args.warmup, 3)
+
+    layer = DeviceLayer(cfg, seed=0, x_seed=rank, keep_host_weights=(rank == 0 and ws == 1 and not args.no_cpu))
+    sampler = ClockSampler(local_rank)
+    main = measure(layer, steps, warmup, ws, device, peaks, sampler)
+    clocks = sampler.summary()
+
+    extras = {}
+    if not args.no_extras and ws == 1:
+        # same layer as a prefill batch (BJ:configs[2]) -- shares the weights already in HBM
+        if args.config == "decode":
+            pf = DeviceLayer(CONFIGS["prefill"], seed=0, x_seed=rank, weights_from=layer)
+            extras["prefill_grouped"] = measure(pf, max(steps // 20, 5), 3, ws, device, peaks, with_e2e=False, prof_steps=5)
+            del pf
+        # the ungrouped comparison run (zero brownout: G = E, identity map)
+        ucfg = identity_variant(cfg)
+        ul = DeviceLayer(ucfg, seed=0, x_seed=rank)
+        extras["ungrouped"] = measure(ul, steps, warmup, ws, device, peaks, with_e2e=False)
+        extras["grouped_over_ungrouped"] = main["tokens_per_s"] / extras["ungrouped"]["tokens_per_s"]
+        if args.config == "decode":
+            upf = DeviceLayer(identity_variant(CONFIGS["prefill"]), seed=0, x_seed=rank, weights_from=ul)
+            extras["prefill_ungrouped"] = measure(upf, max(steps // 20, 5), 3, ws, device, peaks, with_e2e=False, prof_steps=5)
+            del upf
+        del ul
+        torch.cuda.empty_cache()
+
+    cpu = None
+    if rank == 0 and ws == 1 and not args.no_cpu:
+        host = layer.host
+        del layer
+        torch.cuda.empty_cache()
+        cpu = cpu_baseline(host)
+
+    if rank == 0:
+        g1 = main["gemm1"]
+        bound = main["bound"]
+        if bound == "hbm":
+            roof = dict(bound="hbm", achieved=g1["gbs"], peak=peaks["hbm_gbs"], unit="GB/s",
+                        frac=g1["gbs"] / peaks["hbm_gbs"], traffic=load_traffic(args.config + "_gemm1"))
+        else:
+            roof = dict(bound="tensor", achieved=g1["tflops"], peak=peaks["bf16_tflops"], unit="TFLOP/s",
+                        frac=g1["tflops"] / peaks["bf16_tflops"], traffic=load_traffic(args.config + "_gemm1"))
+        roof.update(kernel="gemm_kernel<GEMM1+SwiGLU>", avg_launch_us=g1["avg_us"], launches_timed=g1["launches_timed"],
+                    alg_bytes_per_launch=g1["alg_bytes"], alg_flops_per_launch=g1["alg_flops"], peak_source=peaks["source"],
+                    layer_frac=main["roofline_frac"], layer_bound=bound)
+        weight_bytes = (cfg.G + cfg.S) * 3 * cfg.D * cfg.F * 2
+        line = dict(
+            metric=METRIC, value=main["tokens_per_s"], unit=UNIT, n_gpus=ws, steps=steps, warmup=warmup,
+            ms_per_step=main["ms_per_step"], higher_is_better=True, scaling="weak", vs_baseline=None,
+            dtype="bf16", data="synthetic",
+            config=dict(workload=f"BASELINE.json configs[{ {'tiny':0,'decode':1,'prefill':2,'finegrained':3}.get(args.config, 4)}] '{cfg.name}': "
+                                 f"T={cfg.T} D={cfg.D} F={cfg.F} E={cfg.E} top-{cfg.K} G={cfg.G} S={cfg.S} zipf_s={cfg.zipf_s}, seed 0",
+                        tokens_per_step_per_gpu=cfg.T, parallelism=f"dp{ws} (tokens sharded, weights replicated, no collective)",
+                        l2=f"weights {weight_bytes / 1e6:.0f} MB per step "
+                           + ("> 126 MB L2: streamed from HBM every step, no flush needed" if weight_bytes > 2 * L2_BYTES
+                              else "<= L2: NOT cold (small config)"),
+                        A=main["A"], G_act=main["G_act"], counts=main["counts"], path="auto"),
+            e2e=dict(value=main.get("e2e_tokens_per_s"), unit=UNIT, h2d_bytes_per_step=cfg.T * cfg.D * 2,
+                     d2h_bytes_per_step=cfg.T * cfg.D * 2, api="bm_moe_layer_host (pinned host x -> host out, weights resident)"),
+            gpu_launches=main["gpu_launches"], launches_per_step=main["launches_per_step"],
+            clocks=clocks, roofline=roof, cpu_baseline=cpu,
+            layer=dict(roofline_frac=main["roofline_frac"], bound=bound, achieved_gbs=main["achieved_gbs"],
+                       achieved_tflops=main["achieved_tflops"], t_hbm_us=main["t_hbm_us"], t_flop_us=main["t_flop_us"],
+                       gemm1_us=main["gemm1"]["avg_us"], gemm2_us=main["gemm2"]["avg_us"], device_status=main["device_status"]),
+            extras=extras,
+        )
+        print(json.dumps(line))
+    if ws > 1:
+        torch.distributed.destroy_process_group()
+
+
+# ---------------------------------------------------------------------------------------------------
+# reference arm: the oracle on the host cores (tier framing (4))
+# ---------------------------------------------------------------------------------------------------
+def run_reference(args):
+    rank, _, ws = dist_env()
+    if rank != 0:
+        return
+    import oracle
+    oracle.build()
+    cfg = CONFIGS[args.config]
+    steps, warmup = args.steps, args.warmup
+    L = make_layer(cfg, 0)
+    xb, wr = bf16_bits(L.x), bf16_bits(L.W_router)
+    bias = None if L.router_bias is None else L.router_bias.numpy()
+    W1, W3, W2 = bf16_bits(L.W1), bf16_bits(L.W3), bf16_bits(L.W2)
+    gm = L.group_map.numpy()
+    cores = oracle.num_threads()
+    # bounded sample per step: sized so that steps + warmup end within a few minutes
+    n = min(cfg.T, max(2, cores // max(cfg.K, 1)))
+    sel = np.arange(n, dtype=np.int32)
+
+    def step():
+        r = oracle.route(xb[:n], wr, bias, cfg.K, gm, cfg.G)
+        oracle.moe_forward(xb[:n], r, W1, W3, W2, cfg.S)
+
+    t0 = time.perf_counter()
+    step()
+    t1 = time.perf_counter() - t0
+    budget = 150.0
+    max_steps = max(1, int(budget / max(t1, 1e-3)))
+    w = min(warmup, max(0, max_steps // 4))
+    k = max(1, min(steps, max_steps - w))
+    for _ in range(w):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(k):
+        step()
+    t = time.perf_counter() - t0
+    v = n * k / t
+    sample = f"first {n} of {cfg.T} tokens of '{cfg.name}' per step, {k} steps timed ({t:.1f} s)"
+    print(json.dumps(dict(
+        impl="reference", metric=METRIC, value=v, unit=UNIT, n_gpus=ws, steps=k, warmup=w, ms_per_step=t / k * 1e3,
+        higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64 (router fp32)", data="synthetic",
+        config=dict(workload=f"'{cfg.name}': T={cfg.T} D={cfg.D} F={cfg.F} E={cfg.E} top-{cfg.K} G={cfg.G}, seed 0", sample=sample),
+        cpu_baseline=dict(value=v, unit=UNIT, cores=cores, kind="oracle", sample=sample),
+        e2e=dict(value=v, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="decode", choices=sorted(CONFIGS))
+    ap.add_argument("--no-extras", action="store_true", help="skip the ungrouped / prefill side measurements")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -14,9 +14,11 @@
  * Conventions
  *   - bf16 values are passed as uint16_t storage (bm_bf16).  Row-major, innermost dimension last.
  *   - Every pointer is a DEVICE pointer unless its comment says HOST.  The caller owns all memory;
- *     the library never allocates, frees or synchronises (except bm_moe_layer_host and
- *     bm_device_status, which say so) and borrows the buffers until the work enqueued on `stream`
+ *     the library never allocates, frees or synchronises (except bm_moe_layer_host,
+ *     bm_device_status and the bm_profile_* pair, which say so) and borrows the buffers until the work enqueued on `stream`
  *     has completed.  All device pointers must be 16-byte aligned.
+ *   - The first 256 bytes of `workspace` hold the device status word: zero them once after
+ *     allocation (or call bm_device_status once).
  *   - `stream` is a cudaStream_t (0 = the legacy default stream).
  *   - Return value: BM_OK (0) or a negative bm_status, checked synchronously on the host before
  *     anything is enqueued.  T == 0 is BM_OK and a no-op.  Data-dependent faults (a group_map entry
@@ -143,6 +145,20 @@ int bm_device_status(void *workspace, int32_t *host_out, bm_stream_t stream);
 /* Number of kernel launches the library has enqueued in this process so far (a HOST counter;
  * bench.py reports its difference over the timed region as `gpu_launches`). */
 long long bm_launch_count(void);
+
+/*
+ * Per-kernel device timing for the roofline report (bench.py).  bm_profile_enable(kernel, max_records)
+ * makes every later bm_route / bm_moe_forward call bracket the launches of `kernel` (BM_KERNEL_*) with a
+ * pair of CUDA events on the call's stream, up to max_records pairs; kernel = 0 switches it off and
+ * frees the events.  bm_profile_read SYNCHRONISES on the recorded events, writes the summed elapsed
+ * milliseconds and the number of pairs to HOST pointers and restarts the recording.  Not thread-safe.
+ */
+enum {
+    BM_KERNEL_NONE = 0, BM_KERNEL_ROUTER = 1, BM_KERNEL_PERMUTE = 2, BM_KERNEL_PREP = 3,
+    BM_KERNEL_GEMM1 = 4, BM_KERNEL_GEMM2 = 5, BM_KERNEL_FINALIZE = 6
+};
+int bm_profile_enable(int kernel, int max_records);
+int bm_profile_read(float *total_ms, int *n_records);
 
 /* Human-readable name of a bm_status code.  Never NULL. */
 const char *bm_status_string(int code);

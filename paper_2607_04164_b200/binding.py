@@ -20,7 +20,8 @@ BM_MAX_E, BM_MAX_K, BM_MAX_G = 512, 16, 512
 BM_DECODE_MAX_T = 256
 
 EXPORTS = ["bm_workspace_bytes", "bm_route", "bm_moe_forward", "bm_moe_forward_path", "bm_moe_layer_host",
-           "bm_device_status", "bm_launch_count", "bm_status_string"]
+           "bm_device_status", "bm_launch_count", "bm_status_string", "bm_profile_enable", "bm_profile_read"]
+KERNELS = {"router": 1, "permute": 2, "prep": 3, "gemm1": 4, "gemm2": 5, "finalize": 6}
 
 
 class BmRouting(ctypes.Structure):
@@ -63,6 +64,10 @@ def lib() -> ctypes.CDLL:
         L.bm_device_status.argtypes = [c_void_p, POINTER(c_int32), c_void_p]
         L.bm_launch_count.restype = c_longlong
         L.bm_launch_count.argtypes = []
+        L.bm_profile_enable.restype = c_int
+        L.bm_profile_enable.argtypes = [c_int, c_int]
+        L.bm_profile_read.restype = c_int
+        L.bm_profile_read.argtypes = [POINTER(c_float), POINTER(c_int)]
         L.bm_status_string.restype = ctypes.c_char_p
         L.bm_status_string.argtypes = [c_int]
         _lib = L
@@ -172,3 +177,19 @@ def bm_device_status(workspace, stream=None) -> int:
     if rc != BM_OK:
         raise BmError(rc, "bm_device_status")
     return int(v.value)
+
+
+def profile_enable(kernel: str | None, max_records: int = 0) -> None:
+    """Record CUDA-event pairs around the launches of one kernel kind (KERNELS), None = off."""
+    rc = lib().bm_profile_enable(0 if kernel is None else KERNELS[kernel], max_records)
+    if rc != BM_OK:
+        raise BmError(rc, "bm_profile_enable")
+
+
+def profile_read():
+    """(summed milliseconds, number of event pairs) since the last read; synchronises on the events."""
+    ms, n = c_float(0), c_int(0)
+    rc = lib().bm_profile_read(ctypes.byref(ms), ctypes.byref(n))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_profile_read")
+    return float(ms.value), int(n.value)

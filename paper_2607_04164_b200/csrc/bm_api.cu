@@ -10,6 +10,16 @@ namespace bm {
 static std::atomic<long long> g_launches{0};
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
+static int g_prof_kernel = 0, g_prof_max = 0, g_prof_n = 0;
+static cudaEvent_t *g_prof_start = nullptr, *g_prof_stop = nullptr;
+
+void profile_begin(int kernel, cudaStream_t stream) {
+    if (kernel == g_prof_kernel && g_prof_n < g_prof_max) cudaEventRecord(g_prof_start[g_prof_n], stream);
+}
+void profile_end(int kernel, cudaStream_t stream) {
+    if (kernel == g_prof_kernel && g_prof_n < g_prof_max) cudaEventRecord(g_prof_stop[g_prof_n++], stream);
+}
+
 int num_sms() {
     static int sms = 0;
     if (sms == 0) {
@@ -86,11 +96,15 @@ int bm_route(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, const floa
             return BM_ERR_CUDA;
         return BM_OK;
     }
+    profile_begin(BM_KERNEL_ROUTER, st);
     if (launch_router(x, T, D, W_router, router_bias, E, K, group_map, G, *routing, status, st) != cudaSuccess)
         return BM_ERR_CUDA;
+    profile_end(BM_KERNEL_ROUTER, st);
+    profile_begin(BM_KERNEL_PERMUTE, st);
     if (launch_permute(T, K, G, *routing, reinterpret_cast<int32_t *>(ws + full.block_hist), status, st) !=
         cudaSuccess)
         return BM_ERR_CUDA;
+    profile_end(BM_KERNEL_PERMUTE, st);
     return BM_OK;
 }
 
@@ -170,6 +184,39 @@ int bm_device_status(void *workspace, int32_t *host_out, bm_stream_t stream) {
         cudaMemsetAsync(workspace, 0, sizeof(int32_t), st) != cudaSuccess ||
         cudaStreamSynchronize(st) != cudaSuccess)
         return BM_ERR_CUDA;
+    return BM_OK;
+}
+
+int bm_profile_enable(int kernel, int max_records) {
+    for (int i = 0; i < g_prof_max; ++i) { cudaEventDestroy(g_prof_start[i]); cudaEventDestroy(g_prof_stop[i]); }
+    delete[] g_prof_start; delete[] g_prof_stop;
+    g_prof_start = g_prof_stop = nullptr;
+    g_prof_kernel = 0; g_prof_max = 0; g_prof_n = 0;
+    if (kernel == BM_KERNEL_NONE || max_records <= 0) return BM_OK;
+    if (kernel < BM_KERNEL_ROUTER || kernel > BM_KERNEL_FINALIZE) return BM_ERR_SHAPE;
+    if (device_ok() != 1) return BM_ERR_CUDA;
+    g_prof_start = new cudaEvent_t[max_records];
+    g_prof_stop = new cudaEvent_t[max_records];
+    for (int i = 0; i < max_records; ++i)
+        if (cudaEventCreate(&g_prof_start[i]) != cudaSuccess || cudaEventCreate(&g_prof_stop[i]) != cudaSuccess)
+            return BM_ERR_CUDA;
+    g_prof_kernel = kernel; g_prof_max = max_records;
+    return BM_OK;
+}
+
+int bm_profile_read(float *total_ms, int *n_records) {
+    if (!total_ms || !n_records) return BM_ERR_NULL;
+    float sum = 0.f;
+    for (int i = 0; i < g_prof_n; ++i) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(g_prof_stop[i]) != cudaSuccess ||
+            cudaEventElapsedTime(&ms, g_prof_start[i], g_prof_stop[i]) != cudaSuccess)
+            return BM_ERR_CUDA;
+        sum += ms;
+    }
+    *total_ms = sum;
+    *n_records = g_prof_n;
+    g_prof_n = 0;
     return BM_OK;
 }
 

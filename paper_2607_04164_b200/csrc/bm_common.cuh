@@ -53,6 +53,9 @@ __host__ inline Workspace workspace_layout(int T, int D, int F, int K, int G, in
 // ---------------------------------------------------------------------------------------------
 void count_launch(int n = 1);
 int num_sms();
+// bm_profile_*: record an event pair around the launches of one kernel kind (no-ops unless enabled)
+void profile_begin(int kernel, cudaStream_t stream);
+void profile_end(int kernel, cudaStream_t stream);
 
 // ---------------------------------------------------------------------------------------------
 // Internal kernel launchers (defined in the .cu files, called from bm_api.cu)

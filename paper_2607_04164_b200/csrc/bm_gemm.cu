@@ -491,9 +491,13 @@ cudaError_t launch_gemm(const CUtensorMap &a0, const CUtensorMap &a1, const CUte
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
+    constexpr int kid = (MODE == PF_GEMM1 || MODE == DC_GEMM1) ? BM_KERNEL_GEMM1 : BM_KERNEL_GEMM2;
+    profile_begin(kid, stream);
     kern<<<num_sms(), kThreads, kSmemBytes, stream>>>(a0, a1, w0, w1, p);
     count_launch();
-    return cudaGetLastError();
+    cudaError_t e = cudaGetLastError();
+    profile_end(kid, stream);
+    return e;
 }
 
 }  // namespace
@@ -505,11 +509,13 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
     // step 9 (+ schedule, + zero)
     {
         const int grid = sms * 4;
+        profile_begin(BM_KERNEL_PREP, stream);
         prep_kernel<<<grid, 256, 0, stream>>>(a.x, a.T, a.D, a.K, a.G, a.S, a.r.counts, a.r.offsets, a.r.row_token,
                                               a.sched, a.xs, a.out_acc, a.status);
         count_launch();
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
+        profile_end(BM_KERNEL_PREP, stream);
     }
 
     GemmParams p{};
@@ -555,9 +561,12 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
         int grid = (int)((n8 + 255) / 256);
         if (grid > sms * 8) grid = sms * 8;
         if (grid < 1) grid = 1;
+        profile_begin(BM_KERNEL_FINALIZE, stream);
         finalize_kernel<<<grid, 256, 0, stream>>>(a.out_acc, a.out, n8);
         count_launch();
-        return cudaGetLastError();
+        cudaError_t e = cudaGetLastError();
+        profile_end(BM_KERNEL_FINALIZE, stream);
+        return e;
     }
 }
 
