@@ -245,7 +245,7 @@ def roofline_times(cfg, A, G_act, peaks):
     return flops, nbytes, t_flop, t_hbm
 
 
-def measure(layer, steps, warmup, ws, device, peaks, sampler=None, with_e2e=True, prof_steps=None):
+def measure(layer, steps, warmup, ws, device, peaks, sampler=None, with_e2e=True, prof_steps=None, breakdown=False):
     cfg = layer.cfg
     bm = layer.bm
     l0 = bm.launch_count()
@@ -271,6 +271,10 @@ def measure(layer, steps, warmup, ws, device, peaks, sampler=None, with_e2e=True
                         gbs=kbytes / kt / 1e9, tflops=kflops / kt / 1e12)
     kt2, n2 = kernel_time(layer, "gemm2", ps, 3)
     res["gemm2"] = dict(avg_us=kt2 * 1e6, launches_timed=n2)
+    if breakdown:
+        # every kernel kind in isolation (PDL is off while the library records events)
+        res["breakdown_us"] = {k: kernel_time(layer, k, ps, 2)[0] * 1e6 for k in ("router", "permute", "prep", "finalize")}
+        res["breakdown_us"].update(gemm1=kt * 1e6, gemm2=kt2 * 1e6)
     return res
 
 
@@ -326,7 +330,7 @@ def run_ours(args):
 
     layer = DeviceLayer(cfg, seed=0, x_seed=rank, keep_host_weights=(rank == 0 and ws == 1 and not args.no_cpu))
     sampler = ClockSampler(local_rank)
-    main = measure(layer, steps, warmup, ws, device, peaks, sampler)
+    main = measure(layer, steps, warmup, ws, device, peaks, sampler, breakdown=True)
     clocks = sampler.summary()
 
     extras = {}
@@ -385,7 +389,8 @@ def run_ours(args):
             clocks=clocks, roofline=roof, cpu_baseline=cpu,
             layer=dict(roofline_frac=main["roofline_frac"], bound=bound, achieved_gbs=main["achieved_gbs"],
                        achieved_tflops=main["achieved_tflops"], t_hbm_us=main["t_hbm_us"], t_flop_us=main["t_flop_us"],
-                       gemm1_us=main["gemm1"]["avg_us"], gemm2_us=main["gemm2"]["avg_us"], device_status=main["device_status"]),
+                       gemm1_us=main["gemm1"]["avg_us"], gemm2_us=main["gemm2"]["avg_us"], breakdown_us=main.get("breakdown_us"),
+                       device_status=main["device_status"]),
             extras=extras,
         )
         print(json.dumps(line))

@@ -1,6 +1,7 @@
 // bm_api.cu -- the C-ABI entry points of include/bm.h: argument checking, workspace carving, path
 // dispatch.  No compute happens on the host and there is no CPU fallback.
 #include <atomic>
+#include <cstdlib>
 #include <cstring>
 
 #include "bm_common.cuh"
@@ -18,6 +19,21 @@ void profile_begin(int kernel, cudaStream_t stream) {
 }
 void profile_end(int kernel, cudaStream_t stream) {
     if (kernel == g_prof_kernel && g_prof_n < g_prof_max) cudaEventRecord(g_prof_stop[g_prof_n++], stream);
+}
+
+int tune_int(const char *env_name, int dflt) {
+    const char *v = std::getenv(env_name);
+    if (!v || !*v) return dflt;
+    char *end = nullptr;
+    const long r = std::strtol(v, &end, 10);
+    return (end && *end == '\0') ? (int)r : dflt;
+}
+
+// PDL is off while bm_profile_* records (events between launches would time overlapped kernels) and
+// when BM_PDL=0 is set in the environment.
+bool pdl_enabled() {
+    static const int env = tune_int("BM_PDL", 1);
+    return env != 0 && g_prof_kernel == 0;
 }
 
 int num_sms() {

@@ -57,6 +57,29 @@ int num_sms();
 void profile_begin(int kernel, cudaStream_t stream);
 void profile_end(int kernel, cudaStream_t stream);
 
+// Programmatic dependent launch (PDL).  Every kernel of the path is launched with
+// cudaLaunchAttributeProgrammaticStreamSerialization (unless bm_profile_* is recording or BM_PDL=0), so
+// its prologue overlaps the tail of its predecessor.  Contract for every kernel launched this way:
+// all threads call grid_dep_wait() before touching anything a predecessor wrote (or will overwrite)
+// and before exiting -- it returns once ALL prerequisite grids have completed and flushed, so the chain
+// of launches stays transitively ordered -- and grid_dep_launch() only AFTER that wait.
+bool pdl_enabled();
+int tune_int(const char *env_name, int dflt);      // integer tuning override from the environment
+
+template <typename... KArgs, typename... Args>
+cudaError_t launch_kernel(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream,
+                          Args... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl_enabled() ? 1 : 0;
+    count_launch();
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
 // ---------------------------------------------------------------------------------------------
 // Internal kernel launchers (defined in the .cu files, called from bm_api.cu)
 // ---------------------------------------------------------------------------------------------
@@ -87,6 +110,9 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
 // ---------------------------------------------------------------------------------------------
 // Device helpers
 // ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void grid_dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void grid_dep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 __device__ __forceinline__ float bf16_lo(uint32_t u) { return __uint_as_float(u << 16); }
 __device__ __forceinline__ float bf16_hi(uint32_t u) { return __uint_as_float(u & 0xffff0000u); }
 

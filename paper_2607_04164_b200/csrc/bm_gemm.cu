@@ -27,16 +27,18 @@ namespace bm {
 namespace {
 
 constexpr int kBlockK = 64;                 // bf16 elements per stage row = 128 bytes = one swizzle row
-constexpr int kStages = 4;
+constexpr int kMaxStages = 12;
 constexpr int kTileBytes16K = 128 * 128;    // 128 rows x 128 bytes
-constexpr int kStageBytes = 3 * kTileBytes16K;
 constexpr int kAccStages = 2;
 constexpr int kAccCols = 256;
 constexpr int kTmemCols = kAccStages * kAccCols;
 constexpr int kThreads = 192;
 constexpr int kChunkRows = 128;
 constexpr int kMaxSeg = BM_MAX_G + kMaxShared;
-constexpr size_t kSmemBytes = 1024 /*align slack*/ + (size_t)kStages * kStageBytes + 256;
+constexpr size_t kSmemMax = 232448;         // 227 KB, the per-CTA opt-in limit of sm_100
+constexpr size_t kSmemBars = 256;           // (2*kMaxStages + 2*kAccStages) mbarriers + the TMEM base address
+constexpr size_t kSmemRing = kSmemMax - 1024 /*align slack*/ - kSmemBars;
+static_assert((2 * kMaxStages + 2 * kAccStages) * 8 + 4 <= kSmemBars, "barrier block too small");
 
 enum Mode { PF_GEMM1 = 0, PF_GEMM2 = 1, DC_GEMM1 = 2, DC_GEMM2 = 3 };
 
@@ -48,6 +50,10 @@ static_assert(kSchedChunk0 + kMaxSeg + 1 <= kSchedInts, "sched too small");
 
 struct GemmParams {
     int T, D, F, K, G, S, TK;
+    int stages;         // depth of the shared-memory ring (<= kMaxStages)
+    int stage_bytes;    // bytes of one ring stage (multiple of 1024)
+    int off_b;          // decode: offset of the token rows (MMA B operand) inside a stage
+    int npad_box;       // decode: rows of the token box every stage loads (host: T rounded up to 32, <= 128)
     int kblocks;        // k-blocks of one item (per split)
     int ksplit;         // K splits (DC_GEMM2), else 1
     int R;              // weight rows per tile (prefill: 128 for GEMM1 per matrix, 256 for GEMM2)
@@ -126,20 +132,23 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
 
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + (size_t)kStages * kStageBytes);
-    uint64_t *full = bars;                       // [kStages]
-    uint64_t *empty = bars + kStages;            // [kStages]
-    uint64_t *tfull = bars + 2 * kStages;        // [kAccStages]
+    const int n_stages = p.stages;
+    const uint32_t stage_bytes = (uint32_t)p.stage_bytes;
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + (size_t)n_stages * stage_bytes);
+    uint64_t *full = bars;                       // [kMaxStages]
+    uint64_t *empty = bars + kMaxStages;         // [kMaxStages]
+    uint64_t *tfull = bars + 2 * kMaxStages;     // [kAccStages]
     uint64_t *tempty = tfull + kAccStages;       // [kAccStages]
     uint32_t *tmem_ptr = reinterpret_cast<uint32_t *>(tempty + kAccStages);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
+    // ---- prologue: nothing here depends on a predecessor kernel, so under PDL it overlaps its tail ----
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tmap(&tm_act0);
         ptx::prefetch_tmap(&tm_w0);
         if (kGemm1) { ptx::prefetch_tmap(&tm_act1); ptx::prefetch_tmap(&tm_w1); }
-        for (int i = 0; i < kStages; ++i) { ptx::mbar_init(&full[i], 1); ptx::mbar_init(&empty[i], 1); }
+        for (int i = 0; i < n_stages; ++i) { ptx::mbar_init(&full[i], 1); ptx::mbar_init(&empty[i], 1); }
         for (int i = 0; i < kAccStages; ++i) { ptx::mbar_init(&tfull[i], 1); ptx::mbar_init(&tempty[i], 4); }
         ptx::fence_barrier_init();
     }
@@ -150,92 +159,120 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
     const uint32_t tmem_base = *tmem_ptr;
 
     const int nkb = p.kblocks;
+    // bytes one stage receives: constant per launch (decode always loads the full padded token box)
+    const uint32_t stage_tx = !kDecode ? 3u * kTileBytes16K
+                                       : (uint32_t)((kGemm1 ? 2 : 1) * p.R * 128 + p.npad_box * 128);
 
+    // The producer and the MMA issuer run their loops with the WHOLE warp (warp-uniform control flow keeps
+    // addresses and descriptors in uniform registers) and elect one lane for the issuing instructions: the
+    // single-thread instruction stream per k-block is what paces a decode tile, so it is kept short.
     if (warp == 0) {
         // =========================== TMA producer ===========================
-        if (lane == 0) {
-            int stage = 0;
-            uint32_t phase = 0;
-            Item it;
-            for (int item = blockIdx.x; get_item<MODE>(p, item, it); item += gridDim.x) {
-                const CUtensorMap *tm_act = (kGemm1 && it.shared) ? &tm_act1 : &tm_act0;
-                const int wrow0 = it.wt * p.R;
-                const int npad = (it.n + 31) & ~31;
-                uint32_t bytes;
-                if (MODE == PF_GEMM1) bytes = 3 * kTileBytes16K;
-                else if (MODE == PF_GEMM2) bytes = 3 * kTileBytes16K;
-                else if (MODE == DC_GEMM1) bytes = 2 * p.R * 128 + npad * 128;
-                else bytes = p.R * 128 + npad * 128;
-                const int kb0 = it.ks * nkb;
-                for (int kb = 0; kb < nkb; ++kb) {
-                    ptx::mbar_wait(&empty[stage], phase ^ 1);
-                    uint8_t *st = smem + (size_t)stage * kStageBytes;
-                    ptx::mbar_arrive_expect_tx(&full[stage], bytes);
-                    const int kc = (kb0 + kb) * kBlockK;
+        int stage = 0;
+        uint32_t phase = 0;
+        Item it;
+        int item = blockIdx.x;
+        int kb_first = 0;
+        bool have;
+        if (MODE == DC_GEMM2) {
+            // W2 does not depend on the predecessor (GEMM1): fill the ring with weight tiles BEFORE the
+            // grid-dependency wait, so the HBM stream starts while GEMM1's last CTAs drain.  The schedule
+            // read by get_item was written by the prep kernel, which completed before GEMM1 (which
+            // triggers this launch only after its own wait) let this grid start.
+            have = get_item<MODE>(p, item, it);
+            const int pre = have ? min(n_stages, nkb) : 0;
+            if (ptx::elect_one())
+                for (int kb = 0; kb < pre; ++kb) {
+                    ptx::mbar_arrive_expect_tx(&full[kb], stage_tx);
+                    ptx::tma_load_3d(smem + (size_t)kb * stage_bytes, &tm_w0, &full[kb], (it.ks * nkb + kb) * kBlockK,
+                                     it.wt * p.R, it.u, ptx::kEvictFirst);
+                }
+            __syncwarp();
+            grid_dep_wait();
+            if (ptx::elect_one())
+                for (int kb = 0; kb < pre; ++kb)
+                    ptx::tma_load_2d(smem + (size_t)kb * stage_bytes + p.off_b, &tm_act0, &full[kb],
+                                     (it.ks * nkb + kb) * kBlockK, it.act_row0, ptx::kEvictLast);
+            __syncwarp();
+            kb_first = pre;
+            stage = pre;
+            if (stage == n_stages) { stage = 0; phase = 1; }
+        } else {
+            grid_dep_wait();
+            have = get_item<MODE>(p, item, it);
+        }
+        if (lane == 0) grid_dep_launch();
+        for (; have; item += gridDim.x, have = get_item<MODE>(p, item, it), kb_first = 0) {
+            const CUtensorMap *tm_act = (kGemm1 && it.shared) ? &tm_act1 : &tm_act0;
+            const int wrow0 = it.wt * p.R;
+            int kc = (it.ks * nkb + kb_first) * kBlockK;
+            for (int kb = kb_first; kb < nkb; ++kb, kc += kBlockK) {
+                ptx::mbar_wait(&empty[stage], phase ^ 1);
+                if (ptx::elect_one()) {
+                    uint8_t *st = smem + (size_t)stage * stage_bytes;
+                    ptx::mbar_arrive_expect_tx(&full[stage], stage_tx);
                     if (!kDecode) {
                         // A = 128 activation rows, B = 256 weight rows (W1|W3 tiles, or one W2 tile of 256)
                         ptx::tma_load_2d(st, tm_act, &full[stage], kc, it.act_row0, ptx::kEvictLast);
-                        if (MODE == PF_GEMM1) {
-                            ptx::tma_load_3d(st + kTileBytes16K, &tm_w0, &full[stage], kc, wrow0, it.u, ptx::kEvictFirst);
+                        ptx::tma_load_3d(st + kTileBytes16K, &tm_w0, &full[stage], kc, wrow0, it.u, ptx::kEvictFirst);
+                        if (MODE == PF_GEMM1)
                             ptx::tma_load_3d(st + 2 * kTileBytes16K, &tm_w1, &full[stage], kc, wrow0, it.u, ptx::kEvictFirst);
-                        } else {
-                            ptx::tma_load_3d(st + kTileBytes16K, &tm_w0, &full[stage], kc, wrow0, it.u, ptx::kEvictFirst);
-                        }
                     } else {
                         // M side = R weight rows (streamed once from HBM), N side = the group's token rows
+                        // (one box of npad_box rows; rows past the group's are loaded and never multiplied)
                         ptx::tma_load_3d(st, &tm_w0, &full[stage], kc, wrow0, it.u, ptx::kEvictFirst);
                         if (MODE == DC_GEMM1)
                             ptx::tma_load_3d(st + kTileBytes16K, &tm_w1, &full[stage], kc, wrow0, it.u, ptx::kEvictFirst);
-                        for (int b = 0; b < npad; b += 32)
-                            ptx::tma_load_2d(st + 2 * kTileBytes16K + b * 128, tm_act, &full[stage], kc,
-                                             it.act_row0 + b, ptx::kEvictLast);
+                        ptx::tma_load_2d(st + p.off_b, tm_act, &full[stage], kc, it.act_row0, ptx::kEvictLast);
                     }
-                    if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
+                __syncwarp();
+                if (++stage == n_stages) { stage = 0; phase ^= 1; }
             }
         }
     } else if (warp == 1) {
         // =========================== MMA issuer ===========================
-        if (lane == 0) {
-            int stage = 0;
-            uint32_t phase = 0;
-            int acc = 0;
-            uint32_t acc_phase = 0;
-            Item it;
-            for (int item = blockIdx.x; get_item<MODE>(p, item, it); item += gridDim.x) {
-                const int npad = (it.n + 31) & ~31;
-                const uint32_t idesc = kDecode ? ptx::make_idesc_bf16(128, npad) : ptx::make_idesc_bf16(128, 256);
-                ptx::mbar_wait(&tempty[acc], acc_phase ^ 1);
+        grid_dep_wait();
+        // descriptor low words: (smem address >> 4) | LBO; the high word (SBO, version, swizzle) is constant
+        const uint32_t a_lo0 = ptx::smem_desc_lo(ptx::smem_u32(smem));
+        const uint32_t b_off = (uint32_t)(kDecode ? p.off_b : kTileBytes16K) >> 4;
+        const uint32_t stage_step = stage_bytes >> 4;
+        uint32_t a_lo = a_lo0;
+        int stage = 0;
+        uint32_t phase = 0;
+        int acc = 0;
+        uint32_t acc_phase = 0;
+        Item it;
+        for (int item = blockIdx.x; get_item<MODE>(p, item, it); item += gridDim.x) {
+            const uint32_t idesc = kDecode ? ptx::make_idesc_bf16(128, (it.n + 31) & ~31) : ptx::make_idesc_bf16(128, 256);
+            ptx::mbar_wait(&tempty[acc], acc_phase ^ 1);
+            ptx::tc_fence_after();
+            const uint32_t d_tmem = tmem_base + acc * kAccCols;
+            for (int kb = 0; kb < nkb; ++kb) {
+                ptx::mbar_wait(&full[stage], phase);
                 ptx::tc_fence_after();
-                const uint32_t d_tmem = tmem_base + acc * kAccCols;
-                for (int kb = 0; kb < nkb; ++kb) {
-                    ptx::mbar_wait(&full[stage], phase);
-                    ptx::tc_fence_after();
-                    const uint32_t sbase = ptx::smem_u32(smem + (size_t)stage * kStageBytes);
+                if (ptx::elect_one()) {
 #pragma unroll
                     for (int k = 0; k < kBlockK / 16; ++k) {
                         const uint32_t accum = (kb | k) ? 1u : 0u;
-                        const uint32_t koff = k * 32;      // 16 bf16 = 32 bytes inside the swizzled row
-                        if (!kDecode) {
-                            ptx::mma_bf16_ss(d_tmem, ptx::make_smem_desc_sw128(sbase + koff),
-                                             ptx::make_smem_desc_sw128(sbase + kTileBytes16K + koff), idesc, accum);
-                        } else {
-                            const uint64_t bdesc = ptx::make_smem_desc_sw128(sbase + 2 * kTileBytes16K + koff);
-                            ptx::mma_bf16_ss(d_tmem, ptx::make_smem_desc_sw128(sbase + koff), bdesc, idesc, accum);
-                            if (MODE == DC_GEMM1)
-                                ptx::mma_bf16_ss(d_tmem + 128, ptx::make_smem_desc_sw128(sbase + kTileBytes16K + koff),
-                                                 bdesc, idesc, accum);
-                        }
+                        const uint32_t ko = 2 * k;             // 16 bf16 = 32 bytes = 2 descriptor units
+                        ptx::mma_bf16_ss(d_tmem, ptx::smem_desc(a_lo + ko), ptx::smem_desc(a_lo + b_off + ko), idesc, accum);
+                        if (MODE == DC_GEMM1)
+                            ptx::mma_bf16_ss(d_tmem + 128, ptx::smem_desc(a_lo + (kTileBytes16K >> 4) + ko),
+                                             ptx::smem_desc(a_lo + b_off + ko), idesc, accum);
                     }
                     ptx::mma_commit(&empty[stage]);                  // frees the smem stage when the MMAs retire
                     if (kb == nkb - 1) ptx::mma_commit(&tfull[acc]);   // accumulator complete
-                    if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
-                if (++acc == kAccStages) { acc = 0; acc_phase ^= 1; }
+                __syncwarp();
+                a_lo += stage_step;
+                if (++stage == n_stages) { stage = 0; phase ^= 1; a_lo = a_lo0; }
             }
+            if (++acc == kAccStages) { acc = 0; acc_phase ^= 1; }
         }
     } else {
         // =========================== epilogue (warps 2..5) ===========================
+        grid_dep_wait();
         const int q = warp & 3;                      // TMEM lane quarter this warp may read
         const int row = q * 32 + lane;               // accumulator row (M index) owned by this thread
         int acc = 0;
@@ -366,6 +403,8 @@ prep_kernel(const bm_bf16 *__restrict__ x, int T, int D, int K, int G, int S,
             const int32_t *__restrict__ counts, const int32_t *__restrict__ offsets,
             const int32_t *__restrict__ row_token, int32_t *__restrict__ sched, bm_bf16 *__restrict__ xs,
             float *__restrict__ out_acc, int32_t *__restrict__ status) {
+    grid_dep_wait();
+    grid_dep_launch();
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         int n_seg = 0, chunks = 0;
         bool bad = false;
@@ -404,6 +443,8 @@ prep_kernel(const bm_bf16 *__restrict__ x, int T, int D, int K, int G, int S,
 
 __global__ void __launch_bounds__(256)
 finalize_kernel(const float *__restrict__ out_acc, bm_bf16 *__restrict__ out, size_t n8) {
+    grid_dep_wait();
+    grid_dep_launch();
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n8; i += (size_t)gridDim.x * blockDim.x) {
         const float4 a = reinterpret_cast<const float4 *>(out_acc)[2 * i];
         const float4 b = reinterpret_cast<const float4 *>(out_acc)[2 * i + 1];
@@ -465,20 +506,44 @@ void choose_decode_tiling(int wrows, int kblocks, int n_seg, bool allow_split, i
     double best = -1.0;
     int bestR = 128, bestKs = 1;
     const int max_ks = allow_split ? 16 : 1;
+    int rmax = tune_int("BM_DC_RMAX", 128);
+    rmax = rmax < 32 ? 32 : (rmax > 128 ? 128 : rmax);
     for (int ks = 1; ks <= max_ks; ++ks) {
         if (kblocks % ks != 0 || kblocks / ks < 4) { if (ks > 1) continue; }
-        for (int R = 128; R >= 32; --R) {
+        for (int R = rmax; R >= 32; --R) {
             const int tiles = (wrows + R - 1) / R;
             const long long items = (long long)tiles * n_seg * ks;
             const long long waves = (items + sms - 1) / sms;
             // useful rows / rows paid for, times wave occupancy; mild penalty for tiny tiles
             double eff = (double)wrows / ((double)tiles * R) * (double)items / (double)(waves * sms);
-            eff -= 0.0005 * (128 - R) / 96.0 + 0.002 * (ks - 1);
+            eff -= 0.0005 * (rmax - R) / 96.0 + 0.002 * (ks - 1);
             if (eff > best + 1e-9) { best = eff; bestR = R; bestKs = ks; }
         }
     }
     *R_out = bestR;
     *ks_out = bestKs;
+}
+
+// Ring geometry.  Prefill: 4 stages x (16 KB tokens + 32 KB weights).  Decode: a stage holds the weight
+// tile(s) (16 KB each, R <= 128 rows used) and the token rows padded to 32 (npad_max x 128 B); as many
+// stages as fit in 227 KB, because the bytes in flight per SM are what the HBM stream lives on.
+void ring_geometry(bool decode, bool gemm1, int T, GemmParams *p) {
+    if (!decode) {
+        p->stage_bytes = 3 * kTileBytes16K;
+        p->off_b = kTileBytes16K;
+    } else {
+        const int rows = T < kChunkRows ? T : kChunkRows;
+        const int npad_max = (rows + 31) & ~31;
+        p->off_b = (gemm1 ? 2 : 1) * kTileBytes16K;
+        p->stage_bytes = p->off_b + npad_max * 128;
+        p->npad_box = npad_max;
+    }
+    int st = (int)(kSmemRing / (size_t)p->stage_bytes);
+    const int cap = tune_int(decode ? "BM_DC_STAGES" : "BM_PF_STAGES", kMaxStages);
+    if (st > cap) st = cap;
+    if (st > kMaxStages) st = kMaxStages;
+    if (st < 2) st = 2;
+    p->stages = st;
 }
 
 template <int MODE>
@@ -487,15 +552,14 @@ cudaError_t launch_gemm(const CUtensorMap &a0, const CUtensorMap &a1, const CUte
     auto kern = gemm_kernel<MODE>;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
     constexpr int kid = (MODE == PF_GEMM1 || MODE == DC_GEMM1) ? BM_KERNEL_GEMM1 : BM_KERNEL_GEMM2;
+    const size_t smem = 1024 + (size_t)p.stages * p.stage_bytes + kSmemBars;
     profile_begin(kid, stream);
-    kern<<<num_sms(), kThreads, kSmemBytes, stream>>>(a0, a1, w0, w1, p);
-    count_launch();
-    cudaError_t e = cudaGetLastError();
+    cudaError_t e = launch_kernel(kern, dim3(num_sms()), dim3(kThreads), smem, stream, a0, a1, w0, w1, p);
     profile_end(kid, stream);
     return e;
 }
@@ -510,10 +574,8 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
     {
         const int grid = sms * 4;
         profile_begin(BM_KERNEL_PREP, stream);
-        prep_kernel<<<grid, 256, 0, stream>>>(a.x, a.T, a.D, a.K, a.G, a.S, a.r.counts, a.r.offsets, a.r.row_token,
-                                              a.sched, a.xs, a.out_acc, a.status);
-        count_launch();
-        cudaError_t e = cudaGetLastError();
+        cudaError_t e = launch_kernel(prep_kernel, dim3(grid), dim3(256), 0, stream, a.x, a.T, a.D, a.K, a.G, a.S,
+                                      a.r.counts, a.r.offsets, a.r.row_token, a.sched, a.xs, a.out_acc, a.status);
         if (e != cudaSuccess) return e;
         profile_end(BM_KERNEL_PREP, stream);
     }
@@ -522,6 +584,7 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
     p.T = a.T; p.D = a.D; p.F = a.F; p.K = a.K; p.G = a.G; p.S = a.S; p.TK = TK;
     p.counts = a.r.counts; p.offsets = a.r.offsets; p.row_token = a.r.row_token; p.row_slot = a.r.row_slot;
     p.gate_w = a.r.gate_w; p.sched = a.sched; p.h = a.h; p.out_acc = a.out_acc;
+
 
     const uint64_t h_rows = (uint64_t)TK + (uint64_t)a.S * a.T;
     const int kb1 = (a.D + kBlockK - 1) / kBlockK, kb2 = (a.F + kBlockK - 1) / kBlockK;
@@ -534,6 +597,7 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
             !make_map_3d(&m_w2, a.W2, a.G + a.S, a.D, a.F, 256) || !make_map_2d(&m_h, a.h, h_rows, a.F, 128))
             return cudaErrorInvalidValue;
         p.ksplit = 1;
+        ring_geometry(false, true, a.T, &p);
         p.kblocks = kb1; p.R = 128; p.n_wtiles = (a.F + 127) / 128;
         if ((err = launch_gemm<PF_GEMM1>(m_xs, m_x, m_w1, m_w3, p, stream)) != cudaSuccess) return err;
         p.kblocks = kb2; p.R = 256; p.n_wtiles = (a.D + 255) / 256;
@@ -546,12 +610,18 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
         int R1, R2, ks1, ks2;
         choose_decode_tiling(a.F, kb1, n_seg, false, sms, &R1, &ks1);
         choose_decode_tiling(a.D, kb2, n_seg, true, sms, &R2, &ks2);
-        if (!make_map_2d(&m_xs, a.xs, TK > 0 ? TK : 1, a.D, 32) || !make_map_2d(&m_x, a.x, a.T, a.D, 32) ||
+        if (tune_int("BM_DC_R2", 0) > 0) { R2 = tune_int("BM_DC_R2", 0); ks2 = tune_int("BM_DC_KS2", 1); }
+        if (tune_int("BM_DC_R1", 0) > 0) R1 = tune_int("BM_DC_R1", 0);
+        const int rows_max = a.T < kChunkRows ? a.T : kChunkRows;
+        const int nbox = (rows_max + 31) & ~31;      // token rows every stage loads (ring_geometry: npad_box)
+        if (!make_map_2d(&m_xs, a.xs, TK > 0 ? TK : 1, a.D, nbox) || !make_map_2d(&m_x, a.x, a.T, a.D, nbox) ||
             !make_map_3d(&m_w1, a.W1, a.G + a.S, a.F, a.D, R1) || !make_map_3d(&m_w3, a.W3, a.G + a.S, a.F, a.D, R1) ||
-            !make_map_3d(&m_w2, a.W2, a.G + a.S, a.D, a.F, R2) || !make_map_2d(&m_h, a.h, h_rows, a.F, 32))
+            !make_map_3d(&m_w2, a.W2, a.G + a.S, a.D, a.F, R2) || !make_map_2d(&m_h, a.h, h_rows, a.F, nbox))
             return cudaErrorInvalidValue;
+        ring_geometry(true, true, a.T, &p);
         p.ksplit = 1; p.kblocks = kb1; p.R = R1; p.n_wtiles = (a.F + R1 - 1) / R1;
         if ((err = launch_gemm<DC_GEMM1>(m_xs, m_x, m_w1, m_w3, p, stream)) != cudaSuccess) return err;
+        ring_geometry(true, false, a.T, &p);
         p.ksplit = ks2; p.kblocks = kb2 / ks2; p.R = R2; p.n_wtiles = (a.D + R2 - 1) / R2;
         if ((err = launch_gemm<DC_GEMM2>(m_h, m_h, m_w2, m_w2, p, stream)) != cudaSuccess) return err;
     }
@@ -562,9 +632,7 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
         if (grid > sms * 8) grid = sms * 8;
         if (grid < 1) grid = 1;
         profile_begin(BM_KERNEL_FINALIZE, stream);
-        finalize_kernel<<<grid, 256, 0, stream>>>(a.out_acc, a.out, n8);
-        count_launch();
-        cudaError_t e = cudaGetLastError();
+        cudaError_t e = launch_kernel(finalize_kernel, dim3(grid), dim3(256), 0, stream, (const float *)a.out_acc, a.out, n8);
         profile_end(BM_KERNEL_FINALIZE, stream);
         return e;
     }

@@ -94,6 +94,8 @@ permute_small_kernel(const int32_t *__restrict__ group_ids, int T, int K, int G,
                      int32_t *__restrict__ row_token, int32_t *__restrict__ row_slot,
                      int32_t *__restrict__ slot_row, int32_t *__restrict__ status) {
     extern __shared__ int s_mem[];
+    grid_dep_wait();
+    grid_dep_launch();
     int *whist = s_mem;                  // [kWarps][G]
     int *gsum = whist + kWarps * G;      // [G] -> offsets
     int *tmp = gsum + G;                 // [512]
@@ -131,6 +133,8 @@ __global__ void __launch_bounds__(kWarps * 32)
 permute_hist_kernel(const int32_t *__restrict__ group_ids, int T, int K, int G,
                     int32_t *__restrict__ block_hist) {
     extern __shared__ int s_mem[];
+    grid_dep_wait();
+    grid_dep_launch();
     int *whist = s_mem;                  // [kWarps][G]
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long items = (long long)T * K;
@@ -152,6 +156,8 @@ permute_scan_kernel(int nb, int G, int32_t *__restrict__ block_hist, int32_t *__
     __shared__ int gsum[512];
     __shared__ int tmp[512];
     __shared__ int s_total;
+    grid_dep_wait();
+    grid_dep_launch();
     for (int u = threadIdx.x; u < G; u += blockDim.x) {
         int run = 0;
         for (int b = 0; b < nb; ++b) {          // block_hist[b][u] := rows of group u in blocks before b
@@ -177,6 +183,8 @@ permute_scatter_kernel(const int32_t *__restrict__ group_ids, int T, int K, int 
                        int32_t *__restrict__ row_token, int32_t *__restrict__ row_slot,
                        int32_t *__restrict__ slot_row) {
     extern __shared__ int s_mem[];
+    grid_dep_wait();
+    grid_dep_launch();
     int *whist = s_mem;                  // [kWarps][G]
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long items = (long long)T * K;
@@ -207,17 +215,17 @@ cudaError_t launch_permute(int T, int K, int G, const bm_routing &r, int32_t *bl
     const size_t smem_w = (size_t)kWarps * G * sizeof(int);
     if (nb <= 1) {
         const size_t smem = smem_w + (size_t)(G + 512) * sizeof(int);
-        permute_small_kernel<<<1, kWarps * 32, smem, stream>>>(r.group_ids, T, K, G, r.counts, r.offsets,
-                                                              r.row_token, r.row_slot, r.slot_row, status);
-        count_launch();
-        return cudaGetLastError();
+        return launch_kernel(permute_small_kernel, dim3(1), dim3(kWarps * 32), smem, stream, (const int32_t *)r.group_ids,
+                             T, K, G, r.counts, r.offsets, r.row_token, r.row_slot, r.slot_row, status);
     }
-    permute_hist_kernel<<<nb, kWarps * 32, smem_w, stream>>>(r.group_ids, T, K, G, block_hist);
-    permute_scan_kernel<<<1, 256, 0, stream>>>(nb, G, block_hist, r.counts, r.offsets, status);
-    permute_scatter_kernel<<<nb, kWarps * 32, smem_w, stream>>>(r.group_ids, T, K, G, block_hist, r.offsets,
-                                                                r.row_token, r.row_slot, r.slot_row);
-    count_launch(3);
-    return cudaGetLastError();
+    cudaError_t e = launch_kernel(permute_hist_kernel, dim3(nb), dim3(kWarps * 32), smem_w, stream,
+                                  (const int32_t *)r.group_ids, T, K, G, block_hist);
+    if (e != cudaSuccess) return e;
+    e = launch_kernel(permute_scan_kernel, dim3(1), dim3(256), 0, stream, nb, G, block_hist, r.counts, r.offsets, status);
+    if (e != cudaSuccess) return e;
+    return launch_kernel(permute_scatter_kernel, dim3(nb), dim3(kWarps * 32), smem_w, stream,
+                         (const int32_t *)r.group_ids, T, K, G, (const int32_t *)block_hist, (const int32_t *)r.offsets,
+                         r.row_token, r.row_slot, r.slot_row);
 }
 
 }  // namespace bm

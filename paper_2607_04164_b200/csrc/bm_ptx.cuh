@@ -122,6 +122,16 @@ __device__ __forceinline__ uint64_t make_smem_desc_sw128(uint32_t smem_addr) {
     return d;
 }
 
+// The same descriptor split for a hot loop: the low word carries the address (advance it by bytes >> 4),
+// the high word is constant.
+__device__ __forceinline__ uint32_t smem_desc_lo(uint32_t smem_addr) {
+    return ((smem_addr & 0x3FFFFu) >> 4) | (1u << 16);
+}
+__device__ __forceinline__ uint64_t smem_desc(uint32_t lo) {
+    constexpr uint32_t hi = (1024u >> 4) | (1u << 14) | (2u << 29);
+    return ((uint64_t)hi << 32) | lo;
+}
+
 // Instruction descriptor, kind::f16: bf16 x bf16 -> fp32, both operands K-major.
 //   [4,6) D format: 1 = f32   [7,10) A format: 1 = bf16   [10,13) B format: 1 = bf16
 //   [15] A major: 0 = K   [16] B major: 0 = K   [17,23) N >> 3   [24,29) M >> 4

@@ -29,6 +29,8 @@ router_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *__rest
               int WT, int WE, int32_t *__restrict__ expert_ids, int32_t *__restrict__ group_ids,
               float *__restrict__ gate_w, int32_t *__restrict__ n_slots, int32_t *__restrict__ status) {
     extern __shared__ float s_logits[];   // [TB][E], TB = WT * TOK
+    grid_dep_wait();      // x may come from a predecessor; the routing arrays may still be read by one
+    grid_dep_launch();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int TB = WT * TOK;
     const int t_block = blockIdx.x * TB;
@@ -190,10 +192,8 @@ cudaError_t launch_cfg(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const 
         if (e != cudaSuccess) return e;
     }
     const int grid = (T + TB - 1) / TB;
-    kern<<<grid, kWarps * 32, smem, stream>>>(x, T, D, Wr, bias, E, K, gmap, G, WT, WE, r.expert_ids,
-                                              r.group_ids, r.gate_w, r.n_slots, status);
-    count_launch();
-    return cudaGetLastError();
+    return launch_kernel(kern, dim3(grid), dim3(kWarps * 32), smem, stream, x, T, D, Wr, bias, E, K, gmap, G, WT, WE,
+                         r.expert_ids, r.group_ids, r.gate_w, r.n_slots, status);
 }
 
 }  // namespace
