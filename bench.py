@@ -29,7 +29,7 @@ if ROOT not in sys.path:
 import numpy as np
 import torch
 
-from bm_inputs import CONFIGS, bf16_bits, identity_variant, make_layer
+from bm_inputs import CONFIGS, bf16_bits, get_config, identity_variant, make_layer
 
 METRIC = "moe_layer_tokens_per_s"
 UNIT = "tokens/s"
@@ -325,7 +325,7 @@ def run_ours(args):
     import paper_2607_04164_b200 as bm
     bm.lib()
     peaks = load_peaks()
-    cfg = CONFIGS[args.config]
+    cfg = get_config(args.config)
     steps, warmup = args.steps, max(args.warmup, 3)
 
     layer = DeviceLayer(cfg, seed=0, x_seed=rank, keep_host_weights=(rank == 0 and ws == 1 and not args.no_cpu))
@@ -399,6 +399,138 @@ def run_ours(args):
 
 
 # ---------------------------------------------------------------------------------------------------
+# BJ:configs[4]: the brownout sweep (tokens/s and % roofline per point)
+# ---------------------------------------------------------------------------------------------------
+class SweepWeights:
+    """United weights of one G, kept as L distinct copies so that L * weight_bytes >= 512 MB: successive
+    steps read different addresses and no weight byte is served from the 126 MB L2 (SURVEY.md 8(d),
+    "cold weights"; a real model has 24 such layers)."""
+
+    def __init__(self, cfg, seed=0, min_bytes=512e6):
+        L = make_layer(cfg, seed)
+        one = 3 * cfg.G * cfg.F * cfg.D * 2
+        self.copies = max(1, int(-(-min_bytes // one)))
+        self.W1 = [L.W1.cuda()]
+        self.W3 = [L.W3.cuda()]
+        self.W2 = [L.W2.cuda()]
+        for _ in range(self.copies - 1):
+            self.W1.append(self.W1[0].clone()); self.W3.append(self.W3[0].clone()); self.W2.append(self.W2[0].clone())
+        self.W_router = L.W_router.cuda()
+        self.gmap = L.group_map.cuda()
+
+
+class SweepPoint:
+    def __init__(self, cfg, W):
+        import paper_2607_04164_b200 as bm
+        self.bm, self.cfg, self.W = bm, cfg, W
+        L = make_layer(cfg, 0, weights=False)
+        self.x = L.x.cuda()
+        self.bias = None if L.router_bias is None else L.router_bias.cuda()
+        self.ws = bm.alloc_workspace(cfg.T, cfg.D, cfg.F, cfg.E, cfg.K, cfg.G, cfg.S)
+        self.routing = bm.Routing(cfg.T, cfg.K, cfg.G)
+        self.out = torch.empty((cfg.T, cfg.D), dtype=torch.bfloat16, device="cuda")
+        self.i = 0
+
+    def step(self, stream=None):
+        bm, c, W = self.bm, self.cfg, self.W
+        j = self.i % W.copies
+        self.i += 1
+        bm.bm_route(self.x, W.W_router, self.bias, c.K, W.gmap, c.G, self.routing, self.ws, stream=stream)
+        bm.bm_moe_forward(self.x, self.routing, W.W1[j], W.W3[j], W.W2[j], self.out, self.ws, S=c.S, stream=stream)
+
+
+def time_point(pt, steps, warmup):
+    for _ in range(warmup):
+        pt.step()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        pt.step()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / 1e3 / steps
+
+
+def time_point_graph(pt, steps):
+    """The same steps captured once in a CUDA graph (one graph = one pass over all weight copies) and
+    replayed: removes the host launch cost that dominates the smallest points."""
+    n = pt.W.copies
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        pt.i = 0
+        for _ in range(n):
+            pt.step()
+        side.synchronize()
+        with torch.cuda.graph(g, stream=side):
+            for _ in range(n):
+                pt.step()
+    torch.cuda.synchronize()
+    reps = max(1, steps // n)
+    for _ in range(2):
+        g.replay()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        g.replay()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / 1e3 / (reps * n)
+
+
+def run_sweep(args):
+    """python bench.py --config sweep [--sweep-filter G8] [--out FILE]: the 60 points of BJ:configs[4].
+    One GPU."""
+    from bm_inputs import sweep_points
+    torch.cuda.set_device(0)
+    import paper_2607_04164_b200 as bm
+    bm.lib()
+    peaks = load_peaks()
+    pts = [c for c in sweep_points() if not args.sweep_filter or all(f in c.name.split("_") for f in args.sweep_filter.split(","))]
+    rows, cache = [], {}
+    sampler = ClockSampler(0)
+    with sampler:
+        for cfg in pts:
+            if cfg.G not in cache:
+                cache.clear()
+                torch.cuda.empty_cache()
+                cache[cfg.G] = SweepWeights(cfg)
+            W = cache[cfg.G]
+            pt = SweepPoint(cfg, W)
+            steps = 200 if cfg.T <= 256 else (40 if cfg.T <= 4096 else 12)
+            steps = max(steps // W.copies * W.copies, W.copies)
+            t = time_point(pt, steps, max(3, W.copies))
+            tg = time_point_graph(pt, steps) if cfg.T <= 256 else None
+            status = bm.bm_device_status(pt.ws)
+            counts = pt.routing.counts.cpu().numpy()
+            A, G_act = int(counts.sum()), int((counts > 0).sum())
+            flops, nbytes, t_flop, t_hbm = roofline_times(cfg, A, G_act, peaks)
+            t_best = min(t, tg) if tg else t
+            rows.append(dict(name=cfg.name, G=cfg.G, T=cfg.T, zipf_s=cfg.zipf_s, A=A, G_act=G_act, copies=W.copies,
+                             us_stream=t * 1e6, us_graph=None if tg is None else tg * 1e6,
+                             tokens_per_s=cfg.T / t_best, t_hbm_us=t_hbm * 1e6, t_flop_us=t_flop * 1e6,
+                             bound="hbm" if t_hbm >= t_flop else "tensor", roofline_frac=max(t_hbm, t_flop) / t_best,
+                             achieved_gbs=nbytes / t_best / 1e9, achieved_tflops=flops / t_best / 1e12,
+                             path="decode" if cfg.T <= bm.BM_DECODE_MAX_T else "prefill", device_status=status))
+            sys.stderr.write(f"{cfg.name:24s} A={A:6d} G_act={G_act:3d} stream {t*1e6:9.1f} us"
+                             + (f" graph {tg*1e6:9.1f} us" if tg else " " * 19)
+                             + f"  roof {max(t_hbm, t_flop)*1e6:8.1f} us  frac {rows[-1]['roofline_frac']:.3f}\n")
+            del pt
+    res = dict(metric=METRIC, unit=UNIT, workload="BASELINE.json configs[4] brownout sweep: D=2048 F=1408 E=60 top-4",
+               peaks=peaks, clocks=sampler.summary(), points=rows,
+               timing="CUDA events around `steps` back-to-back layer calls cycling over `copies` weight copies "
+                      "(copies * weight bytes >= 512 MB, so weights are never L2-resident); T <= 256 also replayed "
+                      "from a CUDA graph; tokens_per_s uses the faster of the two")
+    if args.out:
+        with open(args.out, "w") as fh:
+            json.dump(res, fh, indent=1)
+    print(json.dumps(res))
+
+
+# ---------------------------------------------------------------------------------------------------
 # reference arm: the oracle on the host cores (tier framing (4))
 # ---------------------------------------------------------------------------------------------------
 def run_reference(args):
@@ -407,7 +539,7 @@ def run_reference(args):
         return
     import oracle
     oracle.build()
-    cfg = CONFIGS[args.config]
+    cfg = get_config(args.config)
     steps, warmup = args.steps, args.warmup
     L = make_layer(cfg, 0)
     xb, wr = bf16_bits(L.x), bf16_bits(L.W_router)
@@ -452,7 +584,11 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="decode", choices=sorted(CONFIGS))
+    ap.add_argument("--config", default="decode",
+                    help="one of %s, 'sweep' (all 60 points of configs[4]) or one sweep point name such as "
+                         "sweep_G8_T256_s1" % sorted(CONFIGS))
+    ap.add_argument("--sweep-filter", default="", help="comma-separated name parts, e.g. G8,T16 (with --config sweep)")
+    ap.add_argument("--out", default="", help="also write the sweep result to this file")
     ap.add_argument("--no-extras", action="store_true", help="skip the ungrouped / prefill side measurements")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()
@@ -461,7 +597,10 @@ def main():
     else:
         if not torch.cuda.is_available():
             raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
-        run_ours(args)
+        if args.config == "sweep":
+            run_sweep(args)
+        else:
+            run_ours(args)
 
 
 if __name__ == "__main__":

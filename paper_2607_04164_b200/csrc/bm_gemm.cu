@@ -37,7 +37,9 @@ constexpr int kChunkRows = 128;
 constexpr int kMaxSeg = BM_MAX_G + kMaxShared;
 constexpr size_t kSmemMax = 232448;         // 227 KB, the per-CTA opt-in limit of sm_100
 constexpr size_t kSmemBars = 256;           // (2*kMaxStages + 2*kAccStages) mbarriers + the TMEM base address
-constexpr size_t kSmemRing = kSmemMax - 1024 /*align slack*/ - kSmemBars;
+constexpr size_t kEpiStageBytes = 32 * 32 * 4;   // PF_GEMM2: per-epilogue-warp transpose buffer (32 rows x 32 fp32)
+constexpr size_t kSmemEpi = 4 * kEpiStageBytes;
+constexpr size_t kSmemRing = kSmemMax - 1024 /*align slack*/ - kSmemBars;   // minus kSmemEpi for PF_GEMM2
 static_assert((2 * kMaxStages + 2 * kAccStages) * 8 + 4 <= kSmemBars, "barrier block too small");
 
 enum Mode { PF_GEMM1 = 0, PF_GEMM2 = 1, DC_GEMM1 = 2, DC_GEMM2 = 3 };
@@ -140,6 +142,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
     uint64_t *tfull = bars + 2 * kMaxStages;     // [kAccStages]
     uint64_t *tempty = tfull + kAccStages;       // [kAccStages]
     uint32_t *tmem_ptr = reinterpret_cast<uint32_t *>(tempty + kAccStages);
+    uint8_t *epi_stage = reinterpret_cast<uint8_t *>(bars) + kSmemBars;   // [4][kEpiStageBytes], 256-byte aligned
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -305,11 +308,14 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
                     }
                 }
             } else if (MODE == PF_GEMM2) {
-                // row = token row; columns = 256 output features d0..d0+255; scatter-combine with the gate weight
-                const bool row_ok = row < it.n;
-                int tok = 0;
+                // row = token row; columns = 256 output features d0..d0+255; scatter-combine with the gate weight.
+                // The accumulator leaves TMEM with one row per lane; a per-warp shared-memory transpose (32 rows
+                // x 32 columns fp32, 16-byte units xor-swizzled by the row) turns that into row-contiguous
+                // pieces, so every red.global.add.v4.f32 of a warp covers 4 rows x 128 contiguous bytes
+                // (whole L2 lines) instead of 32 scattered 16-byte pieces.
+                int tok = -1;
                 float gw = 1.0f;
-                if (row_ok) {
+                if (row < it.n) {
                     if (it.shared) {
                         tok = it.tok0 + row;
                     } else {
@@ -318,19 +324,29 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
                     }
                 }
                 const int d0 = it.wt * 256;
-                float *orow = p.out_acc + (size_t)tok * p.D + d0;
+                float4 *stg = reinterpret_cast<float4 *>(epi_stage + (size_t)q * kEpiStageBytes);
+                const int rl = lane >> 3, ul = lane & 7;        // read phase: row (mod 4) and 16-byte unit of this lane
 #pragma unroll 1
-                for (int c = 0; c < 256; c += 16) {
-                    uint32_t v[16];
-                    ptx::tmem_ld_x16(t_addr + c, v);
+                for (int c = 0; c < 256; c += 32) {
+                    uint32_t v[32];
+                    ptx::tmem_ld_x32(t_addr + c, v);
                     ptx::tmem_ld_wait();
-                    if (row_ok) {
 #pragma unroll
-                        for (int i = 0; i < 16; i += 4)
-                            if (d0 + c + i + 4 <= p.D)
-                                ptx::red_add_v4_f32(orow + c + i, gw * __uint_as_float(v[i]), gw * __uint_as_float(v[i + 1]),
-                                                    gw * __uint_as_float(v[i + 2]), gw * __uint_as_float(v[i + 3]));
+                    for (int u = 0; u < 8; ++u)
+                        stg[lane * 8 + (u ^ (lane & 7))] =
+                            make_float4(gw * __uint_as_float(v[4 * u]), gw * __uint_as_float(v[4 * u + 1]),
+                                        gw * __uint_as_float(v[4 * u + 2]), gw * __uint_as_float(v[4 * u + 3]));
+                    __syncwarp();
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        const int r = 4 * j + rl;
+                        const float4 o = stg[r * 8 + (ul ^ (r & 7))];
+                        const int tk = __shfl_sync(0xffffffffu, tok, r);
+                        const int d = d0 + c + 4 * ul;
+                        if (tk >= 0 && d + 4 <= p.D)
+                            ptx::red_add_v4_f32(p.out_acc + (size_t)tk * p.D + d, o.x, o.y, o.z, o.w);
                     }
+                    __syncwarp();
                 }
             } else if (MODE == DC_GEMM1) {
                 // row = weight row f (R rows per tile); columns [0,npad) = W1 products per token,
@@ -354,27 +370,46 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
                     }
                 }
             } else {
-                // DC_GEMM2: row = output feature d; columns = token rows of the chunk; partial over this K split
+                // DC_GEMM2: row = output feature d; columns = token rows of the chunk; partial over this K split.
+                // Lane l first fetches token and gate weight of chunk rows l, l+32, ... (one dependent-load chain
+                // per item instead of one per token); the loop broadcasts them with shuffles.
                 const int d = it.wt * p.R + row;
                 const bool d_ok = row < p.R && d < p.D;
-                const int npad = (it.n + 31) & ~31;
-#pragma unroll 1
-                for (int c = 0; c < npad; c += 16) {
-                    uint32_t v[16];
-                    ptx::tmem_ld_x16(t_addr + c, v);
-                    ptx::tmem_ld_wait();
+                int tokr[4];
+                float gwr[4];
 #pragma unroll
-                    for (int i = 0; i < 16; ++i) {
-                        if (c + i < it.n) {              // warp-uniform
-                            int tok;
-                            float gw = 1.0f;
-                            if (it.shared) {
-                                tok = it.tok0 + c + i;
-                            } else {
-                                tok = p.row_token[it.perm_row0 + c + i];
-                                gw = p.gate_w[(size_t)tok * p.K + p.row_slot[it.perm_row0 + c + i]];
+                for (int j = 0; j < 4; ++j) {
+                    const int r = j * 32 + lane;
+                    tokr[j] = -1;
+                    gwr[j] = 1.0f;
+                    if (r < it.n) {
+                        if (it.shared) {
+                            tokr[j] = it.tok0 + r;
+                        } else {
+                            tokr[j] = p.row_token[it.perm_row0 + r];
+                            gwr[j] = p.gate_w[(size_t)tokr[j] * p.K + p.row_slot[it.perm_row0 + r]];
+                        }
+                    }
+                }
+                float *ocol = p.out_acc + d;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    if (j * 32 < it.n) {                 // warp-uniform
+#pragma unroll
+                        for (int hh = 0; hh < 2; ++hh) {
+                            const int c = j * 32 + hh * 16;
+                            if (c < it.n) {              // warp-uniform
+                                uint32_t v[16];
+                                ptx::tmem_ld_x16(t_addr + c, v);
+                                ptx::tmem_ld_wait();
+#pragma unroll
+                                for (int i = 0; i < 16; ++i) {
+                                    const int tok = __shfl_sync(0xffffffffu, tokr[j], hh * 16 + i);
+                                    const float gw = __shfl_sync(0xffffffffu, gwr[j], hh * 16 + i);
+                                    if (tok >= 0 && d_ok)
+                                        ptx::red_add_f32(ocol + (size_t)tok * p.D, gw * __uint_as_float(v[i]));
+                                }
                             }
-                            if (d_ok) ptx::red_add_f32(p.out_acc + (size_t)tok * p.D + d, gw * __uint_as_float(v[i]));
                         }
                     }
                 }
@@ -538,7 +573,7 @@ void ring_geometry(bool decode, bool gemm1, int T, GemmParams *p) {
         p->stage_bytes = p->off_b + npad_max * 128;
         p->npad_box = npad_max;
     }
-    int st = (int)(kSmemRing / (size_t)p->stage_bytes);
+    int st = (int)((kSmemRing - (decode ? 0 : kSmemEpi)) / (size_t)p->stage_bytes);
     const int cap = tune_int(decode ? "BM_DC_STAGES" : "BM_PF_STAGES", kMaxStages);
     if (st > cap) st = cap;
     if (st > kMaxStages) st = kMaxStages;
@@ -557,7 +592,7 @@ cudaError_t launch_gemm(const CUtensorMap &a0, const CUtensorMap &a1, const CUte
         attr_set = true;
     }
     constexpr int kid = (MODE == PF_GEMM1 || MODE == DC_GEMM1) ? BM_KERNEL_GEMM1 : BM_KERNEL_GEMM2;
-    const size_t smem = 1024 + (size_t)p.stages * p.stage_bytes + kSmemBars;
+    const size_t smem = 1024 + (size_t)p.stages * p.stage_bytes + kSmemBars + (MODE == PF_GEMM2 ? kSmemEpi : 0);
     profile_begin(kid, stream);
     cudaError_t e = launch_kernel(kern, dim3(num_sms()), dim3(kThreads), smem, stream, a0, a1, w0, w1, p);
     profile_end(kid, stream);

@@ -15,12 +15,83 @@
 // Small T (decode): TOK = 1, warps split the experts, one CTA per token -> latency-bound, ~2 us.
 // Large T (prefill): TOK = 4, ET = 8, warps split the tokens -> each W_router chunk feeds 32 FMAs.
 #include "bm_common.cuh"
+#include "bm_ptx.cuh"
 
 namespace bm {
 
 namespace {
 
 constexpr int kWarps = 8;
+
+// R2-R5 for one token, executed by one full warp: `l` = its E logits in shared memory.
+// Rank i of the selection lives in lane i (K <= BM_MAX_K = 16 <= 32), so softmax, remap and dedup are
+// lane-parallel; only the two rank-ordered fp32 sums (softmax denominator, merged gate weights) are
+// sequential, as a chain of K shuffles.
+__device__ __forceinline__ void select_and_write(const float *l, int t, int lane, int E, int K,
+                                                 const int32_t *__restrict__ gmap, int G,
+                                                 int32_t *__restrict__ expert_ids, int32_t *__restrict__ group_ids,
+                                                 float *__restrict__ gate_w, int32_t *__restrict__ n_slots,
+                                                 int32_t *__restrict__ status) {
+    // ---- R2: K rounds of warp arg-max; ties -> lower index --------------------------------------
+    unsigned taken = 0;                 // bit c: candidate e = lane + 32*c already selected (E <= 512)
+    int my_e = 0;                       // lane i < K: expert of rank i
+    float my_l = 0.0f;                  //             and its logit
+    bool nonfinite = false;
+    for (int i = 0; i < K; ++i) {
+        // lane-local best: ascending e with a strict '>' keeps the lower index on ties
+        float bv = -INFINITY;
+        int bi = 0x7fffffff;
+        for (int c = 0, e = lane; e < E; ++c, e += 32) {
+            if (taken & (1u << c)) continue;
+            float v = l[e];
+            if (!(fabsf(v) <= 3.402823466e38f)) nonfinite = true;
+            if (v != v) v = -INFINITY;            // NaN: unspecified result, keep indices valid
+            if (bi == 0x7fffffff || v > bv) { bv = v; bi = e; }
+        }
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) {
+            const float ov = __shfl_xor_sync(kFullMask, bv, o);
+            const int oi = __shfl_xor_sync(kFullMask, bi, o);
+            if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+        }
+        if ((bi & 31) == lane) taken |= 1u << (bi >> 5);
+        if (lane == i) { my_e = bi; my_l = l[bi]; }
+    }
+    const bool active = lane < K;
+    // ---- R3: softmax over the selected logits, denominator summed in rank order -------------------
+    const float m = __shfl_sync(kFullMask, my_l, 0);
+    const float w = active ? expf(__fsub_rn(my_l, m)) : 0.0f;
+    float sum = 0.0f;
+    for (int i = 0; i < K; ++i) sum = __fadd_rn(sum, __shfl_sync(kFullMask, w, i));
+    const float wi = active ? __fdiv_rn(w, sum) : 0.0f;
+    // ---- R4: remap ---------------------------------------------------------------------------------
+    int u = -1 - lane;                  // inactive lanes: distinct negative keys, never matched
+    bool bad_map = false;
+    if (active) {
+        u = gmap[my_e];
+        if (u < 0 || u >= G) { bad_map = true; u = u < 0 ? 0 : G - 1; }
+    }
+    // ---- R5: dedup in rank order; the first occurrence keeps the slot, weights added in rank order -----
+    const unsigned peers = __match_any_sync(kFullMask, u);            // lanes (ranks) mapped to the same group
+    const bool first = active && (__ffs(peers) - 1 == lane);
+    const unsigned firsts = __ballot_sync(kFullMask, first);
+    const int n = __popc(firsts);
+    const int slot = __popc(firsts & ((1u << lane) - 1u));
+    float gw = wi;
+    for (int j = 1; j < K; ++j) {
+        const float wj = __shfl_sync(kFullMask, wi, j);
+        if (first && j > lane && ((peers >> j) & 1u)) gw = __fadd_rn(gw, wj);
+    }
+    const size_t base = (size_t)t * K;
+    if (active) {
+        expert_ids[base + lane] = my_e;
+        if (lane >= n) { group_ids[base + lane] = -1; gate_w[base + lane] = 0.0f; }
+    }
+    if (first) { group_ids[base + slot] = u; gate_w[base + slot] = gw; }
+    if (lane == 0) n_slots[t] = n;
+    if (__any_sync(kFullMask, bad_map) && lane == 0) atomicOr(status, BM_DEV_BAD_GROUP_MAP);
+    if (__any_sync(kFullMask, nonfinite) && lane == 0) atomicOr(status, BM_DEV_NONFINITE_LOGIT);
+}
 
 template <int TOK, int ET>
 __global__ void __launch_bounds__(kWarps * 32)
@@ -99,85 +170,197 @@ router_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *__rest
     for (int tl = warp; tl < TB; tl += kWarps) {
         const int t = t_block + tl;
         if (t >= T) break;
-        const float *l = s_logits + tl * E;
-        unsigned taken = 0;                 // bit i: candidate e = lane + 32*i already selected (E <= 512)
-        int sel_e[BM_MAX_K];
-        float sel_l[BM_MAX_K];
-        bool nonfinite = false;
+        select_and_write(s_logits + tl * E, t, lane, E, K, gmap, G, expert_ids, group_ids, gate_w, n_slots, status);
+    }
+}
+
+// -------------------------------------------------------------------------------------------------
+// Throughput shape (T >= BM_ROUTER_TP_MIN_T): the same canonical dot products, operands staged through
+// shared memory by a producer warp.  Persistent CTAs walk token blocks of TB = WT*4 tokens; per pass a
+// block meets EB = WE*8 experts; compute warp (tw, ew) keeps the 4 x 8 register tile acc[token][expert]
+// of its slice -- lane l still owns partial l of every dot product and walks its chunks l, l+32, ... in
+// ascending order, so the association tree is unchanged.  D is walked in slabs of 256 elements (one
+// 16-byte chunk per lane and row).  Slab rows are copied with cp.async.bulk (512 bytes each; every warp
+// issues a few) into a 4-stage ring guarded by full/empty mbarriers, three slabs ahead of the multiply
+// and across passes and blocks, so neither the HBM read of x nor the L2 read of W_router is on the
+// critical path, and the warps never meet at a CTA-wide barrier inside a pass.  E > EB takes ceil(E/EB) passes over the same tokens.
+// -------------------------------------------------------------------------------------------------
+constexpr int kTpStages = 4;
+constexpr int kTpTok = 4;
+constexpr int kSlab = 256;                    // elements per slab row = 512 bytes
+constexpr int kTpMaxThreads = 16 * 32;
+
+__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gsrc, uint32_t bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(ptx::smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(ptx::smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void bar_sync_named(int id, int nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+// Sum of the 32 lane partials of each of this lane's 32 accumulators: the xor butterfly (16, 8, 4, 2, 1)
+// of reading A1, evaluated for all 32 accumulators at once.  At the step with offset o every lane hands
+// over the half of its values whose index bit o differs from its own lane bit o, so a step costs n/2
+// shuffles instead of n; each surviving value is p_l + p_{l xor o} exactly as in the per-accumulator
+// butterfly (fp32 addition is commutative, so both partners of a pair would have computed the same
+// bits).  On return lane l holds in v[0] the finished sum of accumulator index l.
+__device__ __forceinline__ void butterfly32(float (&v)[32], int lane) {
 #pragma unroll
-        for (int i = 0; i < BM_MAX_K; ++i) {
-            if (i < K) {
-                // lane-local best: ascending e with a strict '>' keeps the lower index on ties
-                float bv = -INFINITY;
-                int bi = 0x7fffffff;
-                for (int c = 0, e = lane; e < E; ++c, e += 32) {
-                    if (taken & (1u << c)) continue;
-                    float v = l[e];
-                    if (!(fabsf(v) <= 3.402823466e38f)) nonfinite = true;
-                    if (v != v) v = -INFINITY;            // NaN: unspecified result, keep indices valid
-                    if (bi == 0x7fffffff || v > bv) { bv = v; bi = e; }
-                }
+    for (int o = 16; o >= 1; o >>= 1) {
+        const bool up = (lane & o) != 0;
 #pragma unroll
-                for (int o = 16; o >= 1; o >>= 1) {
-                    const float ov = __shfl_xor_sync(kFullMask, bv, o);
-                    const int oi = __shfl_xor_sync(kFullMask, bi, o);
-                    if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
-                }
-                if ((bi & 31) == lane) taken |= 1u << (bi >> 5);
-                sel_e[i] = bi;
-                sel_l[i] = l[bi];
+        for (int a = 0; a < o; ++a) {
+            const float keep = up ? v[a + o] : v[a];
+            const float send = up ? v[a] : v[a + o];
+            v[a] = __fadd_rn(keep, __shfl_xor_sync(kFullMask, send, o));
+        }
+    }
+}
+
+__global__ void __launch_bounds__(kTpMaxThreads, 1)
+router_tp_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *__restrict__ Wr,
+                 const float *__restrict__ bias, int E, int K, const int32_t *__restrict__ gmap, int G,
+                 int WT, int WE, int n_blocks, int32_t *__restrict__ expert_ids, int32_t *__restrict__ group_ids,
+                 float *__restrict__ gate_w, int32_t *__restrict__ n_slots, int32_t *__restrict__ status) {
+    extern __shared__ __align__(128) uint8_t tp_smem[];
+    const int TB = WT * kTpTok, EB = WE * 8;
+    const int rows = TB + EB;
+    const uint32_t stage_bytes = (uint32_t)rows * (kSlab * 2);
+    uint64_t *full = reinterpret_cast<uint64_t *>(tp_smem + kTpStages * stage_bytes);
+    uint64_t *empty = full + kTpStages;
+    float *s_logits = reinterpret_cast<float *>(empty + kTpStages);   // [TB][E]
+    const int tid = threadIdx.x;
+    const int warp = tid >> 5, lane = tid & 31;
+    const int nw = blockDim.x >> 5;
+    const int n_slabs = (D + kSlab - 1) / kSlab;
+    const int n_pass = (E + EB - 1) / EB;
+    const int tw = warp % WT, ew = warp / WT;
+
+    if (tid == 0) {
+        for (int i = 0; i < kTpStages; ++i) { ptx::mbar_init(&full[i], 1); ptx::mbar_init(&empty[i], nw); }
+        ptx::fence_barrier_init();
+    }
+    __syncthreads();
+    grid_dep_wait();      // x may come from a predecessor; the routing arrays may still be read by one
+    grid_dep_launch();
+
+    // Producer side (spread over the warps): warp w copies the slab rows r = w, w + nw, w + 2 nw, ... with
+    // its lanes 0, 1, 2, ...; warp 0 also posts the byte count.  The producer cursor runs kTpStages - 1
+    // slabs ahead of the consumer cursor, across passes and token blocks.
+    const int my_row = warp + nw * lane;
+    int p_blk = blockIdx.x, p_pass = 0, p_slab = 0, p_stage = 0;
+    uint32_t p_phase = 0;
+    const bm_bf16 *p_src = nullptr;
+    auto produce = [&]() {
+        if (p_blk >= n_blocks) return;
+        if (p_slab == 0 && my_row < rows) {
+            if (my_row < TB) {
+                const int t = p_blk * TB + my_row;
+                p_src = x + (size_t)(t < T ? t : T - 1) * D;          // rows past T: computed and dropped
+            } else {
+                const int e = p_pass * EB + my_row - TB;
+                p_src = Wr + (size_t)(e < E ? e : E - 1) * D;
             }
         }
-        if (lane == 0) {
-            // R3: softmax over the selected logits, sum in rank order
-            float w[BM_MAX_K];
-            const float m = sel_l[0];
-            float sum = 0.0f;
+        const int k0 = p_slab * kSlab;
+        const uint32_t bytes = (uint32_t)min(kSlab, D - k0) * 2u;
+        ptx::mbar_wait(&empty[p_stage], p_phase ^ 1);                 // every warp has released the slab held before
+        if (tid == 0) ptx::mbar_arrive_expect_tx(&full[p_stage], (uint32_t)rows * bytes);
+        if (my_row < rows)
+            bulk_g2s(tp_smem + (size_t)p_stage * stage_bytes + (size_t)my_row * (kSlab * 2), p_src + k0, bytes,
+                     &full[p_stage]);
+        if (++p_stage == kTpStages) { p_stage = 0; p_phase ^= 1; }
+        if (++p_slab == n_slabs) {
+            p_slab = 0;
+            if (++p_pass == n_pass) { p_pass = 0; p_blk += gridDim.x; }
+        }
+    };
+    for (int i = 0; i < kTpStages - 1; ++i) produce();
+
+    int stage = 0;
+    uint32_t phase = 0;
+    for (int blk = blockIdx.x; blk < n_blocks; blk += gridDim.x) {
+        const int t_block = blk * TB;
+        for (int pass = 0; pass < n_pass; ++pass) {
+            float acc[32];                      // index a = token * 8 + expert
 #pragma unroll
-            for (int i = 0; i < BM_MAX_K; ++i)
-                if (i < K) {
-                    w[i] = expf(__fsub_rn(sel_l[i], m));
-                    sum = __fadd_rn(sum, w[i]);
-                }
-            // R4 + R5: remap and dedup in rank order; first occurrence keeps the slot
-            int gid[BM_MAX_K];
-            float gw[BM_MAX_K];
-            int n = 0;
-            bool bad_map = false;
+            for (int a = 0; a < 32; ++a) acc[a] = 0.0f;
+            for (int slab = 0; slab < n_slabs; ++slab) {
+                produce();
+                ptx::mbar_wait(&full[stage], phase);
+                const uint8_t *st = tp_smem + (size_t)stage * stage_bytes;
+                if (slab * kSlab + lane * 8 < D) {
+                    float xf[kTpTok][8];
 #pragma unroll
-            for (int i = 0; i < BM_MAX_K; ++i)
-                if (i < K) {
-                    const float wi = __fdiv_rn(w[i], sum);
-                    int u = gmap[sel_e[i]];
-                    if (u < 0 || u >= G) { bad_map = true; u = u < 0 ? 0 : G - 1; }
-                    int s = n;                                     // index of the slot holding u, else n
+                    for (int i = 0; i < kTpTok; ++i) {
+                        const uint4 v = *reinterpret_cast<const uint4 *>(st + (tw * kTpTok + i) * (kSlab * 2) + lane * 16);
+                        xf[i][0] = bf16_lo(v.x); xf[i][1] = bf16_hi(v.x); xf[i][2] = bf16_lo(v.y); xf[i][3] = bf16_hi(v.y);
+                        xf[i][4] = bf16_lo(v.z); xf[i][5] = bf16_hi(v.z); xf[i][6] = bf16_lo(v.w); xf[i][7] = bf16_hi(v.w);
+                    }
 #pragma unroll
-                    for (int q = BM_MAX_K - 1; q >= 0; --q)
-                        if (q < n && gid[q] == u) s = q;
-                    if (s < n) {
+                    for (int j = 0; j < 8; ++j) {
+                        const uint4 wv = *reinterpret_cast<const uint4 *>(st + (TB + ew * 8 + j) * (kSlab * 2) + lane * 16);
+                        const float w0 = bf16_lo(wv.x), w1 = bf16_hi(wv.x), w2 = bf16_lo(wv.y), w3 = bf16_hi(wv.y);
+                        const float w4 = bf16_lo(wv.z), w5 = bf16_hi(wv.z), w6 = bf16_lo(wv.w), w7 = bf16_hi(wv.w);
 #pragma unroll
-                        for (int q = 0; q < BM_MAX_K; ++q)
-                            if (q == s) gw[q] = __fadd_rn(gw[q], wi);
-                    } else {
-#pragma unroll
-                        for (int q = 0; q < BM_MAX_K; ++q)
-                            if (q == n) { gid[q] = u; gw[q] = wi; }
-                        n++;
+                        for (int i = 0; i < kTpTok; ++i) {
+                            float pacc = acc[i * 8 + j];            // ascending element order inside the chunk
+                            pacc = __fmaf_rn(xf[i][0], w0, pacc);
+                            pacc = __fmaf_rn(xf[i][1], w1, pacc);
+                            pacc = __fmaf_rn(xf[i][2], w2, pacc);
+                            pacc = __fmaf_rn(xf[i][3], w3, pacc);
+                            pacc = __fmaf_rn(xf[i][4], w4, pacc);
+                            pacc = __fmaf_rn(xf[i][5], w5, pacc);
+                            pacc = __fmaf_rn(xf[i][6], w6, pacc);
+                            pacc = __fmaf_rn(xf[i][7], w7, pacc);
+                            acc[i * 8 + j] = pacc;
+                        }
                     }
                 }
-            const size_t base = (size_t)t * K;
-#pragma unroll
-            for (int i = 0; i < BM_MAX_K; ++i)
-                if (i < K) {
-                    expert_ids[base + i] = sel_e[i];
-                    group_ids[base + i] = i < n ? gid[i] : -1;
-                    gate_w[base + i] = i < n ? gw[i] : 0.0f;
-                }
-            n_slots[t] = n;
-            if (bad_map) atomicOr(status, BM_DEV_BAD_GROUP_MAP);
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(&empty[stage]);
+                if (++stage == kTpStages) { stage = 0; phase ^= 1; }
+            }
+            // end of a pass: lane l finishes accumulator l = (token l/8, expert l%8), adds the bias, parks it
+            butterfly32(acc, lane);
+            const int e = pass * EB + ew * 8 + (lane & 7);
+            if (e < E) {
+                float v = acc[0];
+                if (bias) v = __fadd_rn(v, bias[e]);
+                s_logits[(tw * kTpTok + (lane >> 3)) * E + e] = v;
+            }
         }
-        if (nonfinite) atomicOr(status, BM_DEV_NONFINITE_LOGIT);
+        __syncthreads();                        // all logits of the block are parked
+        for (int tl = warp; tl < TB; tl += nw) {
+            const int t = t_block + tl;
+            if (t >= T) break;
+            select_and_write(s_logits + tl * E, t, lane, E, K, gmap, G, expert_ids, group_ids, gate_w, n_slots, status);
+        }
+        __syncthreads();                        // before the next block overwrites them
     }
+}
+
+cudaError_t launch_tp(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const float *bias, int E, int K,
+                      const int32_t *gmap, int G, const bm_routing &r, int32_t *status, cudaStream_t stream) {
+    const int n_etiles = (E + 7) / 8;
+    int WE = 1;
+    while (WE < n_etiles && WE < 8) WE *= 2;
+    const int ncw = WE >= 4 ? 16 : 8;
+    const int WT = ncw / WE;
+    const int TB = WT * kTpTok, EB = WE * 8;
+    const size_t smem = (size_t)kTpStages * (TB + EB) * (kSlab * 2) + 2 * kTpStages * sizeof(uint64_t) +
+                        (size_t)TB * E * sizeof(float);
+    static size_t smem_set = 0;
+    if (smem > 48 * 1024 && smem > smem_set) {
+        cudaError_t e = cudaFuncSetAttribute(router_tp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        smem_set = smem;
+    }
+    const int n_blocks = (T + TB - 1) / TB;
+    const int grid = n_blocks < num_sms() ? n_blocks : num_sms();
+    return launch_kernel(router_tp_kernel, dim3(grid), dim3(ncw * 32), smem, stream, x, T, D, Wr, bias, E, K,
+                         gmap, G, WT, WE, n_blocks, r.expert_ids, r.group_ids, r.gate_w, r.n_slots, status);
 }
 
 template <int TOK, int ET>
@@ -201,10 +384,8 @@ cudaError_t launch_cfg(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const 
 cudaError_t launch_router(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const float *bias, int E,
                           int K, const int32_t *gmap, int G, const bm_routing &r, int32_t *status,
                           cudaStream_t stream) {
-    if (T >= 2048) {
-        // throughput shape: warps split tokens, 4 tokens x 8 experts per register tile
-        return launch_cfg<4, 8>(x, T, D, Wr, bias, E, K, gmap, G, /*WT=*/kWarps, /*WE=*/1, r, status, stream);
-    }
+    if (T >= tune_int("BM_ROUTER_TP_MIN_T", 512))   // throughput shape: operands staged through shared memory
+        return launch_tp(x, T, D, Wr, bias, E, K, gmap, G, r, status, stream);
     // latency shape: one token per warp pass, warps split the experts
     if (E <= 8) {
         int WE = 1;
