@@ -157,6 +157,7 @@ int bm_moe_forward_path(const bm_bf16 *x, int T, int D, const bm_routing *routin
     a.xs = reinterpret_cast<bm_bf16 *>(ws + w.xs);
     a.h = reinterpret_cast<bm_bf16 *>(ws + w.h);
     a.out_acc = reinterpret_cast<float *>(ws + w.out_acc);
+    a.y = reinterpret_cast<bm_bf16 *>(ws + w.y);
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     cudaError_t e;
     if (path == BM_PATH_SIMT) e = launch_forward_simt(a, st);

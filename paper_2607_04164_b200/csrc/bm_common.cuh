@@ -24,12 +24,13 @@ struct Workspace {
     size_t sched;        // int32[kSchedInts] tile-schedule scratch of the forward pass
     size_t xs;           // bf16[T*K, D]    token rows gathered in permuted order (prefill path)
     size_t h;            // bf16[T*K + S*T, F]  SwiGLU intermediate
-    size_t out_acc;      // f32[T, D]       fp32 accumulation of the combine
+    size_t out_acc;      // f32[T, D]       fp32 accumulation of the combine (decode path: split-K partials)
+    size_t y;            // bf16[T*K + S*T, D]  per-row expert outputs (prefill path), combined by combine_kernel
     size_t total;
 };
 
 constexpr int kMaxShared = 16;                                  // S <= 16 always-on shared experts
-constexpr int kSchedInts = 4 + 2 * (BM_MAX_G + kMaxShared) + 8;
+constexpr int kSchedInts = 4 + 4 * (BM_MAX_G + kMaxShared) + 8;
 
 __host__ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -44,6 +45,7 @@ __host__ inline Workspace workspace_layout(int T, int D, int F, int K, int G, in
     w.xs = off;          off = align_up(off + items * D * sizeof(bm_bf16), 1024);
     w.h = off;           off = align_up(off + (items + (size_t)S * T) * F * sizeof(bm_bf16), 1024);
     w.out_acc = off;     off = align_up(off + (size_t)T * D * sizeof(float), 1024);
+    w.y = off;           off = align_up(off + (items + (size_t)S * T) * D * sizeof(bm_bf16), 1024);
     w.total = off;
     return w;
 }
@@ -102,6 +104,7 @@ struct ForwardArgs {
     bm_bf16 *xs;
     bm_bf16 *h;
     float *out_acc;
+    bm_bf16 *y;
 };
 
 cudaError_t launch_forward_simt(const ForwardArgs &a, cudaStream_t stream);

@@ -17,8 +17,10 @@
 // roles from a small device-side schedule (non-empty segments and their 128-row chunks) that the prep
 // kernel builds from counts/offsets -- the host never sees the data-dependent counts.
 //
-// The combine accumulates in fp32 (`out_acc`, red.global.add) because a token's <= K group rows live in
-// different tiles (and, in decode, in different K-splits); a last pass rounds to bf16.
+// Combine.  A token's <= K group rows live in different tiles.  Prefill: GEMM2 stores y rows (bf16, coalesced
+// 128-byte pieces) and combine_kernel sums a token's rows in slot order with the gate weights -- no
+// atomics, deterministic.  Decode: rows also live in different K-splits and there are few of them, so the
+// partials are added in fp32 with red.global.add into `out_acc` and a last pass rounds to bf16.
 #include "bm_common.cuh"
 #include "bm_ptx.cuh"
 
@@ -44,27 +46,47 @@ static_assert((2 * kMaxStages + 2 * kAccStages) * 8 + 4 <= kSmemBars, "barrier b
 
 enum Mode { PF_GEMM1 = 0, PF_GEMM2 = 1, DC_GEMM1 = 2, DC_GEMM2 = 3 };
 
-// schedule (int32) written by the prep kernel
-//   [0] n_seg   [1] total_chunks   [4 .. 4+kMaxSeg) seg_u   [4+kMaxSeg .. 4+2*kMaxSeg+1) seg_chunk0
+// schedule (int32) written by the prep kernel: the non-empty segments (groups, then shared experts)
+//   [0] n_seg   [1] total_chunks
+//   seg_u[kMaxSeg]       weight set of segment s
+//   seg_chunk0[kMaxSeg]  first 128-row chunk of segment s; entry n_seg = total_chunks
+//   seg_rows[kMaxSeg]    rows of segment s (counts[u], or T for a shared expert)
+//   seg_off[kMaxSeg]     first permuted row of segment s (offsets[u]; 0 for a shared expert)
+// Every GEMM CTA copies the live part into shared memory once (SchedView over smem), so that the item
+// enumeration of its three roles never waits on global memory.
 constexpr int kSchedSegU = 4;
-constexpr int kSchedChunk0 = 4 + kMaxSeg;
-static_assert(kSchedChunk0 + kMaxSeg + 1 <= kSchedInts, "sched too small");
+constexpr int kSchedChunk0 = kSchedSegU + kMaxSeg;
+constexpr int kSchedRows = kSchedChunk0 + kMaxSeg;
+constexpr int kSchedOff = kSchedRows + kMaxSeg;
+static_assert(kSchedOff + kMaxSeg + 1 <= kSchedInts, "sched too small");
+
+struct SchedView {
+    int n_seg, total_chunks;
+    const int32_t *u, *chunk0, *rows, *off;
+};
+__device__ __forceinline__ SchedView sched_global(const int32_t *sched) {
+    return SchedView{sched[0], sched[1], sched + kSchedSegU, sched + kSchedChunk0, sched + kSchedRows, sched + kSchedOff};
+}
 
 struct GemmParams {
     int T, D, F, K, G, S, TK;
     int stages;         // depth of the shared-memory ring (<= kMaxStages)
     int stage_bytes;    // bytes of one ring stage (multiple of 1024)
     int off_b;          // decode: offset of the token rows (MMA B operand) inside a stage
-    int npad_box;       // decode: rows of the token box every stage loads (host: T rounded up to 32, <= 128)
+    int wslot;          // decode: bytes between the W1 and W3 tiles of a stage (R*128 rounded up to 1024)
+    int tail_pad;       // decode: bytes kept free after the ring (an M=128 MMA reads 16 KB from a tile base, R < 128 rows of it real)
     int kblocks;        // k-blocks of one item (per split)
     int ksplit;         // K splits (DC_GEMM2), else 1
     int R;              // weight rows per tile (prefill: 128 for GEMM1 per matrix, 256 for GEMM2)
     int n_wtiles;       // tiles along the weight-row dimension
+    int seg_cap;        // G + S + 1: entries per schedule array cached in shared memory
+    int dbg;
     const int32_t *counts, *offsets, *row_token, *row_slot;
     const float *gate_w;
     const int32_t *sched;
     bm_bf16 *h;
     float *out_acc;
+    bm_bf16 *y;
 };
 
 struct Item {
@@ -80,30 +102,27 @@ struct Item {
 };
 
 template <int MODE>
-__device__ __forceinline__ bool get_item(const GemmParams &p, int item, Item &it) {
-    const int32_t *sched = p.sched;
-    const int n_seg = sched[0];
+__device__ __forceinline__ bool get_item(const GemmParams &p, const SchedView &sv, int item, Item &it) {
     const int per_chunk = p.n_wtiles * p.ksplit;
-    const long long n_items = (long long)sched[1] * per_chunk;
+    const long long n_items = (long long)sv.total_chunks * per_chunk;
     if (item >= n_items) return false;
-    const int32_t *chunk0 = sched + kSchedChunk0;
-    int lo = 0, hi = n_seg - 1;               // last segment s with chunk0[s] * per_chunk <= item
+    int lo = 0, hi = sv.n_seg - 1;            // last segment s with chunk0[s] * per_chunk <= item
     while (lo < hi) {
         const int mid = (lo + hi + 1) >> 1;
-        if ((long long)chunk0[mid] * per_chunk <= item) lo = mid; else hi = mid - 1;
+        if ((long long)sv.chunk0[mid] * per_chunk <= item) lo = mid; else hi = mid - 1;
     }
     const int s = lo;
-    const int u = sched[kSchedSegU + s];
-    const int chunks_s = chunk0[s + 1] - chunk0[s];
-    const int local = item - chunk0[s] * per_chunk;
+    const int u = sv.u[s];
+    const int c0 = sv.chunk0[s];
+    const int chunks_s = sv.chunk0[s + 1] - c0;
+    const int local = item - c0 * per_chunk;
     const int chunk = local % chunks_s;
     const int rest = local / chunks_s;
     it.u = u;
     it.ks = rest % p.ksplit;
     it.wt = rest / p.ksplit;
     it.shared = u >= p.G;
-    const int rows = it.shared ? p.T : p.counts[u];
-    it.n = min(kChunkRows, rows - chunk * kChunkRows);
+    it.n = min(kChunkRows, sv.rows[s] - chunk * kChunkRows);
     if (it.shared) {
         it.tok0 = chunk * kChunkRows;
         it.perm_row0 = 0;
@@ -111,7 +130,7 @@ __device__ __forceinline__ bool get_item(const GemmParams &p, int item, Item &it
         it.act_row0 = (MODE == PF_GEMM1 || MODE == DC_GEMM1) ? it.tok0 : it.h_row0;
     } else {
         it.tok0 = 0;
-        it.perm_row0 = p.offsets[u] + chunk * kChunkRows;
+        it.perm_row0 = sv.off[s] + chunk * kChunkRows;
         it.h_row0 = it.perm_row0;
         it.act_row0 = it.perm_row0;
     }
@@ -143,6 +162,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
     uint64_t *tempty = tfull + kAccStages;       // [kAccStages]
     uint32_t *tmem_ptr = reinterpret_cast<uint32_t *>(tempty + kAccStages);
     uint8_t *epi_stage = reinterpret_cast<uint8_t *>(bars) + kSmemBars;   // [4][kEpiStageBytes], 256-byte aligned
+    int32_t *s_sched = reinterpret_cast<int32_t *>(epi_stage + (MODE == PF_GEMM2 ? kSmemEpi : 0));   // [4][seg_cap]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -163,8 +183,44 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
 
     const int nkb = p.kblocks;
     // bytes one stage receives: constant per launch (decode always loads the full padded token box)
-    const uint32_t stage_tx = !kDecode ? 3u * kTileBytes16K
-                                       : (uint32_t)((kGemm1 ? 2 : 1) * p.R * 128 + p.npad_box * 128);
+    // bytes one stage receives.  Decode: the weight box(es) of R rows plus the item's token rows in 32-row
+    // boxes (tok_tx(n)): only the rows the group really has travel from L2.
+    const uint32_t w_tx = !kDecode ? 3u * kTileBytes16K : (uint32_t)((kGemm1 ? 2 : 1) * p.R * 128);
+    auto stage_tx_of = [&](int n) -> uint32_t { return kDecode ? w_tx + (uint32_t)((n + 31) >> 5) * 4096u : w_tx; };
+
+    // DC_GEMM2: W2 does not depend on the predecessor (GEMM1), so warp 0 fills the ring with the weight tiles
+    // of its first item BEFORE the grid-dependency wait: the HBM stream starts while GEMM1's last CTAs
+    // drain.  The schedule it reads (from global memory) was written by the prep kernel, which completed
+    // before GEMM1 (which triggers this launch only after its own wait) let this grid start.
+    Item it0;
+    bool have0 = false;
+    int pre = 0;
+    if (MODE == DC_GEMM2 && warp == 0) {
+        have0 = get_item<MODE>(p, sched_global(p.sched), blockIdx.x, it0);
+        pre = have0 ? min(n_stages, nkb) : 0;
+        if (ptx::elect_one())
+            for (int kb = 0; kb < pre; ++kb) {
+                ptx::mbar_arrive_expect_tx(&full[kb], stage_tx_of(it0.n));
+                ptx::tma_load_3d(smem + (size_t)kb * stage_bytes, &tm_w0, &full[kb], (it0.ks * nkb + kb) * kBlockK,
+                                 it0.wt * p.R, it0.u, ptx::kEvictFirst);
+            }
+        __syncwarp();
+    }
+    grid_dep_wait();
+    // schedule -> shared memory (item enumeration is on the critical path of all three roles)
+    const int cap = p.seg_cap;
+    SchedView sv;
+    sv.n_seg = min(p.sched[0], cap - 1);
+    sv.total_chunks = p.sched[1];
+    sv.u = s_sched; sv.chunk0 = s_sched + cap; sv.rows = s_sched + 2 * cap; sv.off = s_sched + 3 * cap;
+    for (int i = threadIdx.x; i <= sv.n_seg; i += kThreads) {
+        s_sched[i] = p.sched[kSchedSegU + i];
+        s_sched[cap + i] = p.sched[kSchedChunk0 + i];
+        s_sched[2 * cap + i] = p.sched[kSchedRows + i];
+        s_sched[3 * cap + i] = p.sched[kSchedOff + i];
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) grid_dep_launch();
 
     // The producer and the MMA issuer run their loops with the WHOLE warp (warp-uniform control flow keeps
     // addresses and descriptors in uniform registers) and elect one lane for the issuing instructions: the
@@ -178,37 +234,25 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
         int kb_first = 0;
         bool have;
         if (MODE == DC_GEMM2) {
-            // W2 does not depend on the predecessor (GEMM1): fill the ring with weight tiles BEFORE the
-            // grid-dependency wait, so the HBM stream starts while GEMM1's last CTAs drain.  The schedule
-            // read by get_item was written by the prep kernel, which completed before GEMM1 (which
-            // triggers this launch only after its own wait) let this grid start.
-            have = get_item<MODE>(p, item, it);
-            const int pre = have ? min(n_stages, nkb) : 0;
-            if (ptx::elect_one())
-                for (int kb = 0; kb < pre; ++kb) {
-                    ptx::mbar_arrive_expect_tx(&full[kb], stage_tx);
-                    ptx::tma_load_3d(smem + (size_t)kb * stage_bytes, &tm_w0, &full[kb], (it.ks * nkb + kb) * kBlockK,
-                                     it.wt * p.R, it.u, ptx::kEvictFirst);
-                }
-            __syncwarp();
-            grid_dep_wait();
+            it = it0;
+            have = have0;
             if (ptx::elect_one())
                 for (int kb = 0; kb < pre; ++kb)
-                    ptx::tma_load_2d(smem + (size_t)kb * stage_bytes + p.off_b, &tm_act0, &full[kb],
-                                     (it.ks * nkb + kb) * kBlockK, it.act_row0, ptx::kEvictLast);
+                    for (int j = 0; j * 32 < it.n; ++j)
+                        ptx::tma_load_2d(smem + (size_t)kb * stage_bytes + p.off_b + j * 4096, &tm_act0, &full[kb],
+                                         (it.ks * nkb + kb) * kBlockK, it.act_row0 + j * 32, ptx::kEvictLast);
             __syncwarp();
             kb_first = pre;
             stage = pre;
             if (stage == n_stages) { stage = 0; phase = 1; }
         } else {
-            grid_dep_wait();
-            have = get_item<MODE>(p, item, it);
+            have = get_item<MODE>(p, sv, item, it);
         }
-        if (lane == 0) grid_dep_launch();
-        for (; have; item += gridDim.x, have = get_item<MODE>(p, item, it), kb_first = 0) {
+        for (; have; item += gridDim.x, have = get_item<MODE>(p, sv, item, it), kb_first = 0) {
             const CUtensorMap *tm_act = (kGemm1 && it.shared) ? &tm_act1 : &tm_act0;
             const int wrow0 = it.wt * p.R;
             int kc = (it.ks * nkb + kb_first) * kBlockK;
+            const uint32_t stage_tx = stage_tx_of(it.n);
             for (int kb = kb_first; kb < nkb; ++kb, kc += kBlockK) {
                 ptx::mbar_wait(&empty[stage], phase ^ 1);
                 if (ptx::elect_one()) {
@@ -222,11 +266,13 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
                             ptx::tma_load_3d(st + 2 * kTileBytes16K, &tm_w1, &full[stage], kc, wrow0, it.u, ptx::kEvictFirst);
                     } else {
                         // M side = R weight rows (streamed once from HBM), N side = the group's token rows
-                        // (one box of npad_box rows; rows past the group's are loaded and never multiplied)
+                        // (32-row boxes; rows past the group's within the last box are loaded and never stored)
                         ptx::tma_load_3d(st, &tm_w0, &full[stage], kc, wrow0, it.u, ptx::kEvictFirst);
                         if (MODE == DC_GEMM1)
-                            ptx::tma_load_3d(st + kTileBytes16K, &tm_w1, &full[stage], kc, wrow0, it.u, ptx::kEvictFirst);
-                        ptx::tma_load_2d(st + p.off_b, tm_act, &full[stage], kc, it.act_row0, ptx::kEvictLast);
+                            ptx::tma_load_3d(st + p.wslot, &tm_w1, &full[stage], kc, wrow0, it.u, ptx::kEvictFirst);
+                        for (int j = 0; j * 32 < it.n; ++j)
+                            ptx::tma_load_2d(st + p.off_b + j * 4096, tm_act, &full[stage], kc, it.act_row0 + j * 32,
+                                             ptx::kEvictLast);
                     }
                 }
                 __syncwarp();
@@ -235,18 +281,18 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
         }
     } else if (warp == 1) {
         // =========================== MMA issuer ===========================
-        grid_dep_wait();
         // descriptor low words: (smem address >> 4) | LBO; the high word (SBO, version, swizzle) is constant
         const uint32_t a_lo0 = ptx::smem_desc_lo(ptx::smem_u32(smem));
         const uint32_t b_off = (uint32_t)(kDecode ? p.off_b : kTileBytes16K) >> 4;
         const uint32_t stage_step = stage_bytes >> 4;
+        const uint32_t w3_off = (uint32_t)p.wslot >> 4;
         uint32_t a_lo = a_lo0;
         int stage = 0;
         uint32_t phase = 0;
         int acc = 0;
         uint32_t acc_phase = 0;
         Item it;
-        for (int item = blockIdx.x; get_item<MODE>(p, item, it); item += gridDim.x) {
+        for (int item = blockIdx.x; get_item<MODE>(p, sv, item, it); item += gridDim.x) {
             const uint32_t idesc = kDecode ? ptx::make_idesc_bf16(128, (it.n + 31) & ~31) : ptx::make_idesc_bf16(128, 256);
             ptx::mbar_wait(&tempty[acc], acc_phase ^ 1);
             ptx::tc_fence_after();
@@ -261,7 +307,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
                         const uint32_t ko = 2 * k;             // 16 bf16 = 32 bytes = 2 descriptor units
                         ptx::mma_bf16_ss(d_tmem, ptx::smem_desc(a_lo + ko), ptx::smem_desc(a_lo + b_off + ko), idesc, accum);
                         if (MODE == DC_GEMM1)
-                            ptx::mma_bf16_ss(d_tmem + 128, ptx::smem_desc(a_lo + (kTileBytes16K >> 4) + ko),
+                            ptx::mma_bf16_ss(d_tmem + 128, ptx::smem_desc(a_lo + w3_off + ko),
                                              ptx::smem_desc(a_lo + b_off + ko), idesc, accum);
                     }
                     ptx::mma_commit(&empty[stage]);                  // frees the smem stage when the MMAs retire
@@ -275,13 +321,12 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
         }
     } else {
         // =========================== epilogue (warps 2..5) ===========================
-        grid_dep_wait();
         const int q = warp & 3;                      // TMEM lane quarter this warp may read
         const int row = q * 32 + lane;               // accumulator row (M index) owned by this thread
         int acc = 0;
         uint32_t acc_phase = 0;
         Item it;
-        for (int item = blockIdx.x; get_item<MODE>(p, item, it); item += gridDim.x) {
+        for (int item = blockIdx.x; get_item<MODE>(p, sv, item, it); item += gridDim.x) {
             ptx::mbar_wait(&tfull[acc], acc_phase);
             ptx::tc_fence_after();
             const uint32_t t_addr = tmem_base + acc * kAccCols + ((uint32_t)(q * 32) << 16);
@@ -308,43 +353,44 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
                     }
                 }
             } else if (MODE == PF_GEMM2) {
-                // row = token row; columns = 256 output features d0..d0+255; scatter-combine with the gate weight.
-                // The accumulator leaves TMEM with one row per lane; a per-warp shared-memory transpose (32 rows
-                // x 32 columns fp32, 16-byte units xor-swizzled by the row) turns that into row-contiguous
-                // pieces, so every red.global.add.v4.f32 of a warp covers 4 rows x 128 contiguous bytes
-                // (whole L2 lines) instead of 32 scattered 16-byte pieces.
-                int tok = -1;
-                float gw = 1.0f;
-                if (row < it.n) {
-                    if (it.shared) {
-                        tok = it.tok0 + row;
-                    } else {
-                        tok = p.row_token[it.perm_row0 + row];
-                        gw = p.gate_w[(size_t)tok * p.K + p.row_slot[it.perm_row0 + row]];
-                    }
-                }
+                // row = token row of the chunk; columns = 256 output features d0..d0+255 of y_r = H_r . W2[u]^T.
+                // y is stored as bf16 rows (same row numbering as H); combine_kernel applies the gate weights and
+                // sums a token's rows in slot order.  The accumulator leaves TMEM with one row per lane; a
+                // per-warp shared-memory transpose (32 rows x 64 bf16 columns, 16-byte units xor-swizzled by
+                // the row) turns that into row-contiguous pieces, so every 128-bit store instruction of a warp
+                // writes 4 rows x 128 contiguous bytes (whole L2 lines) instead of 32 scattered pieces.
                 const int d0 = it.wt * 256;
-                float4 *stg = reinterpret_cast<float4 *>(epi_stage + (size_t)q * kEpiStageBytes);
+                const int n_q = it.n - q * 32;                     // valid rows of this warp's quarter
+                uint4 *stg = reinterpret_cast<uint4 *>(epi_stage + (size_t)q * kEpiStageBytes);
                 const int rl = lane >> 3, ul = lane & 7;        // read phase: row (mod 4) and 16-byte unit of this lane
+                bm_bf16 *ybase = p.y + (size_t)(it.h_row0 + q * 32) * p.D + d0 + 8 * ul;
 #pragma unroll 1
-                for (int c = 0; c < 256; c += 32) {
-                    uint32_t v[32];
+                for (int c = 0; c < ((p.dbg & 2) ? 0 : 256); c += 64) {
+                    uint32_t v[32], w[32];
                     ptx::tmem_ld_x32(t_addr + c, v);
+                    ptx::tmem_ld_x32(t_addr + c + 32, w);
                     ptx::tmem_ld_wait();
 #pragma unroll
-                    for (int u = 0; u < 8; ++u)
+                    for (int u = 0; u < 4; ++u) {
                         stg[lane * 8 + (u ^ (lane & 7))] =
-                            make_float4(gw * __uint_as_float(v[4 * u]), gw * __uint_as_float(v[4 * u + 1]),
-                                        gw * __uint_as_float(v[4 * u + 2]), gw * __uint_as_float(v[4 * u + 3]));
+                            make_uint4(pack_bf16x2(__uint_as_float(v[8 * u]), __uint_as_float(v[8 * u + 1])),
+                                       pack_bf16x2(__uint_as_float(v[8 * u + 2]), __uint_as_float(v[8 * u + 3])),
+                                       pack_bf16x2(__uint_as_float(v[8 * u + 4]), __uint_as_float(v[8 * u + 5])),
+                                       pack_bf16x2(__uint_as_float(v[8 * u + 6]), __uint_as_float(v[8 * u + 7])));
+                        stg[lane * 8 + ((u + 4) ^ (lane & 7))] =
+                            make_uint4(pack_bf16x2(__uint_as_float(w[8 * u]), __uint_as_float(w[8 * u + 1])),
+                                       pack_bf16x2(__uint_as_float(w[8 * u + 2]), __uint_as_float(w[8 * u + 3])),
+                                       pack_bf16x2(__uint_as_float(w[8 * u + 4]), __uint_as_float(w[8 * u + 5])),
+                                       pack_bf16x2(__uint_as_float(w[8 * u + 6]), __uint_as_float(w[8 * u + 7])));
+                    }
                     __syncwarp();
+                    if (d0 + c + 8 * ul + 8 <= p.D) {
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) {
-                        const int r = 4 * j + rl;
-                        const float4 o = stg[r * 8 + (ul ^ (r & 7))];
-                        const int tk = __shfl_sync(0xffffffffu, tok, r);
-                        const int d = d0 + c + 4 * ul;
-                        if (tk >= 0 && d + 4 <= p.D)
-                            ptx::red_add_v4_f32(p.out_acc + (size_t)tk * p.D + d, o.x, o.y, o.z, o.w);
+                        for (int j = 0; j < 8; ++j) {
+                            const int r = 4 * j + rl;
+                            if (r < n_q && !(p.dbg & 1))
+                                *reinterpret_cast<uint4 *>(ybase + (size_t)r * p.D + c) = stg[r * 8 + (ul ^ (r & 7))];
+                        }
                     }
                     __syncwarp();
                 }
@@ -437,7 +483,7 @@ __global__ void __launch_bounds__(256)
 prep_kernel(const bm_bf16 *__restrict__ x, int T, int D, int K, int G, int S,
             const int32_t *__restrict__ counts, const int32_t *__restrict__ offsets,
             const int32_t *__restrict__ row_token, int32_t *__restrict__ sched, bm_bf16 *__restrict__ xs,
-            float *__restrict__ out_acc, int32_t *__restrict__ status) {
+            float *__restrict__ out_acc, int decode, int32_t *__restrict__ status) {
     grid_dep_wait();
     grid_dep_launch();
     if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -449,6 +495,8 @@ prep_kernel(const bm_bf16 *__restrict__ x, int T, int D, int K, int G, int S,
             if (rows <= 0) continue;
             sched[kSchedSegU + n_seg] = u;
             sched[kSchedChunk0 + n_seg] = chunks;
+            sched[kSchedRows + n_seg] = rows;
+            sched[kSchedOff + n_seg] = u < G ? offsets[u] : 0;
             chunks += (rows + kChunkRows - 1) / kChunkRows;
             ++n_seg;
         }
@@ -457,12 +505,13 @@ prep_kernel(const bm_bf16 *__restrict__ x, int T, int D, int K, int G, int S,
         sched[1] = chunks;
         if (bad) atomicOr(status, BM_DEV_BAD_ROUTING);
     }
-    // zero out_acc
-    const size_t n4 = (size_t)T * D / 4;
+    // zero out_acc (decode path only: the prefill path combines plain y rows)
+    const size_t n4 = decode ? (size_t)T * D / 4 : 0;
     float4 *o4 = reinterpret_cast<float4 *>(out_acc);
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x)
         o4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    // gather: one warp per permuted row
+    // gather: one warp per permuted row.  (A tile::gather4 producer in GEMM1 was measured instead of this
+    // pass: ~12 cycles per 128-byte row made GEMM1 3x slower, so the rows are materialised once here.)
     const int A = min(offsets[G], T * K);
     const int warps = (gridDim.x * blockDim.x) >> 5;
     const int lane = threadIdx.x & 31;
@@ -485,6 +534,63 @@ finalize_kernel(const float *__restrict__ out_acc, bm_bf16 *__restrict__ out, si
         const float4 b = reinterpret_cast<const float4 *>(out_acc)[2 * i + 1];
         reinterpret_cast<uint4 *>(out)[i] = make_uint4(pack_bf16x2(a.x, a.y), pack_bf16x2(a.z, a.w),
                                                        pack_bf16x2(b.x, b.y), pack_bf16x2(b.z, b.w));
+    }
+}
+
+// Prefill combine (F2): out[t] = sum_{s < n_slots[t]} gate_w[t,s] * y[slot_row[t,s]]  (slot order)
+//                               + sum_{j < S} y[TK + j*T + t]                          (shared experts)
+// fp32 accumulation in a fixed order -> deterministic.  One thread per 8 output columns (16 bytes).
+__global__ void __launch_bounds__(256)
+combine_kernel(const bm_bf16 *__restrict__ y, int T, int D, int K, int S, const int32_t *__restrict__ n_slots,
+               const int32_t *__restrict__ slot_row, const float *__restrict__ gate_w, bm_bf16 *__restrict__ out) {
+    grid_dep_wait();
+    grid_dep_launch();
+    const int vec = D / 8;
+    const size_t total = (size_t)T * vec;
+    const size_t TK = (size_t)T * K;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const int t = (int)(i / vec);
+        const int col = (int)(i - (size_t)t * vec) * 8;
+        float acc[8];
+#pragma unroll
+        for (int e = 0; e < 8; ++e) acc[e] = 0.0f;
+        const int n = min(max(n_slots[t], 0), K);
+        // four rows at a time: all row indices, then all loads, then the adds in slot order
+        for (int s0 = 0; s0 < n + S; s0 += 4) {
+            size_t row[4];
+            float gw[4];
+            bool ok[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int s = s0 + q;
+                ok[q] = s < n + S;
+                gw[q] = 1.0f;
+                row[q] = 0;
+                if (s < n) {
+                    const int r = slot_row[(size_t)t * K + s];
+                    ok[q] = r >= 0 && (size_t)r < TK;
+                    row[q] = ok[q] ? (size_t)r : 0;
+                    gw[q] = gate_w[(size_t)t * K + s];
+                } else if (ok[q]) {
+                    row[q] = TK + (size_t)(s - n) * T + t;
+                }
+            }
+            uint4 v[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                v[q] = ok[q] ? *reinterpret_cast<const uint4 *>(y + row[q] * D + col) : make_uint4(0, 0, 0, 0);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                if (!ok[q]) continue;
+                acc[0] = fmaf(gw[q], bf16_lo(v[q].x), acc[0]); acc[1] = fmaf(gw[q], bf16_hi(v[q].x), acc[1]);
+                acc[2] = fmaf(gw[q], bf16_lo(v[q].y), acc[2]); acc[3] = fmaf(gw[q], bf16_hi(v[q].y), acc[3]);
+                acc[4] = fmaf(gw[q], bf16_lo(v[q].z), acc[4]); acc[5] = fmaf(gw[q], bf16_hi(v[q].z), acc[5]);
+                acc[6] = fmaf(gw[q], bf16_lo(v[q].w), acc[6]); acc[7] = fmaf(gw[q], bf16_hi(v[q].w), acc[7]);
+            }
+        }
+        *reinterpret_cast<uint4 *>(out + (size_t)t * D + col) =
+            make_uint4(pack_bf16x2(acc[0], acc[1]), pack_bf16x2(acc[2], acc[3]), pack_bf16x2(acc[4], acc[5]),
+                       pack_bf16x2(acc[6], acc[7]));
     }
 }
 
@@ -535,45 +641,75 @@ bool make_map_3d(CUtensorMap *m, const void *base, uint64_t n, uint64_t rows, ui
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-// Decode tiling: rows-per-tile R in [32,128] and K-split count so that the number of equal-cost items
-// is as close as possible to a multiple of the SM count (static round-robin schedule).
-void choose_decode_tiling(int wrows, int kblocks, int n_seg, bool allow_split, int sms, int *R_out, int *ks_out) {
-    double best = -1.0;
+// Decode tiling: rows-per-tile R in [32,128] and the K-split count, chosen with a small time model of the
+// static round-robin schedule (all figures measured on B200):
+//   * a k-block iteration costs at least t0 whatever R is -- the swap-AB MMA reads a full M=128 A tile
+//     from shared memory per instruction, so 4 (GEMM2) or 8 (GEMM1) MMAs per k-block take ~0.30-0.37 us;
+//   * a wave of `act` concurrent items moves act * item_bytes at the chip's HBM rate, and one SM cannot
+//     pull more than ~0.1 MB/us on its own;
+//   * items / SMs full waves plus one partial wave.
+// Small R (many equal items, perfect wave count) used to win the old "wave occupancy" score and lost up to
+// 40% in practice to the per-k-block floor; large R wins whenever the HBM time of a wave covers it.
+double decode_time_model(int wrows, int kblocks, int n_seg, int R, int ks, int mats, int sms) {
+    const double kChipBytesPerUs = 6.5e6, kSmBytesPerUs = 0.1e6;
+    const double t0 = mats == 2 ? 0.37 : 0.30;
+    const int tiles = (wrows + R - 1) / R;
+    const long long items = (long long)tiles * n_seg * ks;
+    const int kbi = kblocks / ks;
+    const double b_item = (double)R * 128.0 * mats * kbi;
+    const double t_issue = kbi * t0;
+    auto wave = [&](double act) {
+        double t = t_issue;
+        if (b_item * act / kChipBytesPerUs > t) t = b_item * act / kChipBytesPerUs;
+        if (b_item / kSmBytesPerUs > t) t = b_item / kSmBytesPerUs;
+        return t;
+    };
+    const long long full = items / sms, rem = items % sms;
+    double t = (double)full * wave((double)sms) + (rem ? wave((double)rem) : 0.0);
+    return t * (1.0 + 0.01 * (ks - 1));       // split-K: extra fp32 reds in the epilogue
+}
+
+void choose_decode_tiling(int wrows, int kblocks, int n_seg, bool allow_split, int mats, int sms, int *R_out,
+                          int *ks_out) {
+    double best = 1e30;
     int bestR = 128, bestKs = 1;
     const int max_ks = allow_split ? 16 : 1;
     int rmax = tune_int("BM_DC_RMAX", 128);
     rmax = rmax < 32 ? 32 : (rmax > 128 ? 128 : rmax);
     for (int ks = 1; ks <= max_ks; ++ks) {
-        if (kblocks % ks != 0 || kblocks / ks < 4) { if (ks > 1) continue; }
+        if (ks > 1 && (kblocks % ks != 0 || kblocks / ks < 4)) continue;
         for (int R = rmax; R >= 32; --R) {
-            const int tiles = (wrows + R - 1) / R;
-            const long long items = (long long)tiles * n_seg * ks;
-            const long long waves = (items + sms - 1) / sms;
-            // useful rows / rows paid for, times wave occupancy; mild penalty for tiny tiles
-            double eff = (double)wrows / ((double)tiles * R) * (double)items / (double)(waves * sms);
-            eff -= 0.0005 * (rmax - R) / 96.0 + 0.002 * (ks - 1);
-            if (eff > best + 1e-9) { best = eff; bestR = R; bestKs = ks; }
+            const double t = decode_time_model(wrows, kblocks, n_seg, R, ks, mats, sms);
+            if (t < best * 0.99) { best = t; bestR = R; bestKs = ks; }   // within 1%: keep the larger tile
         }
     }
     *R_out = bestR;
     *ks_out = bestKs;
 }
 
-// Ring geometry.  Prefill: 4 stages x (16 KB tokens + 32 KB weights).  Decode: a stage holds the weight
-// tile(s) (16 KB each, R <= 128 rows used) and the token rows padded to 32 (npad_max x 128 B); as many
-// stages as fit in 227 KB, because the bytes in flight per SM are what the HBM stream lives on.
+size_t sched_smem_bytes(int seg_cap) { return ((size_t)4 * seg_cap * sizeof(int32_t) + 255) & ~(size_t)255; }
+
 void ring_geometry(bool decode, bool gemm1, int T, GemmParams *p) {
+    p->tail_pad = 0;
     if (!decode) {
         p->stage_bytes = 3 * kTileBytes16K;
         p->off_b = kTileBytes16K;
+        p->wslot = kTileBytes16K;
     } else {
+        // a stage = the weight tile(s), R rows x 128 B each (slot rounded up to the 1024-byte swizzle atom), and
+        // room for the largest token chunk (rows padded to 32).  An M=128 MMA reads 16 KB from a tile base
+        // whatever R is (rows >= R give accumulator rows that are never stored), so the last tile of the last
+        // stage needs that much addressable shared memory behind it: tail_pad.
         const int rows = T < kChunkRows ? T : kChunkRows;
-        const int npad_max = (rows + 31) & ~31;
-        p->off_b = (gemm1 ? 2 : 1) * kTileBytes16K;
-        p->stage_bytes = p->off_b + npad_max * 128;
-        p->npad_box = npad_max;
+        const int tok_bytes = ((rows + 31) & ~31) * 128;
+        p->wslot = (p->R * 128 + 1023) & ~1023;
+        p->off_b = (gemm1 ? 2 : 1) * p->wslot;
+        p->stage_bytes = p->off_b + tok_bytes;
+        const int behind = p->wslot + tok_bytes;
+        p->tail_pad = behind >= kTileBytes16K ? 0 : kTileBytes16K - behind;
     }
-    int st = (int)((kSmemRing - (decode ? 0 : kSmemEpi)) / (size_t)p->stage_bytes);
+    const size_t fixed = (decode ? 0 : kSmemEpi) + sched_smem_bytes(p->seg_cap) + (size_t)p->tail_pad;
+    int st = (int)((kSmemRing - fixed) / (size_t)p->stage_bytes);
     const int cap = tune_int(decode ? "BM_DC_STAGES" : "BM_PF_STAGES", kMaxStages);
     if (st > cap) st = cap;
     if (st > kMaxStages) st = kMaxStages;
@@ -592,7 +728,8 @@ cudaError_t launch_gemm(const CUtensorMap &a0, const CUtensorMap &a1, const CUte
         attr_set = true;
     }
     constexpr int kid = (MODE == PF_GEMM1 || MODE == DC_GEMM1) ? BM_KERNEL_GEMM1 : BM_KERNEL_GEMM2;
-    const size_t smem = 1024 + (size_t)p.stages * p.stage_bytes + kSmemBars + (MODE == PF_GEMM2 ? kSmemEpi : 0);
+    const size_t smem = 1024 + (size_t)p.stages * p.stage_bytes + kSmemBars + (MODE == PF_GEMM2 ? kSmemEpi : 0) +
+                        sched_smem_bytes(p.seg_cap) + (size_t)p.tail_pad;
     profile_begin(kid, stream);
     cudaError_t e = launch_kernel(kern, dim3(num_sms()), dim3(kThreads), smem, stream, a0, a1, w0, w1, p);
     profile_end(kid, stream);
@@ -610,15 +747,17 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
         const int grid = sms * 4;
         profile_begin(BM_KERNEL_PREP, stream);
         cudaError_t e = launch_kernel(prep_kernel, dim3(grid), dim3(256), 0, stream, a.x, a.T, a.D, a.K, a.G, a.S,
-                                      a.r.counts, a.r.offsets, a.r.row_token, a.sched, a.xs, a.out_acc, a.status);
+                                      a.r.counts, a.r.offsets, a.r.row_token, a.sched, a.xs, a.out_acc, decode ? 1 : 0, a.status);
         if (e != cudaSuccess) return e;
         profile_end(BM_KERNEL_PREP, stream);
     }
 
     GemmParams p{};
+    p.dbg = tune_int("BM_DBG", 0);
+    p.seg_cap = a.G + a.S + 1;
     p.T = a.T; p.D = a.D; p.F = a.F; p.K = a.K; p.G = a.G; p.S = a.S; p.TK = TK;
     p.counts = a.r.counts; p.offsets = a.r.offsets; p.row_token = a.r.row_token; p.row_slot = a.r.row_slot;
-    p.gate_w = a.r.gate_w; p.sched = a.sched; p.h = a.h; p.out_acc = a.out_acc;
+    p.gate_w = a.r.gate_w; p.sched = a.sched; p.h = a.h; p.out_acc = a.out_acc; p.y = a.y;
 
 
     const uint64_t h_rows = (uint64_t)TK + (uint64_t)a.S * a.T;
@@ -643,21 +782,20 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
         n_seg += a.S;
         if (n_seg < 1) n_seg = 1;
         int R1, R2, ks1, ks2;
-        choose_decode_tiling(a.F, kb1, n_seg, false, sms, &R1, &ks1);
-        choose_decode_tiling(a.D, kb2, n_seg, true, sms, &R2, &ks2);
+        choose_decode_tiling(a.F, kb1, n_seg, false, 2, sms, &R1, &ks1);
+        choose_decode_tiling(a.D, kb2, n_seg, true, 1, sms, &R2, &ks2);
         if (tune_int("BM_DC_R2", 0) > 0) { R2 = tune_int("BM_DC_R2", 0); ks2 = tune_int("BM_DC_KS2", 1); }
         if (tune_int("BM_DC_R1", 0) > 0) R1 = tune_int("BM_DC_R1", 0);
-        const int rows_max = a.T < kChunkRows ? a.T : kChunkRows;
-        const int nbox = (rows_max + 31) & ~31;      // token rows every stage loads (ring_geometry: npad_box)
+        const int nbox = 32;                         // token rows travel in 32-row boxes, as many as the chunk has
         if (!make_map_2d(&m_xs, a.xs, TK > 0 ? TK : 1, a.D, nbox) || !make_map_2d(&m_x, a.x, a.T, a.D, nbox) ||
             !make_map_3d(&m_w1, a.W1, a.G + a.S, a.F, a.D, R1) || !make_map_3d(&m_w3, a.W3, a.G + a.S, a.F, a.D, R1) ||
             !make_map_3d(&m_w2, a.W2, a.G + a.S, a.D, a.F, R2) || !make_map_2d(&m_h, a.h, h_rows, a.F, nbox))
             return cudaErrorInvalidValue;
-        ring_geometry(true, true, a.T, &p);
         p.ksplit = 1; p.kblocks = kb1; p.R = R1; p.n_wtiles = (a.F + R1 - 1) / R1;
+        ring_geometry(true, true, a.T, &p);
         if ((err = launch_gemm<DC_GEMM1>(m_xs, m_x, m_w1, m_w3, p, stream)) != cudaSuccess) return err;
-        ring_geometry(true, false, a.T, &p);
         p.ksplit = ks2; p.kblocks = kb2 / ks2; p.R = R2; p.n_wtiles = (a.D + R2 - 1) / R2;
+        ring_geometry(true, false, a.T, &p);
         if ((err = launch_gemm<DC_GEMM2>(m_h, m_h, m_w2, m_w2, p, stream)) != cudaSuccess) return err;
     }
 
@@ -667,7 +805,12 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
         if (grid > sms * 8) grid = sms * 8;
         if (grid < 1) grid = 1;
         profile_begin(BM_KERNEL_FINALIZE, stream);
-        cudaError_t e = launch_kernel(finalize_kernel, dim3(grid), dim3(256), 0, stream, (const float *)a.out_acc, a.out, n8);
+        cudaError_t e;
+        if (decode)
+            e = launch_kernel(finalize_kernel, dim3(grid), dim3(256), 0, stream, (const float *)a.out_acc, a.out, n8);
+        else
+            e = launch_kernel(combine_kernel, dim3(grid), dim3(256), 0, stream, (const bm_bf16 *)a.y, a.T, a.D, a.K, a.S,
+                              (const int32_t *)a.r.n_slots, (const int32_t *)a.r.slot_row, (const float *)a.r.gate_w, a.out);
         profile_end(BM_KERNEL_FINALIZE, stream);
         return e;
     }
