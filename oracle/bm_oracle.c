@@ -1,5 +1,6 @@
 /*
- * bm_oracle.c -- the CPU ORACLE for the grouped MoE-layer forward pass (BrownoutMoE full-brownout path).
+ * bm_oracle.c -- the CPU ORACLE for the grouped MoE-layer forward pass (BrownoutMoE full-brownout path; also
+ *               partial brownout, SURVEY 8(f) NEXT-1, and the united-weight average, NEXT-3).
  *
  * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and bench.py's
  * cpu_baseline / --impl reference legs may build, load or call it.  It shares no code with the CUDA
@@ -60,14 +61,21 @@ float oracle_canon_dot(const uint16_t *x, const uint16_t *w, int D) {
  *   expert_ids, group_ids, slot_row [T*K] i32; gate_w [T*K] f32; n_slots [T]; counts [G]; offsets [G+1];
  *   row_token, row_slot [T*K] (first A = offsets[G] valid, rest -1); logits [T*E] f32 or NULL.
  * Returns 0, or -1 on a bad shape / group_map entry outside [0,G). */
-int oracle_route(const uint16_t *x, int T, int D, const uint16_t *Wr, const float *bias, int E, int K,
-                 const int32_t *gmap, int G,
+/* Partial brownout ("partial-brownout delegates only cold expert tokens to united experts"; P:172
+ * "the original gate still determines the ac[tivated experts]"; "the grouping map determines which
+ * united expert handles tokens originally routed to each cold expert"; A9: the caller says which
+ * experts are cold).  Weight sets are numbered  [0, G) = united experts,  G + e = original expert e.
+ * R4 becomes   u_i = cold[e_i] ? gmap[e_i] : G + e_i   and everything after it runs over NS = G + E sets
+ * (counts [NS], offsets [NS+1]).  cold == NULL is full brownout over NS = G sets (oracle_route). */
+static int route_impl(const uint16_t *x, int T, int D, const uint16_t *Wr, const float *bias, int E, int K,
+                 const int32_t *gmap, int G, const int32_t *cold,
                  int32_t *expert_ids, int32_t *group_ids, float *gate_w, int32_t *n_slots,
                  int32_t *counts, int32_t *offsets, int32_t *row_token, int32_t *row_slot,
                  int32_t *slot_row, float *logits_out) {
     if (T < 0 || D < 8 || D % 8 != 0 || E < 1 || K < 1 || K > E || G < 1) return -1;
     for (int e = 0; e < E; ++e)
         if (gmap[e] < 0 || gmap[e] >= G) return -1;
+    const int NS = cold ? G + E : G;      /* number of weight sets the routing arrays range over */
 
 #pragma omp parallel for schedule(static)
     for (int t = 0; t < T; ++t) {
@@ -107,7 +115,7 @@ int oracle_route(const uint16_t *x, int T, int D, const uint16_t *Wr, const floa
         float *gw = gate_w + (size_t)t * K;
         int n = 0;
         for (int i = 0; i < K; ++i) {
-            int32_t u = gmap[eid[i]];
+            int32_t u = (!cold || cold[eid[i]]) ? gmap[eid[i]] : G + eid[i];
             int s;
             for (s = 0; s < n; ++s)
                 if (gid[s] == u) break;
@@ -130,14 +138,14 @@ int oracle_route(const uint16_t *x, int T, int D, const uint16_t *Wr, const floa
     }
 
     /* R6: histogram and exclusive scan */
-    for (int u = 0; u < G; ++u) counts[u] = 0;
+    for (int u = 0; u < NS; ++u) counts[u] = 0;
     for (int t = 0; t < T; ++t)
         for (int s = 0; s < K; ++s) {
             int32_t u = group_ids[(size_t)t * K + s];
             if (u >= 0) counts[u]++;
         }
     offsets[0] = 0;
-    for (int u = 0; u < G; ++u) offsets[u + 1] = offsets[u] + counts[u];
+    for (int u = 0; u < NS; ++u) offsets[u + 1] = offsets[u] + counts[u];
 
     /* R7: rows ordered by (group, token ascending) */
     for (size_t i = 0; i < (size_t)T * K; ++i) {
@@ -145,7 +153,7 @@ int oracle_route(const uint16_t *x, int T, int D, const uint16_t *Wr, const floa
         row_slot[i] = -1;
         slot_row[i] = -1;
     }
-    for (int u = 0; u < G; ++u) {
+    for (int u = 0; u < NS; ++u) {
         int32_t r = offsets[u];
         for (int t = 0; t < T; ++t)
             for (int s = 0; s < K; ++s)
@@ -155,6 +163,48 @@ int oracle_route(const uint16_t *x, int T, int D, const uint16_t *Wr, const floa
                     slot_row[(size_t)t * K + s] = r;
                     r++;
                 }
+    }
+    return 0;
+}
+
+int oracle_route(const uint16_t *x, int T, int D, const uint16_t *Wr, const float *bias, int E, int K,
+                 const int32_t *gmap, int G,
+                 int32_t *expert_ids, int32_t *group_ids, float *gate_w, int32_t *n_slots,
+                 int32_t *counts, int32_t *offsets, int32_t *row_token, int32_t *row_slot,
+                 int32_t *slot_row, float *logits_out) {
+    return route_impl(x, T, D, Wr, bias, E, K, gmap, G, NULL, expert_ids, group_ids, gate_w, n_slots, counts,
+                      offsets, row_token, row_slot, slot_row, logits_out);
+}
+
+/* cold [E]: non-zero = cold expert (served by its group's united expert).  counts [G+E], offsets [G+E+1]. */
+int oracle_route_partial(const uint16_t *x, int T, int D, const uint16_t *Wr, const float *bias, int E, int K,
+                         const int32_t *gmap, int G, const int32_t *cold,
+                         int32_t *expert_ids, int32_t *group_ids, float *gate_w, int32_t *n_slots,
+                         int32_t *counts, int32_t *offsets, int32_t *row_token, int32_t *row_slot,
+                         int32_t *slot_row, float *logits_out) {
+    if (!cold) return -1;
+    return route_impl(x, T, D, Wr, bias, E, K, gmap, G, cold, expert_ids, group_ids, gate_w, n_slots, counts,
+                      offsets, row_token, row_slot, slot_row, logits_out);
+}
+
+/* United-weight initialisation ("The united expert is initialized as the parameter average of member
+ * experts"; the same average is the convex target of Eq. 5 with uniform weights):
+ *   Wu[u, i] = (1 / |G_u|) * sum_{e : gmap[e] == u} W[e, i]      in fp64, one plain sum in ascending e.
+ * W: [E, n] bf16 (uint16 storage), out: [G, n] fp64; an empty group gives zeros.  Returns 0 or -1. */
+int oracle_unite_weights(const uint16_t *W, int E, long long n, const int32_t *gmap, int G, double *out) {
+    if (E < 1 || G < 1 || n < 0) return -1;
+    for (int e = 0; e < E; ++e)
+        if (gmap[e] < 0 || gmap[e] >= G) return -1;
+#pragma omp parallel for schedule(static)
+    for (int u = 0; u < G; ++u) {
+        int members = 0;
+        for (int e = 0; e < E; ++e) members += (gmap[e] == u);
+        for (long long i = 0; i < n; ++i) {
+            double acc = 0.0;
+            for (int e = 0; e < E; ++e)
+                if (gmap[e] == u) acc += (double)bf16_to_f32(W[(size_t)e * n + i]);
+            out[(size_t)u * n + i] = members ? acc / (double)members : 0.0;
+        }
     }
     return 0;
 }

@@ -42,6 +42,8 @@ def _load():
         _lib = ctypes.CDLL(_LIB)
         _lib.oracle_canon_dot.restype = ctypes.c_float
         _lib.oracle_route.restype = ctypes.c_int
+        _lib.oracle_route_partial.restype = ctypes.c_int
+        _lib.oracle_unite_weights.restype = ctypes.c_int
         _lib.oracle_moe_forward.restype = ctypes.c_int
     return _lib
 
@@ -63,11 +65,14 @@ def canon_dot(x_bits: np.ndarray, w_bits: np.ndarray) -> float:
     return float(_load().oracle_canon_dot(_p(x_bits), _p(w_bits), ctypes.c_int(x_bits.shape[0])))
 
 
-def route(x, W_router, router_bias, K: int, group_map, G: int, want_logits: bool = False) -> SimpleNamespace:
+def route(x, W_router, router_bias, K: int, group_map, G: int, want_logits: bool = False,
+          cold_mask=None) -> SimpleNamespace:
     """R1-R7 (PAPER.md:42 gate + top-K; Eq. 2 group map; readings A1-A7).
 
     x [T,D] uint16, W_router [E,D] uint16, router_bias [E] float32 or None, group_map [E] int32.
-    Returns the routing arrays of SURVEY.md 8(b) as numpy arrays.
+    cold_mask [E] (non-zero = cold) switches to partial brownout: hot experts keep
+    their own weights, numbered as weight sets G + e, and the routing arrays range over G + E sets
+    (returned as r.G).  Returns the routing arrays of SURVEY.md 8(b) as numpy arrays.
     """
     x, W_router = _u16(x), _u16(W_router)
     T, D = x.shape
@@ -76,25 +81,45 @@ def route(x, W_router, router_bias, K: int, group_map, G: int, want_logits: bool
     gmap = np.ascontiguousarray(group_map, dtype=np.int32)
     assert gmap.shape == (E,)
     bias = None if router_bias is None else np.ascontiguousarray(router_bias, dtype=np.float32)
-    r = SimpleNamespace(T=T, E=E, K=K, G=G)
+    cold = None if cold_mask is None else np.ascontiguousarray(cold_mask, dtype=np.int32)
+    NS = G if cold is None else G + E
+    r = SimpleNamespace(T=T, E=E, K=K, G=NS, G_united=G)
     r.expert_ids = np.empty((T, K), np.int32)
     r.group_ids = np.empty((T, K), np.int32)
     r.gate_w = np.empty((T, K), np.float32)
     r.n_slots = np.empty((T,), np.int32)
-    r.counts = np.empty((G,), np.int32)
-    r.offsets = np.empty((G + 1,), np.int32)
+    r.counts = np.empty((NS,), np.int32)
+    r.offsets = np.empty((NS + 1,), np.int32)
     r.row_token = np.empty((T * K,), np.int32)
     r.row_slot = np.empty((T * K,), np.int32)
     r.slot_row = np.empty((T, K), np.int32)
     r.logits = np.empty((T, E), np.float32) if want_logits else None
-    rc = _load().oracle_route(_p(x), T, D, _p(W_router), _p(bias), E, K, _p(gmap), G,
-                              _p(r.expert_ids), _p(r.group_ids), _p(r.gate_w), _p(r.n_slots),
-                              _p(r.counts), _p(r.offsets), _p(r.row_token), _p(r.row_slot),
-                              _p(r.slot_row), _p(r.logits))
+    args = [_p(x), T, D, _p(W_router), _p(bias), E, K, _p(gmap), G]
+    outs = [_p(r.expert_ids), _p(r.group_ids), _p(r.gate_w), _p(r.n_slots), _p(r.counts), _p(r.offsets),
+            _p(r.row_token), _p(r.row_slot), _p(r.slot_row), _p(r.logits)]
+    if cold is None:
+        rc = _load().oracle_route(*args, *outs)
+    else:
+        assert cold.shape == (E,)
+        rc = _load().oracle_route_partial(*args, _p(cold), *outs)
     if rc != 0:
         raise ValueError("oracle_route: bad shape or group_map entry outside [0,G)")
-    r.A = int(r.offsets[G])
+    r.A = int(r.offsets[NS])
     return r
+
+
+def unite_weights(W, group_map, G: int) -> np.ndarray:
+    """Parameter average of the member experts of every group, fp64.
+    W [E, ...] uint16 (bf16 storage) -> [G, ...] float64."""
+    W = _u16(W)
+    E = W.shape[0]
+    n = int(np.prod(W.shape[1:]))
+    gmap = np.ascontiguousarray(group_map, dtype=np.int32)
+    out = np.empty((G,) + W.shape[1:], np.float64)
+    rc = _load().oracle_unite_weights(_p(W), E, ctypes.c_longlong(n), _p(gmap), G, _p(out))
+    if rc != 0:
+        raise ValueError("oracle_unite_weights: bad arguments")
+    return out
 
 
 def moe_forward(x, routing, W1, W3, W2, S: int = 0, sel_tokens=None) -> np.ndarray:

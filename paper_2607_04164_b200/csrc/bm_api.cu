@@ -145,7 +145,14 @@ int bm_moe_forward_path(const bm_bf16 *x, int T, int D, const bm_routing *routin
     if (workspace_bytes < w.total) return BM_ERR_WORKSPACE;
     if (device_ok() != 1) return BM_ERR_CUDA;
 
-    if (path == BM_PATH_AUTO) path = (T <= BM_DECODE_MAX_T) ? BM_PATH_DECODE : BM_PATH_PREFILL;
+    if (path == BM_PATH_AUTO) {
+        // decode (swap-AB weight streaming) for small batches: always up to 64 tokens, and up to
+        // BM_DECODE_MAX_T tokens while a group expects at most ~24 rows (measured crossover at T = 256:
+        // 17 rows/group -> decode 6% faster, 33 rows/group -> prefill tiles 5% faster)
+        const int max_t = tune_int("BM_DECODE_MAX_T", BM_DECODE_MAX_T);
+        const bool few_rows = (long long)T * K <= 24LL * G;
+        path = (T <= 64 || (T <= max_t && few_rows)) ? BM_PATH_DECODE : BM_PATH_PREFILL;
+    }
 
     uint8_t *ws = static_cast<uint8_t *>(workspace);
     ForwardArgs a{};
