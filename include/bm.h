@@ -103,6 +103,34 @@ int bm_route(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, const floa
              size_t workspace_bytes, bm_stream_t stream);
 
 /*
+ * bm_route_partial -- partial brownout.  Cite: "partial-brownout delegates only
+ * cold expert tokens to united experts based on a configurable threshold"; P:172 the original gate still
+ * determines the activated experts; "the grouping map determines which united expert handles tokens
+ * originally routed to each cold expert".  Which experts are cold is the caller's decision (A9: the
+ * paper's threshold criterion lives in its reference [7]).
+ *   cold_mask  [E] i32: non-zero = cold (served by united expert group_map[e]); zero = hot (keeps its own weights)
+ * Weight sets are numbered  [0, G) = united experts,  G + e = original expert e, so the routing arrays range over
+ * G + E sets: routing->G is set to G + E, counts holds G + E and offsets G + E + 1 entries (G + E <= BM_MAX_G), and
+ * the workspace must be sized with bm_workspace_bytes(..., G + E, S).  The forward pass is bm_moe_forward on weights
+ * stacked as [united (G) ; original (E) ; shared (S)]; sets that receive no row cost nothing.  All cold = full
+ * brownout (same arrays as bm_route), all hot = zero brownout.  Everything else as bm_route.
+ */
+int bm_route_partial(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, const float *router_bias, int E,
+                     int K, const int32_t *group_map, int G, const int32_t *cold_mask, bm_routing *routing,
+                     void *workspace, size_t workspace_bytes, bm_stream_t stream);
+
+/*
+ * bm_unite_weights -- united-weight construction.  Cite: "The united expert is
+ * initialized as the parameter average of member experts"; group map: P:118-122 (Eq. 2).
+ *   out[u, i] = (1 / |G_u|) * sum_{e : group_map[e] == u} W[e, i],   members added in ascending e in fp32,
+ *   rounded once to bf16; an empty group gives zeros.
+ *   W    [E, n] bf16 (one expert matrix flattened: n = F*D), n % 8 == 0
+ *   out  [G, n] bf16, overwritten.  Call it once per matrix kind (W1, W3, W2).
+ */
+int bm_unite_weights(const bm_bf16 *W, int E, size_t n, const int32_t *group_map, int G, bm_bf16 *out,
+                     bm_stream_t stream);
+
+/*
  * bm_moe_forward -- steps 9-13: out[t] = sum_s gate_w[t,s] * FFN_{group_ids[t,s]}(x_t) + sum_{j<S} FFN_{G+j}(x_t)
  * with FFN_u(x) = W2[u] . ( SiLU(W1[u] x) * (W3[u] x) )   (P:42 with united experts P:46; SwiGLU: A3).
  * bf16 operands, fp32 accumulation (tensor cores), the intermediate h is rounded to bf16 (A12).

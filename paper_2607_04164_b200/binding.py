@@ -19,7 +19,7 @@ BM_DEV_BAD_GROUP_MAP, BM_DEV_NONFINITE_LOGIT, BM_DEV_BAD_ROUTING = 1, 2, 4
 BM_MAX_E, BM_MAX_K, BM_MAX_G = 512, 16, 512
 BM_DECODE_MAX_T = 256
 
-EXPORTS = ["bm_workspace_bytes", "bm_route", "bm_moe_forward", "bm_moe_forward_path", "bm_moe_layer_host",
+EXPORTS = ["bm_workspace_bytes", "bm_route", "bm_route_partial", "bm_unite_weights", "bm_moe_forward", "bm_moe_forward_path", "bm_moe_layer_host",
            "bm_device_status", "bm_launch_count", "bm_status_string", "bm_profile_enable", "bm_profile_read"]
 KERNELS = {"router": 1, "permute": 2, "prep": 3, "gemm1": 4, "gemm2": 5, "finalize": 6}
 
@@ -51,6 +51,11 @@ def lib() -> ctypes.CDLL:
         L.bm_route.restype = c_int
         L.bm_route.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_int, c_int, c_void_p, c_int,
                                POINTER(BmRouting), c_void_p, c_size_t, c_void_p]
+        L.bm_route_partial.restype = c_int
+        L.bm_route_partial.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_int, c_int, c_void_p, c_int,
+                                       c_void_p, POINTER(BmRouting), c_void_p, c_size_t, c_void_p]
+        L.bm_unite_weights.restype = c_int
+        L.bm_unite_weights.argtypes = [c_void_p, c_int, c_size_t, c_void_p, c_int, c_void_p, c_void_p]
         L.bm_moe_forward.restype = c_int
         L.bm_moe_forward.argtypes = [c_void_p, c_int, c_int, POINTER(BmRouting), c_void_p, c_void_p, c_void_p,
                                      c_int, c_int, c_void_p, c_void_p, c_size_t, c_void_p]
@@ -142,6 +147,32 @@ def bm_route(x, W_router, router_bias, K: int, group_map, G: int, routing: Routi
     if rc != BM_OK:
         raise BmError(rc, "bm_route")
     return routing
+
+
+def bm_route_partial(x, W_router, router_bias, K: int, group_map, G: int, cold_mask, routing: Routing, workspace,
+                     stream=None):
+    """Partial brownout routing (include/bm.h: bm_route_partial).  cold_mask [E] i32; `routing` must have been
+    allocated for G + E weight sets (Routing(T, K, G + E)) and the workspace sized for G + E."""
+    T, D = x.shape
+    E = W_router.shape[0]
+    rc = lib().bm_route_partial(_ptr(x), T, D, _ptr(W_router), _ptr(router_bias), E, K, _ptr(group_map), G,
+                                _ptr(cold_mask), ctypes.byref(routing.c), _ptr(workspace), workspace.numel(),
+                                _stream(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_route_partial")
+    return routing
+
+
+def bm_unite_weights(W, group_map, G: int, out=None, stream=None):
+    """Parameter average of member experts (include/bm.h: bm_unite_weights).  W [E, ...] bf16 -> [G, ...] bf16."""
+    E = W.shape[0]
+    n = W[0].numel()
+    if out is None:
+        out = torch.empty((G,) + tuple(W.shape[1:]), dtype=W.dtype, device=W.device)
+    rc = lib().bm_unite_weights(_ptr(W), E, n, _ptr(group_map), G, _ptr(out), _stream(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_unite_weights")
+    return out
 
 
 def bm_moe_forward(x, routing: Routing, W1, W3, W2, out, workspace, S: int = 0, path: int = BM_PATH_AUTO,

@@ -86,20 +86,24 @@ size_t bm_workspace_bytes(int T_max, int D, int F, int E, int K, int G, int S) {
     return workspace_layout(T_max, D, F, K, G, S).total;
 }
 
-int bm_route(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, const float *router_bias, int E, int K,
-             const int32_t *group_map, int G, bm_routing *routing, void *workspace, size_t workspace_bytes,
-             bm_stream_t stream) {
+// shared body of bm_route (cold_mask == nullptr) and bm_route_partial
+static int route_common(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, const float *router_bias, int E,
+                        int K, const int32_t *group_map, int G, const int32_t *cold_mask, bool partial,
+                        bm_routing *routing, void *workspace, size_t workspace_bytes, bm_stream_t stream) {
     if (!routing) return BM_ERR_NULL;
     int rc = check_shapes(T, D, 8, E, K, G, 0, false);
     if (rc != BM_OK) return rc;
-    routing->T = T; routing->E = E; routing->K = K; routing->G = G;
+    const int NS = partial ? G + E : G;            // weight sets the routing arrays range over
+    if (NS > BM_MAX_G) return BM_ERR_SHAPE;
+    routing->T = T; routing->E = E; routing->K = K; routing->G = NS;
     if (!W_router || !group_map || !workspace || !routing->counts || !routing->offsets) return BM_ERR_NULL;
+    if (partial && !cold_mask) return BM_ERR_NULL;
     if (T > 0 && (!x || !routing->expert_ids || !routing->group_ids || !routing->gate_w || !routing->n_slots ||
                   !routing->row_token || !routing->row_slot || !routing->slot_row))
         return BM_ERR_NULL;
     if (!aligned16(x) || !aligned16(W_router) || !aligned16(workspace)) return BM_ERR_ALIGN;
     // only the routing part of the workspace is needed here (F = 8, S = 0 gives its lower bound)
-    const Workspace full = workspace_layout(T, D, 8, K, G, 0);
+    const Workspace full = workspace_layout(T, D, 8, K, NS, 0);
     if (workspace_bytes < full.sched) return BM_ERR_WORKSPACE;
     if (device_ok() != 1) return BM_ERR_CUDA;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
@@ -107,21 +111,47 @@ int bm_route(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, const floa
     int32_t *status = reinterpret_cast<int32_t *>(ws + full.status);
     if (T == 0) {
         // empty batch: counts = 0, offsets = 0
-        if (cudaMemsetAsync(routing->counts, 0, sizeof(int32_t) * G, st) != cudaSuccess ||
-            cudaMemsetAsync(routing->offsets, 0, sizeof(int32_t) * (G + 1), st) != cudaSuccess)
+        if (cudaMemsetAsync(routing->counts, 0, sizeof(int32_t) * NS, st) != cudaSuccess ||
+            cudaMemsetAsync(routing->offsets, 0, sizeof(int32_t) * (NS + 1), st) != cudaSuccess)
             return BM_ERR_CUDA;
         return BM_OK;
     }
     profile_begin(BM_KERNEL_ROUTER, st);
-    if (launch_router(x, T, D, W_router, router_bias, E, K, group_map, G, *routing, status, st) != cudaSuccess)
+    if (launch_router(x, T, D, W_router, router_bias, E, K, GroupMap{group_map, partial ? cold_mask : nullptr, G},
+                      *routing, status, st) != cudaSuccess)
         return BM_ERR_CUDA;
     profile_end(BM_KERNEL_ROUTER, st);
     profile_begin(BM_KERNEL_PERMUTE, st);
-    if (launch_permute(T, K, G, *routing, reinterpret_cast<int32_t *>(ws + full.block_hist), status, st) !=
+    if (launch_permute(T, K, NS, *routing, reinterpret_cast<int32_t *>(ws + full.block_hist), status, st) !=
         cudaSuccess)
         return BM_ERR_CUDA;
     profile_end(BM_KERNEL_PERMUTE, st);
     return BM_OK;
+}
+
+int bm_route(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, const float *router_bias, int E, int K,
+             const int32_t *group_map, int G, bm_routing *routing, void *workspace, size_t workspace_bytes,
+             bm_stream_t stream) {
+    return route_common(x, T, D, W_router, router_bias, E, K, group_map, G, nullptr, false, routing, workspace,
+                        workspace_bytes, stream);
+}
+
+int bm_route_partial(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, const float *router_bias, int E, int K,
+                     const int32_t *group_map, int G, const int32_t *cold_mask, bm_routing *routing, void *workspace,
+                     size_t workspace_bytes, bm_stream_t stream) {
+    return route_common(x, T, D, W_router, router_bias, E, K, group_map, G, cold_mask, true, routing, workspace,
+                        workspace_bytes, stream);
+}
+
+int bm_unite_weights(const bm_bf16 *W, int E, size_t n, const int32_t *group_map, int G, bm_bf16 *out,
+                     bm_stream_t stream) {
+    if (E < 1 || E > BM_MAX_E || G < 1 || G > BM_MAX_G || n % 8 != 0) return BM_ERR_SHAPE;
+    if (n == 0) return BM_OK;
+    if (!W || !group_map || !out) return BM_ERR_NULL;
+    if (!aligned16(W) || !aligned16(out)) return BM_ERR_ALIGN;
+    if (device_ok() != 1) return BM_ERR_CUDA;
+    return launch_unite(W, E, n, group_map, G, out, reinterpret_cast<cudaStream_t>(stream)) == cudaSuccess
+               ? BM_OK : BM_ERR_CUDA;
 }
 
 int bm_moe_forward_path(const bm_bf16 *x, int T, int D, const bm_routing *routing, const bm_bf16 *W1,

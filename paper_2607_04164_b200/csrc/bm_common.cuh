@@ -85,9 +85,16 @@ cudaError_t launch_kernel(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t 
 // ---------------------------------------------------------------------------------------------
 // Internal kernel launchers (defined in the .cu files, called from bm_api.cu)
 // ---------------------------------------------------------------------------------------------
+// group map of a routing call: gmap [E] with values in [0,G); cold [E] or nullptr.  nullptr = full brownout
+// (every expert e -> set gmap[e]); otherwise partial brownout: cold[e] != 0 -> set gmap[e], else set G + e.
+struct GroupMap {
+    const int32_t *gmap;
+    const int32_t *cold;
+    int G;
+};
+
 cudaError_t launch_router(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const float *bias, int E,
-                          int K, const int32_t *gmap, int G, const bm_routing &r, int32_t *status,
-                          cudaStream_t stream);
+                          int K, GroupMap gm, const bm_routing &r, int32_t *status, cudaStream_t stream);
 
 cudaError_t launch_permute(int T, int K, int G, const bm_routing &r, int32_t *block_hist, int32_t *status,
                            cudaStream_t stream);
@@ -106,6 +113,9 @@ struct ForwardArgs {
     float *out_acc;
     bm_bf16 *y;
 };
+
+cudaError_t launch_unite(const bm_bf16 *W, int E, size_t n, const int32_t *gmap, int G, bm_bf16 *out,
+                         cudaStream_t stream);
 
 cudaError_t launch_forward_simt(const ForwardArgs &a, cudaStream_t stream);
 cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t stream);

@@ -28,7 +28,7 @@ constexpr int kWarps = 8;
 // lane-parallel; only the two rank-ordered fp32 sums (softmax denominator, merged gate weights) are
 // sequential, as a chain of K shuffles.
 __device__ __forceinline__ void select_and_write(const float *l, int t, int lane, int E, int K,
-                                                 const int32_t *__restrict__ gmap, int G,
+                                                 GroupMap gm,
                                                  int32_t *__restrict__ expert_ids, int32_t *__restrict__ group_ids,
                                                  float *__restrict__ gate_w, int32_t *__restrict__ n_slots,
                                                  int32_t *__restrict__ status) {
@@ -68,8 +68,9 @@ __device__ __forceinline__ void select_and_write(const float *l, int t, int lane
     int u = -1 - lane;                  // inactive lanes: distinct negative keys, never matched
     bool bad_map = false;
     if (active) {
-        u = gmap[my_e];
-        if (u < 0 || u >= G) { bad_map = true; u = u < 0 ? 0 : G - 1; }
+        u = gm.gmap[my_e];
+        if (u < 0 || u >= gm.G) { bad_map = true; u = u < 0 ? 0 : gm.G - 1; }
+        if (gm.cold && gm.cold[my_e] == 0) u = gm.G + my_e;        // partial brownout: a hot expert keeps its own set
     }
     // ---- R5: dedup in rank order; the first occurrence keeps the slot, weights added in rank order -----
     const unsigned peers = __match_any_sync(kFullMask, u);            // lanes (ranks) mapped to the same group
@@ -96,7 +97,7 @@ __device__ __forceinline__ void select_and_write(const float *l, int t, int lane
 template <int TOK, int ET>
 __global__ void __launch_bounds__(kWarps * 32)
 router_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *__restrict__ Wr,
-              const float *__restrict__ bias, int E, int K, const int32_t *__restrict__ gmap, int G,
+              const float *__restrict__ bias, int E, int K, GroupMap gm,
               int WT, int WE, int32_t *__restrict__ expert_ids, int32_t *__restrict__ group_ids,
               float *__restrict__ gate_w, int32_t *__restrict__ n_slots, int32_t *__restrict__ status) {
     extern __shared__ float s_logits[];   // [TB][E], TB = WT * TOK
@@ -170,7 +171,7 @@ router_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *__rest
     for (int tl = warp; tl < TB; tl += kWarps) {
         const int t = t_block + tl;
         if (t >= T) break;
-        select_and_write(s_logits + tl * E, t, lane, E, K, gmap, G, expert_ids, group_ids, gate_w, n_slots, status);
+        select_and_write(s_logits + tl * E, t, lane, E, K, gm, expert_ids, group_ids, gate_w, n_slots, status);
     }
 }
 
@@ -195,10 +196,6 @@ __device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gsrc, uint3
                  ::"r"(ptx::smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(ptx::smem_u32(bar))
                  : "memory");
 }
-__device__ __forceinline__ void bar_sync_named(int id, int nthreads) {
-    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
-}
-
 // Sum of the 32 lane partials of each of this lane's 32 accumulators: the xor butterfly (16, 8, 4, 2, 1)
 // of reading A1, evaluated for all 32 accumulators at once.  At the step with offset o every lane hands
 // over the half of its values whose index bit o differs from its own lane bit o, so a step costs n/2
@@ -220,7 +217,7 @@ __device__ __forceinline__ void butterfly32(float (&v)[32], int lane) {
 
 __global__ void __launch_bounds__(kTpMaxThreads, 1)
 router_tp_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *__restrict__ Wr,
-                 const float *__restrict__ bias, int E, int K, const int32_t *__restrict__ gmap, int G,
+                 const float *__restrict__ bias, int E, int K, GroupMap gm,
                  int WT, int WE, int n_blocks, int32_t *__restrict__ expert_ids, int32_t *__restrict__ group_ids,
                  float *__restrict__ gate_w, int32_t *__restrict__ n_slots, int32_t *__restrict__ status) {
     extern __shared__ __align__(128) uint8_t tp_smem[];
@@ -335,14 +332,14 @@ router_tp_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *__r
         for (int tl = warp; tl < TB; tl += nw) {
             const int t = t_block + tl;
             if (t >= T) break;
-            select_and_write(s_logits + tl * E, t, lane, E, K, gmap, G, expert_ids, group_ids, gate_w, n_slots, status);
+            select_and_write(s_logits + tl * E, t, lane, E, K, gm, expert_ids, group_ids, gate_w, n_slots, status);
         }
         __syncthreads();                        // before the next block overwrites them
     }
 }
 
 cudaError_t launch_tp(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const float *bias, int E, int K,
-                      const int32_t *gmap, int G, const bm_routing &r, int32_t *status, cudaStream_t stream) {
+                      GroupMap gm, const bm_routing &r, int32_t *status, cudaStream_t stream) {
     const int n_etiles = (E + 7) / 8;
     int WE = 1;
     while (WE < n_etiles && WE < 8) WE *= 2;
@@ -360,12 +357,12 @@ cudaError_t launch_tp(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const f
     const int n_blocks = (T + TB - 1) / TB;
     const int grid = n_blocks < num_sms() ? n_blocks : num_sms();
     return launch_kernel(router_tp_kernel, dim3(grid), dim3(ncw * 32), smem, stream, x, T, D, Wr, bias, E, K,
-                         gmap, G, WT, WE, n_blocks, r.expert_ids, r.group_ids, r.gate_w, r.n_slots, status);
+                         gm, WT, WE, n_blocks, r.expert_ids, r.group_ids, r.gate_w, r.n_slots, status);
 }
 
 template <int TOK, int ET>
 cudaError_t launch_cfg(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const float *bias, int E, int K,
-                       const int32_t *gmap, int G, int WT, int WE, const bm_routing &r, int32_t *status,
+                       GroupMap gm, int WT, int WE, const bm_routing &r, int32_t *status,
                        cudaStream_t stream) {
     const int TB = WT * TOK;
     const size_t smem = (size_t)TB * E * sizeof(float);
@@ -375,26 +372,26 @@ cudaError_t launch_cfg(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const 
         if (e != cudaSuccess) return e;
     }
     const int grid = (T + TB - 1) / TB;
-    return launch_kernel(kern, dim3(grid), dim3(kWarps * 32), smem, stream, x, T, D, Wr, bias, E, K, gmap, G, WT, WE,
+    return launch_kernel(kern, dim3(grid), dim3(kWarps * 32), smem, stream, x, T, D, Wr, bias, E, K, gm, WT, WE,
                          r.expert_ids, r.group_ids, r.gate_w, r.n_slots, status);
 }
 
 }  // namespace
 
 cudaError_t launch_router(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const float *bias, int E,
-                          int K, const int32_t *gmap, int G, const bm_routing &r, int32_t *status,
+                          int K, GroupMap gm, const bm_routing &r, int32_t *status,
                           cudaStream_t stream) {
     if (T >= tune_int("BM_ROUTER_TP_MIN_T", 512))   // throughput shape: operands staged through shared memory
-        return launch_tp(x, T, D, Wr, bias, E, K, gmap, G, r, status, stream);
+        return launch_tp(x, T, D, Wr, bias, E, K, gm, r, status, stream);
     // latency shape: one token per warp pass, warps split the experts
     if (E <= 8) {
         int WE = 1;
         while (WE * 2 <= E && WE < kWarps) WE *= 2;
-        return launch_cfg<1, 1>(x, T, D, Wr, bias, E, K, gmap, G, kWarps / WE, WE, r, status, stream);
+        return launch_cfg<1, 1>(x, T, D, Wr, bias, E, K, gm, kWarps / WE, WE, r, status, stream);
     }
     int tiles = (E + 7) / 8, WE = 1;
     while (WE * 2 <= tiles && WE < kWarps) WE *= 2;
-    return launch_cfg<1, 8>(x, T, D, Wr, bias, E, K, gmap, G, kWarps / WE, WE, r, status, stream);
+    return launch_cfg<1, 8>(x, T, D, Wr, bias, E, K, gm, kWarps / WE, WE, r, status, stream);
 }
 
 }  // namespace bm
