@@ -531,6 +531,88 @@ def run_sweep(args):
     print(json.dumps(res))
 
 
+def run_next(args):
+    """python bench.py --config next [--out FILE]: the SURVEY.md 8(f) rows that are built -- partial brownout
+    (tokens/s against the fraction of cold experts, Qwen-MoE-like shape of BJ:configs[4], G = 15) and the
+    united-weight parameter average (achieved GB/s).  One GPU; cold weights as in the sweep."""
+    from bm_inputs import make_cold_mask
+    torch.cuda.set_device(0)
+    import paper_2607_04164_b200 as bm
+    bm.lib()
+    peaks = load_peaks()
+    D, F, E, K, G = 2048, 1408, 60, 4, 15
+    NS = G + E
+    one = 3 * NS * F * D * 2
+    copies = max(1, int(-(-512e6 // one)))
+    gen = torch.Generator(device="cuda").manual_seed(1)
+    mk = lambda *sh: (torch.randn(*sh, generator=gen, device="cuda") * 0.02).to(torch.bfloat16)
+    W = [(mk(NS, F, D), mk(NS, F, D), mk(NS, D, F)) for _ in range(copies)]     # [united ; originals], timing only
+    rows = []
+    for T in (16, 256, 4096):
+        cfg = get_config(f"sweep_G{G}_T{T}_s1")
+        L = make_layer(cfg, 0, weights=False)
+        x, Wr, bias, gmap = L.x.cuda(), L.W_router.cuda(), L.router_bias.cuda(), L.group_map.cuda()
+        ws = bm.alloc_workspace(T, D, F, E, K, NS, 0)
+        r = bm.Routing(T, K, NS)
+        out = torch.empty((T, D), dtype=torch.bfloat16, device="cuda")
+        for frac in (0.0, 0.25, 0.5, 0.75, 1.0):
+            cold = make_cold_mask(E, frac, 0).cuda()
+            state = {"i": 0}
+
+            def step():
+                w1, w3, w2 = W[state["i"] % copies]
+                state["i"] += 1
+                bm.bm_route_partial(x, Wr, bias, K, gmap, G, cold, r, ws)
+                bm.bm_moe_forward(x, r, w1, w3, w2, out, ws)
+
+            steps = (200 if T <= 256 else 40) // copies * copies
+            for _ in range(max(3, copies)):
+                step()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(steps):
+                step()
+            e1.record()
+            torch.cuda.synchronize()
+            t = e0.elapsed_time(e1) / 1e3 / steps
+            counts = r.counts.cpu().numpy()
+            A, act = int(counts.sum()), int((counts > 0).sum())
+            flops, nbytes, t_flop, t_hbm = roofline_times(cfg, A, act, peaks)
+            rows.append(dict(T=T, frac_cold=frac, A=A, sets_active=act, us=t * 1e6, tokens_per_s=T / t,
+                             t_hbm_us=t_hbm * 1e6, t_flop_us=t_flop * 1e6, roofline_frac=max(t_hbm, t_flop) / t,
+                             device_status=bm.bm_device_status(ws)))
+            sys.stderr.write(f"partial T={T:5d} cold={frac:4.2f} A={A:6d} sets={act:3d} {t*1e6:9.1f} us  "
+                             f"roof {max(t_hbm, t_flop)*1e6:8.1f} us frac {rows[-1]['roofline_frac']:.3f}\n")
+    # united-weight construction: E = 60 -> G = 15 on one matrix kind
+    Wsrc = mk(E, F, D)
+    gm = make_layer(get_config(f"sweep_G{G}_T16_s1"), 0, weights=False).group_map.cuda()
+    dst = torch.empty((G, F, D), dtype=torch.bfloat16, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    ts = []
+    for i in range(13):
+        flush.zero_()                                    # 256 MB > L2: the sources come from HBM
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        bm.bm_unite_weights(Wsrc, gm, G, out=dst)
+        e1.record()
+        torch.cuda.synchronize()
+        if i >= 3:
+            ts.append(e0.elapsed_time(e1) / 1e3)
+    tu = statistics.median(ts)
+    ub = (E + G) * F * D * 2
+    unite = dict(E=E, G=G, n=F * D, us=tu * 1e6, alg_bytes=ub, achieved_gbs=ub / tu / 1e9,
+                 frac_of_hbm=ub / tu / 1e9 / peaks["hbm_gbs"], l2="flushed with a 256 MB write before every launch")
+    sys.stderr.write(f"unite_weights E={E} G={G}: {tu*1e6:.1f} us, {unite['achieved_gbs']:.0f} GB/s "
+                     f"({unite['frac_of_hbm']:.2f} of measured HBM)\n")
+    res = dict(metric=METRIC, unit=UNIT, workload="SURVEY 8(f): partial brownout at D=2048 F=1408 E=60 top-4 G=15 zipf 1.0; "
+               "united-weight average", peaks=peaks, weight_copies=copies, partial=rows, unite=unite)
+    if args.out:
+        with open(args.out, "w") as fh:
+            json.dump(res, fh, indent=1)
+    print(json.dumps(res))
+
+
 # ---------------------------------------------------------------------------------------------------
 # reference arm: the oracle on the host cores (tier framing (4))
 # ---------------------------------------------------------------------------------------------------
@@ -586,7 +668,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="decode",
-                    help="one of %s, 'sweep' (all 60 points of configs[4]) or one sweep point name such as "
+                    help="one of %s, 'sweep' (all 60 points of configs[4]), 'next' (SURVEY 8(f) rows) or one sweep point name such as "
                          "sweep_G8_T256_s1" % sorted(CONFIGS))
     ap.add_argument("--sweep-filter", default="", help="comma-separated name parts, e.g. G8,T16 (with --config sweep)")
     ap.add_argument("--out", default="", help="also write the sweep result to this file")
@@ -600,6 +682,8 @@ def main():
             raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
         if args.config == "sweep":
             run_sweep(args)
+        elif args.config == "next":
+            run_next(args)
         else:
             run_ours(args)
 

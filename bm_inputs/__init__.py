@@ -13,6 +13,7 @@ from .configs import LayerConfig, CONFIGS, sweep_points, get_config
 from .generate import (
     make_group_map,
     make_router_bias,
+    make_cold_mask,
     make_layer,
     identity_variant,
     bf16_bits,
@@ -25,6 +26,7 @@ __all__ = [
     "get_config",
     "make_group_map",
     "make_router_bias",
+    "make_cold_mask",
     "make_layer",
     "identity_variant",
     "bf16_bits",

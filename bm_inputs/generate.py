@@ -78,6 +78,15 @@ def make_router_bias(E: int, D: int, zipf_s: float, seed: int = 0):
     return (-zipf_s * SKEW_C * sigma * torch.log(rank.to(torch.float64))).to(torch.float32)
 
 
+def make_cold_mask(E: int, frac_cold: float, seed: int = 0) -> torch.Tensor:
+    """Partial-brownout input: i32 [E], 1 = cold.  The round(frac_cold * E) experts that the
+    skew recipe above loads least (largest Zipf rank) are cold -- the paper's cold experts are the rarely
+    activated ones; its threshold criterion itself is in its reference [7] (A9)."""
+    rank = torch.randperm(E, generator=_gen(seed, TID_RANK)) + 1
+    n_cold = int(round(frac_cold * E))
+    return (rank > E - n_cold).to(torch.int32)
+
+
 def _randn_bf16(shape, std: float, gen: torch.Generator) -> torch.Tensor:
     """N(0, std) sampled in fp32, cast to bf16; the leading dim is drawn slice by slice to bound memory."""
     out = torch.empty(shape, dtype=torch.bfloat16)
