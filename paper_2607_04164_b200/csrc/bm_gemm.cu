@@ -486,24 +486,54 @@ prep_kernel(const bm_bf16 *__restrict__ x, int T, int D, int K, int G, int S,
             float *__restrict__ out_acc, int decode, int32_t *__restrict__ status) {
     grid_dep_wait();
     grid_dep_launch();
-    if (blockIdx.x == 0 && threadIdx.x == 0) {
-        int n_seg = 0, chunks = 0;
-        bool bad = false;
-        for (int u = 0; u < G + S; ++u) {
-            const int rows = u < G ? counts[u] : T;
-            if (u < G && (rows < 0 || offsets[u] < 0 || offsets[u] + rows > T * K)) { bad = true; continue; }
-            if (rows <= 0) continue;
-            sched[kSchedSegU + n_seg] = u;
-            sched[kSchedChunk0 + n_seg] = chunks;
-            sched[kSchedRows + n_seg] = rows;
-            sched[kSchedOff + n_seg] = u < G ? offsets[u] : 0;
-            chunks += (rows + kChunkRows - 1) / kChunkRows;
-            ++n_seg;
+    if (blockIdx.x == 0) {
+        // schedule: compact the non-empty segments and prefix-sum their chunk counts.  All rows are fetched in
+        // parallel (one global-memory latency), then warp 0 scans them 32 at a time.
+        __shared__ int s_rows[kMaxSeg], s_off[kMaxSeg];
+        __shared__ int s_bad;
+        const int n = G + S;
+        if (threadIdx.x == 0) s_bad = 0;
+        __syncthreads();
+        for (int u = threadIdx.x; u < n; u += blockDim.x) {
+            int rows = u < G ? counts[u] : T;
+            const int off = u < G ? offsets[u] : 0;
+            if (u < G && (rows < 0 || off < 0 || off + rows > T * K)) { s_bad = 1; rows = 0; }
+            s_rows[u] = rows;
+            s_off[u] = off;
         }
-        sched[kSchedChunk0 + n_seg] = chunks;
-        sched[0] = n_seg;
-        sched[1] = chunks;
-        if (bad) atomicOr(status, BM_DEV_BAD_ROUTING);
+        __syncthreads();
+        if (threadIdx.x < 32) {
+            const int lane = threadIdx.x;
+            int seg_base = 0, chunk_base = 0;
+            for (int u0 = 0; u0 < n; u0 += 32) {
+                const int u = u0 + lane;
+                const int rows = u < n ? s_rows[u] : 0;
+                const bool ne = rows > 0;
+                const int ch = ne ? (rows + kChunkRows - 1) / kChunkRows : 0;
+                const unsigned m = __ballot_sync(kFullMask, ne);
+                const int seg = seg_base + __popc(m & ((1u << lane) - 1u));
+                int inc = ch;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int v = __shfl_up_sync(kFullMask, inc, o);
+                    if (lane >= o) inc += v;
+                }
+                if (ne) {
+                    sched[kSchedSegU + seg] = u;
+                    sched[kSchedChunk0 + seg] = chunk_base + inc - ch;
+                    sched[kSchedRows + seg] = rows;
+                    sched[kSchedOff + seg] = s_off[u];
+                }
+                seg_base += __popc(m);
+                chunk_base += __shfl_sync(kFullMask, inc, 31);
+            }
+            if (lane == 0) {
+                sched[kSchedChunk0 + seg_base] = chunk_base;
+                sched[0] = seg_base;
+                sched[1] = chunk_base;
+                if (s_bad) atomicOr(status, BM_DEV_BAD_ROUTING);
+            }
+        }
     }
     // zero out_acc (decode path only: the prefill path combines plain y rows)
     const size_t n4 = decode ? (size_t)T * D / 4 : 0;

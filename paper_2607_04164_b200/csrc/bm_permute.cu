@@ -29,7 +29,7 @@ constexpr int kItemsPerWarp = kPermItemsPerBlock / kWarps;   // 256
 // Count the items of this warp's slice into whist_w[0..G) (shared memory, zeroed by the caller).
 __device__ __forceinline__ void warp_histogram(const int32_t *__restrict__ group_ids, long long items,
                                                long long first, int *whist_w, int lane) {
-    for (int r = 0; r < kItemsPerWarp; r += 32) {
+    for (int r = 0; r < kItemsPerWarp && first + r < items; r += 32) {      // warp-uniform bound
         const long long i = first + r + lane;
         const int key = (i < items) ? group_ids[i] : -1;
         const unsigned peers = __match_any_sync(kFullMask, key);
@@ -43,7 +43,7 @@ __device__ __forceinline__ void warp_permute(const int32_t *__restrict__ group_i
                                              long long first, int K, int *wbase_w, int lane, int A,
                                              int32_t *__restrict__ row_token, int32_t *__restrict__ row_slot,
                                              int32_t *__restrict__ slot_row) {
-    for (int r = 0; r < kItemsPerWarp; r += 32) {
+    for (int r = 0; r < kItemsPerWarp && first + r < items; r += 32) {      // warp-uniform bound
         const long long i = first + r + lane;
         const int key = (i < items) ? group_ids[i] : -1;
         const unsigned peers = __match_any_sync(kFullMask, key);

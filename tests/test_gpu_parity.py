@@ -36,6 +36,7 @@ ROUTE_SHAPES = [
     (3001, 264, 13, 5, 7, 1.0),        # T >= 2048: throughput router; ragged D (264 = 256 + 8), odd E
     (4096, 2048, 60, 4, 8, 1.0),
     (300, 64, 200, 16, 97, 0.0),       # many experts, K = BM_MAX_K
+    (700, 72, 200, 16, 97, 1.0),       # the same through the staged throughput router: 4 expert passes, ragged slab
     (2500, 128, 512, 3, 512, 0.0),     # E = BM_MAX_E, G = BM_MAX_G
 ]
 
@@ -205,7 +206,18 @@ def test_finegrained_config_full_size_sampled():
     _sampled_parity(CONFIGS["finegrained"], 24)                 # BJ:configs[3], shared experts, uneven groups
 
 
-@pytest.mark.parametrize("name", ["sweep_G8_T1_s1", "sweep_G15_T16_s2", "sweep_G60_T256_s0", "sweep_G30_T4096_s1"])
+@pytest.mark.parametrize("name", ["sweep_G8_T1_s1", "sweep_G15_T16_s2", "sweep_G60_T256_s0", "sweep_G30_T256_s1",
+                                  "sweep_G30_T4096_s1", "sweep_G8_T16384_s2"])
 def test_sweep_points_sampled(name):
     from bm_inputs import get_config
     _sampled_parity(get_config(name), 16)                       # BJ:configs[4]
+
+
+def test_prefill_path_is_deterministic():
+    # the prefill combine sums a token's rows in slot order (no atomics): two runs give identical bits
+    rng = np.random.default_rng(9)
+    L = rand_layer(rng, T=600, D=512, F=384, E=16, K=4, G=5, S=1, bias=True)
+    d = to_device(L)
+    _, out1, _ = gpu_layer(L, PATHS["prefill"], d)
+    _, out2, _ = gpu_layer(L, PATHS["prefill"], d)
+    assert (out1 == out2).all()
