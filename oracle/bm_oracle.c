@@ -305,3 +305,23 @@ int oracle_moe_forward(const uint16_t *x, int T, int D, int K, int G,
     free(sel_index);
     return 0;
 }
+
+/* Calibration forward: the output of EVERY original expert on every calibration token,
+ * f_e(x_t) = FFN_e(x_t), the quantity P:147-149 (Eq. 5) averages and P:170 takes cosine similarities of.
+ * W1, W3: [E, F, D]; W2: [E, D, F]; out: [E, T, D] fp64. */
+int oracle_expert_outputs(const uint16_t *x, int T, int D, const uint16_t *W1, const uint16_t *W3,
+                          const uint16_t *W2, int E, int F, double *out) {
+    if (T < 0 || D < 1 || F < 1 || E < 1) return -1;
+    const size_t wsz = (size_t)F * D;
+#pragma omp parallel
+    {
+        double *h = (double *)malloc(sizeof(double) * (size_t)F);
+#pragma omp for schedule(dynamic, 1) collapse(2)
+        for (int e = 0; e < E; ++e)
+            for (int t = 0; t < T; ++t)
+                ffn_f64(x + (size_t)t * D, W1 + e * wsz, W3 + e * wsz, W2 + e * wsz, D, F, h,
+                        out + ((size_t)e * T + t) * D);
+        free(h);
+    }
+    return 0;
+}

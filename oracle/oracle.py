@@ -45,6 +45,7 @@ def _load():
         _lib.oracle_route_partial.restype = ctypes.c_int
         _lib.oracle_unite_weights.restype = ctypes.c_int
         _lib.oracle_moe_forward.restype = ctypes.c_int
+        _lib.oracle_expert_outputs.restype = ctypes.c_int
     return _lib
 
 
@@ -147,6 +148,81 @@ def moe_forward(x, routing, W1, W3, W2, S: int = 0, sel_tokens=None) -> np.ndarr
     if rc != 0:
         raise ValueError("oracle_moe_forward: bad arguments")
     return out
+
+
+# ---------------------------------------------------------------------------------------------------
+# Calibration forward: the forward half of the reward evaluation of PAPER.md 4.3
+# ---------------------------------------------------------------------------------------------------
+def expert_histogram(expert_ids, E: int) -> np.ndarray:
+    """Routing frequency w_e, "how often expert e is selected by the gating function on the calibration
+    dataset" (PAPER.md:127), as integer counts over the ranked top-K ids [T, K]."""
+    w = np.zeros(E, np.int64)
+    for e in np.asarray(expert_ids).ravel():
+        w[int(e)] += 1
+    return w
+
+
+def expert_outputs(x, W1, W3, W2) -> np.ndarray:
+    """f_e(x_t) for every original expert e and token t, fp64 [E, T, D] (Eq. 5's f_e)."""
+    x, W1, W3, W2 = _u16(x), _u16(W1), _u16(W3), _u16(W2)
+    T, D = x.shape
+    E, F = W1.shape[0], W1.shape[1]
+    assert W1.shape == (E, F, D) and W3.shape == (E, F, D) and W2.shape == (E, D, F)
+    out = np.empty((E, T, D), np.float64)
+    rc = _load().oracle_expert_outputs(_p(x), T, D, _p(W1), _p(W3), _p(W2), E, F, _p(out))
+    if rc != 0:
+        raise ValueError("oracle_expert_outputs: bad arguments")
+    return out
+
+
+def cosine_matrix(Y) -> tuple:
+    """Pairwise cosine similarity matrix of expert outputs from calibration data.  Reading A19:
+    expert e is the vector of all its outputs, Y[e] flattened over tokens and features;
+    gram[e, e'] = <Y_e, Y_e'>,  cos[e, e'] = gram[e, e'] / (|Y_e| |Y_e'|).  Returns (gram, cos), fp64 [E, E]."""
+    Y = np.asarray(Y, np.float64)
+    E = Y.shape[0]
+    gram = np.zeros((E, E))
+    for a in range(E):
+        for b in range(E):
+            gram[a, b] = float(np.sum(Y[a] * Y[b]))
+    norm = np.sqrt(np.diag(gram))
+    cos = np.zeros((E, E))
+    for a in range(E):
+        for b in range(E):
+            cos[a, b] = gram[a, b] / (norm[a] * norm[b]) if norm[a] > 0 and norm[b] > 0 else 0.0
+    return gram, cos
+
+
+def group_mse(Y, U, w, group_map, G: int) -> tuple:
+    """Eq. 5 and Eq. 6 for a given united-expert output U [G, T, D]:
+        alpha_e = w_e / sum_{e' in G_k} w_e',   t_k(x) = sum_{e in G_k} alpha_e f_e(x)          (5)
+        MSE_r = E_x || f_{u_r}(x) - t_r(x) ||_2^2   (mean over calibration tokens of the squared L2 norm, Eq. 9)
+        beta_r = sum_{e in G_r} w_e,  MSE_total = sum_r beta_r MSE_r                             (6)
+    Reading A20: w_e are the routing counts normalised to sum 1 (frequencies); a group none of whose members
+    was ever selected has beta_r = 0 and takes uniform alpha (its term vanishes); an empty group has MSE_r = 0.
+    Returns (mse [G], mse_total, target [G, T, D])."""
+    Y, U = np.asarray(Y, np.float64), np.asarray(U, np.float64)
+    w = np.asarray(w, np.float64)
+    gmap = np.asarray(group_map)
+    wn = w / w.sum() if w.sum() > 0 else np.zeros_like(w)
+    T = Y.shape[1]
+    mse = np.zeros(G)
+    target = np.zeros_like(U)
+    total = 0.0
+    for r in range(G):
+        members = [e for e in range(len(gmap)) if gmap[e] == r]
+        if not members:
+            continue
+        beta = sum(wn[e] for e in members)
+        t = np.zeros_like(U[r])
+        for e in members:
+            alpha = wn[e] / beta if beta > 0 else 1.0 / len(members)
+            t = t + alpha * Y[e]
+        target[r] = t
+        diff = U[r] - t
+        mse[r] = float(np.sum(diff * diff)) / T if T > 0 else 0.0
+        total += beta * mse[r]
+    return mse, total, target
 
 
 def num_threads() -> int:

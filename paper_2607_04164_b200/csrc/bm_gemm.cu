@@ -21,6 +21,8 @@
 // 128-byte pieces) and combine_kernel sums a token's rows in slot order with the gate weights -- no
 // atomics, deterministic.  Decode: rows also live in different K-splits and there are few of them, so the
 // partials are added in fp32 with red.global.add into `out_acc` and a last pass rounds to bf16.
+#include <algorithm>
+
 #include "bm_common.cuh"
 #include "bm_ptx.cuh"
 
@@ -569,58 +571,60 @@ finalize_kernel(const float *__restrict__ out_acc, bm_bf16 *__restrict__ out, si
 
 // Prefill combine (F2): out[t] = sum_{s < n_slots[t]} gate_w[t,s] * y[slot_row[t,s]]  (slot order)
 //                               + sum_{j < S} y[TK + j*T + t]                          (shared experts)
-// fp32 accumulation in a fixed order -> deterministic.  One thread per 8 output columns (16 bytes).
+// fp32 accumulation in a fixed order -> deterministic.  One warp per token: lane s holds row and weight of
+// source s (K + S <= 32), the warp walks the D columns 16 bytes per lane (512 contiguous bytes per row and
+// step), four source rows in flight.
 __global__ void __launch_bounds__(256)
 combine_kernel(const bm_bf16 *__restrict__ y, int T, int D, int K, int S, const int32_t *__restrict__ n_slots,
                const int32_t *__restrict__ slot_row, const float *__restrict__ gate_w, bm_bf16 *__restrict__ out) {
     grid_dep_wait();
     grid_dep_launch();
+    const int lane = threadIdx.x & 31;
     const int vec = D / 8;
-    const size_t total = (size_t)T * vec;
     const size_t TK = (size_t)T * K;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
-        const int t = (int)(i / vec);
-        const int col = (int)(i - (size_t)t * vec) * 8;
-        float acc[8];
-#pragma unroll
-        for (int e = 0; e < 8; ++e) acc[e] = 0.0f;
+    const int warps = (gridDim.x * blockDim.x) >> 5;
+    for (int t = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; t < T; t += warps) {
         const int n = min(max(n_slots[t], 0), K);
-        // four rows at a time: all row indices, then all loads, then the adds in slot order
-        for (int s0 = 0; s0 < n + S; s0 += 4) {
-            size_t row[4];
-            float gw[4];
-            bool ok[4];
+        const int n_src = n + S;
+        long long my_row = -1;                                   // -1: skip (invalid slot_row)
+        float my_gw = 1.0f;
+        if (lane < n) {
+            const int r = slot_row[(size_t)t * K + lane];
+            if (r >= 0 && (size_t)r < TK) my_row = r;
+            my_gw = gate_w[(size_t)t * K + lane];
+        } else if (lane < n_src) {
+            my_row = (long long)TK + (long long)(lane - n) * T + t;
+        }
+        for (int c = lane; c < vec; c += 32) {
+            float acc[8];
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const int s = s0 + q;
-                ok[q] = s < n + S;
-                gw[q] = 1.0f;
-                row[q] = 0;
-                if (s < n) {
-                    const int r = slot_row[(size_t)t * K + s];
-                    ok[q] = r >= 0 && (size_t)r < TK;
-                    row[q] = ok[q] ? (size_t)r : 0;
-                    gw[q] = gate_w[(size_t)t * K + s];
-                } else if (ok[q]) {
-                    row[q] = TK + (size_t)(s - n) * T + t;
+            for (int e = 0; e < 8; ++e) acc[e] = 0.0f;
+            for (int s0 = 0; s0 < n_src; s0 += 4) {
+                uint4 v[4];
+                float gw[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const int src = min(s0 + q, 31);
+                    const long long row = __shfl_sync(kFullMask, my_row, src);
+                    gw[q] = __shfl_sync(kFullMask, my_gw, src);
+                    const bool ok = s0 + q < n_src && row >= 0;
+                    if (!ok) gw[q] = 0.0f;
+                    v[q] = ok ? *reinterpret_cast<const uint4 *>(y + (size_t)row * D + (size_t)c * 8) : make_uint4(0, 0, 0, 0);
+                }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    if (s0 + q < n_src) {                        // warp-uniform; skipped sources add nothing
+                        acc[0] = fmaf(gw[q], bf16_lo(v[q].x), acc[0]); acc[1] = fmaf(gw[q], bf16_hi(v[q].x), acc[1]);
+                        acc[2] = fmaf(gw[q], bf16_lo(v[q].y), acc[2]); acc[3] = fmaf(gw[q], bf16_hi(v[q].y), acc[3]);
+                        acc[4] = fmaf(gw[q], bf16_lo(v[q].z), acc[4]); acc[5] = fmaf(gw[q], bf16_hi(v[q].z), acc[5]);
+                        acc[6] = fmaf(gw[q], bf16_lo(v[q].w), acc[6]); acc[7] = fmaf(gw[q], bf16_hi(v[q].w), acc[7]);
+                    }
                 }
             }
-            uint4 v[4];
-#pragma unroll
-            for (int q = 0; q < 4; ++q)
-                v[q] = ok[q] ? *reinterpret_cast<const uint4 *>(y + row[q] * D + col) : make_uint4(0, 0, 0, 0);
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                if (!ok[q]) continue;
-                acc[0] = fmaf(gw[q], bf16_lo(v[q].x), acc[0]); acc[1] = fmaf(gw[q], bf16_hi(v[q].x), acc[1]);
-                acc[2] = fmaf(gw[q], bf16_lo(v[q].y), acc[2]); acc[3] = fmaf(gw[q], bf16_hi(v[q].y), acc[3]);
-                acc[4] = fmaf(gw[q], bf16_lo(v[q].z), acc[4]); acc[5] = fmaf(gw[q], bf16_hi(v[q].z), acc[5]);
-                acc[6] = fmaf(gw[q], bf16_lo(v[q].w), acc[6]); acc[7] = fmaf(gw[q], bf16_hi(v[q].w), acc[7]);
-            }
+            *reinterpret_cast<uint4 *>(out + (size_t)t * D + (size_t)c * 8) =
+                make_uint4(pack_bf16x2(acc[0], acc[1]), pack_bf16x2(acc[2], acc[3]), pack_bf16x2(acc[4], acc[5]),
+                           pack_bf16x2(acc[6], acc[7]));
         }
-        *reinterpret_cast<uint4 *>(out + (size_t)t * D + col) =
-            make_uint4(pack_bf16x2(acc[0], acc[1]), pack_bf16x2(acc[2], acc[3]), pack_bf16x2(acc[4], acc[5]),
-                       pack_bf16x2(acc[6], acc[7]));
     }
 }
 
@@ -839,7 +843,8 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
         if (decode)
             e = launch_kernel(finalize_kernel, dim3(grid), dim3(256), 0, stream, (const float *)a.out_acc, a.out, n8);
         else
-            e = launch_kernel(combine_kernel, dim3(grid), dim3(256), 0, stream, (const bm_bf16 *)a.y, a.T, a.D, a.K, a.S,
+            e = launch_kernel(combine_kernel, dim3((unsigned)std::min<long long>(((long long)a.T + 7) / 8, (long long)sms * 8)),
+                              dim3(256), 0, stream, (const bm_bf16 *)a.y, a.T, a.D, a.K, a.S,
                               (const int32_t *)a.r.n_slots, (const int32_t *)a.r.slot_row, (const float *)a.r.gate_w, a.out);
         profile_end(BM_KERNEL_FINALIZE, stream);
         return e;

@@ -28,8 +28,8 @@ constexpr int kItemsPerWarp = kPermItemsPerBlock / kWarps;   // 256
 
 // Count the items of this warp's slice into whist_w[0..G) (shared memory, zeroed by the caller).
 __device__ __forceinline__ void warp_histogram(const int32_t *__restrict__ group_ids, long long items,
-                                               long long first, int *whist_w, int lane) {
-    for (int r = 0; r < kItemsPerWarp && first + r < items; r += 32) {      // warp-uniform bound
+                                               long long first, int *whist_w, int lane, int per_warp = kItemsPerWarp) {
+    for (int r = 0; r < per_warp && first + r < items; r += 32) {      // warp-uniform bound
         const long long i = first + r + lane;
         const int key = (i < items) ? group_ids[i] : -1;
         const unsigned peers = __match_any_sync(kFullMask, key);
@@ -42,8 +42,8 @@ __device__ __forceinline__ void warp_histogram(const int32_t *__restrict__ group
 __device__ __forceinline__ void warp_permute(const int32_t *__restrict__ group_ids, long long items,
                                              long long first, int K, int *wbase_w, int lane, int A,
                                              int32_t *__restrict__ row_token, int32_t *__restrict__ row_slot,
-                                             int32_t *__restrict__ slot_row) {
-    for (int r = 0; r < kItemsPerWarp && first + r < items; r += 32) {      // warp-uniform bound
+                                             int32_t *__restrict__ slot_row, int per_warp = kItemsPerWarp) {
+    for (int r = 0; r < per_warp && first + r < items; r += 32) {      // warp-uniform bound
         const long long i = first + r + lane;
         const int key = (i < items) ? group_ids[i] : -1;
         const unsigned peers = __match_any_sync(kFullMask, key);
@@ -69,17 +69,20 @@ __device__ __forceinline__ void warp_permute(const int32_t *__restrict__ group_i
 
 // Block-wide exclusive scan of v[0..n) (n <= 512) in shared memory; returns the total in *total.
 __device__ void block_exclusive_scan(int *v, int n, int *tmp, int *total) {
-    // Hillis-Steele over 512 slots with 256 threads, two slots per thread
+    // Hillis-Steele over 512 slots by the first 256 threads of the block, two slots per thread
     for (int i = threadIdx.x; i < 512; i += blockDim.x) tmp[i] = i < n ? v[i] : 0;
     __syncthreads();
+    const bool act = threadIdx.x < 256;
     for (int d = 1; d < 512; d <<= 1) {
         int a0 = 0, a1 = 0;
         const int i0 = threadIdx.x, i1 = threadIdx.x + 256;
-        if (i0 >= d) a0 = tmp[i0 - d];
-        if (i1 >= d) a1 = tmp[i1 - d];
+        if (act && i0 >= d) a0 = tmp[i0 - d];
+        if (act && i1 >= d) a1 = tmp[i1 - d];
         __syncthreads();
-        tmp[i0] += a0;
-        tmp[i1] += a1;
+        if (act) {
+            tmp[i0] += a0;
+            tmp[i1] += a1;
+        }
         __syncthreads();
     }
     for (int i = threadIdx.x; i < n; i += blockDim.x) v[i] = tmp[i] - v[i];   // inclusive -> exclusive
@@ -88,27 +91,30 @@ __device__ void block_exclusive_scan(int *v, int n, int *tmp, int *total) {
 }
 
 // ---- T*K <= 2048: everything in one CTA --------------------------------------------------------
+// (One CTA of 32 warps for up to 32768 items was measured too: 31-46 us against 20-24 us for the three-kernel
+// path -- the serial rounds of one CTA expose every global-load latency.)
 __global__ void __launch_bounds__(kWarps * 32)
-permute_small_kernel(const int32_t *__restrict__ group_ids, int T, int K, int G,
+permute_small_kernel(const int32_t *__restrict__ group_ids, int T, int K, int G, int per_warp,
                      int32_t *__restrict__ counts, int32_t *__restrict__ offsets,
                      int32_t *__restrict__ row_token, int32_t *__restrict__ row_slot,
                      int32_t *__restrict__ slot_row, int32_t *__restrict__ status) {
     extern __shared__ int s_mem[];
     grid_dep_wait();
     grid_dep_launch();
-    int *whist = s_mem;                  // [kWarps][G]
-    int *gsum = whist + kWarps * G;      // [G] -> offsets
+    const int nw = blockDim.x >> 5;      // 8 warps x 256 items (T*K <= 2048) or 32 warps x per_warp items
+    int *whist = s_mem;                  // [nw][G]
+    int *gsum = whist + nw * G;          // [G] -> offsets
     int *tmp = gsum + G;                 // [512]
     __shared__ int s_total;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long items = (long long)T * K;
-    for (int i = threadIdx.x; i < kWarps * G; i += blockDim.x) whist[i] = 0;
+    for (int i = threadIdx.x; i < nw * G; i += blockDim.x) whist[i] = 0;
     __syncthreads();
-    warp_histogram(group_ids, items, (long long)warp * kItemsPerWarp, whist + warp * G, lane);
+    warp_histogram(group_ids, items, (long long)warp * per_warp, whist + warp * G, lane, per_warp);
     __syncthreads();
     for (int u = threadIdx.x; u < G; u += blockDim.x) {
         int run = 0;
-        for (int w = 0; w < kWarps; ++w) {      // whist[w][u] := rows of group u in warps before w
+        for (int w = 0; w < nw; ++w) {          // whist[w][u] := rows of group u in warps before w
             const int c = whist[w * G + u];
             whist[w * G + u] = run;
             run += c;
@@ -120,12 +126,12 @@ permute_small_kernel(const int32_t *__restrict__ group_ids, int T, int K, int G,
     block_exclusive_scan(gsum, G, tmp, &s_total);
     for (int u = threadIdx.x; u < G; u += blockDim.x) {
         offsets[u] = gsum[u];
-        for (int w = 0; w < kWarps; ++w) whist[w * G + u] += gsum[u];
+        for (int w = 0; w < nw; ++w) whist[w * G + u] += gsum[u];
     }
     if (threadIdx.x == 0) { offsets[G] = s_total; status[1] = s_total; }
     __syncthreads();
-    warp_permute(group_ids, items, (long long)warp * kItemsPerWarp, K, whist + warp * G, lane, s_total,
-                 row_token, row_slot, slot_row);
+    warp_permute(group_ids, items, (long long)warp * per_warp, K, whist + warp * G, lane, s_total,
+                 row_token, row_slot, slot_row, per_warp);
 }
 
 // ---- general case: P1 / P2 / P3 ---------------------------------------------------------------
@@ -216,7 +222,7 @@ cudaError_t launch_permute(int T, int K, int G, const bm_routing &r, int32_t *bl
     if (nb <= 1) {
         const size_t smem = smem_w + (size_t)(G + 512) * sizeof(int);
         return launch_kernel(permute_small_kernel, dim3(1), dim3(kWarps * 32), smem, stream, (const int32_t *)r.group_ids,
-                             T, K, G, r.counts, r.offsets, r.row_token, r.row_slot, r.slot_row, status);
+                             T, K, G, kItemsPerWarp, r.counts, r.offsets, r.row_token, r.row_slot, r.slot_row, status);
     }
     cudaError_t e = launch_kernel(permute_hist_kernel, dim3(nb), dim3(kWarps * 32), smem_w, stream,
                                   (const int32_t *)r.group_ids, T, K, G, block_hist);

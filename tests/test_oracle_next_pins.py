@@ -172,3 +172,81 @@ def test_united_expert_of_identical_members_reproduces_the_ungrouped_layer():
     U = [oracle.unite_weights(bf16_bits(w), gmap, G) for w in Wo]
     for u_avg, w in zip(U, (L.W1, L.W3, L.W2)):
         assert (u_avg == f64(w)).all()
+
+
+# --------------------------------------------------------------------------------------------
+# calibration forward (NEXT-2): routing frequency, expert outputs, cosine matrix, Eq. 5 / Eq. 6
+# --------------------------------------------------------------------------------------------
+def test_expert_histogram_counts_selections():
+    rng = np.random.default_rng(50)
+    L = rand_layer(rng, T=300, D=16, F=8, E=10, K=3, G=10, gmap=np.arange(10), bias=True)
+    r = _route(L)
+    w = oracle.expert_histogram(r.expert_ids, 10)
+    assert w.sum() == 300 * 3
+    # identity map: selecting expert e == visiting group e, whose rows R6 counted independently
+    assert (w == r.counts).all()
+    assert (oracle.expert_histogram(np.array([[2, 0], [2, 1]]), 4) == [1, 1, 2, 0]).all()
+
+
+def test_expert_outputs_match_library_matmuls_and_the_layer():
+    rng = np.random.default_rng(51)
+    E, T, D, F = 5, 12, 16, 24
+    L = rand_layer(rng, T=T, D=D, F=F, E=E, K=1, G=E, gmap=np.arange(E))
+    Y = oracle.expert_outputs(bf16_bits(L.x), bf16_bits(L.W1), bf16_bits(L.W3), bf16_bits(L.W2))
+    x, W1, W3, W2 = f64(L.x), f64(L.W1), f64(L.W3), f64(L.W2)
+    for e in range(E):
+        for t in range(T):
+            assert np.abs(Y[e, t] - ffn_def(x[t], W1[e], W3[e], W2[e])).max() <= 1e-12 * (1 + np.abs(Y[e, t]).max())
+    # top-1 layer (gate weight exactly 1): the layer output of token t is the output of the expert it chose
+    r = _route(L)
+    out = oracle.moe_forward(bf16_bits(L.x), r, bf16_bits(L.W1), bf16_bits(L.W3), bf16_bits(L.W2), 0)
+    for t in range(T):
+        assert np.abs(out[t] - Y[r.expert_ids[t, 0], t]).max() <= 1e-12 * (1 + np.abs(out[t]).max())
+
+
+def test_cosine_matrix_closed_forms():
+    rng = np.random.default_rng(52)
+    a = rng.standard_normal((7, 5))
+    b = rng.standard_normal((7, 5))
+    b_perp = b - a * (np.sum(a * b) / np.sum(a * a))            # orthogonal to a as a flattened vector
+    Y = np.stack([a, 3.0 * a, -2.0 * a, b_perp, a + b_perp])
+    gram, cos = oracle.cosine_matrix(Y)
+    assert np.allclose(np.diag(cos), 1.0, atol=1e-12) and np.allclose(cos, cos.T, atol=1e-15)
+    assert abs(cos[0, 1] - 1) <= 1e-12 and abs(cos[0, 2] + 1) <= 1e-12 and abs(cos[0, 3]) <= 1e-12
+    na, nb = np.sqrt(np.sum(a * a)), np.sqrt(np.sum(b_perp * b_perp))
+    assert abs(cos[0, 4] - na / np.sqrt(na * na + nb * nb)) <= 1e-12      # angle of a sum of orthogonal vectors
+    assert abs(gram[1, 2] + 6.0 * na * na) <= 1e-9
+    assert np.abs(cos).max() <= 1 + 1e-12
+    assert np.allclose(gram, np.einsum("etd,ftd->ef", Y, Y), rtol=1e-12, atol=1e-12)   # library contraction
+
+
+def test_group_mse_hand_worked_and_special_cases():
+    # Eq. 5 by hand: members with outputs 1 and 3, selected 1 and 3 times -> alpha = 1/4, 3/4 -> target 2.5;
+    # united output 2 -> MSE_0 = 0.25.  Second group: a single member (7), united output 7 -> MSE_1 = 0.
+    # w = [1, 3, 4] -> frequencies 1/8, 3/8, 4/8 -> beta = [1/2, 1/2] -> MSE_total = 0.125   (Eq. 6)
+    Y = np.array([[[1.0]], [[3.0]], [[7.0]]])
+    U = np.array([[[2.0]], [[7.0]]])
+    mse, total, target = oracle.group_mse(Y, U, [1, 3, 4], [0, 0, 1], 2)
+    assert target.ravel().tolist() == [2.5, 7.0] and mse.tolist() == [0.25, 0.0] and total == 0.125
+    # mean over tokens of the squared L2 norm over features (Eq. 9): T = 2, D = 2, differences (1, 2) and (0, 2)
+    Y = np.zeros((1, 2, 2))
+    U = np.array([[[1.0, 2.0], [0.0, 2.0]]])
+    mse, total, _ = oracle.group_mse(Y, U, [5], [0], 1)
+    assert mse.tolist() == [(1 + 4 + 0 + 4) / 2] and total == mse[0]
+    # identical members: any alpha gives the member itself; a united expert equal to it has zero error
+    rng = np.random.default_rng(53)
+    a = rng.standard_normal((6, 4))
+    Y = np.stack([a, a, rng.standard_normal((6, 4))])
+    U = np.stack([a, Y[2]])
+    mse, total, _ = oracle.group_mse(Y, U, [2, 9, 1], [0, 0, 1], 2)
+    assert np.abs(mse).max() <= 1e-28 and total <= 1e-28
+    # a never-selected group carries no weight (beta = 0); an empty group contributes nothing
+    Y = np.array([[[1.0]], [[5.0]]])
+    U = np.array([[[0.0]], [[0.0]], [[9.0]]])
+    mse, total, target = oracle.group_mse(Y, U, [4, 0], [0, 1, ][:2], 3)
+    assert mse.tolist() == [1.0, 25.0, 0.0] and total == 1.0
+    # the convex target lies between the member outputs (Eq. 5 is a convex combination)
+    Y = rng.standard_normal((4, 3, 2))
+    _, _, target = oracle.group_mse(Y, np.zeros((1, 3, 2)), [1, 2, 3, 4], [0, 0, 0, 0], 1)
+    assert (target[0] <= Y.max(0) + 1e-12).all() and (target[0] >= Y.min(0) - 1e-12).all()
+    assert np.allclose(target[0], np.tensordot(np.array([1, 2, 3, 4]) / 10.0, Y, axes=1), atol=1e-14)
