@@ -19,7 +19,9 @@ BM_DEV_BAD_GROUP_MAP, BM_DEV_NONFINITE_LOGIT, BM_DEV_BAD_ROUTING = 1, 2, 4
 BM_MAX_E, BM_MAX_K, BM_MAX_G = 512, 16, 512
 BM_DECODE_MAX_T = 256
 
-EXPORTS = ["bm_workspace_bytes", "bm_route", "bm_route_partial", "bm_unite_weights", "bm_moe_forward", "bm_moe_forward_path", "bm_moe_layer_host",
+EXPORTS = ["bm_workspace_bytes", "bm_route", "bm_route_partial", "bm_unite_weights", "bm_expert_histogram",
+           "bm_expert_outputs", "bm_gram_workspace_bytes", "bm_cosine_gram", "bm_mse_workspace_bytes", "bm_group_mse",
+           "bm_moe_forward", "bm_moe_forward_path", "bm_moe_layer_host",
            "bm_device_status", "bm_launch_count", "bm_status_string", "bm_profile_enable", "bm_profile_read"]
 KERNELS = {"router": 1, "permute": 2, "prep": 3, "gemm1": 4, "gemm2": 5, "finalize": 6}
 
@@ -56,6 +58,20 @@ def lib() -> ctypes.CDLL:
                                        c_void_p, POINTER(BmRouting), c_void_p, c_size_t, c_void_p]
         L.bm_unite_weights.restype = c_int
         L.bm_unite_weights.argtypes = [c_void_p, c_int, c_size_t, c_void_p, c_int, c_void_p, c_void_p]
+        L.bm_expert_histogram.restype = c_int
+        L.bm_expert_histogram.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p]
+        L.bm_expert_outputs.restype = c_int
+        L.bm_expert_outputs.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_void_p, c_int, c_int, c_void_p,
+                                        c_void_p, c_size_t, c_void_p]
+        L.bm_gram_workspace_bytes.restype = c_size_t
+        L.bm_gram_workspace_bytes.argtypes = [c_int]
+        L.bm_cosine_gram.restype = c_int
+        L.bm_cosine_gram.argtypes = [c_void_p, c_int, c_size_t, c_void_p, c_void_p, c_void_p, c_size_t, c_void_p]
+        L.bm_mse_workspace_bytes.restype = c_size_t
+        L.bm_mse_workspace_bytes.argtypes = [c_int]
+        L.bm_group_mse.restype = c_int
+        L.bm_group_mse.argtypes = [c_void_p, c_void_p, c_int, c_int, c_void_p, c_void_p, c_int, c_int, c_void_p,
+                                   c_void_p, c_void_p, c_size_t, c_void_p]
         L.bm_moe_forward.restype = c_int
         L.bm_moe_forward.argtypes = [c_void_p, c_int, c_int, POINTER(BmRouting), c_void_p, c_void_p, c_void_p,
                                      c_int, c_int, c_void_p, c_void_p, c_size_t, c_void_p]
@@ -173,6 +189,58 @@ def bm_unite_weights(W, group_map, G: int, out=None, stream=None):
     if rc != BM_OK:
         raise BmError(rc, "bm_unite_weights")
     return out
+
+
+def bm_expert_histogram(expert_ids, E: int, stream=None):
+    """w[e] = how often expert e was selected (include/bm.h: bm_expert_histogram).  expert_ids [T,K] i32 -> [E] i32."""
+    T, K = expert_ids.shape
+    w = torch.empty(E, dtype=torch.int32, device=expert_ids.device)
+    rc = lib().bm_expert_histogram(_ptr(expert_ids), T, K, E, _ptr(w), _stream(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_expert_histogram")
+    return w
+
+
+def bm_expert_outputs(x, W1, W3, W2, y=None, workspace=None, stream=None):
+    """y[e,t,:] = FFN_e(x_t) for every expert and token (include/bm.h: bm_expert_outputs) -> [E,T,D] bf16."""
+    T, D = x.shape
+    E, F = W1.shape[0], W1.shape[1]
+    if y is None:
+        y = torch.empty((E, T, D), dtype=torch.bfloat16, device=x.device)
+    if workspace is None:
+        workspace = alloc_workspace(T, D, F, E, 1, 1, E)
+    rc = lib().bm_expert_outputs(_ptr(x), T, D, _ptr(W1), _ptr(W3), _ptr(W2), E, F, _ptr(y), _ptr(workspace),
+                                 workspace.numel(), _stream(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_expert_outputs")
+    return y
+
+
+def bm_cosine_gram(Y, stream=None):
+    """(gram, cosine) [E,E] f32 of the expert outputs Y [E, ...] bf16 (include/bm.h: bm_cosine_gram)."""
+    E = Y.shape[0]
+    n = Y[0].numel()
+    gram = torch.empty((E, E), dtype=torch.float32, device=Y.device)
+    cos = torch.empty((E, E), dtype=torch.float32, device=Y.device)
+    ws = torch.empty(int(lib().bm_gram_workspace_bytes(E)), dtype=torch.uint8, device=Y.device)
+    rc = lib().bm_cosine_gram(_ptr(Y), E, n, _ptr(gram), _ptr(cos), _ptr(ws), ws.numel(), _stream(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_cosine_gram")
+    return gram, cos
+
+
+def bm_group_mse(Y, U, w, group_map, stream=None):
+    """(mse [G] f32, mse_total [1] f32) of Eq. 5-6 (include/bm.h: bm_group_mse).  Y [E,T,D], U [G,T,D] bf16."""
+    E, T, D = Y.shape
+    G = U.shape[0]
+    mse = torch.empty(G, dtype=torch.float32, device=Y.device)
+    tot = torch.empty(1, dtype=torch.float32, device=Y.device)
+    ws = torch.empty(int(lib().bm_mse_workspace_bytes(G)), dtype=torch.uint8, device=Y.device)
+    rc = lib().bm_group_mse(_ptr(Y), _ptr(U), T, D, _ptr(w), _ptr(group_map), E, G, _ptr(mse), _ptr(tot), _ptr(ws),
+                            ws.numel(), _stream(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_group_mse")
+    return mse, tot
 
 
 def bm_moe_forward(x, routing: Routing, W1, W3, W2, out, workspace, S: int = 0, path: int = BM_PATH_AUTO,

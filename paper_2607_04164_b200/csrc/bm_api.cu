@@ -154,6 +154,67 @@ int bm_unite_weights(const bm_bf16 *W, int E, size_t n, const int32_t *group_map
                ? BM_OK : BM_ERR_CUDA;
 }
 
+int bm_expert_histogram(const int32_t *expert_ids, int T, int K, int E, int32_t *w, bm_stream_t stream) {
+    if (T < 0 || K < 1 || E < 1 || E > BM_MAX_E || (long long)T * K > 0x3fffffffLL) return BM_ERR_SHAPE;
+    if (!w || (T > 0 && !expert_ids)) return BM_ERR_NULL;
+    if (device_ok() != 1) return BM_ERR_CUDA;
+    return launch_expert_hist(expert_ids, (long long)T * K, E, w, reinterpret_cast<cudaStream_t>(stream)) == cudaSuccess
+               ? BM_OK : BM_ERR_CUDA;
+}
+
+int bm_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 *W1, const bm_bf16 *W3, const bm_bf16 *W2, int E,
+                      int F, bm_bf16 *y, void *workspace, size_t workspace_bytes, bm_stream_t stream) {
+    if (T < 0 || D < 8 || D % 8 != 0 || F < 8 || F % 8 != 0 || E < 1 || E > BM_MAX_G) return BM_ERR_SHAPE;
+    if ((long long)T * E > 0x3fffffffLL) return BM_ERR_SHAPE;
+    if (T == 0) return BM_OK;
+    if (!x || !W1 || !W3 || !W2 || !y || !workspace) return BM_ERR_NULL;
+    if (!aligned16(x) || !aligned16(W1) || !aligned16(W3) || !aligned16(W2) || !aligned16(y) || !aligned16(workspace))
+        return BM_ERR_ALIGN;
+    const Workspace w = workspace_layout(T, D, F, 1, 1, E);
+    if (workspace_bytes < w.total) return BM_ERR_WORKSPACE;
+    if (device_ok() != 1) return BM_ERR_CUDA;
+    uint8_t *ws = static_cast<uint8_t *>(workspace);
+    return launch_expert_outputs(x, T, D, W1, W3, W2, E, F, y, reinterpret_cast<int32_t *>(ws + w.sched),
+                                 reinterpret_cast<bm_bf16 *>(ws + w.h), reinterpret_cast<cudaStream_t>(stream)) == cudaSuccess
+               ? BM_OK : BM_ERR_CUDA;
+}
+
+size_t bm_gram_workspace_bytes(int E) {
+    if (E < 1 || E > 128) return 0;
+    return (size_t)256 * E * E * sizeof(float);          // one partial tile per CTA, any SM count up to 256
+}
+
+int bm_cosine_gram(const bm_bf16 *Y, int E, size_t n, float *gram, float *cosine, void *workspace,
+                   size_t workspace_bytes, bm_stream_t stream) {
+    if (E < 1 || E > 128 || n % 8 != 0 || n == 0 || n > 0x7fffff00ull) return BM_ERR_SHAPE;
+    if (!Y || !gram || !workspace) return BM_ERR_NULL;
+    if (!aligned16(Y) || !aligned16(workspace)) return BM_ERR_ALIGN;
+    if (workspace_bytes < bm_gram_workspace_bytes(E)) return BM_ERR_WORKSPACE;
+    if (device_ok() != 1) return BM_ERR_CUDA;
+    if (num_sms() > 256) return BM_ERR_CUDA;
+    return launch_gram(Y, E, n, gram, cosine, static_cast<float *>(workspace), reinterpret_cast<cudaStream_t>(stream)) ==
+                   cudaSuccess
+               ? BM_OK : BM_ERR_CUDA;
+}
+
+size_t bm_mse_workspace_bytes(int G) {
+    if (G < 1 || G > BM_MAX_G) return 0;
+    return ((size_t)256 * 8 + (size_t)G) * sizeof(float) * 2;   // >= G * blocks-per-group partial sums (see launch_group_mse)
+}
+
+int bm_group_mse(const bm_bf16 *Y, const bm_bf16 *U, int T, int D, const int32_t *w, const int32_t *group_map, int E,
+                 int G, float *mse, float *mse_total, void *workspace, size_t workspace_bytes, bm_stream_t stream) {
+    if (T < 1 || D < 8 || D % 8 != 0 || E < 1 || E > BM_MAX_E || G < 1 || G > BM_MAX_G) return BM_ERR_SHAPE;
+    if (!Y || !U || !w || !group_map || !mse || !mse_total || !workspace) return BM_ERR_NULL;
+    if (!aligned16(Y) || !aligned16(U)) return BM_ERR_ALIGN;
+    if (workspace_bytes < bm_mse_workspace_bytes(G)) return BM_ERR_WORKSPACE;
+    if (device_ok() != 1) return BM_ERR_CUDA;
+    if ((size_t)(mse_blocks() / G + 1) * G * sizeof(float) > workspace_bytes) return BM_ERR_WORKSPACE;
+    return launch_group_mse(Y, U, T, D, w, group_map, E, G, mse, mse_total, static_cast<float *>(workspace),
+                            reinterpret_cast<cudaStream_t>(stream)) == cudaSuccess
+               ? BM_OK : BM_ERR_CUDA;
+}
+
 int bm_moe_forward_path(const bm_bf16 *x, int T, int D, const bm_routing *routing, const bm_bf16 *W1,
                         const bm_bf16 *W3, const bm_bf16 *W2, int F, int S, bm_bf16 *out, void *workspace,
                         size_t workspace_bytes, bm_stream_t stream, int path) {

@@ -117,6 +117,18 @@ struct ForwardArgs {
 cudaError_t launch_unite(const bm_bf16 *W, int E, size_t n, const int32_t *gmap, int G, bm_bf16 *out,
                          cudaStream_t stream);
 
+cudaError_t launch_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 *W1, const bm_bf16 *W3,
+                                  const bm_bf16 *W2, int E, int F, bm_bf16 *y, int32_t *sched, bm_bf16 *h,
+                                  cudaStream_t stream);
+
+cudaError_t launch_expert_hist(const int32_t *expert_ids, long long items, int E, int32_t *w, cudaStream_t stream);
+size_t gram_workspace_bytes(int E);
+cudaError_t launch_gram(const bm_bf16 *Y, int E, size_t n, float *gram, float *cosine, float *partial,
+                        cudaStream_t stream);
+int mse_blocks();
+cudaError_t launch_group_mse(const bm_bf16 *Y, const bm_bf16 *U, int T, int D, const int32_t *w, const int32_t *gmap,
+                             int E, int G, float *mse, float *mse_total, float *part, cudaStream_t stream);
+
 cudaError_t launch_forward_simt(const ForwardArgs &a, cudaStream_t stream);
 cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t stream);
 

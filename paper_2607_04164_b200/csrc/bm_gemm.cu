@@ -569,6 +569,24 @@ finalize_kernel(const float *__restrict__ out_acc, bm_bf16 *__restrict__ out, si
     }
 }
 
+// Schedule of the all-experts forward (calibration, NEXT-2): E segments of T rows each, every one a "shared"
+// segment (weight set j on every token), so GEMM1 reads x directly and GEMM2 writes y row j*T + t.
+__global__ void __launch_bounds__(256)
+dense_sched_kernel(int32_t *__restrict__ sched, int E, int T) {
+    grid_dep_wait();
+    grid_dep_launch();
+    const int cps = (T + kChunkRows - 1) / kChunkRows;
+    for (int j = threadIdx.x; j <= E; j += blockDim.x) {
+        sched[kSchedChunk0 + j] = j * cps;
+        if (j < E) {
+            sched[kSchedSegU + j] = j;
+            sched[kSchedRows + j] = T;
+            sched[kSchedOff + j] = 0;
+        }
+    }
+    if (threadIdx.x == 0) { sched[0] = E; sched[1] = E * cps; }
+}
+
 // Prefill combine (F2): out[t] = sum_{s < n_slots[t]} gate_w[t,s] * y[slot_row[t,s]]  (slot order)
 //                               + sum_{j < S} y[TK + j*T + t]                          (shared experts)
 // fp32 accumulation in a fixed order -> deterministic.  One warp per token: lane s holds row and weight of
@@ -849,6 +867,29 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
         profile_end(BM_KERNEL_FINALIZE, stream);
         return e;
     }
+}
+
+// f_e(x_t) for every expert and token (calibration forward): the prefill GEMM kernels over a
+// dense schedule (G = 0 routed groups, S = E always-on weight sets); y: [E, T, D] bf16.
+cudaError_t launch_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 *W1, const bm_bf16 *W3,
+                                  const bm_bf16 *W2, int E, int F, bm_bf16 *y, int32_t *sched, bm_bf16 *h,
+                                  cudaStream_t stream) {
+    cudaError_t err = launch_kernel(dense_sched_kernel, dim3(1), dim3(256), 0, stream, sched, E, T);
+    if (err != cudaSuccess) return err;
+    GemmParams p{};
+    p.seg_cap = E + 1;
+    p.T = T; p.D = D; p.F = F; p.K = 1; p.G = 0; p.S = E; p.TK = 0;
+    p.sched = sched; p.h = h; p.y = y;
+    p.ksplit = 1;
+    CUtensorMap m_x, m_w1, m_w3, m_w2, m_h;
+    if (!make_map_2d(&m_x, x, T, D, 128) || !make_map_3d(&m_w1, W1, E, F, D, 128) || !make_map_3d(&m_w3, W3, E, F, D, 128) ||
+        !make_map_3d(&m_w2, W2, E, D, F, 256) || !make_map_2d(&m_h, h, (uint64_t)E * T, F, 128))
+        return cudaErrorInvalidValue;
+    ring_geometry(false, true, T, &p);
+    p.kblocks = (D + kBlockK - 1) / kBlockK; p.R = 128; p.n_wtiles = (F + 127) / 128;
+    if ((err = launch_gemm<PF_GEMM1>(m_x, m_x, m_w1, m_w3, p, stream)) != cudaSuccess) return err;
+    p.kblocks = (F + kBlockK - 1) / kBlockK; p.R = 256; p.n_wtiles = (D + 255) / 256;
+    return launch_gemm<PF_GEMM2>(m_h, m_h, m_w2, m_w2, p, stream);
 }
 
 }  // namespace bm

@@ -104,3 +104,111 @@ def test_unite_weights_matches_oracle(E, G, shape):
         m = np.nonzero(gmap == u)[0]
         if len(m) == 1:
             assert (out[u].cpu().view(torch.uint16) == W[m[0]].view(torch.uint16)).all()
+
+
+# ---------------------------------------------------------------------------------------------------
+# calibration forward (NEXT-2)
+# ---------------------------------------------------------------------------------------------------
+def _calib_case(seed, T, D, F, E, K, G):
+    cfg = LayerConfig("cal", T=T, D=D, F=F, E=E, K=K, G=G, zipf_s=1.0)
+    L = make_layer(cfg, seed, weights=False)
+    Wo = _orig(seed, E, F, D)
+    return cfg, L, Wo
+
+
+@pytest.mark.parametrize("T,D,F,E,K,G", [(96, 256, 320, 12, 3, 4), (700, 512, 264, 60, 4, 15), (5, 64, 64, 3, 1, 2)])
+def test_expert_histogram_and_outputs(T, D, F, E, K, G):
+    import paper_2607_04164_b200 as bm
+    cfg, L, Wo = _calib_case(2, T, D, F, E, K, G)
+    bias = None if L.router_bias is None else L.router_bias.numpy()
+    o = oracle.route(bf16_bits(L.x), bf16_bits(L.W_router), bias, K, L.group_map.numpy(), G)
+    # routing frequency: exact
+    w = bm.bm_expert_histogram(torch.as_tensor(o.expert_ids).cuda(), E)
+    assert (w.cpu().numpy() == oracle.expert_histogram(o.expert_ids, E)).all()
+    # all-expert outputs: the hot path's tolerance
+    Y = bm.bm_expert_outputs(L.x.cuda(), Wo[0].cuda(), Wo[1].cuda(), Wo[2].cuda())
+    torch.cuda.synchronize()
+    ref = oracle.expert_outputs(bf16_bits(L.x), bf16_bits(Wo[0]), bf16_bits(Wo[1]), bf16_bits(Wo[2]))
+    assert_out_close(Y.float().cpu().numpy().astype(np.float64).reshape(E * T, D), ref.reshape(E * T, D))
+
+
+@pytest.mark.parametrize("E,T,D", [(12, 96, 256), (60, 300, 512), (128, 40, 64), (3, 5, 8)])
+def test_cosine_gram_matches_oracle(E, T, D):
+    import paper_2607_04164_b200 as bm
+    rng = np.random.default_rng(E)
+    base = rng.standard_normal((4, T, D))
+    mix = rng.standard_normal((E, 4)) * np.array([2.0, 1.0, 0.5, 0.25])        # correlated experts
+    Y = bf16_tensor(np.tensordot(mix, base, axes=1) + 0.3 * rng.standard_normal((E, T, D)))
+    if E >= 3:
+        Y[1] = Y[0]                                                        # identical pair -> cos 1
+        Y[2] = -Y[0]                                                       # negated -> cos -1
+    gram, cos = bm.bm_cosine_gram(Y.cuda())
+    torch.cuda.synchronize()
+    g_ref, c_ref = oracle.cosine_matrix(Y.double().numpy())
+    gram, cos = gram.cpu().numpy().astype(np.float64), cos.cpu().numpy().astype(np.float64)
+    # same bf16 inputs on both sides: only the fp32 accumulation order differs (n terms, products exact in fp32 pairs)
+    scale = np.sqrt(np.outer(np.diag(g_ref), np.diag(g_ref)))
+    assert (np.abs(gram - g_ref) <= 1e-5 * scale).all()
+    assert (np.abs(cos - c_ref) <= 2e-5).all()
+    assert np.allclose(gram, gram.T, rtol=0, atol=1e-6 * scale.max())
+    if E >= 3:
+        assert abs(cos[0, 1] - 1) <= 2e-5 and abs(cos[0, 2] + 1) <= 2e-5
+    # determinism: partial tiles are summed in a fixed order
+    gram2, _ = bm.bm_cosine_gram(Y.cuda())
+    assert (gram2.cpu().numpy() == gram.astype(np.float32)).all()
+
+
+@pytest.mark.parametrize("E,G,T,D", [(12, 4, 96, 256), (60, 15, 200, 512), (5, 8, 7, 16)])
+def test_group_mse_matches_oracle(E, G, T, D):
+    import paper_2607_04164_b200 as bm
+    rng = np.random.default_rng(E + G)
+    Y = bf16_tensor(rng.standard_normal((E, T, D)))
+    U = bf16_tensor(rng.standard_normal((G, T, D)) * 0.5)
+    gmap = rng.integers(0, G, size=E).astype(np.int32)
+    w = rng.integers(0, 50, size=E).astype(np.int32)
+    w[gmap == gmap[0]] = 0                                                # one never-selected group (A20)
+    mse, tot = bm.bm_group_mse(Y.cuda(), U.cuda(), torch.as_tensor(w).cuda(), torch.as_tensor(gmap).cuda())
+    torch.cuda.synchronize()
+    m_ref, t_ref, _ = oracle.group_mse(Y.double().numpy(), U.double().numpy(), w, gmap, G)
+    mse, tot = mse.cpu().numpy().astype(np.float64), float(tot.cpu()[0])
+    assert (np.abs(mse - m_ref) <= 1e-4 * m_ref + 1e-6).all()              # same bf16 inputs; fp32 target and squares
+    assert abs(tot - t_ref) <= 1e-4 * t_ref + 1e-6
+    for r in range(G):
+        if not (gmap == r).any():
+            assert mse[r] == 0.0
+
+
+def test_calibration_pipeline_end_to_end_against_oracle():
+    """Routing frequency -> all-expert outputs -> united experts by parameter average (NEXT-3) -> their outputs ->
+    Eq. 5-6, every stage on the GPU, against the fp64 oracle fed with the same inputs only."""
+    import paper_2607_04164_b200 as bm
+    T, D, F, E, K, G = 256, 256, 192, 16, 2, 4
+    cfg, L, Wo = _calib_case(3, T, D, F, E, K, G)
+    gmap = L.group_map.numpy()
+    bias = L.router_bias.numpy()
+    xd, gm = L.x.cuda(), L.group_map.cuda()
+    ws = bm.alloc_workspace(T, D, F, E, K, G, 0)
+    r = bm.Routing(T, K, G)
+    bm.bm_route(xd, L.W_router.cuda(), L.router_bias.cuda(), K, gm, G, r, ws)
+    w = bm.bm_expert_histogram(r.view(T)["expert_ids"], E)
+    Wd = [t.cuda() for t in Wo]
+    Y = bm.bm_expert_outputs(xd, *Wd)
+    Ud = [bm.bm_unite_weights(t, gm, G) for t in Wd]
+    U = bm.bm_expert_outputs(xd, *Ud)
+    mse, tot = bm.bm_group_mse(Y, U, w, gm)
+    gram, cos = bm.bm_cosine_gram(Y)
+    torch.cuda.synchronize()
+    # oracle chain (fp64; the united weights are rounded to bf16 as the GPU stores them -- A18)
+    o = oracle.route(bf16_bits(L.x), bf16_bits(L.W_router), bias, K, gmap, G)
+    w_ref = oracle.expert_histogram(o.expert_ids, E)
+    assert (w.cpu().numpy() == w_ref).all()
+    Y_ref = oracle.expert_outputs(bf16_bits(L.x), *[bf16_bits(t) for t in Wo])
+    Uw = [bf16_tensor(oracle.unite_weights(bf16_bits(t), gmap, G)) for t in Wo]
+    U_ref = oracle.expert_outputs(bf16_bits(L.x), *[bf16_bits(t) for t in Uw])
+    m_ref, t_ref, _ = oracle.group_mse(Y_ref, U_ref, w_ref, gmap, G)
+    _, c_ref = oracle.cosine_matrix(Y_ref)
+    # bf16 outputs on the GPU side: each y carries 2^-9 relative rounding noise -> 2e-2 relative on the MSE, 5e-3 on cos
+    mse = mse.cpu().numpy().astype(np.float64)
+    assert (np.abs(mse - m_ref) <= 2e-2 * m_ref + 1e-7).all(), (mse, m_ref)
+    assert abs(float(tot.cpu()[0]) - t_ref) <= 2e-2 * t_ref + 1e-7
+    assert np.abs(cos.cpu().numpy() - c_ref).max() <= 5e-3
