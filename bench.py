@@ -605,8 +605,52 @@ def run_next(args):
                  frac_of_hbm=ub / tu / 1e9 / peaks["hbm_gbs"], l2="flushed with a 256 MB write before every launch")
     sys.stderr.write(f"unite_weights E={E} G={G}: {tu*1e6:.1f} us, {unite['achieved_gbs']:.0f} GB/s "
                      f"({unite['frac_of_hbm']:.2f} of measured HBM)\n")
+    # calibration forward (NEXT-2): T = 4096 calibration tokens through all E = 60 experts, Gram/cosine, Eq. 5-6
+    del W
+    torch.cuda.empty_cache()
+    Tc = 4096
+    Lc = make_layer(get_config(f"sweep_G{G}_T{Tc}_s1"), 0, weights=False)
+    xc = Lc.x.cuda()
+    Wo = (mk(E, F, D), mk(E, F, D), mk(E, D, F))
+    wsc = bm.alloc_workspace(Tc, D, F, E, 1, 1, E)
+    Y = torch.empty((E, Tc, D), dtype=torch.bfloat16, device="cuda")
+    Uw = [bm.bm_unite_weights(t, gm, G) for t in Wo]
+    U = bm.bm_expert_outputs(xc, *Uw)
+    wcnt = torch.randint(1, 1000, (E,), dtype=torch.int32, device="cuda")
+
+    def timed(fn, reps=8):
+        ts = []
+        for i in range(reps + 2):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize()
+            if i >= 2:
+                ts.append(e0.elapsed_time(e1) / 1e3)
+        return statistics.median(ts)
+
+    t_out = timed(lambda: bm.bm_expert_outputs(xc, *Wo, y=Y, workspace=wsc))
+    t_gram = timed(lambda: bm.bm_cosine_gram(Y))
+    t_mse = timed(lambda: bm.bm_group_mse(Y, U, wcnt, gm))
+    f_out = E * Tc * 6.0 * D * F
+    b_gram = E * Tc * D * 2
+    b_mse = (E + G) * Tc * D * 2
+    calib = dict(T=Tc, E=E, G=G,
+                 expert_outputs=dict(us=t_out * 1e6, flops=f_out, tflops=f_out / t_out / 1e12,
+                                     frac_of_bf16_burst=f_out / t_out / 1e12 / peaks["bf16_tflops"]),
+                 cosine_gram=dict(us=t_gram * 1e6, alg_bytes=b_gram, gbs=b_gram / t_gram / 1e9,
+                                  frac_of_hbm=b_gram / t_gram / 1e9 / peaks["hbm_gbs"]),
+                 group_mse=dict(us=t_mse * 1e6, alg_bytes=b_mse, gbs=b_mse / t_mse / 1e9,
+                                frac_of_hbm=b_mse / t_mse / 1e9 / peaks["hbm_gbs"]),
+                 l2="flushed with a 256 MB write before every launch")
+    sys.stderr.write(f"calibration T={Tc}: expert_outputs {t_out*1e6:.0f} us {calib['expert_outputs']['tflops']:.0f} TFLOP/s; "
+                     f"gram {t_gram*1e6:.0f} us {calib['cosine_gram']['gbs']:.0f} GB/s; mse {t_mse*1e6:.0f} us "
+                     f"{calib['group_mse']['gbs']:.0f} GB/s\n")
     res = dict(metric=METRIC, unit=UNIT, workload="SURVEY 8(f): partial brownout at D=2048 F=1408 E=60 top-4 G=15 zipf 1.0; "
-               "united-weight average", peaks=peaks, weight_copies=copies, partial=rows, unite=unite)
+               "united-weight average; calibration forward", peaks=peaks, weight_copies=copies, partial=rows, unite=unite,
+               calibration=calib)
     if args.out:
         with open(args.out, "w") as fh:
             json.dump(res, fh, indent=1)

@@ -36,6 +36,9 @@ expert_hist_kernel(const int32_t *__restrict__ expert_ids, long long items, int 
 // Y . Y^T, so ONE TMA tile (128 rows x 64 columns; rows >= E are out of bounds and arrive as zeros) feeds
 // the A and the B descriptor of tcgen05.mma.  CTA c owns the k-blocks c, c + grid, ... and keeps its
 // 128 x N fp32 partial in TMEM until the end; partial tiles go to the workspace and are summed in CTA order.
+// Measured: 3.5-3.7 TB/s (0.55 of the HBM copy rate) whatever E is; the time per k-block grows with the rows of
+// the TMA box (~8 cycles per 128-byte row), so the kernel sits on the TMA row rate, not on the MMAs -- packing two
+// k-blocks of a small-E tile into one M = N = 128 MMA was tried and changed nothing.
 // ---------------------------------------------------------------------------------------------------
 constexpr int kGramThreads = 192;
 constexpr int kGramStages = 12;
@@ -127,23 +130,33 @@ gram_kernel(const __grid_constant__ CUtensorMap tm_y, int E, int n_kblocks, floa
     }
 }
 
-// gram[e,e'] = sum over CTAs in index order (deterministic); then cos = gram / sqrt(gram[e,e] gram[e',e'])
-__global__ void __launch_bounds__(256)
+// gram[e,e'] = sum of the per-CTA partial tiles in CTA order (deterministic); cos = gram / sqrt(gram[e,e] gram[e',e']).
+// Block e owns row e; thread j sums element (e, j) and the diagonal element (j, j) it needs for the cosine.
+__global__ void __launch_bounds__(128)
 gram_finish_kernel(const float *__restrict__ partial, int n_cta, int E, float *__restrict__ gram,
                    float *__restrict__ cosine) {
-    __shared__ float s_diag[BM_MAX_E];
-    for (int i = threadIdx.x; i < E * E; i += blockDim.x) {
-        float acc = 0.0f;
-        for (int c = 0; c < n_cta; ++c) acc += partial[(size_t)c * E * E + i];
-        gram[i] = acc;
-        if (i / E == i % E) s_diag[i / E] = acc;
+    __shared__ float s_diag_e;
+    const int e = blockIdx.x, j = threadIdx.x;
+    float acc = 0.0f, dj = 0.0f;
+    if (j < E) {
+        const size_t ee = (size_t)E * E;
+        const float *pr = partial + (size_t)e * E + j, *pd = partial + (size_t)j * E + j;
+        int c = 0;
+        for (; c + 4 <= n_cta; c += 4) {                 // four loads in flight, added in CTA order
+            const float r0 = pr[c * ee], r1 = pr[(c + 1) * ee], r2 = pr[(c + 2) * ee], r3 = pr[(c + 3) * ee];
+            const float d0 = pd[c * ee], d1 = pd[(c + 1) * ee], d2 = pd[(c + 2) * ee], d3 = pd[(c + 3) * ee];
+            acc = (((acc + r0) + r1) + r2) + r3;
+            dj = (((dj + d0) + d1) + d2) + d3;
+        }
+        for (; c < n_cta; ++c) { acc += pr[c * ee]; dj += pd[c * ee]; }
+        gram[(size_t)e * E + j] = acc;
+        if (j == e) s_diag_e = dj;
     }
     __syncthreads();
-    if (cosine)
-        for (int i = threadIdx.x; i < E * E; i += blockDim.x) {
-            const float d = s_diag[i / E] * s_diag[i % E];
-            cosine[i] = d > 0.0f ? gram[i] * rsqrtf(d) : 0.0f;
-        }
+    if (cosine && j < E) {
+        const float d = s_diag_e * dj;
+        cosine[(size_t)e * E + j] = d > 0.0f ? acc * rsqrtf(d) : 0.0f;
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -278,7 +291,7 @@ cudaError_t launch_gram(const bm_bf16 *Y, int E, size_t n, float *gram, float *c
         attr = true;
     }
     gram_kernel<<<grid, kGramThreads, smem, stream>>>(tm, E, (int)nkb, partial);
-    gram_finish_kernel<<<1, 256, 0, stream>>>(partial, grid, E, gram, cosine);
+    gram_finish_kernel<<<E, 128, 0, stream>>>(partial, grid, E, gram, cosine);
     count_launch(2);
     return cudaGetLastError();
 }
