@@ -82,7 +82,6 @@ struct GemmParams {
     int R;              // weight rows per tile (prefill: 128 for GEMM1 per matrix, 256 for GEMM2)
     int n_wtiles;       // tiles along the weight-row dimension
     int seg_cap;        // G + S + 1: entries per schedule array cached in shared memory
-    int dbg;
     const int32_t *counts, *offsets, *row_token, *row_slot;
     const float *gate_w;
     const int32_t *sched;
@@ -367,7 +366,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
                 const int rl = lane >> 3, ul = lane & 7;        // read phase: row (mod 4) and 16-byte unit of this lane
                 bm_bf16 *ybase = p.y + (size_t)(it.h_row0 + q * 32) * p.D + d0 + 8 * ul;
 #pragma unroll 1
-                for (int c = 0; c < ((p.dbg & 2) ? 0 : 256); c += 64) {
+                for (int c = 0; c < 256; c += 64) {
                     uint32_t v[32], w[32];
                     ptx::tmem_ld_x32(t_addr + c, v);
                     ptx::tmem_ld_x32(t_addr + c + 32, w);
@@ -390,7 +389,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
 #pragma unroll
                         for (int j = 0; j < 8; ++j) {
                             const int r = 4 * j + rl;
-                            if (r < n_q && !(p.dbg & 1))
+                            if (r < n_q)
                                 *reinterpret_cast<uint4 *>(ybase + (size_t)r * p.D + c) = stg[r * 8 + (ul ^ (r & 7))];
                         }
                     }
@@ -805,7 +804,6 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
     }
 
     GemmParams p{};
-    p.dbg = tune_int("BM_DBG", 0);
     p.seg_cap = a.G + a.S + 1;
     p.T = a.T; p.D = a.D; p.F = a.F; p.K = a.K; p.G = a.G; p.S = a.S; p.TK = TK;
     p.counts = a.r.counts; p.offsets = a.r.offsets; p.row_token = a.r.row_token; p.row_slot = a.r.row_slot;
