@@ -30,7 +30,7 @@ struct Workspace {
 };
 
 constexpr int kMaxShared = 16;                                  // S <= 16 always-on shared experts
-constexpr int kSchedInts = 4 + 4 * (BM_MAX_G + kMaxShared) + 8;
+constexpr int kSchedInts = 4 + 5 * (BM_MAX_G + kMaxShared) + 8;
 
 __host__ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 

@@ -60,14 +60,16 @@ constexpr int kSchedSegU = 4;
 constexpr int kSchedChunk0 = kSchedSegU + kMaxSeg;
 constexpr int kSchedRows = kSchedChunk0 + kMaxSeg;
 constexpr int kSchedOff = kSchedRows + kMaxSeg;
-static_assert(kSchedOff + kMaxSeg + 1 <= kSchedInts, "sched too small");
+constexpr int kSchedPair0 = kSchedOff + kMaxSeg;      // first chunk PAIR of segment s (CTA-pair prefill tiles); [2] = total
+static_assert(kSchedPair0 + kMaxSeg + 1 <= kSchedInts, "sched too small");
 
 struct SchedView {
-    int n_seg, total_chunks;
-    const int32_t *u, *chunk0, *rows, *off;
+    int n_seg, total_chunks, total_pairs;
+    const int32_t *u, *chunk0, *rows, *off, *pair0;
 };
 __device__ __forceinline__ SchedView sched_global(const int32_t *sched) {
-    return SchedView{sched[0], sched[1], sched + kSchedSegU, sched + kSchedChunk0, sched + kSchedRows, sched + kSchedOff};
+    return SchedView{sched[0], sched[1], sched[2], sched + kSchedSegU, sched + kSchedChunk0, sched + kSchedRows,
+                     sched + kSchedOff, sched + kSchedPair0};
 }
 
 struct GemmParams {
@@ -102,28 +104,35 @@ struct Item {
     bool shared;
 };
 
-template <int MODE>
-__device__ __forceinline__ bool get_item(const GemmParams &p, const SchedView &sv, int item, Item &it) {
+// K2 (CTA-pair prefill tiles): an item is a PAIR of consecutive 128-row chunks of one segment on one weight
+// tile; `rank` (0 or 1) picks this CTA's chunk.  A segment with an odd chunk count leaves rank 1 of its last
+// pair without rows (it.n = 0: it loads a valid tile, multiplies it and stores nothing).
+template <int MODE, bool K2 = false>
+__device__ __forceinline__ bool get_item(const GemmParams &p, const SchedView &sv, int item, Item &it, int rank = 0) {
     const int per_chunk = p.n_wtiles * p.ksplit;
-    const long long n_items = (long long)sv.total_chunks * per_chunk;
+    const int32_t *first = K2 ? sv.pair0 : sv.chunk0;
+    const long long n_items = (long long)(K2 ? sv.total_pairs : sv.total_chunks) * per_chunk;
     if (item >= n_items) return false;
-    int lo = 0, hi = sv.n_seg - 1;            // last segment s with chunk0[s] * per_chunk <= item
+    int lo = 0, hi = sv.n_seg - 1;            // last segment s with first[s] * per_chunk <= item
     while (lo < hi) {
         const int mid = (lo + hi + 1) >> 1;
-        if ((long long)sv.chunk0[mid] * per_chunk <= item) lo = mid; else hi = mid - 1;
+        if ((long long)first[mid] * per_chunk <= item) lo = mid; else hi = mid - 1;
     }
     const int s = lo;
     const int u = sv.u[s];
-    const int c0 = sv.chunk0[s];
-    const int chunks_s = sv.chunk0[s + 1] - c0;
+    const int c0 = first[s];
+    const int units_s = first[s + 1] - c0;
     const int local = item - c0 * per_chunk;
-    const int chunk = local % chunks_s;
-    const int rest = local / chunks_s;
+    const int unit = local % units_s;
+    const int rest = local / units_s;
+    int chunk = K2 ? 2 * unit + rank : unit;
     it.u = u;
     it.ks = rest % p.ksplit;
     it.wt = rest / p.ksplit;
     it.shared = u >= p.G;
-    it.n = min(kChunkRows, sv.rows[s] - chunk * kChunkRows);
+    const int rows = sv.rows[s];
+    it.n = min(kChunkRows, rows - chunk * kChunkRows);
+    if (K2 && it.n <= 0) { it.n = 0; chunk = 0; }        // absent half of the last pair: point at real rows
     if (it.shared) {
         it.tok0 = chunk * kChunkRows;
         it.perm_row0 = 0;
@@ -142,7 +151,7 @@ __device__ __forceinline__ float silu_mul(float a, float b) {
     return __fdividef(a, 1.0f + __expf(-a)) * b;
 }
 
-template <int MODE>
+template <int MODE, bool K2 = false>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D]; GEMM2: H [TK+S*T, F]
             const __grid_constant__ CUtensorMap tm_act1,   // GEMM1: x [T, D] (shared experts); GEMM2: unused
@@ -151,6 +160,12 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
             const GemmParams p) {
     constexpr bool kDecode = (MODE == DC_GEMM1 || MODE == DC_GEMM2);
     constexpr bool kGemm1 = (MODE == PF_GEMM1 || MODE == DC_GEMM1);
+    static_assert(!K2 || !kDecode, "CTA pairs are a prefill-tile feature");
+    // K2: the two CTAs of a cluster form a CTA pair; rank 0 (the leader) issues the M = 256 MMAs for both
+    const uint32_t rank = K2 ? ptx::cluster_ctarank() : 0u;
+    const bool leader = rank == 0;
+    const int item0 = K2 ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;
+    const int item_stride = K2 ? (int)(gridDim.x >> 1) : (int)gridDim.x;
 
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -163,7 +178,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
     uint64_t *tempty = tfull + kAccStages;       // [kAccStages]
     uint32_t *tmem_ptr = reinterpret_cast<uint32_t *>(tempty + kAccStages);
     uint8_t *epi_stage = reinterpret_cast<uint8_t *>(bars) + kSmemBars;   // [4][kEpiStageBytes], 256-byte aligned
-    int32_t *s_sched = reinterpret_cast<int32_t *>(epi_stage + (MODE == PF_GEMM2 ? kSmemEpi : 0));   // [4][seg_cap]
+    int32_t *s_sched = reinterpret_cast<int32_t *>(epi_stage + (MODE == PF_GEMM2 ? kSmemEpi : 0));   // [5][seg_cap]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -173,12 +188,16 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
         ptx::prefetch_tmap(&tm_w0);
         if (kGemm1) { ptx::prefetch_tmap(&tm_act1); ptx::prefetch_tmap(&tm_w1); }
         for (int i = 0; i < n_stages; ++i) { ptx::mbar_init(&full[i], 1); ptx::mbar_init(&empty[i], 1); }
-        for (int i = 0; i < kAccStages; ++i) { ptx::mbar_init(&tfull[i], 1); ptx::mbar_init(&tempty[i], 4); }
+        // K2: the leader's tempty collects the 4 epilogue warps of BOTH CTAs
+        for (int i = 0; i < kAccStages; ++i) { ptx::mbar_init(&tfull[i], 1); ptx::mbar_init(&tempty[i], K2 ? 8 : 4); }
         ptx::fence_barrier_init();
     }
-    if (warp == 1) ptx::tmem_alloc(tmem_ptr, kTmemCols);
+    if (warp == 1) {
+        if (K2) ptx::tmem_alloc_pair(tmem_ptr, kTmemCols); else ptx::tmem_alloc(tmem_ptr, kTmemCols);
+    }
     ptx::tc_fence_before();
     __syncthreads();
+    if (K2) ptx::cluster_sync_all();      // both CTAs' barriers exist before either signals the other
     ptx::tc_fence_after();
     const uint32_t tmem_base = *tmem_ptr;
 
@@ -186,7 +205,8 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
     // bytes one stage receives: constant per launch (decode always loads the full padded token box)
     // bytes one stage receives.  Decode: the weight box(es) of R rows plus the item's token rows in 32-row
     // boxes (tok_tx(n)): only the rows the group really has travel from L2.
-    const uint32_t w_tx = !kDecode ? 3u * kTileBytes16K : (uint32_t)((kGemm1 ? 2 : 1) * p.R * 128);
+    // K2: a CTA stages A (16 KB) + its half of B (16 KB); the leader's barrier counts both CTAs' bytes
+    const uint32_t w_tx = K2 ? 4u * kTileBytes16K : !kDecode ? 3u * kTileBytes16K : (uint32_t)((kGemm1 ? 2 : 1) * p.R * 128);
     auto stage_tx_of = [&](int n) -> uint32_t { return kDecode ? w_tx + (uint32_t)((n + 31) >> 5) * 4096u : w_tx; };
 
     // DC_GEMM2: W2 does not depend on the predecessor (GEMM1), so warp 0 fills the ring with the weight tiles
@@ -197,7 +217,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
     bool have0 = false;
     int pre = 0;
     if (MODE == DC_GEMM2 && warp == 0) {
-        have0 = get_item<MODE>(p, sched_global(p.sched), blockIdx.x, it0);
+        have0 = get_item<MODE, false>(p, sched_global(p.sched), blockIdx.x, it0);
         pre = have0 ? min(n_stages, nkb) : 0;
         if (ptx::elect_one())
             for (int kb = 0; kb < pre; ++kb) {
@@ -213,12 +233,15 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
     SchedView sv;
     sv.n_seg = min(p.sched[0], cap - 1);
     sv.total_chunks = p.sched[1];
+    sv.total_pairs = p.sched[2];
     sv.u = s_sched; sv.chunk0 = s_sched + cap; sv.rows = s_sched + 2 * cap; sv.off = s_sched + 3 * cap;
+    sv.pair0 = s_sched + 4 * cap;
     for (int i = threadIdx.x; i <= sv.n_seg; i += kThreads) {
         s_sched[i] = p.sched[kSchedSegU + i];
         s_sched[cap + i] = p.sched[kSchedChunk0 + i];
         s_sched[2 * cap + i] = p.sched[kSchedRows + i];
         s_sched[3 * cap + i] = p.sched[kSchedOff + i];
+        s_sched[4 * cap + i] = p.sched[kSchedPair0 + i];
     }
     __syncthreads();
     if (threadIdx.x == 0) grid_dep_launch();
@@ -231,7 +254,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
         int stage = 0;
         uint32_t phase = 0;
         Item it;
-        int item = blockIdx.x;
+        int item = item0;
         int kb_first = 0;
         bool have;
         if (MODE == DC_GEMM2) {
@@ -247,16 +270,28 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
             stage = pre;
             if (stage == n_stages) { stage = 0; phase = 1; }
         } else {
-            have = get_item<MODE>(p, sv, item, it);
+            have = get_item<MODE, K2>(p, sv, item, it, rank);
         }
-        for (; have; item += gridDim.x, have = get_item<MODE>(p, sv, item, it), kb_first = 0) {
+        for (; have; item += item_stride, have = get_item<MODE, K2>(p, sv, item, it, rank), kb_first = 0) {
             const CUtensorMap *tm_act = (kGemm1 && it.shared) ? &tm_act1 : &tm_act0;
             const int wrow0 = it.wt * p.R;
             int kc = (it.ks * nkb + kb_first) * kBlockK;
             const uint32_t stage_tx = stage_tx_of(it.n);
             for (int kb = kb_first; kb < nkb; ++kb, kc += kBlockK) {
                 ptx::mbar_wait(&empty[stage], phase ^ 1);
-                if (ptx::elect_one()) {
+                if (K2) {
+                    if (ptx::elect_one()) {
+                        uint8_t *st = smem + (size_t)stage * stage_bytes;
+                        if (leader) ptx::mbar_arrive_expect_tx(&full[stage], stage_tx);
+                        ptx::tma_load_2d_pair(st, tm_act, &full[stage], kc, it.act_row0, ptx::kEvictLast);
+                        if (MODE == PF_GEMM1)       // B rows 0-127 = the W1 tile (leader), 128-255 = the W3 tile (peer)
+                            ptx::tma_load_3d_pair(st + kTileBytes16K, leader ? &tm_w0 : &tm_w1, &full[stage], kc, wrow0, it.u,
+                                                  ptx::kEvictFirst);
+                        else                        // each CTA half of the 256 W2 rows
+                            ptx::tma_load_3d_pair(st + kTileBytes16K, &tm_w0, &full[stage], kc, wrow0 + (int)rank * 128, it.u,
+                                                  ptx::kEvictFirst);
+                    }
+                } else if (ptx::elect_one()) {
                     uint8_t *st = smem + (size_t)stage * stage_bytes;
                     ptx::mbar_arrive_expect_tx(&full[stage], stage_tx);
                     if (!kDecode) {
@@ -293,8 +328,10 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
         int acc = 0;
         uint32_t acc_phase = 0;
         Item it;
-        for (int item = blockIdx.x; get_item<MODE>(p, sv, item, it); item += gridDim.x) {
-            const uint32_t idesc = kDecode ? ptx::make_idesc_bf16(128, (it.n + 31) & ~31) : ptx::make_idesc_bf16(128, 256);
+        // K2: only the leader issues MMAs (for both CTAs); the peer's warp 1 just keeps the TMEM allocation
+        for (int item = item0; (!K2 || leader) && get_item<MODE, K2>(p, sv, item, it, rank); item += item_stride) {
+            const uint32_t idesc = kDecode ? ptx::make_idesc_bf16(128, (it.n + 31) & ~31)
+                                           : ptx::make_idesc_bf16(K2 ? 256 : 128, 256);
             ptx::mbar_wait(&tempty[acc], acc_phase ^ 1);
             ptx::tc_fence_after();
             const uint32_t d_tmem = tmem_base + acc * kAccCols;
@@ -306,13 +343,21 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
                     for (int k = 0; k < kBlockK / 16; ++k) {
                         const uint32_t accum = (kb | k) ? 1u : 0u;
                         const uint32_t ko = 2 * k;             // 16 bf16 = 32 bytes = 2 descriptor units
-                        ptx::mma_bf16_ss(d_tmem, ptx::smem_desc(a_lo + ko), ptx::smem_desc(a_lo + b_off + ko), idesc, accum);
+                        if (K2)
+                            ptx::mma_bf16_ss_pair(d_tmem, ptx::smem_desc(a_lo + ko), ptx::smem_desc(a_lo + b_off + ko), idesc, accum);
+                        else
+                            ptx::mma_bf16_ss(d_tmem, ptx::smem_desc(a_lo + ko), ptx::smem_desc(a_lo + b_off + ko), idesc, accum);
                         if (MODE == DC_GEMM1)
                             ptx::mma_bf16_ss(d_tmem + 128, ptx::smem_desc(a_lo + w3_off + ko),
                                              ptx::smem_desc(a_lo + b_off + ko), idesc, accum);
                     }
-                    ptx::mma_commit(&empty[stage]);                  // frees the smem stage when the MMAs retire
-                    if (kb == nkb - 1) ptx::mma_commit(&tfull[acc]);   // accumulator complete
+                    if (K2) {       // the same barriers in both CTAs
+                        ptx::mma_commit_pair(&empty[stage]);
+                        if (kb == nkb - 1) ptx::mma_commit_pair(&tfull[acc]);
+                    } else {
+                        ptx::mma_commit(&empty[stage]);                  // frees the smem stage when the MMAs retire
+                        if (kb == nkb - 1) ptx::mma_commit(&tfull[acc]);   // accumulator complete
+                    }
                 }
                 __syncwarp();
                 a_lo += stage_step;
@@ -327,7 +372,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
         int acc = 0;
         uint32_t acc_phase = 0;
         Item it;
-        for (int item = blockIdx.x; get_item<MODE>(p, sv, item, it); item += gridDim.x) {
+        for (int item = item0; get_item<MODE, K2>(p, sv, item, it, rank); item += item_stride) {
             ptx::mbar_wait(&tfull[acc], acc_phase);
             ptx::tc_fence_after();
             const uint32_t t_addr = tmem_base + acc * kAccCols + ((uint32_t)(q * 32) << 16);
@@ -464,16 +509,20 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
             // release the accumulator stage
             ptx::tc_fence_before();
             __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(&tempty[acc]);
+            if (lane == 0) {
+                if (K2) ptx::mbar_arrive_cluster(ptx::mapa_u32(&tempty[acc], 0));      // the leader's barrier
+                else ptx::mbar_arrive(&tempty[acc]);
+            }
             if (++acc == kAccStages) { acc = 0; acc_phase ^= 1; }
         }
     }
 
     ptx::tc_fence_before();
     __syncthreads();
+    if (K2) ptx::cluster_sync_all();      // the peer's shared memory, barriers and TMEM stay alive until both are done
     if (warp == 1) {
         ptx::tc_fence_after();
-        ptx::tmem_dealloc(tmem_base, kTmemCols);
+        if (K2) ptx::tmem_dealloc_pair(tmem_base, kTmemCols); else ptx::tmem_dealloc(tmem_base, kTmemCols);
     }
 }
 
@@ -505,7 +554,7 @@ prep_kernel(const bm_bf16 *__restrict__ x, int T, int D, int K, int G, int S,
         __syncthreads();
         if (threadIdx.x < 32) {
             const int lane = threadIdx.x;
-            int seg_base = 0, chunk_base = 0;
+            int seg_base = 0, chunk_base = 0, pair_base = 0;
             for (int u0 = 0; u0 < n; u0 += 32) {
                 const int u = u0 + lane;
                 const int rows = u < n ? s_rows[u] : 0;
@@ -513,25 +562,31 @@ prep_kernel(const bm_bf16 *__restrict__ x, int T, int D, int K, int G, int S,
                 const int ch = ne ? (rows + kChunkRows - 1) / kChunkRows : 0;
                 const unsigned m = __ballot_sync(kFullMask, ne);
                 const int seg = seg_base + __popc(m & ((1u << lane) - 1u));
-                int inc = ch;
+                const int pr = (ch + 1) >> 1;
+                int inc = ch, incp = pr;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
                     const int v = __shfl_up_sync(kFullMask, inc, o);
-                    if (lane >= o) inc += v;
+                    const int vp = __shfl_up_sync(kFullMask, incp, o);
+                    if (lane >= o) { inc += v; incp += vp; }
                 }
                 if (ne) {
                     sched[kSchedSegU + seg] = u;
                     sched[kSchedChunk0 + seg] = chunk_base + inc - ch;
                     sched[kSchedRows + seg] = rows;
                     sched[kSchedOff + seg] = s_off[u];
+                    sched[kSchedPair0 + seg] = pair_base + incp - pr;
                 }
                 seg_base += __popc(m);
                 chunk_base += __shfl_sync(kFullMask, inc, 31);
+                pair_base += __shfl_sync(kFullMask, incp, 31);
             }
             if (lane == 0) {
                 sched[kSchedChunk0 + seg_base] = chunk_base;
+                sched[kSchedPair0 + seg_base] = pair_base;
                 sched[0] = seg_base;
                 sched[1] = chunk_base;
+                sched[2] = pair_base;
                 if (s_bad) atomicOr(status, BM_DEV_BAD_ROUTING);
             }
         }
@@ -577,13 +632,14 @@ dense_sched_kernel(int32_t *__restrict__ sched, int E, int T) {
     const int cps = (T + kChunkRows - 1) / kChunkRows;
     for (int j = threadIdx.x; j <= E; j += blockDim.x) {
         sched[kSchedChunk0 + j] = j * cps;
+        sched[kSchedPair0 + j] = j * ((cps + 1) >> 1);
         if (j < E) {
             sched[kSchedSegU + j] = j;
             sched[kSchedRows + j] = T;
             sched[kSchedOff + j] = 0;
         }
     }
-    if (threadIdx.x == 0) { sched[0] = E; sched[1] = E * cps; }
+    if (threadIdx.x == 0) { sched[0] = E; sched[1] = E * cps; sched[2] = E * ((cps + 1) >> 1); }
 }
 
 // Prefill combine (F2): out[t] = sum_{s < n_slots[t]} gate_w[t,s] * y[slot_row[t,s]]  (slot order)
@@ -738,12 +794,12 @@ void choose_decode_tiling(int wrows, int kblocks, int n_seg, bool allow_split, i
     *ks_out = bestKs;
 }
 
-size_t sched_smem_bytes(int seg_cap) { return ((size_t)4 * seg_cap * sizeof(int32_t) + 255) & ~(size_t)255; }
+size_t sched_smem_bytes(int seg_cap) { return ((size_t)5 * seg_cap * sizeof(int32_t) + 255) & ~(size_t)255; }
 
-void ring_geometry(bool decode, bool gemm1, int T, GemmParams *p) {
+void ring_geometry(bool decode, bool gemm1, int T, GemmParams *p, bool pair = false) {
     p->tail_pad = 0;
     if (!decode) {
-        p->stage_bytes = 3 * kTileBytes16K;
+        p->stage_bytes = (pair ? 2 : 3) * kTileBytes16K;      // a CTA of a pair stages half of the B rows
         p->off_b = kTileBytes16K;
         p->wslot = kTileBytes16K;
     } else {
@@ -768,10 +824,10 @@ void ring_geometry(bool decode, bool gemm1, int T, GemmParams *p) {
     p->stages = st;
 }
 
-template <int MODE>
+template <int MODE, bool K2 = false>
 cudaError_t launch_gemm(const CUtensorMap &a0, const CUtensorMap &a1, const CUtensorMap &w0, const CUtensorMap &w1,
                         const GemmParams &p, cudaStream_t stream) {
-    auto kern = gemm_kernel<MODE>;
+    auto kern = gemm_kernel<MODE, K2>;
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
@@ -782,7 +838,23 @@ cudaError_t launch_gemm(const CUtensorMap &a0, const CUtensorMap &a1, const CUte
     const size_t smem = 1024 + (size_t)p.stages * p.stage_bytes + kSmemBars + (MODE == PF_GEMM2 ? kSmemEpi : 0) +
                         sched_smem_bytes(p.seg_cap) + (size_t)p.tail_pad;
     profile_begin(kid, stream);
-    cudaError_t e = launch_kernel(kern, dim3(num_sms()), dim3(kThreads), smem, stream, a0, a1, w0, w1, p);
+    cudaError_t e;
+    if (!K2) {
+        e = launch_kernel(kern, dim3(num_sms()), dim3(kThreads), smem, stream, a0, a1, w0, w1, p);
+    } else {
+        // CTA pairs: clusters of two CTAs (one TPC each), one pair per two SMs
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(num_sms() & ~1); cfg.blockDim = dim3(kThreads); cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+        cudaLaunchAttribute attr[2];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[1].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = pdl_enabled() ? 2 : 1;
+        count_launch();
+        e = cudaLaunchKernelEx(&cfg, kern, a0, a1, w0, w1, p);
+    }
     profile_end(kid, stream);
     return e;
 }
@@ -821,11 +893,24 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
             !make_map_3d(&m_w2, a.W2, a.G + a.S, a.D, a.F, 256) || !make_map_2d(&m_h, a.h, h_rows, a.F, 128))
             return cudaErrorInvalidValue;
         p.ksplit = 1;
-        ring_geometry(false, true, a.T, &p);
+        // CTA pairs (cta_group::2, M = 256 per pair): a pair shares the weight tile, so a CTA stages 32 KB per
+        // k-block instead of 48 KB (measured: GEMM1 232 -> 201 us at BJ:configs[3]).  A segment with an odd chunk
+        // count wastes half a pair, so pairs are used when a group expects >= 4 chunks (measured: no gain at
+        // 273 rows/group, 7% slower at 107 rows/group).  BM_PF_PAIR=0/1 overrides.
+        const int pair_env = tune_int("BM_PF_PAIR", -1);
+        const bool many_rows = (long long)a.T * a.K >= 4LL * kChunkRows * a.G;
+        const bool pair = (sms & 1) == 0 && (pair_env < 0 ? many_rows : pair_env != 0);
+        CUtensorMap m_w2h;
+        if (pair && !make_map_3d(&m_w2h, a.W2, a.G + a.S, a.D, a.F, 128)) return cudaErrorInvalidValue;
+        ring_geometry(false, true, a.T, &p, pair);
         p.kblocks = kb1; p.R = 128; p.n_wtiles = (a.F + 127) / 128;
-        if ((err = launch_gemm<PF_GEMM1>(m_xs, m_x, m_w1, m_w3, p, stream)) != cudaSuccess) return err;
+        err = pair ? launch_gemm<PF_GEMM1, true>(m_xs, m_x, m_w1, m_w3, p, stream)
+                   : launch_gemm<PF_GEMM1>(m_xs, m_x, m_w1, m_w3, p, stream);
+        if (err != cudaSuccess) return err;
         p.kblocks = kb2; p.R = 256; p.n_wtiles = (a.D + 255) / 256;
-        if ((err = launch_gemm<PF_GEMM2>(m_h, m_h, m_w2, m_w2, p, stream)) != cudaSuccess) return err;
+        err = pair ? launch_gemm<PF_GEMM2, true>(m_h, m_h, m_w2h, m_w2h, p, stream)
+                   : launch_gemm<PF_GEMM2>(m_h, m_h, m_w2, m_w2, p, stream);
+        if (err != cudaSuccess) return err;
     } else {
         // segments expected to be non-empty (host guess; the data-dependent truth lives on the device)
         int n_seg = a.G < TK ? a.G : TK;
@@ -879,15 +964,17 @@ cudaError_t launch_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 
     p.T = T; p.D = D; p.F = F; p.K = 1; p.G = 0; p.S = E; p.TK = 0;
     p.sched = sched; p.h = h; p.y = y;
     p.ksplit = 1;
+    const bool pair = (num_sms() & 1) == 0 && T >= 4 * kChunkRows && tune_int("BM_PF_PAIR", -1) != 0;   // as launch_forward_tc
     CUtensorMap m_x, m_w1, m_w3, m_w2, m_h;
     if (!make_map_2d(&m_x, x, T, D, 128) || !make_map_3d(&m_w1, W1, E, F, D, 128) || !make_map_3d(&m_w3, W3, E, F, D, 128) ||
-        !make_map_3d(&m_w2, W2, E, D, F, 256) || !make_map_2d(&m_h, h, (uint64_t)E * T, F, 128))
+        !make_map_3d(&m_w2, W2, E, D, F, pair ? 128 : 256) || !make_map_2d(&m_h, h, (uint64_t)E * T, F, 128))
         return cudaErrorInvalidValue;
-    ring_geometry(false, true, T, &p);
+    ring_geometry(false, true, T, &p, pair);
     p.kblocks = (D + kBlockK - 1) / kBlockK; p.R = 128; p.n_wtiles = (F + 127) / 128;
-    if ((err = launch_gemm<PF_GEMM1>(m_x, m_x, m_w1, m_w3, p, stream)) != cudaSuccess) return err;
+    err = pair ? launch_gemm<PF_GEMM1, true>(m_x, m_x, m_w1, m_w3, p, stream) : launch_gemm<PF_GEMM1>(m_x, m_x, m_w1, m_w3, p, stream);
+    if (err != cudaSuccess) return err;
     p.kblocks = (F + kBlockK - 1) / kBlockK; p.R = 256; p.n_wtiles = (D + 255) / 256;
-    return launch_gemm<PF_GEMM2>(m_h, m_h, m_w2, m_w2, p, stream);
+    return pair ? launch_gemm<PF_GEMM2, true>(m_h, m_h, m_w2, m_w2, p, stream) : launch_gemm<PF_GEMM2>(m_h, m_h, m_w2, m_w2, p, stream);
 }
 
 }  // namespace bm
