@@ -68,25 +68,36 @@ __device__ __forceinline__ void warp_permute(const int32_t *__restrict__ group_i
 }
 
 // Block-wide exclusive scan of v[0..n) (n <= 512) in shared memory; returns the total in *total.
+// Exclusive scan of v[0..n) (n <= 512, shared memory) in place; *total = sum.  Warp 0 does it: lane l owns the 16
+// consecutive slots 16l..16l+15 (serial prefix), the lane totals are scanned with shuffles.  Ends with a barrier.
 __device__ void block_exclusive_scan(int *v, int n, int *tmp, int *total) {
-    // Hillis-Steele over 512 slots by the first 256 threads of the block, two slots per thread
-    for (int i = threadIdx.x; i < 512; i += blockDim.x) tmp[i] = i < n ? v[i] : 0;
+    (void)tmp;
     __syncthreads();
-    const bool act = threadIdx.x < 256;
-    for (int d = 1; d < 512; d <<= 1) {
-        int a0 = 0, a1 = 0;
-        const int i0 = threadIdx.x, i1 = threadIdx.x + 256;
-        if (act && i0 >= d) a0 = tmp[i0 - d];
-        if (act && i1 >= d) a1 = tmp[i1 - d];
-        __syncthreads();
-        if (act) {
-            tmp[i0] += a0;
-            tmp[i1] += a1;
+    if (threadIdx.x < 32) {
+        const int lane = threadIdx.x;
+        int loc[16];
+        int sum = 0;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            const int idx = lane * 16 + i;
+            const int x = idx < n ? v[idx] : 0;
+            loc[i] = sum;
+            sum += x;
         }
-        __syncthreads();
+        int inc = sum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int y = __shfl_up_sync(kFullMask, inc, o);
+            if (lane >= o) inc += y;
+        }
+        const int base = inc - sum;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            const int idx = lane * 16 + i;
+            if (idx < n) v[idx] = base + loc[i];
+        }
+        if (lane == 31) *total = inc;
     }
-    for (int i = threadIdx.x; i < n; i += blockDim.x) v[i] = tmp[i] - v[i];   // inclusive -> exclusive
-    if (threadIdx.x == 0) *total = n > 0 ? tmp[n - 1] : 0;
     __syncthreads();
 }
 
