@@ -221,3 +221,22 @@ def test_prefill_path_is_deterministic():
     _, out1, _ = gpu_layer(L, PATHS["prefill"], d)
     _, out2, _ = gpu_layer(L, PATHS["prefill"], d)
     assert (out1 == out2).all()
+
+
+@pytest.mark.parametrize("T,D,F,E,K,G,S", FWD_SHAPES + [(1100, 256, 384, 6, 2, 3, 0), (2048, 128, 256, 4, 1, 2, 1)])
+def test_prefill_cta_pairs_forced_on_ragged_shapes(T, D, F, E, K, G, S, monkeypatch):
+    """The CTA-pair prefill tiles (cta_group::2) are normally used only when a group expects >= 4 chunks; forcing
+    them (BM_PF_PAIR=1, read on every call) on small and ragged shapes exercises odd chunk counts (a pair whose
+    second CTA has no rows), single-chunk segments and shared experts."""
+    monkeypatch.setenv("BM_PF_PAIR", "1")
+    rng = np.random.default_rng(T * 11 + F)
+    L = rand_layer(rng, T=T, D=D, F=F, E=E, K=K, G=G, S=S, bias=True, wstd=0.02 if D >= 1024 else 0.05)
+    g, out, status = gpu_layer(L, PATHS["prefill"])
+    o = oracle_route(L)
+    assert status == 0
+    assert_routing_equal(g, o)
+    assert_out_close(out, oracle_forward(L, o))
+    monkeypatch.setenv("BM_PF_PAIR", "0")
+    _, out1, _ = gpu_layer(L, PATHS["prefill"])
+    # same tiles, same k order, same epilogue: the pair and the single-CTA kernels agree bit for bit
+    assert (out == out1).all()
