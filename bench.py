@@ -154,10 +154,13 @@ def max_over_ranks(v: float, ws: int, device) -> float:
 class DeviceLayer:
     """One layer resident in HBM: weights, router, group map, workspace, routing arrays."""
 
-    def __init__(self, cfg, seed, x_seed, weights_from=None, keep_host_weights=False):
+    def __init__(self, cfg, seed, x_seed, weights_from=None, keep_host_weights=False, tp=None):
         import paper_2607_04164_b200 as bm
         self.bm, self.cfg = bm, cfg
+        self.tp = tp                       # (rank, world): tensor parallelism over F, else None
         L = make_layer(cfg, seed, weights=weights_from is None)
+        if tp is not None:
+            L.W1, L.W3, L.W2 = bm.shard_f(L.W1, L.W3, L.W2, *tp)
         if x_seed != seed:   # ranks share the layer, not the tokens
             L.x = make_layer(cfg, x_seed, weights=False).x
         self.host = L
@@ -171,7 +174,8 @@ class DeviceLayer:
                 L.W1 = L.W3 = L.W2 = None      # free the host copies (1.4 - 2.8 GB)
         else:
             self.W1, self.W3, self.W2 = weights_from.W1, weights_from.W3, weights_from.W2
-        self.ws = bm.alloc_workspace(cfg.T, cfg.D, cfg.F, cfg.E, cfg.K, cfg.G, cfg.S)
+        self.ws = bm.alloc_workspace(cfg.T, cfg.D, self.W1.shape[1], cfg.E, cfg.K, cfg.G, cfg.S)
+        self.partial = torch.empty((cfg.T, cfg.D), dtype=torch.float32, device="cuda") if tp is not None else None
         self.routing = bm.Routing(cfg.T, cfg.K, cfg.G)
         self.out = torch.empty((cfg.T, cfg.D), dtype=torch.bfloat16, device="cuda")
         self.x_pinned = L.x.pin_memory()
@@ -181,7 +185,10 @@ class DeviceLayer:
     def step(self):
         bm, c = self.bm, self.cfg
         bm.bm_route(self.x, self.W_router, self.bias, c.K, self.gmap, c.G, self.routing, self.ws)
-        bm.bm_moe_forward(self.x, self.routing, self.W1, self.W3, self.W2, self.out, self.ws, S=c.S)
+        if self.tp is not None:     # F-sharded weights: fp32 partial, NCCL all-reduce, one rounding
+            bm.tp_moe_forward(self.x, self.routing, self.W1, self.W3, self.W2, self.out, self.ws, S=c.S, partial=self.partial)
+        else:
+            bm.bm_moe_forward(self.x, self.routing, self.W1, self.W3, self.W2, self.out, self.ws, S=c.S)
 
     def step_host(self):
         bm, c = self.bm, self.cfg
@@ -254,15 +261,18 @@ def measure(layer, steps, warmup, ws, device, peaks, sampler=None, with_e2e=True
     status = bm.bm_device_status(layer.ws)
     A, G_act, counts = layer.realised()
     flops, nbytes, t_flop, t_hbm = roofline_times(cfg, A, G_act, peaks)
+    if getattr(layer, "tp", None) is not None:      # F sharded over ws GPUs: the roofline of the whole job has ws x the peaks
+        t_flop, t_hbm = t_flop / ws, t_hbm / ws
     t_step = t / steps
-    res = dict(tokens_per_s=ws * cfg.T / t_step, ms_per_step=t_step * 1e3, A=A, G_act=G_act, counts=counts,
+    n_rep = 1 if getattr(layer, "tp", None) is not None else ws      # tp: all ranks work on the same tokens
+    res = dict(tokens_per_s=n_rep * cfg.T / t_step, ms_per_step=t_step * 1e3, A=A, G_act=G_act, counts=counts,
                flops=flops, bytes=nbytes, t_flop_us=t_flop * 1e6, t_hbm_us=t_hbm * 1e6,
                bound="hbm" if t_hbm >= t_flop else "tensor", roofline_frac=max(t_flop, t_hbm) / t_step,
                achieved_gbs=nbytes / t_step / 1e9, achieved_tflops=flops / t_step / 1e12,
                launches_per_step=launches_per_step, gpu_launches=launches_per_step * steps, device_status=status)
-    if with_e2e:
+    if with_e2e and getattr(layer, "tp", None) is None:
         te = timed_loop(layer.step_host, max(steps // 2, 3), max(warmup // 2, 3), ws, device)
-        res["e2e_tokens_per_s"] = ws * cfg.T / (te / max(steps // 2, 3))
+        res["e2e_tokens_per_s"] = n_rep * cfg.T / (te / max(steps // 2, 3))
     # dominant kernel: GEMM1 + SwiGLU (two thirds of the weight bytes / FLOPs)
     ps = prof_steps or min(steps, 50)
     kt, n = kernel_time(layer, "gemm1", ps, 3)
@@ -328,7 +338,9 @@ def run_ours(args):
     cfg = get_config(args.config)
     steps, warmup = args.steps, max(args.warmup, 3)
 
-    layer = DeviceLayer(cfg, seed=0, x_seed=rank, keep_host_weights=(rank == 0 and ws == 1 and not args.no_cpu))
+    tp = (rank, ws) if (args.parallel == "tp" and ws > 1) else None
+    # dp: every rank its own tokens (weak scaling); tp: the same tokens on every rank, F sharded (strong scaling)
+    layer = DeviceLayer(cfg, seed=0, x_seed=0 if tp else rank, keep_host_weights=(rank == 0 and ws == 1 and not args.no_cpu), tp=tp)
     sampler = ClockSampler(local_rank)
     main = measure(layer, steps, warmup, ws, device, peaks, sampler, breakdown=True)
     clocks = sampler.summary()
@@ -374,11 +386,12 @@ def run_ours(args):
         weight_bytes = (cfg.G + cfg.S) * 3 * cfg.D * cfg.F * 2
         line = dict(
             metric=METRIC, value=main["tokens_per_s"], unit=UNIT, n_gpus=ws, steps=steps, warmup=warmup,
-            ms_per_step=main["ms_per_step"], higher_is_better=True, scaling="weak", vs_baseline=None,
+            ms_per_step=main["ms_per_step"], higher_is_better=True, scaling="strong" if tp else "weak", vs_baseline=None,
             dtype="bf16", data="synthetic",
             config=dict(workload=f"BASELINE.json configs[{ {'tiny':0,'decode':1,'prefill':2,'finegrained':3}.get(args.config, 4)}] '{cfg.name}': "
                                  f"T={cfg.T} D={cfg.D} F={cfg.F} E={cfg.E} top-{cfg.K} G={cfg.G} S={cfg.S} zipf_s={cfg.zipf_s}, seed 0",
-                        tokens_per_step_per_gpu=cfg.T, parallelism=f"dp{ws} (tokens sharded, weights replicated, no collective)",
+                        tokens_per_step_per_gpu=cfg.T, parallelism=(f"tp{ws} (F sharded, routing replicated, one fp32 all-reduce of out per layer)" if tp
+                                     else f"dp{ws} (tokens sharded, weights replicated, no collective)"),
                         l2=f"weights {weight_bytes / 1e6:.0f} MB per step "
                            + ("> 126 MB L2: streamed from HBM every step, no flush needed" if weight_bytes > 2 * L2_BYTES
                               else "<= L2: NOT cold (small config)"),
@@ -426,7 +439,8 @@ class SweepPoint:
         L = make_layer(cfg, 0, weights=False)
         self.x = L.x.cuda()
         self.bias = None if L.router_bias is None else L.router_bias.cuda()
-        self.ws = bm.alloc_workspace(cfg.T, cfg.D, cfg.F, cfg.E, cfg.K, cfg.G, cfg.S)
+        self.ws = bm.alloc_workspace(cfg.T, cfg.D, self.W1.shape[1], cfg.E, cfg.K, cfg.G, cfg.S)
+        self.partial = torch.empty((cfg.T, cfg.D), dtype=torch.float32, device="cuda") if tp is not None else None
         self.routing = bm.Routing(cfg.T, cfg.K, cfg.G)
         self.out = torch.empty((cfg.T, cfg.D), dtype=torch.bfloat16, device="cuda")
         self.i = 0
@@ -716,6 +730,8 @@ def main():
                          "sweep_G8_T256_s1" % sorted(CONFIGS))
     ap.add_argument("--sweep-filter", default="", help="comma-separated name parts, e.g. G8,T16 (with --config sweep)")
     ap.add_argument("--out", default="", help="also write the sweep result to this file")
+    ap.add_argument("--parallel", default="dp", choices=["dp", "tp"],
+                    help="N > 1: dp = tokens sharded, no collective (default); tp = F sharded + all-reduce (P:289-295)")
     ap.add_argument("--no-extras", action="store_true", help="skip the ungrouped / prefill side measurements")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()

@@ -176,6 +176,21 @@ int bm_moe_forward(const bm_bf16 *x, int T, int D, const bm_routing *routing, co
                    const bm_bf16 *W3, const bm_bf16 *W2, int F, int S, bm_bf16 *out, void *workspace,
                    size_t workspace_bytes, bm_stream_t stream);
 
+/*
+ * Tensor parallelism over F (the paper scales with tensor parallelism).
+ * SwiGLU is elementwise over the F hidden features, so with W1, W3 row-sharded and W2 column-sharded over N ranks
+ *     FFN_u(x) = sum_r W2_r[u] . ( SiLU(W1_r[u] x) * (W3_r[u] x) ),     W1_r, W3_r [G+S, F/N, D],  W2_r [G+S, D, F/N]
+ * and the layer output is the sum over ranks of the per-rank layer outputs (routing is replicated).
+ * bm_moe_forward_f32 is bm_moe_forward on one rank's shard that leaves the fp32 sums in out_f32 [T,D] (no bf16
+ * rounding); the caller all-reduces out_f32 over the ranks (NCCL, torch.distributed) and rounds once with
+ * bm_round_bf16.  out_f32 is overwritten.  The SIMT cross-check path has no fp32 variant.
+ * bm_round_bf16: out[i] = bf16(in[i]), round to nearest even, n % 8 == 0.
+ */
+int bm_moe_forward_f32(const bm_bf16 *x, int T, int D, const bm_routing *routing, const bm_bf16 *W1,
+                       const bm_bf16 *W3, const bm_bf16 *W2, int F, int S, float *out_f32, void *workspace,
+                       size_t workspace_bytes, bm_stream_t stream);
+int bm_round_bf16(const float *in, size_t n, bm_bf16 *out, bm_stream_t stream);
+
 /* Same as bm_moe_forward with the execution path forced (BM_PATH_*); used by tests and the bench to
  * exercise every path on any shape.  BM_ERR_PATH if the path cannot run the shape. */
 int bm_moe_forward_path(const bm_bf16 *x, int T, int D, const bm_routing *routing, const bm_bf16 *W1,

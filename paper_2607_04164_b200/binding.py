@@ -21,7 +21,7 @@ BM_DECODE_MAX_T = 256
 
 EXPORTS = ["bm_workspace_bytes", "bm_route", "bm_route_partial", "bm_unite_weights", "bm_expert_histogram",
            "bm_expert_outputs", "bm_gram_workspace_bytes", "bm_cosine_gram", "bm_mse_workspace_bytes", "bm_group_mse",
-           "bm_moe_forward", "bm_moe_forward_path", "bm_moe_layer_host",
+           "bm_moe_forward", "bm_moe_forward_path", "bm_moe_forward_f32", "bm_round_bf16", "bm_moe_layer_host",
            "bm_device_status", "bm_launch_count", "bm_status_string", "bm_profile_enable", "bm_profile_read"]
 KERNELS = {"router": 1, "permute": 2, "prep": 3, "gemm1": 4, "gemm2": 5, "finalize": 6}
 
@@ -75,6 +75,10 @@ def lib() -> ctypes.CDLL:
         L.bm_moe_forward.restype = c_int
         L.bm_moe_forward.argtypes = [c_void_p, c_int, c_int, POINTER(BmRouting), c_void_p, c_void_p, c_void_p,
                                      c_int, c_int, c_void_p, c_void_p, c_size_t, c_void_p]
+        L.bm_moe_forward_f32.restype = c_int
+        L.bm_moe_forward_f32.argtypes = L.bm_moe_forward.argtypes
+        L.bm_round_bf16.restype = c_int
+        L.bm_round_bf16.argtypes = [c_void_p, c_size_t, c_void_p, c_void_p]
         L.bm_moe_forward_path.restype = c_int
         L.bm_moe_forward_path.argtypes = L.bm_moe_forward.argtypes + [c_int]
         L.bm_moe_layer_host.restype = c_int
@@ -253,6 +257,27 @@ def bm_moe_forward(x, routing: Routing, W1, W3, W2, out, workspace, S: int = 0, 
                                    _ptr(out), _ptr(workspace), workspace.numel(), _stream(stream), path)
     if rc != BM_OK:
         raise BmError(rc, "bm_moe_forward")
+    return out
+
+
+def bm_moe_forward_f32(x, routing: Routing, W1, W3, W2, out_f32, workspace, S: int = 0, stream=None):
+    """One rank's fp32 partial of a layer whose F dimension is sharded (include/bm.h: bm_moe_forward_f32)."""
+    T, D = x.shape
+    F = W1.shape[1]
+    rc = lib().bm_moe_forward_f32(_ptr(x), T, D, ctypes.byref(routing.c), _ptr(W1), _ptr(W3), _ptr(W2), F, S,
+                                  _ptr(out_f32), _ptr(workspace), workspace.numel(), _stream(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_moe_forward_f32")
+    return out_f32
+
+
+def bm_round_bf16(src, out=None, stream=None):
+    """bf16(fp32), round to nearest even (include/bm.h: bm_round_bf16)."""
+    if out is None:
+        out = torch.empty(src.shape, dtype=torch.bfloat16, device=src.device)
+    rc = lib().bm_round_bf16(_ptr(src), src.numel(), _ptr(out), _stream(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_round_bf16")
     return out
 
 

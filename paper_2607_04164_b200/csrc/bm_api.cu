@@ -215,21 +215,22 @@ int bm_group_mse(const bm_bf16 *Y, const bm_bf16 *U, int T, int D, const int32_t
                ? BM_OK : BM_ERR_CUDA;
 }
 
-int bm_moe_forward_path(const bm_bf16 *x, int T, int D, const bm_routing *routing, const bm_bf16 *W1,
-                        const bm_bf16 *W3, const bm_bf16 *W2, int F, int S, bm_bf16 *out, void *workspace,
-                        size_t workspace_bytes, bm_stream_t stream, int path) {
+static int forward_common(const bm_bf16 *x, int T, int D, const bm_routing *routing, const bm_bf16 *W1,
+                          const bm_bf16 *W3, const bm_bf16 *W2, int F, int S, bm_bf16 *out, float *out_f32,
+                          void *workspace, size_t workspace_bytes, bm_stream_t stream, int path) {
     if (!routing) return BM_ERR_NULL;
     const int K = routing->K, G = routing->G;
     int rc = check_shapes(T, D, F, routing->E, K, G, S, true);
     if (rc != BM_OK) return rc;
     if (routing->T != T) return BM_ERR_SHAPE;
     if (path < BM_PATH_AUTO || path > BM_PATH_SIMT) return BM_ERR_PATH;
+    if (out_f32 && path == BM_PATH_SIMT) return BM_ERR_PATH;
     if (T == 0) return BM_OK;
-    if (!x || !W1 || !W3 || !W2 || !out || !workspace || !routing->group_ids || !routing->gate_w ||
+    if (!x || !W1 || !W3 || !W2 || (!out && !out_f32) || !workspace || !routing->group_ids || !routing->gate_w ||
         !routing->n_slots || !routing->counts || !routing->offsets || !routing->row_token || !routing->row_slot ||
         !routing->slot_row)
         return BM_ERR_NULL;
-    if (!aligned16(x) || !aligned16(W1) || !aligned16(W3) || !aligned16(W2) || !aligned16(out) ||
+    if (!aligned16(x) || !aligned16(W1) || !aligned16(W3) || !aligned16(W2) || !aligned16(out) || !aligned16(out_f32) ||
         !aligned16(workspace))
         return BM_ERR_ALIGN;
     const Workspace w = workspace_layout(T, D, F, K, G, S);
@@ -249,7 +250,7 @@ int bm_moe_forward_path(const bm_bf16 *x, int T, int D, const bm_routing *routin
     ForwardArgs a{};
     a.x = x; a.T = T; a.D = D; a.F = F; a.K = K; a.G = G; a.S = S;
     a.r = *routing;
-    a.W1 = W1; a.W3 = W3; a.W2 = W2; a.out = out;
+    a.W1 = W1; a.W3 = W3; a.W2 = W2; a.out = out; a.out_f32 = out_f32;
     a.status = reinterpret_cast<int32_t *>(ws + w.status);
     a.sched = reinterpret_cast<int32_t *>(ws + w.sched);
     a.xs = reinterpret_cast<bm_bf16 *>(ws + w.xs);
@@ -261,6 +262,30 @@ int bm_moe_forward_path(const bm_bf16 *x, int T, int D, const bm_routing *routin
     if (path == BM_PATH_SIMT) e = launch_forward_simt(a, st);
     else e = launch_forward_tc(a, path == BM_PATH_DECODE, st);
     return e == cudaSuccess ? BM_OK : BM_ERR_CUDA;
+}
+
+int bm_moe_forward_path(const bm_bf16 *x, int T, int D, const bm_routing *routing, const bm_bf16 *W1,
+                        const bm_bf16 *W3, const bm_bf16 *W2, int F, int S, bm_bf16 *out, void *workspace,
+                        size_t workspace_bytes, bm_stream_t stream, int path) {
+    if (!out && T > 0) return BM_ERR_NULL;
+    return forward_common(x, T, D, routing, W1, W3, W2, F, S, out, nullptr, workspace, workspace_bytes, stream, path);
+}
+
+int bm_moe_forward_f32(const bm_bf16 *x, int T, int D, const bm_routing *routing, const bm_bf16 *W1, const bm_bf16 *W3,
+                       const bm_bf16 *W2, int F, int S, float *out_f32, void *workspace, size_t workspace_bytes,
+                       bm_stream_t stream) {
+    if (!out_f32 && T > 0) return BM_ERR_NULL;
+    return forward_common(x, T, D, routing, W1, W3, W2, F, S, nullptr, out_f32, workspace, workspace_bytes, stream,
+                          BM_PATH_AUTO);
+}
+
+int bm_round_bf16(const float *in, size_t n, bm_bf16 *out, bm_stream_t stream) {
+    if (n % 8 != 0) return BM_ERR_SHAPE;
+    if (n == 0) return BM_OK;
+    if (!in || !out) return BM_ERR_NULL;
+    if (!aligned16(in) || !aligned16(out)) return BM_ERR_ALIGN;
+    if (device_ok() != 1) return BM_ERR_CUDA;
+    return launch_round_bf16(in, n, out, reinterpret_cast<cudaStream_t>(stream)) == cudaSuccess ? BM_OK : BM_ERR_CUDA;
 }
 
 int bm_moe_forward(const bm_bf16 *x, int T, int D, const bm_routing *routing, const bm_bf16 *W1, const bm_bf16 *W3,

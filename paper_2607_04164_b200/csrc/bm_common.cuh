@@ -112,6 +112,7 @@ struct ForwardArgs {
     bm_bf16 *h;
     float *out_acc;
     bm_bf16 *y;
+    float *out_f32;      // non-null: leave the fp32 sums here instead of writing bf16 `out` (tensor-parallel partial)
 };
 
 cudaError_t launch_unite(const bm_bf16 *W, int E, size_t n, const int32_t *gmap, int G, bm_bf16 *out,
@@ -128,6 +129,8 @@ cudaError_t launch_gram(const bm_bf16 *Y, int E, size_t n, float *gram, float *c
 int mse_blocks();
 cudaError_t launch_group_mse(const bm_bf16 *Y, const bm_bf16 *U, int T, int D, const int32_t *w, const int32_t *gmap,
                              int E, int G, float *mse, float *mse_total, float *part, cudaStream_t stream);
+
+cudaError_t launch_round_bf16(const float *in, size_t n, bm_bf16 *out, cudaStream_t stream);
 
 cudaError_t launch_forward_simt(const ForwardArgs &a, cudaStream_t stream);
 cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t stream);

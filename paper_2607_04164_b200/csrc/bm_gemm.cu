@@ -649,7 +649,8 @@ dense_sched_kernel(int32_t *__restrict__ sched, int E, int T) {
 // step), four source rows in flight.
 __global__ void __launch_bounds__(256)
 combine_kernel(const bm_bf16 *__restrict__ y, int T, int D, int K, int S, const int32_t *__restrict__ n_slots,
-               const int32_t *__restrict__ slot_row, const float *__restrict__ gate_w, bm_bf16 *__restrict__ out) {
+               const int32_t *__restrict__ slot_row, const float *__restrict__ gate_w, bm_bf16 *__restrict__ out,
+               float *__restrict__ out_f32) {
     grid_dep_wait();
     grid_dep_launch();
     const int lane = threadIdx.x & 31;
@@ -694,9 +695,15 @@ combine_kernel(const bm_bf16 *__restrict__ y, int T, int D, int K, int S, const 
                     }
                 }
             }
-            *reinterpret_cast<uint4 *>(out + (size_t)t * D + (size_t)c * 8) =
-                make_uint4(pack_bf16x2(acc[0], acc[1]), pack_bf16x2(acc[2], acc[3]), pack_bf16x2(acc[4], acc[5]),
-                           pack_bf16x2(acc[6], acc[7]));
+            if (out_f32) {      // tensor-parallel partial: the fp32 sums, rounded after the cross-rank reduction
+                float4 *o = reinterpret_cast<float4 *>(out_f32 + (size_t)t * D + (size_t)c * 8);
+                o[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
+                o[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
+            } else {
+                *reinterpret_cast<uint4 *>(out + (size_t)t * D + (size_t)c * 8) =
+                    make_uint4(pack_bf16x2(acc[0], acc[1]), pack_bf16x2(acc[2], acc[3]), pack_bf16x2(acc[4], acc[5]),
+                               pack_bf16x2(acc[6], acc[7]));
+            }
         }
     }
 }
@@ -865,12 +872,15 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
     const int TK = a.T * a.K;
     const int sms = num_sms();
 
+    // tensor-parallel partial (out_f32): the decode path accumulates straight into the caller's buffer
+    float *acc_buf = (decode && a.out_f32) ? a.out_f32 : a.out_acc;
+
     // step 9 (+ schedule, + zero)
     {
         const int grid = sms * 4;
         profile_begin(BM_KERNEL_PREP, stream);
         cudaError_t e = launch_kernel(prep_kernel, dim3(grid), dim3(256), 0, stream, a.x, a.T, a.D, a.K, a.G, a.S,
-                                      a.r.counts, a.r.offsets, a.r.row_token, a.sched, a.xs, a.out_acc, decode ? 1 : 0, a.status);
+                                      a.r.counts, a.r.offsets, a.r.row_token, a.sched, a.xs, acc_buf, decode ? 1 : 0, a.status);
         if (e != cudaSuccess) return e;
         profile_end(BM_KERNEL_PREP, stream);
     }
@@ -879,7 +889,7 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
     p.seg_cap = a.G + a.S + 1;
     p.T = a.T; p.D = a.D; p.F = a.F; p.K = a.K; p.G = a.G; p.S = a.S; p.TK = TK;
     p.counts = a.r.counts; p.offsets = a.r.offsets; p.row_token = a.r.row_token; p.row_slot = a.r.row_slot;
-    p.gate_w = a.r.gate_w; p.sched = a.sched; p.h = a.h; p.out_acc = a.out_acc; p.y = a.y;
+    p.gate_w = a.r.gate_w; p.sched = a.sched; p.h = a.h; p.out_acc = acc_buf; p.y = a.y;
 
 
     const uint64_t h_rows = (uint64_t)TK + (uint64_t)a.S * a.T;
@@ -942,11 +952,13 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
         profile_begin(BM_KERNEL_FINALIZE, stream);
         cudaError_t e;
         if (decode)
-            e = launch_kernel(finalize_kernel, dim3(grid), dim3(256), 0, stream, (const float *)a.out_acc, a.out, n8);
+            e = a.out_f32 ? cudaSuccess      // the fp32 sums already are the result
+                          : launch_kernel(finalize_kernel, dim3(grid), dim3(256), 0, stream, (const float *)a.out_acc, a.out, n8);
         else
             e = launch_kernel(combine_kernel, dim3((unsigned)std::min<long long>(((long long)a.T + 7) / 8, (long long)sms * 8)),
                               dim3(256), 0, stream, (const bm_bf16 *)a.y, a.T, a.D, a.K, a.S,
-                              (const int32_t *)a.r.n_slots, (const int32_t *)a.r.slot_row, (const float *)a.r.gate_w, a.out);
+                              (const int32_t *)a.r.n_slots, (const int32_t *)a.r.slot_row, (const float *)a.r.gate_w, a.out,
+                              a.out_f32);
         profile_end(BM_KERNEL_FINALIZE, stream);
         return e;
     }
@@ -975,6 +987,14 @@ cudaError_t launch_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 
     if (err != cudaSuccess) return err;
     p.kblocks = (F + kBlockK - 1) / kBlockK; p.R = 256; p.n_wtiles = (D + 255) / 256;
     return pair ? launch_gemm<PF_GEMM2, true>(m_h, m_h, m_w2, m_w2, p, stream) : launch_gemm<PF_GEMM2>(m_h, m_h, m_w2, m_w2, p, stream);
+}
+
+cudaError_t launch_round_bf16(const float *in, size_t n, bm_bf16 *out, cudaStream_t stream) {
+    const size_t n8 = n / 8;
+    long long grid = (long long)((n8 + 255) / 256);
+    if (grid > num_sms() * 8) grid = num_sms() * 8;
+    if (grid < 1) grid = 1;
+    return launch_kernel(finalize_kernel, dim3((unsigned)grid), dim3(256), 0, stream, in, out, n8);
 }
 
 }  // namespace bm

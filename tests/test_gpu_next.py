@@ -212,3 +212,45 @@ def test_calibration_pipeline_end_to_end_against_oracle():
     assert (np.abs(mse - m_ref) <= 2e-2 * m_ref + 1e-7).all(), (mse, m_ref)
     assert abs(float(tot.cpu()[0]) - t_ref) <= 2e-2 * t_ref + 1e-7
     assert np.abs(cos.cpu().numpy() - c_ref).max() <= 5e-3
+
+
+# ---------------------------------------------------------------------------------------------------
+# tensor parallelism over F (NEXT-4): the ranks emulated one after the other on one GPU
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("T,world", [(48, 2), (700, 4), (3000, 2)])
+def test_tensor_parallel_partials_sum_to_the_layer(T, world):
+    import paper_2607_04164_b200 as bm
+    from paper_2607_04164_b200.tp import shard_f
+    cfg = LayerConfig("tp", T=T, D=512, F=1408, E=16, K=4, G=4, S=1, zipf_s=1.0)
+    L = make_layer(cfg, 4)
+    bias = L.router_bias.numpy()
+    o = oracle.route(bf16_bits(L.x), bf16_bits(L.W_router), bias, cfg.K, L.group_map.numpy(), cfg.G)
+    ref = oracle.moe_forward(bf16_bits(L.x), o, bf16_bits(L.W1), bf16_bits(L.W3), bf16_bits(L.W2), cfg.S)
+    xd = L.x.cuda()
+    r = bm.Routing(T, cfg.K, cfg.G)
+    total = torch.zeros((T, cfg.D), dtype=torch.float32, device="cuda")
+    for rank in range(world):
+        W1r, W3r, W2r = [t.cuda() for t in shard_f(L.W1, L.W3, L.W2, rank, world)]
+        ws = bm.alloc_workspace(T, cfg.D, W1r.shape[1], cfg.E, cfg.K, cfg.G, cfg.S)
+        bm.bm_route(xd, L.W_router.cuda(), L.router_bias.cuda(), cfg.K, L.group_map.cuda(), cfg.G, r, ws)
+        part = torch.full((T, cfg.D), float("nan"), dtype=torch.float32, device="cuda")
+        bm.bm_moe_forward_f32(xd, r, W1r, W3r, W2r, part, ws, S=cfg.S)
+        total += part                                   # stands in for the NCCL all-reduce
+        assert bm.bm_device_status(ws) == 0
+    out = bm.bm_round_bf16(total)
+    torch.cuda.synchronize()
+    assert_routing_equal(routing_to_numpy(r, T), o)
+    assert_out_close(out.float().cpu().numpy().astype(np.float64), ref)
+    # one rank = the plain layer: tp_moe_forward without a process group is bm_moe_forward
+    ws = bm.alloc_workspace(T, cfg.D, cfg.F, cfg.E, cfg.K, cfg.G, cfg.S)
+    W = [t.cuda() for t in (L.W1, L.W3, L.W2)]
+    a = torch.empty((T, cfg.D), dtype=torch.bfloat16, device="cuda")
+    b = torch.empty_like(a)
+    bm.tp_moe_forward(xd, r, *W, a, ws, S=cfg.S)
+    bm.bm_moe_forward(xd, r, *W, b, ws, S=cfg.S)
+    torch.cuda.synchronize()
+    assert_out_close(a.float().cpu().numpy().astype(np.float64), ref)
+    if T > 256:                                         # prefill path: fixed summation order -> the same bits
+        assert (a == b).all()
+    else:                                               # decode path: fp32 reds arrive in any order
+        assert (a.float() - b.float()).abs().max() <= 2.0 ** -7 * b.float().abs().max()
