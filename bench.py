@@ -662,9 +662,49 @@ def run_next(args):
     sys.stderr.write(f"calibration T={Tc}: expert_outputs {t_out*1e6:.0f} us {calib['expert_outputs']['tflops']:.0f} TFLOP/s; "
                      f"gram {t_gram*1e6:.0f} us {calib['cosine_gram']['gbs']:.0f} GB/s; mse {t_mse*1e6:.0f} us "
                      f"{calib['group_mse']['gbs']:.0f} GB/s\n")
+    # tensor parallelism over F (NEXT-4), the per-rank part only: rank 0's shard of BJ:configs[1] / [2] at world = 1..8,
+    # timed on this one GPU (route + bm_moe_forward_f32 + bm_round_bf16; the all-reduce between them is not run)
+    del Y, U, Wo, Uw, wsc
+    torch.cuda.empty_cache()
+    tp_rows = []
+    for name in ("decode", "prefill"):
+        cfgt = CONFIGS[name]
+        Lt = make_layer(cfgt, 0, weights=False)
+        xt, Wrt, bt, gmt = Lt.x.cuda(), Lt.W_router.cuda(), Lt.router_bias.cuda(), Lt.group_map.cuda()
+        for world in (1, 2, 4, 8):
+            Fr = bm.tp.shard_bounds(cfgt.F, 0, world)[1]
+            n_sets = cfgt.G + cfgt.S
+            w1 = mk(n_sets, Fr, cfgt.D); w3 = mk(n_sets, Fr, cfgt.D); w2 = mk(n_sets, cfgt.D, Fr)
+            wst = bm.alloc_workspace(cfgt.T, cfgt.D, Fr, cfgt.E, cfgt.K, cfgt.G, cfgt.S)
+            rt = bm.Routing(cfgt.T, cfgt.K, cfgt.G)
+            part = torch.empty((cfgt.T, cfgt.D), dtype=torch.float32, device="cuda")
+            outt = torch.empty((cfgt.T, cfgt.D), dtype=torch.bfloat16, device="cuda")
+
+            def step_tp():
+                bm.bm_route(xt, Wrt, bt, cfgt.K, gmt, cfgt.G, rt, wst)
+                bm.bm_moe_forward_f32(xt, rt, w1, w3, w2, part, wst, S=cfgt.S)
+                bm.bm_round_bf16(part, outt)
+
+            nst = 100 if name == "decode" else 10
+            for _ in range(5):
+                step_tp()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(nst):
+                step_tp()
+            e1.record()
+            torch.cuda.synchronize()
+            tt = e0.elapsed_time(e1) / 1e3 / nst
+            ar_bytes = cfgt.T * cfgt.D * 4
+            tp_rows.append(dict(config=name, world=world, F_shard=Fr, us_per_rank=tt * 1e6, allreduce_bytes=ar_bytes if world > 1 else 0,
+                                note="per-rank compute only, measured on one GPU; the NCCL all-reduce of out_f32 is not included"))
+            sys.stderr.write(f"tp {name} world={world} F_shard={Fr}: {tt*1e6:.1f} us per rank (+ all-reduce of {ar_bytes/1e6:.2f} MB)\n")
+            del w1, w3, w2, wst
+            torch.cuda.empty_cache()
     res = dict(metric=METRIC, unit=UNIT, workload="SURVEY 8(f): partial brownout at D=2048 F=1408 E=60 top-4 G=15 zipf 1.0; "
-               "united-weight average; calibration forward", peaks=peaks, weight_copies=copies, partial=rows, unite=unite,
-               calibration=calib)
+               "united-weight average; calibration forward; per-rank part of tensor parallelism over F", peaks=peaks,
+               weight_copies=copies, partial=rows, unite=unite, calibration=calib, tp_per_rank=tp_rows)
     if args.out:
         with open(args.out, "w") as fh:
             json.dump(res, fh, indent=1)

@@ -12,3 +12,4 @@ from .binding import (  # noqa: F401
     workspace_bytes, KERNELS,
 )
 from .tp import shard_f, tp_moe_forward  # noqa: F401,E402
+from . import tp  # noqa: F401,E402
