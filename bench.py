@@ -300,7 +300,7 @@ def load_traffic(kind):
     return None
 
 
-def cpu_baseline(L, budget_s=12.0):
+def cpu_baseline(L, budget_s=20.0):
     """The oracle as it stands (never tuned for this), timed on this box's host cores on a bounded sample
     of the same workload: whole batches of the layer if one takes seconds, else a token prefix."""
     import oracle
