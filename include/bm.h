@@ -1,7 +1,9 @@
 /*
- * bm.h -- C ABI of the B200-native grouped MoE-layer forward pass (BrownoutMoE full-brownout path).
+ * bm.h -- C ABI of the B200-native grouped MoE-layer forward pass (BrownoutMoE full-brownout path), plus the
+ *         SURVEY.md 8(f) rows built on it: partial brownout, united-weight construction, the calibration forward and
+ *         the per-rank partial of a tensor-parallel layer.
  *
- * The operation (PAPER.md = /root/reference/PAPER.md, "P:NN" = line NN; readings A1..A14 = DESIGN.md):
+ * The operation (PAPER.md = /root/reference/PAPER.md, "P:NN" = line NN; readings A1..A20 = DESIGN.md):
  *   P:42   MoE layer with E experts and top-K routing:  h_t = sum_{i<=K} g_i(x_t) * FFN_i(x_t),
  *          g_i the gating score.
  *   P:46   united experts / full brownout: every routed expert e is served by the united expert of its
@@ -164,13 +166,15 @@ int bm_group_mse(const bm_bf16 *Y, const bm_bf16 *U, int T, int D, const int32_t
 /*
  * bm_moe_forward -- steps 9-13: out[t] = sum_s gate_w[t,s] * FFN_{group_ids[t,s]}(x_t) + sum_{j<S} FFN_{G+j}(x_t)
  * with FFN_u(x) = W2[u] . ( SiLU(W1[u] x) * (W3[u] x) )   (P:42 with united experts P:46; SwiGLU: A3).
- * bf16 operands, fp32 accumulation (tensor cores), the intermediate h is rounded to bf16 (A12).
+ * bf16 operands, fp32 accumulation (tensor cores), the intermediate h is rounded to bf16 (A12); on the prefill
+ * path the per-row expert outputs are rounded to bf16 before the fp32 gate-weighted sum, which is taken in slot
+ * order (deterministic); the decode path adds fp32 partial sums with reductions whose order may vary.
  *   x        [T,D]      bf16
  *   routing  as produced by bm_route (or any arrays satisfying the same invariants), same T
  *   W1, W3   [G+S,F,D]  bf16 (united experts 0..G-1, then the S always-on shared experts, A11)
  *   W2       [G+S,D,F]  bf16
  *   out      [T,D]      bf16, overwritten
- * The path (decode / prefill) is picked from T, a host value.
+ * The path (decode / prefill, see BM_PATH_AUTO) is picked from the host values T, K and G.
  */
 int bm_moe_forward(const bm_bf16 *x, int T, int D, const bm_routing *routing, const bm_bf16 *W1,
                    const bm_bf16 *W3, const bm_bf16 *W2, int F, int S, bm_bf16 *out, void *workspace,
