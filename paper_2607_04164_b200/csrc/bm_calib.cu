@@ -36,9 +36,12 @@ expert_hist_kernel(const int32_t *__restrict__ expert_ids, long long items, int 
 // Y . Y^T, so ONE TMA tile (128 rows x 64 columns; rows >= E are out of bounds and arrive as zeros) feeds
 // the A and the B descriptor of tcgen05.mma.  CTA c owns the k-blocks c, c + grid, ... and keeps its
 // 128 x N fp32 partial in TMEM until the end; partial tiles go to the workspace and are summed in CTA order.
-// Measured: 3.5-3.7 TB/s (0.55 of the HBM copy rate) whatever E is; the time per k-block grows with the rows of
-// the TMA box (~8 cycles per 128-byte row), so the kernel sits on the TMA row rate, not on the MMAs -- packing two
-// k-blocks of a small-E tile into one M = N = 128 MMA was tried and changed nothing.
+// Measured: 3.5-3.7 TB/s (0.55 of the HBM copy rate) whatever E is.  The cause is the layout, not the MMAs: the E rows
+// of a tile are n*2 bytes (16 MB at T = 4096, D = 2048) apart, so every TMA box gathers 128-byte pieces from E distant
+// DRAM pages.  A stand-alone TMA streaming probe shows the same: 128 x 128-byte boxes reach 7.0 TB/s with an 8 KB row
+// stride and 4.5 TB/s with an 8 MB row stride (148 CTAs; 142 vs 62 GB/s per SM with 17 CTAs).  Packing two k-blocks of
+// a small-E tile into one M = N = 128 MMA was tried and changed nothing.  A token-major output layout [T, E, D] of
+// bm_expert_outputs would give the Gram kernel 4 KB row strides; that is the lead for a later round.
 // ---------------------------------------------------------------------------------------------------
 constexpr int kGramThreads = 192;
 constexpr int kGramStages = 12;
