@@ -7,6 +7,11 @@
 #include <stdint.h>
 
 namespace bm {
+
+// host: plain (unswizzled) 2-D tensor map over a row-major bf16 matrix (defined in bm_gemm.cu)
+bool make_map_2d_plain(CUtensorMap *m, const void *base, uint64_t rows, uint64_t cols, uint32_t box_rows,
+                       uint32_t box_cols);
+
 namespace ptx {
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) {

@@ -33,6 +33,8 @@ __device__ __forceinline__ void select_and_write(const float *l, int t, int lane
                                                  float *__restrict__ gate_w, int32_t *__restrict__ n_slots,
                                                  int32_t *__restrict__ status) {
     // ---- R2: K rounds of warp arg-max; ties -> lower index --------------------------------------
+    // A round is two warp reductions (redux.sync): the maximum of an order-preserving integer image of the
+    // lane-local best values, then the minimum expert index among the lanes that hold that maximum.
     unsigned taken = 0;                 // bit c: candidate e = lane + 32*c already selected (E <= 512)
     int my_e = 0;                       // lane i < K: expert of rank i
     float my_l = 0.0f;                  //             and its logit
@@ -48,14 +50,15 @@ __device__ __forceinline__ void select_and_write(const float *l, int t, int lane
             if (v != v) v = -INFINITY;            // NaN: unspecified result, keep indices valid
             if (bi == 0x7fffffff || v > bv) { bv = v; bi = e; }
         }
-#pragma unroll
-        for (int o = 16; o >= 1; o >>= 1) {
-            const float ov = __shfl_xor_sync(kFullMask, bv, o);
-            const int oi = __shfl_xor_sync(kFullMask, bi, o);
-            if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
-        }
-        if ((bi & 31) == lane) taken |= 1u << (bi >> 5);
-        if (lane == i) { my_e = bi; my_l = l[bi]; }
+        // monotone map float -> uint32 (a < b  <=>  key(a) < key(b)); -0 is first folded onto +0 so that the
+        // two compare equal as they do under '=='; a lane without candidates gets key 0, below every float
+        const uint32_t u = __float_as_uint(__fadd_rn(bv, 0.0f));
+        uint32_t key = (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+        if (bi == 0x7fffffff) key = 0u;
+        const uint32_t kmax = __reduce_max_sync(kFullMask, key);
+        const int win = __reduce_min_sync(kFullMask, (key == kmax) ? bi : 0x7fffffff);
+        if ((win & 31) == lane) taken |= 1u << (win >> 5);
+        if (lane == i) { my_e = win; my_l = l[win]; }
     }
     const bool active = lane < K;
     // ---- R3: softmax over the selected logits, denominator summed in rank order -------------------
@@ -177,25 +180,27 @@ router_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *__rest
 
 // -------------------------------------------------------------------------------------------------
 // Throughput shape (T >= BM_ROUTER_TP_MIN_T): the same canonical dot products, operands staged through
-// shared memory by a producer warp.  Persistent CTAs walk token blocks of TB = WT*4 tokens; per pass a
-// block meets EB = WE*8 experts; compute warp (tw, ew) keeps the 4 x 8 register tile acc[token][expert]
-// of its slice -- lane l still owns partial l of every dot product and walks its chunks l, l+32, ... in
-// ascending order, so the association tree is unchanged.  D is walked in slabs of 256 elements (one
-// 16-byte chunk per lane and row).  Slab rows are copied with cp.async.bulk (512 bytes each; every warp
-// issues a few) into a 4-stage ring guarded by full/empty mbarriers, three slabs ahead of the multiply
-// and across passes and blocks, so neither the HBM read of x nor the L2 read of W_router is on the
-// critical path, and the warps never meet at a CTA-wide barrier inside a pass.  E > EB takes ceil(E/EB) passes over the same tokens.
+// shared memory by TMA.  Persistent CTAs walk token blocks of TB = WT*8 tokens; per pass a block meets
+// EB = WE*8 experts; compute warp (tw, ew) keeps the 8 x 8 register tile acc[token][expert] of its slice --
+// lane l still owns partial l of every dot product and walks its chunks l, l+32, ... in ascending order, so
+// the association tree is unchanged.  D is walked in slabs of 256 elements (one 16-byte chunk per lane and
+// row).  A producer warp (one elected lane) fetches a slab with two tensor copies -- the x tile [TB, 256]
+// and the W_router tile [EB, 256], rows past T or E zero-filled and never stored -- into a 4-stage ring
+// guarded by full/empty mbarriers, three slabs ahead of the multiply and across passes and blocks, so
+// neither the HBM read of x nor the L2 read of W_router is on the critical path and the compute warps
+// never meet a CTA-wide barrier inside a pass.  (The first version copied row by row with per-lane
+// cp.async.bulk: the copy instruction takes its operands from uniform registers, so the compiler serialises
+// the lanes -- 16% of all executed instructions and a quarter of the stall samples in ncu.)
+// The multiply is FFMA2 (two fp32 FMAs per instruction; the FMA pipe issues it at the rate of a scalar FFMA).
+// E > EB takes ceil(E/EB) passes over the same tokens.
 // -------------------------------------------------------------------------------------------------
 constexpr int kTpStages = 4;
-constexpr int kTpTok = 4;
 constexpr int kSlab = 256;                    // elements per slab row = 512 bytes
-constexpr int kTpMaxThreads = 16 * 32;
+constexpr int kTpTok = 8;                     // tokens of a compute warp's register tile
+constexpr int kTpComputeWarps = 8;
+constexpr int kTpSelectWarps = 3;
+constexpr int kTpThreads = (kTpComputeWarps + 1 + kTpSelectWarps) * 32;      // + the producer warp + the select warps
 
-__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gsrc, uint32_t bytes, uint64_t *bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(ptx::smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(ptx::smem_u32(bar))
-                 : "memory");
-}
 // Sum of the 32 lane partials of each of this lane's 32 accumulators: the xor butterfly (16, 8, 4, 2, 1)
 // of reading A1, evaluated for all 32 accumulators at once.  At the step with offset o every lane hands
 // over the half of its values whose index bit o differs from its own lane bit o, so a step costs n/2
@@ -215,9 +220,36 @@ __device__ __forceinline__ void butterfly32(float (&v)[32], int lane) {
     }
 }
 
-__global__ void __launch_bounds__(kTpMaxThreads, 1)
-router_tp_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *__restrict__ Wr,
-                 const float *__restrict__ bias, int E, int K, GroupMap gm,
+// Two fp32 fused multiply-adds in one instruction (FFMA2): d0 = fma(x, w0, d0), d1 = fma(x, w1, d1), each
+// rounded to nearest exactly like __fmaf_rn, so the canonical order (A1) is untouched -- the two halves are
+// the accumulators of two neighbouring experts.  ptxas folds the duplicated x into the scalar-broadcast
+// operand form (FFMA2 Rd, Rx.F32, Rw.F32x2, Rd.F32x2), so no instruction is spent on it.
+__device__ __forceinline__ void fma2(float &d0, float &d1, float x, float w0, float w1) {
+    uint64_t a, b, c;
+    asm("mov.b64 %0, {%1, %1};" : "=l"(a) : "f"(x));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(b) : "f"(w0), "f"(w1));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(c) : "f"(d0), "f"(d1));
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c) : "l"(a), "l"(b));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(d0), "=f"(d1) : "l"(c));
+}
+// bf16 -> fp32 of the low half through PRMT, so that the unpack stays on the ALU pipe (the compiler turns a
+// plain shift into IMAD.U32 half of the time, which competes with FFMA2 for the FMA pipe)
+__device__ __forceinline__ float bf16_lo_alu(uint32_t u) { return __uint_as_float(__byte_perm(u, 0u, 0x1044)); }
+
+// Wait of a helper role (producer lane, select warps): backs off between polls so that it does not take
+// issue slots from the compute warps; bounded like ptx::mbar_wait (a protocol bug traps instead of hanging).
+__device__ __forceinline__ void mbar_wait_sleep(uint64_t *bar, uint32_t parity) {
+    uint32_t spins = 0;
+    while (!ptx::mbar_try_wait(bar, parity)) {
+        __nanosleep(64);
+        if (++spins > (1u << 24)) __trap();
+    }
+}
+
+__global__ void __launch_bounds__(kTpThreads, 1)
+router_tp_kernel(const __grid_constant__ CUtensorMap tm_x,      // x [T, D], box 256 x TB
+                 const __grid_constant__ CUtensorMap tm_w,      // W_router [E, D], box 256 x EB
+                 int T, int D, const float *__restrict__ bias, int E, int K, GroupMap gm,
                  int WT, int WE, int n_blocks, int32_t *__restrict__ expert_ids, int32_t *__restrict__ group_ids,
                  float *__restrict__ gate_w, int32_t *__restrict__ n_slots, int32_t *__restrict__ status) {
     extern __shared__ __align__(128) uint8_t tp_smem[];
@@ -226,65 +258,83 @@ router_tp_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *__r
     const uint32_t stage_bytes = (uint32_t)rows * (kSlab * 2);
     uint64_t *full = reinterpret_cast<uint64_t *>(tp_smem + kTpStages * stage_bytes);
     uint64_t *empty = full + kTpStages;
-    float *s_logits = reinterpret_cast<float *>(empty + kTpStages);   // [TB][E]
+    uint64_t *lfull = empty + kTpStages;                              // logits of a block parked / consumed
+    uint64_t *lempty = lfull + 2;
+    float *s_logits = reinterpret_cast<float *>(lempty + 2);          // [2][TB][E]
     const int tid = threadIdx.x;
     const int warp = tid >> 5, lane = tid & 31;
-    const int nw = blockDim.x >> 5;
     const int n_slabs = (D + kSlab - 1) / kSlab;
     const int n_pass = (E + EB - 1) / EB;
-    const int tw = warp % WT, ew = warp / WT;
 
     if (tid == 0) {
-        for (int i = 0; i < kTpStages; ++i) { ptx::mbar_init(&full[i], 1); ptx::mbar_init(&empty[i], nw); }
+        for (int i = 0; i < kTpStages; ++i) {
+            ptx::mbar_init(&full[i], 1);
+            ptx::mbar_init(&empty[i], kTpComputeWarps);
+        }
+        for (int i = 0; i < 2; ++i) {
+            ptx::mbar_init(&lfull[i], kTpComputeWarps);
+            ptx::mbar_init(&lempty[i], kTpSelectWarps);
+        }
         ptx::fence_barrier_init();
+        ptx::prefetch_tmap(&tm_x);
+        ptx::prefetch_tmap(&tm_w);
     }
     __syncthreads();
     grid_dep_wait();      // x may come from a predecessor; the routing arrays may still be read by one
     grid_dep_launch();
 
-    // Producer side (spread over the warps): warp w copies the slab rows r = w, w + nw, w + 2 nw, ... with
-    // its lanes 0, 1, 2, ...; warp 0 also posts the byte count.  The producer cursor runs kTpStages - 1
-    // slabs ahead of the consumer cursor, across passes and token blocks.
-    const int my_row = warp + nw * lane;
-    int p_blk = blockIdx.x, p_pass = 0, p_slab = 0, p_stage = 0;
-    uint32_t p_phase = 0;
-    const bm_bf16 *p_src = nullptr;
-    auto produce = [&]() {
-        if (p_blk >= n_blocks) return;
-        if (p_slab == 0 && my_row < rows) {
-            if (my_row < TB) {
-                const int t = p_blk * TB + my_row;
-                p_src = x + (size_t)(t < T ? t : T - 1) * D;          // rows past T: computed and dropped
-            } else {
-                const int e = p_pass * EB + my_row - TB;
-                p_src = Wr + (size_t)(e < E ? e : E - 1) * D;
+    if (warp == kTpComputeWarps) {
+        // ---- producer: one lane, two tensor copies per slab -----------------------------------------
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int blk = blockIdx.x; blk < n_blocks; blk += gridDim.x)
+                for (int pass = 0; pass < n_pass; ++pass)
+                    for (int slab = 0; slab < n_slabs; ++slab) {
+                        mbar_wait_sleep(&empty[stage], phase ^ 1);    // slab held before released by every compute warp
+                        uint8_t *st = tp_smem + (size_t)stage * stage_bytes;
+                        ptx::mbar_arrive_expect_tx(&full[stage], stage_bytes);
+                        ptx::tma_load_2d(st, &tm_x, &full[stage], slab * kSlab, blk * TB, ptx::kEvictNormal);
+                        ptx::tma_load_2d(st + (size_t)TB * (kSlab * 2), &tm_w, &full[stage], slab * kSlab, pass * EB,
+                                         ptx::kEvictLast);
+                        if (++stage == kTpStages) { stage = 0; phase ^= 1; }
+                    }
+        }
+        return;
+    }
+    if (warp > kTpComputeWarps) {
+        // ---- select warps: R2-R5 of block i while the compute warps multiply block i + 1 -----------------
+        const int sw = warp - kTpComputeWarps - 1;
+        int it = 0;
+        for (int blk = blockIdx.x; blk < n_blocks; blk += gridDim.x, ++it) {
+            const int buf = it & 1;
+            mbar_wait_sleep(&lfull[buf], (it >> 1) & 1);
+            const float *lg = s_logits + (size_t)buf * TB * E;
+            // the CTA's last block: the compute warps have nothing left to multiply and take a share (below)
+            const int stride = blk + (int)gridDim.x >= n_blocks ? kTpSelectWarps + kTpComputeWarps : kTpSelectWarps;
+            for (int tl = sw; tl < TB; tl += stride) {
+                const int t = blk * TB + tl;
+                if (t >= T) break;
+                select_and_write(lg + tl * E, t, lane, E, K, gm, expert_ids, group_ids, gate_w, n_slots, status);
             }
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&lempty[buf]);
         }
-        const int k0 = p_slab * kSlab;
-        const uint32_t bytes = (uint32_t)min(kSlab, D - k0) * 2u;
-        ptx::mbar_wait(&empty[p_stage], p_phase ^ 1);                 // every warp has released the slab held before
-        if (tid == 0) ptx::mbar_arrive_expect_tx(&full[p_stage], (uint32_t)rows * bytes);
-        if (my_row < rows)
-            bulk_g2s(tp_smem + (size_t)p_stage * stage_bytes + (size_t)my_row * (kSlab * 2), p_src + k0, bytes,
-                     &full[p_stage]);
-        if (++p_stage == kTpStages) { p_stage = 0; p_phase ^= 1; }
-        if (++p_slab == n_slabs) {
-            p_slab = 0;
-            if (++p_pass == n_pass) { p_pass = 0; p_blk += gridDim.x; }
-        }
-    };
-    for (int i = 0; i < kTpStages - 1; ++i) produce();
+        return;
+    }
 
+    const int tw = warp % WT, ew = warp / WT;
     int stage = 0;
     uint32_t phase = 0;
-    for (int blk = blockIdx.x; blk < n_blocks; blk += gridDim.x) {
-        const int t_block = blk * TB;
+    int it = 0;
+    for (int blk = blockIdx.x; blk < n_blocks; blk += gridDim.x, ++it) {
+        const int buf = it & 1;
+        float *lg = s_logits + (size_t)buf * TB * E;
         for (int pass = 0; pass < n_pass; ++pass) {
-            float acc[32];                      // index a = token * 8 + expert
+            float acc[kTpTok * 8];              // index a = token * 8 + expert
 #pragma unroll
-            for (int a = 0; a < 32; ++a) acc[a] = 0.0f;
+            for (int a = 0; a < kTpTok * 8; ++a) acc[a] = 0.0f;
             for (int slab = 0; slab < n_slabs; ++slab) {
-                produce();
                 ptx::mbar_wait(&full[stage], phase);
                 const uint8_t *st = tp_smem + (size_t)stage * stage_bytes;
                 if (slab * kSlab + lane * 8 < D) {
@@ -292,26 +342,29 @@ router_tp_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *__r
 #pragma unroll
                     for (int i = 0; i < kTpTok; ++i) {
                         const uint4 v = *reinterpret_cast<const uint4 *>(st + (tw * kTpTok + i) * (kSlab * 2) + lane * 16);
-                        xf[i][0] = bf16_lo(v.x); xf[i][1] = bf16_hi(v.x); xf[i][2] = bf16_lo(v.y); xf[i][3] = bf16_hi(v.y);
-                        xf[i][4] = bf16_lo(v.z); xf[i][5] = bf16_hi(v.z); xf[i][6] = bf16_lo(v.w); xf[i][7] = bf16_hi(v.w);
+                        xf[i][0] = bf16_lo_alu(v.x); xf[i][1] = bf16_hi(v.x); xf[i][2] = bf16_lo_alu(v.y); xf[i][3] = bf16_hi(v.y);
+                        xf[i][4] = bf16_lo_alu(v.z); xf[i][5] = bf16_hi(v.z); xf[i][6] = bf16_lo_alu(v.w); xf[i][7] = bf16_hi(v.w);
                     }
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) {
-                        const uint4 wv = *reinterpret_cast<const uint4 *>(st + (TB + ew * 8 + j) * (kSlab * 2) + lane * 16);
-                        const float w0 = bf16_lo(wv.x), w1 = bf16_hi(wv.x), w2 = bf16_lo(wv.y), w3 = bf16_hi(wv.y);
-                        const float w4 = bf16_lo(wv.z), w5 = bf16_hi(wv.z), w6 = bf16_lo(wv.w), w7 = bf16_hi(wv.w);
+                    for (int j = 0; j < 8; j += 2) {        // experts j, j + 1 share one FFMA2
+                        const uint8_t *wp = st + (TB + ew * 8 + j) * (kSlab * 2) + lane * 16;
+                        const uint4 wa = *reinterpret_cast<const uint4 *>(wp);
+                        const uint4 wb = *reinterpret_cast<const uint4 *>(wp + kSlab * 2);
+                        const float a0 = bf16_lo_alu(wa.x), a1 = bf16_hi(wa.x), a2 = bf16_lo_alu(wa.y), a3 = bf16_hi(wa.y);
+                        const float a4 = bf16_lo_alu(wa.z), a5 = bf16_hi(wa.z), a6 = bf16_lo_alu(wa.w), a7 = bf16_hi(wa.w);
+                        const float b0 = bf16_lo_alu(wb.x), b1 = bf16_hi(wb.x), b2 = bf16_lo_alu(wb.y), b3 = bf16_hi(wb.y);
+                        const float b4 = bf16_lo_alu(wb.z), b5 = bf16_hi(wb.z), b6 = bf16_lo_alu(wb.w), b7 = bf16_hi(wb.w);
 #pragma unroll
                         for (int i = 0; i < kTpTok; ++i) {
-                            float pacc = acc[i * 8 + j];            // ascending element order inside the chunk
-                            pacc = __fmaf_rn(xf[i][0], w0, pacc);
-                            pacc = __fmaf_rn(xf[i][1], w1, pacc);
-                            pacc = __fmaf_rn(xf[i][2], w2, pacc);
-                            pacc = __fmaf_rn(xf[i][3], w3, pacc);
-                            pacc = __fmaf_rn(xf[i][4], w4, pacc);
-                            pacc = __fmaf_rn(xf[i][5], w5, pacc);
-                            pacc = __fmaf_rn(xf[i][6], w6, pacc);
-                            pacc = __fmaf_rn(xf[i][7], w7, pacc);
-                            acc[i * 8 + j] = pacc;
+                            float &p = acc[i * 8 + j], &q = acc[i * 8 + j + 1];   // ascending element order inside the chunk
+                            fma2(p, q, xf[i][0], a0, b0);
+                            fma2(p, q, xf[i][1], a1, b1);
+                            fma2(p, q, xf[i][2], a2, b2);
+                            fma2(p, q, xf[i][3], a3, b3);
+                            fma2(p, q, xf[i][4], a4, b4);
+                            fma2(p, q, xf[i][5], a5, b5);
+                            fma2(p, q, xf[i][6], a6, b6);
+                            fma2(p, q, xf[i][7], a7, b7);
                         }
                     }
                 }
@@ -319,22 +372,34 @@ router_tp_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *__r
                 if (lane == 0) ptx::mbar_arrive(&empty[stage]);
                 if (++stage == kTpStages) { stage = 0; phase ^= 1; }
             }
-            // end of a pass: lane l finishes accumulator l = (token l/8, expert l%8), adds the bias, parks it
-            butterfly32(acc, lane);
+            // end of a pass: per group of 4 tokens, lane l finishes accumulator l = (token l/8, expert l%8),
+            // adds the bias, parks it
             const int e = pass * EB + ew * 8 + (lane & 7);
-            if (e < E) {
-                float v = acc[0];
-                if (bias) v = __fadd_rn(v, bias[e]);
-                s_logits[(tw * kTpTok + (lane >> 3)) * E + e] = v;
+            if (pass == 0) ptx::mbar_wait(&lempty[buf], ((it >> 1) & 1) ^ 1);   // the block parked here two blocks ago is consumed
+#pragma unroll
+            for (int h = 0; h < kTpTok / 4; ++h) {
+                butterfly32(*reinterpret_cast<float(*)[32]>(&acc[h * 32]), lane);
+                if (e < E) {
+                    float v = acc[h * 32];
+                    if (bias) v = __fadd_rn(v, bias[e]);
+                    lg[(tw * kTpTok + h * 4 + (lane >> 3)) * E + e] = v;
+                }
             }
         }
-        __syncthreads();                        // all logits of the block are parked
-        for (int tl = warp; tl < TB; tl += nw) {
-            const int t = t_block + tl;
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(&lfull[buf]);      // this warp's share of the block's logits is parked
+    }
+    if (it > 0) {
+        // last block of this CTA: help the select warps (tokens kTpSelectWarps + warp, + 11, ...)
+        const int li = it - 1, buf = li & 1;
+        const int blk = blockIdx.x + li * (int)gridDim.x;
+        ptx::mbar_wait(&lfull[buf], (li >> 1) & 1);
+        const float *lg = s_logits + (size_t)buf * TB * E;
+        for (int tl = kTpSelectWarps + warp; tl < TB; tl += kTpSelectWarps + kTpComputeWarps) {
+            const int t = blk * TB + tl;
             if (t >= T) break;
-            select_and_write(s_logits + tl * E, t, lane, E, K, gm, expert_ids, group_ids, gate_w, n_slots, status);
+            select_and_write(lg + tl * E, t, lane, E, K, gm, expert_ids, group_ids, gate_w, n_slots, status);
         }
-        __syncthreads();                        // before the next block overwrites them
     }
 }
 
@@ -342,21 +407,24 @@ cudaError_t launch_tp(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const f
                       GroupMap gm, const bm_routing &r, int32_t *status, cudaStream_t stream) {
     const int n_etiles = (E + 7) / 8;
     int WE = 1;
-    while (WE < n_etiles && WE < 8) WE *= 2;
-    const int ncw = WE >= 4 ? 16 : 8;
-    const int WT = ncw / WE;
+    while (WE < n_etiles && WE < kTpComputeWarps) WE *= 2;
+    const int WT = kTpComputeWarps / WE;
     const int TB = WT * kTpTok, EB = WE * 8;
-    const size_t smem = (size_t)kTpStages * (TB + EB) * (kSlab * 2) + 2 * kTpStages * sizeof(uint64_t) +
-                        (size_t)TB * E * sizeof(float);
+    const size_t smem = (size_t)kTpStages * (TB + EB) * (kSlab * 2) + (2 * kTpStages + 4) * sizeof(uint64_t) +
+                        2 * (size_t)TB * E * sizeof(float);
     static size_t smem_set = 0;
     if (smem > 48 * 1024 && smem > smem_set) {
         cudaError_t e = cudaFuncSetAttribute(router_tp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         smem_set = smem;
     }
+    CUtensorMap m_x, m_w;
+    if (!make_map_2d_plain(&m_x, x, (uint64_t)T, (uint64_t)D, (uint32_t)TB, kSlab) ||
+        !make_map_2d_plain(&m_w, Wr, (uint64_t)E, (uint64_t)D, (uint32_t)EB, kSlab))
+        return cudaErrorInvalidValue;
     const int n_blocks = (T + TB - 1) / TB;
     const int grid = n_blocks < num_sms() ? n_blocks : num_sms();
-    return launch_kernel(router_tp_kernel, dim3(grid), dim3(ncw * 32), smem, stream, x, T, D, Wr, bias, E, K,
+    return launch_kernel(router_tp_kernel, dim3(grid), dim3(kTpThreads), smem, stream, m_x, m_w, T, D, bias, E, K,
                          gm, WT, WE, n_blocks, r.expert_ids, r.group_ids, r.gate_w, r.n_slots, status);
 }
 
