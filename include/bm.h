@@ -60,10 +60,13 @@ enum { BM_DEV_BAD_GROUP_MAP = 1, BM_DEV_NONFINITE_LOGIT = 2, BM_DEV_BAD_ROUTING 
 
 /* execution path of bm_moe_forward_path */
 enum {
-    BM_PATH_AUTO = 0,    /* DECODE if T <= 64, or T <= BM_DECODE_MAX_T and T*K <= 24*G (few rows per group); else PREFILL */
+    BM_PATH_AUTO = 0,    /* GEMV if T*K <= G (a weight set expects at most ~1 row: single-token decode); else DECODE if
+                            T <= 64, or T <= BM_DECODE_MAX_T and T*K <= 24*G (few rows per group); else PREFILL */
     BM_PATH_DECODE = 1,  /* weight-streaming, weights on the MMA M side (small M; HBM-bound)   */
     BM_PATH_PREFILL = 2, /* 128-token x 256-column tcgen05 tiles (large M; tensor-pipe-bound)  */
-    BM_PATH_SIMT = 3     /* plain CUDA-core kernels; a debugging cross-check, never picked by AUTO */
+    BM_PATH_SIMT = 3,    /* plain CUDA-core kernels; a debugging cross-check, never picked by AUTO */
+    BM_PATH_GEMV = 4     /* weight-streaming matrix-vector products on the CUDA cores (FFMA2), <= 8 rows of a set per
+                            pass over its weights; y rows in bf16 + the prefill path's combine (deterministic)    */
 };
 enum { BM_DECODE_MAX_T = 256 };
 

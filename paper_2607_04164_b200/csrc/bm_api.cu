@@ -223,7 +223,7 @@ static int forward_common(const bm_bf16 *x, int T, int D, const bm_routing *rout
     int rc = check_shapes(T, D, F, routing->E, K, G, S, true);
     if (rc != BM_OK) return rc;
     if (routing->T != T) return BM_ERR_SHAPE;
-    if (path < BM_PATH_AUTO || path > BM_PATH_SIMT) return BM_ERR_PATH;
+    if (path < BM_PATH_AUTO || path > BM_PATH_GEMV) return BM_ERR_PATH;
     if (out_f32 && path == BM_PATH_SIMT) return BM_ERR_PATH;
     if (T == 0) return BM_OK;
     if (!x || !W1 || !W3 || !W2 || (!out && !out_f32) || !workspace || !routing->group_ids || !routing->gate_w ||
@@ -244,6 +244,11 @@ static int forward_common(const bm_bf16 *x, int T, int D, const bm_routing *rout
         const int max_t = tune_int("BM_DECODE_MAX_T", BM_DECODE_MAX_T);
         const bool few_rows = (long long)T * K <= 24LL * G;
         path = (T <= 64 || (T <= max_t && few_rows)) ? BM_PATH_DECODE : BM_PATH_PREFILL;
+        // matrix-vector streaming when a weight set expects at most ~1 row (single-token decode above all):
+        // the tcgen05 k-block loop has a latency floor that such a step never fills (see bm_gemv.cu)
+        const int gemv_rows = tune_int("BM_GEMV_ROWS", 1);
+        constexpr int kGemvSharedMaxT = 8;     // an always-on shared expert meets all T tokens: one pass of <= 8 rows
+        if ((S == 0 || T <= kGemvSharedMaxT) && (long long)T * K <= (long long)gemv_rows * G) path = BM_PATH_GEMV;
     }
 
     uint8_t *ws = static_cast<uint8_t *>(workspace);
@@ -260,6 +265,7 @@ static int forward_common(const bm_bf16 *x, int T, int D, const bm_routing *rout
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     cudaError_t e;
     if (path == BM_PATH_SIMT) e = launch_forward_simt(a, st);
+    else if (path == BM_PATH_GEMV) e = launch_forward_gemv(a, st);
     else e = launch_forward_tc(a, path == BM_PATH_DECODE, st);
     return e == cudaSuccess ? BM_OK : BM_ERR_CUDA;
 }

@@ -134,6 +134,8 @@ cudaError_t launch_round_bf16(const float *in, size_t n, bm_bf16 *out, cudaStrea
 
 cudaError_t launch_forward_simt(const ForwardArgs &a, cudaStream_t stream);
 cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t stream);
+cudaError_t launch_forward_gemv(const ForwardArgs &a, cudaStream_t stream);
+cudaError_t launch_combine(const ForwardArgs &a, cudaStream_t stream);
 
 // ---------------------------------------------------------------------------------------------
 // Device helpers

@@ -650,14 +650,17 @@ dense_sched_kernel(int32_t *__restrict__ sched, int E, int T) {
 __global__ void __launch_bounds__(256)
 combine_kernel(const bm_bf16 *__restrict__ y, int T, int D, int K, int S, const int32_t *__restrict__ n_slots,
                const int32_t *__restrict__ slot_row, const float *__restrict__ gate_w, bm_bf16 *__restrict__ out,
-               float *__restrict__ out_f32) {
+               float *__restrict__ out_f32, int split) {
     grid_dep_wait();
     grid_dep_launch();
     const int lane = threadIdx.x & 31;
     const int vec = D / 8;
     const size_t TK = (size_t)T * K;
     const int warps = (gridDim.x * blockDim.x) >> 5;
-    for (int t = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; t < T; t += warps) {
+    // a warp item = (token, column slice); split > 1 spreads a token's columns over several warps (small T)
+    const long long items = (long long)T * split;
+    for (long long item = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; item < items; item += warps) {
+        const int t = (int)(item / split), sl = (int)(item - (long long)t * split);
         const int n = min(max(n_slots[t], 0), K);
         const int n_src = n + S;
         long long my_row = -1;                                   // -1: skip (invalid slot_row)
@@ -669,7 +672,9 @@ combine_kernel(const bm_bf16 *__restrict__ y, int T, int D, int K, int S, const 
         } else if (lane < n_src) {
             my_row = (long long)TK + (long long)(lane - n) * T + t;
         }
-        for (int c = lane; c < vec; c += 32) {
+        for (int c0 = sl * 32; c0 < vec; c0 += 32 * split) {      // warp-uniform trip count: the shuffles below need every lane
+            const int c = c0 + lane;
+            const bool col_ok = c < vec;
             float acc[8];
 #pragma unroll
             for (int e = 0; e < 8; ++e) acc[e] = 0.0f;
@@ -681,7 +686,7 @@ combine_kernel(const bm_bf16 *__restrict__ y, int T, int D, int K, int S, const 
                     const int src = min(s0 + q, 31);
                     const long long row = __shfl_sync(kFullMask, my_row, src);
                     gw[q] = __shfl_sync(kFullMask, my_gw, src);
-                    const bool ok = s0 + q < n_src && row >= 0;
+                    const bool ok = s0 + q < n_src && row >= 0 && col_ok;
                     if (!ok) gw[q] = 0.0f;
                     v[q] = ok ? *reinterpret_cast<const uint4 *>(y + (size_t)row * D + (size_t)c * 8) : make_uint4(0, 0, 0, 0);
                 }
@@ -695,6 +700,7 @@ combine_kernel(const bm_bf16 *__restrict__ y, int T, int D, int K, int S, const 
                     }
                 }
             }
+            if (!col_ok) continue;
             if (out_f32) {      // tensor-parallel partial: the fp32 sums, rounded after the cross-rank reduction
                 float4 *o = reinterpret_cast<float4 *>(out_f32 + (size_t)t * D + (size_t)c * 8);
                 o[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
@@ -883,6 +889,27 @@ bool make_map_2d_plain(CUtensorMap *m, const void *base, uint64_t rows, uint64_t
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+static cudaError_t launch_combine_raw(const ForwardArgs &a, cudaStream_t stream) {
+    // one warp per token; with few tokens a token's 32-chunk column slices go to different warps
+    const int n_slices = (a.D / 8 + 31) / 32;
+    int split = 1;
+    while (split < n_slices && (long long)a.T * split * 2 <= (long long)num_sms() * 8) split *= 2;
+    if (split > n_slices) split = n_slices;
+    const long long items = (long long)a.T * split;
+    return launch_kernel(combine_kernel, dim3((unsigned)std::min<long long>((items + 7) / 8, (long long)num_sms() * 8)),
+                         dim3(256), 0, stream, (const bm_bf16 *)a.y, a.T, a.D, a.K, a.S,
+                         (const int32_t *)a.r.n_slots, (const int32_t *)a.r.slot_row, (const float *)a.r.gate_w, a.out,
+                         a.out_f32, split);
+}
+
+// F2 over bf16 y rows (prefill and GEMV paths), bracketed as BM_KERNEL_FINALIZE for the profile hooks
+cudaError_t launch_combine(const ForwardArgs &a, cudaStream_t stream) {
+    profile_begin(BM_KERNEL_FINALIZE, stream);
+    cudaError_t e = launch_combine_raw(a, stream);
+    profile_end(BM_KERNEL_FINALIZE, stream);
+    return e;
+}
+
 cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t stream) {
     const int TK = a.T * a.K;
     const int sms = num_sms();
@@ -970,10 +997,7 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
             e = a.out_f32 ? cudaSuccess      // the fp32 sums already are the result
                           : launch_kernel(finalize_kernel, dim3(grid), dim3(256), 0, stream, (const float *)a.out_acc, a.out, n8);
         else
-            e = launch_kernel(combine_kernel, dim3((unsigned)std::min<long long>(((long long)a.T + 7) / 8, (long long)sms * 8)),
-                              dim3(256), 0, stream, (const bm_bf16 *)a.y, a.T, a.D, a.K, a.S,
-                              (const int32_t *)a.r.n_slots, (const int32_t *)a.r.slot_row, (const float *)a.r.gate_w, a.out,
-                              a.out_f32);
+            e = launch_combine_raw(a, stream);
         profile_end(BM_KERNEL_FINALIZE, stream);
         return e;
     }

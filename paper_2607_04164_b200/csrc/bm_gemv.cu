@@ -1,0 +1,269 @@
+// bm_gemv.cu -- BM_PATH_GEMV: steps 10-12 for very small batches (a weight set meets ~1-4 token rows:
+// single-token decode, T*K <= 4*G) as weight-streaming matrix-vector products on the CUDA cores.
+//
+// Cite: PAPER.md:42 (expert FFN, gate-weighted sum), PAPER.md:46 (united experts cut "the number of experts
+// loaded during inference": at these sizes the layer IS the weight load), A3, A11, A12.
+//
+// Why not the tcgen05 decode path here: its k-block loop has a floor of ~0.3 us per 64 columns whatever
+// the tile holds, so one token on four groups costs 12 + 7 us of MMA pipeline for 7 + 3.5 us of HBM time,
+// plus a gather/schedule kernel and TMEM/tensor-map set-up in each GEMM.  With <= 8 rows per weight set the
+// FMA work is a few percent of the CUDA cores' rate, so plain 128-bit streaming loads with FFMA2 keep up
+// with HBM and the kernels start at once.
+//
+// Both products are one kernel template.  A "unit" q of a weight set u is a pair of weight rows that
+// share one FFMA2 per element:
+//   SWIGLU:  rows W1[u][q,:] and W3[u][q,:]  (q < F, input x rows, length D)   -> h[r,q] = SiLU(a) * b
+//   plain :  rows W2[u][2q,:] and W2[u][2q+1,:] (q < D/2, input h rows, length F) -> y[r,2q], y[r,2q+1]
+// The active sets' units form one index space that is cut into equal contiguous ranges, one per CTA (the
+// counts are read on the device; the host never sees them).  A CTA stages the <= 8 input rows of the set
+// in shared memory, then each warp takes units q, q + warps, ...: lane l streams the 16-byte chunks l,
+// l+32, ... of both weight rows (software-pipelined, see warp_units), multiplies them into one fp32 accumulator
+// pair per input row, and the warp adds the lane partials with a shuffle butterfly.  A set with more than
+// 8 rows takes several passes over its weights (correct, slower; BM_PATH_AUTO does not send such shapes
+// here).  gemv2 writes bf16 y rows; the prefill path's combine_kernel applies the gate weights in slot order
+// (deterministic), so the result is defined exactly like the prefill path's.
+#include "bm_common.cuh"
+
+namespace bm {
+
+namespace {
+
+constexpr int kGvThreads = 512;
+constexpr int kGvWarps = kGvThreads / 32;
+constexpr int kGvRows = 8;          // input rows staged per pass
+
+__device__ __forceinline__ uint4 ld_stream(const uint4 *p) {
+    uint4 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void fma2(float &d0, float &d1, float x, float w0, float w1) {
+    uint64_t a, b, c;
+    asm("mov.b64 %0, {%1, %1};" : "=l"(a) : "f"(x));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(b) : "f"(w0), "f"(w1));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(c) : "f"(d0), "f"(d1));
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c) : "l"(a), "l"(b));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(d0), "=f"(d1) : "l"(c));
+}
+
+// One warp's units q0, q0 + warps, ... < qb of one weight set against the R staged input rows (R: compile time).
+// The weight stream is software-pipelined: the loads of step s + 1 (a step = U chunks per lane of both rows;
+// the next step may belong to the next unit) are issued before the multiply of step s, from two register
+// buffers, so a warp always has a step of loads in flight -- without it every step paid a full HBM latency
+// (measured: 3 TB/s instead of 6 at T = 16, G = 60).
+template <int R, bool SWIGLU>
+__device__ __forceinline__ void warp_units(const bm_bf16 *__restrict__ base_a, const bm_bf16 *__restrict__ base_b,
+                                           size_t stride_q, int n8, int q0, int qb, const uint8_t *s_in, int in_bytes,
+                                           int lane, int nr, bm_bf16 *__restrict__ outp, size_t orow0, int OUT) {
+    constexpr int U = R <= 4 ? 4 : 2;           // chunks of each row per lane and step (fewer with 8 rows: registers)
+    const int iters = (n8 + 32 * U - 1) / (32 * U);
+    float acc[R][2];
+#pragma unroll
+    for (int r = 0; r < R; ++r) acc[r][0] = acc[r][1] = 0.0f;
+
+    // (always writes the buffers -- a conditionally written register array ends up in local memory)
+    auto load = [&](bool on, int q, int it, uint4 (&va)[U], uint4 (&vb)[U]) {
+        const uint4 *wa = reinterpret_cast<const uint4 *>(base_a + (size_t)q * stride_q);
+        const uint4 *wb = reinterpret_cast<const uint4 *>(base_b + (size_t)q * stride_q);
+#pragma unroll
+        for (int i = 0; i < U; ++i) {
+            const int c = (it * U + i) * 32 + lane;
+            const bool ok = on && c < n8;
+            va[i] = ok ? ld_stream(wa + c) : make_uint4(0u, 0u, 0u, 0u);
+            vb[i] = ok ? ld_stream(wb + c) : make_uint4(0u, 0u, 0u, 0u);
+        }
+    };
+    auto compute = [&](int it, const uint4 (&va)[U], const uint4 (&vb)[U]) {
+#pragma unroll
+        for (int i = 0; i < U; ++i) {
+            const int c = (it * U + i) * 32 + lane;
+            if (c < n8) {
+                const uint32_t a[4] = {va[i].x, va[i].y, va[i].z, va[i].w};
+                const uint32_t b[4] = {vb[i].x, vb[i].y, vb[i].z, vb[i].w};
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const uint4 xv = *reinterpret_cast<const uint4 *>(s_in + (size_t)r * in_bytes + (size_t)c * 16);
+                    const uint32_t x[4] = {xv.x, xv.y, xv.z, xv.w};
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        fma2(acc[r][0], acc[r][1], bf16_lo(x[k]), bf16_lo(a[k]), bf16_lo(b[k]));
+                        fma2(acc[r][0], acc[r][1], bf16_hi(x[k]), bf16_hi(a[k]), bf16_hi(b[k]));
+                    }
+                }
+            }
+        }
+    };
+    auto finish = [&](int q) {          // lane r keeps and stores the sums of row r; rows past nr are dropped
+        float ma = 0.0f, mb = 0.0f;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            float a = acc[r][0], b = acc[r][1];
+#pragma unroll
+            for (int o = 16; o >= 1; o >>= 1) {
+                a += __shfl_xor_sync(kFullMask, a, o);
+                b += __shfl_xor_sync(kFullMask, b, o);
+            }
+            if (lane == r) { ma = a; mb = b; }
+            acc[r][0] = acc[r][1] = 0.0f;
+        }
+        if (lane < nr) {
+            const size_t orow = (orow0 + (size_t)lane) * (size_t)OUT;
+            if (SWIGLU) outp[orow + q] = (bm_bf16)f32_to_bf16_bits(ma / (1.0f + expf(-ma)) * mb);
+            else *reinterpret_cast<uint32_t *>(outp + orow + 2 * (size_t)q) = pack_bf16x2(ma, mb);
+        }
+    };
+
+    uint4 a0[U], b0[U], a1[U], b1[U];
+    int q = q0, it = 0;
+    load(q < qb, q, 0, a0, b0);
+    while (q < qb) {
+        int qn = q, itn = it + 1;
+        if (itn == iters) { itn = 0; qn += kGvWarps; }
+        load(qn < qb, qn, itn, a1, b1);
+        compute(it, a0, b0);
+        if (it == iters - 1) finish(q);
+        q = qn; it = itn;
+        if (q >= qb) break;
+        qn = q; itn = it + 1;
+        if (itn == iters) { itn = 0; qn += kGvWarps; }
+        load(qn < qb, qn, itn, a0, b0);
+        compute(it, a1, b1);
+        if (it == iters - 1) finish(q);
+        q = qn; it = itn;
+    }
+}
+
+struct GemvArgs {
+    const bm_bf16 *in;          // SWIGLU: x [T, IN]; plain: h [TK + S*T, IN]
+    const bm_bf16 *Wa, *Wb;     // SWIGLU: W1, W3 [G+S, F, D]; plain: W2 twice [G+S, D, F]
+    bm_bf16 *outp;              // SWIGLU: h [TK + S*T, F]; plain: y [TK + S*T, D]
+    const int32_t *offsets;     // [G+1]
+    const int32_t *row_token;   // [TK]
+    int T, TK, G, S;
+    int IN;                     // length of an input row (D or F)
+    int OUT;                    // length of an output row (F or D)
+    int NQ;                     // units per set (F or D/2)
+};
+
+template <bool SWIGLU>
+__global__ void __launch_bounds__(kGvThreads, 1)
+gemv_kernel(GemvArgs p, int rows_cap) {
+    extern __shared__ __align__(16) uint8_t gv_smem[];
+    __shared__ int s_nact;
+    const int in_bytes = p.IN * 2, n8 = p.IN / 8;
+    uint8_t *s_in = gv_smem;                                              // [rows_cap][IN] bf16
+    int *s_set = reinterpret_cast<int *>(gv_smem + (size_t)rows_cap * in_bytes);   // active sets, ascending
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int nsets = p.G + p.S;
+    grid_dep_wait();      // routing arrays, x / h come from predecessors
+    grid_dep_launch();
+
+    if (warp == 0) {
+        int n = 0;
+        for (int base = 0; base < nsets; base += 32) {
+            const int u = base + lane;
+            bool act = false;
+            if (u < nsets) act = (u < p.G ? p.offsets[u + 1] - p.offsets[u] : p.T) > 0;
+            const unsigned m = __ballot_sync(kFullMask, act);
+            if (act) s_set[n + __popc(m & ((1u << lane) - 1u))] = u;
+            n += __popc(m);
+        }
+        if (lane == 0) s_nact = n;
+    }
+    __syncthreads();
+    const long long total = (long long)s_nact * p.NQ;
+    const long long per = (total + gridDim.x - 1) / gridDim.x;
+    const long long lo = (long long)blockIdx.x * per;
+    const long long hi = lo + per < total ? lo + per : total;
+
+    for (long long pos = lo; pos < hi;) {
+        const int k = (int)(pos / p.NQ);
+        const int u = s_set[k];
+        const int qa = (int)(pos - (long long)k * p.NQ);
+        const int qb = (int)((hi - pos) < (long long)(p.NQ - qa) ? qa + (hi - pos) : p.NQ);
+        long long row0;
+        int cnt;
+        if (u < p.G) {
+            row0 = p.offsets[u];
+            cnt = p.offsets[u + 1] - (int)row0;
+            if (row0 < 0 || row0 > p.TK) cnt = 0;
+            if (cnt > p.TK - (int)row0) cnt = p.TK - (int)row0;
+        } else {
+            row0 = (long long)p.TK + (long long)(u - p.G) * p.T;
+            cnt = p.T;
+        }
+        for (int base = 0; base < cnt; base += rows_cap) {
+            const int nr = cnt - base < rows_cap ? cnt - base : rows_cap;
+            __syncthreads();                                   // the readers of the rows staged before are done
+            for (int idx = tid; idx < nr * n8; idx += kGvThreads) {
+                const int r = idx / n8, c = idx - r * n8;
+                long long src;
+                if (SWIGLU) {
+                    int tok = u < p.G ? p.row_token[row0 + base + r] : base + r;
+                    tok = tok < 0 ? 0 : (tok >= p.T ? p.T - 1 : tok);
+                    src = tok;
+                } else {
+                    src = row0 + base + r;
+                }
+                *reinterpret_cast<uint4 *>(s_in + (size_t)r * in_bytes + (size_t)c * 16) =
+                    __ldg(reinterpret_cast<const uint4 *>(p.in + (size_t)src * p.IN) + c);
+            }
+            __syncthreads();
+            const bm_bf16 *base_a, *base_b;
+            size_t stride_q;
+            if (SWIGLU) {
+                base_a = p.Wa + (size_t)u * p.NQ * p.IN;
+                base_b = p.Wb + (size_t)u * p.NQ * p.IN;
+                stride_q = (size_t)p.IN;
+            } else {
+                base_a = p.Wa + (size_t)u * p.OUT * p.IN;
+                base_b = base_a + p.IN;
+                stride_q = 2 * (size_t)p.IN;
+            }
+            const size_t orow0 = (size_t)(row0 + base);
+            // rows past nr (up to the next power of two) are stale shared memory: computed, never stored
+            if (nr == 1) warp_units<1, SWIGLU>(base_a, base_b, stride_q, n8, qa + warp, qb, s_in, in_bytes, lane, nr, p.outp, orow0, p.OUT);
+            else if (nr == 2) warp_units<2, SWIGLU>(base_a, base_b, stride_q, n8, qa + warp, qb, s_in, in_bytes, lane, nr, p.outp, orow0, p.OUT);
+            else if (nr <= 4) warp_units<4, SWIGLU>(base_a, base_b, stride_q, n8, qa + warp, qb, s_in, in_bytes, lane, nr, p.outp, orow0, p.OUT);
+            else warp_units<8, SWIGLU>(base_a, base_b, stride_q, n8, qa + warp, qb, s_in, in_bytes, lane, nr, p.outp, orow0, p.OUT);
+        }
+        pos += qb - qa;
+    }
+}
+
+template <bool SWIGLU>
+cudaError_t launch_gemv(const GemvArgs &p, int kid, cudaStream_t stream) {
+    int rows_cap = kGvRows;
+    while (rows_cap > 1 && (size_t)rows_cap * p.IN * 2 > 200 * 1024) rows_cap >>= 1;
+    const size_t smem = (size_t)rows_cap * p.IN * 2 + (size_t)(p.G + p.S) * sizeof(int);
+    if (smem > 220 * 1024) return cudaErrorInvalidValue;
+    auto kern = gemv_kernel<SWIGLU>;
+    static size_t smem_set = 0;
+    if (smem > 48 * 1024 && smem > smem_set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        smem_set = smem;
+    }
+    profile_begin(kid, stream);
+    cudaError_t e = launch_kernel(kern, dim3(num_sms()), dim3(kGvThreads), smem, stream, p, rows_cap);
+    profile_end(kid, stream);
+    return e;
+}
+
+}  // namespace
+
+cudaError_t launch_forward_gemv(const ForwardArgs &a, cudaStream_t stream) {
+    GemvArgs p{};
+    p.offsets = a.r.offsets; p.row_token = a.r.row_token;
+    p.T = a.T; p.TK = a.T * a.K; p.G = a.G; p.S = a.S;
+    p.in = a.x; p.Wa = a.W1; p.Wb = a.W3; p.outp = a.h; p.IN = a.D; p.OUT = a.F; p.NQ = a.F;
+    cudaError_t e = launch_gemv<true>(p, BM_KERNEL_GEMM1, stream);
+    if (e != cudaSuccess) return e;
+    p.in = a.h; p.Wa = a.W2; p.Wb = a.W2; p.outp = a.y; p.IN = a.F; p.OUT = a.D; p.NQ = a.D / 2;
+    e = launch_gemv<false>(p, BM_KERNEL_GEMM2, stream);
+    if (e != cudaSuccess) return e;
+    return launch_combine(a, stream);
+}
+
+}  // namespace bm

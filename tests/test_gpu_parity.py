@@ -12,7 +12,7 @@ from helpers import bf16_tensor, rand_layer
 
 pytestmark = pytest.mark.gpu
 
-PATHS = {"simt": 3, "decode": 1, "prefill": 2}
+PATHS = {"simt": 3, "decode": 1, "prefill": 2, "gemv": 4}
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -98,7 +98,7 @@ def test_device_status_flags_bad_group_map_and_nonfinite():
 # ---------------------------------------------------------------------------------------------------
 # forward: every path on shapes spanning several tiles and ragged tails
 # ---------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("path", ["simt", "decode", "prefill"])
+@pytest.mark.parametrize("path", ["simt", "decode", "prefill", "gemv"])
 @pytest.mark.parametrize("seed", [0, 1, 2])
 def test_tiny_config_all_paths(path, seed):
     L = make_layer(CONFIGS["tiny"], seed)                      # BJ:configs[0]
@@ -120,7 +120,7 @@ FWD_SHAPES = [
 ]
 
 
-@pytest.mark.parametrize("path", ["simt", "decode", "prefill"])
+@pytest.mark.parametrize("path", ["simt", "decode", "prefill", "gemv"])
 @pytest.mark.parametrize("T,D,F,E,K,G,S", FWD_SHAPES)
 def test_forward_parity_ragged_shapes(path, T, D, F, E, K, G, S):
     rng = np.random.default_rng(T * 7 + F)
@@ -130,6 +130,34 @@ def test_forward_parity_ragged_shapes(path, T, D, F, E, K, G, S):
     assert status == 0
     assert_routing_equal(g, o)
     assert_out_close(out, oracle_forward(L, o))
+
+
+GEMV_SHAPES = [
+    # T, D, F, E, K, G, S -- the shapes BM_PATH_AUTO sends to the matrix-vector path (T*K <= 4*G)
+    (1, 2048, 1408, 60, 4, 60, 0),        # BJ:configs[4], single-token decode
+    (1, 2048, 1408, 60, 4, 8, 0),
+    (16, 2048, 1408, 60, 4, 30, 0),       # random map: some sets have more than 8 rows (several passes)
+    (2, 4096, 14336, 8, 2, 1, 0),         # Mixtral shape: h rows of 28 KB, 4 staged rows at most
+    (3, 264, 1000, 16, 4, 16, 2),         # shared experts, ragged chunk counts (33 and 125 chunks)
+    (7, 4096, 72, 9, 3, 9, 0),
+]
+
+
+@pytest.mark.parametrize("T,D,F,E,K,G,S", GEMV_SHAPES)
+def test_gemv_path_parity(T, D, F, E, K, G, S):
+    rng = np.random.default_rng(T * 31 + G)
+    L = rand_layer(rng, T=T, D=D, F=F, E=E, K=K, G=G, S=S, bias=True, wstd=0.02 if D >= 1024 else 0.05)
+    o = oracle_route(L)
+    want = oracle_forward(L, o)
+    for path in (PATHS["gemv"], 0):                            # forced, and as BM_PATH_AUTO picks it
+        g, out, status = gpu_layer(L, path)
+        assert status == 0
+        assert_routing_equal(g, o)
+        assert_out_close(out, want)
+    # the matrix-vector path defines out exactly like the prefill path (bf16 y rows, slot-order combine)
+    _, out_g, _ = gpu_layer(L, PATHS["gemv"])
+    _, out_g2, _ = gpu_layer(L, PATHS["gemv"])
+    assert np.array_equal(np.asarray(out_g), np.asarray(out_g2)), "gemv path must be deterministic"
 
 
 def test_empty_groups_and_empty_batch():
