@@ -14,7 +14,8 @@ constexpr unsigned kFullMask = 0xffffffffu;
 // ---------------------------------------------------------------------------------------------
 // Workspace layout (host-computed; all sections 1024-byte aligned).  Shapes only, never data.
 // ---------------------------------------------------------------------------------------------
-constexpr int kPermItemsPerBlock = 2048;   // (token, slot) items per CTA of the permutation kernels
+constexpr int kPermItemsPerBlock = 512;    // (token, slot) items per CTA of the three-kernel permutation
+constexpr int kPermSmallItems = 2048;      // up to this many items one CTA does the whole permutation in one launch
 constexpr int kMaxSchedTiles = 1 << 20;
 
 struct Workspace {

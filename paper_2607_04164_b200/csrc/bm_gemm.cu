@@ -647,6 +647,8 @@ dense_sched_kernel(int32_t *__restrict__ sched, int E, int T) {
 // fp32 accumulation in a fixed order -> deterministic.  One warp per token: lane s holds row and weight of
 // source s (K + S <= 32), the warp walks the D columns 16 bytes per lane (512 contiguous bytes per row and
 // step), four source rows in flight.
+constexpr int kCombineBatch = 4;     // source rows in flight per lane (8 measured slower: 79 -> 117 us at BJ:configs[2])
+
 __global__ void __launch_bounds__(256)
 combine_kernel(const bm_bf16 *__restrict__ y, int T, int D, int K, int S, const int32_t *__restrict__ n_slots,
                const int32_t *__restrict__ slot_row, const float *__restrict__ gate_w, bm_bf16 *__restrict__ out,
@@ -678,11 +680,11 @@ combine_kernel(const bm_bf16 *__restrict__ y, int T, int D, int K, int S, const 
             float acc[8];
 #pragma unroll
             for (int e = 0; e < 8; ++e) acc[e] = 0.0f;
-            for (int s0 = 0; s0 < n_src; s0 += 4) {
-                uint4 v[4];
-                float gw[4];
+            for (int s0 = 0; s0 < n_src; s0 += kCombineBatch) {
+                uint4 v[kCombineBatch];
+                float gw[kCombineBatch];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
+                for (int q = 0; q < kCombineBatch; ++q) {
                     const int src = min(s0 + q, 31);
                     const long long row = __shfl_sync(kFullMask, my_row, src);
                     gw[q] = __shfl_sync(kFullMask, my_gw, src);
@@ -691,7 +693,7 @@ combine_kernel(const bm_bf16 *__restrict__ y, int T, int D, int K, int S, const 
                     v[q] = ok ? *reinterpret_cast<const uint4 *>(y + (size_t)row * D + (size_t)c * 8) : make_uint4(0, 0, 0, 0);
                 }
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
+                for (int q = 0; q < kCombineBatch; ++q) {
                     if (s0 + q < n_src) {                        // warp-uniform; skipped sources add nothing
                         acc[0] = fmaf(gw[q], bf16_lo(v[q].x), acc[0]); acc[1] = fmaf(gw[q], bf16_hi(v[q].x), acc[1]);
                         acc[2] = fmaf(gw[q], bf16_lo(v[q].y), acc[2]); acc[3] = fmaf(gw[q], bf16_hi(v[q].y), acc[3]);
@@ -893,7 +895,7 @@ static cudaError_t launch_combine_raw(const ForwardArgs &a, cudaStream_t stream)
     // one warp per token; with few tokens a token's 32-chunk column slices go to different warps
     const int n_slices = (a.D / 8 + 31) / 32;
     int split = 1;
-    while (split < n_slices && (long long)a.T * split * 2 <= (long long)num_sms() * 8) split *= 2;
+    while (split < n_slices && (long long)a.T * split < (long long)num_sms() * tune_int("BM_COMBINE_WARPS", 64)) split *= 2;   // fill the SMs' warp slots
     if (split > n_slices) split = n_slices;
     const long long items = (long long)a.T * split;
     return launch_kernel(combine_kernel, dim3((unsigned)std::min<long long>((items + 7) / 8, (long long)num_sms() * 8)),
