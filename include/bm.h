@@ -19,8 +19,9 @@
  *     the library never allocates, frees or synchronises (except bm_moe_layer_host,
  *     bm_device_status and the bm_profile_* pair, which say so) and borrows the buffers until the work enqueued on `stream`
  *     has completed.  All device pointers must be 16-byte aligned.
- *   - The first 256 bytes of `workspace` hold the device status word: zero them once after
- *     allocation (or call bm_device_status once).
+ *   - The first 4096 bytes of `workspace` hold the device status word and the arrival counters of the
+ *     small-batch router: zero them once after allocation.  Kernels put the counters back to zero, so
+ *     calls that complete leave the head ready for the next call; after a failed launch zero it again.
  *   - `stream` is a cudaStream_t (0 = the legacy default stream).
  *   - Return value: BM_OK (0) or a negative bm_status, checked synchronously on the host before
  *     anything is enqueued.  T == 0 is BM_OK and a no-op.  Data-dependent faults (a group_map entry

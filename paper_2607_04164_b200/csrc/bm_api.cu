@@ -117,13 +117,14 @@ static int route_common(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router,
         return BM_OK;
     }
     profile_begin(BM_KERNEL_ROUTER, st);
+    bool fused_permute = false;
     if (launch_router(x, T, D, W_router, router_bias, E, K, GroupMap{group_map, partial ? cold_mask : nullptr, G},
-                      *routing, status, st) != cudaSuccess)
+                      *routing, status, reinterpret_cast<float *>(ws + full.route_logits), &fused_permute, st) != cudaSuccess)
         return BM_ERR_CUDA;
     profile_end(BM_KERNEL_ROUTER, st);
     profile_begin(BM_KERNEL_PERMUTE, st);
-    if (launch_permute(T, K, NS, *routing, reinterpret_cast<int32_t *>(ws + full.block_hist), status, st) !=
-        cudaSuccess)
+    if (!fused_permute &&
+        launch_permute(T, K, NS, *routing, reinterpret_cast<int32_t *>(ws + full.block_hist), status, st) != cudaSuccess)
         return BM_ERR_CUDA;
     profile_end(BM_KERNEL_PERMUTE, st);
     return BM_OK;

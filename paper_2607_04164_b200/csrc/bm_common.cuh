@@ -20,8 +20,11 @@ constexpr int kMaxSchedTiles = 1 << 20;
 
 struct Workspace {
     // byte offsets from the workspace base
-    size_t status;       // int32[64]: [0] device status bits, [1] A (copy of offsets[G]), [2..] counters
+    size_t status;       // int32[1024]: [0] device status bits, [1] A (copy of offsets[G]), [2] tokens routed (split
+                         // router), [64..64+512) expert slices done per token (split router); zeroed once by the caller,
+                         // the counters are put back to zero by the kernel that used them
     size_t block_hist;   // int32[nb * G]   per-block group histograms / bases of the permutation
+    size_t route_logits; // f32[min(T, 512) * BM_MAX_E]  logits of the split router (T < 512), gathered by a token's last CTA
     size_t sched;        // int32[kSchedInts] tile-schedule scratch of the forward pass
     size_t xs;           // bf16[T*K, D]    token rows gathered in permuted order (prefill path)
     size_t h;            // bf16[T*K + S*T, F]  SwiGLU intermediate
@@ -30,6 +33,10 @@ struct Workspace {
     size_t total;
 };
 
+constexpr int kStatusInts = 1024;                               // the zero-once head of the workspace (4096 bytes)
+constexpr int kSplitRouterMaxT = 512;                           // the split (latency) router serves T < 512
+constexpr int kStatusTokCnt = 64;                               // status[64 + t]: expert slices of token t done
+constexpr int kStatusDone = 2;                                  // status[2]: tokens routed
 constexpr int kMaxShared = 16;                                  // S <= 16 always-on shared experts
 constexpr int kSchedInts = 4 + 5 * (BM_MAX_G + kMaxShared) + 8;
 
@@ -40,8 +47,9 @@ __host__ inline Workspace workspace_layout(int T, int D, int F, int K, int G, in
     size_t off = 0;
     const size_t items = (size_t)T * K;
     const size_t nb = (items + kPermItemsPerBlock - 1) / kPermItemsPerBlock;
-    w.status = off;      off = align_up(off + 64 * sizeof(int32_t), 1024);
+    w.status = off;      off = align_up(off + kStatusInts * sizeof(int32_t), 1024);
     w.block_hist = off;  off = align_up(off + (nb > 0 ? nb : 1) * (size_t)G * sizeof(int32_t), 1024);
+    w.route_logits = off; off = align_up(off + (size_t)(T < kSplitRouterMaxT ? T : kSplitRouterMaxT) * BM_MAX_E * sizeof(float), 1024);
     w.sched = off;       off = align_up(off + kSchedInts * sizeof(int32_t), 1024);
     w.xs = off;          off = align_up(off + items * D * sizeof(bm_bf16), 1024);
     w.h = off;           off = align_up(off + (items + (size_t)S * T) * F * sizeof(bm_bf16), 1024);
@@ -94,8 +102,10 @@ struct GroupMap {
     int G;
 };
 
+// *fused_permute is set when the router kernel also ran the permutation (small batches: its last CTA does it)
 cudaError_t launch_router(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const float *bias, int E,
-                          int K, GroupMap gm, const bm_routing &r, int32_t *status, cudaStream_t stream);
+                          int K, GroupMap gm, const bm_routing &r, int32_t *status, float *route_logits,
+                          bool *fused_permute, cudaStream_t stream);
 
 cudaError_t launch_permute(int T, int K, int G, const bm_routing &r, int32_t *block_hist, int32_t *status,
                            cudaStream_t stream);

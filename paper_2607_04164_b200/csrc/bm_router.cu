@@ -14,7 +14,10 @@
 // keeps a register tile acc[TOK][ET] (TOK tokens x ET experts) and walks D once per expert tile.
 // Small T (decode): TOK = 1, warps split the experts, one CTA per token -> latency-bound, ~2 us.
 // Large T (prefill): TOK = 4, ET = 8, warps split the tokens -> each W_router chunk feeds 32 FMAs.
+#include <algorithm>
+
 #include "bm_common.cuh"
+#include "bm_permute.cuh"
 #include "bm_ptx.cuh"
 
 namespace bm {
@@ -176,6 +179,104 @@ router_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *__rest
         if (t >= T) break;
         select_and_write(s_logits + tl * E, t, lane, E, K, gm, expert_ids, group_ids, gate_w, n_slots, status);
     }
+}
+
+// -------------------------------------------------------------------------------------------------
+// Latency shape with the experts of a token spread over CTAs (T <= 16, E > 8).  CTA (es, t) computes the
+// logits of 8 * ET experts of token t -- a warp owns ET dot products in the canonical order -- and parks them
+// in a global scratch row.  The CTA that completes a token (arrival counter) runs R2-R5 for it; the CTA that
+// completes the batch runs the whole permutation R6-R8 when it fits one CTA (T*K <= 2048), which saves the
+// launch of the permutation kernel.  Counters live in the zero-once head of the workspace and are put back
+// to zero by the CTA that consumed them.  Writers fence before they signal (the threadFenceReduction
+// pattern); the consumers read the other CTAs' results with ld.global.cg.
+// One token on one CTA (router_kernel) streams all of W_router through a single SM: 7 us at E = 60, D = 2048.
+// -------------------------------------------------------------------------------------------------
+template <int ET>
+__global__ void __launch_bounds__(kWarps * 32)
+router_split_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *__restrict__ Wr,
+                    const float *__restrict__ bias, int E, int K, GroupMap gm, int ES, float *__restrict__ logits_ws,
+                    int fuse_permute, int per_warp, bm_routing r, int32_t *__restrict__ status) {
+    extern __shared__ int rs_dyn[];       // float [E] for the select, then the permutation's scratch
+    __shared__ int s_flag, s_total;
+    grid_dep_wait();      // x may come from a predecessor; the routing arrays may still be read by one
+    grid_dep_launch();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int t = blockIdx.y;
+    const int e0 = (blockIdx.x * kWarps + warp) * ET;
+
+    // ---- R1: ET logits per warp ---------------------------------------------------------------
+    if (e0 < E) {
+        const bm_bf16 *xrow = x + (size_t)t * D;
+        const bm_bf16 *wrow[ET];
+#pragma unroll
+        for (int j = 0; j < ET; ++j) wrow[j] = Wr + (size_t)(e0 + j < E ? e0 + j : E - 1) * D;
+        float acc[ET];
+#pragma unroll
+        for (int j = 0; j < ET; ++j) acc[j] = 0.0f;
+#pragma unroll 4
+        for (int k = lane * 8; k < D; k += 256) {
+            const uint4 xv = __ldg(reinterpret_cast<const uint4 *>(xrow + k));
+            uint4 wv[ET];
+#pragma unroll
+            for (int j = 0; j < ET; ++j) wv[j] = __ldg(reinterpret_cast<const uint4 *>(wrow[j] + k));
+#pragma unroll
+            for (int j = 0; j < ET; ++j) {
+                float p = acc[j];                    // ascending element order inside the chunk
+                p = __fmaf_rn(bf16_lo(xv.x), bf16_lo(wv[j].x), p);
+                p = __fmaf_rn(bf16_hi(xv.x), bf16_hi(wv[j].x), p);
+                p = __fmaf_rn(bf16_lo(xv.y), bf16_lo(wv[j].y), p);
+                p = __fmaf_rn(bf16_hi(xv.y), bf16_hi(wv[j].y), p);
+                p = __fmaf_rn(bf16_lo(xv.z), bf16_lo(wv[j].z), p);
+                p = __fmaf_rn(bf16_hi(xv.z), bf16_hi(wv[j].z), p);
+                p = __fmaf_rn(bf16_lo(xv.w), bf16_lo(wv[j].w), p);
+                p = __fmaf_rn(bf16_hi(xv.w), bf16_hi(wv[j].w), p);
+                acc[j] = p;
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < ET; ++j) {
+            float p = acc[j];
+#pragma unroll
+            for (int o = 16; o >= 1; o >>= 1) p = __fadd_rn(p, __shfl_xor_sync(kFullMask, p, o));
+            if (lane == 0 && e0 + j < E) {
+                if (bias) p = __fadd_rn(p, bias[e0 + j]);
+                __stcg(logits_ws + (size_t)t * E + e0 + j, p);
+            }
+        }
+        if (lane == 0) __threadfence();
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        s_flag = atomicAdd(status + kStatusTokCnt + t, 1) == ES - 1;
+    }
+    __syncthreads();
+    if (!s_flag) return;
+
+    // ---- R2-R5: this CTA completed token t -------------------------------------------------------
+    if (warp == 0) {
+        __threadfence();
+        float *s_l = reinterpret_cast<float *>(rs_dyn);
+        for (int e = lane; e < E; e += 32) s_l[e] = __ldcg(logits_ws + (size_t)t * E + e);
+        __syncwarp();
+        select_and_write(s_l, t, lane, E, K, gm, r.expert_ids, r.group_ids, r.gate_w, r.n_slots, status);
+        if (lane == 0) status[kStatusTokCnt + t] = 0;
+        __threadfence();
+    }
+    if (!fuse_permute) return;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        s_flag = atomicAdd(status + kStatusDone, 1) == T - 1;
+        if (s_flag) status[kStatusDone] = 0;
+    }
+    __syncthreads();
+    if (!s_flag) return;
+
+    // ---- R6-R8: this CTA completed the batch ---------------------------------------------------------
+    __threadfence();
+    permute_block_small(r.group_ids, T, K, r.G, per_warp, r.counts, r.offsets, r.row_token, r.row_slot, r.slot_row,
+                        status, rs_dyn, &s_total);
 }
 
 // -------------------------------------------------------------------------------------------------
@@ -447,10 +548,24 @@ cudaError_t launch_cfg(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const 
 }  // namespace
 
 cudaError_t launch_router(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const float *bias, int E,
-                          int K, GroupMap gm, const bm_routing &r, int32_t *status,
-                          cudaStream_t stream) {
-    if (T >= tune_int("BM_ROUTER_TP_MIN_T", 512))   // throughput shape: operands staged through shared memory
+                          int K, GroupMap gm, const bm_routing &r, int32_t *status, float *route_logits,
+                          bool *fused_permute, cudaStream_t stream) {
+    *fused_permute = false;
+    if (T >= tune_int("BM_ROUTER_TP_MIN_T", kSplitRouterMaxT))   // throughput shape: operands staged through shared memory
         return launch_tp(x, T, D, Wr, bias, E, K, gm, r, status, stream);
+    // (measured: 2 us faster than router + permutation kernels at T = 1, even at T = 16, slower from T = 64 on:
+    // more CTAs and two rounds of arrival counters)
+    if (E > 8 && T <= tune_int("BM_ROUTER_SPLIT_MAX_T", 16)) {
+        // latency shape, experts spread over CTAs; the last CTA also permutes when one CTA can
+        constexpr int ET = 2;
+        const int ES = (E + kWarps * ET - 1) / (kWarps * ET);
+        const bool fuse = (long long)T * K <= kPermSmallItems;
+        size_t smem = (size_t)E * sizeof(float);
+        if (fuse) smem = std::max(smem, (size_t)(kWarps * r.G + r.G + 512) * sizeof(int));
+        *fused_permute = fuse;
+        return launch_kernel(router_split_kernel<ET>, dim3(ES, T), dim3(kWarps * 32), smem, stream, x, T, D, Wr, bias, E, K,
+                             gm, ES, route_logits, fuse ? 1 : 0, kPermSmallItems / kWarps, r, status);
+    }
     // latency shape: one token per warp pass, warps split the experts
     if (E <= 8) {
         int WE = 1;
