@@ -37,14 +37,17 @@ constexpr int kAccStages = 2;
 constexpr int kAccCols = 256;
 constexpr int kTmemCols = kAccStages * kAccCols;
 constexpr int kThreads = 192;
+constexpr int kGatherCopyThreads = 128; // GA: warps 6..9 gather the token rows of GEMM1's A tile
+constexpr int kGatherRelays = 6;        // + warps 10..15, which relay "copies landed" to the stages' full barriers (ring stage s -> relay s % 6)
+constexpr int kGatherThreads = kGatherCopyThreads + 32 * kGatherRelays;
 constexpr int kChunkRows = 128;
 constexpr int kMaxSeg = BM_MAX_G + kMaxShared;
 constexpr size_t kSmemMax = 232448;         // 227 KB, the per-CTA opt-in limit of sm_100
-constexpr size_t kSmemBars = 256;           // (2*kMaxStages + 2*kAccStages) mbarriers + the TMEM base address
+constexpr size_t kSmemBars = 512;           // (3*kMaxStages + 2*kAccStages) mbarriers + the TMEM base address
 constexpr size_t kEpiStageBytes = 32 * 32 * 4;   // PF_GEMM2: per-epilogue-warp transpose buffer (32 rows x 32 fp32)
 constexpr size_t kSmemEpi = 4 * kEpiStageBytes;
 constexpr size_t kSmemRing = kSmemMax - 1024 /*align slack*/ - kSmemBars;   // minus kSmemEpi for PF_GEMM2
-static_assert((2 * kMaxStages + 2 * kAccStages) * 8 + 4 <= kSmemBars, "barrier block too small");
+static_assert((3 * kMaxStages + 2 * kAccStages + 1) * 8 <= kSmemBars, "barrier block too small");
 
 enum Mode { PF_GEMM1 = 0, PF_GEMM2 = 1, DC_GEMM1 = 2, DC_GEMM2 = 3 };
 
@@ -85,6 +88,7 @@ struct GemmParams {
     int n_wtiles;       // tiles along the weight-row dimension
     int seg_cap;        // G + S + 1: entries per schedule array cached in shared memory
     const int32_t *counts, *offsets, *row_token, *row_slot;
+    const bm_bf16 *x;   // GA: token rows gathered straight from x [T, D]
     const float *gate_w;
     const int32_t *sched;
     bm_bf16 *h;
@@ -151,8 +155,8 @@ __device__ __forceinline__ float silu_mul(float a, float b) {
     return __fdividef(a, 1.0f + __expf(-a)) * b;
 }
 
-template <int MODE, bool K2 = false>
-__global__ void __launch_bounds__(kThreads, 1)
+template <int MODE, bool K2 = false, bool GA = false>
+__global__ void __launch_bounds__(kThreads + (GA ? kGatherThreads : 0), 1)
 gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D]; GEMM2: H [TK+S*T, F]
             const __grid_constant__ CUtensorMap tm_act1,   // GEMM1: x [T, D] (shared experts); GEMM2: unused
             const __grid_constant__ CUtensorMap tm_w0,     // GEMM1: W1 [G+S, F, D]; GEMM2: W2 [G+S, D, F]
@@ -161,6 +165,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
     constexpr bool kDecode = (MODE == DC_GEMM1 || MODE == DC_GEMM2);
     constexpr bool kGemm1 = (MODE == PF_GEMM1 || MODE == DC_GEMM1);
     static_assert(!K2 || !kDecode, "CTA pairs are a prefill-tile feature");
+    static_assert(!GA || MODE == PF_GEMM1, "the in-kernel gather feeds GEMM1's activation tile");
     // K2: the two CTAs of a cluster form a CTA pair; rank 0 (the leader) issues the M = 256 MMAs for both
     const uint32_t rank = K2 ? ptx::cluster_ctarank() : 0u;
     const bool leader = rank == 0;
@@ -177,6 +182,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
     uint64_t *tfull = bars + 2 * kMaxStages;     // [kAccStages]
     uint64_t *tempty = tfull + kAccStages;       // [kAccStages]
     uint32_t *tmem_ptr = reinterpret_cast<uint32_t *>(tempty + kAccStages);
+    uint64_t *gfull = tempty + kAccStages + 1;   // [kMaxStages] GA: the gather threads' copies of a stage have landed
     uint8_t *epi_stage = reinterpret_cast<uint8_t *>(bars) + kSmemBars;   // [4][kEpiStageBytes], 256-byte aligned
     int32_t *s_sched = reinterpret_cast<int32_t *>(epi_stage + (MODE == PF_GEMM2 ? kSmemEpi : 0));   // [5][seg_cap]
 
@@ -187,7 +193,9 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
         ptx::prefetch_tmap(&tm_act0);
         ptx::prefetch_tmap(&tm_w0);
         if (kGemm1) { ptx::prefetch_tmap(&tm_act1); ptx::prefetch_tmap(&tm_w1); }
-        for (int i = 0; i < n_stages; ++i) { ptx::mbar_init(&full[i], 1); ptx::mbar_init(&empty[i], 1); }
+        // GA: a stage is full when the TMA bytes (weights) have landed AND the relay warp (both CTAs' under K2) has signalled that the gathered rows are in place
+        for (int i = 0; i < n_stages; ++i) { ptx::mbar_init(&full[i], GA ? 1 + (K2 ? 2 : 1) : 1); ptx::mbar_init(&empty[i], 1); }
+        if (GA) for (int i = 0; i < n_stages; ++i) ptx::mbar_init(&gfull[i], kGatherCopyThreads);
         // K2: the leader's tempty collects the 4 epilogue warps of BOTH CTAs
         for (int i = 0; i < kAccStages; ++i) { ptx::mbar_init(&tfull[i], 1); ptx::mbar_init(&tempty[i], K2 ? 8 : 4); }
         ptx::fence_barrier_init();
@@ -206,7 +214,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
     // bytes one stage receives.  Decode: the weight box(es) of R rows plus the item's token rows in 32-row
     // boxes (tok_tx(n)): only the rows the group really has travel from L2.
     // K2: a CTA stages A (16 KB) + its half of B (16 KB); the leader's barrier counts both CTAs' bytes
-    const uint32_t w_tx = K2 ? 4u * kTileBytes16K : !kDecode ? 3u * kTileBytes16K : (uint32_t)((kGemm1 ? 2 : 1) * p.R * 128);
+    const uint32_t w_tx = GA ? 2u * kTileBytes16K : K2 ? 4u * kTileBytes16K : !kDecode ? 3u * kTileBytes16K : (uint32_t)((kGemm1 ? 2 : 1) * p.R * 128);
     auto stage_tx_of = [&](int n) -> uint32_t { return kDecode ? w_tx + (uint32_t)((n + 31) >> 5) * 4096u : w_tx; };
 
     // DC_GEMM2: W2 does not depend on the predecessor (GEMM1), so warp 0 fills the ring with the weight tiles
@@ -236,7 +244,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
     sv.total_pairs = p.sched[2];
     sv.u = s_sched; sv.chunk0 = s_sched + cap; sv.rows = s_sched + 2 * cap; sv.off = s_sched + 3 * cap;
     sv.pair0 = s_sched + 4 * cap;
-    for (int i = threadIdx.x; i <= sv.n_seg; i += kThreads) {
+    for (int i = threadIdx.x; i <= sv.n_seg; i += (int)blockDim.x) {
         s_sched[i] = p.sched[kSchedSegU + i];
         s_sched[cap + i] = p.sched[kSchedChunk0 + i];
         s_sched[2 * cap + i] = p.sched[kSchedRows + i];
@@ -283,7 +291,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
                     if (ptx::elect_one()) {
                         uint8_t *st = smem + (size_t)stage * stage_bytes;
                         if (leader) ptx::mbar_arrive_expect_tx(&full[stage], stage_tx);
-                        ptx::tma_load_2d_pair(st, tm_act, &full[stage], kc, it.act_row0, ptx::kEvictLast);
+                        if (!GA) ptx::tma_load_2d_pair(st, tm_act, &full[stage], kc, it.act_row0, ptx::kEvictLast);
                         if (MODE == PF_GEMM1)       // B rows 0-127 = the W1 tile (leader), 128-255 = the W3 tile (peer)
                             ptx::tma_load_3d_pair(st + kTileBytes16K, leader ? &tm_w0 : &tm_w1, &full[stage], kc, wrow0, it.u,
                                                   ptx::kEvictFirst);
@@ -296,7 +304,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
                     ptx::mbar_arrive_expect_tx(&full[stage], stage_tx);
                     if (!kDecode) {
                         // A = 128 activation rows, B = 256 weight rows (W1|W3 tiles, or one W2 tile of 256)
-                        ptx::tma_load_2d(st, tm_act, &full[stage], kc, it.act_row0, ptx::kEvictLast);
+                        if (!GA) ptx::tma_load_2d(st, tm_act, &full[stage], kc, it.act_row0, ptx::kEvictLast);
                         ptx::tma_load_3d(st + kTileBytes16K, &tm_w0, &full[stage], kc, wrow0, it.u, ptx::kEvictFirst);
                         if (MODE == PF_GEMM1)
                             ptx::tma_load_3d(st + 2 * kTileBytes16K, &tm_w1, &full[stage], kc, wrow0, it.u, ptx::kEvictFirst);
@@ -365,7 +373,77 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
             }
             if (++acc == kAccStages) { acc = 0; acc_phase ^= 1; }
         }
-    } else {
+    } else if (GA && warp >= 6 && warp < 10) {
+        // =========================== gather (warps 6..9, GA) ===========================
+        // Step 9 inside GEMM1: the gather threads copy the 128 rows of the item's A tile straight from x -- 128 bytes per
+        // row and k-block as eight 16-byte cp.async, written in the 128B-swizzle layout TMA would have produced (16-byte
+        // chunk j of row r at chunk j ^ (r & 7)); columns past D are zero-filled like TMA's out-of-bounds fill.
+        // Thread g = (row group rg = g / 8, chunk j = g % 8) copies chunk j of rows rg, rg + 16, ..., rg + 112: eight
+        // neighbouring lanes cover one row's 128 contiguous bytes, so a warp instruction touches 4 rows x 4 sectors
+        // (one row per lane scattered every 16-byte piece into its own sector request: 2-4x slower GEMM1).
+        // Completion is signalled by the hardware: cp.async.mbarrier.arrive.noinc makes the thread's arrival on the
+        // stage's gfull barrier happen when its copies have landed, so the thread never waits for its own copies and
+        // the whole ring depth stays in flight (a cp.async.wait_group + arrive version kept only 2-3 k-blocks in
+        // flight: 3x slower with CTA pairs).  This replaces the xs pass of the prep kernel: A*D*4 bytes of HBM
+        // traffic and a launch-wide pass less.
+        const int g = (int)threadIdx.x - kThreads;
+        const int j = g & 7, rg = g >> 3;
+        uint32_t dst_off[8];             // row * 128 + swizzled chunk offset
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const int r = rg + 16 * i;
+            dst_off[i] = (uint32_t)r * 128u + ((uint32_t)(j ^ (r & 7)) << 4);
+        }
+        int stage = 0;
+        uint32_t phase = 0;
+        Item it;
+        for (int item = item0; get_item<MODE, K2>(p, sv, item, it, rank); item += item_stride) {
+            const bm_bf16 *src[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const int r = rg + 16 * i;
+                const int rr = it.n > 0 ? min(r, it.n - 1) : 0;      // rows past the chunk's: a valid row, never stored
+                int tok = it.shared ? it.tok0 + rr : p.row_token[it.perm_row0 + rr];
+                tok = tok < 0 ? 0 : (tok >= p.T ? p.T - 1 : tok);
+                src[i] = p.x + (size_t)tok * p.D + j * 8;
+            }
+            for (int kb = 0; kb < nkb; ++kb) {
+                ptx::mbar_wait(&empty[stage], phase ^ 1);
+                const uint32_t dst = ptx::smem_u32(smem + (size_t)stage * stage_bytes);
+                const int kc = kb * kBlockK;
+                const bool in = kc + j * 8 < p.D;                    // columns past D: zero fill, like TMA
+#pragma unroll
+                for (int i = 0; i < 8; ++i) ptx::cp_async_16(dst + dst_off[i], src[i] + (in ? kc : 0), in ? 16u : 0u);
+                ptx::cp_async_mbar_arrive_noinc(&gfull[stage]);
+                if (++stage == n_stages) { stage = 0; phase ^= 1; }
+            }
+        }
+    } else if (GA && warp >= 10) {
+        // =========================== gather relays (warps 10..15, GA) ===========================
+        // Relay w owns the ring stages s = w, w + 6, ... (one relay per stage keeps the waits on a stage's barrier in
+        // phase order): for each k-block of such a stage it waits until all 128 gather threads' copies
+        // have landed, fences them towards the async proxy (tcgen05.mma reads shared memory through it) and
+        // arrives on the stage's full barrier -- the leader's under K2.  Fence + cluster-scope arrive cost one relay
+        // about a k-block's time (ncu: the single relay of the first version was the kernel's bottleneck with CTA
+        // pairs, GEMM1 3x slower), so up to six work side by side.
+        const uint32_t full_base = K2 ? ptx::mapa_u32(&full[0], 0) : ptx::smem_u32(&full[0]);
+        const int rw = warp - 10;
+        int n = 0;                       // running k-block number of this CTA
+        Item it;
+        for (int item = item0; get_item<MODE, K2>(p, sv, item, it, rank); item += item_stride) {
+            for (int kb = 0; kb < nkb; ++kb, ++n) {
+                const int stage = n % n_stages;
+                if (stage % kGatherRelays != rw) continue;
+                ptx::mbar_wait(&gfull[stage], (uint32_t)(n / n_stages) & 1u);
+                if (lane == 0) {
+                    ptx::fence_proxy_async_smem();
+                    if (K2) ptx::mbar_arrive_cluster(full_base + (uint32_t)stage * 8u);
+                    else ptx::mbar_arrive(&full[stage]);
+                }
+                __syncwarp();
+            }
+        }
+    } else if (!GA || warp < 6) {
         // =========================== epilogue (warps 2..5) ===========================
         const int q = warp & 3;                      // TMEM lane quarter this warp may read
         const int row = q * 32 + lane;               // accumulator row (M index) owned by this thread
@@ -598,6 +676,7 @@ prep_kernel(const bm_bf16 *__restrict__ x, int T, int D, int K, int G, int S,
         o4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     // gather: one warp per permuted row.  (A tile::gather4 producer in GEMM1 was measured instead of this
     // pass: ~12 cycles per 128-byte row made GEMM1 3x slower, so the rows are materialised once here.)
+    if (!xs) return;                     // prefill tiles: GEMM1 gathers the rows itself (GA)
     const int A = min(offsets[G], T * K);
     const int warps = (gridDim.x * blockDim.x) >> 5;
     const int lane = threadIdx.x & 31;
@@ -839,10 +918,11 @@ void ring_geometry(bool decode, bool gemm1, int T, GemmParams *p, bool pair = fa
     p->stages = st;
 }
 
-template <int MODE, bool K2 = false>
+template <int MODE, bool K2 = false, bool GA = false>
 cudaError_t launch_gemm(const CUtensorMap &a0, const CUtensorMap &a1, const CUtensorMap &w0, const CUtensorMap &w1,
                         const GemmParams &p, cudaStream_t stream) {
-    auto kern = gemm_kernel<MODE, K2>;
+    auto kern = gemm_kernel<MODE, K2, GA>;
+    constexpr int kBlock = kThreads + (GA ? kGatherThreads : 0);
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
@@ -855,11 +935,11 @@ cudaError_t launch_gemm(const CUtensorMap &a0, const CUtensorMap &a1, const CUte
     profile_begin(kid, stream);
     cudaError_t e;
     if (!K2) {
-        e = launch_kernel(kern, dim3(num_sms()), dim3(kThreads), smem, stream, a0, a1, w0, w1, p);
+        e = launch_kernel(kern, dim3(num_sms()), dim3(kBlock), smem, stream, a0, a1, w0, w1, p);
     } else {
         // CTA pairs: clusters of two CTAs (one TPC each), one pair per two SMs
         cudaLaunchConfig_t cfg{};
-        cfg.gridDim = dim3(num_sms() & ~1); cfg.blockDim = dim3(kThreads); cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+        cfg.gridDim = dim3(num_sms() & ~1); cfg.blockDim = dim3(kBlock); cfg.dynamicSmemBytes = smem; cfg.stream = stream;
         cudaLaunchAttribute attr[2];
         attr[0].id = cudaLaunchAttributeClusterDimension;
         attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
@@ -919,12 +999,27 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
     // tensor-parallel partial (out_f32): the decode path accumulates straight into the caller's buffer
     float *acc_buf = (decode && a.out_f32) ? a.out_f32 : a.out_acc;
 
+    // CTA pairs (cta_group::2, M = 256 per pair): a pair shares the weight tile, so a CTA stages 32 KB per
+    // k-block instead of 48 KB (measured: GEMM1 232 -> 201 us at BJ:configs[3]).  A segment with an odd chunk
+    // count wastes half a pair, so pairs are used when a group expects >= 4 chunks (measured: no gain at
+    // 273 rows/group, 7% slower at 107 rows/group).  BM_PF_PAIR=0/1 overrides.
+    const int pair_env = tune_int("BM_PF_PAIR", -1);
+    const bool many_rows = (long long)a.T * a.K >= 4LL * kChunkRows * a.G;
+    const bool pair = !decode && (sms & 1) == 0 && (pair_env < 0 ? many_rows : pair_env != 0);
+    // GA: GEMM1's own warps gather the token rows (single-CTA prefill tiles); the prep kernel then only builds the
+    // schedule.  Measured (T = 4096, G = 60): step 410 -> 398 us (GEMM1 +14 us, gather pass -20 us, A*D*4 bytes of
+    // HBM traffic less).  Not with CTA pairs: the peer's "rows landed" must reach the leader's barrier through a
+    // fence and a cluster-scope arrive per k-block, which lengthens the ring's turn-around -- GEMM1 30-36% slower
+    // than the TMA-fed pair kernel even with one relay warp per ring stage (BM_PF_GATHER=2 forces it).
+    const int ga_env = tune_int("BM_PF_GATHER", 1);
+    const bool gather_in_gemm = !decode && (ga_env == 2 || (ga_env == 1 && !pair));
+
     // step 9 (+ schedule, + zero)
     {
         const int grid = sms * 4;
         profile_begin(BM_KERNEL_PREP, stream);
         cudaError_t e = launch_kernel(prep_kernel, dim3(grid), dim3(256), 0, stream, a.x, a.T, a.D, a.K, a.G, a.S,
-                                      a.r.counts, a.r.offsets, a.r.row_token, a.sched, a.xs, acc_buf, decode ? 1 : 0, a.status);
+                                      a.r.counts, a.r.offsets, a.r.row_token, a.sched, gather_in_gemm ? nullptr : a.xs, acc_buf, decode ? 1 : 0, a.status);
         if (e != cudaSuccess) return e;
         profile_end(BM_KERNEL_PREP, stream);
     }
@@ -933,7 +1028,7 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
     p.seg_cap = a.G + a.S + 1;
     p.T = a.T; p.D = a.D; p.F = a.F; p.K = a.K; p.G = a.G; p.S = a.S; p.TK = TK;
     p.counts = a.r.counts; p.offsets = a.r.offsets; p.row_token = a.r.row_token; p.row_slot = a.r.row_slot;
-    p.gate_w = a.r.gate_w; p.sched = a.sched; p.h = a.h; p.out_acc = acc_buf; p.y = a.y;
+    p.gate_w = a.r.gate_w; p.sched = a.sched; p.h = a.h; p.out_acc = acc_buf; p.y = a.y; p.x = a.x;
 
 
     const uint64_t h_rows = (uint64_t)TK + (uint64_t)a.S * a.T;
@@ -947,19 +1042,16 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
             !make_map_3d(&m_w2, a.W2, a.G + a.S, a.D, a.F, 256) || !make_map_2d(&m_h, a.h, h_rows, a.F, 128))
             return cudaErrorInvalidValue;
         p.ksplit = 1;
-        // CTA pairs (cta_group::2, M = 256 per pair): a pair shares the weight tile, so a CTA stages 32 KB per
-        // k-block instead of 48 KB (measured: GEMM1 232 -> 201 us at BJ:configs[3]).  A segment with an odd chunk
-        // count wastes half a pair, so pairs are used when a group expects >= 4 chunks (measured: no gain at
-        // 273 rows/group, 7% slower at 107 rows/group).  BM_PF_PAIR=0/1 overrides.
-        const int pair_env = tune_int("BM_PF_PAIR", -1);
-        const bool many_rows = (long long)a.T * a.K >= 4LL * kChunkRows * a.G;
-        const bool pair = (sms & 1) == 0 && (pair_env < 0 ? many_rows : pair_env != 0);
         CUtensorMap m_w2h;
         if (pair && !make_map_3d(&m_w2h, a.W2, a.G + a.S, a.D, a.F, 128)) return cudaErrorInvalidValue;
         ring_geometry(false, true, a.T, &p, pair);
         p.kblocks = kb1; p.R = 128; p.n_wtiles = (a.F + 127) / 128;
-        err = pair ? launch_gemm<PF_GEMM1, true>(m_xs, m_x, m_w1, m_w3, p, stream)
-                   : launch_gemm<PF_GEMM1>(m_xs, m_x, m_w1, m_w3, p, stream);
+        if (gather_in_gemm)
+            err = pair ? launch_gemm<PF_GEMM1, true, true>(m_xs, m_x, m_w1, m_w3, p, stream)
+                       : launch_gemm<PF_GEMM1, false, true>(m_xs, m_x, m_w1, m_w3, p, stream);
+        else
+            err = pair ? launch_gemm<PF_GEMM1, true>(m_xs, m_x, m_w1, m_w3, p, stream)
+                       : launch_gemm<PF_GEMM1>(m_xs, m_x, m_w1, m_w3, p, stream);
         if (err != cudaSuccess) return err;
         p.kblocks = kb2; p.R = 256; p.n_wtiles = (a.D + 255) / 256;
         err = pair ? launch_gemm<PF_GEMM2, true>(m_h, m_h, m_w2h, m_w2h, p, stream)
@@ -1015,7 +1107,7 @@ cudaError_t launch_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 
     GemmParams p{};
     p.seg_cap = E + 1;
     p.T = T; p.D = D; p.F = F; p.K = 1; p.G = 0; p.S = E; p.TK = 0;
-    p.sched = sched; p.h = h; p.y = y;
+    p.sched = sched; p.h = h; p.y = y; p.x = x;
     p.ksplit = 1;
     const bool pair = (num_sms() & 1) == 0 && T >= 4 * kChunkRows && tune_int("BM_PF_PAIR", -1) != 0;   // as launch_forward_tc
     CUtensorMap m_x, m_w1, m_w3, m_w2, m_h;
