@@ -199,6 +199,45 @@ int bm_moe_forward_f32(const bm_bf16 *x, int T, int D, const bm_routing *routing
                        size_t workspace_bytes, bm_stream_t stream);
 int bm_round_bf16(const float *in, size_t n, bm_bf16 *out, bm_stream_t stream);
 
+/*
+ * SLO-aware latency control (PAPER.md 4.5): host logic that decides how aggressively the runtime applies
+ * united experts.  "When recent P90 latency exceeds the SLO, the threshold is multiplicatively reduced to lower
+ * latency.  When latency falls below a warning line, the threshold is linearly increased to improve accuracy."
+ * (P:259); threshold = 1.0 means no merging, threshold = 0 all cold-expert calls go to united experts.
+ * The paper prints no constants and Eq. 10-11 only state the objective, so every constant is a caller-set field
+ * (reading A21).  All pointers are HOST pointers; nothing here touches the GPU.
+ *
+ *   bm_salc_init     fills *c: threshold = 1 (zero brownout), empty latency window.  BM_ERR_SHAPE unless
+ *                    slo > 0, 0 < warn_frac <= 1, 0 < decrease < 1, increase > 0, 1 <= window <= BM_SALC_MAX_WINDOW.
+ *   bm_salc_observe  records one request latency (same unit as slo) in the sliding window of the last `window`
+ *                    observations and applies one control step on the window's P90 (nearest-rank: the
+ *                    ceil(0.9 n)-th smallest of the n latencies held):
+ *                        P90 > slo              -> threshold *= decrease
+ *                        P90 < warn_frac * slo  -> threshold  = min(1, threshold + increase)
+ *                        otherwise              -> unchanged
+ *                    Returns the new threshold (a negative bm_status as a double on a NULL / NaN argument).
+ *   bm_salc_cold_mask  turns a threshold into the cold_mask of bm_route_partial: the n_cold = round((1 - threshold) E)
+ *                    experts with the smallest routing frequency w[e] (bm_expert_histogram; ties -> lower index
+ *                    colder) are cold.  The paper defines "cold" only in its ref. [7]; this rule is reading A17's
+ *                    caller-supplied mask made concrete for the controller and is the one bench.py --config next uses.
+ */
+enum { BM_SALC_MAX_WINDOW = 256 };
+typedef struct {
+    double slo;          /* latency objective                                             */
+    double warn_frac;    /* warning line as a fraction of slo                             */
+    double decrease;     /* multiplicative factor applied above the SLO, in (0, 1)        */
+    double increase;     /* additive step applied below the warning line                  */
+    double threshold;    /* state: in [0, 1]                                              */
+    int32_t window;      /* observations the P90 is taken over                            */
+    int32_t count;       /* state: observations held (<= window)                          */
+    int32_t head;        /* state: next slot of the ring                                  */
+    double lat[BM_SALC_MAX_WINDOW];   /* state: ring of the last latencies                */
+} bm_salc;
+int bm_salc_init(bm_salc *c, double slo, double warn_frac, double decrease, double increase, int window);
+double bm_salc_observe(bm_salc *c, double latency);
+double bm_salc_p90(const bm_salc *c);    /* P90 of the window (0 when empty) */
+int bm_salc_cold_mask(const int32_t *w /*HOST [E]*/, int E, double threshold, int32_t *cold_mask /*HOST [E]*/);
+
 /* Same as bm_moe_forward with the execution path forced (BM_PATH_*); used by tests and the bench to
  * exercise every path on any shape.  BM_ERR_PATH if the path cannot run the shape. */
 int bm_moe_forward_path(const bm_bf16 *x, int T, int D, const bm_routing *routing, const bm_bf16 *W1,

@@ -22,8 +22,19 @@ BM_DECODE_MAX_T = 256
 EXPORTS = ["bm_workspace_bytes", "bm_route", "bm_route_partial", "bm_unite_weights", "bm_expert_histogram",
            "bm_expert_outputs", "bm_gram_workspace_bytes", "bm_cosine_gram", "bm_mse_workspace_bytes", "bm_group_mse",
            "bm_moe_forward", "bm_moe_forward_path", "bm_moe_forward_f32", "bm_round_bf16", "bm_moe_layer_host",
-           "bm_device_status", "bm_launch_count", "bm_status_string", "bm_profile_enable", "bm_profile_read"]
+           "bm_device_status", "bm_launch_count", "bm_status_string", "bm_profile_enable", "bm_profile_read",
+           "bm_salc_init", "bm_salc_observe", "bm_salc_p90", "bm_salc_cold_mask"]
 KERNELS = {"router": 1, "permute": 2, "prep": 3, "gemm1": 4, "gemm2": 5, "finalize": 6}
+
+
+BM_SALC_MAX_WINDOW = 256
+
+
+class BmSalc(ctypes.Structure):
+    """include/bm.h: bm_salc (host-side SLO-aware latency controller, PAPER.md 4.5)."""
+    _fields_ = [("slo", ctypes.c_double), ("warn_frac", ctypes.c_double), ("decrease", ctypes.c_double),
+                ("increase", ctypes.c_double), ("threshold", ctypes.c_double), ("window", c_int32),
+                ("count", c_int32), ("head", c_int32), ("lat", ctypes.c_double * BM_SALC_MAX_WINDOW)]
 
 
 class BmRouting(ctypes.Structure):
@@ -79,6 +90,14 @@ def lib() -> ctypes.CDLL:
         L.bm_moe_forward_f32.argtypes = L.bm_moe_forward.argtypes
         L.bm_round_bf16.restype = c_int
         L.bm_round_bf16.argtypes = [c_void_p, c_size_t, c_void_p, c_void_p]
+        L.bm_salc_init.restype = c_int
+        L.bm_salc_init.argtypes = [POINTER(BmSalc), ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double, c_int]
+        L.bm_salc_observe.restype = ctypes.c_double
+        L.bm_salc_observe.argtypes = [POINTER(BmSalc), ctypes.c_double]
+        L.bm_salc_p90.restype = ctypes.c_double
+        L.bm_salc_p90.argtypes = [POINTER(BmSalc)]
+        L.bm_salc_cold_mask.restype = c_int
+        L.bm_salc_cold_mask.argtypes = [c_void_p, c_int, ctypes.c_double, c_void_p]
         L.bm_moe_forward_path.restype = c_int
         L.bm_moe_forward_path.argtypes = L.bm_moe_forward.argtypes + [c_int]
         L.bm_moe_layer_host.restype = c_int
@@ -279,6 +298,36 @@ def bm_round_bf16(src, out=None, stream=None):
     if rc != BM_OK:
         raise BmError(rc, "bm_round_bf16")
     return out
+
+
+class Salc:
+    """SLO-aware latency controller (include/bm.h: bm_salc_*; host logic, no GPU)."""
+
+    def __init__(self, slo, warn_frac=0.8, decrease=0.7, increase=0.05, window=32):
+        self.c = BmSalc()
+        rc = lib().bm_salc_init(ctypes.byref(self.c), slo, warn_frac, decrease, increase, window)
+        if rc != BM_OK:
+            raise BmError(rc, "bm_salc_init")
+
+    def observe(self, latency) -> float:
+        return lib().bm_salc_observe(ctypes.byref(self.c), float(latency))
+
+    def p90(self) -> float:
+        return lib().bm_salc_p90(ctypes.byref(self.c))
+
+    @property
+    def threshold(self) -> float:
+        return self.c.threshold
+
+
+def bm_salc_cold_mask(w, threshold):
+    """cold_mask [E] int32 (host tensor) for bm_route_partial from routing frequencies w [E] (host int32)."""
+    w = w.to(dtype=torch.int32, device="cpu").contiguous()
+    mask = torch.zeros_like(w)
+    rc = lib().bm_salc_cold_mask(w.data_ptr(), w.numel(), float(threshold), mask.data_ptr())
+    if rc != BM_OK:
+        raise BmError(rc, "bm_salc_cold_mask")
+    return mask
 
 
 def bm_moe_layer_host(x_host, W_router, router_bias, K, group_map, G, W1, W3, W2, S, out_host, x_dev, out_dev,
