@@ -174,8 +174,7 @@ class DeviceLayer:
                 L.W1 = L.W3 = L.W2 = None      # free the host copies (1.4 - 2.8 GB)
         else:
             self.W1, self.W3, self.W2 = weights_from.W1, weights_from.W3, weights_from.W2
-        self.ws = bm.alloc_workspace(cfg.T, cfg.D, self.W1.shape[1], cfg.E, cfg.K, cfg.G, cfg.S)
-        self.partial = torch.empty((cfg.T, cfg.D), dtype=torch.float32, device="cuda") if tp is not None else None
+        self.ws = bm.alloc_workspace(cfg.T, cfg.D, cfg.F, cfg.E, cfg.K, cfg.G, cfg.S)
         self.routing = bm.Routing(cfg.T, cfg.K, cfg.G)
         self.out = torch.empty((cfg.T, cfg.D), dtype=torch.bfloat16, device="cuda")
         self.x_pinned = L.x.pin_memory()
@@ -439,8 +438,7 @@ class SweepPoint:
         L = make_layer(cfg, 0, weights=False)
         self.x = L.x.cuda()
         self.bias = None if L.router_bias is None else L.router_bias.cuda()
-        self.ws = bm.alloc_workspace(cfg.T, cfg.D, self.W1.shape[1], cfg.E, cfg.K, cfg.G, cfg.S)
-        self.partial = torch.empty((cfg.T, cfg.D), dtype=torch.float32, device="cuda") if tp is not None else None
+        self.ws = bm.alloc_workspace(cfg.T, cfg.D, cfg.F, cfg.E, cfg.K, cfg.G, cfg.S)
         self.routing = bm.Routing(cfg.T, cfg.K, cfg.G)
         self.out = torch.empty((cfg.T, cfg.D), dtype=torch.bfloat16, device="cuda")
         self.i = 0
@@ -528,7 +526,7 @@ def run_sweep(args):
                              tokens_per_s=cfg.T / t_best, t_hbm_us=t_hbm * 1e6, t_flop_us=t_flop * 1e6,
                              bound="hbm" if t_hbm >= t_flop else "tensor", roofline_frac=max(t_hbm, t_flop) / t_best,
                              achieved_gbs=nbytes / t_best / 1e9, achieved_tflops=flops / t_best / 1e12,
-                             path="decode" if (cfg.T <= 64 or (cfg.T <= bm.BM_DECODE_MAX_T and cfg.T * cfg.K <= 24 * cfg.G)) else "prefill",
+                             path="gemv" if cfg.T * cfg.K <= cfg.G else "decode" if (cfg.T <= 64 or (cfg.T <= bm.BM_DECODE_MAX_T and cfg.T * cfg.K <= 24 * cfg.G)) else "prefill",
                              device_status=status))
             sys.stderr.write(f"{cfg.name:24s} A={A:6d} G_act={G_act:3d} stream {t*1e6:9.1f} us"
                              + (f" graph {tg*1e6:9.1f} us" if tg else " " * 19)

@@ -509,6 +509,7 @@ cudaError_t launch_tp(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const f
     const int n_etiles = (E + 7) / 8;
     int WE = 1;
     while (WE < n_etiles && WE < kTpComputeWarps) WE *= 2;
+    if (tune_int("BM_ROUTER_WE", 0) > 0) WE = tune_int("BM_ROUTER_WE", 0);
     const int WT = kTpComputeWarps / WE;
     const int TB = WT * kTpTok, EB = WE * 8;
     const size_t smem = (size_t)kTpStages * (TB + EB) * (kSlab * 2) + (2 * kTpStages + 4) * sizeof(uint64_t) +
