@@ -243,7 +243,7 @@ static int forward_common(const bm_bf16 *x, int T, int D, const bm_routing *rout
         // BM_DECODE_MAX_T tokens while a group expects at most ~24 rows (measured crossover at T = 256:
         // 17 rows/group -> decode 6% faster, 33 rows/group -> prefill tiles 5% faster)
         const int max_t = tune_int("BM_DECODE_MAX_T", BM_DECODE_MAX_T);
-        const bool few_rows = (long long)T * K <= 24LL * G;
+        const bool few_rows = (long long)T * K <= (long long)tune_int("BM_DECODE_ROWS", 24) * G;
         path = (T <= 64 || (T <= max_t && few_rows)) ? BM_PATH_DECODE : BM_PATH_PREFILL;
         // matrix-vector streaming when a weight set expects at most ~1 row (single-token decode above all):
         // the tcgen05 k-block loop has a latency floor that such a step never fills (see bm_gemv.cu)

@@ -723,18 +723,32 @@ dense_sched_kernel(int32_t *__restrict__ sched, int E, int T) {
 
 // Prefill combine (F2): out[t] = sum_{s < n_slots[t]} gate_w[t,s] * y[slot_row[t,s]]  (slot order)
 //                               + sum_{j < S} y[TK + j*T + t]                          (shared experts)
-// fp32 accumulation in a fixed order -> deterministic.  One warp per token: lane s holds row and weight of
-// source s (K + S <= 32), the warp walks the D columns 16 bytes per lane (512 contiguous bytes per row and
-// step), four source rows in flight.
+// fp32 accumulation in a fixed order -> deterministic.  A warp item = (token, column slice); lane s parks the
+// row pointer and weight of source s (K + S <= 32) in shared memory once per item, then the warp walks its
+// columns 16 bytes per lane (512 contiguous bytes per row and step), four source rows in flight; the eight
+// products of a 16-byte chunk are four FFMA2 (the weight is the broadcast operand).  (The first version re-read
+// row and weight with three shuffles per source and chunk: 67 instructions per 512-byte row load, issue-bound
+// at 4 TB/s.)
 constexpr int kCombineBatch = 4;     // source rows in flight per lane (8 measured slower: 79 -> 117 us at BJ:configs[2])
+
+__device__ __forceinline__ void fma2_bcast(float &d0, float &d1, float x, float w0, float w1) {
+    uint64_t a, b, c;
+    asm("mov.b64 %0, {%1, %1};" : "=l"(a) : "f"(x));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(b) : "f"(w0), "f"(w1));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(c) : "f"(d0), "f"(d1));
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c) : "l"(a), "l"(b));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(d0), "=f"(d1) : "l"(c));
+}
 
 __global__ void __launch_bounds__(256)
 combine_kernel(const bm_bf16 *__restrict__ y, int T, int D, int K, int S, const int32_t *__restrict__ n_slots,
                const int32_t *__restrict__ slot_row, const float *__restrict__ gate_w, bm_bf16 *__restrict__ out,
                float *__restrict__ out_f32, int split) {
+    __shared__ const uint4 *s_src[8][32];     // per warp: row pointers of the item's sources (nullptr: skip)
+    __shared__ float s_gw[8][32];
     grid_dep_wait();
     grid_dep_launch();
-    const int lane = threadIdx.x & 31;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int vec = D / 8;
     const size_t TK = (size_t)T * K;
     const int warps = (gridDim.x * blockDim.x) >> 5;
@@ -744,16 +758,20 @@ combine_kernel(const bm_bf16 *__restrict__ y, int T, int D, int K, int S, const 
         const int t = (int)(item / split), sl = (int)(item - (long long)t * split);
         const int n = min(max(n_slots[t], 0), K);
         const int n_src = n + S;
-        long long my_row = -1;                                   // -1: skip (invalid slot_row)
+        const uint4 *my_src = nullptr;                           // nullptr: skip (invalid slot_row)
         float my_gw = 1.0f;
         if (lane < n) {
             const int r = slot_row[(size_t)t * K + lane];
-            if (r >= 0 && (size_t)r < TK) my_row = r;
+            if (r >= 0 && (size_t)r < TK) my_src = reinterpret_cast<const uint4 *>(y + (size_t)r * D);
             my_gw = gate_w[(size_t)t * K + lane];
         } else if (lane < n_src) {
-            my_row = (long long)TK + (long long)(lane - n) * T + t;
+            my_src = reinterpret_cast<const uint4 *>(y + (TK + (size_t)(lane - n) * T + t) * D);
         }
-        for (int c0 = sl * 32; c0 < vec; c0 += 32 * split) {      // warp-uniform trip count: the shuffles below need every lane
+        __syncwarp();                                            // the previous item's readers are done
+        s_src[w][lane] = my_src;
+        s_gw[w][lane] = my_src ? my_gw : 0.0f;
+        __syncwarp();
+        for (int c0 = sl * 32; c0 < vec; c0 += 32 * split) {
             const int c = c0 + lane;
             const bool col_ok = c < vec;
             float acc[8];
@@ -765,19 +783,18 @@ combine_kernel(const bm_bf16 *__restrict__ y, int T, int D, int K, int S, const 
 #pragma unroll
                 for (int q = 0; q < kCombineBatch; ++q) {
                     const int src = min(s0 + q, 31);
-                    const long long row = __shfl_sync(kFullMask, my_row, src);
-                    gw[q] = __shfl_sync(kFullMask, my_gw, src);
-                    const bool ok = s0 + q < n_src && row >= 0 && col_ok;
-                    if (!ok) gw[q] = 0.0f;
-                    v[q] = ok ? *reinterpret_cast<const uint4 *>(y + (size_t)row * D + (size_t)c * 8) : make_uint4(0, 0, 0, 0);
+                    const uint4 *ptr = s_src[w][src];            // broadcast reads
+                    gw[q] = s_gw[w][src];
+                    const bool ok = s0 + q < n_src && ptr != nullptr && col_ok;
+                    v[q] = ok ? ptr[c] : make_uint4(0, 0, 0, 0);
                 }
 #pragma unroll
                 for (int q = 0; q < kCombineBatch; ++q) {
-                    if (s0 + q < n_src) {                        // warp-uniform; skipped sources add nothing
-                        acc[0] = fmaf(gw[q], bf16_lo(v[q].x), acc[0]); acc[1] = fmaf(gw[q], bf16_hi(v[q].x), acc[1]);
-                        acc[2] = fmaf(gw[q], bf16_lo(v[q].y), acc[2]); acc[3] = fmaf(gw[q], bf16_hi(v[q].y), acc[3]);
-                        acc[4] = fmaf(gw[q], bf16_lo(v[q].z), acc[4]); acc[5] = fmaf(gw[q], bf16_hi(v[q].z), acc[5]);
-                        acc[6] = fmaf(gw[q], bf16_lo(v[q].w), acc[6]); acc[7] = fmaf(gw[q], bf16_hi(v[q].w), acc[7]);
+                    if (s0 + q < n_src) {                        // warp-uniform; skipped sources add nothing (weight 0, value 0)
+                        fma2_bcast(acc[0], acc[1], gw[q], bf16_lo(v[q].x), bf16_hi(v[q].x));
+                        fma2_bcast(acc[2], acc[3], gw[q], bf16_lo(v[q].y), bf16_hi(v[q].y));
+                        fma2_bcast(acc[4], acc[5], gw[q], bf16_lo(v[q].z), bf16_hi(v[q].z));
+                        fma2_bcast(acc[6], acc[7], gw[q], bf16_lo(v[q].w), bf16_hi(v[q].w));
                     }
                 }
             }

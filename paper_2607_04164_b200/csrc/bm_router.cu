@@ -246,10 +246,7 @@ router_split_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *
         if (lane == 0) __threadfence();
     }
     __syncthreads();
-    if (threadIdx.x == 0) {
-        __threadfence();
-        s_flag = atomicAdd(status + kStatusTokCnt + t, 1) == ES - 1;
-    }
+    if (threadIdx.x == 0) s_flag = atomicAdd(status + kStatusTokCnt + t, 1) == ES - 1;   // (the writers fenced above)
     __syncthreads();
     if (!s_flag) return;
 
@@ -265,8 +262,7 @@ router_split_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *
     }
     if (!fuse_permute) return;
     __syncthreads();
-    if (threadIdx.x == 0) {
-        __threadfence();
+    if (threadIdx.x == 0) {                // (warp 0 fenced its routing rows above)
         s_flag = atomicAdd(status + kStatusDone, 1) == T - 1;
         if (s_flag) status[kStatusDone] = 0;
     }
