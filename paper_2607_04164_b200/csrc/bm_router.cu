@@ -335,10 +335,11 @@ __device__ __forceinline__ float bf16_lo_alu(uint32_t u) { return __uint_as_floa
 
 // Wait of a helper role (producer lane, select warps): backs off between polls so that it does not take
 // issue slots from the compute warps; bounded like ptx::mbar_wait (a protocol bug traps instead of hanging).
+template <unsigned NS>
 __device__ __forceinline__ void mbar_wait_sleep(uint64_t *bar, uint32_t parity) {
     uint32_t spins = 0;
     while (!ptx::mbar_try_wait(bar, parity)) {
-        __nanosleep(64);
+        __nanosleep(NS);
         if (++spins > (1u << 24)) __trap();
     }
 }
@@ -388,7 +389,7 @@ router_tp_kernel(const __grid_constant__ CUtensorMap tm_x,      // x [T, D], box
             for (int blk = blockIdx.x; blk < n_blocks; blk += gridDim.x)
                 for (int pass = 0; pass < n_pass; ++pass)
                     for (int slab = 0; slab < n_slabs; ++slab) {
-                        mbar_wait_sleep(&empty[stage], phase ^ 1);    // slab held before released by every compute warp
+                        mbar_wait_sleep<64>(&empty[stage], phase ^ 1);    // slab held before released by every compute warp
                         uint8_t *st = tp_smem + (size_t)stage * stage_bytes;
                         ptx::mbar_arrive_expect_tx(&full[stage], stage_bytes);
                         ptx::tma_load_2d(st, &tm_x, &full[stage], slab * kSlab, blk * TB, ptx::kEvictNormal);
@@ -405,7 +406,7 @@ router_tp_kernel(const __grid_constant__ CUtensorMap tm_x,      // x [T, D], box
         int it = 0;
         for (int blk = blockIdx.x; blk < n_blocks; blk += gridDim.x, ++it) {
             const int buf = it & 1;
-            mbar_wait_sleep(&lfull[buf], (it >> 1) & 1);
+            mbar_wait_sleep<400>(&lfull[buf], (it >> 1) & 1);     // a block takes microseconds: poll rarely
             const float *lg = s_logits + (size_t)buf * TB * E;
             // the CTA's last block: the compute warps have nothing left to multiply and take a share (below)
             const int stride = blk + (int)gridDim.x >= n_blocks ? kTpSelectWarps + kTpComputeWarps : kTpSelectWarps;
