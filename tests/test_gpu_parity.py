@@ -268,3 +268,42 @@ def test_prefill_cta_pairs_forced_on_ragged_shapes(T, D, F, E, K, G, S, monkeypa
     _, out1, _ = gpu_layer(L, PATHS["prefill"])
     # same tiles, same k order, same epilogue: the pair and the single-CTA kernels agree bit for bit
     assert (out == out1).all()
+
+
+# ---------------------------------------------------------------------------------------------------
+# seeded random shapes through every path and kernel variant (the environment switches are read per call)
+# ---------------------------------------------------------------------------------------------------
+VARIANTS = [
+    (0, {}),                                                   # BM_PATH_AUTO
+    (PATHS["gemv"], {}),
+    (PATHS["decode"], {}),
+    (PATHS["prefill"], {"BM_PF_GATHER": "1", "BM_PF_PAIR": "0"}),   # GEMM1 gathers its rows itself
+    (PATHS["prefill"], {"BM_PF_GATHER": "2", "BM_PF_PAIR": "1"}),   # the same with CTA pairs
+    (PATHS["prefill"], {"BM_PF_GATHER": "0", "BM_PF_PAIR": "1"}),   # TMA-fed CTA pairs
+    (0, {"BM_ROUTER_TP_MIN_T": "1"}),                           # throughput router on any T
+    (0, {"BM_ROUTER_SPLIT_MAX_T": "511"}),                      # split router (+ fused permutation) on any T < 512
+]
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_random_shapes_all_variants(seed, monkeypatch):
+    rng = np.random.default_rng(1000 + seed)
+    T = int(rng.integers(1, 1400 if seed % 2 else 40))
+    D = int(rng.choice([64, 72, 128, 264, 512, 1024]))
+    F = int(rng.choice([64, 72, 264, 384, 1000]))
+    E = int(rng.integers(2, 70))
+    K = int(rng.integers(1, min(E, 8) + 1))
+    G = int(rng.integers(1, E + 1))
+    S = int(rng.integers(0, 3))
+    L = rand_layer(rng, T=T, D=D, F=F, E=E, K=K, G=G, S=S, bias=bool(rng.integers(0, 2)), wstd=0.02 if D >= 512 else 0.05)
+    o = oracle_route(L)
+    want = oracle_forward(L, o)
+    for path, env in VARIANTS:
+        for k, v in env.items():
+            monkeypatch.setenv(k, v)
+        g, out, status = gpu_layer(L, path)
+        for k in env:
+            monkeypatch.delenv(k)
+        assert status == 0, (path, env)
+        assert_routing_equal(g, o)
+        assert_out_close(out, want)
