@@ -30,7 +30,7 @@ constexpr int kItemsPerWarp = kPermItemsPerWarp;
 // ---- T*K <= 2048: everything in one CTA --------------------------------------------------------
 // (One CTA of 32 warps for up to 32768 items was measured too: 31-46 us against 20-24 us for the three-kernel
 // path -- the serial rounds of one CTA expose every global-load latency.)
-__global__ void __launch_bounds__(kWarps * 32)
+__global__ void __launch_bounds__(1024)
 permute_small_kernel(const int32_t *__restrict__ group_ids, int T, int K, int G, int per_warp,
                      int32_t *__restrict__ counts, int32_t *__restrict__ offsets,
                      int32_t *__restrict__ row_token, int32_t *__restrict__ row_slot,
@@ -135,9 +135,21 @@ cudaError_t launch_permute(int T, int K, int G, const bm_routing &r, int32_t *bl
     const int nb = (int)((items + kPermItemsPerBlock - 1) / kPermItemsPerBlock);
     const size_t smem_w = (size_t)kWarps * G * sizeof(int);
     if (items <= kPermSmallItems) {
-        const size_t smem = smem_w + (size_t)(G + 512) * sizeof(int);
-        return launch_kernel(permute_small_kernel, dim3(1), dim3(kWarps * 32), smem, stream, (const int32_t *)r.group_ids,
-                             T, K, G, kPermSmallItems / kWarps, r.counts, r.offsets, r.row_token, r.row_slot, r.slot_row, status);
+        // few items: 8 warps; otherwise 16 warps with a few rounds of 32 items each, so the serial chain of
+        // rounds (load -> match -> shared-memory update, twice) stays short
+        int nw = tune_int("BM_PERM_SMALL_WARPS", 0);
+        if (nw <= 0) nw = items <= 256 ? 8 : 16;      // measured at 1024 items: 8 warps 10.2, 16 warps 8.7, 32 warps 9.9 us
+        int per_warp = (int)((items + nw - 1) / nw);
+        per_warp = (per_warp + 31) / 32 * 32;
+        const size_t smem = (size_t)nw * G * sizeof(int) + (size_t)(G + 512) * sizeof(int);
+        static size_t smem_set = 0;
+        if (smem > 48 * 1024 && smem > smem_set) {
+            cudaError_t e = cudaFuncSetAttribute(permute_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+            smem_set = smem;
+        }
+        return launch_kernel(permute_small_kernel, dim3(1), dim3(nw * 32), smem, stream, (const int32_t *)r.group_ids,
+                             T, K, G, per_warp, r.counts, r.offsets, r.row_token, r.row_slot, r.slot_row, status);
     }
     cudaError_t e = launch_kernel(permute_hist_kernel, dim3(nb), dim3(kWarps * 32), smem_w, stream,
                                   (const int32_t *)r.group_ids, T, K, G, block_hist);

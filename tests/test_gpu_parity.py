@@ -234,7 +234,8 @@ def test_finegrained_config_full_size_sampled():
     _sampled_parity(CONFIGS["finegrained"], 24)                 # BJ:configs[3], shared experts, uneven groups
 
 
-@pytest.mark.parametrize("name", ["sweep_G8_T1_s1", "sweep_G15_T16_s2", "sweep_G60_T256_s0", "sweep_G30_T256_s1",
+@pytest.mark.parametrize("name", ["sweep_G8_T1_s1", "sweep_G60_T1_s1", "sweep_G15_T16_s2", "sweep_G60_T256_s0",
+                                  "sweep_G30_T256_s1", "sweep_G60_T4096_s1",       # single-CTA tiles, in-kernel gather
                                   "sweep_G30_T4096_s1", "sweep_G8_T16384_s2"])
 def test_sweep_points_sampled(name):
     from bm_inputs import get_config
