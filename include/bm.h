@@ -170,15 +170,16 @@ int bm_group_mse(const bm_bf16 *Y, const bm_bf16 *U, int T, int D, const int32_t
 /*
  * bm_moe_forward -- steps 9-13: out[t] = sum_s gate_w[t,s] * FFN_{group_ids[t,s]}(x_t) + sum_{j<S} FFN_{G+j}(x_t)
  * with FFN_u(x) = W2[u] . ( SiLU(W1[u] x) * (W3[u] x) )   (P:42 with united experts P:46; SwiGLU: A3).
- * bf16 operands, fp32 accumulation (tensor cores), the intermediate h is rounded to bf16 (A12); on the prefill
- * path the per-row expert outputs are rounded to bf16 before the fp32 gate-weighted sum, which is taken in slot
- * order (deterministic); the decode path adds fp32 partial sums with reductions whose order may vary.
+ * bf16 operands, fp32 accumulation (tensor cores; CUDA-core FFMA2 on the matrix-vector path), the intermediate h
+ * is rounded to bf16 (A12); on the prefill and matrix-vector paths the per-row expert outputs are rounded to bf16
+ * before the fp32 gate-weighted sum, which is taken in slot order (deterministic); the decode path adds fp32
+ * partial sums with reductions whose order may vary.
  *   x        [T,D]      bf16
  *   routing  as produced by bm_route (or any arrays satisfying the same invariants), same T
  *   W1, W3   [G+S,F,D]  bf16 (united experts 0..G-1, then the S always-on shared experts, A11)
  *   W2       [G+S,D,F]  bf16
  *   out      [T,D]      bf16, overwritten
- * The path (decode / prefill, see BM_PATH_AUTO) is picked from the host values T, K and G.
+ * The path (matrix-vector / decode / prefill, see BM_PATH_AUTO) is picked from the host values T, K, G and S.
  */
 int bm_moe_forward(const bm_bf16 *x, int T, int D, const bm_routing *routing, const bm_bf16 *W1,
                    const bm_bf16 *W3, const bm_bf16 *W2, int F, int S, bm_bf16 *out, void *workspace,

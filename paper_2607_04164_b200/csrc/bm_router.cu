@@ -182,8 +182,8 @@ router_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *__rest
 }
 
 // -------------------------------------------------------------------------------------------------
-// Latency shape with the experts of a token spread over CTAs (T <= 16, E > 8).  CTA (es, t) computes the
-// logits of 8 * ET experts of token t -- a warp owns ET dot products in the canonical order -- and parks them
+// Latency shape with the experts of a token spread over 32 warps and, for E > 64, over CTAs (T <= 16, E > 8).
+// CTA (es, t) computes the logits of 32 * ET experts of token t -- a warp owns ET dot products in the canonical order -- and parks them
 // in a global scratch row.  The CTA that completes a token (arrival counter) runs R2-R5 for it; the CTA that
 // completes the batch runs the whole permutation R6-R8 when it fits one CTA (T*K <= 2048), which saves the
 // launch of the permutation kernel.  Counters live in the zero-once head of the workspace and are put back
@@ -191,8 +191,10 @@ router_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *__rest
 // pattern); the consumers read the other CTAs' results with ld.global.cg.
 // One token on one CTA (router_kernel) streams all of W_router through a single SM: 7 us at E = 60, D = 2048.
 // -------------------------------------------------------------------------------------------------
+constexpr int kSplitWarps = 32;        // a CTA of 32 warps x ET experts: E <= 64 needs one CTA per token and no arrival counter
+
 template <int ET>
-__global__ void __launch_bounds__(kWarps * 32)
+__global__ void __launch_bounds__(kSplitWarps * 32)
 router_split_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *__restrict__ Wr,
                     const float *__restrict__ bias, int E, int K, GroupMap gm, int ES, float *__restrict__ logits_ws,
                     int fuse_permute, int per_warp, bm_routing r, int32_t *__restrict__ status) {
@@ -202,7 +204,7 @@ router_split_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *
     grid_dep_launch();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int t = blockIdx.y;
-    const int e0 = (blockIdx.x * kWarps + warp) * ET;
+    const int e0 = (blockIdx.x * kSplitWarps + warp) * ET;
 
     // ---- R1: ET logits per warp ---------------------------------------------------------------
     if (e0 < E) {
@@ -240,34 +242,41 @@ router_split_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *
             for (int o = 16; o >= 1; o >>= 1) p = __fadd_rn(p, __shfl_xor_sync(kFullMask, p, o));
             if (lane == 0 && e0 + j < E) {
                 if (bias) p = __fadd_rn(p, bias[e0 + j]);
-                __stcg(logits_ws + (size_t)t * E + e0 + j, p);
+                if (ES > 1) __stcg(logits_ws + (size_t)t * E + e0 + j, p);
+                else reinterpret_cast<float *>(rs_dyn)[e0 + j] = p;      // one CTA per token: the logits stay on chip
             }
         }
-        if (lane == 0) __threadfence();
+        if (lane == 0 && ES > 1) __threadfence();
     }
     __syncthreads();
-    if (threadIdx.x == 0) s_flag = atomicAdd(status + kStatusTokCnt + t, 1) == ES - 1;   // (the writers fenced above)
-    __syncthreads();
-    if (!s_flag) return;
+    if (ES > 1) {                          // several CTAs share the token: the last one to arrive goes on
+        if (threadIdx.x == 0) s_flag = atomicAdd(status + kStatusTokCnt + t, 1) == ES - 1;   // (the writers fenced above)
+        __syncthreads();
+        if (!s_flag) return;
+    }
 
     // ---- R2-R5: this CTA completed token t -------------------------------------------------------
     if (warp == 0) {
-        __threadfence();
         float *s_l = reinterpret_cast<float *>(rs_dyn);
-        for (int e = lane; e < E; e += 32) s_l[e] = __ldcg(logits_ws + (size_t)t * E + e);
-        __syncwarp();
+        if (ES > 1) {
+            __threadfence();
+            for (int e = lane; e < E; e += 32) s_l[e] = __ldcg(logits_ws + (size_t)t * E + e);
+            __syncwarp();
+        }
         select_and_write(s_l, t, lane, E, K, gm, r.expert_ids, r.group_ids, r.gate_w, r.n_slots, status);
-        if (lane == 0) status[kStatusTokCnt + t] = 0;
+        if (lane == 0 && ES > 1) status[kStatusTokCnt + t] = 0;
         __threadfence();
     }
     if (!fuse_permute) return;
     __syncthreads();
-    if (threadIdx.x == 0) {                // (warp 0 fenced its routing rows above)
-        s_flag = atomicAdd(status + kStatusDone, 1) == T - 1;
-        if (s_flag) status[kStatusDone] = 0;
+    if (T > 1) {                           // the CTA that completes the batch goes on
+        if (threadIdx.x == 0) {            // (warp 0 fenced its routing rows above)
+            s_flag = atomicAdd(status + kStatusDone, 1) == T - 1;
+            if (s_flag) status[kStatusDone] = 0;
+        }
+        __syncthreads();
+        if (!s_flag) return;
     }
-    __syncthreads();
-    if (!s_flag) return;
 
     // ---- R6-R8: this CTA completed the batch ---------------------------------------------------------
     __threadfence();
@@ -556,13 +565,21 @@ cudaError_t launch_router(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, con
     if (E > 8 && T <= tune_int("BM_ROUTER_SPLIT_MAX_T", 16)) {
         // latency shape, experts spread over CTAs; the last CTA also permutes when one CTA can
         constexpr int ET = 2;
-        const int ES = (E + kWarps * ET - 1) / (kWarps * ET);
+        const int ES = (E + kSplitWarps * ET - 1) / (kSplitWarps * ET);
         const bool fuse = (long long)T * K <= kPermSmallItems;
         size_t smem = (size_t)E * sizeof(float);
-        if (fuse) smem = std::max(smem, (size_t)(kWarps * r.G + r.G + 512) * sizeof(int));
+        if (fuse) smem = std::max(smem, (size_t)(kSplitWarps * r.G + r.G + 512) * sizeof(int));
+        static size_t smem_set = 0;
+        if (smem > 48 * 1024 && smem > smem_set) {
+            cudaError_t e = cudaFuncSetAttribute(router_split_kernel<ET>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+            smem_set = smem;
+        }
+        int per_warp = (int)(((long long)T * K + kSplitWarps - 1) / kSplitWarps);
+        per_warp = (per_warp + 31) / 32 * 32;
         *fused_permute = fuse;
-        return launch_kernel(router_split_kernel<ET>, dim3(ES, T), dim3(kWarps * 32), smem, stream, x, T, D, Wr, bias, E, K,
-                             gm, ES, route_logits, fuse ? 1 : 0, kPermSmallItems / kWarps, r, status);
+        return launch_kernel(router_split_kernel<ET>, dim3(ES, T), dim3(kSplitWarps * 32), smem, stream, x, T, D, Wr, bias, E, K,
+                             gm, ES, route_logits, fuse ? 1 : 0, per_warp, r, status);
     }
     // latency shape: one token per warp pass, warps split the experts
     if (E <= 8) {
