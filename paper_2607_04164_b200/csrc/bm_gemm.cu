@@ -894,13 +894,18 @@ void choose_decode_tiling(int wrows, int kblocks, int n_seg, bool allow_split, i
     const int max_ks = allow_split ? 16 : 1;
     int rmax = tune_int("BM_DC_RMAX", 128);
     rmax = rmax < 32 ? 32 : (rmax > 128 ? 128 : rmax);
+    const int ks_force = allow_split ? tune_int("BM_DC_KS_FORCE", 0) : 0;
     for (int ks = 1; ks <= max_ks; ++ks) {
         if (ks > 1 && (kblocks % ks != 0 || kblocks / ks < 4)) continue;
+        if (ks_force > 0 && ks != ks_force && kblocks % ks_force == 0 && kblocks / ks_force >= 4) continue;
         for (int R = rmax; R >= 32; --R) {
             const double t = decode_time_model(wrows, kblocks, n_seg, R, ks, mats, sms);
             if (t < best * 0.99) { best = t; bestR = R; bestKs = ks; }   // within 1%: keep the larger tile
         }
     }
+    // Long K (Mixtral's F = 14336: 224 k-blocks): the model is blind to the ramp and tail of few long items --
+    // measured at BJ:configs[1], GEMM2 83.3 us with one split, 80.1 us with four (81.3 with two, 80.7 with eight).
+    if (allow_split && ks_force <= 0 && bestKs == 1 && kblocks >= 128 && kblocks % 4 == 0) bestKs = 4;
     *R_out = bestR;
     *ks_out = bestKs;
 }
