@@ -56,6 +56,16 @@ def test_partial_brownout_small(path, frac_cold):
         assert (o.counts[cfg.G:] == 0).all()
 
 
+@pytest.mark.parametrize("T", [1, 3, 16])
+def test_partial_brownout_single_token_decode(T):
+    # small batches: split router with the cold mask (+ fused permutation over G + E sets), matrix-vector forward
+    cfg = LayerConfig("pbd", T=T, D=2048, F=1408, E=60, K=4, G=15, zipf_s=1.0)
+    rng = np.random.default_rng(7 + T)
+    cold = (rng.random(cfg.E) < 0.5).astype(np.int32)
+    _run_partial(cfg, 2, cold)                                  # BM_PATH_AUTO
+    _run_partial(cfg, 2, cold, 4)                               # BM_PATH_GEMV forced
+
+
 def test_partial_brownout_qwen_shape_prefill():
     # BJ:configs[4] shape (E=60, top-4) with the 20 least-loaded experts ... here: a seeded half of the experts cold
     cfg = LayerConfig("pbq", T=1500, D=2048, F=1408, E=60, K=4, G=15, zipf_s=1.0)
