@@ -308,3 +308,34 @@ def test_random_shapes_all_variants(seed, monkeypatch):
         assert status == 0, (path, env)
         assert_routing_equal(g, o)
         assert_out_close(out, want)
+
+
+# ---------------------------------------------------------------------------------------------------
+# bm_moe_layer_host: the end-to-end call (pinned host x -> host out); the data changes between calls, the
+# buffers do not
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("own_stream", [False, True])
+def test_layer_host_repeated_calls_with_new_data(own_stream):
+    import paper_2607_04164_b200 as bm
+    rng = np.random.default_rng(77)
+    T, D, F, E, K, G, S = 48, 256, 320, 12, 3, 4, 1
+    L = rand_layer(rng, T=T, D=D, F=F, E=E, K=K, G=G, S=S, bias=True)
+    d = to_device(L)
+    ws = bm.alloc_workspace(T, D, F, E, K, G, S)
+    r = bm.Routing(T, K, G)
+    x_pin = torch.empty((T, D), dtype=torch.bfloat16).pin_memory()
+    out_pin = torch.empty((T, D), dtype=torch.bfloat16).pin_memory()
+    x_dev = torch.empty((T, D), dtype=torch.bfloat16, device="cuda")
+    out_dev = torch.empty((T, D), dtype=torch.bfloat16, device="cuda")
+    stream = torch.cuda.Stream() if own_stream else None
+    torch.cuda.synchronize()
+    for it in range(4):
+        L.x = L.x.roll(it + 1, 0).flip(1).contiguous()              # new data in the same buffers
+        x_pin.copy_(L.x)
+        out_pin.fill_(float("nan"))
+        bm.bm_moe_layer_host(x_pin, d.W_router, d.router_bias, K, d.group_map, G, d.W1, d.W3, d.W2, S, out_pin,
+                             x_dev, out_dev, r, ws, stream=stream)
+        o = oracle_route(L)
+        assert_routing_equal(routing_to_numpy(r, T), o)
+        assert_out_close(out_pin.float().numpy().astype(np.float64), oracle_forward(L, o))
+    assert bm.bm_device_status(ws) == 0
