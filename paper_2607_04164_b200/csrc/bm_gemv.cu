@@ -52,8 +52,8 @@ __device__ __forceinline__ void fma2(float &d0, float &d1, float x, float w0, fl
 // the next step may belong to the next unit) are issued before the multiply of step s, from two register
 // buffers, so a warp always has a step of loads in flight -- without it every step paid a full HBM latency
 // (measured: 3 TB/s instead of 6 at T = 16, G = 60).
-template <int R, bool SWIGLU>
-__device__ __forceinline__ void warp_units(const bm_bf16 *__restrict__ base_a, const bm_bf16 *__restrict__ base_b,
+template <int R, bool SWIGLU, typename StageFn>
+__device__ __forceinline__ void warp_units(StageFn stage_rows, const bm_bf16 *__restrict__ base_a, const bm_bf16 *__restrict__ base_b,
                                            size_t stride_q, int n8, int q0, int qb, const uint8_t *s_in, int in_bytes,
                                            int lane, int nr, bm_bf16 *__restrict__ outp, size_t orow0, int OUT) {
     constexpr int U = R <= 4 ? 4 : 2;           // chunks of each row per lane and step (fewer with 8 rows: registers)
@@ -117,6 +117,9 @@ __device__ __forceinline__ void warp_units(const bm_bf16 *__restrict__ base_a, c
     uint4 a0[U], b0[U], a1[U], b1[U];
     int q = q0, it = 0;
     load(q < qb, q, 0, a0, b0);
+    // the input rows are staged (by all threads of the CTA) while this first step of weight loads is in flight: the
+    // weights do not depend on them, and the staging is two dependent global round trips (row_token -> x row)
+    stage_rows();
     while (q < qb) {
         int qn = q, itn = it + 1;
         if (itn == iters) { itn = 0; qn += kGvWarps; }
@@ -195,21 +198,23 @@ gemv_kernel(GemvArgs p, int rows_cap) {
         }
         for (int base = 0; base < cnt; base += rows_cap) {
             const int nr = cnt - base < rows_cap ? cnt - base : rows_cap;
-            __syncthreads();                                   // the readers of the rows staged before are done
-            for (int idx = tid; idx < nr * n8; idx += kGvThreads) {
-                const int r = idx / n8, c = idx - r * n8;
-                long long src;
-                if (SWIGLU) {
-                    int tok = u < p.G ? p.row_token[row0 + base + r] : base + r;
-                    tok = tok < 0 ? 0 : (tok >= p.T ? p.T - 1 : tok);
-                    src = tok;
-                } else {
-                    src = row0 + base + r;
+            auto stage_rows = [&]() {
+                __syncthreads();                               // the readers of the rows staged before are done
+                for (int idx = tid; idx < nr * n8; idx += kGvThreads) {
+                    const int r = idx / n8, c = idx - r * n8;
+                    long long src;
+                    if (SWIGLU) {
+                        int tok = u < p.G ? p.row_token[row0 + base + r] : base + r;
+                        tok = tok < 0 ? 0 : (tok >= p.T ? p.T - 1 : tok);
+                        src = tok;
+                    } else {
+                        src = row0 + base + r;
+                    }
+                    *reinterpret_cast<uint4 *>(s_in + (size_t)r * in_bytes + (size_t)c * 16) =
+                        __ldg(reinterpret_cast<const uint4 *>(p.in + (size_t)src * p.IN) + c);
                 }
-                *reinterpret_cast<uint4 *>(s_in + (size_t)r * in_bytes + (size_t)c * 16) =
-                    __ldg(reinterpret_cast<const uint4 *>(p.in + (size_t)src * p.IN) + c);
-            }
-            __syncthreads();
+                __syncthreads();
+            };
             const bm_bf16 *base_a, *base_b;
             size_t stride_q;
             if (SWIGLU) {
@@ -223,10 +228,10 @@ gemv_kernel(GemvArgs p, int rows_cap) {
             }
             const size_t orow0 = (size_t)(row0 + base);
             // rows past nr (up to the next power of two) are stale shared memory: computed, never stored
-            if (nr == 1) warp_units<1, SWIGLU>(base_a, base_b, stride_q, n8, qa + warp, qb, s_in, in_bytes, lane, nr, p.outp, orow0, p.OUT);
-            else if (nr == 2) warp_units<2, SWIGLU>(base_a, base_b, stride_q, n8, qa + warp, qb, s_in, in_bytes, lane, nr, p.outp, orow0, p.OUT);
-            else if (nr <= 4) warp_units<4, SWIGLU>(base_a, base_b, stride_q, n8, qa + warp, qb, s_in, in_bytes, lane, nr, p.outp, orow0, p.OUT);
-            else warp_units<8, SWIGLU>(base_a, base_b, stride_q, n8, qa + warp, qb, s_in, in_bytes, lane, nr, p.outp, orow0, p.OUT);
+            if (nr == 1) warp_units<1, SWIGLU>(stage_rows, base_a, base_b, stride_q, n8, qa + warp, qb, s_in, in_bytes, lane, nr, p.outp, orow0, p.OUT);
+            else if (nr == 2) warp_units<2, SWIGLU>(stage_rows, base_a, base_b, stride_q, n8, qa + warp, qb, s_in, in_bytes, lane, nr, p.outp, orow0, p.OUT);
+            else if (nr <= 4) warp_units<4, SWIGLU>(stage_rows, base_a, base_b, stride_q, n8, qa + warp, qb, s_in, in_bytes, lane, nr, p.outp, orow0, p.OUT);
+            else warp_units<8, SWIGLU>(stage_rows, base_a, base_b, stride_q, n8, qa + warp, qb, s_in, in_bytes, lane, nr, p.outp, orow0, p.OUT);
         }
         pos += qb - qa;
     }
