@@ -280,6 +280,45 @@ router_split_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *
 
     // ---- R6-R8: this CTA completed the batch ---------------------------------------------------------
     __threadfence();
+    const int items = T * K;
+    if (items <= 32) {
+        // at most 32 (token, slot) items: no histograms or scans -- every thread counts the keys below / equal to
+        // its group from the 32 keys in shared memory; item i's row = #(keys < key_i) + #(j < i with key_j = key_i),
+        // the stable order of R7
+        __shared__ int s_keys[32];
+        if (threadIdx.x < 32) s_keys[threadIdx.x] = (int)threadIdx.x < items ? __ldcg(r.group_ids + threadIdx.x) : -1;
+        __syncthreads();
+        const int G = r.G;
+        for (int u = threadIdx.x; u <= G; u += blockDim.x) {
+            int less = 0, eq = 0;
+            for (int i = 0; i < items; ++i) {
+                const int k = s_keys[i];
+                less += (k >= 0 && k < u) ? 1 : 0;
+                eq += (k == u) ? 1 : 0;
+            }
+            if (u < G) r.counts[u] = eq;
+            r.offsets[u] = less;
+            if (u == G) status[1] = less;
+        }
+        if ((int)threadIdx.x < items) {
+            const int i = threadIdx.x, k = s_keys[i];
+            int A = 0, row = 0;
+            for (int j = 0; j < items; ++j) {
+                const int kj = s_keys[j];
+                A += kj >= 0 ? 1 : 0;
+                row += (kj >= 0 && (kj < k || (kj == k && j < i))) ? 1 : 0;
+            }
+            if (k >= 0) {
+                r.row_token[row] = i / K;
+                r.row_slot[row] = i % K;
+                r.slot_row[i] = row;
+            } else {
+                r.slot_row[i] = -1;
+            }
+            if (i >= A) { r.row_token[i] = -1; r.row_slot[i] = -1; }
+        }
+        return;
+    }
     permute_block_small(r.group_ids, T, K, r.G, per_warp, r.counts, r.offsets, r.row_token, r.row_slot, r.slot_row,
                         status, rs_dyn, &s_total);
 }
