@@ -191,6 +191,7 @@ router_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *__rest
 // pattern); the consumers read the other CTAs' results with ld.global.cg.
 // One token on one CTA (router_kernel) streams all of W_router through a single SM: 7 us at E = 60, D = 2048.
 // -------------------------------------------------------------------------------------------------
+constexpr int kTinyPermItems = 128;    // up to this many (token, slot) items the fused permutation needs no scans
 constexpr int kSplitWarps = 32;        // a CTA of 32 warps x ET experts: E <= 64 needs one CTA per token and no arrival counter
 
 template <int ET>
@@ -281,12 +282,12 @@ router_split_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *
     // ---- R6-R8: this CTA completed the batch ---------------------------------------------------------
     __threadfence();
     const int items = T * K;
-    if (items <= 32) {
-        // at most 32 (token, slot) items: no histograms or scans -- every thread counts the keys below / equal to
-        // its group from the 32 keys in shared memory; item i's row = #(keys < key_i) + #(j < i with key_j = key_i),
+    if (items <= kTinyPermItems) {
+        // at most 128 (token, slot) items: no histograms or scans -- every thread counts the keys below / equal to
+        // its group from the keys in shared memory; item i's row = #(keys < key_i) + #(j < i with key_j = key_i),
         // the stable order of R7
-        __shared__ int s_keys[32];
-        if (threadIdx.x < 32) s_keys[threadIdx.x] = (int)threadIdx.x < items ? __ldcg(r.group_ids + threadIdx.x) : -1;
+        __shared__ int s_keys[kTinyPermItems];
+        if (threadIdx.x < kTinyPermItems) s_keys[threadIdx.x] = (int)threadIdx.x < items ? __ldcg(r.group_ids + threadIdx.x) : -1;
         __syncthreads();
         const int G = r.G;
         for (int u = threadIdx.x; u <= G; u += blockDim.x) {
