@@ -67,7 +67,7 @@ enum {
     BM_PATH_PREFILL = 2, /* 128-token x 256-column tcgen05 tiles (large M; tensor-pipe-bound)  */
     BM_PATH_SIMT = 3,    /* plain CUDA-core kernels; a debugging cross-check, never picked by AUTO */
     BM_PATH_GEMV = 4     /* weight-streaming matrix-vector products on the CUDA cores (FFMA2), <= 8 rows of a set per
-                            pass over its weights; y rows in bf16 + the prefill path's combine (deterministic)    */
+                            pass over its weights; W2 stage fused with the slot-order combine (deterministic)    */
 };
 enum { BM_DECODE_MAX_T = 256 };
 
@@ -171,9 +171,9 @@ int bm_group_mse(const bm_bf16 *Y, const bm_bf16 *U, int T, int D, const int32_t
  * bm_moe_forward -- steps 9-13: out[t] = sum_s gate_w[t,s] * FFN_{group_ids[t,s]}(x_t) + sum_{j<S} FFN_{G+j}(x_t)
  * with FFN_u(x) = W2[u] . ( SiLU(W1[u] x) * (W3[u] x) )   (P:42 with united experts P:46; SwiGLU: A3).
  * bf16 operands, fp32 accumulation (tensor cores; CUDA-core FFMA2 on the matrix-vector path), the intermediate h
- * is rounded to bf16 (A12); on the prefill and matrix-vector paths the per-row expert outputs are rounded to bf16
- * before the fp32 gate-weighted sum, which is taken in slot order (deterministic); the decode path adds fp32
- * partial sums with reductions whose order may vary.
+ * is rounded to bf16 (A12); on the prefill path the per-row expert outputs are rounded to bf16 before the fp32
+ * gate-weighted sum; that sum is taken in slot order on the prefill and matrix-vector paths (deterministic), while
+ * the decode path adds fp32 partial sums with reductions whose order may vary.
  *   x        [T,D]      bf16
  *   routing  as produced by bm_route (or any arrays satisfying the same invariants), same T
  *   W1, W3   [G+S,F,D]  bf16 (united experts 0..G-1, then the S always-on shared experts, A11)

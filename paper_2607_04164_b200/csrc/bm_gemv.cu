@@ -20,8 +20,8 @@
 // l+32, ... of both weight rows (software-pipelined, see warp_units), multiplies them into one fp32 accumulator
 // pair per input row, and the warp adds the lane partials with a shuffle butterfly.  A set with more than
 // 8 rows takes several passes over its weights (correct, slower; BM_PATH_AUTO does not send such shapes
-// here).  gemv2 writes bf16 y rows; the prefill path's combine_kernel applies the gate weights in slot order
-// (deterministic), so the result is defined exactly like the prefill path's.
+// here).  The W2 stage is normally the fused token-major kernel below (gemv2_combine_kernel); the set-major plain
+// kernel writing bf16 y rows + the prefill path's combine_kernel remain as the fallback for huge K + S or F.
 #include "bm_common.cuh"
 
 namespace bm {
@@ -256,6 +256,154 @@ cudaError_t launch_gemv(const GemvArgs &p, int kid, cudaStream_t stream) {
     return e;
 }
 
+// -------------------------------------------------------------------------------------------------
+// W2 stage and gate-weighted combine in one kernel (token-major): a CTA owns a range of output column pairs of
+// one token; its units are (source s, column pair q): rows W2[u_s][2q], W2[u_s][2q+1] against the source's h row.
+// A warp walks its units in one software-pipelined stream (as warp_units), parks (y[2q], y[2q+1]) of every
+// source in shared memory as fp32, and after a barrier the CTA adds them in slot order with the gate weights
+// and stores bf16 out (or the fp32 sums for the tensor-parallel partial) -- no y rows in global memory and no
+// combine launch (3 of the ~30 us of a single-token step).  Deterministic: fixed slot order, one warp per unit.
+// -------------------------------------------------------------------------------------------------
+struct Gemv2Args {
+    const bm_bf16 *h;           // [TK + S*T, F]
+    const bm_bf16 *W2;          // [G+S, D, F]
+    bm_bf16 *out;               // [T, D] or nullptr
+    float *out_f32;             // [T, D] or nullptr
+    const int32_t *group_ids, *slot_row, *n_slots;
+    const float *gate_w;
+    int T, K, G, S, D, F;
+};
+
+__global__ void __launch_bounds__(kGvThreads, 1)
+gemv2_combine_kernel(Gemv2Args p, int max_src, int max_q) {
+    extern __shared__ __align__(16) uint8_t gv_smem[];
+    __shared__ int s_u[32], s_row[32];
+    __shared__ float s_gw[32];
+    const int in_bytes = p.F * 2, n8 = p.F / 8, NQ = p.D / 2;
+    uint8_t *s_in = gv_smem;                                                   // [max_src][F] bf16
+    float *s_y = reinterpret_cast<float *>(gv_smem + (size_t)max_src * in_bytes);   // [max_src][2 * max_q]
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const long long TK = (long long)p.T * p.K;
+    grid_dep_wait();      // h comes from the W1/W3 stage, the routing arrays from bm_route
+    grid_dep_launch();
+    const long long total = (long long)p.T * NQ;
+    const long long per = (total + gridDim.x - 1) / gridDim.x;      // <= max_q by the host's choice
+    const long long lo = (long long)blockIdx.x * per;
+    const long long hi = lo + per < total ? lo + per : total;
+    constexpr int U = 4;
+    const int iters = (n8 + 32 * U - 1) / (32 * U);
+
+    for (long long pos = lo; pos < hi;) {
+        const int t = (int)(pos / NQ);
+        const int qa = (int)(pos - (long long)t * NQ);
+        const int qb = (int)((hi - pos) < (long long)(NQ - qa) ? qa + (hi - pos) : NQ);
+        const int nq = qb - qa;
+        __syncthreads();                                   // the previous segment's tables and buffers are free
+        int n_src = min(max(p.n_slots[t], 0), p.K) + p.S;
+        n_src = n_src < max_src ? n_src : max_src;
+        if (tid < 32) {
+            const int n = n_src - p.S;
+            int u = 0, row = -1;
+            float gw = 0.0f;
+            if (tid < n) {
+                u = p.group_ids[(size_t)t * p.K + tid];
+                row = p.slot_row[(size_t)t * p.K + tid];
+                gw = p.gate_w[(size_t)t * p.K + tid];
+                if (u < 0 || u >= p.G || row < 0 || row >= TK) { u = 0; row = -1; gw = 0.0f; }
+            } else if (tid < n_src) {
+                u = p.G + (tid - n);
+                row = (int)(TK + (long long)(tid - n) * p.T + t);
+                gw = 1.0f;
+            }
+            s_u[tid] = u; s_row[tid] = row; s_gw[tid] = gw;
+        }
+        __syncthreads();
+        const int n_units = n_src * nq;                    // unit v = (source v / nq, column pair qa + v % nq)
+        float acc0 = 0.0f, acc1 = 0.0f;
+        auto load = [&](bool on, int v, int it, uint4 (&va)[U], uint4 (&vb)[U]) {
+            const int sidx = on ? v / nq : 0;
+            const int q = qa + v - sidx * nq;
+            const uint4 *wa = reinterpret_cast<const uint4 *>(p.W2 + ((size_t)s_u[sidx] * p.D + 2 * (size_t)q) * p.F);
+            const uint4 *wb = wa + n8;
+#pragma unroll
+            for (int i = 0; i < U; ++i) {
+                const int c = (it * U + i) * 32 + lane;
+                const bool ok = on && c < n8 && s_row[sidx] >= 0;
+                va[i] = ok ? ld_stream(wa + c) : make_uint4(0u, 0u, 0u, 0u);
+                vb[i] = ok ? ld_stream(wb + c) : make_uint4(0u, 0u, 0u, 0u);
+            }
+        };
+        auto compute = [&](int v, int it, const uint4 (&va)[U], const uint4 (&vb)[U]) {
+            const int sidx = v / nq;
+            const uint8_t *xrow = s_in + (size_t)sidx * in_bytes;
+#pragma unroll
+            for (int i = 0; i < U; ++i) {
+                const int c = (it * U + i) * 32 + lane;
+                if (c < n8) {
+                    const uint32_t a[4] = {va[i].x, va[i].y, va[i].z, va[i].w};
+                    const uint32_t b[4] = {vb[i].x, vb[i].y, vb[i].z, vb[i].w};
+                    const uint4 xv = *reinterpret_cast<const uint4 *>(xrow + (size_t)c * 16);
+                    const uint32_t x[4] = {xv.x, xv.y, xv.z, xv.w};
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        fma2(acc0, acc1, bf16_lo(x[k]), bf16_lo(a[k]), bf16_lo(b[k]));
+                        fma2(acc0, acc1, bf16_hi(x[k]), bf16_hi(a[k]), bf16_hi(b[k]));
+                    }
+                }
+            }
+        };
+        auto finish = [&](int v) {
+            float a = acc0, b = acc1;
+#pragma unroll
+            for (int o = 16; o >= 1; o >>= 1) {
+                a += __shfl_xor_sync(kFullMask, a, o);
+                b += __shfl_xor_sync(kFullMask, b, o);
+            }
+            if (lane == 0) {
+                const int sidx = v / nq;
+                *reinterpret_cast<float2 *>(s_y + ((size_t)sidx * max_q + (v - sidx * nq)) * 2) = make_float2(a, b);
+            }
+            acc0 = acc1 = 0.0f;
+        };
+        uint4 a0[U], b0[U], a1[U], b1[U];
+        int v = warp, it = 0;
+        load(v < n_units, v, 0, a0, b0);
+        // stage the sources' h rows while the first weight loads are in flight (invalid sources: zeros)
+        for (int idx = tid; idx < n_src * n8; idx += kGvThreads) {
+            const int r = idx / n8, c = idx - r * n8;
+            const int row = s_row[r];
+            *reinterpret_cast<uint4 *>(s_in + (size_t)r * in_bytes + (size_t)c * 16) =
+                row >= 0 ? __ldg(reinterpret_cast<const uint4 *>(p.h + (size_t)row * p.F) + c) : make_uint4(0u, 0u, 0u, 0u);
+        }
+        __syncthreads();
+        while (v < n_units) {
+            int vn = v, itn = it + 1;
+            if (itn == iters) { itn = 0; vn += kGvWarps; }
+            load(vn < n_units, vn, itn, a1, b1);
+            compute(v, it, a0, b0);
+            if (it == iters - 1) finish(v);
+            v = vn; it = itn;
+            if (v >= n_units) break;
+            vn = v; itn = it + 1;
+            if (itn == iters) { itn = 0; vn += kGvWarps; }
+            load(vn < n_units, vn, itn, a0, b0);
+            compute(v, it, a1, b1);
+            if (it == iters - 1) finish(v);
+            v = vn; it = itn;
+        }
+        __syncthreads();
+        // F2: slot order, fp32
+        for (int i = tid; i < 2 * nq; i += kGvThreads) {
+            float o = 0.0f;
+            for (int sidx = 0; sidx < n_src; ++sidx) o = fmaf(s_gw[sidx], s_y[((size_t)sidx * max_q) * 2 + i], o);
+            const size_t oi = (size_t)t * p.D + 2 * (size_t)qa + i;
+            if (p.out_f32) p.out_f32[oi] = o;
+            else p.out[oi] = (bm_bf16)f32_to_bf16_bits(o);
+        }
+        pos += nq;
+    }
+}
+
 }  // namespace
 
 cudaError_t launch_forward_gemv(const ForwardArgs &a, cudaStream_t stream) {
@@ -265,6 +413,27 @@ cudaError_t launch_forward_gemv(const ForwardArgs &a, cudaStream_t stream) {
     p.in = a.x; p.Wa = a.W1; p.Wb = a.W3; p.outp = a.h; p.IN = a.D; p.OUT = a.F; p.NQ = a.F;
     cudaError_t e = launch_gemv<true>(p, BM_KERNEL_GEMM1, stream);
     if (e != cudaSuccess) return e;
+    // W2 stage: fused with the combine when the per-CTA buffers fit (they do unless K + S or F is huge)
+    const int max_src = a.K + a.S;
+    const long long total = (long long)a.T * (a.D / 2);
+    const int max_q = (int)((total + num_sms() - 1) / num_sms());
+    const size_t smem2 = (size_t)max_src * a.F * 2 + (size_t)max_src * max_q * 2 * sizeof(float);
+    if (max_src <= 32 && smem2 <= 200 * 1024 && tune_int("BM_GEMV_FUSE", 1) != 0) {
+        Gemv2Args q{};
+        q.h = a.h; q.W2 = a.W2; q.out = a.out_f32 ? nullptr : a.out; q.out_f32 = a.out_f32;
+        q.group_ids = a.r.group_ids; q.slot_row = a.r.slot_row; q.n_slots = a.r.n_slots; q.gate_w = a.r.gate_w;
+        q.T = a.T; q.K = a.K; q.G = a.G; q.S = a.S; q.D = a.D; q.F = a.F;
+        static size_t smem_set = 0;
+        if (smem2 > 48 * 1024 && smem2 > smem_set) {
+            e = cudaFuncSetAttribute(gemv2_combine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
+            if (e != cudaSuccess) return e;
+            smem_set = smem2;
+        }
+        profile_begin(BM_KERNEL_GEMM2, stream);
+        e = launch_kernel(gemv2_combine_kernel, dim3(num_sms()), dim3(kGvThreads), smem2, stream, q, max_src, max_q);
+        profile_end(BM_KERNEL_GEMM2, stream);
+        return e;
+    }
     p.in = a.h; p.Wa = a.W2; p.Wb = a.W2; p.outp = a.y; p.IN = a.F; p.OUT = a.D; p.NQ = a.D / 2;
     e = launch_gemv<false>(p, BM_KERNEL_GEMM2, stream);
     if (e != cudaSuccess) return e;

@@ -227,7 +227,7 @@ def test_calibration_pipeline_end_to_end_against_oracle():
 # ---------------------------------------------------------------------------------------------------
 # tensor parallelism over F (NEXT-4): the ranks emulated one after the other on one GPU
 # ---------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("T,world", [(48, 2), (700, 4), (3000, 2)])
+@pytest.mark.parametrize("T,world", [(1, 2), (48, 2), (700, 4), (3000, 2)])     # T = 1: matrix-vector path, fp32 partial
 def test_tensor_parallel_partials_sum_to_the_layer(T, world):
     import paper_2607_04164_b200 as bm
     from paper_2607_04164_b200.tp import shard_f
