@@ -245,11 +245,14 @@ static int forward_common(const bm_bf16 *x, int T, int D, const bm_routing *rout
         const int max_t = tune_int("BM_DECODE_MAX_T", BM_DECODE_MAX_T);
         const bool few_rows = (long long)T * K <= (long long)tune_int("BM_DECODE_ROWS", 24) * G;
         path = (T <= 64 || (T <= max_t && few_rows)) ? BM_PATH_DECODE : BM_PATH_PREFILL;
-        // matrix-vector streaming when a weight set expects at most ~1 row (single-token decode above all):
-        // the tcgen05 k-block loop has a latency floor that such a step never fills (see bm_gemv.cu)
+        // matrix-vector streaming for one or two tokens whose sets expect at most ~1 row (single-token decode above
+        // all): the tcgen05 k-block loop has a latency floor that such a step never fills (see bm_gemv.cu).
+        // Measured (D = 2048, F = 1408, E = 60, top-4; matrix-vector / tensor path): T = 1: 29-30 / 36-39 us,
+        // T = 2: 42-44 / 43-45 us, T = 3: 53-55 / 51-53 us, T = 8 at G = 60: 93 / 77 us -- beyond two tokens the
+        // token-major W2 stage re-reads weight rows per (token, source) and the equal unit ranges lose balance.
         const int gemv_rows = tune_int("BM_GEMV_ROWS", 1);
-        constexpr int kGemvSharedMaxT = 8;     // an always-on shared expert meets all T tokens: one pass of <= 8 rows
-        if ((S == 0 || T <= kGemvSharedMaxT) && (long long)T * K <= (long long)gemv_rows * G) path = BM_PATH_GEMV;
+        const int gemv_max_t = tune_int("BM_GEMV_MAX_T", 2);
+        if (T <= gemv_max_t && (long long)T * K <= (long long)gemv_rows * G) path = BM_PATH_GEMV;
     }
 
     uint8_t *ws = static_cast<uint8_t *>(workspace);

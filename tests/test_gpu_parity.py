@@ -133,7 +133,7 @@ def test_forward_parity_ragged_shapes(path, T, D, F, E, K, G, S):
 
 
 GEMV_SHAPES = [
-    # T, D, F, E, K, G, S -- the shapes BM_PATH_AUTO sends to the matrix-vector path (T*K <= 4*G)
+    # T, D, F, E, K, G, S -- small batches for the matrix-vector path (BM_PATH_AUTO picks it for T <= 2 with T*K <= G)
     (1, 2048, 1408, 60, 4, 60, 0),        # BJ:configs[4], single-token decode
     (1, 2048, 1408, 60, 4, 8, 0),
     (16, 2048, 1408, 60, 4, 30, 0),       # random map: some sets have more than 8 rows (several passes)
