@@ -526,7 +526,7 @@ def run_sweep(args):
                              tokens_per_s=cfg.T / t_best, t_hbm_us=t_hbm * 1e6, t_flop_us=t_flop * 1e6,
                              bound="hbm" if t_hbm >= t_flop else "tensor", roofline_frac=max(t_hbm, t_flop) / t_best,
                              achieved_gbs=nbytes / t_best / 1e9, achieved_tflops=flops / t_best / 1e12,
-                             path="gemv" if (cfg.T <= 2 and cfg.T * cfg.K <= cfg.G) else "decode" if (cfg.T <= 64 or (cfg.T <= bm.BM_DECODE_MAX_T and cfg.T * cfg.K <= 24 * cfg.G)) else "prefill",
+                             path="gemv" if (cfg.T <= 2 and cfg.T * cfg.K <= cfg.G) else "decode" if (cfg.T <= 64 or (cfg.T <= 192 and cfg.T * cfg.K <= 128 * cfg.G) or (cfg.T <= bm.BM_DECODE_MAX_T and cfg.T * cfg.K <= 24 * cfg.G)) else "prefill",
                              device_status=status))
             sys.stderr.write(f"{cfg.name:24s} A={A:6d} G_act={G_act:3d} stream {t*1e6:9.1f} us"
                              + (f" graph {tg*1e6:9.1f} us" if tg else " " * 19)

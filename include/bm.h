@@ -62,7 +62,8 @@ enum { BM_DEV_BAD_GROUP_MAP = 1, BM_DEV_NONFINITE_LOGIT = 2, BM_DEV_BAD_ROUTING 
 /* execution path of bm_moe_forward_path */
 enum {
     BM_PATH_AUTO = 0,    /* GEMV if T <= 2 and T*K <= G (a weight set expects at most ~1 row: single-token decode); else DECODE if
-                            T <= 64, or T <= BM_DECODE_MAX_T and T*K <= 24*G (few rows per group); else PREFILL */
+                            T <= 64, or T <= 192 and T*K <= 128*G (one chunk per group), or T <= BM_DECODE_MAX_T and
+                            T*K <= 24*G (few rows per group); else PREFILL */
     BM_PATH_DECODE = 1,  /* weight-streaming, weights on the MMA M side (small M; HBM-bound)   */
     BM_PATH_PREFILL = 2, /* 128-token x 256-column tcgen05 tiles (large M; tensor-pipe-bound)  */
     BM_PATH_SIMT = 3,    /* plain CUDA-core kernels; a debugging cross-check, never picked by AUTO */
