@@ -70,7 +70,7 @@ enum {
     BM_PATH_GEMV = 4     /* weight-streaming matrix-vector products on the CUDA cores (FFMA2), <= 8 rows of a set per
                             pass over its weights; W2 stage fused with the slot-order combine (deterministic)    */
 };
-enum { BM_DECODE_MAX_T = 256 };
+enum { BM_DECODE_MAX_T = 384 };
 
 /*
  * Routing of one batch: the result of steps R1-R7.  A host struct of device

@@ -17,7 +17,7 @@ BM_OK = 0
 BM_PATH_AUTO, BM_PATH_DECODE, BM_PATH_PREFILL, BM_PATH_SIMT, BM_PATH_GEMV = 0, 1, 2, 3, 4
 BM_DEV_BAD_GROUP_MAP, BM_DEV_NONFINITE_LOGIT, BM_DEV_BAD_ROUTING = 1, 2, 4
 BM_MAX_E, BM_MAX_K, BM_MAX_G = 512, 16, 512
-BM_DECODE_MAX_T = 256
+BM_DECODE_MAX_T = 384
 
 EXPORTS = ["bm_workspace_bytes", "bm_route", "bm_route_partial", "bm_unite_weights", "bm_expert_histogram",
            "bm_expert_outputs", "bm_gram_workspace_bytes", "bm_cosine_gram", "bm_mse_workspace_bytes", "bm_group_mse",

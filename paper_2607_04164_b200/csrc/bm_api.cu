@@ -241,10 +241,10 @@ static int forward_common(const bm_bf16 *x, int T, int D, const bm_routing *rout
     if (path == BM_PATH_AUTO) {
         // decode (swap-AB weight streaming) for small batches: always up to 64 tokens; up to BM_DECODE_MID_T = 192
         // tokens while a group expects at most one 128-row chunk (the weights then stream once); up to
-        // BM_DECODE_MAX_T = 256 tokens while a group expects at most ~24 rows.  Measured decode / prefill path (us):
+        // BM_DECODE_MAX_T = 384 tokens while a group expects at most ~24 rows.  Measured decode / prefill path (us):
         //   D = 2048, F = 1408, E = 60, top-4:  G = 8: T = 128 60 / 70, T = 192 65 / 67, T = 256 70 / 63;
         //                                       G = 15: T = 128 72 / 80, T = 192 82 / 81, T = 256 95 / 86;
-        //                                       G = 30: T = 192 118 / 122, T = 256 127 / 123;  G = 60: T = 256 185 / 195
+        //                                       G = 30: T = 192 118 / 122, T = 256 127 / 123;  G = 60: T = 256 185 / 195, T = 320 194 / 206, T = 512 204 / 202
         //   D = 4096, F = 14336, E = 8, top-2:  G = 4: T = 128 244 / 284, T = 192 283 / 316, T = 256 297 / 299
         const int max_t = tune_int("BM_DECODE_MAX_T", BM_DECODE_MAX_T);
         const int mid_t = tune_int("BM_DECODE_MID_T", 192);
