@@ -1023,10 +1023,12 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
 
     // CTA pairs (cta_group::2, M = 256 per pair): a pair shares the weight tile, so a CTA stages 32 KB per
     // k-block instead of 48 KB (measured: GEMM1 232 -> 201 us at BJ:configs[3]).  A segment with an odd chunk
-    // count wastes half a pair, so pairs are used when a group expects >= 4 chunks (measured: no gain at
-    // 273 rows/group, 7% slower at 107 rows/group).  BM_PF_PAIR=0/1 overrides.
+    // count wastes half a pair, so pairs are used when a group expects >= 3 chunks.  Measured layer times, pairs /
+    // single CTAs (which gather their rows themselves), D = 2048, F = 1408, E = 60, top-4: 410 rows per group
+    // 253 / 274 us (G = 30, T = 3072) and 511 / 525 us (G = 60, T = 6144); 273 rows per group 198 / 206 us (G = 30)
+    // but 402 / 392 us (G = 60); 137-205 rows per group 293 / 267 and 348 / 338 us.  BM_PF_PAIR=0/1 overrides.
     const int pair_env = tune_int("BM_PF_PAIR", -1);
-    const bool many_rows = (long long)a.T * a.K >= 4LL * kChunkRows * a.G;
+    const bool many_rows = (long long)a.T * a.K >= 3LL * kChunkRows * a.G;
     const bool pair = !decode && (sms & 1) == 0 && (pair_env < 0 ? many_rows : pair_env != 0);
     // GA: GEMM1's own warps gather the token rows (single-CTA prefill tiles); the prep kernel then only builds the
     // schedule.  Measured (T = 4096, G = 60): step 410 -> 398 us (GEMM1 +14 us, gather pass -20 us, A*D*4 bytes of
@@ -1131,7 +1133,7 @@ cudaError_t launch_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 
     p.T = T; p.D = D; p.F = F; p.K = 1; p.G = 0; p.S = E; p.TK = 0;
     p.sched = sched; p.h = h; p.y = y; p.x = x;
     p.ksplit = 1;
-    const bool pair = (num_sms() & 1) == 0 && T >= 4 * kChunkRows && tune_int("BM_PF_PAIR", -1) != 0;   // as launch_forward_tc
+    const bool pair = (num_sms() & 1) == 0 && T >= 3 * kChunkRows && tune_int("BM_PF_PAIR", -1) != 0;   // as launch_forward_tc
     CUtensorMap m_x, m_w1, m_w3, m_w2, m_h;
     if (!make_map_2d(&m_x, x, T, D, 128) || !make_map_3d(&m_w1, W1, E, F, D, 128) || !make_map_3d(&m_w3, W3, E, F, D, 128) ||
         !make_map_3d(&m_w2, W2, E, D, F, pair ? 128 : 256) || !make_map_2d(&m_h, h, (uint64_t)E * T, F, 128))

@@ -1,5 +1,5 @@
-// bm_gemv.cu -- BM_PATH_GEMV: steps 10-12 for very small batches (a weight set meets ~1-4 token rows:
-// single-token decode, T*K <= 4*G) as weight-streaming matrix-vector products on the CUDA cores.
+// bm_gemv.cu -- BM_PATH_GEMV: steps 10-12 for very small batches (a weight set meets about one token row:
+// single-token decode; BM_PATH_AUTO: T <= 2 and T*K <= G) as weight-streaming matrix-vector products on the CUDA cores.
 //
 // Cite: PAPER.md:42 (expert FFN, gate-weighted sum), PAPER.md:46 (united experts cut "the number of experts
 // loaded during inference": at these sizes the layer IS the weight load), A3, A11, A12.
