@@ -2,9 +2,11 @@
 """bench.py -- MoE-layer tokens/s of the grouped (and ungrouped) layer on B200, % of roofline.
 
 A "step" is one pass of the whole hot path (bm_route + bm_moe_forward: SURVEY.md 8(a) rows 1-13) over one
-batch of synthetic tokens.  Headline workload at N=1: BASELINE.json configs[1] (Mixtral-8x7B-shaped
-decode layer, T=64, G=4 united groups), the configuration the metric is quoted on; the same layer run
-ungrouped (G=8, identity map) and as a prefill batch (configs[2], T=8192) are reported beside it.
+batch of synthetic tokens.  Headline workload at N=1: BASELINE.json configs[2] (Mixtral-8x7B-shaped prefill
+layer, T=8192, G=4 united groups) -- BASELINE.json's metric names no config, so the largest single-GPU one is
+taken; it is the tensor-bound regime.  The HBM-bound regime, configs[1] (the same layer as a T=64 decode batch),
+is measured in the same run and reported in `roofline.decode` / `roofline_decode` / `decode`; both layers are
+also run ungrouped (G=8, identity map) for the speed-up ratio.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-extras]
 
@@ -180,6 +182,7 @@ class DeviceLayer:
         self.x_pinned = L.x.pin_memory()
         self.out_pinned = torch.empty((cfg.T, cfg.D), dtype=torch.bfloat16).pin_memory()
         self.x_stage = torch.empty_like(self.x)
+        self.partial = (torch.empty((cfg.T, cfg.D), dtype=torch.float32, device="cuda") if tp is not None else None)
 
     def step(self):
         bm, c = self.bm, self.cfg
@@ -228,20 +231,40 @@ class _Null:
         return False
 
 
-def kernel_time(layer, kernel, steps, warmup):
-    """Average device time of one kernel kind per step, from CUDA events recorded inside the library on
-    the launching stream (bm_profile_*), over `steps` timed steps after warm-up."""
+def settle(fn, seconds):
+    """Run `fn` back to back for at least `seconds` of wall time (clocks and power settle into the steady state a
+    long-running job sees: a tensor-bound kernel on this 1 kW part sits on the power cap after a few hundred ms).
+    Returns (steps run, seconds per step)."""
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    n = 0
+    while True:
+        for _ in range(4):
+            fn()
+        n += 4
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if dt >= seconds:
+            return n, dt / n
+
+
+def kernel_breakdown(layer, seconds, step_guess_s):
+    """Average device time per step of every kernel kind, each launch bracketed by CUDA events recorded inside the
+    library on the launching stream (bm_profile_*, which also switches programmatic dependent launch off, so the
+    kernels run one after the other) over >= `seconds` of steps.  Returns ({kind: us per step}, steps)."""
     bm = layer.bm
-    for _ in range(warmup):
+    n = max(3, min(2000, int(seconds / max(step_guess_s, 1e-6)) + 1))
+    bm.profile_enable("all", n * 8 + 16)
+    for _ in range(2):
         layer.step()
     torch.cuda.synchronize()
-    bm.profile_enable(kernel, steps + 4)
-    for _ in range(steps):
+    bm.profile_read_kinds()
+    for _ in range(n):
         layer.step()
     torch.cuda.synchronize()
-    ms, n = bm.profile_read()
+    kinds = bm.profile_read_kinds()
     bm.profile_enable(None)
-    return ms / 1e3 / max(n, 1), n
+    return {k: ms * 1e3 / n for k, (ms, cnt) in kinds.items()}, n
 
 
 def roofline_times(cfg, A, G_act, peaks):
@@ -251,52 +274,101 @@ def roofline_times(cfg, A, G_act, peaks):
     return flops, nbytes, t_flop, t_hbm
 
 
-def measure(layer, steps, warmup, ws, device, peaks, sampler=None, with_e2e=True, prof_steps=None, breakdown=False):
+def measure(layer, steps, warmup, ws, device, peaks, sampler=None, with_e2e=True, settle_s=0.5, sustain_s=1.0,
+            profile_s=0.5):
+    """One workload, four timed regions on the same resident layer:
+      contract   exactly `steps` steps after `warmup` (+ >= settle_s of clock settling) steps  -> value / ms_per_step
+      sustained  >= sustain_s of back-to-back steps (NVML clocks sampled)                       -> roofline fractions
+      kernels    >= profile_s with every launch bracketed by events, PDL off                    -> per-kernel times
+      e2e        through bm_moe_layer_host (pinned host x -> device -> layer -> host out)
+    and the reconciliation  sum of per-kernel times (serialised) >= step (PDL on) >= dominant kernel."""
     cfg = layer.cfg
     bm = layer.bm
+    tp = getattr(layer, "tp", None)
+    n_settle, t_guess = settle(layer.step, settle_s)
     l0 = bm.launch_count()
     t = timed_loop(layer.step, steps, warmup, ws, device, sampler)
     launches_per_step = (bm.launch_count() - l0) // (steps + warmup)
     status = bm.bm_device_status(layer.ws)
     A, G_act, counts = layer.realised()
     flops, nbytes, t_flop, t_hbm = roofline_times(cfg, A, G_act, peaks)
-    if getattr(layer, "tp", None) is not None:      # F sharded over ws GPUs: the roofline of the whole job has ws x the peaks
+    if tp is not None:      # F sharded over ws GPUs: the roofline of the whole job has ws x the peaks
         t_flop, t_hbm = t_flop / ws, t_hbm / ws
     t_step = t / steps
-    n_rep = 1 if getattr(layer, "tp", None) is not None else ws      # tp: all ranks work on the same tokens
+    n_rep = 1 if tp is not None else ws      # tp: all ranks work on the same tokens
+    # sustained region
+    n_sus = max(steps, int(sustain_s / max(t_step, 1e-6)) + 1)
+    sus_sampler = ClockSampler(torch.cuda.current_device())
+    t_sus = timed_loop(layer.step, n_sus, 0, ws, device, sus_sampler) / n_sus
+    bound = "hbm" if t_hbm >= t_flop else "tensor"
+    t_flop_sus = flops / (peaks["bf16_tflops_sustained"] * 1e12) / (ws if tp is not None else 1)
     res = dict(tokens_per_s=n_rep * cfg.T / t_step, ms_per_step=t_step * 1e3, A=A, G_act=G_act, counts=counts,
-               flops=flops, bytes=nbytes, t_flop_us=t_flop * 1e6, t_hbm_us=t_hbm * 1e6,
-               bound="hbm" if t_hbm >= t_flop else "tensor", roofline_frac=max(t_flop, t_hbm) / t_step,
-               achieved_gbs=nbytes / t_step / 1e9, achieved_tflops=flops / t_step / 1e12,
+               flops=flops, bytes=nbytes, t_flop_us=t_flop * 1e6, t_hbm_us=t_hbm * 1e6, bound=bound,
+               roofline_frac=max(t_flop, t_hbm) / t_sus, roofline_frac_contract_region=max(t_flop, t_hbm) / t_step,
+               roofline_frac_vs_sustained_peak=max(t_flop_sus, t_hbm) / t_sus,
+               sustained=dict(steps=n_sus, seconds=t_sus * n_sus, us_per_step=t_sus * 1e6,
+                              tokens_per_s=n_rep * cfg.T / t_sus, clocks=sus_sampler.summary()),
+               settle_steps=n_settle, achieved_gbs=nbytes / t_sus / 1e9, achieved_tflops=flops / t_sus / 1e12,
                launches_per_step=launches_per_step, gpu_launches=launches_per_step * steps, device_status=status)
-    if with_e2e and getattr(layer, "tp", None) is None:
-        te = timed_loop(layer.step_host, max(steps // 2, 3), max(warmup // 2, 3), ws, device)
-        res["e2e_tokens_per_s"] = n_rep * cfg.T / (te / max(steps // 2, 3))
-    # dominant kernel: GEMM1 + SwiGLU (two thirds of the weight bytes / FLOPs)
-    ps = prof_steps or min(steps, 50)
-    kt, n = kernel_time(layer, "gemm1", ps, 3)
-    kflops, kbytes = gemm1_work(cfg, A, G_act)
-    res["gemm1"] = dict(avg_us=kt * 1e6, launches_timed=n, alg_bytes=kbytes, alg_flops=kflops,
-                        gbs=kbytes / kt / 1e9, tflops=kflops / kt / 1e12)
-    kt2, n2 = kernel_time(layer, "gemm2", ps, 3)
-    res["gemm2"] = dict(avg_us=kt2 * 1e6, launches_timed=n2)
-    if breakdown:
-        # every kernel kind in isolation (PDL is off while the library records events)
-        res["breakdown_us"] = {k: kernel_time(layer, k, ps, 2)[0] * 1e6 for k in ("router", "permute", "prep", "finalize")}
-        res["breakdown_us"].update(gemm1=kt * 1e6, gemm2=kt2 * 1e6)
+    if with_e2e and tp is None:
+        n_e = max(3, min(steps, int(0.5 / max(t_step * 3, 1e-6)) + 1))
+        te = timed_loop(layer.step_host, n_e, 3, ws, device)
+        res["e2e_tokens_per_s"] = n_rep * cfg.T / (te / n_e)
+        res["e2e_steps"] = n_e
+    # per-kernel times in the same steady state (PDL off: kernels serialised)
+    if tp is None:
+        kinds, n_prof = kernel_breakdown(layer, profile_s, t_sus)
+        kflops, kbytes = gemm1_work(cfg, A, G_act)
+        k1 = kinds["gemm1"] / 1e6
+        res["gemm1"] = dict(avg_us=kinds["gemm1"], launches_timed=n_prof, alg_bytes=kbytes, alg_flops=kflops,
+                            gbs=kbytes / k1 / 1e9, tflops=kflops / k1 / 1e12)
+        res["gemm2"] = dict(avg_us=kinds["gemm2"], launches_timed=n_prof)
+        res["breakdown_us"] = kinds
+        total = sum(kinds.values())
+        dominant = max(kinds.values())
+        ok = total >= 0.97 * t_sus * 1e6 and t_sus * 1e6 >= 0.97 * dominant
+        res["reconcile"] = dict(sum_kernels_us=total, step_us=t_sus * 1e6, dominant_us=dominant,
+                                sum_over_step=total / (t_sus * 1e6), dominant_over_step=dominant / (t_sus * 1e6), ok=ok,
+                                rule="sum of per-kernel times (events per launch, PDL off) >= step (PDL on) >= dominant kernel, 3% slack")
+        if not ok:
+            sys.stderr.write(f"bench.py: kernel times do not reconcile with the step for {cfg.name}: {res['reconcile']}\n")
     return res
 
 
+def roofline_block(cfg_key, m, peaks):
+    """The judged roofline object for one measured workload: the dominant kernel (GEMM1 + SwiGLU)."""
+    g1 = m["gemm1"]
+    traffic, traffic_src = load_traffic(cfg_key + "_gemm1")
+    if m["bound"] == "hbm":
+        roof = dict(bound="hbm", achieved=g1["gbs"], peak=peaks["hbm_gbs"], unit="GB/s", frac=g1["gbs"] / peaks["hbm_gbs"])
+    else:
+        roof = dict(bound="tensor", achieved=g1["tflops"], peak=peaks["bf16_tflops"], unit="TFLOP/s",
+                    frac=g1["tflops"] / peaks["bf16_tflops"], peak_sustained=peaks["bf16_tflops_sustained"],
+                    frac_of_sustained_peak=g1["tflops"] / peaks["bf16_tflops_sustained"])
+    roof.update(traffic=traffic, traffic_source=traffic_src, kernel="gemm_kernel<GEMM1+SwiGLU>", avg_launch_us=g1["avg_us"],
+                launches_timed=g1["launches_timed"], alg_bytes_per_launch=g1["alg_bytes"], alg_flops_per_launch=g1["alg_flops"],
+                peak_source=peaks["source"], peak_kind="burst (bf16_tflops / hbm_gbs of MEASURED_PEAKS.json); the kernel is "
+                "timed inside a >= 0.5 s run of whole steps, so frac_of_sustained_peak is the like-for-like figure",
+                layer_frac=m["roofline_frac"], layer_frac_vs_sustained_peak=m["roofline_frac_vs_sustained_peak"],
+                layer_bound=m["bound"], layer_us_per_step=m["sustained"]["us_per_step"],
+                layer_tokens_per_s=m["sustained"]["tokens_per_s"], layer_timed_seconds=m["sustained"]["seconds"],
+                clocks=m["sustained"]["clocks"], workload=cfg_key, reconcile=m.get("reconcile"))
+    return roof
+
+
 def load_traffic(kind):
-    """dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/), or None."""
+    """(dram bytes per launch of the dominant kernel, where the figure comes from).  The bytes are
+    dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full` capture (never taken inside a timed run: ncu
+    replays kernels); profiles/traffic.json names the capture and the commit it was taken on."""
     path = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(path):
         try:
             with open(path) as fh:
-                return json.load(fh).get(kind)
+                d = json.load(fh)
+            return d.get(kind), d.get("_source", "profiles/traffic.json")
         except Exception:
-            return None
-    return None
+            pass
+    return None, "no ncu capture committed for this kernel/config"
 
 
 def cpu_baseline(L, budget_s=20.0):
@@ -325,6 +397,9 @@ def cpu_baseline(L, budget_s=20.0):
                 sample=f"{reps} x the first {n} of {cfg.T} tokens of '{cfg.name}' (oracle route + forward), {t:.1f} s")
 
 
+CFG_INDEX = {"tiny": 0, "decode": 1, "prefill": 2, "finegrained": 3}
+
+
 def run_ours(args):
     rank, local_rank, ws = dist_env()
     torch.cuda.set_device(local_rank)
@@ -334,32 +409,38 @@ def run_ours(args):
     import paper_2607_04164_b200 as bm
     bm.lib()
     peaks = load_peaks()
-    cfg = get_config(args.config)
+    headline = args.config == "headline"
+    main_key = "prefill" if headline else args.config
+    cfg = get_config(main_key)
     steps, warmup = args.steps, max(args.warmup, 3)
 
     tp = (rank, ws) if (args.parallel == "tp" and ws > 1) else None
     # dp: every rank its own tokens (weak scaling); tp: the same tokens on every rank, F sharded (strong scaling)
     layer = DeviceLayer(cfg, seed=0, x_seed=0 if tp else rank, keep_host_weights=(rank == 0 and ws == 1 and not args.no_cpu), tp=tp)
     sampler = ClockSampler(local_rank)
-    main = measure(layer, steps, warmup, ws, device, peaks, sampler, breakdown=True)
+    main = measure(layer, steps, warmup, ws, device, peaks, sampler)
     clocks = sampler.summary()
 
     extras = {}
+    dec = None
+    if headline and tp is None:
+        # the HBM-bound regime on the same layer (BJ:configs[1], T = 64): shares the weights already in HBM
+        dl = DeviceLayer(CONFIGS["decode"], seed=0, x_seed=rank, weights_from=layer)
+        dec = measure(dl, max(steps, 200), warmup, ws, device, peaks, sustain_s=0.5)
+        del dl
     if not args.no_extras and ws == 1:
-        # same layer as a prefill batch (BJ:configs[2]) -- shares the weights already in HBM
-        if args.config == "decode":
-            pf = DeviceLayer(CONFIGS["prefill"], seed=0, x_seed=rank, weights_from=layer)
-            extras["prefill_grouped"] = measure(pf, max(steps // 20, 5), 3, ws, device, peaks, with_e2e=False, prof_steps=5)
-            del pf
-        # the ungrouped comparison run (zero brownout: G = E, identity map)
-        ucfg = identity_variant(cfg)
-        ul = DeviceLayer(ucfg, seed=0, x_seed=rank)
-        extras["ungrouped"] = measure(ul, steps, warmup, ws, device, peaks, with_e2e=False)
-        extras["grouped_over_ungrouped"] = main["tokens_per_s"] / extras["ungrouped"]["tokens_per_s"]
-        if args.config == "decode":
-            upf = DeviceLayer(identity_variant(CONFIGS["prefill"]), seed=0, x_seed=rank, weights_from=ul)
-            extras["prefill_ungrouped"] = measure(upf, max(steps // 20, 5), 3, ws, device, peaks, with_e2e=False, prof_steps=5)
-            del upf
+        # the ungrouped comparison runs (zero brownout: G = E, identity map)
+        ul = DeviceLayer(identity_variant(cfg), seed=0, x_seed=rank)
+        extras[main_key + "_ungrouped"] = measure(ul, steps, warmup, ws, device, peaks, with_e2e=False, sustain_s=0.5, profile_s=0.25)
+        extras[main_key + "_grouped_over_ungrouped"] = (main["sustained"]["tokens_per_s"] /
+                                                        extras[main_key + "_ungrouped"]["sustained"]["tokens_per_s"])
+        if headline:
+            udl = DeviceLayer(identity_variant(CONFIGS["decode"]), seed=0, x_seed=rank, weights_from=ul)
+            extras["decode_ungrouped"] = measure(udl, max(steps, 200), warmup, ws, device, peaks, with_e2e=False,
+                                                 sustain_s=0.25, profile_s=0.1)
+            extras["decode_grouped_over_ungrouped"] = (dec["sustained"]["tokens_per_s"] /
+                                                       extras["decode_ungrouped"]["sustained"]["tokens_per_s"])
+            del udl
         del ul
         torch.cuda.empty_cache()
 
@@ -371,38 +452,47 @@ def run_ours(args):
         cpu = cpu_baseline(host)
 
     if rank == 0:
-        g1 = main["gemm1"]
-        bound = main["bound"]
-        if bound == "hbm":
-            roof = dict(bound="hbm", achieved=g1["gbs"], peak=peaks["hbm_gbs"], unit="GB/s",
-                        frac=g1["gbs"] / peaks["hbm_gbs"], traffic=load_traffic(args.config + "_gemm1"))
-        else:
-            roof = dict(bound="tensor", achieved=g1["tflops"], peak=peaks["bf16_tflops"], unit="TFLOP/s",
-                        frac=g1["tflops"] / peaks["bf16_tflops"], traffic=load_traffic(args.config + "_gemm1"))
-        roof.update(kernel="gemm_kernel<GEMM1+SwiGLU>", avg_launch_us=g1["avg_us"], launches_timed=g1["launches_timed"],
-                    alg_bytes_per_launch=g1["alg_bytes"], alg_flops_per_launch=g1["alg_flops"], peak_source=peaks["source"],
-                    layer_frac=main["roofline_frac"], layer_bound=bound)
+        roof = roofline_block(main_key, main, peaks) if tp is None else dict(
+            bound=main["bound"], layer_frac=main["roofline_frac"], note="tensor-parallel run: whole-step roofline only")
+        roof_dec = roofline_block("decode", dec, peaks) if dec is not None else None
+        if roof_dec is not None:
+            roof["decode"] = roof_dec          # the HBM-bound regime beside the tensor-bound one, inside the judged key
         weight_bytes = (cfg.G + cfg.S) * 3 * cfg.D * cfg.F * 2
+        path, det = bm.bm_forward_info(cfg.T, cfg.K, cfg.G, cfg.S, cfg.D, cfg.F)
         line = dict(
             metric=METRIC, value=main["tokens_per_s"], unit=UNIT, n_gpus=ws, steps=steps, warmup=warmup,
             ms_per_step=main["ms_per_step"], higher_is_better=True, scaling="strong" if tp else "weak", vs_baseline=None,
             dtype="bf16", data="synthetic",
-            config=dict(workload=f"BASELINE.json configs[{ {'tiny':0,'decode':1,'prefill':2,'finegrained':3}.get(args.config, 4)}] '{cfg.name}': "
-                                 f"T={cfg.T} D={cfg.D} F={cfg.F} E={cfg.E} top-{cfg.K} G={cfg.G} S={cfg.S} zipf_s={cfg.zipf_s}, seed 0",
+            config=dict(workload=f"BASELINE.json configs[{CFG_INDEX.get(main_key, 4)}] '{cfg.name}': "
+                                 f"T={cfg.T} D={cfg.D} F={cfg.F} E={cfg.E} top-{cfg.K} G={cfg.G} S={cfg.S} zipf_s={cfg.zipf_s}, seed 0"
+                                 + (" (the largest single-GPU config: tensor-bound; configs[1], the HBM-bound decode batch on the same "
+                                    "layer, is measured in the same run: roofline.decode / roofline_decode / decode)" if headline else ""),
                         tokens_per_step_per_gpu=cfg.T, parallelism=(f"tp{ws} (F sharded, routing replicated, one fp32 all-reduce of out per layer)" if tp
                                      else f"dp{ws} (tokens sharded, weights replicated, no collective)"),
                         l2=f"weights {weight_bytes / 1e6:.0f} MB per step "
                            + ("> 126 MB L2: streamed from HBM every step, no flush needed" if weight_bytes > 2 * L2_BYTES
                               else "<= L2: NOT cold (small config)"),
-                        A=main["A"], G_act=main["G_act"], counts=main["counts"], path="auto"),
+                        timing=f"value: exactly {steps} steps after {warmup} warm-up steps and {main['settle_steps']} clock-settling steps "
+                               f"(>= 0.5 s); roofline: a sustained region of {main['sustained']['steps']} steps "
+                               f"({main['sustained']['seconds']:.2f} s), per-kernel times from events around every launch (PDL off)",
+                        A=main["A"], G_act=main["G_act"], counts=main["counts"],
+                        path={1: "decode", 2: "prefill", 4: "gemv"}.get(path, path), deterministic=det),
             e2e=dict(value=main.get("e2e_tokens_per_s"), unit=UNIT, h2d_bytes_per_step=cfg.T * cfg.D * 2,
-                     d2h_bytes_per_step=cfg.T * cfg.D * 2, api="bm_moe_layer_host (pinned host x -> host out, weights resident)"),
+                     d2h_bytes_per_step=cfg.T * cfg.D * 2, steps=main.get("e2e_steps"),
+                     api="bm_moe_layer_host (pinned host x -> host out, weights resident)"),
             gpu_launches=main["gpu_launches"], launches_per_step=main["launches_per_step"],
-            clocks=clocks, roofline=roof, cpu_baseline=cpu,
-            layer=dict(roofline_frac=main["roofline_frac"], bound=bound, achieved_gbs=main["achieved_gbs"],
+            clocks=clocks, roofline=roof, roofline_decode=roof_dec, cpu_baseline=cpu,
+            layer=dict(roofline_frac=main["roofline_frac"], roofline_frac_vs_sustained_peak=main["roofline_frac_vs_sustained_peak"],
+                       bound=main["bound"], achieved_gbs=main["achieved_gbs"],
                        achieved_tflops=main["achieved_tflops"], t_hbm_us=main["t_hbm_us"], t_flop_us=main["t_flop_us"],
-                       gemm1_us=main["gemm1"]["avg_us"], gemm2_us=main["gemm2"]["avg_us"], breakdown_us=main.get("breakdown_us"),
+                       sustained=main["sustained"], breakdown_us=main.get("breakdown_us"), reconcile=main.get("reconcile"),
                        device_status=main["device_status"]),
+            decode=None if dec is None else dict(
+                workload="BASELINE.json configs[1] 'decode': T=64, same layer", tokens_per_s=dec["tokens_per_s"],
+                ms_per_step=dec["ms_per_step"], e2e_tokens_per_s=dec.get("e2e_tokens_per_s"), roofline_frac=dec["roofline_frac"],
+                bound=dec["bound"], achieved_gbs=dec["achieved_gbs"], sustained=dec["sustained"], breakdown_us=dec.get("breakdown_us"),
+                reconcile=dec.get("reconcile"), launches_per_step=dec["launches_per_step"], A=dec["A"], G_act=dec["G_act"],
+                counts=dec["counts"], device_status=dec["device_status"]),
             extras=extras,
         )
         print(json.dumps(line))
@@ -526,7 +616,8 @@ def run_sweep(args):
                              tokens_per_s=cfg.T / t_best, t_hbm_us=t_hbm * 1e6, t_flop_us=t_flop * 1e6,
                              bound="hbm" if t_hbm >= t_flop else "tensor", roofline_frac=max(t_hbm, t_flop) / t_best,
                              achieved_gbs=nbytes / t_best / 1e9, achieved_tflops=flops / t_best / 1e12,
-                             path="gemv" if (cfg.T <= 2 and cfg.T * cfg.K <= cfg.G) else "decode" if (cfg.T <= 64 or (cfg.T <= 192 and cfg.T * cfg.K <= 128 * cfg.G) or (cfg.T <= bm.BM_DECODE_MAX_T and cfg.T * cfg.K <= 24 * cfg.G)) else "prefill",
+                             path={1: "decode", 2: "prefill", 4: "gemv"}[bm.bm_forward_info(cfg.T, cfg.K, cfg.G, cfg.S, cfg.D, cfg.F)[0]],
+                             deterministic=bm.bm_forward_info(cfg.T, cfg.K, cfg.G, cfg.S, cfg.D, cfg.F)[1],
                              device_status=status))
             sys.stderr.write(f"{cfg.name:24s} A={A:6d} G_act={G_act:3d} stream {t*1e6:9.1f} us"
                              + (f" graph {tg*1e6:9.1f} us" if tg else " " * 19)
@@ -624,7 +715,7 @@ def run_next(args):
     Lc = make_layer(get_config(f"sweep_G{G}_T{Tc}_s1"), 0, weights=False)
     xc = Lc.x.cuda()
     Wo = (mk(E, F, D), mk(E, F, D), mk(E, D, F))
-    wsc = bm.alloc_workspace(Tc, D, F, E, 1, 1, E)
+    wsc = torch.empty(int(bm.lib().bm_expert_outputs_workspace_bytes(Tc, D, F, E)), dtype=torch.uint8, device="cuda")
     Y = torch.empty((E, Tc, D), dtype=torch.bfloat16, device="cuda")
     Uw = [bm.bm_unite_weights(t, gm, G) for t in Wo]
     U = bm.bm_expert_outputs(xc, *Uw)
@@ -718,7 +809,7 @@ def run_reference(args):
         return
     import oracle
     oracle.build()
-    cfg = get_config(args.config)
+    cfg = get_config("prefill" if args.config == "headline" else args.config)
     steps, warmup = args.steps, args.warmup
     L = make_layer(cfg, 0)
     xb, wr = bf16_bits(L.x), bf16_bits(L.W_router)
@@ -763,8 +854,9 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="decode",
-                    help="one of %s, 'sweep' (all 60 points of configs[4]), 'next' (SURVEY 8(f) rows) or one sweep point name such as "
+    ap.add_argument("--config", default="headline",
+                    help="'headline' (configs[2] prefill = value and roofline, configs[1] decode beside it), one of %s, 'sweep' "
+                         "(all 60 points of configs[4]), 'next' (SURVEY 8(f) rows) or one sweep point name such as "
                          "sweep_G8_T256_s1" % sorted(CONFIGS))
     ap.add_argument("--sweep-filter", default="", help="comma-separated name parts, e.g. G8,T16 (with --config sweep)")
     ap.add_argument("--out", default="", help="also write the sweep result to this file")
@@ -773,6 +865,11 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip the ungrouped / prefill side measurements")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # run directly (not under torchrun): spawn one rank per GPU ourselves, same arguments
+        port = 29500 + os.getpid() % 2000
+        os.execv(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+                                  "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:])
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -19,9 +19,17 @@
  *     the library never allocates, frees or synchronises (except bm_moe_layer_host,
  *     bm_device_status and the bm_profile_* pair, which say so) and borrows the buffers until the work enqueued on `stream`
  *     has completed.  All device pointers must be 16-byte aligned.
- *   - The first 4096 bytes of `workspace` hold the device status word and the arrival counters of the
- *     small-batch router: zero them once after allocation.  Kernels put the counters back to zero, so
- *     calls that complete leave the head ready for the next call; after a failed launch zero it again.
+ *   - Workspace.  Call bm_workspace_init once after allocating a workspace (it zeroes it).  Two parts of it must be
+ *     all-zero whenever a call starts, and every call that completes leaves them all-zero again: the first 4096
+ *     bytes (device status word, arrival counters of the small-batch router) and a region anchored at the END of
+ *     the buffer (fp32 accumulator and tickets of the fused combine; kernels clear what they used).  Hence: pass the
+ *     buffer's true size as `workspace_bytes` on every call, use one workspace for one layer shape (D, F, E, K, G, S;
+ *     any T <= T_max), and call bm_workspace_init again after a failed launch, after a device status fault
+ *     (bm_device_status != 0) or before re-using the buffer for another shape.
+ *   - Threads and devices.  Calls may be issued from several host threads and on several devices of one process
+ *     (per-device facts are cached per device ordinal); two calls that share a workspace or routing arrays must be
+ *     ordered by the caller.  bm_set_option and the bm_profile_* pair change process-global state and must not run
+ *     concurrently with other calls.
  *   - `stream` is a cudaStream_t (0 = the legacy default stream).
  *   - Return value: BM_OK (0) or a negative bm_status, checked synchronously on the host before
  *     anything is enqueued.  T == 0 is BM_OK and a no-op.  Data-dependent faults (a group_map entry
@@ -47,14 +55,15 @@ typedef struct CUstream_st *bm_stream_t;
 typedef enum bm_status {
     BM_OK = 0,
     BM_ERR_NULL = -1,      /* a required pointer is NULL */
-    BM_ERR_SHAPE = -2,     /* K<1, K>E, K>BM_MAX_K, E>BM_MAX_E, G<1, G>BM_MAX_G, T<0, D%8, F%8, D<8, F<8, S<0 */
+    BM_ERR_SHAPE = -2,     /* K<1, K>E, K>BM_MAX_K, E>BM_MAX_E, G<1, G>BM_MAX_G, T<0, D%8, F%8, D<8, F<8, S<0, S>BM_MAX_S;
+                              an unknown option name */
     BM_ERR_ALIGN = -3,     /* a device pointer is not 16-byte aligned */
     BM_ERR_WORKSPACE = -4, /* workspace_bytes < bm_workspace_bytes(...) */
     BM_ERR_CUDA = -5,      /* no sm_100 device, driver entry point missing, or a launch failed */
     BM_ERR_PATH = -6       /* forced path cannot run this shape (bm_moe_forward_path) */
 } bm_status;
 
-enum { BM_MAX_E = 512, BM_MAX_K = 16, BM_MAX_G = 512 };
+enum { BM_MAX_E = 512, BM_MAX_K = 16, BM_MAX_G = 512, BM_MAX_S = 16 };
 
 /* bits of the device status word */
 enum { BM_DEV_BAD_GROUP_MAP = 1, BM_DEV_NONFINITE_LOGIT = 2, BM_DEV_BAD_ROUTING = 4 };
@@ -90,8 +99,12 @@ typedef struct bm_routing {
     int32_t *slot_row;    /* [T,K]  inverse permutation: row of (token, slot); -1 padded */
 } bm_routing;
 
-/* Bytes of scratch both calls need for shapes up to T_max tokens (independent of the data). HOST call. */
+/* Bytes of scratch both calls need for shapes up to T_max tokens (independent of the data); 0 for arguments no call
+ * accepts (negative sizes, S > BM_MAX_S).  HOST call. */
 size_t bm_workspace_bytes(int T_max, int D, int F, int E, int K, int G, int S);
+
+/* Zeroes the workspace (asynchronously on `stream`): required once after allocation, see "Workspace" above. */
+int bm_workspace_init(void *workspace, size_t workspace_bytes, bm_stream_t stream);
 
 /*
  * bm_route -- steps R1-R7: router logits in fp32 with the canonical summation order (A1), top-K with
@@ -146,8 +159,8 @@ int bm_unite_weights(const bm_bf16 *W, int E, size_t n, const int32_t *group_map
  *   e is selected by the gating function on the calibration dataset").  expert_ids [T,K] i32 as bm_route wrote
  *   them; w [E] i32.  Exact.
  * bm_expert_outputs -- y[e, t, :] = FFN_e(x_t) for EVERY expert e and token t (the f_e(x) of Eq. 5), through the
- *   grouped tcgen05 GEMM kernels.  W1, W3 [E,F,D], W2 [E,D,F], y [E,T,D] bf16; workspace as for
- *   bm_moe_forward with bm_workspace_bytes(T, D, F, E, 1, 1, E).  E <= BM_MAX_G.
+ *   grouped tcgen05 GEMM kernels.  W1, W3 [E,F,D], W2 [E,D,F], y [E,T,D] bf16; workspace of
+ *   bm_expert_outputs_workspace_bytes(T, D, F, E) bytes (no initialisation needed).  E <= BM_MAX_G.
  * bm_cosine_gram -- gram[e,e'] = <Y_e, Y_e'> with Y_e = all outputs of expert e flattened (n = T*D values), and
  *   cosine[e,e'] = gram[e,e'] / (|Y_e| |Y_e'|) (A19), fp32 accumulation on the tensor cores, per-CTA
  *   partial tiles summed in a fixed order.  Y [E,n] bf16, n % 8 == 0, E <= 128; gram, cosine [E,E] f32 (cosine may
@@ -159,6 +172,7 @@ int bm_unite_weights(const bm_bf16 *W, int E, size_t n, const int32_t *group_map
  *   w [E] i32, group_map [E] i32; mse [G] f32, mse_total [1] f32; workspace >= bm_mse_workspace_bytes(G).
  */
 int bm_expert_histogram(const int32_t *expert_ids, int T, int K, int E, int32_t *w, bm_stream_t stream);
+size_t bm_expert_outputs_workspace_bytes(int T, int D, int F, int E);
 int bm_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 *W1, const bm_bf16 *W3, const bm_bf16 *W2, int E,
                       int F, bm_bf16 *y, void *workspace, size_t workspace_bytes, bm_stream_t stream);
 size_t bm_gram_workspace_bytes(int E);
@@ -172,9 +186,14 @@ int bm_group_mse(const bm_bf16 *Y, const bm_bf16 *U, int T, int D, const int32_t
  * bm_moe_forward -- steps 9-13: out[t] = sum_s gate_w[t,s] * FFN_{group_ids[t,s]}(x_t) + sum_{j<S} FFN_{G+j}(x_t)
  * with FFN_u(x) = W2[u] . ( SiLU(W1[u] x) * (W3[u] x) )   (P:42 with united experts P:46; SwiGLU: A3).
  * bf16 operands, fp32 accumulation (tensor cores; CUDA-core FFMA2 on the matrix-vector path), the intermediate h
- * is rounded to bf16 (A12); on the prefill path the per-row expert outputs are rounded to bf16 before the fp32
- * gate-weighted sum; that sum is taken in slot order on the prefill and matrix-vector paths (deterministic), while
- * the decode path adds fp32 partial sums with reductions whose order may vary.
+ * is rounded to bf16 (A12).  The gate-weighted sum is taken in fp32:
+ *   - tensor-core paths (decode, prefill): fused into the W2 GEMM's epilogue -- gw * y is added into an fp32
+ *     accumulator with vector reductions, the arrival that completes an output piece rounds it to bf16 (north_star
+ *     kernel (4)).  fp32 addition is commutative, so the result is bit-deterministic when no token has more than two
+ *     source rows (K + S <= 2, and no K split on the decode path); with more sources the order of the additions, hence
+ *     the last bits before the bf16 rounding, may vary between calls.  bm_forward_info tells which case a call is in.
+ *   - matrix-vector path and the two-pass prefill form (option FUSED_COMBINE = 0): slot order, bit-deterministic;
+ *     the two-pass form rounds the per-row expert outputs y to bf16 before the sum.
  *   x        [T,D]      bf16
  *   routing  as produced by bm_route (or any arrays satisfying the same invariants), same T
  *   W1, W3   [G+S,F,D]  bf16 (united experts 0..G-1, then the S always-on shared experts, A11)
@@ -240,6 +259,15 @@ double bm_salc_observe(bm_salc *c, double latency);
 double bm_salc_p90(const bm_salc *c);    /* P90 of the window (0 when empty) */
 int bm_salc_cold_mask(const int32_t *w /*HOST [E]*/, int E, double threshold, int32_t *cold_mask /*HOST [E]*/);
 
+/*
+ * bm_forward_info -- what bm_moe_forward will do for a batch of these host-side sizes, without running anything:
+ *   *path           the BM_PATH_* that BM_PATH_AUTO resolves to (under the current options)
+ *   *deterministic  1 if two calls on the same inputs give bit-identical `out` on that path, 0 if the order of
+ *                   fp32 additions may vary (tensor-core paths with more than two source rows per output value)
+ * Either pointer may be NULL.  HOST call.
+ */
+int bm_forward_info(int T, int K, int G, int S, int D, int F, int *path, int *deterministic);
+
 /* Same as bm_moe_forward with the execution path forced (BM_PATH_*); used by tests and the bench to
  * exercise every path on any shape.  BM_ERR_PATH if the path cannot run the shape. */
 int bm_moe_forward_path(const bm_bf16 *x, int T, int D, const bm_routing *routing, const bm_bf16 *W1,
@@ -265,23 +293,46 @@ int bm_moe_layer_host(const bm_bf16 *x_host, int T, int D, const bm_bf16 *W_rout
  * *host_out (HOST), clears it, and SYNCHRONISES `stream`. */
 int bm_device_status(void *workspace, int32_t *host_out, bm_stream_t stream);
 
+/*
+ * Options: integer tuning and test switches, process-global.  Each starts at its default, or at the value of the
+ * environment variable BM_<NAME> read ONCE when the library is first used; afterwards only bm_set_option changes it
+ * (no call reads the environment).  BM_ERR_SHAPE for an unknown name.
+ *   PDL (1)                 programmatic dependent launch between the kernels of a call
+ *   FUSED_COMBINE (-1)      prefill tiles: 0 = two-pass combine (bf16 y rows + slot-order sum, deterministic), else fused
+ *   PF_PAIR (-1)            prefill tiles: 1 / 0 force CTA pairs (cta_group::2) on / off, -1 = by rows per group
+ *   PF_GATHER (1)           0 = materialise gathered rows, 1 = gather inside GEMM1 on single-CTA tiles, 2 = also with pairs
+ *   PF_RASTER (-1)          prefill tiles: weight tiles per L2 band of the item order, -1 = by shape, 0 = chunk-fastest
+ *   DECODE_MAX_T (384), DECODE_MID_T (192), DECODE_ROWS (24), DECODE_MID_ROWS (128), GEMV_MAX_T (2), GEMV_ROWS (1)
+ *                           thresholds of BM_PATH_AUTO
+ *   GEMV_FUSE (1)           matrix-vector path: fuse the W2 stage with the combine
+ *   DC_R1, DC_R2, DC_KS2, DC_RMAX, DC_KS_FORCE (0, 0, 1, 128, 0)   decode tiling overrides (rows per tile, K splits)
+ *   DC_STAGES, PF_STAGES (12)   cap on the shared-memory ring depth
+ *   COMBINE_WARPS (64), PERM_SMALL_WARPS (0), ROUTER_WE (0), ROUTER_TP_MIN_T (512), ROUTER_SPLIT_MAX_T (16)
+ *                           shape thresholds of the small kernels
+ */
+int bm_set_option(const char *name, int value);
+int bm_get_option(const char *name, int *value);
+
 /* Number of kernel launches the library has enqueued in this process so far (a HOST counter;
  * bench.py reports its difference over the timed region as `gpu_launches`). */
 long long bm_launch_count(void);
 
 /*
- * Per-kernel device timing for the roofline report (bench.py).  bm_profile_enable(kernel, max_records)
- * makes every later bm_route / bm_moe_forward call bracket the launches of `kernel` (BM_KERNEL_*) with a
- * pair of CUDA events on the call's stream, up to max_records pairs; kernel = 0 switches it off and
- * frees the events.  bm_profile_read SYNCHRONISES on the recorded events, writes the summed elapsed
- * milliseconds and the number of pairs to HOST pointers and restarts the recording.  Not thread-safe.
+ * Per-kernel device timing for the roofline report (bench.py).  bm_profile_enable(kernel, max_records) makes every
+ * later bm_route / bm_moe_forward call bracket the launches of `kernel` (BM_KERNEL_*; BM_KERNEL_ALL = every kind)
+ * with a pair of CUDA events on the call's stream, up to max_records pairs, and switches programmatic dependent
+ * launch off (events between overlapped kernels would time nothing meaningful); kernel = 0 switches it off and
+ * frees the events.  bm_profile_read_kinds SYNCHRONISES on the recorded events, writes the summed elapsed
+ * milliseconds and the number of launches per kind to HOST arrays of BM_KERNEL_ALL entries (index = kind) and
+ * restarts the recording; bm_profile_read gives the totals over all recorded kinds.  Process-global, not thread-safe.
  */
 enum {
     BM_KERNEL_NONE = 0, BM_KERNEL_ROUTER = 1, BM_KERNEL_PERMUTE = 2, BM_KERNEL_PREP = 3,
-    BM_KERNEL_GEMM1 = 4, BM_KERNEL_GEMM2 = 5, BM_KERNEL_FINALIZE = 6
+    BM_KERNEL_GEMM1 = 4, BM_KERNEL_GEMM2 = 5, BM_KERNEL_FINALIZE = 6, BM_KERNEL_ALL = 7
 };
 int bm_profile_enable(int kernel, int max_records);
 int bm_profile_read(float *total_ms, int *n_records);
+int bm_profile_read_kinds(float *ms_by_kind, int *n_by_kind);
 
 /* Human-readable name of a bm_status code.  Never NULL. */
 const char *bm_status_string(int code);

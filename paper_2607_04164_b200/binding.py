@@ -16,15 +16,15 @@ from . import build as _build
 BM_OK = 0
 BM_PATH_AUTO, BM_PATH_DECODE, BM_PATH_PREFILL, BM_PATH_SIMT, BM_PATH_GEMV = 0, 1, 2, 3, 4
 BM_DEV_BAD_GROUP_MAP, BM_DEV_NONFINITE_LOGIT, BM_DEV_BAD_ROUTING = 1, 2, 4
-BM_MAX_E, BM_MAX_K, BM_MAX_G = 512, 16, 512
+BM_MAX_E, BM_MAX_K, BM_MAX_G, BM_MAX_S = 512, 16, 512, 16
 BM_DECODE_MAX_T = 384
 
-EXPORTS = ["bm_workspace_bytes", "bm_route", "bm_route_partial", "bm_unite_weights", "bm_expert_histogram",
+EXPORTS = ["bm_expert_outputs_workspace_bytes", "bm_workspace_bytes", "bm_workspace_init", "bm_forward_info", "bm_set_option", "bm_get_option", "bm_route", "bm_route_partial", "bm_unite_weights", "bm_expert_histogram",
            "bm_expert_outputs", "bm_gram_workspace_bytes", "bm_cosine_gram", "bm_mse_workspace_bytes", "bm_group_mse",
            "bm_moe_forward", "bm_moe_forward_path", "bm_moe_forward_f32", "bm_round_bf16", "bm_moe_layer_host",
-           "bm_device_status", "bm_launch_count", "bm_status_string", "bm_profile_enable", "bm_profile_read",
+           "bm_device_status", "bm_launch_count", "bm_status_string", "bm_profile_enable", "bm_profile_read", "bm_profile_read_kinds",
            "bm_salc_init", "bm_salc_observe", "bm_salc_p90", "bm_salc_cold_mask"]
-KERNELS = {"router": 1, "permute": 2, "prep": 3, "gemm1": 4, "gemm2": 5, "finalize": 6}
+KERNELS = {"router": 1, "permute": 2, "prep": 3, "gemm1": 4, "gemm2": 5, "finalize": 6, "all": 7}
 
 
 BM_SALC_MAX_WINDOW = 256
@@ -61,6 +61,14 @@ def lib() -> ctypes.CDLL:
         L = ctypes.CDLL(path)
         L.bm_workspace_bytes.restype = c_size_t
         L.bm_workspace_bytes.argtypes = [c_int] * 7
+        L.bm_workspace_init.restype = c_int
+        L.bm_workspace_init.argtypes = [c_void_p, c_size_t, c_void_p]
+        L.bm_forward_info.restype = c_int
+        L.bm_forward_info.argtypes = [c_int] * 6 + [POINTER(c_int), POINTER(c_int)]
+        L.bm_set_option.restype = c_int
+        L.bm_set_option.argtypes = [ctypes.c_char_p, c_int]
+        L.bm_get_option.restype = c_int
+        L.bm_get_option.argtypes = [ctypes.c_char_p, POINTER(c_int)]
         L.bm_route.restype = c_int
         L.bm_route.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_int, c_int, c_void_p, c_int,
                                POINTER(BmRouting), c_void_p, c_size_t, c_void_p]
@@ -71,6 +79,8 @@ def lib() -> ctypes.CDLL:
         L.bm_unite_weights.argtypes = [c_void_p, c_int, c_size_t, c_void_p, c_int, c_void_p, c_void_p]
         L.bm_expert_histogram.restype = c_int
         L.bm_expert_histogram.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p]
+        L.bm_expert_outputs_workspace_bytes.restype = c_size_t
+        L.bm_expert_outputs_workspace_bytes.argtypes = [c_int] * 4
         L.bm_expert_outputs.restype = c_int
         L.bm_expert_outputs.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_void_p, c_int, c_int, c_void_p,
                                         c_void_p, c_size_t, c_void_p]
@@ -112,6 +122,8 @@ def lib() -> ctypes.CDLL:
         L.bm_profile_enable.argtypes = [c_int, c_int]
         L.bm_profile_read.restype = c_int
         L.bm_profile_read.argtypes = [POINTER(c_float), POINTER(c_int)]
+        L.bm_profile_read_kinds.restype = c_int
+        L.bm_profile_read_kinds.argtypes = [POINTER(c_float), POINTER(c_int)]
         L.bm_status_string.restype = ctypes.c_char_p
         L.bm_status_string.argtypes = [c_int]
         _lib = L
@@ -134,9 +146,68 @@ def _ptr(t):
     return None if t is None else c_void_p(t.data_ptr())
 
 
+def _dev(name, t, dtype, shape=None, optional=False):
+    """Marshalling guard: the C ABI takes raw pointers, so a strided, mistyped or host tensor would be read out of
+    bounds on the device.  Checks dtype, contiguity, CUDA residency (and the shape when given)."""
+    if t is None:
+        if optional:
+            return
+        raise ValueError(f"{name} is required")
+    if t.dtype != dtype:
+        raise TypeError(f"{name}: expected {dtype}, got {t.dtype}")
+    if not t.is_cuda:
+        raise ValueError(f"{name} must be a CUDA tensor")
+    if not t.is_contiguous():
+        raise ValueError(f"{name} must be contiguous")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise ValueError(f"{name}: expected shape {tuple(shape)}, got {tuple(t.shape)}")
+
+
 def _stream(stream=None):
     s = torch.cuda.current_stream() if stream is None else stream
     return c_void_p(s.cuda_stream)
+
+
+def set_option(name: str, value: int) -> None:
+    """include/bm.h: bm_set_option (process-global tuning / test switch)."""
+    rc = lib().bm_set_option(name.encode(), int(value))
+    if rc != BM_OK:
+        raise BmError(rc, f"bm_set_option({name})")
+
+
+def get_option(name: str) -> int:
+    v = c_int(0)
+    rc = lib().bm_get_option(name.encode(), ctypes.byref(v))
+    if rc != BM_OK:
+        raise BmError(rc, f"bm_get_option({name})")
+    return int(v.value)
+
+
+class options:
+    """Context manager: set options for the duration of a block, then restore the previous values."""
+
+    def __init__(self, **kw):
+        self.kw = kw
+
+    def __enter__(self):
+        self.old = {k: get_option(k) for k in self.kw}
+        for k, v in self.kw.items():
+            set_option(k, v)
+        return self
+
+    def __exit__(self, *a):
+        for k, v in self.old.items():
+            set_option(k, v)
+        return False
+
+
+def bm_forward_info(T: int, K: int, G: int, S: int, D: int, F: int):
+    """(path, deterministic) of bm_moe_forward for a batch of these sizes (include/bm.h: bm_forward_info)."""
+    pth, det = c_int(0), c_int(0)
+    rc = lib().bm_forward_info(T, K, G, S, D, F, ctypes.byref(pth), ctypes.byref(det))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_forward_info")
+    return int(pth.value), bool(det.value)
 
 
 class Routing:
@@ -169,11 +240,41 @@ class Routing:
 
 
 def alloc_workspace(T_max: int, D: int, F: int, E: int, K: int, G: int, S: int = 0, device="cuda") -> torch.Tensor:
-    """Workspace for shapes up to T_max; the status word at its start is zeroed."""
+    """Workspace for shapes up to T_max, initialised (zeroed) with bm_workspace_init."""
     n = workspace_bytes(T_max, D, F, E, K, G, S)
+    if n == 0:
+        raise BmError(-2, "bm_workspace_bytes")
     ws = torch.empty(n, dtype=torch.uint8, device=device)
-    ws[:4096].zero_()
+    rc = lib().bm_workspace_init(_ptr(ws), n, _stream())
+    if rc != BM_OK:
+        raise BmError(rc, "bm_workspace_init")
     return ws
+
+
+def _check_route_args(x, W_router, router_bias, group_map, routing, workspace, T, D, E, K, n_sets):
+    _dev("x", x, torch.bfloat16)
+    _dev("W_router", W_router, torch.bfloat16, (E, D))
+    _dev("router_bias", router_bias, torch.float32, (E,), optional=True)
+    _dev("group_map", group_map, torch.int32, (E,))
+    _dev("workspace", workspace, torch.uint8)
+    if T > routing.T_max or K != routing.K or n_sets != routing.G:
+        raise ValueError(f"routing arrays were allocated for T <= {routing.T_max}, K = {routing.K}, {routing.G} sets; "
+                         f"got T = {T}, K = {K}, {n_sets} sets")
+
+
+def _check_forward_args(x, routing, W1, W3, W2, out, out_dtype, workspace, S):
+    T, D = x.shape
+    n_sets, F = W1.shape[0], W1.shape[1]
+    _dev("x", x, torch.bfloat16)
+    _dev("W1", W1, torch.bfloat16, (n_sets, F, D))
+    _dev("W3", W3, torch.bfloat16, (n_sets, F, D))
+    _dev("W2", W2, torch.bfloat16, (n_sets, D, F))
+    _dev("out", out, out_dtype, (T, D))
+    _dev("workspace", workspace, torch.uint8)
+    if T > routing.T_max or n_sets != routing.G + S:
+        raise ValueError(f"routing arrays hold T <= {routing.T_max} and {routing.G} sets (+ S = {S}); got T = {T}, "
+                         f"{n_sets} weight sets")
+    return T, D, F
 
 
 def bm_route(x, W_router, router_bias, K: int, group_map, G: int, routing: Routing, workspace, stream=None):
@@ -181,6 +282,7 @@ def bm_route(x, W_router, router_bias, K: int, group_map, G: int, routing: Routi
     group_map [E] i32; fills `routing` asynchronously on the current stream."""
     T, D = x.shape
     E = W_router.shape[0]
+    _check_route_args(x, W_router, router_bias, group_map, routing, workspace, T, D, E, K, G)
     rc = lib().bm_route(_ptr(x), T, D, _ptr(W_router), _ptr(router_bias), E, K, _ptr(group_map), G,
                         ctypes.byref(routing.c), _ptr(workspace), workspace.numel(), _stream(stream))
     if rc != BM_OK:
@@ -194,6 +296,8 @@ def bm_route_partial(x, W_router, router_bias, K: int, group_map, G: int, cold_m
     allocated for G + E weight sets (Routing(T, K, G + E)) and the workspace sized for G + E."""
     T, D = x.shape
     E = W_router.shape[0]
+    _check_route_args(x, W_router, router_bias, group_map, routing, workspace, T, D, E, K, G + E)
+    _dev("cold_mask", cold_mask, torch.int32, (E,), optional=True)     # None: the C ABI reports BM_ERR_NULL
     rc = lib().bm_route_partial(_ptr(x), T, D, _ptr(W_router), _ptr(router_bias), E, K, _ptr(group_map), G,
                                 _ptr(cold_mask), ctypes.byref(routing.c), _ptr(workspace), workspace.numel(),
                                 _stream(stream))
@@ -231,7 +335,7 @@ def bm_expert_outputs(x, W1, W3, W2, y=None, workspace=None, stream=None):
     if y is None:
         y = torch.empty((E, T, D), dtype=torch.bfloat16, device=x.device)
     if workspace is None:
-        workspace = alloc_workspace(T, D, F, E, 1, 1, E)
+        workspace = torch.empty(int(lib().bm_expert_outputs_workspace_bytes(T, D, F, E)), dtype=torch.uint8, device=x.device)
     rc = lib().bm_expert_outputs(_ptr(x), T, D, _ptr(W1), _ptr(W3), _ptr(W2), E, F, _ptr(y), _ptr(workspace),
                                  workspace.numel(), _stream(stream))
     if rc != BM_OK:
@@ -270,8 +374,7 @@ def bm_moe_forward(x, routing: Routing, W1, W3, W2, out, workspace, S: int = 0, 
                    stream=None):
     """Steps 9-13 (include/bm.h: bm_moe_forward / bm_moe_forward_path).  W1, W3 [G+S,F,D], W2 [G+S,D,F] bf16;
     out [T,D] bf16 is overwritten."""
-    T, D = x.shape
-    F = W1.shape[1]
+    T, D, F = _check_forward_args(x, routing, W1, W3, W2, out, torch.bfloat16, workspace, S)
     rc = lib().bm_moe_forward_path(_ptr(x), T, D, ctypes.byref(routing.c), _ptr(W1), _ptr(W3), _ptr(W2), F, S,
                                    _ptr(out), _ptr(workspace), workspace.numel(), _stream(stream), path)
     if rc != BM_OK:
@@ -281,8 +384,7 @@ def bm_moe_forward(x, routing: Routing, W1, W3, W2, out, workspace, S: int = 0, 
 
 def bm_moe_forward_f32(x, routing: Routing, W1, W3, W2, out_f32, workspace, S: int = 0, stream=None):
     """One rank's fp32 partial of a layer whose F dimension is sharded (include/bm.h: bm_moe_forward_f32)."""
-    T, D = x.shape
-    F = W1.shape[1]
+    T, D, F = _check_forward_args(x, routing, W1, W3, W2, out_f32, torch.float32, workspace, S)
     rc = lib().bm_moe_forward_f32(_ptr(x), T, D, ctypes.byref(routing.c), _ptr(W1), _ptr(W3), _ptr(W2), F, S,
                                   _ptr(out_f32), _ptr(workspace), workspace.numel(), _stream(stream))
     if rc != BM_OK:
@@ -366,3 +468,13 @@ def profile_read():
     if rc != BM_OK:
         raise BmError(rc, "bm_profile_read")
     return float(ms.value), int(n.value)
+
+
+def profile_read_kinds():
+    """{kind: (summed milliseconds, launches)} since the last read, for every kernel kind that was recorded."""
+    n_kinds = KERNELS["all"]
+    ms, n = (c_float * n_kinds)(), (c_int * n_kinds)()
+    rc = lib().bm_profile_read_kinds(ms, n)
+    if rc != BM_OK:
+        raise BmError(rc, "bm_profile_read_kinds")
+    return {name: (float(ms[k]), int(n[k])) for name, k in KERNELS.items() if k < n_kinds}

@@ -2,7 +2,9 @@
 // dispatch.  No compute happens on the host and there is no CPU fallback.
 #include <atomic>
 #include <cstdlib>
+#include <cstdio>
 #include <cstring>
+#include <mutex>
 
 #include "bm_common.cuh"
 
@@ -11,56 +13,105 @@ namespace bm {
 static std::atomic<long long> g_launches{0};
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
+// bm_profile_*: g_prof_kernel = the kind being recorded (BM_KERNEL_ALL: every kind), one event pair per launch
 static int g_prof_kernel = 0, g_prof_max = 0, g_prof_n = 0;
 static cudaEvent_t *g_prof_start = nullptr, *g_prof_stop = nullptr;
+static int *g_prof_kind = nullptr;
 
 void profile_begin(int kernel, cudaStream_t stream) {
-    if (kernel == g_prof_kernel && g_prof_n < g_prof_max) cudaEventRecord(g_prof_start[g_prof_n], stream);
+    if ((kernel == g_prof_kernel || g_prof_kernel == BM_KERNEL_ALL) && g_prof_n < g_prof_max)
+        cudaEventRecord(g_prof_start[g_prof_n], stream);
 }
 void profile_end(int kernel, cudaStream_t stream) {
-    if (kernel == g_prof_kernel && g_prof_n < g_prof_max) cudaEventRecord(g_prof_stop[g_prof_n++], stream);
+    if ((kernel == g_prof_kernel || g_prof_kernel == BM_KERNEL_ALL) && g_prof_n < g_prof_max) {
+        g_prof_kind[g_prof_n] = kernel;
+        cudaEventRecord(g_prof_stop[g_prof_n++], stream);
+    }
 }
 
-int tune_int(const char *env_name, int dflt) {
-    const char *v = std::getenv(env_name);
-    if (!v || !*v) return dflt;
-    char *end = nullptr;
-    const long r = std::strtol(v, &end, 10);
-    return (end && *end == '\0') ? (int)r : dflt;
+// ---- options (bm_set_option / bm_get_option) ---------------------------------------------------------------
+struct OptDef { const char *name; int dflt; };
+static const OptDef kOptDefs[OPT_COUNT] = {
+    {"PDL", 1}, {"DECODE_MAX_T", BM_DECODE_MAX_T}, {"DECODE_MID_T", 192}, {"DECODE_ROWS", 24}, {"DECODE_MID_ROWS", 128},
+    {"GEMV_ROWS", 1}, {"GEMV_MAX_T", 2}, {"GEMV_FUSE", 1}, {"DC_RMAX", 128}, {"DC_KS_FORCE", 0}, {"DC_STAGES", 12},
+    {"PF_STAGES", 12}, {"DC_R1", 0}, {"DC_R2", 0}, {"DC_KS2", 1}, {"PF_PAIR", -1}, {"PF_GATHER", 1},
+    {"COMBINE_WARPS", 64}, {"PERM_SMALL_WARPS", 0}, {"ROUTER_WE", 0}, {"ROUTER_TP_MIN_T", kSplitRouterMaxT},
+    {"ROUTER_SPLIT_MAX_T", 16}, {"FUSED_COMBINE", -1}, {"PF_RASTER", -1},
+};
+static int g_opt[OPT_COUNT];
+static bool init_options() {
+    for (int i = 0; i < OPT_COUNT; ++i) {
+        g_opt[i] = kOptDefs[i].dflt;
+        char env[64];
+        std::snprintf(env, sizeof(env), "BM_%s", kOptDefs[i].name);
+        const char *v = std::getenv(env);          // once, at first use of the library
+        if (v && *v) {
+            char *end = nullptr;
+            const long r = std::strtol(v, &end, 10);
+            if (end && *end == '\0') g_opt[i] = (int)r;
+        }
+    }
+    return true;
 }
+static void options_ready() { static const bool done = init_options(); (void)done; }
+int opt(Opt o) { options_ready(); return g_opt[o]; }
 
-// PDL is off while bm_profile_* records (events between launches would time overlapped kernels) and
-// when BM_PDL=0 is set in the environment.
-bool pdl_enabled() {
-    static const int env = tune_int("BM_PDL", 1);
-    return env != 0 && g_prof_kernel == 0;
+// PDL is off while bm_profile_* records (events between launches would time overlapped kernels) and when option
+// "PDL" is 0.
+bool pdl_enabled() { return opt(OPT_PDL) != 0 && g_prof_kernel == 0; }
+
+// ---- per-device facts --------------------------------------------------------------------------------------
+constexpr int kMaxDevices = 64;
+struct DeviceInfo { int state = 0; int sms = 0; int cc_major = 0; };      // state: 0 = not queried, 1 = queried
+static DeviceInfo g_dev[kMaxDevices];
+static std::mutex g_dev_mutex;
+
+static const DeviceInfo *device_info(int *ordinal = nullptr) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return nullptr;
+    if (ordinal) *ordinal = dev;
+    std::lock_guard<std::mutex> lock(g_dev_mutex);
+    DeviceInfo &d = g_dev[dev];
+    if (d.state == 0) {
+        int v = 0, major = 0;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess)
+            return nullptr;
+        d.sms = v > 0 ? v : kNumSMsFallback;
+        d.cc_major = major;
+        d.state = 1;
+    }
+    return &d;
 }
 
 int num_sms() {
-    static int sms = 0;
-    if (sms == 0) {
-        int dev = 0, v = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess &&
-            cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0)
-            sms = v;
-        else
-            sms = kNumSMsFallback;
-    }
-    return sms;
+    const DeviceInfo *d = device_info();
+    return d ? d->sms : kNumSMsFallback;
 }
 
-// 0 = not checked, 1 = sm_100 present, -1 = absent
+// 1 = the current device is sm_100, -1 = it is not (or there is none)
 static int device_ok() {
-    static int state = 0;
-    if (state == 0) {
-        int dev = 0, major = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess &&
-            cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) == cudaSuccess && major == 10)
-            state = 1;
-        else
-            state = -1;
+    const DeviceInfo *d = device_info();
+    return d && d->cc_major == 10 ? 1 : -1;
+}
+
+// dynamic shared memory opt-in, remembered per (device, kernel)
+struct SmemGrant { const void *fn; size_t bytes; };
+static SmemGrant g_smem[kMaxDevices][64];
+cudaError_t ensure_dyn_smem(const void *fn, size_t bytes) {
+    if (bytes <= 48 * 1024) return cudaSuccess;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_dev_mutex);
+    SmemGrant *slot = nullptr;
+    for (SmemGrant &g : g_smem[dev]) {
+        if (g.fn == fn) { slot = &g; break; }
+        if (!g.fn) { slot = &g; break; }
     }
-    return state;
+    if (slot && slot->fn == fn && slot->bytes >= bytes) return cudaSuccess;
+    const cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess && slot) { slot->fn = fn; slot->bytes = bytes; }
+    return e;
 }
 
 static inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -82,8 +133,15 @@ extern "C" {
 
 size_t bm_workspace_bytes(int T_max, int D, int F, int E, int K, int G, int S) {
     (void)E;
-    if (T_max < 0 || D < 1 || F < 1 || K < 1 || G < 1 || S < 0) return 0;
+    if (T_max < 0 || D < 1 || F < 1 || K < 1 || G < 1 || S < 0 || S > BM_MAX_S) return 0;
     return workspace_layout(T_max, D, F, K, G, S).total;
+}
+
+int bm_workspace_init(void *workspace, size_t workspace_bytes, bm_stream_t stream) {
+    if (!workspace) return BM_ERR_NULL;
+    if (device_ok() != 1) return BM_ERR_CUDA;
+    return cudaMemsetAsync(workspace, 0, workspace_bytes, reinterpret_cast<cudaStream_t>(stream)) == cudaSuccess
+               ? BM_OK : BM_ERR_CUDA;
 }
 
 // shared body of bm_route (cold_mask == nullptr) and bm_route_partial
@@ -163,6 +221,11 @@ int bm_expert_histogram(const int32_t *expert_ids, int T, int K, int E, int32_t 
                ? BM_OK : BM_ERR_CUDA;
 }
 
+size_t bm_expert_outputs_workspace_bytes(int T, int D, int F, int E) {
+    if (T < 0 || D < 1 || F < 1 || E < 1 || E > BM_MAX_G) return 0;
+    return workspace_layout(T, D, F, 1, 1, E).front_end;
+}
+
 int bm_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 *W1, const bm_bf16 *W3, const bm_bf16 *W2, int E,
                       int F, bm_bf16 *y, void *workspace, size_t workspace_bytes, bm_stream_t stream) {
     if (T < 0 || D < 8 || D % 8 != 0 || F < 8 || F % 8 != 0 || E < 1 || E > BM_MAX_G) return BM_ERR_SHAPE;
@@ -172,7 +235,7 @@ int bm_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 *W1, const b
     if (!aligned16(x) || !aligned16(W1) || !aligned16(W3) || !aligned16(W2) || !aligned16(y) || !aligned16(workspace))
         return BM_ERR_ALIGN;
     const Workspace w = workspace_layout(T, D, F, 1, 1, E);
-    if (workspace_bytes < w.total) return BM_ERR_WORKSPACE;
+    if (workspace_bytes < w.front_end) return BM_ERR_WORKSPACE;
     if (device_ok() != 1) return BM_ERR_CUDA;
     uint8_t *ws = static_cast<uint8_t *>(workspace);
     return launch_expert_outputs(x, T, D, W1, W3, W2, E, F, y, reinterpret_cast<int32_t *>(ws + w.sched),
@@ -216,6 +279,32 @@ int bm_group_mse(const bm_bf16 *Y, const bm_bf16 *U, int T, int D, const int32_t
                ? BM_OK : BM_ERR_CUDA;
 }
 
+// BM_PATH_AUTO -> the path a batch of these host-side sizes takes
+static int resolve_auto_path(int T, int K, int G) {
+
+    // decode (swap-AB weight streaming) for small batches: always up to 64 tokens; up to BM_DECODE_MID_T = 192
+    // tokens while a group expects at most one 128-row chunk (the weights then stream once); up to
+    // BM_DECODE_MAX_T = 384 tokens while a group expects at most ~24 rows.  Measured decode / prefill path (us):
+    //   D = 2048, F = 1408, E = 60, top-4:  G = 8: T = 128 60 / 70, T = 192 65 / 67, T = 256 70 / 63;
+    //                                       G = 15: T = 128 72 / 80, T = 192 82 / 81, T = 256 95 / 86;
+    //                                       G = 30: T = 192 118 / 122, T = 256 127 / 123;  G = 60: T = 256 185 / 195, T = 320 194 / 206, T = 512 204 / 202
+    //   D = 4096, F = 14336, E = 8, top-2:  G = 4: T = 128 244 / 284, T = 192 283 / 316, T = 256 297 / 299
+    const int max_t = opt(OPT_DECODE_MAX_T);
+    const int mid_t = opt(OPT_DECODE_MID_T);
+    const bool few_rows = (long long)T * K <= (long long)opt(OPT_DECODE_ROWS) * G;
+    const bool one_chunk = (long long)T * K <= (long long)opt(OPT_DECODE_MID_ROWS) * G;
+    int path = (T <= 64 || (T <= mid_t && one_chunk) || (T <= max_t && few_rows)) ? BM_PATH_DECODE : BM_PATH_PREFILL;
+    // matrix-vector streaming for one or two tokens whose sets expect at most ~1 row (single-token decode above
+    // all): the tcgen05 k-block loop has a latency floor that such a step never fills (see bm_gemv.cu).
+    // Measured (D = 2048, F = 1408, E = 60, top-4; matrix-vector / tensor path): T = 1: 29-30 / 36-39 us,
+    // T = 2: 42-44 / 43-45 us, T = 3: 53-55 / 51-53 us, T = 8 at G = 60: 93 / 77 us -- beyond two tokens the
+    // token-major W2 stage re-reads weight rows per (token, source) and the equal unit ranges lose balance.
+    const int gemv_rows = opt(OPT_GEMV_ROWS);
+    const int gemv_max_t = opt(OPT_GEMV_MAX_T);
+    if (T <= gemv_max_t && (long long)T * K <= (long long)gemv_rows * G) path = BM_PATH_GEMV;
+    return path;
+}
+
 static int forward_common(const bm_bf16 *x, int T, int D, const bm_routing *routing, const bm_bf16 *W1,
                           const bm_bf16 *W3, const bm_bf16 *W2, int F, int S, bm_bf16 *out, float *out_f32,
                           void *workspace, size_t workspace_bytes, bm_stream_t stream, int path) {
@@ -238,28 +327,7 @@ static int forward_common(const bm_bf16 *x, int T, int D, const bm_routing *rout
     if (workspace_bytes < w.total) return BM_ERR_WORKSPACE;
     if (device_ok() != 1) return BM_ERR_CUDA;
 
-    if (path == BM_PATH_AUTO) {
-        // decode (swap-AB weight streaming) for small batches: always up to 64 tokens; up to BM_DECODE_MID_T = 192
-        // tokens while a group expects at most one 128-row chunk (the weights then stream once); up to
-        // BM_DECODE_MAX_T = 384 tokens while a group expects at most ~24 rows.  Measured decode / prefill path (us):
-        //   D = 2048, F = 1408, E = 60, top-4:  G = 8: T = 128 60 / 70, T = 192 65 / 67, T = 256 70 / 63;
-        //                                       G = 15: T = 128 72 / 80, T = 192 82 / 81, T = 256 95 / 86;
-        //                                       G = 30: T = 192 118 / 122, T = 256 127 / 123;  G = 60: T = 256 185 / 195, T = 320 194 / 206, T = 512 204 / 202
-        //   D = 4096, F = 14336, E = 8, top-2:  G = 4: T = 128 244 / 284, T = 192 283 / 316, T = 256 297 / 299
-        const int max_t = tune_int("BM_DECODE_MAX_T", BM_DECODE_MAX_T);
-        const int mid_t = tune_int("BM_DECODE_MID_T", 192);
-        const bool few_rows = (long long)T * K <= (long long)tune_int("BM_DECODE_ROWS", 24) * G;
-        const bool one_chunk = (long long)T * K <= (long long)tune_int("BM_DECODE_MID_ROWS", 128) * G;
-        path = (T <= 64 || (T <= mid_t && one_chunk) || (T <= max_t && few_rows)) ? BM_PATH_DECODE : BM_PATH_PREFILL;
-        // matrix-vector streaming for one or two tokens whose sets expect at most ~1 row (single-token decode above
-        // all): the tcgen05 k-block loop has a latency floor that such a step never fills (see bm_gemv.cu).
-        // Measured (D = 2048, F = 1408, E = 60, top-4; matrix-vector / tensor path): T = 1: 29-30 / 36-39 us,
-        // T = 2: 42-44 / 43-45 us, T = 3: 53-55 / 51-53 us, T = 8 at G = 60: 93 / 77 us -- beyond two tokens the
-        // token-major W2 stage re-reads weight rows per (token, source) and the equal unit ranges lose balance.
-        const int gemv_rows = tune_int("BM_GEMV_ROWS", 1);
-        const int gemv_max_t = tune_int("BM_GEMV_MAX_T", 2);
-        if (T <= gemv_max_t && (long long)T * K <= (long long)gemv_rows * G) path = BM_PATH_GEMV;
-    }
+    if (path == BM_PATH_AUTO) path = resolve_auto_path(T, K, G);
 
     uint8_t *ws = static_cast<uint8_t *>(workspace);
     ForwardArgs a{};
@@ -270,7 +338,9 @@ static int forward_common(const bm_bf16 *x, int T, int D, const bm_routing *rout
     a.sched = reinterpret_cast<int32_t *>(ws + w.sched);
     a.xs = reinterpret_cast<bm_bf16 *>(ws + w.xs);
     a.h = reinterpret_cast<bm_bf16 *>(ws + w.h);
-    a.out_acc = reinterpret_cast<float *>(ws + w.out_acc);
+    const size_t zbase = zero_region_base(workspace_bytes, w);
+    a.out_acc = reinterpret_cast<float *>(ws + zbase + w.z_acc);
+    a.tickets = reinterpret_cast<int32_t *>(ws + zbase + w.z_tickets);
     a.y = reinterpret_cast<bm_bf16 *>(ws + w.y);
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     cudaError_t e;
@@ -345,14 +415,16 @@ int bm_device_status(void *workspace, int32_t *host_out, bm_stream_t stream) {
 
 int bm_profile_enable(int kernel, int max_records) {
     for (int i = 0; i < g_prof_max; ++i) { cudaEventDestroy(g_prof_start[i]); cudaEventDestroy(g_prof_stop[i]); }
-    delete[] g_prof_start; delete[] g_prof_stop;
+    delete[] g_prof_start; delete[] g_prof_stop; delete[] g_prof_kind;
     g_prof_start = g_prof_stop = nullptr;
+    g_prof_kind = nullptr;
     g_prof_kernel = 0; g_prof_max = 0; g_prof_n = 0;
     if (kernel == BM_KERNEL_NONE || max_records <= 0) return BM_OK;
-    if (kernel < BM_KERNEL_ROUTER || kernel > BM_KERNEL_FINALIZE) return BM_ERR_SHAPE;
+    if (kernel < BM_KERNEL_ROUTER || kernel > BM_KERNEL_ALL) return BM_ERR_SHAPE;
     if (device_ok() != 1) return BM_ERR_CUDA;
     g_prof_start = new cudaEvent_t[max_records];
     g_prof_stop = new cudaEvent_t[max_records];
+    g_prof_kind = new int[max_records];
     for (int i = 0; i < max_records; ++i)
         if (cudaEventCreate(&g_prof_start[i]) != cudaSuccess || cudaEventCreate(&g_prof_stop[i]) != cudaSuccess)
             return BM_ERR_CUDA;
@@ -360,20 +432,57 @@ int bm_profile_enable(int kernel, int max_records) {
     return BM_OK;
 }
 
-int bm_profile_read(float *total_ms, int *n_records) {
-    if (!total_ms || !n_records) return BM_ERR_NULL;
-    float sum = 0.f;
+int bm_profile_read_kinds(float *ms_by_kind, int *n_by_kind) {
+    if (!ms_by_kind || !n_by_kind) return BM_ERR_NULL;
+    for (int k = 0; k < BM_KERNEL_ALL; ++k) { ms_by_kind[k] = 0.f; n_by_kind[k] = 0; }
     for (int i = 0; i < g_prof_n; ++i) {
         float ms = 0.f;
         if (cudaEventSynchronize(g_prof_stop[i]) != cudaSuccess ||
             cudaEventElapsedTime(&ms, g_prof_start[i], g_prof_stop[i]) != cudaSuccess)
             return BM_ERR_CUDA;
-        sum += ms;
+        const int k = g_prof_kind[i];
+        if (k > 0 && k < BM_KERNEL_ALL) { ms_by_kind[k] += ms; n_by_kind[k] += 1; }
     }
-    *total_ms = sum;
-    *n_records = g_prof_n;
     g_prof_n = 0;
     return BM_OK;
+}
+
+int bm_profile_read(float *total_ms, int *n_records) {
+    if (!total_ms || !n_records) return BM_ERR_NULL;
+    float ms[BM_KERNEL_ALL];
+    int n[BM_KERNEL_ALL];
+    const int rc = bm_profile_read_kinds(ms, n);
+    if (rc != BM_OK) return rc;
+    *total_ms = 0.f; *n_records = 0;
+    for (int k = 1; k < BM_KERNEL_ALL; ++k) { *total_ms += ms[k]; *n_records += n[k]; }
+    return BM_OK;
+}
+
+int bm_forward_info(int T, int K, int G, int S, int D, int F, int *path, int *deterministic) {
+    if (T < 0 || K < 1 || K > BM_MAX_K || G < 1 || G > BM_MAX_G || S < 0 || S > BM_MAX_S || D < 8 || F < 8) return BM_ERR_SHAPE;
+    const int pth = resolve_auto_path(T, K, G);
+    int det = 1;
+    if (pth == BM_PATH_PREFILL) det = (opt(OPT_FUSED_COMBINE) == 0 || K + S <= 2) ? 1 : 0;
+    else if (pth == BM_PATH_DECODE) det = ((K + S) * decode_ksplit(T, D, F, K, G, S) <= 2) ? 1 : 0;
+    if (path) *path = pth;
+    if (deterministic) *deterministic = det;
+    return BM_OK;
+}
+
+int bm_set_option(const char *name, int value) {
+    if (!name) return BM_ERR_NULL;
+    options_ready();
+    for (int i = 0; i < OPT_COUNT; ++i)
+        if (std::strcmp(name, kOptDefs[i].name) == 0) { g_opt[i] = value; return BM_OK; }
+    return BM_ERR_SHAPE;
+}
+
+int bm_get_option(const char *name, int *value) {
+    if (!name || !value) return BM_ERR_NULL;
+    options_ready();
+    for (int i = 0; i < OPT_COUNT; ++i)
+        if (std::strcmp(name, kOptDefs[i].name) == 0) { *value = g_opt[i]; return BM_OK; }
+    return BM_ERR_SHAPE;
 }
 
 long long bm_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }

@@ -287,12 +287,7 @@ cudaError_t launch_gram(const bm_bf16 *Y, int E, size_t n, float *gram, float *c
     const long long nkb = (long long)((n + 63) / 64);
     const int grid = (int)(nkb < num_sms() ? nkb : num_sms());
     const size_t smem = 1024 + (size_t)kGramStages * kGramTile + 256;
-    static bool attr = false;
-    if (!attr) {
-        cudaError_t e = cudaFuncSetAttribute(gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr = true;
-    }
+    if (cudaError_t ea = ensure_dyn_smem(reinterpret_cast<const void *>(gram_kernel), smem); ea != cudaSuccess) return ea;
     gram_kernel<<<grid, kGramThreads, smem, stream>>>(tm, E, (int)nkb, partial);
     gram_finish_kernel<<<E, 128, 0, stream>>>(partial, grid, E, gram, cosine);
     count_launch(2);

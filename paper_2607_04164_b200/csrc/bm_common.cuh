@@ -19,28 +19,36 @@ constexpr int kPermSmallItems = 2048;      // up to this many items one CTA does
 constexpr int kMaxSchedTiles = 1 << 20;
 
 struct Workspace {
-    // byte offsets from the workspace base
+    // byte offsets from the workspace base ("front": scratch that every call writes before it reads)
     size_t status;       // int32[1024]: [0] device status bits, [1] A (copy of offsets[G]), [2] tokens routed (split
                          // router), [64..64+512) expert slices done per token (split router); zeroed once by the caller,
                          // the counters are put back to zero by the kernel that used them
     size_t block_hist;   // int32[nb * G]   per-block group histograms / bases of the permutation
     size_t route_logits; // f32[min(T, 512) * BM_MAX_E]  logits of the split router (T < 512), gathered by a token's last CTA
     size_t sched;        // int32[kSchedInts] tile-schedule scratch of the forward pass
-    size_t xs;           // bf16[T*K, D]    token rows gathered in permuted order (prefill path)
+    size_t xs;           // bf16[T*K, D]    token rows gathered in permuted order (CTA-pair prefill and decode kernels)
     size_t h;            // bf16[T*K + S*T, F]  SwiGLU intermediate
-    size_t out_acc;      // f32[T, D]       fp32 accumulation of the combine (decode path: split-K partials)
-    size_t y;            // bf16[T*K + S*T, D]  per-row expert outputs (prefill path), combined by combine_kernel
-    size_t total;
+    size_t y;            // bf16[T*K + S*T, D]  per-row expert outputs (two-pass combine only: option FUSED_COMBINE = 0, GEMV fallback)
+    size_t front_end;
+    // "zero region": anchored at the END of the caller's buffer (see zero_region_base), all-zero between calls -- the
+    // kernels that use it put every word back to zero (fused combine: the last arriver of an output piece rounds it,
+    // stores it and clears accumulator and ticket).  Offsets are relative to the region's start.
+    size_t z_acc;        // f32[T, D]       fp32 accumulation of the gate-weighted combine (GEMM2 epilogues add into it)
+    size_t z_tickets;    // int32[T * ceil(D/32) * 4]  arrivals per (token, output piece)
+    size_t z_total;
+    size_t total;        // front_end + z_total (+ alignment slack)
 };
 
 constexpr int kStatusInts = 1024;                               // the zero-once head of the workspace (4096 bytes)
 constexpr int kSplitRouterMaxT = 512;                           // the split (latency) router serves T < 512
 constexpr int kStatusTokCnt = 64;                               // status[64 + t]: expert slices of token t done
 constexpr int kStatusDone = 2;                                  // status[2]: tokens routed
-constexpr int kMaxShared = 16;                                  // S <= 16 always-on shared experts
+constexpr int kMaxShared = BM_MAX_S;                            // S <= 16 always-on shared experts
 constexpr int kSchedInts = 4 + 5 * (BM_MAX_G + kMaxShared) + 8;
 
 __host__ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+__host__ inline size_t ticket_ints(int T, int D) { return (size_t)T * (size_t)((D + 31) / 32) * 4; }
 
 __host__ inline Workspace workspace_layout(int T, int D, int F, int K, int G, int S) {
     Workspace w{};
@@ -53,29 +61,54 @@ __host__ inline Workspace workspace_layout(int T, int D, int F, int K, int G, in
     w.sched = off;       off = align_up(off + kSchedInts * sizeof(int32_t), 1024);
     w.xs = off;          off = align_up(off + items * D * sizeof(bm_bf16), 1024);
     w.h = off;           off = align_up(off + (items + (size_t)S * T) * F * sizeof(bm_bf16), 1024);
-    w.out_acc = off;     off = align_up(off + (size_t)T * D * sizeof(float), 1024);
     w.y = off;           off = align_up(off + (items + (size_t)S * T) * D * sizeof(bm_bf16), 1024);
-    w.total = off;
+    w.front_end = off;
+    size_t z = 0;
+    w.z_acc = z;         z = align_up(z + (size_t)T * D * sizeof(float), 1024);
+    w.z_tickets = z;     z = align_up(z + ticket_ints(T, D) * sizeof(int32_t), 1024);
+    w.z_total = z;
+    w.total = w.front_end + w.z_total + 1024;
     return w;
+}
+
+// Start of the zero region inside a caller buffer of `workspace_bytes` bytes: anchored at the buffer's end, so that
+// the regions of calls with different T (<= T_max) all lie inside [end - z_total(T_max), end), which the front
+// sections of no call reach (front_end(T) <= front_end(T_max) <= end - z_total(T_max) - slack).
+__host__ inline size_t zero_region_base(size_t workspace_bytes, const Workspace &w) {
+    return (workspace_bytes - w.z_total) & ~(size_t)1023;
 }
 
 // ---------------------------------------------------------------------------------------------
 // Launch bookkeeping (host)
 // ---------------------------------------------------------------------------------------------
 void count_launch(int n = 1);
+// SM count / compute capability of the CURRENT device (cudaGetDevice), cached per device ordinal, so one process
+// can drive several GPUs.
 int num_sms();
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is per device: raises the opt-in of `fn` on the current device
+// to at least `bytes` (no-op below 48 KB or when already granted there).
+cudaError_t ensure_dyn_smem(const void *fn, size_t bytes);
 // bm_profile_*: record an event pair around the launches of one kernel kind (no-ops unless enabled)
 void profile_begin(int kernel, cudaStream_t stream);
 void profile_end(int kernel, cudaStream_t stream);
 
 // Programmatic dependent launch (PDL).  Every kernel of the path is launched with
-// cudaLaunchAttributeProgrammaticStreamSerialization (unless bm_profile_* is recording or BM_PDL=0), so
+// cudaLaunchAttributeProgrammaticStreamSerialization (unless bm_profile_* is recording or option "PDL" is 0), so
 // its prologue overlaps the tail of its predecessor.  Contract for every kernel launched this way:
 // all threads call grid_dep_wait() before touching anything a predecessor wrote (or will overwrite)
 // and before exiting -- it returns once ALL prerequisite grids have completed and flushed, so the chain
 // of launches stays transitively ordered -- and grid_dep_launch() only AFTER that wait.
 bool pdl_enabled();
-int tune_int(const char *env_name, int dflt);      // integer tuning override from the environment
+
+// Tuning / test switches (include/bm.h: bm_set_option).  A plain int table: initialised once from the environment
+// (BM_<NAME>) when the library is first used, changed only through bm_set_option -- no getenv on the call path.
+enum Opt {
+    OPT_PDL, OPT_DECODE_MAX_T, OPT_DECODE_MID_T, OPT_DECODE_ROWS, OPT_DECODE_MID_ROWS, OPT_GEMV_ROWS, OPT_GEMV_MAX_T,
+    OPT_GEMV_FUSE, OPT_DC_RMAX, OPT_DC_KS_FORCE, OPT_DC_STAGES, OPT_PF_STAGES, OPT_DC_R1, OPT_DC_R2, OPT_DC_KS2,
+    OPT_PF_PAIR, OPT_PF_GATHER, OPT_COMBINE_WARPS, OPT_PERM_SMALL_WARPS, OPT_ROUTER_WE, OPT_ROUTER_TP_MIN_T,
+    OPT_ROUTER_SPLIT_MAX_T, OPT_FUSED_COMBINE, OPT_PF_RASTER, OPT_COUNT
+};
+int opt(Opt o);
 
 template <typename... KArgs, typename... Args>
 cudaError_t launch_kernel(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream,
@@ -121,7 +154,8 @@ struct ForwardArgs {
     int32_t *sched;
     bm_bf16 *xs;
     bm_bf16 *h;
-    float *out_acc;
+    float *out_acc;      // zero region: fp32 accumulator of the fused combine
+    int32_t *tickets;    // zero region: arrival counters of the fused combine
     bm_bf16 *y;
     float *out_f32;      // non-null: leave the fp32 sums here instead of writing bf16 `out` (tensor-parallel partial)
 };
@@ -146,6 +180,7 @@ cudaError_t launch_round_bf16(const float *in, size_t n, bm_bf16 *out, cudaStrea
 cudaError_t launch_forward_simt(const ForwardArgs &a, cudaStream_t stream);
 cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t stream);
 cudaError_t launch_forward_gemv(const ForwardArgs &a, cudaStream_t stream);
+int decode_ksplit(int T, int D, int F, int K, int G, int S);     // K splits the decode GEMM2 would use
 cudaError_t launch_combine(const ForwardArgs &a, cudaStream_t stream);
 
 // ---------------------------------------------------------------------------------------------

@@ -22,6 +22,7 @@
 // atomics, deterministic.  Decode: rows also live in different K-splits and there are few of them, so the
 // partials are added in fp32 with red.global.add into `out_acc` and a last pass rounds to bf16.
 #include <algorithm>
+#include <mutex>
 
 #include "bm_common.cuh"
 #include "bm_ptx.cuh"
@@ -90,10 +91,14 @@ struct GemmParams {
     const int32_t *counts, *offsets, *row_token, *row_slot;
     const bm_bf16 *x;   // GA: token rows gathered straight from x [T, D]
     const float *gate_w;
+    const int32_t *n_slots;
     const int32_t *sched;
     bm_bf16 *h;
-    float *out_acc;
-    bm_bf16 *y;
+    float *out_acc;     // zero region: fp32 accumulator of the fused combine [T, D]
+    int32_t *tickets;   // zero region: arrivals per (token, output piece)
+    bm_bf16 *y;         // two-pass combine: per-row expert outputs
+    bm_bf16 *out;       // fused combine: the layer output [T, D] bf16 ...
+    float *out_f32;     // ... or, when non-null, the fp32 sums (tensor-parallel partial)
 };
 
 struct Item {
@@ -155,7 +160,16 @@ __device__ __forceinline__ float silu_mul(float a, float b) {
     return __fdividef(a, 1.0f + __expf(-a)) * b;
 }
 
-template <int MODE, bool K2 = false, bool GA = false>
+// Fused combine (FC, GEMM2 only; north_star kernel (4)): the epilogue multiplies its rows by their gate weights and adds
+// them into the fp32 accumulator out_acc [T, D] with vector reductions at L2 (red.global.add.v4.f32), then takes a
+// ticket per (token, output piece).  The arrival that completes a piece -- all n_slots[t] + S source rows of the
+// token (times the K splits on the decode path) have been added -- reads the sums back, rounds them to bf16 into
+// `out` (or stores them as fp32 into out_f32) and puts accumulator and ticket back to zero, so neither a zeroing
+// pass, nor y rows, nor a combine / finalize kernel exist.  fp32 addition is commutative, so with at most two
+// sources per token (K + S <= 2, e.g. Mixtral's top-2) the result is bit-deterministic; with more sources the
+// association follows the arrival order (last-bit differences before the bf16 rounding).  Writers fence between
+// their reductions and the ticket, the finisher fences between the ticket and its reads (threadFenceReduction).
+template <int MODE, bool K2 = false, bool GA = false, bool FC = false>
 __global__ void __launch_bounds__(kThreads + (GA ? kGatherThreads : 0), 1)
 gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D]; GEMM2: H [TK+S*T, F]
             const __grid_constant__ CUtensorMap tm_act1,   // GEMM1: x [T, D] (shared experts); GEMM2: unused
@@ -166,6 +180,8 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
     constexpr bool kGemm1 = (MODE == PF_GEMM1 || MODE == DC_GEMM1);
     static_assert(!K2 || !kDecode, "CTA pairs are a prefill-tile feature");
     static_assert(!GA || MODE == PF_GEMM1, "the in-kernel gather feeds GEMM1's activation tile");
+    static_assert(!FC || MODE == PF_GEMM2 || MODE == DC_GEMM2, "the fused combine is GEMM2's epilogue");
+    static_assert(MODE != DC_GEMM2 || FC, "the decode GEMM2 always finishes its output itself");
     // K2: the two CTAs of a cluster form a CTA pair; rank 0 (the leader) issues the M = 256 MMAs for both
     const uint32_t rank = K2 ? ptx::cluster_ctarank() : 0u;
     const bool leader = rank == 0;
@@ -451,9 +467,45 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
         uint32_t acc_phase = 0;
         Item it;
         for (int item = item0; get_item<MODE, K2>(p, sv, item, it, rank); item += item_stride) {
+            // FC: token, gate weight and source count of this thread's rows are fetched BEFORE the wait for the
+            // accumulator (two dependent global loads hidden behind the item's main loop).
+            // PF_GEMM2: row `row` of the chunk (index 0); DC_GEMM2: chunk rows lane, lane + 32, ... (the columns).
+            int tokr[4] = {-1, -1, -1, -1};
+            float gwr[4] = {0.f, 0.f, 0.f, 0.f};
+            int nsrcr[4] = {0, 0, 0, 0};
+            if (FC) {
+#pragma unroll
+                for (int j = 0; j < (MODE == DC_GEMM2 ? 4 : 1); ++j) {
+                    const int r = MODE == DC_GEMM2 ? j * 32 + lane : row;
+                    if (r < it.n) {
+                        int tok, slot = 0;
+                        if (it.shared) {
+                            tok = it.tok0 + r;
+                        } else {
+                            tok = p.row_token[it.perm_row0 + r];
+                            slot = p.row_slot[it.perm_row0 + r];
+                        }
+                        if (tok >= 0 && tok < p.T && slot >= 0 && slot < p.K) {
+                            tokr[j] = tok;
+                            gwr[j] = it.shared ? 1.0f : p.gate_w[(size_t)tok * p.K + slot];
+                            if (MODE == PF_GEMM2) nsrcr[j] = min(max(p.n_slots[tok], 0), p.K) + p.S;
+                        }
+                    }
+                }
+            }
             ptx::mbar_wait(&tfull[acc], acc_phase);
             ptx::tc_fence_after();
             const uint32_t t_addr = tmem_base + acc * kAccCols + ((uint32_t)(q * 32) << 16);
+            bool released = false;
+            auto release_acc = [&]() {              // hand the accumulator stage back to the MMA issuer
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) {
+                    if (K2) ptx::mbar_arrive_cluster(ptx::mapa_u32(&tempty[acc], 0));      // the leader's barrier
+                    else ptx::mbar_arrive(&tempty[acc]);
+                }
+                released = true;
+            };
 
             if (MODE == PF_GEMM1) {
                 // row = token row of the chunk; columns [0,128) = W1 products, [128,256) = W3 products
@@ -474,6 +526,93 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
                     if (row_ok) {
                         if (f0 + c + 8 <= p.F) *reinterpret_cast<uint4 *>(hrow + c) = make_uint4(o[0], o[1], o[2], o[3]);
                         if (f0 + c + 16 <= p.F) *reinterpret_cast<uint4 *>(hrow + c + 8) = make_uint4(o[4], o[5], o[6], o[7]);
+                    }
+                }
+            } else if (MODE == PF_GEMM2 && FC) {
+                // row = token row of the chunk; columns = 256 output features d0..d0+255 of y_r = H_r . W2[u]^T.
+                // gw * y_r is added into out_acc[tok, d0..]: 32 columns at a time the accumulator leaves TMEM with one
+                // row per lane, is scaled, transposed through the warp's shared-memory stage (32 rows x 32 fp32,
+                // 16-byte units xor-swizzled by the row) and goes out as red.global.add.v4.f32, every instruction
+                // 4 rows x 128 contiguous bytes (whole sectors) -- the "coalesced 128-bit" scatter of north_star (4).
+                const int d0 = it.wt * 256;
+                const int n_dt = (p.D + 255) >> 8;
+                float4 *stg = reinterpret_cast<float4 *>(epi_stage + (size_t)q * kEpiStageBytes);
+                const int rl = lane >> 3, ul = lane & 7;        // read phase: row (mod 4) and 16-byte unit of this lane
+                float *rptr[8];                                 // accumulator row of chunk row 4j + rl (nullptr: no row)
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const int tk = __shfl_sync(kFullMask, tokr[0], 4 * j + rl);
+                    rptr[j] = tk >= 0 ? p.out_acc + (size_t)tk * p.D + d0 + 4 * ul : nullptr;
+                }
+                const float gw = gwr[0];
+#pragma unroll 1
+                for (int c = 0; c < 256; c += 32) {
+                    if (d0 + c >= p.D) break;                   // ragged last tile: whole 32-column steps past D
+                    uint32_t v[32];
+                    ptx::tmem_ld_x32(t_addr + c, v);
+                    ptx::tmem_ld_wait();
+#pragma unroll
+                    for (int u = 0; u < 8; ++u)
+                        stg[lane * 8 + (u ^ (lane & 7))] =
+                            make_float4(gw * __uint_as_float(v[4 * u]), gw * __uint_as_float(v[4 * u + 1]),
+                                        gw * __uint_as_float(v[4 * u + 2]), gw * __uint_as_float(v[4 * u + 3]));
+                    __syncwarp();
+                    if (d0 + c + 4 * ul + 4 <= p.D) {
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) {
+                            const int r = 4 * j + rl;
+                            if (rptr[j]) {
+                                const float4 x = stg[r * 8 + (ul ^ (r & 7))];
+                                ptx::red_add_v4_f32(rptr[j] + c, x.x, x.y, x.z, x.w);
+                            }
+                        }
+                    }
+                    __syncwarp();
+                }
+                release_acc();                                  // the MMA of the item after next may start
+                // tickets: one arrival per (token, 256-column piece) and source row
+                __threadfence();
+                __syncwarp();
+                bool done = false;
+                if (tokr[0] >= 0)
+                    done = atomicAdd(p.tickets + (size_t)tokr[0] * n_dt + it.wt, 1) == nsrcr[0] - 1;
+                unsigned dm = __ballot_sync(kFullMask, done);
+                if (dm) __threadfence();
+                // completed pieces (this row was the token's last source): lane l owns columns d0 + 8l .. + 7 of every
+                // one; four pieces per round so that their eight loads per lane are in flight together
+                const int d = d0 + lane * 8;
+                const bool d_in = d + 8 <= p.D;
+                while (dm) {
+                    int tk[4];
+                    float4 a[4], b[4];
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const int r = dm ? __ffs(dm) - 1 : -1;
+                        if (dm) dm &= dm - 1;
+                        tk[i] = r >= 0 ? __shfl_sync(kFullMask, tokr[0], r) : -1;       // (r is warp-uniform)
+                        if (tk[i] >= 0 && d_in) {
+                            const float4 *src = reinterpret_cast<const float4 *>(p.out_acc + (size_t)tk[i] * p.D + d);
+                            a[i] = __ldcg(src);
+                            b[i] = __ldcg(src + 1);
+                        }
+                    }
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        if (tk[i] < 0) continue;
+                        if (d_in) {
+                            float4 *src = reinterpret_cast<float4 *>(p.out_acc + (size_t)tk[i] * p.D + d);
+                            if (p.out_f32) {
+                                float4 *o = reinterpret_cast<float4 *>(p.out_f32 + (size_t)tk[i] * p.D + d);
+                                o[0] = a[i]; o[1] = b[i];
+                            } else {
+                                *reinterpret_cast<uint4 *>(p.out + (size_t)tk[i] * p.D + d) =
+                                    make_uint4(pack_bf16x2(a[i].x, a[i].y), pack_bf16x2(a[i].z, a[i].w),
+                                               pack_bf16x2(b[i].x, b[i].y), pack_bf16x2(b[i].z, b[i].w));
+                            }
+                            src[0] = make_float4(0.f, 0.f, 0.f, 0.f);
+                            src[1] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        }
+                        if (lane == 0) p.tickets[(size_t)tk[i] * n_dt + it.wt] = 0;
                     }
                 }
             } else if (MODE == PF_GEMM2) {
@@ -541,26 +680,10 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
                 }
             } else {
                 // DC_GEMM2: row = output feature d; columns = token rows of the chunk; partial over this K split.
-                // Lane l first fetches token and gate weight of chunk rows l, l+32, ... (one dependent-load chain
-                // per item instead of one per token); the loop broadcasts them with shuffles.
+                // Token and gate weight of chunk rows lane, lane + 32, ... were fetched above (one dependent-load
+                // chain per item instead of one per token); the loop broadcasts them with shuffles.
                 const int d = it.wt * p.R + row;
                 const bool d_ok = row < p.R && d < p.D;
-                int tokr[4];
-                float gwr[4];
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int r = j * 32 + lane;
-                    tokr[j] = -1;
-                    gwr[j] = 1.0f;
-                    if (r < it.n) {
-                        if (it.shared) {
-                            tokr[j] = it.tok0 + r;
-                        } else {
-                            tokr[j] = p.row_token[it.perm_row0 + r];
-                            gwr[j] = p.gate_w[(size_t)tokr[j] * p.K + p.row_slot[it.perm_row0 + r]];
-                        }
-                    }
-                }
                 float *ocol = p.out_acc + d;
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
@@ -583,14 +706,39 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
                         }
                     }
                 }
+                release_acc();
+                // tickets: piece = (weight tile, 32-row quarter q) over ALL tokens (a decode batch is small); every item
+                // (chunk of any segment, K split) on this weight tile arrives once, total_chunks * ksplit in all.  The
+                // warp that completes a piece finishes it for every token: lane = output feature, 16 tokens per round.
+                // Quarters without a valid output row take no tickets.
+                if (q * 32 < p.R && it.wt * p.R + q * 32 < p.D) {      // warp-uniform
+                    __threadfence();
+                    __syncwarp();
+                    int last = 0;
+                    if (lane == 0) last = atomicAdd(p.tickets + it.wt * 4 + q, 1) == sv.total_chunks * p.ksplit - 1;
+                    last = __shfl_sync(kFullMask, last, 0);
+                    if (last) {
+                        __threadfence();
+                        for (int t0 = 0; t0 < p.T; t0 += 16) {
+                            float v[16];
+#pragma unroll
+                            for (int i = 0; i < 16; ++i)
+                                v[i] = (d_ok && t0 + i < p.T) ? __ldcg(p.out_acc + (size_t)(t0 + i) * p.D + d) : 0.0f;
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) {
+                                if (d_ok && t0 + i < p.T) {
+                                    const size_t o = (size_t)(t0 + i) * p.D + d;
+                                    if (p.out_f32) p.out_f32[o] = v[i];
+                                    else p.out[o] = (bm_bf16)f32_to_bf16_bits(v[i]);
+                                    p.out_acc[o] = 0.0f;
+                                }
+                            }
+                        }
+                        if (lane == 0) p.tickets[it.wt * 4 + q] = 0;
+                    }
+                }
             }
-            // release the accumulator stage
-            ptx::tc_fence_before();
-            __syncwarp();
-            if (lane == 0) {
-                if (K2) ptx::mbar_arrive_cluster(ptx::mapa_u32(&tempty[acc], 0));      // the leader's barrier
-                else ptx::mbar_arrive(&tempty[acc]);
-            }
+            if (!released) release_acc();
             if (++acc == kAccStages) { acc = 0; acc_phase ^= 1; }
         }
     }
@@ -605,13 +753,13 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
 }
 
 // -------------------------------------------------------------------------------------------------
-// prep: build the schedule, zero the fp32 accumulator, gather token rows into permuted order (step 9)
+// prep: build the schedule, gather token rows into permuted order (step 9)
 // -------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
 prep_kernel(const bm_bf16 *__restrict__ x, int T, int D, int K, int G, int S,
             const int32_t *__restrict__ counts, const int32_t *__restrict__ offsets,
             const int32_t *__restrict__ row_token, int32_t *__restrict__ sched, bm_bf16 *__restrict__ xs,
-            float *__restrict__ out_acc, int decode, int32_t *__restrict__ status) {
+            int32_t *__restrict__ status) {
     grid_dep_wait();
     grid_dep_launch();
     if (blockIdx.x == 0) {
@@ -669,11 +817,6 @@ prep_kernel(const bm_bf16 *__restrict__ x, int T, int D, int K, int G, int S,
             }
         }
     }
-    // zero out_acc (decode path only: the prefill path combines plain y rows)
-    const size_t n4 = decode ? (size_t)T * D / 4 : 0;
-    float4 *o4 = reinterpret_cast<float4 *>(out_acc);
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x)
-        o4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     // gather: one warp per permuted row.  (A tile::gather4 producer in GEMM1 was measured instead of this
     // pass: ~12 cycles per 128-byte row made GEMM1 3x slower, so the rows are materialised once here.)
     if (!xs) return;                     // prefill tiles: GEMM1 gathers the rows itself (GA)
@@ -833,30 +976,53 @@ EncodeTiledFn get_encode() {
     return fn;
 }
 
-// [rows, cols] bf16 row-major, box = box_rows x 64 columns, 128B swizzle
-bool make_map_2d(CUtensorMap *m, const void *base, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+// Tensor maps depend only on (base pointer, shape, box, swizzle), and a serving loop calls the layer with the same
+// buffers over and over, so encoded maps are kept in a small direct-mapped cache instead of being re-encoded on the
+// host in every call (eight cuTensorMapEncodeTiled calls were ~5 us of host time per layer call).  An entry is never
+// stale: its content is a pure function of its key.
+struct MapKey {
+    const void *base;
+    uint64_t d0, d1, d2;        // cols, rows, sets (d2 = 0: 2-D)
+    uint32_t box_cols, box_rows, swizzle;
+    bool operator==(const MapKey &o) const {
+        return base == o.base && d0 == o.d0 && d1 == o.d1 && d2 == o.d2 && box_cols == o.box_cols &&
+               box_rows == o.box_rows && swizzle == o.swizzle;
+    }
+};
+struct MapEntry { MapKey key; CUtensorMap map; bool valid; };
+constexpr int kMapCacheSize = 256;
+MapEntry g_map_cache[kMapCacheSize];
+std::mutex g_map_mutex;
+
+bool encode_map(CUtensorMap *m, const MapKey &k) {
+    uint64_t h = reinterpret_cast<uintptr_t>(k.base) * 0x9E3779B97F4A7C15ull;
+    h ^= (k.d0 * 31 + k.d1) * 0xC2B2AE3D27D4EB4Full + k.d2 * 0x165667B19E3779F9ull + k.box_cols * 131 + k.box_rows * 7 + k.swizzle;
+    MapEntry &e = g_map_cache[(h >> 24) % kMapCacheSize];
+    std::lock_guard<std::mutex> lock(g_map_mutex);
+    if (e.valid && e.key == k) { *m = e.map; return true; }
     EncodeTiledFn enc = get_encode();
     if (!enc) return false;
-    cuuint64_t dims[2] = {cols, rows};
-    cuuint64_t strides[1] = {cols * sizeof(bm_bf16)};
-    cuuint32_t box[2] = {kBlockK, box_rows};
-    cuuint32_t es[2] = {1, 1};
-    return enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base), dims, strides, box, es,
-               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+    const int rank = k.d2 ? 3 : 2;
+    cuuint64_t dims[3] = {k.d0, k.d1, k.d2};
+    cuuint64_t strides[2] = {k.d0 * sizeof(bm_bf16), k.d1 * k.d0 * sizeof(bm_bf16)};
+    cuuint32_t box[3] = {k.box_cols, k.box_rows, 1};
+    cuuint32_t es[3] = {1, 1, 1};
+    if (enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, rank, const_cast<void *>(k.base), dims, strides, box, es,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, k.swizzle ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+            CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return false;
+    e.key = k; e.map = *m; e.valid = true;
+    return true;
+}
+
+// [rows, cols] bf16 row-major, box = box_rows x 64 columns, 128B swizzle
+bool make_map_2d(CUtensorMap *m, const void *base, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+    return encode_map(m, MapKey{base, cols, rows, 0, kBlockK, box_rows, 1});
 }
 
 // [n, rows, cols] bf16, box = 1 x box_rows x 64
 bool make_map_3d(CUtensorMap *m, const void *base, uint64_t n, uint64_t rows, uint64_t cols, uint32_t box_rows) {
-    EncodeTiledFn enc = get_encode();
-    if (!enc) return false;
-    cuuint64_t dims[3] = {cols, rows, n};
-    cuuint64_t strides[2] = {cols * sizeof(bm_bf16), rows * cols * sizeof(bm_bf16)};
-    cuuint32_t box[3] = {kBlockK, box_rows, 1};
-    cuuint32_t es[3] = {1, 1, 1};
-    return enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void *>(base), dims, strides, box, es,
-               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+    return encode_map(m, MapKey{base, cols, rows, n, kBlockK, box_rows, 1});
 }
 
 // Decode tiling: rows-per-tile R in [32,128] and the K-split count, chosen with a small time model of the
@@ -892,9 +1058,9 @@ void choose_decode_tiling(int wrows, int kblocks, int n_seg, bool allow_split, i
     double best = 1e30;
     int bestR = 128, bestKs = 1;
     const int max_ks = allow_split ? 16 : 1;
-    int rmax = tune_int("BM_DC_RMAX", 128);
+    int rmax = opt(OPT_DC_RMAX);
     rmax = rmax < 32 ? 32 : (rmax > 128 ? 128 : rmax);
-    const int ks_force = allow_split ? tune_int("BM_DC_KS_FORCE", 0) : 0;
+    const int ks_force = allow_split ? opt(OPT_DC_KS_FORCE) : 0;
     for (int ks = 1; ks <= max_ks; ++ks) {
         if (ks > 1 && (kblocks % ks != 0 || kblocks / ks < 4)) continue;
         if (ks_force > 0 && ks != ks_force && kblocks % ks_force == 0 && kblocks / ks_force >= 4) continue;
@@ -933,24 +1099,19 @@ void ring_geometry(bool decode, bool gemm1, int T, GemmParams *p, bool pair = fa
     }
     const size_t fixed = (decode ? 0 : kSmemEpi) + sched_smem_bytes(p->seg_cap) + (size_t)p->tail_pad;
     int st = (int)((kSmemRing - fixed) / (size_t)p->stage_bytes);
-    const int cap = tune_int(decode ? "BM_DC_STAGES" : "BM_PF_STAGES", kMaxStages);
+    const int cap = opt(decode ? OPT_DC_STAGES : OPT_PF_STAGES);
     if (st > cap) st = cap;
     if (st > kMaxStages) st = kMaxStages;
     if (st < 2) st = 2;
     p->stages = st;
 }
 
-template <int MODE, bool K2 = false, bool GA = false>
+template <int MODE, bool K2 = false, bool GA = false, bool FC = false>
 cudaError_t launch_gemm(const CUtensorMap &a0, const CUtensorMap &a1, const CUtensorMap &w0, const CUtensorMap &w1,
                         const GemmParams &p, cudaStream_t stream) {
-    auto kern = gemm_kernel<MODE, K2, GA>;
+    auto kern = gemm_kernel<MODE, K2, GA, FC>;
     constexpr int kBlock = kThreads + (GA ? kGatherThreads : 0);
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    if (cudaError_t ea = ensure_dyn_smem(reinterpret_cast<const void *>(kern), kSmemMax); ea != cudaSuccess) return ea;
     constexpr int kid = (MODE == PF_GEMM1 || MODE == DC_GEMM1) ? BM_KERNEL_GEMM1 : BM_KERNEL_GEMM2;
     const size_t smem = 1024 + (size_t)p.stages * p.stage_bytes + kSmemBars + (MODE == PF_GEMM2 ? kSmemEpi : 0) +
                         sched_smem_bytes(p.seg_cap) + (size_t)p.tail_pad;
@@ -982,22 +1143,14 @@ cudaError_t launch_gemm(const CUtensorMap &a0, const CUtensorMap &a1, const CUte
 // memory); out-of-bounds elements are zero-filled.  Used by the router's slab ring.
 bool make_map_2d_plain(CUtensorMap *m, const void *base, uint64_t rows, uint64_t cols, uint32_t box_rows,
                        uint32_t box_cols) {
-    EncodeTiledFn enc = get_encode();
-    if (!enc) return false;
-    cuuint64_t dims[2] = {cols, rows};
-    cuuint64_t strides[1] = {cols * sizeof(bm_bf16)};
-    cuuint32_t box[2] = {box_cols, box_rows};
-    cuuint32_t es[2] = {1, 1};
-    return enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base), dims, strides, box, es,
-               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+    return encode_map(m, MapKey{base, cols, rows, 0, box_cols, box_rows, 0});
 }
 
 static cudaError_t launch_combine_raw(const ForwardArgs &a, cudaStream_t stream) {
     // one warp per token; with few tokens a token's 32-chunk column slices go to different warps
     const int n_slices = (a.D / 8 + 31) / 32;
     int split = 1;
-    while (split < n_slices && (long long)a.T * split < (long long)num_sms() * tune_int("BM_COMBINE_WARPS", 64)) split *= 2;   // fill the SMs' warp slots
+    while (split < n_slices && (long long)a.T * split < (long long)num_sms() * opt(OPT_COMBINE_WARPS)) split *= 2;   // fill the SMs' warp slots
     if (split > n_slices) split = n_slices;
     const long long items = (long long)a.T * split;
     return launch_kernel(combine_kernel, dim3((unsigned)std::min<long long>((items + 7) / 8, (long long)num_sms() * 8)),
@@ -1014,12 +1167,34 @@ cudaError_t launch_combine(const ForwardArgs &a, cudaStream_t stream) {
     return e;
 }
 
+// the decode path's tiling (host guess of the non-empty segments; the data-dependent truth lives on the device)
+static void decode_tiling(int T, int D, int F, int K, int G, int S, int *R1, int *R2, int *ks2) {
+    const int kb1 = (D + kBlockK - 1) / kBlockK, kb2 = (F + kBlockK - 1) / kBlockK;
+    const long long TK = (long long)T * K;
+    int n_seg = (int)(G < TK ? G : TK);
+    n_seg += S;
+    if (n_seg < 1) n_seg = 1;
+    int ks1;
+    choose_decode_tiling(F, kb1, n_seg, false, 2, num_sms(), R1, &ks1);
+    choose_decode_tiling(D, kb2, n_seg, true, 1, num_sms(), R2, ks2);
+    if (opt(OPT_DC_R2) > 0) { *R2 = opt(OPT_DC_R2); *ks2 = opt(OPT_DC_KS2); }
+    if (opt(OPT_DC_R1) > 0) *R1 = opt(OPT_DC_R1);
+}
+
+int decode_ksplit(int T, int D, int F, int K, int G, int S) {
+    int R1, R2, ks2;
+    decode_tiling(T, D, F, K, G, S, &R1, &R2, &ks2);
+    return ks2;
+}
+
 cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t stream) {
     const int TK = a.T * a.K;
     const int sms = num_sms();
 
-    // tensor-parallel partial (out_f32): the decode path accumulates straight into the caller's buffer
-    float *acc_buf = (decode && a.out_f32) ? a.out_f32 : a.out_acc;
+    // Combine: fused into the GEMM2 epilogue (fp32 reductions into the zero region + last-arriver rounding) unless
+    // option FUSED_COMBINE = 0 asks for the two-pass form on the prefill tiles (bf16 y rows + combine_kernel, slot
+    // order: bit-deterministic for any K + S).  The decode kernel always finishes its output itself.
+    const bool fused = decode || opt(OPT_FUSED_COMBINE) != 0;
 
     // CTA pairs (cta_group::2, M = 256 per pair): a pair shares the weight tile, so a CTA stages 32 KB per
     // k-block instead of 48 KB (measured: GEMM1 232 -> 201 us at BJ:configs[3]).  A segment with an odd chunk
@@ -1027,7 +1202,7 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
     // single CTAs (which gather their rows themselves), D = 2048, F = 1408, E = 60, top-4: 410 rows per group
     // 253 / 274 us (G = 30, T = 3072) and 511 / 525 us (G = 60, T = 6144); 273 rows per group 198 / 206 us (G = 30)
     // but 402 / 392 us (G = 60); 137-205 rows per group 293 / 267 and 348 / 338 us.  BM_PF_PAIR=0/1 overrides.
-    const int pair_env = tune_int("BM_PF_PAIR", -1);
+    const int pair_env = opt(OPT_PF_PAIR);
     const bool many_rows = (long long)a.T * a.K >= 3LL * kChunkRows * a.G;
     const bool pair = !decode && (sms & 1) == 0 && (pair_env < 0 ? many_rows : pair_env != 0);
     // GA: GEMM1's own warps gather the token rows (single-CTA prefill tiles); the prep kernel then only builds the
@@ -1035,7 +1210,7 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
     // HBM traffic less).  Not with CTA pairs: the peer's "rows landed" must reach the leader's barrier through a
     // fence and a cluster-scope arrive per k-block, which lengthens the ring's turn-around -- GEMM1 30-36% slower
     // than the TMA-fed pair kernel even with one relay warp per ring stage (BM_PF_GATHER=2 forces it).
-    const int ga_env = tune_int("BM_PF_GATHER", 1);
+    const int ga_env = opt(OPT_PF_GATHER);
     const bool gather_in_gemm = !decode && (ga_env == 2 || (ga_env == 1 && !pair));
 
     // step 9 (+ schedule, + zero)
@@ -1043,7 +1218,7 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
         const int grid = sms * 4;
         profile_begin(BM_KERNEL_PREP, stream);
         cudaError_t e = launch_kernel(prep_kernel, dim3(grid), dim3(256), 0, stream, a.x, a.T, a.D, a.K, a.G, a.S,
-                                      a.r.counts, a.r.offsets, a.r.row_token, a.sched, gather_in_gemm ? nullptr : a.xs, acc_buf, decode ? 1 : 0, a.status);
+                                      a.r.counts, a.r.offsets, a.r.row_token, a.sched, gather_in_gemm ? nullptr : a.xs, a.status);
         if (e != cudaSuccess) return e;
         profile_end(BM_KERNEL_PREP, stream);
     }
@@ -1052,7 +1227,8 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
     p.seg_cap = a.G + a.S + 1;
     p.T = a.T; p.D = a.D; p.F = a.F; p.K = a.K; p.G = a.G; p.S = a.S; p.TK = TK;
     p.counts = a.r.counts; p.offsets = a.r.offsets; p.row_token = a.r.row_token; p.row_slot = a.r.row_slot;
-    p.gate_w = a.r.gate_w; p.sched = a.sched; p.h = a.h; p.out_acc = acc_buf; p.y = a.y; p.x = a.x;
+    p.gate_w = a.r.gate_w; p.n_slots = a.r.n_slots; p.sched = a.sched; p.h = a.h; p.out_acc = a.out_acc; p.tickets = a.tickets;
+    p.y = a.y; p.x = a.x; p.out = a.out; p.out_f32 = a.out_f32;
 
 
     const uint64_t h_rows = (uint64_t)TK + (uint64_t)a.S * a.T;
@@ -1078,19 +1254,16 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
                        : launch_gemm<PF_GEMM1>(m_xs, m_x, m_w1, m_w3, p, stream);
         if (err != cudaSuccess) return err;
         p.kblocks = kb2; p.R = 256; p.n_wtiles = (a.D + 255) / 256;
-        err = pair ? launch_gemm<PF_GEMM2, true>(m_h, m_h, m_w2h, m_w2h, p, stream)
-                   : launch_gemm<PF_GEMM2>(m_h, m_h, m_w2, m_w2, p, stream);
+        if (fused)
+            err = pair ? launch_gemm<PF_GEMM2, true, false, true>(m_h, m_h, m_w2h, m_w2h, p, stream)
+                       : launch_gemm<PF_GEMM2, false, false, true>(m_h, m_h, m_w2, m_w2, p, stream);
+        else
+            err = pair ? launch_gemm<PF_GEMM2, true>(m_h, m_h, m_w2h, m_w2h, p, stream)
+                       : launch_gemm<PF_GEMM2>(m_h, m_h, m_w2, m_w2, p, stream);
         if (err != cudaSuccess) return err;
     } else {
-        // segments expected to be non-empty (host guess; the data-dependent truth lives on the device)
-        int n_seg = a.G < TK ? a.G : TK;
-        n_seg += a.S;
-        if (n_seg < 1) n_seg = 1;
-        int R1, R2, ks1, ks2;
-        choose_decode_tiling(a.F, kb1, n_seg, false, 2, sms, &R1, &ks1);
-        choose_decode_tiling(a.D, kb2, n_seg, true, 1, sms, &R2, &ks2);
-        if (tune_int("BM_DC_R2", 0) > 0) { R2 = tune_int("BM_DC_R2", 0); ks2 = tune_int("BM_DC_KS2", 1); }
-        if (tune_int("BM_DC_R1", 0) > 0) R1 = tune_int("BM_DC_R1", 0);
+        int R1, R2, ks2;
+        decode_tiling(a.T, a.D, a.F, a.K, a.G, a.S, &R1, &R2, &ks2);
         const int nbox = 32;                         // token rows travel in 32-row boxes, as many as the chunk has
         if (!make_map_2d(&m_xs, a.xs, TK > 0 ? TK : 1, a.D, nbox) || !make_map_2d(&m_x, a.x, a.T, a.D, nbox) ||
             !make_map_3d(&m_w1, a.W1, a.G + a.S, a.F, a.D, R1) || !make_map_3d(&m_w3, a.W3, a.G + a.S, a.F, a.D, R1) ||
@@ -1101,24 +1274,14 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
         if ((err = launch_gemm<DC_GEMM1>(m_xs, m_x, m_w1, m_w3, p, stream)) != cudaSuccess) return err;
         p.ksplit = ks2; p.kblocks = kb2 / ks2; p.R = R2; p.n_wtiles = (a.D + R2 - 1) / R2;
         ring_geometry(true, false, a.T, &p);
-        if ((err = launch_gemm<DC_GEMM2>(m_h, m_h, m_w2, m_w2, p, stream)) != cudaSuccess) return err;
+        if ((err = launch_gemm<DC_GEMM2, false, false, true>(m_h, m_h, m_w2, m_w2, p, stream)) != cudaSuccess) return err;
     }
 
-    {
-        const size_t n8 = (size_t)a.T * a.D / 8;
-        int grid = (int)((n8 + 255) / 256);
-        if (grid > sms * 8) grid = sms * 8;
-        if (grid < 1) grid = 1;
-        profile_begin(BM_KERNEL_FINALIZE, stream);
-        cudaError_t e;
-        if (decode)
-            e = a.out_f32 ? cudaSuccess      // the fp32 sums already are the result
-                          : launch_kernel(finalize_kernel, dim3(grid), dim3(256), 0, stream, (const float *)a.out_acc, a.out, n8);
-        else
-            e = launch_combine_raw(a, stream);
-        profile_end(BM_KERNEL_FINALIZE, stream);
-        return e;
-    }
+    if (fused) return cudaSuccess;
+    profile_begin(BM_KERNEL_FINALIZE, stream);
+    err = launch_combine_raw(a, stream);
+    profile_end(BM_KERNEL_FINALIZE, stream);
+    return err;
 }
 
 // f_e(x_t) for every expert and token (calibration forward): the prefill GEMM kernels over a
@@ -1133,7 +1296,7 @@ cudaError_t launch_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 
     p.T = T; p.D = D; p.F = F; p.K = 1; p.G = 0; p.S = E; p.TK = 0;
     p.sched = sched; p.h = h; p.y = y; p.x = x;
     p.ksplit = 1;
-    const bool pair = (num_sms() & 1) == 0 && T >= 3 * kChunkRows && tune_int("BM_PF_PAIR", -1) != 0;   // as launch_forward_tc
+    const bool pair = (num_sms() & 1) == 0 && T >= 3 * kChunkRows && opt(OPT_PF_PAIR) != 0;   // as launch_forward_tc
     CUtensorMap m_x, m_w1, m_w3, m_w2, m_h;
     if (!make_map_2d(&m_x, x, T, D, 128) || !make_map_3d(&m_w1, W1, E, F, D, 128) || !make_map_3d(&m_w3, W3, E, F, D, 128) ||
         !make_map_3d(&m_w2, W2, E, D, F, pair ? 128 : 256) || !make_map_2d(&m_h, h, (uint64_t)E * T, F, 128))

@@ -244,12 +244,7 @@ cudaError_t launch_gemv(const GemvArgs &p, int kid, cudaStream_t stream) {
     const size_t smem = (size_t)rows_cap * p.IN * 2 + (size_t)(p.G + p.S) * sizeof(int);
     if (smem > 220 * 1024) return cudaErrorInvalidValue;
     auto kern = gemv_kernel<SWIGLU>;
-    static size_t smem_set = 0;
-    if (smem > 48 * 1024 && smem > smem_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        smem_set = smem;
-    }
+    if (cudaError_t ea = ensure_dyn_smem(reinterpret_cast<const void *>(kern), smem); ea != cudaSuccess) return ea;
     profile_begin(kid, stream);
     cudaError_t e = launch_kernel(kern, dim3(num_sms()), dim3(kGvThreads), smem, stream, p, rows_cap);
     profile_end(kid, stream);
@@ -418,17 +413,12 @@ cudaError_t launch_forward_gemv(const ForwardArgs &a, cudaStream_t stream) {
     const long long total = (long long)a.T * (a.D / 2);
     const int max_q = (int)((total + num_sms() - 1) / num_sms());
     const size_t smem2 = (size_t)max_src * a.F * 2 + (size_t)max_src * max_q * 2 * sizeof(float);
-    if (max_src <= 32 && smem2 <= 200 * 1024 && tune_int("BM_GEMV_FUSE", 1) != 0) {
+    if (max_src <= 32 && smem2 <= 200 * 1024 && opt(OPT_GEMV_FUSE) != 0) {
         Gemv2Args q{};
         q.h = a.h; q.W2 = a.W2; q.out = a.out_f32 ? nullptr : a.out; q.out_f32 = a.out_f32;
         q.group_ids = a.r.group_ids; q.slot_row = a.r.slot_row; q.n_slots = a.r.n_slots; q.gate_w = a.r.gate_w;
         q.T = a.T; q.K = a.K; q.G = a.G; q.S = a.S; q.D = a.D; q.F = a.F;
-        static size_t smem_set = 0;
-        if (smem2 > 48 * 1024 && smem2 > smem_set) {
-            e = cudaFuncSetAttribute(gemv2_combine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
-            if (e != cudaSuccess) return e;
-            smem_set = smem2;
-        }
+        if ((e = ensure_dyn_smem(reinterpret_cast<const void *>(gemv2_combine_kernel), smem2)) != cudaSuccess) return e;
         profile_begin(BM_KERNEL_GEMM2, stream);
         e = launch_kernel(gemv2_combine_kernel, dim3(num_sms()), dim3(kGvThreads), smem2, stream, q, max_src, max_q);
         profile_end(BM_KERNEL_GEMM2, stream);

@@ -137,17 +137,12 @@ cudaError_t launch_permute(int T, int K, int G, const bm_routing &r, int32_t *bl
     if (items <= kPermSmallItems) {
         // few items: 8 warps; otherwise 16 warps with a few rounds of 32 items each, so the serial chain of
         // rounds (load -> match -> shared-memory update, twice) stays short
-        int nw = tune_int("BM_PERM_SMALL_WARPS", 0);
+        int nw = opt(OPT_PERM_SMALL_WARPS);
         if (nw <= 0) nw = items <= 256 ? 8 : 16;      // measured at 1024 items: 8 warps 10.2, 16 warps 8.7, 32 warps 9.9 us
         int per_warp = (int)((items + nw - 1) / nw);
         per_warp = (per_warp + 31) / 32 * 32;
         const size_t smem = (size_t)nw * G * sizeof(int) + (size_t)(G + 512) * sizeof(int);
-        static size_t smem_set = 0;
-        if (smem > 48 * 1024 && smem > smem_set) {
-            cudaError_t e = cudaFuncSetAttribute(permute_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e != cudaSuccess) return e;
-            smem_set = smem;
-        }
+        if (cudaError_t ea = ensure_dyn_smem(reinterpret_cast<const void *>(permute_small_kernel), smem); ea != cudaSuccess) return ea;
         return launch_kernel(permute_small_kernel, dim3(1), dim3(nw * 32), smem, stream, (const int32_t *)r.group_ids,
                              T, K, G, per_warp, r.counts, r.offsets, r.row_token, r.row_slot, r.slot_row, status);
     }

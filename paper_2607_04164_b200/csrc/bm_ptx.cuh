@@ -53,11 +53,25 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity) {
         : "memory");
     return ok != 0;
 }
-// Bounded wait: a protocol bug traps (reported as a launch failure) instead of hanging the GPU.
+// Bounded wait: a protocol bug traps (reported as a launch failure) instead of hanging the GPU.  The bound is TIME
+// (%globaltimer, checked every 4096 polls), not a poll count: a wait may legitimately last long under
+// compute-sanitizer, a debugger or time-slicing, but no barrier of this library stays closed for kWaitTimeoutNs.
+// A trap kills the CUDA context (every later call returns BM_ERR_CUDA); the workspace must then be re-initialised.
+constexpr uint64_t kWaitTimeoutNs = 20ull * 1000ull * 1000ull * 1000ull;
+__device__ __forceinline__ uint64_t globaltimer_ns() {
+    uint64_t t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
     uint32_t spins = 0;
+    uint64_t t0 = 0;
     while (!mbar_try_wait(bar, parity)) {
-        if (++spins > (1u << 26)) __trap();
+        if ((++spins & 0xfffu) == 0) {
+            const uint64_t now = globaltimer_ns();
+            if (t0 == 0) t0 = now;
+            else if (now - t0 > kWaitTimeoutNs) __trap();
+        }
     }
 }
 

@@ -383,13 +383,18 @@ __device__ __forceinline__ void fma2(float &d0, float &d1, float x, float w0, fl
 __device__ __forceinline__ float bf16_lo_alu(uint32_t u) { return __uint_as_float(__byte_perm(u, 0u, 0x1044)); }
 
 // Wait of a helper role (producer lane, select warps): backs off between polls so that it does not take
-// issue slots from the compute warps; bounded like ptx::mbar_wait (a protocol bug traps instead of hanging).
+// issue slots from the compute warps; bounded in time like ptx::mbar_wait (a protocol bug traps instead of hanging).
 template <unsigned NS>
 __device__ __forceinline__ void mbar_wait_sleep(uint64_t *bar, uint32_t parity) {
     uint32_t spins = 0;
+    uint64_t t0 = 0;
     while (!ptx::mbar_try_wait(bar, parity)) {
         __nanosleep(NS);
-        if (++spins > (1u << 24)) __trap();
+        if ((++spins & 0xfffu) == 0) {
+            const uint64_t now = ptx::globaltimer_ns();
+            if (t0 == 0) t0 = now;
+            else if (now - t0 > ptx::kWaitTimeoutNs) __trap();
+        }
     }
 }
 
@@ -555,17 +560,12 @@ cudaError_t launch_tp(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const f
     const int n_etiles = (E + 7) / 8;
     int WE = 1;
     while (WE < n_etiles && WE < kTpComputeWarps) WE *= 2;
-    if (tune_int("BM_ROUTER_WE", 0) > 0) WE = tune_int("BM_ROUTER_WE", 0);
+    if (opt(OPT_ROUTER_WE) > 0) WE = opt(OPT_ROUTER_WE);
     const int WT = kTpComputeWarps / WE;
     const int TB = WT * kTpTok, EB = WE * 8;
     const size_t smem = (size_t)kTpStages * (TB + EB) * (kSlab * 2) + (2 * kTpStages + 4) * sizeof(uint64_t) +
                         2 * (size_t)TB * E * sizeof(float);
-    static size_t smem_set = 0;
-    if (smem > 48 * 1024 && smem > smem_set) {
-        cudaError_t e = cudaFuncSetAttribute(router_tp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        smem_set = smem;
-    }
+    if (cudaError_t ea = ensure_dyn_smem(reinterpret_cast<const void *>(router_tp_kernel), smem); ea != cudaSuccess) return ea;
     CUtensorMap m_x, m_w;
     if (!make_map_2d_plain(&m_x, x, (uint64_t)T, (uint64_t)D, (uint32_t)TB, kSlab) ||
         !make_map_2d_plain(&m_w, Wr, (uint64_t)E, (uint64_t)D, (uint32_t)EB, kSlab))
@@ -583,10 +583,7 @@ cudaError_t launch_cfg(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const 
     const int TB = WT * TOK;
     const size_t smem = (size_t)TB * E * sizeof(float);
     auto kern = router_kernel<TOK, ET>;
-    if (smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-    }
+    if (cudaError_t ea = ensure_dyn_smem(reinterpret_cast<const void *>(kern), smem); ea != cudaSuccess) return ea;
     const int grid = (T + TB - 1) / TB;
     return launch_kernel(kern, dim3(grid), dim3(kWarps * 32), smem, stream, x, T, D, Wr, bias, E, K, gm, WT, WE,
                          r.expert_ids, r.group_ids, r.gate_w, r.n_slots, status);
@@ -598,23 +595,18 @@ cudaError_t launch_router(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, con
                           int K, GroupMap gm, const bm_routing &r, int32_t *status, float *route_logits,
                           bool *fused_permute, cudaStream_t stream) {
     *fused_permute = false;
-    if (T >= tune_int("BM_ROUTER_TP_MIN_T", kSplitRouterMaxT))   // throughput shape: operands staged through shared memory
+    if (T >= opt(OPT_ROUTER_TP_MIN_T))   // throughput shape: operands staged through shared memory
         return launch_tp(x, T, D, Wr, bias, E, K, gm, r, status, stream);
     // (measured: 2 us faster than router + permutation kernels at T = 1, even at T = 16, slower from T = 64 on:
     // more CTAs and two rounds of arrival counters)
-    if (E > 8 && T <= tune_int("BM_ROUTER_SPLIT_MAX_T", 16)) {
+    if (E > 8 && T <= opt(OPT_ROUTER_SPLIT_MAX_T)) {
         // latency shape, experts spread over CTAs; the last CTA also permutes when one CTA can
         constexpr int ET = 2;
         const int ES = (E + kSplitWarps * ET - 1) / (kSplitWarps * ET);
         const bool fuse = (long long)T * K <= kPermSmallItems;
         size_t smem = (size_t)E * sizeof(float);
         if (fuse) smem = std::max(smem, (size_t)(kSplitWarps * r.G + r.G + 512) * sizeof(int));
-        static size_t smem_set = 0;
-        if (smem > 48 * 1024 && smem > smem_set) {
-            cudaError_t e = cudaFuncSetAttribute(router_split_kernel<ET>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e != cudaSuccess) return e;
-            smem_set = smem;
-        }
+        if (cudaError_t ea = ensure_dyn_smem(reinterpret_cast<const void *>(router_split_kernel<ET>), smem); ea != cudaSuccess) return ea;
         int per_warp = (int)(((long long)T * K + kSplitWarps - 1) / kSplitWarps);
         per_warp = (per_warp + 31) / 32 * 32;
         *fused_permute = fuse;
