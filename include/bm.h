@@ -301,7 +301,10 @@ int bm_device_status(void *workspace, int32_t *host_out, bm_stream_t stream);
  *   FUSED_COMBINE (-1)      prefill tiles: 0 = two-pass combine (bf16 y rows + slot-order sum, deterministic), else fused
  *   PF_PAIR (-1)            prefill tiles: 1 / 0 force CTA pairs (cta_group::2) on / off, -1 = by rows per group
  *   PF_GATHER (1)           0 = materialise gathered rows, 1 = gather inside GEMM1 on single-CTA tiles, 2 = also with pairs
- *   PF_RASTER (-1)          prefill tiles: weight tiles per L2 band of the item order, -1 = by shape, 0 = chunk-fastest
+ *   PF_G1_BC, PF_G2_BC, PF_G2_BW (-1)   prefill tiles: L2 bands of the item order -- chunk units per band in GEMM1 / GEMM2,
+ *                           weight tiles per band in GEMM2; <= 0 = one band (chunk-fastest order, the default)
+ *   PF_G1_HINTS, PF_G2_HINTS (-1)       L2 eviction hints of the prefill tiles' TMA loads: 10 * activations + weights with
+ *                           0 = evict_first, 1 = normal, 2 = evict_last; -1 = default (21)
  *   DECODE_MAX_T (384), DECODE_MID_T (192), DECODE_ROWS (24), DECODE_MID_ROWS (128), GEMV_MAX_T (2), GEMV_ROWS (1)
  *                           thresholds of BM_PATH_AUTO
  *   GEMV_FUSE (1)           matrix-vector path: fuse the W2 stage with the combine

@@ -87,6 +87,9 @@ struct GemmParams {
     int ksplit;         // K splits (DC_GEMM2), else 1
     int R;              // weight rows per tile (prefill: 128 for GEMM1 per matrix, 256 for GEMM2)
     int n_wtiles;       // tiles along the weight-row dimension
+    int band_c;         // prefill item order: chunk units (chunks, or chunk pairs) per L2 band ...
+    int band_w;         // ... and weight tiles per band (see get_item); <= 0: one band
+    int hints;          // L2 eviction hints of the TMA loads, 10 * activations + weights: 0 = evict_first, 1 = normal, 2 = evict_last
     int seg_cap;        // G + S + 1: entries per schedule array cached in shared memory
     const int32_t *counts, *offsets, *row_token, *row_slot;
     const bm_bf16 *x;   // GA: token rows gathered straight from x [T, D]
@@ -132,8 +135,30 @@ __device__ __forceinline__ bool get_item(const GemmParams &p, const SchedView &s
     const int c0 = first[s];
     const int units_s = first[s + 1] - c0;
     const int local = item - c0 * per_chunk;
-    const int unit = local % units_s;
-    const int rest = local / units_s;
+    int unit, rest;
+    if (MODE == PF_GEMM1 || MODE == PF_GEMM2) {
+        // L2-aware item order.  The CTAs work on ~148 consecutive items at a time, all streaming through K in step, so
+        // what reaches DRAM is the set of DISTINCT operand tiles of those items plus whatever L2 cannot keep until the
+        // next visit.  A segment's (chunk unit x weight tile) grid is therefore walked in bands:
+        //   [weight-tile band of band_w][chunk band of band_c][weight tile in band][chunk unit in band]   (unit fastest)
+        // GEMM1 uses one weight band (band_w = all): a chunk band's token rows (band_c x 128/256 rows x D) stay in L2
+        // while all weight tiles stream past once.  GEMM2's operands are K = F long: a band of band_w W2 tiles is kept
+        // while the H rows of the chunk bands stream past.  The plain chunk-fastest order of round 1 re-read the token
+        // rows of a large group (60 MB at BJ:configs[2]) for every weight tile: 3.4x / 4.7x the algorithmic DRAM bytes.
+        const int Bw = (p.band_w > 0 && p.band_w < p.n_wtiles) ? p.band_w : p.n_wtiles;
+        const int Bc = (p.band_c > 0 && p.band_c < units_s) ? p.band_c : units_s;
+        const int per_wb = units_s * Bw;
+        const int wb = local / per_wb, r1 = local - wb * per_wb;
+        const int bw = min(Bw, p.n_wtiles - wb * Bw);
+        const int cb = r1 / (Bc * bw), r2 = r1 - cb * (Bc * bw);
+        const int bc = min(Bc, units_s - cb * Bc);
+        const int wt_in = r2 / bc;
+        unit = cb * Bc + (r2 - wt_in * bc);
+        rest = wb * Bw + wt_in;
+    } else {
+        unit = local % units_s;
+        rest = local / units_s;
+    }
     int chunk = K2 ? 2 * unit + rank : unit;
     it.u = u;
     it.ks = rest % p.ksplit;
@@ -296,6 +321,8 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
         } else {
             have = get_item<MODE, K2>(p, sv, item, it, rank);
         }
+        auto policy = [](int h) { return h == 0 ? ptx::kEvictFirst : (h == 1 ? ptx::kEvictNormal : ptx::kEvictLast); };
+        const uint64_t pol_a = policy(p.hints / 10), pol_w = policy(p.hints % 10);
         for (; have; item += item_stride, have = get_item<MODE, K2>(p, sv, item, it, rank), kb_first = 0) {
             const CUtensorMap *tm_act = (kGemm1 && it.shared) ? &tm_act1 : &tm_act0;
             const int wrow0 = it.wt * p.R;
@@ -307,32 +334,32 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
                     if (ptx::elect_one()) {
                         uint8_t *st = smem + (size_t)stage * stage_bytes;
                         if (leader) ptx::mbar_arrive_expect_tx(&full[stage], stage_tx);
-                        if (!GA) ptx::tma_load_2d_pair(st, tm_act, &full[stage], kc, it.act_row0, ptx::kEvictLast);
+                        if (!GA) ptx::tma_load_2d_pair(st, tm_act, &full[stage], kc, it.act_row0, pol_a);
                         if (MODE == PF_GEMM1)       // B rows 0-127 = the W1 tile (leader), 128-255 = the W3 tile (peer)
                             ptx::tma_load_3d_pair(st + kTileBytes16K, leader ? &tm_w0 : &tm_w1, &full[stage], kc, wrow0, it.u,
-                                                  ptx::kEvictFirst);
+                                                  pol_w);
                         else                        // each CTA half of the 256 W2 rows
                             ptx::tma_load_3d_pair(st + kTileBytes16K, &tm_w0, &full[stage], kc, wrow0 + (int)rank * 128, it.u,
-                                                  ptx::kEvictFirst);
+                                                  pol_w);
                     }
                 } else if (ptx::elect_one()) {
                     uint8_t *st = smem + (size_t)stage * stage_bytes;
                     ptx::mbar_arrive_expect_tx(&full[stage], stage_tx);
                     if (!kDecode) {
                         // A = 128 activation rows, B = 256 weight rows (W1|W3 tiles, or one W2 tile of 256)
-                        if (!GA) ptx::tma_load_2d(st, tm_act, &full[stage], kc, it.act_row0, ptx::kEvictLast);
-                        ptx::tma_load_3d(st + kTileBytes16K, &tm_w0, &full[stage], kc, wrow0, it.u, ptx::kEvictFirst);
+                        if (!GA) ptx::tma_load_2d(st, tm_act, &full[stage], kc, it.act_row0, pol_a);
+                        ptx::tma_load_3d(st + kTileBytes16K, &tm_w0, &full[stage], kc, wrow0, it.u, pol_w);
                         if (MODE == PF_GEMM1)
-                            ptx::tma_load_3d(st + 2 * kTileBytes16K, &tm_w1, &full[stage], kc, wrow0, it.u, ptx::kEvictFirst);
+                            ptx::tma_load_3d(st + 2 * kTileBytes16K, &tm_w1, &full[stage], kc, wrow0, it.u, pol_w);
                     } else {
                         // M side = R weight rows (streamed once from HBM), N side = the group's token rows
                         // (32-row boxes; rows past the group's within the last box are loaded and never stored)
-                        ptx::tma_load_3d(st, &tm_w0, &full[stage], kc, wrow0, it.u, ptx::kEvictFirst);
+                        ptx::tma_load_3d(st, &tm_w0, &full[stage], kc, wrow0, it.u, pol_w);
                         if (MODE == DC_GEMM1)
-                            ptx::tma_load_3d(st + p.wslot, &tm_w1, &full[stage], kc, wrow0, it.u, ptx::kEvictFirst);
+                            ptx::tma_load_3d(st + p.wslot, &tm_w1, &full[stage], kc, wrow0, it.u, pol_w);
                         for (int j = 0; j * 32 < it.n; ++j)
                             ptx::tma_load_2d(st + p.off_b + j * 4096, tm_act, &full[stage], kc, it.act_row0 + j * 32,
-                                             ptx::kEvictLast);
+                                             pol_a);
                     }
                 }
                 __syncwarp();
@@ -1224,6 +1251,7 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
     }
 
     GemmParams p{};
+    p.hints = 20;            // activations evict_last, weights evict_first (decode: the weights stream once)
     p.seg_cap = a.G + a.S + 1;
     p.T = a.T; p.D = a.D; p.F = a.F; p.K = a.K; p.G = a.G; p.S = a.S; p.TK = TK;
     p.counts = a.r.counts; p.offsets = a.r.offsets; p.row_token = a.r.row_token; p.row_slot = a.r.row_slot;
@@ -1246,6 +1274,16 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
         if (pair && !make_map_3d(&m_w2h, a.W2, a.G + a.S, a.D, a.F, 128)) return cudaErrorInvalidValue;
         ring_geometry(false, true, a.T, &p, pair);
         p.kblocks = kb1; p.R = 128; p.n_wtiles = (a.F + 127) / 128;
+        // L2 behaviour of the prefill tiles (ncu at BJ:configs[2], DRAM bytes read by GEMM1 / GEMM2; algorithmic 1.06 / 0.90 GB):
+        //   weights evict_first (round 1)             4.64 / 5.81 GB   -- a weight tile is shared by every chunk of its group, but
+        //   weights evict_normal or evict_last        1.95 / 3.65 GB      an evict_first line is gone before the other CTAs ask for it
+        //   + chunk bands of 8 / 16 pairs (GEMM1)     4.1 / 2.2 GB     -- fewer CTAs share a weight tile at a time: worse
+        //   + square bands 9 chunks x 8 tiles (GEMM2) 4.3 GB           -- worse as well
+        // so the hints changed (cold-cache kernel time -7% / -8.5%) and the band order stays available but off (options
+        // PF_G1_BC, PF_G2_BC, PF_G2_BW; get_item).
+        p.band_c = opt(OPT_PF_G1_BC) > 0 ? opt(OPT_PF_G1_BC) : 0;
+        p.band_w = 0;
+        p.hints = opt(OPT_PF_G1_HINTS) >= 0 ? opt(OPT_PF_G1_HINTS) : 21;
         if (gather_in_gemm)
             err = pair ? launch_gemm<PF_GEMM1, true, true>(m_xs, m_x, m_w1, m_w3, p, stream)
                        : launch_gemm<PF_GEMM1, false, true>(m_xs, m_x, m_w1, m_w3, p, stream);
@@ -1254,6 +1292,9 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
                        : launch_gemm<PF_GEMM1>(m_xs, m_x, m_w1, m_w3, p, stream);
         if (err != cudaSuccess) return err;
         p.kblocks = kb2; p.R = 256; p.n_wtiles = (a.D + 255) / 256;
+        p.band_w = opt(OPT_PF_G2_BW) > 0 ? opt(OPT_PF_G2_BW) : 0;
+        p.band_c = opt(OPT_PF_G2_BC) > 0 ? opt(OPT_PF_G2_BC) : 0;
+        p.hints = opt(OPT_PF_G2_HINTS) >= 0 ? opt(OPT_PF_G2_HINTS) : 21;
         if (fused)
             err = pair ? launch_gemm<PF_GEMM2, true, false, true>(m_h, m_h, m_w2h, m_w2h, p, stream)
                        : launch_gemm<PF_GEMM2, false, false, true>(m_h, m_h, m_w2, m_w2, p, stream);
@@ -1292,6 +1333,7 @@ cudaError_t launch_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 
     cudaError_t err = launch_kernel(dense_sched_kernel, dim3(1), dim3(256), 0, stream, sched, E, T);
     if (err != cudaSuccess) return err;
     GemmParams p{};
+    p.hints = 20;
     p.seg_cap = E + 1;
     p.T = T; p.D = D; p.F = F; p.K = 1; p.G = 0; p.S = E; p.TK = 0;
     p.sched = sched; p.h = h; p.y = y; p.x = x;
