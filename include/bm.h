@@ -307,6 +307,8 @@ int bm_device_status(void *workspace, int32_t *host_out, bm_stream_t stream);
  *                           0 = evict_first, 1 = normal, 2 = evict_last; -1 = default (21)
  *   DECODE_MAX_T (384), DECODE_MID_T (192), DECODE_ROWS (24), DECODE_MID_ROWS (128), GEMV_MAX_T (2), GEMV_ROWS (1)
  *                           thresholds of BM_PATH_AUTO
+ *   DC_DENSE_MAX_T (64)     decode kernels: up to this many tokens (<= 64) every active set multiplies all T tokens (no gather)
+ *   DC_PREFETCH_MB (48)     decode GEMM1: megabytes of W1 / W3 it asks L2 to fetch while it still waits for the routing; 0 = off
  *   GEMV_FUSE (1)           matrix-vector path: fuse the W2 stage with the combine
  *   DC_R1, DC_R2, DC_KS2, DC_RMAX, DC_KS_FORCE (0, 0, 1, 128, 0)   decode tiling overrides (rows per tile, K splits)
  *   DC_STAGES, PF_STAGES (12)   cap on the shared-memory ring depth

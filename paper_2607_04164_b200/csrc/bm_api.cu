@@ -36,7 +36,7 @@ static const OptDef kOptDefs[OPT_COUNT] = {
     {"GEMV_ROWS", 1}, {"GEMV_MAX_T", 2}, {"GEMV_FUSE", 1}, {"DC_RMAX", 128}, {"DC_KS_FORCE", 0}, {"DC_STAGES", 12},
     {"PF_STAGES", 12}, {"DC_R1", 0}, {"DC_R2", 0}, {"DC_KS2", 1}, {"PF_PAIR", -1}, {"PF_GATHER", 1},
     {"COMBINE_WARPS", 64}, {"PERM_SMALL_WARPS", 0}, {"ROUTER_WE", 0}, {"ROUTER_TP_MIN_T", kSplitRouterMaxT},
-    {"ROUTER_SPLIT_MAX_T", 16}, {"FUSED_COMBINE", -1}, {"PF_G1_BC", -1}, {"PF_G2_BC", -1}, {"PF_G2_BW", -1}, {"PF_G1_HINTS", -1}, {"PF_G2_HINTS", -1},
+    {"ROUTER_SPLIT_MAX_T", 16}, {"FUSED_COMBINE", -1}, {"PF_G1_BC", -1}, {"PF_G2_BC", -1}, {"PF_G2_BW", -1}, {"PF_G1_HINTS", -1}, {"PF_G2_HINTS", -1}, {"DC_DENSE_MAX_T", kDenseMaxT}, {"DC_PREFETCH_MB", 48}, {"DC_KPACK", 2},
 };
 static int g_opt[OPT_COUNT];
 static bool init_options() {
@@ -238,8 +238,8 @@ int bm_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 *W1, const b
     if (workspace_bytes < w.front_end) return BM_ERR_WORKSPACE;
     if (device_ok() != 1) return BM_ERR_CUDA;
     uint8_t *ws = static_cast<uint8_t *>(workspace);
-    return launch_expert_outputs(x, T, D, W1, W3, W2, E, F, y, reinterpret_cast<int32_t *>(ws + w.sched),
-                                 reinterpret_cast<bm_bf16 *>(ws + w.h), reinterpret_cast<cudaStream_t>(stream)) == cudaSuccess
+    return launch_expert_outputs(x, T, D, W1, W3, W2, E, F, y, reinterpret_cast<bm_bf16 *>(ws + w.h),
+                                 reinterpret_cast<cudaStream_t>(stream)) == cudaSuccess
                ? BM_OK : BM_ERR_CUDA;
 }
 
@@ -335,7 +335,6 @@ static int forward_common(const bm_bf16 *x, int T, int D, const bm_routing *rout
     a.r = *routing;
     a.W1 = W1; a.W3 = W3; a.W2 = W2; a.out = out; a.out_f32 = out_f32;
     a.status = reinterpret_cast<int32_t *>(ws + w.status);
-    a.sched = reinterpret_cast<int32_t *>(ws + w.sched);
     a.xs = reinterpret_cast<bm_bf16 *>(ws + w.xs);
     a.h = reinterpret_cast<bm_bf16 *>(ws + w.h);
     const size_t zbase = zero_region_base(workspace_bytes, w);
@@ -463,7 +462,7 @@ int bm_forward_info(int T, int K, int G, int S, int D, int F, int *path, int *de
     const int pth = resolve_auto_path(T, K, G);
     int det = 1;
     if (pth == BM_PATH_PREFILL) det = (opt(OPT_FUSED_COMBINE) == 0 || K + S <= 2) ? 1 : 0;
-    else if (pth == BM_PATH_DECODE) det = ((K + S) * decode_ksplit(T, D, F, K, G, S) <= 2) ? 1 : 0;
+    else if (pth == BM_PATH_DECODE) det = ((K + S) * decode_ksplit(T, D, F, K, G, S) <= 2) ? 1 : 0;   // fp32 reds either way
     if (path) *path = pth;
     if (deterministic) *deterministic = det;
     return BM_OK;

@@ -48,6 +48,17 @@ constexpr int kSchedInts = 4 + 5 * (BM_MAX_G + kMaxShared) + 8;
 
 __host__ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+// Rows of the SwiGLU intermediate H: one per (token, slot) assignment and per (shared expert, token); the dense decode
+// kernels (T <= kDenseMaxT) instead keep a row per (active weight set, token).  Monotone in T.
+constexpr int kDenseMaxT = 64;
+__host__ inline size_t h_rows_needed(int T, int K, int G, int S) {
+    const size_t items = (size_t)T * K;
+    const size_t td = T < kDenseMaxT ? T : kDenseMaxT;
+    const size_t sets = (size_t)G < td * K ? (size_t)G : td * K;
+    const size_t plain = items + (size_t)S * T, dense = (sets + S) * td;
+    return plain > dense ? plain : dense;
+}
+
 __host__ inline size_t ticket_ints(int T, int D) { return (size_t)T * (size_t)((D + 31) / 32) * 4; }
 
 __host__ inline Workspace workspace_layout(int T, int D, int F, int K, int G, int S) {
@@ -60,7 +71,7 @@ __host__ inline Workspace workspace_layout(int T, int D, int F, int K, int G, in
     w.route_logits = off; off = align_up(off + (size_t)(T < kSplitRouterMaxT ? T : kSplitRouterMaxT) * BM_MAX_E * sizeof(float), 1024);
     w.sched = off;       off = align_up(off + kSchedInts * sizeof(int32_t), 1024);
     w.xs = off;          off = align_up(off + items * D * sizeof(bm_bf16), 1024);
-    w.h = off;           off = align_up(off + (items + (size_t)S * T) * F * sizeof(bm_bf16), 1024);
+    w.h = off;           off = align_up(off + h_rows_needed(T, K, G, S) * F * sizeof(bm_bf16), 1024);
     w.y = off;           off = align_up(off + (items + (size_t)S * T) * D * sizeof(bm_bf16), 1024);
     w.front_end = off;
     size_t z = 0;
@@ -106,7 +117,7 @@ enum Opt {
     OPT_PDL, OPT_DECODE_MAX_T, OPT_DECODE_MID_T, OPT_DECODE_ROWS, OPT_DECODE_MID_ROWS, OPT_GEMV_ROWS, OPT_GEMV_MAX_T,
     OPT_GEMV_FUSE, OPT_DC_RMAX, OPT_DC_KS_FORCE, OPT_DC_STAGES, OPT_PF_STAGES, OPT_DC_R1, OPT_DC_R2, OPT_DC_KS2,
     OPT_PF_PAIR, OPT_PF_GATHER, OPT_COMBINE_WARPS, OPT_PERM_SMALL_WARPS, OPT_ROUTER_WE, OPT_ROUTER_TP_MIN_T,
-    OPT_ROUTER_SPLIT_MAX_T, OPT_FUSED_COMBINE, OPT_PF_G1_BC, OPT_PF_G2_BC, OPT_PF_G2_BW, OPT_PF_G1_HINTS, OPT_PF_G2_HINTS, OPT_COUNT
+    OPT_ROUTER_SPLIT_MAX_T, OPT_FUSED_COMBINE, OPT_PF_G1_BC, OPT_PF_G2_BC, OPT_PF_G2_BW, OPT_PF_G1_HINTS, OPT_PF_G2_HINTS, OPT_DC_DENSE_MAX_T, OPT_DC_PREFETCH_MB, OPT_DC_KPACK, OPT_COUNT
 };
 int opt(Opt o);
 
@@ -151,7 +162,6 @@ struct ForwardArgs {
     bm_bf16 *out;
     // workspace sections
     int32_t *status;
-    int32_t *sched;
     bm_bf16 *xs;
     bm_bf16 *h;
     float *out_acc;      // zero region: fp32 accumulator of the fused combine
@@ -164,8 +174,7 @@ cudaError_t launch_unite(const bm_bf16 *W, int E, size_t n, const int32_t *gmap,
                          cudaStream_t stream);
 
 cudaError_t launch_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 *W1, const bm_bf16 *W3,
-                                  const bm_bf16 *W2, int E, int F, bm_bf16 *y, int32_t *sched, bm_bf16 *h,
-                                  cudaStream_t stream);
+                                  const bm_bf16 *W2, int E, int F, bm_bf16 *y, bm_bf16 *h, cudaStream_t stream);
 
 cudaError_t launch_expert_hist(const int32_t *expert_ids, long long items, int E, int32_t *w, cudaStream_t stream);
 size_t gram_workspace_bytes(int E);

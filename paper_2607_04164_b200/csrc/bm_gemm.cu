@@ -52,30 +52,13 @@ static_assert((3 * kMaxStages + 2 * kAccStages + 1) * 8 <= kSmemBars, "barrier b
 
 enum Mode { PF_GEMM1 = 0, PF_GEMM2 = 1, DC_GEMM1 = 2, DC_GEMM2 = 3 };
 
-// schedule (int32) written by the prep kernel: the non-empty segments (groups, then shared experts)
-//   [0] n_seg   [1] total_chunks
-//   seg_u[kMaxSeg]       weight set of segment s
-//   seg_chunk0[kMaxSeg]  first 128-row chunk of segment s; entry n_seg = total_chunks
-//   seg_rows[kMaxSeg]    rows of segment s (counts[u], or T for a shared expert)
-//   seg_off[kMaxSeg]     first permuted row of segment s (offsets[u]; 0 for a shared expert)
-// Every GEMM CTA copies the live part into shared memory once (SchedView over smem), so that the item
-// enumeration of its three roles never waits on global memory.
-constexpr int kSchedSegU = 4;
-constexpr int kSchedChunk0 = kSchedSegU + kMaxSeg;
-constexpr int kSchedRows = kSchedChunk0 + kMaxSeg;
-constexpr int kSchedOff = kSchedRows + kMaxSeg;
-constexpr int kSchedPair0 = kSchedOff + kMaxSeg;      // first chunk PAIR of segment s (CTA-pair prefill tiles); [2] = total
-static_assert(kSchedPair0 + kMaxSeg + 1 <= kSchedInts, "sched too small");
-
+// schedule: the non-empty segments (groups, then shared experts), five int arrays of seg_cap entries in each CTA's
+// shared memory (build_schedule):  u = weight set; chunk0 = first 128-row chunk (entry n_seg = total); rows;
+// off = first permuted row (offsets[u]; 0 for a shared expert); pair0 = first chunk PAIR (CTA-pair tiles).
 struct SchedView {
     int n_seg, total_chunks, total_pairs;
     const int32_t *u, *chunk0, *rows, *off, *pair0;
 };
-__device__ __forceinline__ SchedView sched_global(const int32_t *sched) {
-    return SchedView{sched[0], sched[1], sched[2], sched + kSchedSegU, sched + kSchedChunk0, sched + kSchedRows,
-                     sched + kSchedOff, sched + kSchedPair0};
-}
-
 struct GemmParams {
     int T, D, F, K, G, S, TK;
     int stages;         // depth of the shared-memory ring (<= kMaxStages)
@@ -84,18 +67,26 @@ struct GemmParams {
     int wslot;          // decode: bytes between the W1 and W3 tiles of a stage (R*128 rounded up to 1024)
     int tail_pad;       // decode: bytes kept free after the ring (an M=128 MMA reads 16 KB from a tile base, R < 128 rows of it real)
     int kblocks;        // k-blocks of one item (per split)
+    int kpack;          // decode: k-blocks per ring stage (1 or 2; kblocks % kpack == 0).  The single-thread issue loop costs
+                        // ~0.25 us per barrier turn whatever the tile holds, so a stage carries two k-blocks when it can
+    int mini_bytes;     // decode: bytes of one k-block inside a stage (stage_bytes = kpack * mini_bytes)
     int ksplit;         // K splits (DC_GEMM2), else 1
     int R;              // weight rows per tile (prefill: 128 for GEMM1 per matrix, 256 for GEMM2)
     int n_wtiles;       // tiles along the weight-row dimension
     int band_c;         // prefill item order: chunk units (chunks, or chunk pairs) per L2 band ...
     int band_w;         // ... and weight tiles per band (see get_item); <= 0: one band
+    const bm_bf16 *w1, *w3;   // DC_GEMM1: weight arrays, for the L2 prefetch before the grid-dependency wait
+    unsigned long long pf_set_bytes, pf_bytes;   // bytes of one weight set (F * D * 2) and how many leading bytes of each to prefetch
+    int dense;          // decode, T <= 64: every active set takes ALL T tokens as its rows (no gather, no permutation needed):
+                        // H row = segment * T + token; GEMM2 weighs token t of set u with its gate weight, 0 if not routed there
+    int32_t *status;    // device status word (BM_DEV_BAD_ROUTING)
+    const int32_t *group_ids;
     int hints;          // L2 eviction hints of the TMA loads, 10 * activations + weights: 0 = evict_first, 1 = normal, 2 = evict_last
     int seg_cap;        // G + S + 1: entries per schedule array cached in shared memory
     const int32_t *counts, *offsets, *row_token, *row_slot;
     const bm_bf16 *x;   // GA: token rows gathered straight from x [T, D]
     const float *gate_w;
     const int32_t *n_slots;
-    const int32_t *sched;
     bm_bf16 *h;
     float *out_acc;     // zero region: fp32 accumulator of the fused combine [T, D]
     int32_t *tickets;   // zero region: arrivals per (token, output piece)
@@ -167,7 +158,12 @@ __device__ __forceinline__ bool get_item(const GemmParams &p, const SchedView &s
     const int rows = sv.rows[s];
     it.n = min(kChunkRows, rows - chunk * kChunkRows);
     if (K2 && it.n <= 0) { it.n = 0; chunk = 0; }        // absent half of the last pair: point at real rows
-    if (it.shared) {
+    if (p.dense) {
+        it.tok0 = chunk * kChunkRows;
+        it.perm_row0 = 0;
+        it.h_row0 = s * p.T + it.tok0;
+        it.act_row0 = (MODE == PF_GEMM1 || MODE == DC_GEMM1) ? it.tok0 : it.h_row0;
+    } else if (it.shared) {
         it.tok0 = chunk * kChunkRows;
         it.perm_row0 = 0;
         it.h_row0 = p.TK + (u - p.G) * p.T + it.tok0;
@@ -179,6 +175,63 @@ __device__ __forceinline__ bool get_item(const GemmParams &p, const SchedView &s
         it.act_row0 = it.perm_row0;
     }
     return true;
+}
+
+// The schedule, built by warp 0 of every CTA in its own shared memory straight from counts / offsets (one coalesced
+// global read, then ballot + shuffle scans 32 sets at a time): the non-empty segments (groups, then the S shared
+// experts with T rows each), their first chunk / chunk pair, rows and first permuted row.  Round 1 had a prep kernel
+// write this to global memory and every CTA copy it -- the same latency on the critical path plus a launch.
+// hdr[0..2] = segments, chunks, chunk pairs.  dense: an active group takes all T tokens as rows.
+__device__ __forceinline__ void build_schedule(const GemmParams &p, int32_t *s_sched, int cap, int *hdr) {
+    const int lane = threadIdx.x & 31;
+    const int n = p.G + p.S;
+    int seg_base = 0, chunk_base = 0, pair_base = 0;
+    bool bad = false;
+    for (int u0 = 0; u0 < n; u0 += 32) {
+        const int u = u0 + lane;
+        int rows = 0, off = 0;
+        if (u < n) {
+            if (u < p.G) {
+                rows = p.counts[u];
+                off = p.offsets[u];
+                if (rows < 0 || off < 0 || off + rows > p.TK) { bad = true; rows = 0; }
+                if (p.dense && rows > 0) rows = p.T;
+            } else {
+                rows = p.T;
+            }
+        }
+        const bool ne = rows > 0;
+        const int ch = ne ? (rows + kChunkRows - 1) / kChunkRows : 0;
+        const unsigned m = __ballot_sync(kFullMask, ne);
+        const int seg = seg_base + __popc(m & ((1u << lane) - 1u));
+        const int pr = (ch + 1) >> 1;
+        int inc = ch, incp = pr;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(kFullMask, inc, o);
+            const int vp = __shfl_up_sync(kFullMask, incp, o);
+            if (lane >= o) { inc += v; incp += vp; }
+        }
+        if (ne && seg < cap - 1) {
+            s_sched[seg] = u;
+            s_sched[cap + seg] = chunk_base + inc - ch;
+            s_sched[2 * cap + seg] = rows;
+            s_sched[3 * cap + seg] = off;
+            s_sched[4 * cap + seg] = pair_base + incp - pr;
+        }
+        seg_base += __popc(m);
+        chunk_base += __shfl_sync(kFullMask, inc, 31);
+        pair_base += __shfl_sync(kFullMask, incp, 31);
+    }
+    bad = __any_sync(kFullMask, bad);
+    if (lane == 0) {
+        if (seg_base > cap - 1) seg_base = cap - 1;
+        s_sched[cap + seg_base] = chunk_base;
+        s_sched[4 * cap + seg_base] = pair_base;
+        hdr[0] = seg_base; hdr[1] = chunk_base; hdr[2] = pair_base;
+        if (bad && blockIdx.x == 0 && p.status) atomicOr(p.status, BM_DEV_BAD_ROUTING);
+    }
+    __syncwarp();
 }
 
 __device__ __forceinline__ float silu_mul(float a, float b) {
@@ -206,7 +259,6 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
     static_assert(!K2 || !kDecode, "CTA pairs are a prefill-tile feature");
     static_assert(!GA || MODE == PF_GEMM1, "the in-kernel gather feeds GEMM1's activation tile");
     static_assert(!FC || MODE == PF_GEMM2 || MODE == DC_GEMM2, "the fused combine is GEMM2's epilogue");
-    static_assert(MODE != DC_GEMM2 || FC, "the decode GEMM2 always finishes its output itself");
     // K2: the two CTAs of a cluster form a CTA pair; rank 0 (the leader) issues the M = 256 MMAs for both
     const uint32_t rank = K2 ? ptx::cluster_ctarank() : 0u;
     const bool leader = rank == 0;
@@ -250,49 +302,60 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
     ptx::tc_fence_after();
     const uint32_t tmem_base = *tmem_ptr;
 
-    const int nkb = p.kblocks;
+    const int kp = kDecode ? p.kpack : 1;                 // k-blocks per ring stage
+    const int nkb = p.kblocks / kp;                       // ring stages of one item
+    const uint32_t mini = kDecode ? (uint32_t)p.mini_bytes : stage_bytes;
     // bytes one stage receives: constant per launch (decode always loads the full padded token box)
     // bytes one stage receives.  Decode: the weight box(es) of R rows plus the item's token rows in 32-row
     // boxes (tok_tx(n)): only the rows the group really has travel from L2.
     // K2: a CTA stages A (16 KB) + its half of B (16 KB); the leader's barrier counts both CTAs' bytes
     const uint32_t w_tx = GA ? 2u * kTileBytes16K : K2 ? 4u * kTileBytes16K : !kDecode ? 3u * kTileBytes16K : (uint32_t)((kGemm1 ? 2 : 1) * p.R * 128);
-    auto stage_tx_of = [&](int n) -> uint32_t { return kDecode ? w_tx + (uint32_t)((n + 31) >> 5) * 4096u : w_tx; };
+    auto stage_tx_of = [&](int n) -> uint32_t { return kDecode ? (uint32_t)kp * (w_tx + (uint32_t)((n + 31) >> 5) * 4096u) : w_tx; };
 
-    // DC_GEMM2: W2 does not depend on the predecessor (GEMM1), so warp 0 fills the ring with the weight tiles
-    // of its first item BEFORE the grid-dependency wait: the HBM stream starts while GEMM1's last CTAs
-    // drain.  The schedule it reads (from global memory) was written by the prep kernel, which completed
-    // before GEMM1 (which triggers this launch only after its own wait) let this grid start.
+    // Schedule (build_schedule): from counts / offsets, which bm_route's kernels wrote.  GEMM1 is their direct
+    // successor and builds it after the grid-dependency wait.  GEMM2 builds it BEFORE the wait: its predecessor GEMM1
+    // let this grid start only after its own wait had returned, i.e. after the routing kernels had completed.
+    // DC_GEMM2: W2 does not depend on GEMM1 either, so warp 0 also fills the ring with the weight tiles of its first
+    // item before the wait: the HBM stream starts while GEMM1's last CTAs drain.
+    int *s_hdr = reinterpret_cast<int *>(gfull + kMaxStages);
+    const int cap = p.seg_cap;
+    SchedView sv;
+    sv.u = s_sched; sv.chunk0 = s_sched + cap; sv.rows = s_sched + 2 * cap; sv.off = s_sched + 3 * cap;
+    sv.pair0 = s_sched + 4 * cap;
     Item it0;
     bool have0 = false;
     int pre = 0;
+    if (!kGemm1 && warp == 0) build_schedule(p, s_sched, cap, s_hdr);
     if (MODE == DC_GEMM2 && warp == 0) {
-        have0 = get_item<MODE, false>(p, sched_global(p.sched), blockIdx.x, it0);
+        sv.n_seg = s_hdr[0]; sv.total_chunks = s_hdr[1]; sv.total_pairs = s_hdr[2];
+        have0 = get_item<MODE, false>(p, sv, blockIdx.x, it0);
         pre = have0 ? min(n_stages, nkb) : 0;
         if (ptx::elect_one())
             for (int kb = 0; kb < pre; ++kb) {
                 ptx::mbar_arrive_expect_tx(&full[kb], stage_tx_of(it0.n));
-                ptx::tma_load_3d(smem + (size_t)kb * stage_bytes, &tm_w0, &full[kb], (it0.ks * nkb + kb) * kBlockK,
-                                 it0.wt * p.R, it0.u, ptx::kEvictFirst);
+                for (int kk = 0; kk < kp; ++kk)
+                    ptx::tma_load_3d(smem + (size_t)kb * stage_bytes + kk * mini, &tm_w0, &full[kb],
+                                     ((it0.ks * nkb + kb) * kp + kk) * kBlockK, it0.wt * p.R, it0.u, ptx::kEvictFirst);
             }
         __syncwarp();
     }
-    grid_dep_wait();
-    // schedule -> shared memory (item enumeration is on the critical path of all three roles)
-    const int cap = p.seg_cap;
-    SchedView sv;
-    sv.n_seg = min(p.sched[0], cap - 1);
-    sv.total_chunks = p.sched[1];
-    sv.total_pairs = p.sched[2];
-    sv.u = s_sched; sv.chunk0 = s_sched + cap; sv.rows = s_sched + 2 * cap; sv.off = s_sched + 3 * cap;
-    sv.pair0 = s_sched + 4 * cap;
-    for (int i = threadIdx.x; i <= sv.n_seg; i += (int)blockDim.x) {
-        s_sched[i] = p.sched[kSchedSegU + i];
-        s_sched[cap + i] = p.sched[kSchedChunk0 + i];
-        s_sched[2 * cap + i] = p.sched[kSchedRows + i];
-        s_sched[3 * cap + i] = p.sched[kSchedOff + i];
-        s_sched[4 * cap + i] = p.sched[kSchedPair0 + i];
+    if (MODE == DC_GEMM1 && warp == 2 && p.pf_bytes) {
+        // The weights do not depend on the routing, and while the router runs HBM is idle: every CTA asks L2 for its
+        // share of the leading pf_bytes of each W1 / W3 set (16 KB pieces, round-robin over the grid) before it waits
+        // for the routing.  Sets that turn out inactive cost idle bandwidth only.
+        const unsigned long long pieces_per_set = p.pf_bytes >> 14;
+        const unsigned long long total = pieces_per_set * 2ull * (unsigned long long)(p.G + p.S);
+        for (unsigned long long i = (unsigned long long)blockIdx.x * 32 + lane; i < total; i += (unsigned long long)gridDim.x * 32) {
+            const unsigned long long set2 = i / pieces_per_set, piece = i - set2 * pieces_per_set;
+            const bm_bf16 *base = (set2 & 1) ? p.w3 : p.w1;
+            const char *addr = reinterpret_cast<const char *>(base) + (set2 >> 1) * p.pf_set_bytes + (piece << 14);
+            ptx::prefetch_l2_bulk(addr, 16384u);
+        }
     }
+    grid_dep_wait();
+    if (kGemm1 && warp == 0) build_schedule(p, s_sched, cap, s_hdr);
     __syncthreads();
+    sv.n_seg = s_hdr[0]; sv.total_chunks = s_hdr[1]; sv.total_pairs = s_hdr[2];
     if (threadIdx.x == 0) grid_dep_launch();
 
     // The producer and the MMA issuer run their loops with the WHOLE warp (warp-uniform control flow keeps
@@ -311,9 +374,10 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
             have = have0;
             if (ptx::elect_one())
                 for (int kb = 0; kb < pre; ++kb)
-                    for (int j = 0; j * 32 < it.n; ++j)
-                        ptx::tma_load_2d(smem + (size_t)kb * stage_bytes + p.off_b + j * 4096, &tm_act0, &full[kb],
-                                         (it.ks * nkb + kb) * kBlockK, it.act_row0 + j * 32, ptx::kEvictLast);
+                    for (int kk = 0; kk < kp; ++kk)
+                        for (int j = 0; j * 32 < it.n; ++j)
+                            ptx::tma_load_2d(smem + (size_t)kb * stage_bytes + kk * mini + p.off_b + j * 4096, &tm_act0, &full[kb],
+                                             ((it.ks * nkb + kb) * kp + kk) * kBlockK, it.act_row0 + j * 32, ptx::kEvictLast);
             __syncwarp();
             kb_first = pre;
             stage = pre;
@@ -324,11 +388,11 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
         auto policy = [](int h) { return h == 0 ? ptx::kEvictFirst : (h == 1 ? ptx::kEvictNormal : ptx::kEvictLast); };
         const uint64_t pol_a = policy(p.hints / 10), pol_w = policy(p.hints % 10);
         for (; have; item += item_stride, have = get_item<MODE, K2>(p, sv, item, it, rank), kb_first = 0) {
-            const CUtensorMap *tm_act = (kGemm1 && it.shared) ? &tm_act1 : &tm_act0;
+            const CUtensorMap *tm_act = (kGemm1 && (it.shared || p.dense)) ? &tm_act1 : &tm_act0;
             const int wrow0 = it.wt * p.R;
-            int kc = (it.ks * nkb + kb_first) * kBlockK;
+            int kc = (it.ks * nkb + kb_first) * kp * kBlockK;
             const uint32_t stage_tx = stage_tx_of(it.n);
-            for (int kb = kb_first; kb < nkb; ++kb, kc += kBlockK) {
+            for (int kb = kb_first; kb < nkb; ++kb, kc += kp * kBlockK) {
                 ptx::mbar_wait(&empty[stage], phase ^ 1);
                 if (K2) {
                     if (ptx::elect_one()) {
@@ -354,12 +418,15 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
                     } else {
                         // M side = R weight rows (streamed once from HBM), N side = the group's token rows
                         // (32-row boxes; rows past the group's within the last box are loaded and never stored)
-                        ptx::tma_load_3d(st, &tm_w0, &full[stage], kc, wrow0, it.u, pol_w);
-                        if (MODE == DC_GEMM1)
-                            ptx::tma_load_3d(st + p.wslot, &tm_w1, &full[stage], kc, wrow0, it.u, pol_w);
-                        for (int j = 0; j * 32 < it.n; ++j)
-                            ptx::tma_load_2d(st + p.off_b + j * 4096, tm_act, &full[stage], kc, it.act_row0 + j * 32,
-                                             pol_a);
+                        for (int kk = 0; kk < kp; ++kk, st += mini) {
+                            const int kcc = kc + kk * kBlockK;
+                            ptx::tma_load_3d(st, &tm_w0, &full[stage], kcc, wrow0, it.u, pol_w);
+                            if (MODE == DC_GEMM1)
+                                ptx::tma_load_3d(st + p.wslot, &tm_w1, &full[stage], kcc, wrow0, it.u, pol_w);
+                            for (int j = 0; j * 32 < it.n; ++j)
+                                ptx::tma_load_2d(st + p.off_b + j * 4096, tm_act, &full[stage], kcc, it.act_row0 + j * 32,
+                                                 pol_a);
+                        }
                     }
                 }
                 __syncwarp();
@@ -390,17 +457,20 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
                 ptx::mbar_wait(&full[stage], phase);
                 ptx::tc_fence_after();
                 if (ptx::elect_one()) {
+                    for (int kk = 0; kk < kp; ++kk) {
+                        const uint32_t a_kk = a_lo + (uint32_t)kk * (mini >> 4);
 #pragma unroll
-                    for (int k = 0; k < kBlockK / 16; ++k) {
-                        const uint32_t accum = (kb | k) ? 1u : 0u;
-                        const uint32_t ko = 2 * k;             // 16 bf16 = 32 bytes = 2 descriptor units
-                        if (K2)
-                            ptx::mma_bf16_ss_pair(d_tmem, ptx::smem_desc(a_lo + ko), ptx::smem_desc(a_lo + b_off + ko), idesc, accum);
-                        else
-                            ptx::mma_bf16_ss(d_tmem, ptx::smem_desc(a_lo + ko), ptx::smem_desc(a_lo + b_off + ko), idesc, accum);
-                        if (MODE == DC_GEMM1)
-                            ptx::mma_bf16_ss(d_tmem + 128, ptx::smem_desc(a_lo + w3_off + ko),
-                                             ptx::smem_desc(a_lo + b_off + ko), idesc, accum);
+                        for (int k = 0; k < kBlockK / 16; ++k) {
+                            const uint32_t accum = (kb | kk | k) ? 1u : 0u;
+                            const uint32_t ko = 2 * k;             // 16 bf16 = 32 bytes = 2 descriptor units
+                            if (K2)
+                                ptx::mma_bf16_ss_pair(d_tmem, ptx::smem_desc(a_kk + ko), ptx::smem_desc(a_kk + b_off + ko), idesc, accum);
+                            else
+                                ptx::mma_bf16_ss(d_tmem, ptx::smem_desc(a_kk + ko), ptx::smem_desc(a_kk + b_off + ko), idesc, accum);
+                            if (MODE == DC_GEMM1)
+                                ptx::mma_bf16_ss(d_tmem + 128, ptx::smem_desc(a_kk + w3_off + ko),
+                                                 ptx::smem_desc(a_kk + b_off + ko), idesc, accum);
+                        }
                     }
                     if (K2) {       // the same barriers in both CTAs
                         ptx::mma_commit_pair(&empty[stage]);
@@ -500,11 +570,22 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
             int tokr[4] = {-1, -1, -1, -1};
             float gwr[4] = {0.f, 0.f, 0.f, 0.f};
             int nsrcr[4] = {0, 0, 0, 0};
-            if (FC) {
+            if (FC || MODE == DC_GEMM2) {
 #pragma unroll
                 for (int j = 0; j < (MODE == DC_GEMM2 ? 4 : 1); ++j) {
                     const int r = MODE == DC_GEMM2 ? j * 32 + lane : row;
-                    if (r < it.n) {
+                    if (r < it.n && p.dense && !it.shared) {
+                        // dense decode: column r is token tok0 + r; it counts only if the token was routed to this set
+                        const int tok = it.tok0 + r;
+                        if (tok < p.T) {
+                            const int ns = min(max(p.n_slots[tok], 0), p.K);
+                            for (int sl = 0; sl < ns; ++sl)
+                                if (p.group_ids[(size_t)tok * p.K + sl] == it.u) {
+                                    tokr[j] = tok;
+                                    gwr[j] = p.gate_w[(size_t)tok * p.K + sl];
+                                }
+                        }
+                    } else if (r < it.n) {
                         int tok, slot = 0;
                         if (it.shared) {
                             tok = it.tok0 + r;
@@ -734,30 +815,39 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
                     }
                 }
                 release_acc();
-                // tickets: piece = (weight tile, 32-row quarter q) over ALL tokens (a decode batch is small); every item
-                // (chunk of any segment, K split) on this weight tile arrives once, total_chunks * ksplit in all.  The
-                // warp that completes a piece finishes it for every token: lane = output feature, 16 tokens per round.
-                // Quarters without a valid output row take no tickets.
-                if (q * 32 < p.R && it.wt * p.R + q * 32 < p.D) {      // warp-uniform
+                // FC: tickets, piece = (weight tile, 32-row quarter q) over ALL tokens (a decode batch is small); every item
+                // (chunk of any segment, K split) on this weight tile arrives once, total_chunks * ksplit in all.  The warp
+                // that completes a piece finishes it for every token.  Quarters without a valid output row take no tickets.
+                // (Taking all tickets once at the end of the kernel instead -- one fence per warp -- was measured slower:
+                // every piece then completes in the kernel's tail.)  Without FC a finalize kernel rounds and clears.
+                if (FC && q * 32 < p.R && it.wt * p.R + q * 32 < p.D) {      // warp-uniform
                     __threadfence();
                     __syncwarp();
                     int last = 0;
                     if (lane == 0) last = atomicAdd(p.tickets + it.wt * 4 + q, 1) == sv.total_chunks * p.ksplit - 1;
                     last = __shfl_sync(kFullMask, last, 0);
                     if (last) {
+                        // lane = (token sub-row lane / 8, four output features 4 * (lane % 8) .. + 3): R is a multiple of 4
+                        // on this kernel, so a 32-feature quarter is made of whole 16-byte pieces; 64 tokens per round
                         __threadfence();
-                        for (int t0 = 0; t0 < p.T; t0 += 16) {
-                            float v[16];
-#pragma unroll
-                            for (int i = 0; i < 16; ++i)
-                                v[i] = (d_ok && t0 + i < p.T) ? __ldcg(p.out_acc + (size_t)(t0 + i) * p.D + d) : 0.0f;
+                        const int dq = it.wt * p.R + q * 32 + 4 * (lane & 7);
+                        const bool q_ok = q * 32 + 4 * (lane & 7) < p.R && dq < p.D;
+                        for (int t0 = lane >> 3; t0 < p.T; t0 += 64) {
+                            float4 v[16];
 #pragma unroll
                             for (int i = 0; i < 16; ++i) {
-                                if (d_ok && t0 + i < p.T) {
-                                    const size_t o = (size_t)(t0 + i) * p.D + d;
-                                    if (p.out_f32) p.out_f32[o] = v[i];
-                                    else p.out[o] = (bm_bf16)f32_to_bf16_bits(v[i]);
-                                    p.out_acc[o] = 0.0f;
+                                const int t = t0 + 4 * i;
+                                v[i] = (q_ok && t < p.T) ? __ldcg(reinterpret_cast<const float4 *>(p.out_acc + (size_t)t * p.D + dq))
+                                                         : make_float4(0.f, 0.f, 0.f, 0.f);
+                            }
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) {
+                                const int t = t0 + 4 * i;
+                                if (q_ok && t < p.T) {
+                                    const size_t o = (size_t)t * p.D + dq;
+                                    if (p.out_f32) *reinterpret_cast<float4 *>(p.out_f32 + o) = v[i];
+                                    else *reinterpret_cast<uint2 *>(p.out + o) = make_uint2(pack_bf16x2(v[i].x, v[i].y), pack_bf16x2(v[i].z, v[i].w));
+                                    *reinterpret_cast<float4 *>(p.out_acc + o) = make_float4(0.f, 0.f, 0.f, 0.f);
                                 }
                             }
                         }
@@ -780,74 +870,16 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
 }
 
 // -------------------------------------------------------------------------------------------------
-// prep: build the schedule, gather token rows into permuted order (step 9)
+// gather (step 9, only for the kernels that take their token rows by TMA from xs: CTA-pair prefill tiles and the
+// decode kernel beyond 64 tokens): one warp per permuted row.  (A tile::gather4 producer in GEMM1 was measured
+// instead of this pass: ~12 cycles per 128-byte row made GEMM1 3x slower.)
 // -------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-prep_kernel(const bm_bf16 *__restrict__ x, int T, int D, int K, int G, int S,
-            const int32_t *__restrict__ counts, const int32_t *__restrict__ offsets,
-            const int32_t *__restrict__ row_token, int32_t *__restrict__ sched, bm_bf16 *__restrict__ xs,
-            int32_t *__restrict__ status) {
+gather_kernel(const bm_bf16 *__restrict__ x, int T, int D, int K, int G, const int32_t *__restrict__ offsets,
+              const int32_t *__restrict__ row_token, bm_bf16 *__restrict__ xs) {
     grid_dep_wait();
     grid_dep_launch();
-    if (blockIdx.x == 0) {
-        // schedule: compact the non-empty segments and prefix-sum their chunk counts.  All rows are fetched in
-        // parallel (one global-memory latency), then warp 0 scans them 32 at a time.
-        __shared__ int s_rows[kMaxSeg], s_off[kMaxSeg];
-        __shared__ int s_bad;
-        const int n = G + S;
-        if (threadIdx.x == 0) s_bad = 0;
-        __syncthreads();
-        for (int u = threadIdx.x; u < n; u += blockDim.x) {
-            int rows = u < G ? counts[u] : T;
-            const int off = u < G ? offsets[u] : 0;
-            if (u < G && (rows < 0 || off < 0 || off + rows > T * K)) { s_bad = 1; rows = 0; }
-            s_rows[u] = rows;
-            s_off[u] = off;
-        }
-        __syncthreads();
-        if (threadIdx.x < 32) {
-            const int lane = threadIdx.x;
-            int seg_base = 0, chunk_base = 0, pair_base = 0;
-            for (int u0 = 0; u0 < n; u0 += 32) {
-                const int u = u0 + lane;
-                const int rows = u < n ? s_rows[u] : 0;
-                const bool ne = rows > 0;
-                const int ch = ne ? (rows + kChunkRows - 1) / kChunkRows : 0;
-                const unsigned m = __ballot_sync(kFullMask, ne);
-                const int seg = seg_base + __popc(m & ((1u << lane) - 1u));
-                const int pr = (ch + 1) >> 1;
-                int inc = ch, incp = pr;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const int v = __shfl_up_sync(kFullMask, inc, o);
-                    const int vp = __shfl_up_sync(kFullMask, incp, o);
-                    if (lane >= o) { inc += v; incp += vp; }
-                }
-                if (ne) {
-                    sched[kSchedSegU + seg] = u;
-                    sched[kSchedChunk0 + seg] = chunk_base + inc - ch;
-                    sched[kSchedRows + seg] = rows;
-                    sched[kSchedOff + seg] = s_off[u];
-                    sched[kSchedPair0 + seg] = pair_base + incp - pr;
-                }
-                seg_base += __popc(m);
-                chunk_base += __shfl_sync(kFullMask, inc, 31);
-                pair_base += __shfl_sync(kFullMask, incp, 31);
-            }
-            if (lane == 0) {
-                sched[kSchedChunk0 + seg_base] = chunk_base;
-                sched[kSchedPair0 + seg_base] = pair_base;
-                sched[0] = seg_base;
-                sched[1] = chunk_base;
-                sched[2] = pair_base;
-                if (s_bad) atomicOr(status, BM_DEV_BAD_ROUTING);
-            }
-        }
-    }
-    // gather: one warp per permuted row.  (A tile::gather4 producer in GEMM1 was measured instead of this
-    // pass: ~12 cycles per 128-byte row made GEMM1 3x slower, so the rows are materialised once here.)
-    if (!xs) return;                     // prefill tiles: GEMM1 gathers the rows itself (GA)
-    const int A = min(offsets[G], T * K);
+    const int A = min(max(offsets[G], 0), T * K);
     const int warps = (gridDim.x * blockDim.x) >> 5;
     const int lane = threadIdx.x & 31;
     const int vec = D / 8;
@@ -860,35 +892,24 @@ prep_kernel(const bm_bf16 *__restrict__ x, int T, int D, int K, int G, int S,
     }
 }
 
+// out = bf16(acc) (or a copy into out_f32).  clear != 0: acc is the zero region's accumulator and is put back to zero
+// (decode beyond 64 tokens, where the in-kernel finish costs more than this pass).
 __global__ void __launch_bounds__(256)
-finalize_kernel(const float *__restrict__ out_acc, bm_bf16 *__restrict__ out, size_t n8) {
+finalize_kernel(float *__restrict__ acc, bm_bf16 *__restrict__ out, float *__restrict__ out_f32, size_t n8, int clear) {
     grid_dep_wait();
     grid_dep_launch();
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n8; i += (size_t)gridDim.x * blockDim.x) {
-        const float4 a = reinterpret_cast<const float4 *>(out_acc)[2 * i];
-        const float4 b = reinterpret_cast<const float4 *>(out_acc)[2 * i + 1];
-        reinterpret_cast<uint4 *>(out)[i] = make_uint4(pack_bf16x2(a.x, a.y), pack_bf16x2(a.z, a.w),
-                                                       pack_bf16x2(b.x, b.y), pack_bf16x2(b.z, b.w));
-    }
-}
-
-// Schedule of the all-experts forward (calibration, NEXT-2): E segments of T rows each, every one a "shared"
-// segment (weight set j on every token), so GEMM1 reads x directly and GEMM2 writes y row j*T + t.
-__global__ void __launch_bounds__(256)
-dense_sched_kernel(int32_t *__restrict__ sched, int E, int T) {
-    grid_dep_wait();
-    grid_dep_launch();
-    const int cps = (T + kChunkRows - 1) / kChunkRows;
-    for (int j = threadIdx.x; j <= E; j += blockDim.x) {
-        sched[kSchedChunk0 + j] = j * cps;
-        sched[kSchedPair0 + j] = j * ((cps + 1) >> 1);
-        if (j < E) {
-            sched[kSchedSegU + j] = j;
-            sched[kSchedRows + j] = T;
-            sched[kSchedOff + j] = 0;
+        float4 *src = reinterpret_cast<float4 *>(acc) + 2 * i;
+        const float4 a = src[0], b = src[1];
+        if (out_f32) {
+            reinterpret_cast<float4 *>(out_f32)[2 * i] = a;
+            reinterpret_cast<float4 *>(out_f32)[2 * i + 1] = b;
+        } else {
+            reinterpret_cast<uint4 *>(out)[i] = make_uint4(pack_bf16x2(a.x, a.y), pack_bf16x2(a.z, a.w),
+                                                           pack_bf16x2(b.x, b.y), pack_bf16x2(b.z, b.w));
         }
+        if (clear) { src[0] = make_float4(0.f, 0.f, 0.f, 0.f); src[1] = make_float4(0.f, 0.f, 0.f, 0.f); }
     }
-    if (threadIdx.x == 0) { sched[0] = E; sched[1] = E * cps; sched[2] = E * ((cps + 1) >> 1); }
 }
 
 // Prefill combine (F2): out[t] = sum_{s < n_slots[t]} gate_w[t,s] * y[slot_row[t,s]]  (slot order)
@@ -1092,6 +1113,7 @@ void choose_decode_tiling(int wrows, int kblocks, int n_seg, bool allow_split, i
         if (ks > 1 && (kblocks % ks != 0 || kblocks / ks < 4)) continue;
         if (ks_force > 0 && ks != ks_force && kblocks % ks_force == 0 && kblocks / ks_force >= 4) continue;
         for (int R = rmax; R >= 32; --R) {
+            if (mats == 1 && (R & 3)) continue;      // GEMM2: whole 16-byte pieces per 32-row quarter (the fused finish)
             const double t = decode_time_model(wrows, kblocks, n_seg, R, ks, mats, sms);
             if (t < best * 0.99) { best = t; bestR = R; bestKs = ks; }   // within 1%: keep the larger tile
         }
@@ -1120,11 +1142,19 @@ void ring_geometry(bool decode, bool gemm1, int T, GemmParams *p, bool pair = fa
         const int tok_bytes = ((rows + 31) & ~31) * 128;
         p->wslot = (p->R * 128 + 1023) & ~1023;
         p->off_b = (gemm1 ? 2 : 1) * p->wslot;
-        p->stage_bytes = p->off_b + tok_bytes;
+        p->mini_bytes = p->off_b + tok_bytes;
+        const int kp_opt = opt(OPT_DC_KPACK);
+        p->kpack = (kp_opt >= 1 && kp_opt <= 2 ? kp_opt : 2);
+        if (p->kblocks % p->kpack != 0) p->kpack = 1;
+        p->stage_bytes = p->kpack * p->mini_bytes;
         const int behind = p->wslot + tok_bytes;
         p->tail_pad = behind >= kTileBytes16K ? 0 : kTileBytes16K - behind;
     }
     const size_t fixed = (decode ? 0 : kSmemEpi) + sched_smem_bytes(p->seg_cap) + (size_t)p->tail_pad;
+    if (decode && p->kpack == 2 && (kSmemRing - fixed) / (size_t)p->stage_bytes < 3) {     // keep at least a 3-deep ring
+        p->kpack = 1;
+        p->stage_bytes = p->mini_bytes;
+    }
     int st = (int)((kSmemRing - fixed) / (size_t)p->stage_bytes);
     const int cap = opt(decode ? OPT_DC_STAGES : OPT_PF_STAGES);
     if (st > cap) st = cap;
@@ -1204,7 +1234,7 @@ static void decode_tiling(int T, int D, int F, int K, int G, int S, int *R1, int
     int ks1;
     choose_decode_tiling(F, kb1, n_seg, false, 2, num_sms(), R1, &ks1);
     choose_decode_tiling(D, kb2, n_seg, true, 1, num_sms(), R2, ks2);
-    if (opt(OPT_DC_R2) > 0) { *R2 = opt(OPT_DC_R2); *ks2 = opt(OPT_DC_KS2); }
+    if (opt(OPT_DC_R2) > 0) { *R2 = std::max(32, std::min(128, opt(OPT_DC_R2)) & ~3); *ks2 = std::max(1, opt(OPT_DC_KS2)); }
     if (opt(OPT_DC_R1) > 0) *R1 = opt(OPT_DC_R1);
 }
 
@@ -1221,7 +1251,10 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
     // Combine: fused into the GEMM2 epilogue (fp32 reductions into the zero region + last-arriver rounding) unless
     // option FUSED_COMBINE = 0 asks for the two-pass form on the prefill tiles (bf16 y rows + combine_kernel, slot
     // order: bit-deterministic for any K + S).  The decode kernel always finishes its output itself.
-    const bool fused = decode || opt(OPT_FUSED_COMBINE) != 0;
+    // The decode kernel finishes its output itself up to 64 tokens; beyond, its items are so short that the fence and
+    // ticket per item cost more than a separate pass (G = 60, T = 256: 218 us fused, 185 us with the finalize kernel).
+    const int fc_opt = opt(OPT_FUSED_COMBINE);
+    const bool fused = decode ? (fc_opt < 0 ? a.T <= kDenseMaxT : fc_opt != 0) : fc_opt != 0;
 
     // CTA pairs (cta_group::2, M = 256 per pair): a pair shares the weight tile, so a CTA stages 32 KB per
     // k-block instead of 48 KB (measured: GEMM1 232 -> 201 us at BJ:configs[3]).  A segment with an odd chunk
@@ -1232,34 +1265,39 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
     const int pair_env = opt(OPT_PF_PAIR);
     const bool many_rows = (long long)a.T * a.K >= 3LL * kChunkRows * a.G;
     const bool pair = !decode && (sms & 1) == 0 && (pair_env < 0 ? many_rows : pair_env != 0);
-    // GA: GEMM1's own warps gather the token rows (single-CTA prefill tiles); the prep kernel then only builds the
-    // schedule.  Measured (T = 4096, G = 60): step 410 -> 398 us (GEMM1 +14 us, gather pass -20 us, A*D*4 bytes of
-    // HBM traffic less).  Not with CTA pairs: the peer's "rows landed" must reach the leader's barrier through a
-    // fence and a cluster-scope arrive per k-block, which lengthens the ring's turn-around -- GEMM1 30-36% slower
-    // than the TMA-fed pair kernel even with one relay warp per ring stage (BM_PF_GATHER=2 forces it).
+    // GA: GEMM1's own warps gather the token rows (single-CTA prefill tiles).  Measured (T = 4096, G = 60): step
+    // 410 -> 398 us (GEMM1 +14 us, gather pass -20 us, A*D*4 bytes of HBM traffic less).  Not with CTA pairs: the peer's
+    // "rows landed" must reach the leader's barrier through a fence and a cluster-scope arrive per k-block, which
+    // lengthens the ring's turn-around -- GEMM1 30-36% slower than the TMA-fed pair kernel even with one relay warp
+    // per ring stage (option PF_GATHER = 2 forces it).
     const int ga_env = opt(OPT_PF_GATHER);
     const bool gather_in_gemm = !decode && (ga_env == 2 || (ga_env == 1 && !pair));
+    // Dense decode (T <= DC_DENSE_MAX_T = 64): every active weight set multiplies ALL T tokens (the MMA N side is the
+    // token block of x itself, <= 64 columns: free under the weight stream) and GEMM2's epilogue weighs token t of
+    // set u with its gate weight, zero where t was not routed to u.  No gathered copy of x, no dependence on the
+    // permutation: the step is router (+ permutation for the API) -> GEMM1 -> GEMM2.
+    const bool dense = decode && a.T <= std::min(opt(OPT_DC_DENSE_MAX_T), kDenseMaxT);
 
-    // step 9 (+ schedule, + zero)
-    {
-        const int grid = sms * 4;
+    // step 9 for the kernels that read token rows from xs
+    if (!gather_in_gemm && !dense && TK > 0) {
         profile_begin(BM_KERNEL_PREP, stream);
-        cudaError_t e = launch_kernel(prep_kernel, dim3(grid), dim3(256), 0, stream, a.x, a.T, a.D, a.K, a.G, a.S,
-                                      a.r.counts, a.r.offsets, a.r.row_token, a.sched, gather_in_gemm ? nullptr : a.xs, a.status);
+        cudaError_t e = launch_kernel(gather_kernel, dim3(sms * 4), dim3(256), 0, stream, a.x, a.T, a.D, a.K, a.G,
+                                      (const int32_t *)a.r.offsets, (const int32_t *)a.r.row_token, a.xs);
         if (e != cudaSuccess) return e;
         profile_end(BM_KERNEL_PREP, stream);
     }
 
     GemmParams p{};
     p.hints = 20;            // activations evict_last, weights evict_first (decode: the weights stream once)
+    p.dense = dense ? 1 : 0;
+    p.status = a.status;
     p.seg_cap = a.G + a.S + 1;
     p.T = a.T; p.D = a.D; p.F = a.F; p.K = a.K; p.G = a.G; p.S = a.S; p.TK = TK;
     p.counts = a.r.counts; p.offsets = a.r.offsets; p.row_token = a.r.row_token; p.row_slot = a.r.row_slot;
-    p.gate_w = a.r.gate_w; p.n_slots = a.r.n_slots; p.sched = a.sched; p.h = a.h; p.out_acc = a.out_acc; p.tickets = a.tickets;
+    p.gate_w = a.r.gate_w; p.n_slots = a.r.n_slots; p.group_ids = a.r.group_ids; p.h = a.h; p.out_acc = a.out_acc; p.tickets = a.tickets;
     p.y = a.y; p.x = a.x; p.out = a.out; p.out_f32 = a.out_f32;
 
-
-    const uint64_t h_rows = (uint64_t)TK + (uint64_t)a.S * a.T;
+    const uint64_t h_rows = h_rows_needed(a.T, a.K, a.G, a.S);
     const int kb1 = (a.D + kBlockK - 1) / kBlockK, kb2 = (a.F + kBlockK - 1) / kBlockK;
     CUtensorMap m_xs, m_x, m_w1, m_w3, m_w2, m_h;
     cudaError_t err;
@@ -1312,10 +1350,27 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
             return cudaErrorInvalidValue;
         p.ksplit = 1; p.kblocks = kb1; p.R = R1; p.n_wtiles = (a.F + R1 - 1) / R1;
         ring_geometry(true, true, a.T, &p);
+        {
+            // L2 prefetch budget (option DC_PREFETCH_MB, default 48 MB): spread evenly over the W1 / W3 sets, whole 16 KB pieces
+            const unsigned long long set_bytes = (unsigned long long)a.F * a.D * 2ull;
+            unsigned long long per = ((unsigned long long)std::max(opt(OPT_DC_PREFETCH_MB), 0) << 20) / (2ull * (a.G + a.S));
+            if (per > set_bytes) per = set_bytes;
+            p.w1 = a.W1; p.w3 = a.W3; p.pf_set_bytes = set_bytes; p.pf_bytes = per & ~16383ull;
+        }
         if ((err = launch_gemm<DC_GEMM1>(m_xs, m_x, m_w1, m_w3, p, stream)) != cudaSuccess) return err;
         p.ksplit = ks2; p.kblocks = kb2 / ks2; p.R = R2; p.n_wtiles = (a.D + R2 - 1) / R2;
         ring_geometry(true, false, a.T, &p);
-        if ((err = launch_gemm<DC_GEMM2, false, false, true>(m_h, m_h, m_w2, m_w2, p, stream)) != cudaSuccess) return err;
+        err = fused ? launch_gemm<DC_GEMM2, false, false, true>(m_h, m_h, m_w2, m_w2, p, stream)
+                    : launch_gemm<DC_GEMM2>(m_h, m_h, m_w2, m_w2, p, stream);
+        if (err != cudaSuccess) return err;
+        if (!fused) {
+            const size_t n8 = (size_t)a.T * a.D / 8;
+            int grid = (int)std::min<size_t>((n8 + 255) / 256, (size_t)sms * 8);
+            profile_begin(BM_KERNEL_FINALIZE, stream);
+            err = launch_kernel(finalize_kernel, dim3(grid < 1 ? 1 : grid), dim3(256), 0, stream, a.out_acc, a.out, a.out_f32, n8, 1);
+            profile_end(BM_KERNEL_FINALIZE, stream);
+        }
+        return err;
     }
 
     if (fused) return cudaSuccess;
@@ -1328,15 +1383,13 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
 // f_e(x_t) for every expert and token (calibration forward): the prefill GEMM kernels over a
 // dense schedule (G = 0 routed groups, S = E always-on weight sets); y: [E, T, D] bf16.
 cudaError_t launch_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 *W1, const bm_bf16 *W3,
-                                  const bm_bf16 *W2, int E, int F, bm_bf16 *y, int32_t *sched, bm_bf16 *h,
-                                  cudaStream_t stream) {
-    cudaError_t err = launch_kernel(dense_sched_kernel, dim3(1), dim3(256), 0, stream, sched, E, T);
-    if (err != cudaSuccess) return err;
+                                  const bm_bf16 *W2, int E, int F, bm_bf16 *y, bm_bf16 *h, cudaStream_t stream) {
+    cudaError_t err;
     GemmParams p{};
     p.hints = 20;
     p.seg_cap = E + 1;
     p.T = T; p.D = D; p.F = F; p.K = 1; p.G = 0; p.S = E; p.TK = 0;
-    p.sched = sched; p.h = h; p.y = y; p.x = x;
+    p.h = h; p.y = y; p.x = x;
     p.ksplit = 1;
     const bool pair = (num_sms() & 1) == 0 && T >= 3 * kChunkRows && opt(OPT_PF_PAIR) != 0;   // as launch_forward_tc
     CUtensorMap m_x, m_w1, m_w3, m_w2, m_h;
@@ -1356,7 +1409,8 @@ cudaError_t launch_round_bf16(const float *in, size_t n, bm_bf16 *out, cudaStrea
     long long grid = (long long)((n8 + 255) / 256);
     if (grid > num_sms() * 8) grid = num_sms() * 8;
     if (grid < 1) grid = 1;
-    return launch_kernel(finalize_kernel, dim3((unsigned)grid), dim3(256), 0, stream, in, out, n8);
+    return launch_kernel(finalize_kernel, dim3((unsigned)grid), dim3(256), 0, stream, const_cast<float *>(in), out,
+                         (float *)nullptr, n8, 0);
 }
 
 }  // namespace bm
