@@ -862,6 +862,8 @@ def main():
     ap.add_argument("--out", default="", help="also write the sweep result to this file")
     ap.add_argument("--parallel", default="dp", choices=["dp", "tp"],
                     help="N > 1: dp = tokens sharded, no collective (default); tp = F sharded + all-reduce (P:289-295)")
+    ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
+                    help="library option for this run (include/bm.h: bm_set_option), e.g. --opt ROUTER_FILTER=0; repeatable")
     ap.add_argument("--no-extras", action="store_true", help="skip the ungrouped / prefill side measurements")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()
@@ -875,6 +877,11 @@ def main():
     else:
         if not torch.cuda.is_available():
             raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+        if args.opt:
+            import paper_2607_04164_b200 as bm
+            for kv in args.opt:
+                name, _, val = kv.partition("=")
+                bm.set_option(name, int(val))
         if args.config == "sweep":
             run_sweep(args)
         elif args.config == "next":

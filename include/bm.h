@@ -192,8 +192,8 @@ int bm_group_mse(const bm_bf16 *Y, const bm_bf16 *U, int T, int D, const int32_t
  *     kernel (4)).  fp32 addition is commutative, so the result is bit-deterministic when no token has more than two
  *     source rows (K + S <= 2, and no K split on the decode path); with more sources the order of the additions, hence
  *     the last bits before the bf16 rounding, may vary between calls.  bm_forward_info tells which case a call is in.
- *   - matrix-vector path and the two-pass prefill form (option FUSED_COMBINE = 0): slot order, bit-deterministic;
- *     the two-pass form rounds the per-row expert outputs y to bf16 before the sum.
+ *   - matrix-vector path and the two-pass prefill form (F < 4096 by default, or option FUSED_COMBINE = 0): slot order,
+ *     bit-deterministic; the two-pass form rounds the per-row expert outputs y to bf16 before the sum.
  *   x        [T,D]      bf16
  *   routing  as produced by bm_route (or any arrays satisfying the same invariants), same T
  *   W1, W3   [G+S,F,D]  bf16 (united experts 0..G-1, then the S always-on shared experts, A11)
@@ -298,7 +298,9 @@ int bm_device_status(void *workspace, int32_t *host_out, bm_stream_t stream);
  * environment variable BM_<NAME> read ONCE when the library is first used; afterwards only bm_set_option changes it
  * (no call reads the environment).  BM_ERR_SHAPE for an unknown name.
  *   PDL (1)                 programmatic dependent launch between the kernels of a call
- *   FUSED_COMBINE (-1)      prefill tiles: 0 = two-pass combine (bf16 y rows + slot-order sum, deterministic), else fused
+ *   FUSED_COMBINE (-1)      1 = combine fused into the W2 GEMM epilogue, 0 = separate pass (prefill tiles: bf16 y rows +
+ *                           slot-order sum, deterministic; decode kernel: finalize pass); -1 = by shape: prefill tiles fused
+ *                           from F = 4096 on, decode kernel up to 64 tokens
  *   PF_PAIR (-1)            prefill tiles: 1 / 0 force CTA pairs (cta_group::2) on / off, -1 = by rows per group
  *   PF_GATHER (1)           0 = materialise gathered rows, 1 = gather inside GEMM1 on single-CTA tiles, 2 = also with pairs
  *   PF_G1_BC, PF_G2_BC, PF_G2_BW (-1)   prefill tiles: L2 bands of the item order -- chunk units per band in GEMM1 / GEMM2,
@@ -312,6 +314,8 @@ int bm_device_status(void *workspace, int32_t *host_out, bm_stream_t stream);
  *   GEMV_FUSE (1)           matrix-vector path: fuse the W2 stage with the combine
  *   DC_R1, DC_R2, DC_KS2, DC_RMAX, DC_KS_FORCE (0, 0, 1, 128, 0)   decode tiling overrides (rows per tile, K splits)
  *   DC_STAGES, PF_STAGES (12)   cap on the shared-memory ring depth
+ *   ROUTER_FILTER (1)       T >= 512, E <= 256, K <= 8: tensor-core filter + canonical refinement of the candidates; 0 = all E dots
+ *   DC_KPACK (2)            decode kernels: k-blocks per ring stage
  *   COMBINE_WARPS (64), PERM_SMALL_WARPS (0), ROUTER_WE (0), ROUTER_TP_MIN_T (512), ROUTER_SPLIT_MAX_T (16)
  *                           shape thresholds of the small kernels
  */

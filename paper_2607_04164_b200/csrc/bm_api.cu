@@ -36,7 +36,7 @@ static const OptDef kOptDefs[OPT_COUNT] = {
     {"GEMV_ROWS", 1}, {"GEMV_MAX_T", 2}, {"GEMV_FUSE", 1}, {"DC_RMAX", 128}, {"DC_KS_FORCE", 0}, {"DC_STAGES", 12},
     {"PF_STAGES", 12}, {"DC_R1", 0}, {"DC_R2", 0}, {"DC_KS2", 1}, {"PF_PAIR", -1}, {"PF_GATHER", 1},
     {"COMBINE_WARPS", 64}, {"PERM_SMALL_WARPS", 0}, {"ROUTER_WE", 0}, {"ROUTER_TP_MIN_T", kSplitRouterMaxT},
-    {"ROUTER_SPLIT_MAX_T", 16}, {"FUSED_COMBINE", -1}, {"PF_G1_BC", -1}, {"PF_G2_BC", -1}, {"PF_G2_BW", -1}, {"PF_G1_HINTS", -1}, {"PF_G2_HINTS", -1}, {"DC_DENSE_MAX_T", kDenseMaxT}, {"DC_PREFETCH_MB", 48}, {"DC_KPACK", 2},
+    {"ROUTER_SPLIT_MAX_T", 16}, {"FUSED_COMBINE", -1}, {"PF_G1_BC", -1}, {"PF_G2_BC", -1}, {"PF_G2_BW", -1}, {"PF_G1_HINTS", -1}, {"PF_G2_HINTS", -1}, {"DC_DENSE_MAX_T", kDenseMaxT}, {"DC_PREFETCH_MB", 48}, {"DC_KPACK", 2}, {"ROUTER_FILTER", 1},
 };
 static int g_opt[OPT_COUNT];
 static bool init_options() {
@@ -461,7 +461,11 @@ int bm_forward_info(int T, int K, int G, int S, int D, int F, int *path, int *de
     if (T < 0 || K < 1 || K > BM_MAX_K || G < 1 || G > BM_MAX_G || S < 0 || S > BM_MAX_S || D < 8 || F < 8) return BM_ERR_SHAPE;
     const int pth = resolve_auto_path(T, K, G);
     int det = 1;
-    if (pth == BM_PATH_PREFILL) det = (opt(OPT_FUSED_COMBINE) == 0 || K + S <= 2) ? 1 : 0;
+    if (pth == BM_PATH_PREFILL) {
+        const int fc = opt(OPT_FUSED_COMBINE);
+        const bool fused = fc < 0 ? F >= 4096 : fc != 0;          // as launch_forward_tc
+        det = (!fused || K + S <= 2) ? 1 : 0;
+    }
     else if (pth == BM_PATH_DECODE) det = ((K + S) * decode_ksplit(T, D, F, K, G, S) <= 2) ? 1 : 0;   // fp32 reds either way
     if (path) *path = pth;
     if (deterministic) *deterministic = det;

@@ -24,7 +24,7 @@ struct Workspace {
                          // router), [64..64+512) expert slices done per token (split router); zeroed once by the caller,
                          // the counters are put back to zero by the kernel that used them
     size_t block_hist;   // int32[nb * G]   per-block group histograms / bases of the permutation
-    size_t route_logits; // f32[min(T, 512) * BM_MAX_E]  logits of the split router (T < 512), gathered by a token's last CTA
+    size_t route_logits; // router scratch: logits of the split router (T < 512) / row norms and candidate masks of the filter router
     size_t sched;        // int32[kSchedInts] tile-schedule scratch of the forward pass
     size_t xs;           // bf16[T*K, D]    token rows gathered in permuted order (CTA-pair prefill and decode kernels)
     size_t h;            // bf16[T*K + S*T, F]  SwiGLU intermediate
@@ -68,7 +68,11 @@ __host__ inline Workspace workspace_layout(int T, int D, int F, int K, int G, in
     const size_t nb = (items + kPermItemsPerBlock - 1) / kPermItemsPerBlock;
     w.status = off;      off = align_up(off + kStatusInts * sizeof(int32_t), 1024);
     w.block_hist = off;  off = align_up(off + (nb > 0 ? nb : 1) * (size_t)G * sizeof(int32_t), 1024);
-    w.route_logits = off; off = align_up(off + (size_t)(T < kSplitRouterMaxT ? T : kSplitRouterMaxT) * BM_MAX_E * sizeof(float), 1024);
+    {   // split router (T < 512): logits [T][E]; filter router (T >= 512): row norms [T + E] and candidate masks [T][8]
+        const size_t split = (size_t)(T < kSplitRouterMaxT ? T : kSplitRouterMaxT) * BM_MAX_E * sizeof(float);
+        const size_t filter = ((size_t)T + BM_MAX_E + 4) * sizeof(float) + (size_t)T * 8 * sizeof(uint32_t);
+        w.route_logits = off; off = align_up(off + (split > filter ? split : filter), 1024);
+    }
     w.sched = off;       off = align_up(off + kSchedInts * sizeof(int32_t), 1024);
     w.xs = off;          off = align_up(off + items * D * sizeof(bm_bf16), 1024);
     w.h = off;           off = align_up(off + h_rows_needed(T, K, G, S) * F * sizeof(bm_bf16), 1024);
@@ -117,7 +121,7 @@ enum Opt {
     OPT_PDL, OPT_DECODE_MAX_T, OPT_DECODE_MID_T, OPT_DECODE_ROWS, OPT_DECODE_MID_ROWS, OPT_GEMV_ROWS, OPT_GEMV_MAX_T,
     OPT_GEMV_FUSE, OPT_DC_RMAX, OPT_DC_KS_FORCE, OPT_DC_STAGES, OPT_PF_STAGES, OPT_DC_R1, OPT_DC_R2, OPT_DC_KS2,
     OPT_PF_PAIR, OPT_PF_GATHER, OPT_COMBINE_WARPS, OPT_PERM_SMALL_WARPS, OPT_ROUTER_WE, OPT_ROUTER_TP_MIN_T,
-    OPT_ROUTER_SPLIT_MAX_T, OPT_FUSED_COMBINE, OPT_PF_G1_BC, OPT_PF_G2_BC, OPT_PF_G2_BW, OPT_PF_G1_HINTS, OPT_PF_G2_HINTS, OPT_DC_DENSE_MAX_T, OPT_DC_PREFETCH_MB, OPT_DC_KPACK, OPT_COUNT
+    OPT_ROUTER_SPLIT_MAX_T, OPT_FUSED_COMBINE, OPT_PF_G1_BC, OPT_PF_G2_BC, OPT_PF_G2_BW, OPT_PF_G1_HINTS, OPT_PF_G2_HINTS, OPT_DC_DENSE_MAX_T, OPT_DC_PREFETCH_MB, OPT_DC_KPACK, OPT_ROUTER_FILTER, OPT_COUNT
 };
 int opt(Opt o);
 

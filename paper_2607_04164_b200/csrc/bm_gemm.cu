@@ -1198,6 +1198,10 @@ cudaError_t launch_gemm(const CUtensorMap &a0, const CUtensorMap &a1, const CUte
 
 // [rows, cols] bf16 row-major, box = box_rows x box_cols, no swizzle (rows of a box are contiguous in shared
 // memory); out-of-bounds elements are zero-filled.  Used by the router's slab ring.
+bool make_map_2d_sw128(CUtensorMap *m, const void *base, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+    return make_map_2d(m, base, rows, cols, box_rows);
+}
+
 bool make_map_2d_plain(CUtensorMap *m, const void *base, uint64_t rows, uint64_t cols, uint32_t box_rows,
                        uint32_t box_cols) {
     return encode_map(m, MapKey{base, cols, rows, 0, box_cols, box_rows, 0});
@@ -1253,8 +1257,12 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
     // order: bit-deterministic for any K + S).  The decode kernel always finishes its output itself.
     // The decode kernel finishes its output itself up to 64 tokens; beyond, its items are so short that the fence and
     // ticket per item cost more than a separate pass (G = 60, T = 256: 218 us fused, 185 us with the finalize kernel).
+    // Prefill tiles: the fused epilogue (scale, transpose, vector reductions, fence, ticket, finish) takes ~10 us per
+    // 128 x 256 tile and hides behind the tile's main loop only when the W2 reduction is long: fused from F = 4096 on
+    // (Mixtral: 56 us per tile; also where the outputs are large enough for the fp32 sum to matter against the
+    // tolerance), the two-pass form below (Qwen-like F = 1408: 6 us per tile; measured 5-10% faster there).
     const int fc_opt = opt(OPT_FUSED_COMBINE);
-    const bool fused = decode ? (fc_opt < 0 ? a.T <= kDenseMaxT : fc_opt != 0) : fc_opt != 0;
+    const bool fused = decode ? (fc_opt < 0 ? a.T <= kDenseMaxT : fc_opt != 0) : (fc_opt < 0 ? a.F >= 4096 : fc_opt != 0);
 
     // CTA pairs (cta_group::2, M = 256 per pair): a pair shares the weight tile, so a CTA stages 32 KB per
     // k-block instead of 48 KB (measured: GEMM1 232 -> 201 us at BJ:configs[3]).  A segment with an odd chunk
@@ -1321,7 +1329,9 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
         // PF_G1_BC, PF_G2_BC, PF_G2_BW; get_item).
         p.band_c = opt(OPT_PF_G1_BC) > 0 ? opt(OPT_PF_G1_BC) : 0;
         p.band_w = 0;
-        p.hints = opt(OPT_PF_G1_HINTS) >= 0 ? opt(OPT_PF_G1_HINTS) : 21;
+        // (with single-CTA tiles a group has at most ~2 chunks: its weights stream once -> evict_first, as on the decode path;
+        //  G = 8, T = 256: 69 -> 64 us)
+        p.hints = opt(OPT_PF_G1_HINTS) >= 0 ? opt(OPT_PF_G1_HINTS) : (pair ? 21 : 20);
         if (gather_in_gemm)
             err = pair ? launch_gemm<PF_GEMM1, true, true>(m_xs, m_x, m_w1, m_w3, p, stream)
                        : launch_gemm<PF_GEMM1, false, true>(m_xs, m_x, m_w1, m_w3, p, stream);
@@ -1332,7 +1342,7 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
         p.kblocks = kb2; p.R = 256; p.n_wtiles = (a.D + 255) / 256;
         p.band_w = opt(OPT_PF_G2_BW) > 0 ? opt(OPT_PF_G2_BW) : 0;
         p.band_c = opt(OPT_PF_G2_BC) > 0 ? opt(OPT_PF_G2_BC) : 0;
-        p.hints = opt(OPT_PF_G2_HINTS) >= 0 ? opt(OPT_PF_G2_HINTS) : 21;
+        p.hints = opt(OPT_PF_G2_HINTS) >= 0 ? opt(OPT_PF_G2_HINTS) : (pair ? 21 : 20);
         if (fused)
             err = pair ? launch_gemm<PF_GEMM2, true, false, true>(m_h, m_h, m_w2h, m_w2h, p, stream)
                        : launch_gemm<PF_GEMM2, false, false, true>(m_h, m_h, m_w2, m_w2, p, stream);

@@ -12,6 +12,9 @@ namespace bm {
 bool make_map_2d_plain(CUtensorMap *m, const void *base, uint64_t rows, uint64_t cols, uint32_t box_rows,
                        uint32_t box_cols);
 
+// host: 2-D tensor map over a row-major bf16 matrix, box = box_rows x 64 columns, 128-byte swizzle (bm_gemm.cu)
+bool make_map_2d_sw128(CUtensorMap *m, const void *base, uint64_t rows, uint64_t cols, uint32_t box_rows);
+
 namespace ptx {
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) {

@@ -576,6 +576,327 @@ cudaError_t launch_tp(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const f
                          gm, WT, WE, n_blocks, r.expert_ids, r.group_ids, r.gate_w, r.n_slots, status);
 }
 
+// -------------------------------------------------------------------------------------------------
+// Filter + refine (T >= 512, E <= 256, K <= 8).  The canonical fp32 dot products decide the routing bit for bit, but
+// only the K largest of a token's E logits matter, so:
+//   1. row_norm_kernel    |x_t| and |Wr_e| (one warp per row)
+//   2. router_filter_kernel   approximate logits a[t,e] = x_t . Wr_e on the tensor cores (tcgen05, bf16 products are exact,
+//      fp32 accumulation in the hardware's order), tau_t = the K-th largest a[t,.] + bias, and the candidate set
+//          C_t = { e : a[t,e] + bias_e >= tau_t - 2 beta[t,e] },   beta[t,e] = kappa |x_t| |Wr_e|
+//      where beta bounds |a[t,e] - canonical logit|: both are fp32 evaluations of the same sum of exact products, each
+//      within (number of additions) * 2^-23 * sum_i |x_i w_i| <= D 2^-23 |x_t| |Wr_e| of the real value (Cauchy-Schwarz);
+//      kappa = 2 D 2^-23 + 2^-18 leaves a factor of two and room for the bias addition.
+//      Every e outside C_t has canonical logit < tau_t - beta <= the canonical logit of each of the K experts with the
+//      largest a[t,.], so it cannot be among the canonical top-K: the refinement over C_t alone is exact, ties included.
+//      A token with a non-finite a[t,.] keeps all E experts.
+//   3. router_refine_kernel   canonical dots (A1) for the candidates only -- K + ~0.1 of E = 60 -- then R2-R5 as everywhere.
+// The FMA work falls from T E D to ~T K D (T = 4096, E = 60: 51 -> ~15 us for the whole routing step).
+// -------------------------------------------------------------------------------------------------
+constexpr int kFlThreads = 192;
+constexpr int kFlMaxE = 256, kFlMaxK = 8;
+constexpr int kFlXTile = 128 * 128;                 // bytes: 128 token rows x 64 bf16
+
+__global__ void __launch_bounds__(256)
+row_norm_kernel(const bm_bf16 *__restrict__ x, int T, const bm_bf16 *__restrict__ Wr, int E, int D, float *__restrict__ norms) {
+    grid_dep_wait();
+    grid_dep_launch();
+    const int lane = threadIdx.x & 31;
+    const int warps = (gridDim.x * blockDim.x) >> 5;
+    for (int r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; r < T + E; r += warps) {
+        const uint4 *row = reinterpret_cast<const uint4 *>(r < T ? x + (size_t)r * D : Wr + (size_t)(r - T) * D);
+        float s = 0.0f;
+        for (int i = lane; i < D / 8; i += 32) {
+            const uint4 v = __ldg(row + i);
+            const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+            for (int k = 0; k < 4; ++k) { const float a = bf16_lo(w[k]), b = bf16_hi(w[k]); s = fmaf(a, a, s); s = fmaf(b, b, s); }
+        }
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) s += __shfl_xor_sync(kFullMask, s, o);
+        if (lane == 0) norms[r] = sqrtf(s) * 1.0001f;          // rounded up a little: it feeds an upper bound
+    }
+}
+
+__global__ void __launch_bounds__(kFlThreads, 1)
+router_filter_kernel(const __grid_constant__ CUtensorMap tm_x,      // x [T, D], box 128 rows x 64, 128B swizzle
+                     const __grid_constant__ CUtensorMap tm_w,      // W_router [E, D], box N rows x 64 (rows >= E: zeros)
+                     int T, int D, int E, int K, int N, int BR, int n_blocks, int n_stages, const float *__restrict__ bias,
+                     const float *__restrict__ norms, float kappa, int mask_words, uint32_t *__restrict__ mask) {
+    extern __shared__ uint8_t fl_smem_raw[];
+    uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(fl_smem_raw) + 1023) & ~uintptr_t(1023));
+    // a stage = two k-blocks (the single-thread issue loop costs ~0.3 us per barrier turn whatever the tiles hold), each
+    // an x tile of BR token rows (the slot keeps 128 rows: the M = 128 MMA reads that much; rows >= BR are never used)
+    // and a W_router tile of N rows
+    const uint32_t x_bytes = (uint32_t)BR * 128u, w_bytes = (uint32_t)N * 128u;
+    const uint32_t x_slot = (x_bytes + 1023u) & ~1023u;
+    const uint32_t half_bytes = x_slot + ((w_bytes + 1023u) & ~1023u);
+    const uint32_t stage_bytes = 2u * half_bytes;
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + (size_t)n_stages * stage_bytes + kFlXTile);   // (+ the MMA's 16 KB read window)
+    uint64_t *empty = full + 16;
+    uint64_t *tfull = empty + 16;        // [2]
+    uint64_t *tempty = tfull + 2;        // [2]
+    uint32_t *tmem_ptr = reinterpret_cast<uint32_t *>(tempty + 2);
+    float *s_wn = reinterpret_cast<float *>(tmem_ptr + 2);          // [kFlMaxE] |Wr_e|
+    float *s_bias = s_wn + kFlMaxE;                                 // [kFlMaxE]
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int nkb = ((D + 63) / 64 + 1) / 2;          // stages per block (columns past D arrive as zeros)
+
+    if (warp == 0 && lane == 0) {
+        ptx::prefetch_tmap(&tm_x);
+        ptx::prefetch_tmap(&tm_w);
+        for (int i = 0; i < n_stages; ++i) { ptx::mbar_init(&full[i], 1); ptx::mbar_init(&empty[i], 1); }
+        for (int i = 0; i < 2; ++i) { ptx::mbar_init(&tfull[i], 1); ptx::mbar_init(&tempty[i], 4); }
+        ptx::fence_barrier_init();
+    }
+    if (warp == 1) ptx::tmem_alloc(tmem_ptr, 512);
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem_base = *tmem_ptr;
+    grid_dep_wait();          // x may come from a predecessor; norms from row_norm_kernel
+    if (threadIdx.x == 0) grid_dep_launch();
+
+    if (warp == 0) {
+        int stage = 0;
+        uint32_t phase = 0;
+        for (int blk = blockIdx.x; blk < n_blocks; blk += gridDim.x)
+            for (int kb = 0; kb < nkb; ++kb) {
+                ptx::mbar_wait(&empty[stage], phase ^ 1);
+                if (ptx::elect_one()) {
+                    uint8_t *st = smem + (size_t)stage * stage_bytes;
+                    ptx::mbar_arrive_expect_tx(&full[stage], 2u * (x_bytes + w_bytes));
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        ptx::tma_load_2d(st + h * half_bytes, &tm_x, &full[stage], (2 * kb + h) * 64, blk * BR, ptx::kEvictNormal);
+                        ptx::tma_load_2d(st + h * half_bytes + x_slot, &tm_w, &full[stage], (2 * kb + h) * 64, 0, ptx::kEvictLast);
+                    }
+                }
+                __syncwarp();
+                if (++stage == n_stages) { stage = 0; phase ^= 1; }
+            }
+    } else if (warp == 1) {
+        const uint32_t idesc = ptx::make_idesc_bf16(128, N);
+        const uint32_t a_lo0 = ptx::smem_desc_lo(ptx::smem_u32(smem));
+        int stage = 0, acc = 0;
+        uint32_t phase = 0, acc_phase = 0;
+        for (int blk = blockIdx.x; blk < n_blocks; blk += gridDim.x) {
+            ptx::mbar_wait(&tempty[acc], acc_phase ^ 1);
+            ptx::tc_fence_after();
+            for (int kb = 0; kb < nkb; ++kb) {
+                ptx::mbar_wait(&full[stage], phase);
+                ptx::tc_fence_after();
+                if (ptx::elect_one()) {
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const uint32_t a_lo = a_lo0 + stage * (stage_bytes >> 4) + h * (half_bytes >> 4);
+#pragma unroll
+                        for (int k = 0; k < 4; ++k)
+                            ptx::mma_bf16_ss(tmem_base + acc * 256, ptx::smem_desc(a_lo + 2 * k),
+                                             ptx::smem_desc(a_lo + (x_slot >> 4) + 2 * k), idesc, (kb | h | k) ? 1u : 0u);
+                    }
+                    ptx::mma_commit(&empty[stage]);
+                    if (kb == nkb - 1) ptx::mma_commit(&tfull[acc]);
+                }
+                __syncwarp();
+                if (++stage == n_stages) { stage = 0; phase ^= 1; }
+            }
+            if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+        }
+    } else {
+        // epilogue: thread = token row of the block (TMEM lane); pass 1 finds tau (K-th largest of a + bias), pass 2 marks
+        const int q = warp & 3;
+        const int epi_tid = (warp - 2) * 32 + lane;
+        for (int e = epi_tid; e < kFlMaxE; e += 128) {
+            s_wn[e] = e < E ? norms[T + e] : 0.0f;
+            s_bias[e] = (bias && e < E) ? bias[e] : 0.0f;
+        }
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        int acc = 0;
+        uint32_t acc_phase = 0;
+        for (int blk = blockIdx.x; blk < n_blocks; blk += gridDim.x) {
+            const int row = q * 32 + lane;
+            const int t = row < BR ? blk * BR + row : T;       // rows >= BR of the accumulator hold nothing
+            const float xn = t < T ? norms[t] : 0.0f;
+            ptx::mbar_wait(&tfull[acc], acc_phase);
+            ptx::tc_fence_after();
+            if (q * 32 >= BR) {                                // warp-uniform: just hand the accumulator back
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(&tempty[acc]);
+                if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+                continue;
+            }
+            const uint32_t t_addr = tmem_base + acc * 256 + ((uint32_t)(q * 32) << 16);
+            float top[kFlMaxK];
+#pragma unroll
+            for (int i = 0; i < kFlMaxK; ++i) top[i] = -INFINITY;
+            bool finite = true;
+            for (int c = 0; c < N; c += 16) {
+                uint32_t v[16];
+                ptx::tmem_ld_x16(t_addr + c, v);
+                ptx::tmem_ld_wait();
+#pragma unroll
+                for (int i = 0; i < 16; ++i) {
+                    if (c + i < E) {
+                        float a = __uint_as_float(v[i]) + s_bias[c + i];
+                        if (!(fabsf(a) <= 3.0e38f)) finite = false;
+                        // insert into the descending top-K list (registers, fully unrolled)
+#pragma unroll
+                        for (int j = 0; j < kFlMaxK; ++j) {
+                            const float hi = fmaxf(top[j], a);
+                            a = fminf(top[j], a);
+                            top[j] = hi;
+                        }
+                    }
+                }
+            }
+            float tau = top[0];
+#pragma unroll
+            for (int j = 1; j < kFlMaxK; ++j) if (j < K) tau = top[j];
+            const float slack = 2.0f * kappa * xn;
+            for (int w = 0; w < mask_words; ++w) {
+                uint32_t v[32];
+                uint32_t bits = 0;
+                if (w * 32 < N) {
+                    ptx::tmem_ld_x16(t_addr + w * 32, *reinterpret_cast<uint32_t(*)[16]>(&v[0]));
+                    if (w * 32 + 16 < N) ptx::tmem_ld_x16(t_addr + w * 32 + 16, *reinterpret_cast<uint32_t(*)[16]>(&v[16]));
+                    ptx::tmem_ld_wait();
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) {
+                        const int e = w * 32 + i;
+                        if (e < E && (i < 16 || w * 32 + 16 < N)) {
+                            const float a = __uint_as_float(v[i]) + s_bias[e];
+                            if (!finite || a >= tau - slack * s_wn[e]) bits |= 1u << i;
+                        }
+                    }
+                }
+                if (t < T) mask[(size_t)t * mask_words + w] = bits;
+            }
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&tempty[acc]);
+            if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+        }
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        ptx::tc_fence_after();
+        ptx::tmem_dealloc(tmem_base, 512);
+    }
+}
+
+// NB canonical dot products (A1) of one token against candidates ce[0..NB): lane l owns the 8-element chunks l, l + 32, ...
+// in ascending order with fmaf from 0, then the xor butterfly, then the bias -- bit for bit what router_kernel does.
+template <int NB>
+__device__ __forceinline__ void refine_dots(const bm_bf16 *__restrict__ xrow, const bm_bf16 *__restrict__ Wr,
+                                            const float *__restrict__ bias, int D, const int (&ce)[4], float *l, int lane) {
+    const bm_bf16 *wrow[NB];
+    float acc[NB];
+#pragma unroll
+    for (int j = 0; j < NB; ++j) { wrow[j] = Wr + (size_t)ce[j] * D; acc[j] = 0.0f; }
+#pragma unroll 4
+    for (int k = lane * 8; k < D; k += 256) {
+        const uint4 xv = __ldg(reinterpret_cast<const uint4 *>(xrow + k));
+        uint4 wv[NB];
+#pragma unroll
+        for (int j = 0; j < NB; ++j) wv[j] = __ldg(reinterpret_cast<const uint4 *>(wrow[j] + k));
+#pragma unroll
+        for (int j = 0; j < NB; ++j) {
+            float p = acc[j];                    // ascending element order inside the chunk
+            p = __fmaf_rn(bf16_lo(xv.x), bf16_lo(wv[j].x), p);
+            p = __fmaf_rn(bf16_hi(xv.x), bf16_hi(wv[j].x), p);
+            p = __fmaf_rn(bf16_lo(xv.y), bf16_lo(wv[j].y), p);
+            p = __fmaf_rn(bf16_hi(xv.y), bf16_hi(wv[j].y), p);
+            p = __fmaf_rn(bf16_lo(xv.z), bf16_lo(wv[j].z), p);
+            p = __fmaf_rn(bf16_hi(xv.z), bf16_hi(wv[j].z), p);
+            p = __fmaf_rn(bf16_lo(xv.w), bf16_lo(wv[j].w), p);
+            p = __fmaf_rn(bf16_hi(xv.w), bf16_hi(wv[j].w), p);
+            acc[j] = p;
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < NB; ++j) {
+        float p = acc[j];
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) p = __fadd_rn(p, __shfl_xor_sync(kFullMask, p, o));
+        if (lane == 0) {
+            if (bias) p = __fadd_rn(p, bias[ce[j]]);
+            l[ce[j]] = p;
+        }
+    }
+}
+
+// canonical dot products (A1) of the candidates only, then R2-R5; one warp per token, up to four candidates at a time
+__global__ void __launch_bounds__(kWarps * 32)
+router_refine_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 *__restrict__ Wr,
+                     const float *__restrict__ bias, int E, int K, GroupMap gm, const uint32_t *__restrict__ mask,
+                     int mask_words, int32_t *__restrict__ expert_ids, int32_t *__restrict__ group_ids,
+                     float *__restrict__ gate_w, int32_t *__restrict__ n_slots, int32_t *__restrict__ status) {
+    extern __shared__ float s_rl[];       // [kWarps][E]
+    grid_dep_wait();
+    grid_dep_launch();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float *l = s_rl + (size_t)warp * E;
+    const int n_warps = gridDim.x * kWarps;
+    for (int t = blockIdx.x * kWarps + warp; t < T; t += n_warps) {
+        // experts outside the candidate set: a finite value below every real logit, never selected (the set holds >= K)
+        for (int e = lane; e < E; e += 32) l[e] = -3.0e38f;
+        __syncwarp();
+        const bm_bf16 *xrow = x + (size_t)t * D;
+        for (int w = 0; w < mask_words; ++w) {
+            uint32_t bits = mask[(size_t)t * mask_words + w];
+            if (w == mask_words - 1 && (E & 31)) bits &= (1u << (E & 31)) - 1u;
+            while (bits) {
+                const int nb = min(__popc(bits), 4);
+                int ce[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    ce[j] = w * 32 + (bits ? __ffs(bits) - 1 : 0);
+                    if (j < nb) bits &= bits - 1;
+                }
+                if (nb == 4) refine_dots<4>(xrow, Wr, bias, D, ce, l, lane);
+                else if (nb == 3) refine_dots<3>(xrow, Wr, bias, D, ce, l, lane);
+                else if (nb == 2) refine_dots<2>(xrow, Wr, bias, D, ce, l, lane);
+                else refine_dots<1>(xrow, Wr, bias, D, ce, l, lane);
+            }
+        }
+        __syncwarp();
+        select_and_write(l, t, lane, E, K, gm, expert_ids, group_ids, gate_w, n_slots, status);
+        __syncwarp();
+    }
+}
+
+cudaError_t launch_filter_router(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const float *bias, int E, int K,
+                                 GroupMap gm, const bm_routing &r, int32_t *status, float *scratch, cudaStream_t stream) {
+    const int sms = num_sms();
+    float *norms = scratch;                                              // [T + E]
+    const int mask_words = (E + 31) / 32;
+    uint32_t *mask = reinterpret_cast<uint32_t *>(scratch + (((size_t)T + E + 3) & ~(size_t)3));     // [T][mask_words]
+    cudaError_t e = launch_kernel(row_norm_kernel, dim3(std::min((T + E + 7) / 8, sms * 8)), dim3(256), 0, stream, x, T, Wr, E, D, norms);
+    if (e != cudaSuccess) return e;
+    const int N = std::max(16, (E + 15) & ~15);
+    // token rows per CTA block: as many blocks as SMs when the batch allows it (the kernel streams x once: HBM / latency bound)
+    const int BR = T >= 128 * sms ? 128 : (T >= 64 * sms ? 64 : 32);
+    const size_t stage_bytes = 2 * ((((size_t)BR * 128 + 1023) & ~(size_t)1023) + (((size_t)N * 128 + 1023) & ~(size_t)1023));
+    int n_stages = (int)((184 * 1024) / stage_bytes);
+    n_stages = n_stages > 12 ? 12 : n_stages;
+    const size_t smem = 1024 + (size_t)n_stages * stage_bytes + kFlXTile + 36 * 8 + 16 + 2 * kFlMaxE * sizeof(float);
+    if ((e = ensure_dyn_smem(reinterpret_cast<const void *>(router_filter_kernel), smem)) != cudaSuccess) return e;
+    CUtensorMap m_x, m_w;
+    if (!make_map_2d_sw128(&m_x, x, (uint64_t)T, (uint64_t)D, (uint32_t)BR) || !make_map_2d_sw128(&m_w, Wr, (uint64_t)E, (uint64_t)D, (uint32_t)N))
+        return cudaErrorInvalidValue;
+    const int n_blocks = (T + BR - 1) / BR;
+    const float kappa = 2.0f * (float)D * 1.1920929e-7f + 3.8146973e-6f;     // 2 D 2^-23 + 2^-18
+    e = launch_kernel(router_filter_kernel, dim3(std::min(n_blocks, sms)), dim3(kFlThreads), smem, stream, m_x, m_w, T, D, E, K, N,
+                      BR, n_blocks, n_stages, bias, (const float *)norms, kappa, mask_words, mask);
+    if (e != cudaSuccess) return e;
+    const size_t smem_r = (size_t)kWarps * E * sizeof(float);
+    return launch_kernel(router_refine_kernel, dim3(std::min((T + kWarps - 1) / kWarps, sms * 8)), dim3(kWarps * 32), smem_r, stream,
+                         x, T, D, Wr, bias, E, K, gm, (const uint32_t *)mask, mask_words, r.expert_ids, r.group_ids, r.gate_w,
+                         r.n_slots, status);
+}
+
 template <int TOK, int ET>
 cudaError_t launch_cfg(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const float *bias, int E, int K,
                        GroupMap gm, int WT, int WE, const bm_routing &r, int32_t *status,
@@ -595,8 +916,13 @@ cudaError_t launch_router(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, con
                           int K, GroupMap gm, const bm_routing &r, int32_t *status, float *route_logits,
                           bool *fused_permute, cudaStream_t stream) {
     *fused_permute = false;
-    if (T >= opt(OPT_ROUTER_TP_MIN_T))   // throughput shape: operands staged through shared memory
+    if (T >= opt(OPT_ROUTER_TP_MIN_T)) {
+        // throughput shapes: tensor-core filter + canonical refinement of the candidates when the shape allows it,
+        // else all E canonical dots with the operands staged through shared memory
+        if (opt(OPT_ROUTER_FILTER) != 0 && E <= kFlMaxE && K <= kFlMaxK && K < E && D % 8 == 0)
+            return launch_filter_router(x, T, D, Wr, bias, E, K, gm, r, status, route_logits, stream);
         return launch_tp(x, T, D, Wr, bias, E, K, gm, r, status, stream);
+    }
     // (measured: 2 us faster than router + permutation kernels at T = 1, even at T = 16, slower from T = 64 on:
     // more CTAs and two rounds of arrival counters)
     if (E > 8 && T <= opt(OPT_ROUTER_SPLIT_MAX_T)) {

@@ -35,6 +35,6 @@ def tp_moe_forward(x, routing, W1_r, W3_r, W2_r, out, workspace, S: int = 0, gro
     if partial is None:
         partial = torch.empty((T, D), dtype=torch.float32, device=x.device)
     bm.bm_moe_forward_f32(x, routing, W1_r, W3_r, W2_r, partial, workspace, S=S)
-    if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
+    if dist.is_available() and dist.is_initialized():        # (also with one rank: the same call path)
         dist.all_reduce(partial, op=dist.ReduceOp.SUM, group=group)
     return bm.bm_round_bf16(partial, out)

@@ -268,3 +268,35 @@ def test_tensor_parallel_partials_sum_to_the_layer(T, world):
         assert (a == b).all()
     else:                                               # fused combine, K + S = 5 sources: fp32 adds arrive in any order
         assert (a.float() - b.float()).abs().max() <= 2.0 ** -7 * b.float().abs().max()
+
+
+def test_tp_moe_forward_under_a_real_nccl_process_group():
+    """The collective call path of tensor parallelism (tp.py: bm_moe_forward_f32 -> dist.all_reduce -> bm_round_bf16)
+    executed on hardware: a one-rank NCCL process group (one GPU per box here).  The sum over one rank is the rank's
+    partial, so the result must equal the plain layer within the fp32-order tolerance; what this covers is that NCCL
+    accepts the fp32 partial buffer on the library's stream and that the rounding pass follows it."""
+    import os
+    import torch.distributed as dist
+    import paper_2607_04164_b200 as bm
+    if dist.is_initialized():
+        pytest.skip("a process group already exists in this process")
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    os.environ.setdefault("MASTER_PORT", str(29600 + os.getpid() % 300))
+    dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+    try:
+        for T in (48, 700):
+            cfg = LayerConfig("tpn", T=T, D=512, F=704, E=16, K=2, G=4, S=0, zipf_s=1.0)
+            L = make_layer(cfg, 5)
+            o = oracle.route(bf16_bits(L.x), bf16_bits(L.W_router), L.router_bias.numpy(), cfg.K, L.group_map.numpy(), cfg.G)
+            ref = oracle.moe_forward(bf16_bits(L.x), o, bf16_bits(L.W1), bf16_bits(L.W3), bf16_bits(L.W2), cfg.S)
+            xd = L.x.cuda()
+            r = bm.Routing(T, cfg.K, cfg.G)
+            ws = bm.alloc_workspace(T, cfg.D, cfg.F, cfg.E, cfg.K, cfg.G, cfg.S)
+            bm.bm_route(xd, L.W_router.cuda(), L.router_bias.cuda(), cfg.K, L.group_map.cuda(), cfg.G, r, ws)
+            out = torch.full((T, cfg.D), float("nan"), dtype=torch.bfloat16, device="cuda")
+            bm.tp_moe_forward(xd, r, L.W1.cuda(), L.W3.cuda(), L.W2.cuda(), out, ws, S=cfg.S)
+            torch.cuda.synchronize()
+            assert dist.get_world_size() == 1 and dist.get_backend() == "nccl"
+            assert_out_close(out.float().cpu().numpy().astype(np.float64), ref)
+    finally:
+        dist.destroy_process_group()

@@ -309,8 +309,11 @@ def test_prefill_path_determinism_as_bm_forward_info_reports_it():
             outs = [gpu_layer(L, 0, d)[1] for _ in range(4)]
         for o2 in outs[1:]:
             assert (outs[0] == o2).all()
-    path, det = bm.bm_forward_info(600, 4, 5, 1, 512, 384)
+    with bm.options(FUSED_COMBINE=1):
+        path, det = bm.bm_forward_info(600, 4, 5, 1, 512, 384)
     assert path == PATHS["prefill"] and not det                # fused, five sources per token
+    assert bm.bm_forward_info(600, 4, 5, 1, 512, 384)[1]       # F < 4096: two-pass by default
+    assert not bm.bm_forward_info(600, 4, 5, 1, 512, 4096)[1]  # F >= 4096: fused by default
     assert bm.bm_forward_info(1, 4, 60, 0, 2048, 1408) == (PATHS["gemv"], True)
 
 
@@ -348,6 +351,10 @@ VARIANTS = [
     (PATHS["prefill"], {"PF_GATHER": 0, "PF_PAIR": 1}),         # TMA-fed CTA pairs
     (PATHS["prefill"], {"FUSED_COMBINE": 0}),                  # two-pass combine (bf16 y rows, slot order)
     (PATHS["prefill"], {"FUSED_COMBINE": 0, "PF_PAIR": 1}),
+    (PATHS["prefill"], {"FUSED_COMBINE": 1}),                  # combine fused into the W2 GEMM epilogue
+    (PATHS["prefill"], {"FUSED_COMBINE": 1, "PF_PAIR": 1}),
+    (PATHS["decode"], {"FUSED_COMBINE": 0}),                   # decode kernel + finalize pass
+    (PATHS["decode"], {"FUSED_COMBINE": 1, "DC_DENSE_MAX_T": 0}),   # gathered rows, in-kernel finish
     (0, {"ROUTER_TP_MIN_T": 1}),                               # throughput router on any T
     (0, {"ROUTER_SPLIT_MAX_T": 511}),                          # split router (+ fused permutation) on any T < 512
 ]
