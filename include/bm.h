@@ -314,7 +314,8 @@ int bm_device_status(void *workspace, int32_t *host_out, bm_stream_t stream);
  *   GEMV_FUSE (1)           matrix-vector path: fuse the W2 stage with the combine
  *   DC_R1, DC_R2, DC_KS2, DC_RMAX, DC_KS_FORCE (0, 0, 1, 128, 0)   decode tiling overrides (rows per tile, K splits)
  *   DC_STAGES, PF_STAGES (12)   cap on the shared-memory ring depth
- *   ROUTER_FILTER (1)       T >= 512, E <= 256, K <= 8: tensor-core filter + canonical refinement of the candidates; 0 = all E dots
+ *   ROUTER_FILTER (1)       T >= 512, E <= 256, K <= 8, E >= 4K + 8: tensor-core filter + canonical refinement of the
+ *                           candidates; 0 = all E dots; 2 = the filter whenever the kernel supports the shape
  *   DC_KPACK (2)            decode kernels: k-blocks per ring stage
  *   COMBINE_WARPS (64), PERM_SMALL_WARPS (0), ROUTER_WE (0), ROUTER_TP_MIN_T (512), ROUTER_SPLIT_MAX_T (16)
  *                           shape thresholds of the small kernels

@@ -45,12 +45,16 @@ ROUTE_SHAPES = [
 def test_routing_bit_exact(T, D, E, K, G, s):
     cfg = LayerConfig("t", T=T, D=D, F=8, E=E, K=K, G=G, zipf_s=s,
                       gmap_kind="identity" if G == E else "balanced")
+    import paper_2607_04164_b200 as bm
     for seed in range(2):
         L = make_layer(cfg, seed, weights=False)
-        r, ws, _ = gpu_route(L)
-        import paper_2607_04164_b200 as bm
-        assert bm.bm_device_status(ws) == 0
-        assert_routing_equal(routing_to_numpy(r, T), oracle_route(L))
+        o = oracle_route(L)
+        # T >= 512: all E canonical dots (0), the tensor-core filter + refinement by the default rule (1) and forced (2)
+        for filt in ((0, 1, 2) if T >= 512 else (1,)):
+            with bm.options(ROUTER_FILTER=filt):
+                r, ws, _ = gpu_route(L)
+            assert bm.bm_device_status(ws) == 0
+            assert_routing_equal(routing_to_numpy(r, T), o)
 
 
 def test_routing_ties_and_degenerate_rows():
@@ -64,8 +68,12 @@ def test_routing_ties_and_degenerate_rows():
         L.W_router[E - 1] = L.W_router[0]                      # a guaranteed tie pair
         L.router_bias = None
         L.group_map = torch.as_tensor((np.arange(E) % G).astype(np.int32))
-        r, ws, _ = gpu_route(L)
+        import paper_2607_04164_b200 as bm
+        with bm.options(ROUTER_FILTER=2):                      # ties at the boundary through the filter's candidate rule too
+            r, ws, _ = gpu_route(L)
         o = oracle_route(L, want_logits=True)
+        assert_routing_equal(routing_to_numpy(r, T), o)
+        r, ws, _ = gpu_route(L)
         srt = np.sort(o.logits, axis=1)[:, ::-1]
         if K < E:
             assert (srt[:, K - 1] == srt[:, K]).any()          # ties at the selection boundary exist
@@ -355,7 +363,8 @@ VARIANTS = [
     (PATHS["prefill"], {"FUSED_COMBINE": 1, "PF_PAIR": 1}),
     (PATHS["decode"], {"FUSED_COMBINE": 0}),                   # decode kernel + finalize pass
     (PATHS["decode"], {"FUSED_COMBINE": 1, "DC_DENSE_MAX_T": 0}),   # gathered rows, in-kernel finish
-    (0, {"ROUTER_TP_MIN_T": 1}),                               # throughput router on any T
+    (0, {"ROUTER_TP_MIN_T": 1, "ROUTER_FILTER": 0}),           # throughput router (all E canonical dots) on any T
+    (0, {"ROUTER_TP_MIN_T": 1, "ROUTER_FILTER": 2}),           # tensor-core filter + refinement on any T
     (0, {"ROUTER_SPLIT_MAX_T": 511}),                          # split router (+ fused permutation) on any T < 512
 ]
 
