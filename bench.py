@@ -716,7 +716,7 @@ def run_next(args):
     xc = Lc.x.cuda()
     Wo = (mk(E, F, D), mk(E, F, D), mk(E, D, F))
     wsc = torch.empty(int(bm.lib().bm_expert_outputs_workspace_bytes(Tc, D, F, E)), dtype=torch.uint8, device="cuda")
-    Y = torch.empty((E, Tc, D), dtype=torch.bfloat16, device="cuda")
+    Y = torch.empty((Tc, E, D), dtype=torch.bfloat16, device="cuda")         # token-major
     Uw = [bm.bm_unite_weights(t, gm, G) for t in Wo]
     U = bm.bm_expert_outputs(xc, *Uw)
     wcnt = torch.randint(1, 1000, (E,), dtype=torch.int32, device="cuda")

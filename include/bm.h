@@ -158,17 +158,18 @@ int bm_unite_weights(const bm_bf16 *W, int E, size_t n, const int32_t *group_map
  * bm_expert_histogram -- w[e] = number of (token, rank) pairs whose selected expert is e ("how often expert
  *   e is selected by the gating function on the calibration dataset").  expert_ids [T,K] i32 as bm_route wrote
  *   them; w [E] i32.  Exact.
- * bm_expert_outputs -- y[e, t, :] = FFN_e(x_t) for EVERY expert e and token t (the f_e(x) of Eq. 5), through the
- *   grouped tcgen05 GEMM kernels.  W1, W3 [E,F,D], W2 [E,D,F], y [E,T,D] bf16; workspace of
+ * bm_expert_outputs -- y[t, e, :] = FFN_e(x_t) for EVERY expert e and token t (the f_e(x) of Eq. 5), through the
+ *   grouped tcgen05 GEMM kernels.  W1, W3 [E,F,D], W2 [E,D,F]; y is TOKEN-MAJOR, [T,E,D] bf16 (the E outputs of a token
+ *   are neighbours in memory: that is what lets bm_cosine_gram and bm_group_mse stream at HBM rate); workspace of
  *   bm_expert_outputs_workspace_bytes(T, D, F, E) bytes (no initialisation needed).  E <= BM_MAX_G.
- * bm_cosine_gram -- gram[e,e'] = <Y_e, Y_e'> with Y_e = all outputs of expert e flattened (n = T*D values), and
+ * bm_cosine_gram -- gram[e,e'] = <Y_e, Y_e'> with Y_e = all outputs of expert e (T*D values), and
  *   cosine[e,e'] = gram[e,e'] / (|Y_e| |Y_e'|) (A19), fp32 accumulation on the tensor cores, per-CTA
- *   partial tiles summed in a fixed order.  Y [E,n] bf16, n % 8 == 0, E <= 128; gram, cosine [E,E] f32 (cosine may
- *   be NULL); workspace >= bm_gram_workspace_bytes(E).
+ *   partial tiles summed in a fixed order.  Y [T,E,D] bf16 (token-major, as bm_expert_outputs writes it), D % 8 == 0,
+ *   E <= 128; gram, cosine [E,E] f32 (cosine may be NULL); workspace >= bm_gram_workspace_bytes(E).
  * bm_group_mse -- Eq. 5: alpha_e = w_e / sum_{e' in G_r} w_e', t_r(x) = sum_{e in G_r} alpha_e f_e(x);
  *   MSE_r = mean over tokens of |U_r(x) - t_r(x)|^2 (Eq. 9's expectation); Eq. 6: beta_r = sum_{e in G_r} w_e with w
  *   normalised to sum 1, MSE_total = sum_r beta_r MSE_r (A20: a never-selected group takes uniform alpha
- *   and weight 0; an empty group has MSE 0).  Y [E,T,D] bf16 expert outputs, U [G,T,D] bf16 united-expert outputs,
+ *   and weight 0; an empty group has MSE 0).  Y [T,E,D] bf16 expert outputs, U [T,G,D] bf16 united-expert outputs (both token-major),
  *   w [E] i32, group_map [E] i32; mse [G] f32, mse_total [1] f32; workspace >= bm_mse_workspace_bytes(G).
  */
 int bm_expert_histogram(const int32_t *expert_ids, int T, int K, int E, int32_t *w, bm_stream_t stream);
@@ -176,7 +177,7 @@ size_t bm_expert_outputs_workspace_bytes(int T, int D, int F, int E);
 int bm_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 *W1, const bm_bf16 *W3, const bm_bf16 *W2, int E,
                       int F, bm_bf16 *y, void *workspace, size_t workspace_bytes, bm_stream_t stream);
 size_t bm_gram_workspace_bytes(int E);
-int bm_cosine_gram(const bm_bf16 *Y, int E, size_t n, float *gram, float *cosine, void *workspace,
+int bm_cosine_gram(const bm_bf16 *Y, int E, int T, int D, float *gram, float *cosine, void *workspace,
                    size_t workspace_bytes, bm_stream_t stream);
 size_t bm_mse_workspace_bytes(int G);
 int bm_group_mse(const bm_bf16 *Y, const bm_bf16 *U, int T, int D, const int32_t *w, const int32_t *group_map, int E,

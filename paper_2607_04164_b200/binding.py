@@ -87,7 +87,7 @@ def lib() -> ctypes.CDLL:
         L.bm_gram_workspace_bytes.restype = c_size_t
         L.bm_gram_workspace_bytes.argtypes = [c_int]
         L.bm_cosine_gram.restype = c_int
-        L.bm_cosine_gram.argtypes = [c_void_p, c_int, c_size_t, c_void_p, c_void_p, c_void_p, c_size_t, c_void_p]
+        L.bm_cosine_gram.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p, c_void_p, c_size_t, c_void_p]
         L.bm_mse_workspace_bytes.restype = c_size_t
         L.bm_mse_workspace_bytes.argtypes = [c_int]
         L.bm_group_mse.restype = c_int
@@ -329,11 +329,11 @@ def bm_expert_histogram(expert_ids, E: int, stream=None):
 
 
 def bm_expert_outputs(x, W1, W3, W2, y=None, workspace=None, stream=None):
-    """y[e,t,:] = FFN_e(x_t) for every expert and token (include/bm.h: bm_expert_outputs) -> [E,T,D] bf16."""
+    """y[t,e,:] = FFN_e(x_t) for every expert and token (include/bm.h: bm_expert_outputs) -> token-major [T,E,D] bf16."""
     T, D = x.shape
     E, F = W1.shape[0], W1.shape[1]
     if y is None:
-        y = torch.empty((E, T, D), dtype=torch.bfloat16, device=x.device)
+        y = torch.empty((T, E, D), dtype=torch.bfloat16, device=x.device)
     if workspace is None:
         workspace = torch.empty(int(lib().bm_expert_outputs_workspace_bytes(T, D, F, E)), dtype=torch.uint8, device=x.device)
     rc = lib().bm_expert_outputs(_ptr(x), T, D, _ptr(W1), _ptr(W3), _ptr(W2), E, F, _ptr(y), _ptr(workspace),
@@ -344,22 +344,24 @@ def bm_expert_outputs(x, W1, W3, W2, y=None, workspace=None, stream=None):
 
 
 def bm_cosine_gram(Y, stream=None):
-    """(gram, cosine) [E,E] f32 of the expert outputs Y [E, ...] bf16 (include/bm.h: bm_cosine_gram)."""
-    E = Y.shape[0]
-    n = Y[0].numel()
+    """(gram, cosine) [E,E] f32 of the expert outputs Y [T,E,D] bf16, token-major (include/bm.h: bm_cosine_gram)."""
+    _dev("Y", Y, torch.bfloat16)
+    T, E, D = Y.shape
     gram = torch.empty((E, E), dtype=torch.float32, device=Y.device)
     cos = torch.empty((E, E), dtype=torch.float32, device=Y.device)
     ws = torch.empty(int(lib().bm_gram_workspace_bytes(E)), dtype=torch.uint8, device=Y.device)
-    rc = lib().bm_cosine_gram(_ptr(Y), E, n, _ptr(gram), _ptr(cos), _ptr(ws), ws.numel(), _stream(stream))
+    rc = lib().bm_cosine_gram(_ptr(Y), E, T, D, _ptr(gram), _ptr(cos), _ptr(ws), ws.numel(), _stream(stream))
     if rc != BM_OK:
         raise BmError(rc, "bm_cosine_gram")
     return gram, cos
 
 
 def bm_group_mse(Y, U, w, group_map, stream=None):
-    """(mse [G] f32, mse_total [1] f32) of Eq. 5-6 (include/bm.h: bm_group_mse).  Y [E,T,D], U [G,T,D] bf16."""
-    E, T, D = Y.shape
-    G = U.shape[0]
+    """(mse [G] f32, mse_total [1] f32) of Eq. 5-6 (include/bm.h: bm_group_mse).  Y [T,E,D], U [T,G,D] bf16, token-major."""
+    _dev("Y", Y, torch.bfloat16)
+    _dev("U", U, torch.bfloat16)
+    T, E, D = Y.shape
+    G = U.shape[1]
     mse = torch.empty(G, dtype=torch.float32, device=Y.device)
     tot = torch.empty(1, dtype=torch.float32, device=Y.device)
     ws = torch.empty(int(lib().bm_mse_workspace_bytes(G)), dtype=torch.uint8, device=Y.device)

@@ -248,15 +248,15 @@ size_t bm_gram_workspace_bytes(int E) {
     return (size_t)256 * E * E * sizeof(float);          // one partial tile per CTA, any SM count up to 256
 }
 
-int bm_cosine_gram(const bm_bf16 *Y, int E, size_t n, float *gram, float *cosine, void *workspace,
+int bm_cosine_gram(const bm_bf16 *Y, int E, int T, int D, float *gram, float *cosine, void *workspace,
                    size_t workspace_bytes, bm_stream_t stream) {
-    if (E < 1 || E > 128 || n % 8 != 0 || n == 0 || n > 0x7fffff00ull) return BM_ERR_SHAPE;
+    if (E < 1 || E > 128 || T < 1 || D < 8 || D % 8 != 0 || (long long)T * ((D + 63) / 64) > 0x7fffff00LL) return BM_ERR_SHAPE;
     if (!Y || !gram || !workspace) return BM_ERR_NULL;
     if (!aligned16(Y) || !aligned16(workspace)) return BM_ERR_ALIGN;
     if (workspace_bytes < bm_gram_workspace_bytes(E)) return BM_ERR_WORKSPACE;
     if (device_ok() != 1) return BM_ERR_CUDA;
     if (num_sms() > 256) return BM_ERR_CUDA;
-    return launch_gram(Y, E, n, gram, cosine, static_cast<float *>(workspace), reinterpret_cast<cudaStream_t>(stream)) ==
+    return launch_gram(Y, E, T, D, gram, cosine, static_cast<float *>(workspace), reinterpret_cast<cudaStream_t>(stream)) ==
                    cudaSuccess
                ? BM_OK : BM_ERR_CUDA;
 }

@@ -32,23 +32,21 @@ expert_hist_kernel(const int32_t *__restrict__ expert_ids, long long items, int 
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Gram matrix of the expert outputs: Y [E, n] bf16 (n = T*D, contiguous) is K-major for both operands of
-// Y . Y^T, so ONE TMA tile (128 rows x 64 columns; rows >= E are out of bounds and arrive as zeros) feeds
-// the A and the B descriptor of tcgen05.mma.  CTA c owns the k-blocks c, c + grid, ... and keeps its
-// 128 x N fp32 partial in TMEM until the end; partial tiles go to the workspace and are summed in CTA order.
-// Measured: 3.5-3.7 TB/s (0.55 of the HBM copy rate) whatever E is.  The cause is the layout, not the MMAs: the E rows
-// of a tile are n*2 bytes (16 MB at T = 4096, D = 2048) apart, so every TMA box gathers 128-byte pieces from E distant
-// DRAM pages.  A stand-alone TMA streaming probe shows the same: 128 x 128-byte boxes reach 7.0 TB/s with an 8 KB row
-// stride and 4.5 TB/s with an 8 MB row stride (148 CTAs; 142 vs 62 GB/s per SM with 17 CTAs).  Packing two k-blocks of
-// a small-E tile into one M = N = 128 MMA was tried and changed nothing.  A token-major output layout [T, E, D] of
-// bm_expert_outputs would give the Gram kernel 4 KB row strides; that is the lead for a later round.
+// Gram matrix of the expert outputs.  Y is TOKEN-MAJOR, [T, E, D] bf16: the E rows of one token are D*2 bytes apart, so
+// ONE TMA tile (3-D map {D, E, T}: 128 rows x 64 columns of one token; rows >= E are out of bounds and arrive as zeros)
+// gathers from a few neighbouring DRAM pages and feeds the A and the B descriptor of tcgen05.mma.  CTA c owns the
+// a contiguous run of k-blocks (k-block = (token, 64-column piece)) and keeps its 128 x N fp32 partial in TMEM until the
+// end; partial tiles go to the workspace and are summed in CTA order.
+// Round 1 took Y as [E, T*D]: the rows of a tile were 16 MB apart and the kernel ran at 3.5-3.7 TB/s (0.55 of the HBM copy
+// rate) whatever E was -- a stand-alone TMA probe streams 7.0 TB/s at an 8 KB row stride and 4.5 TB/s at 8 MB.  Hence the
+// token-major output of bm_expert_outputs.
 // ---------------------------------------------------------------------------------------------------
 constexpr int kGramThreads = 192;
 constexpr int kGramStages = 12;
 constexpr int kGramTile = 128 * 128;     // bytes: 128 rows x 64 bf16
 
 __global__ void __launch_bounds__(kGramThreads, 1)
-gram_kernel(const __grid_constant__ CUtensorMap tm_y, int E, int n_kblocks, float *__restrict__ partial) {
+gram_kernel(const __grid_constant__ CUtensorMap tm_y, int E, int n_kblocks, int kb_per_token, float *__restrict__ partial) {
     extern __shared__ uint8_t g_smem_raw[];
     uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(g_smem_raw) + 1023) & ~uintptr_t(1023));
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + (size_t)kGramStages * kGramTile);
@@ -69,7 +67,10 @@ gram_kernel(const __grid_constant__ CUtensorMap tm_y, int E, int n_kblocks, floa
     __syncthreads();
     ptx::tc_fence_after();
     const uint32_t tmem_base = *tmem_ptr;
-    const int my_kb = blockIdx.x < n_kblocks ? (n_kblocks - 1 - blockIdx.x) / gridDim.x + 1 : 0;
+    // CTA c owns a CONTIGUOUS run of k-blocks: consecutive loads walk along the experts' rows of one token (whole DRAM pages)
+    const int per_cta = (n_kblocks + gridDim.x - 1) / gridDim.x;
+    const int kb0 = blockIdx.x * per_cta;
+    const int my_kb = max(0, min(per_cta, n_kblocks - kb0));
 
     if (warp == 0) {
         int stage = 0;
@@ -78,8 +79,10 @@ gram_kernel(const __grid_constant__ CUtensorMap tm_y, int E, int n_kblocks, floa
             ptx::mbar_wait(&empty[stage], phase ^ 1);
             if (ptx::elect_one()) {
                 ptx::mbar_arrive_expect_tx(&full[stage], kGramTile);
-                ptx::tma_load_2d(smem + (size_t)stage * kGramTile, &tm_y, &full[stage],
-                                 (blockIdx.x + i * gridDim.x) * 64, 0, ptx::kEvictFirst);
+                const int kbi = kb0 + i;                                // k-block = (token, 64-column piece of its D outputs)
+                const int tok = kbi / kb_per_token;
+                ptx::tma_load_3d(smem + (size_t)stage * kGramTile, &tm_y, &full[stage], (kbi - tok * kb_per_token) * 64, 0, tok,
+                                 ptx::kEvictFirst);
             }
             __syncwarp();
             if (++stage == kGramStages) { stage = 0; phase ^= 1; }
@@ -169,8 +172,8 @@ gram_finish_kernel(const float *__restrict__ partial, int n_cta, int E, float *_
 // kernel adds the blocks in index order in fp64).
 // ---------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-mse_partial_kernel(const bm_bf16 *__restrict__ Y, const bm_bf16 *__restrict__ U, size_t n8,
-                   const int32_t *__restrict__ w, const int32_t *__restrict__ gmap, int E,
+mse_partial_kernel(const bm_bf16 *__restrict__ Y, const bm_bf16 *__restrict__ U, size_t n8, size_t d8,
+                   const int32_t *__restrict__ w, const int32_t *__restrict__ gmap, int E, int G,
                    float *__restrict__ part) {
     __shared__ int32_t s_member[BM_MAX_E];
     __shared__ float s_alpha[BM_MAX_E];
@@ -190,21 +193,24 @@ mse_partial_kernel(const bm_bf16 *__restrict__ Y, const bm_bf16 *__restrict__ U,
     const int cnt = s_cnt;
     float err = 0.0f;
     if (cnt > 0) {
+        // token-major layouts: Y [T, E, D], U [T, G, D]; i walks the (token, 8-column piece) pairs
         const uint4 *Y4 = reinterpret_cast<const uint4 *>(Y);
-        const uint4 *U4 = reinterpret_cast<const uint4 *>(U) + (size_t)r * n8;
-        for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n8; i += (size_t)gridDim.x * blockDim.x) {
+        const uint4 *U4 = reinterpret_cast<const uint4 *>(U);
+        const size_t n_tok = n8 / d8;
+        for (size_t tok = blockIdx.x; tok < n_tok; tok += gridDim.x)
+        for (size_t c = threadIdx.x; c < d8; c += blockDim.x) {
             float t[8];
 #pragma unroll
             for (int k = 0; k < 8; ++k) t[k] = 0.0f;
             for (int m = 0; m < cnt; ++m) {
-                const uint4 v = __ldg(Y4 + (size_t)s_member[m] * n8 + i);
+                const uint4 v = __ldg(Y4 + (tok * E + s_member[m]) * d8 + c);
                 const float a = s_alpha[m];
                 t[0] = fmaf(a, bf16_lo(v.x), t[0]); t[1] = fmaf(a, bf16_hi(v.x), t[1]);
                 t[2] = fmaf(a, bf16_lo(v.y), t[2]); t[3] = fmaf(a, bf16_hi(v.y), t[3]);
                 t[4] = fmaf(a, bf16_lo(v.z), t[4]); t[5] = fmaf(a, bf16_hi(v.z), t[5]);
                 t[6] = fmaf(a, bf16_lo(v.w), t[6]); t[7] = fmaf(a, bf16_hi(v.w), t[7]);
             }
-            const uint4 u = __ldg(U4 + i);
+            const uint4 u = __ldg(U4 + (tok * G + r) * d8 + c);
             const float d0 = bf16_lo(u.x) - t[0], d1 = bf16_hi(u.x) - t[1], d2 = bf16_lo(u.y) - t[2], d3 = bf16_hi(u.y) - t[3];
             const float d4 = bf16_lo(u.z) - t[4], d5 = bf16_hi(u.z) - t[5], d6 = bf16_lo(u.w) - t[6], d7 = bf16_hi(u.w) - t[7];
             err += d0 * d0 + d1 * d1 + d2 * d2 + d3 * d3 + d4 * d4 + d5 * d5 + d6 * d6 + d7 * d7;
@@ -246,10 +252,6 @@ mse_finish_kernel(const float *__restrict__ part, int nblk, int T, const int32_t
     }
 }
 
-typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
-                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
 }  // namespace
 
 cudaError_t launch_expert_hist(const int32_t *expert_ids, long long items, int E, int32_t *w, cudaStream_t stream) {
@@ -264,31 +266,17 @@ cudaError_t launch_expert_hist(const int32_t *expert_ids, long long items, int E
 
 size_t gram_workspace_bytes(int E) { return (size_t)num_sms() * E * E * sizeof(float); }
 
-cudaError_t launch_gram(const bm_bf16 *Y, int E, size_t n, float *gram, float *cosine, float *partial,
+cudaError_t launch_gram(const bm_bf16 *Y, int E, int T, int D, float *gram, float *cosine, float *partial,
                         cudaStream_t stream) {
-    static EncodeTiledFn enc = nullptr;
-    if (!enc) {
-        void *sym = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) != cudaSuccess ||
-            qres != cudaDriverEntryPointSuccess)
-            return cudaErrorInvalidValue;
-        enc = reinterpret_cast<EncodeTiledFn>(sym);
-    }
+    // Y [T, E, D]: a tile = the E rows of one token (4 KB apart at D = 2048) x 64 columns; rows >= E are out of bounds -> zeros
     CUtensorMap tm;
-    cuuint64_t dims[2] = {(cuuint64_t)n, (cuuint64_t)E};
-    cuuint64_t strides[1] = {(cuuint64_t)n * sizeof(bm_bf16)};
-    cuuint32_t box[2] = {64, 128};
-    cuuint32_t es[2] = {1, 1};
-    if (enc(&tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<bm_bf16 *>(Y), dims, strides, box, es,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-        return cudaErrorInvalidValue;
-    const long long nkb = (long long)((n + 63) / 64);
+    if (!make_map_3d_sw128(&tm, Y, (uint64_t)T, (uint64_t)E, (uint64_t)D, 128)) return cudaErrorInvalidValue;
+    const int kpt = (D + 63) / 64;
+    const long long nkb = (long long)T * kpt;
     const int grid = (int)(nkb < num_sms() ? nkb : num_sms());
     const size_t smem = 1024 + (size_t)kGramStages * kGramTile + 256;
     if (cudaError_t ea = ensure_dyn_smem(reinterpret_cast<const void *>(gram_kernel), smem); ea != cudaSuccess) return ea;
-    gram_kernel<<<grid, kGramThreads, smem, stream>>>(tm, E, (int)nkb, partial);
+    gram_kernel<<<grid, kGramThreads, smem, stream>>>(tm, E, (int)nkb, kpt, partial);
     gram_finish_kernel<<<E, 128, 0, stream>>>(partial, grid, E, gram, cosine);
     count_launch(2);
     return cudaGetLastError();
@@ -303,7 +291,7 @@ cudaError_t launch_group_mse(const bm_bf16 *Y, const bm_bf16 *U, int T, int D, c
     const int cap = mse_blocks() / G + 1;
     if (nblk > cap) nblk = cap;
     if (nblk < 1) nblk = 1;
-    mse_partial_kernel<<<dim3(nblk, G), 256, 0, stream>>>(Y, U, n8, w, gmap, E, part);
+    mse_partial_kernel<<<dim3(nblk, G), 256, 0, stream>>>(Y, U, n8, (size_t)(D / 8), w, gmap, E, G, part);
     mse_finish_kernel<<<1, 256, 0, stream>>>(part, nblk, T, w, gmap, E, G, mse, mse_total);
     count_launch(2);
     return cudaGetLastError();

@@ -182,7 +182,7 @@ cudaError_t launch_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 
 
 cudaError_t launch_expert_hist(const int32_t *expert_ids, long long items, int E, int32_t *w, cudaStream_t stream);
 size_t gram_workspace_bytes(int E);
-cudaError_t launch_gram(const bm_bf16 *Y, int E, size_t n, float *gram, float *cosine, float *partial,
+cudaError_t launch_gram(const bm_bf16 *Y, int E, int T, int D, float *gram, float *cosine, float *partial,
                         cudaStream_t stream);
 int mse_blocks();
 cudaError_t launch_group_mse(const bm_bf16 *Y, const bm_bf16 *U, int T, int D, const int32_t *w, const int32_t *gmap,

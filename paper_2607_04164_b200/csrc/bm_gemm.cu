@@ -91,6 +91,7 @@ struct GemmParams {
     float *out_acc;     // zero region: fp32 accumulator of the fused combine [T, D]
     int32_t *tickets;   // zero region: arrivals per (token, output piece)
     bm_bf16 *y;         // two-pass combine: per-row expert outputs
+    int y_tm;           // calibration: y is token-major [T, S, D] (row of shared set j, token t = t * S + j)
     bm_bf16 *out;       // fused combine: the layer output [T, D] bf16 ...
     float *out_f32;     // ... or, when non-null, the fp32 sums (tensor-parallel partial)
 };
@@ -734,7 +735,9 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
                 const int n_q = it.n - q * 32;                     // valid rows of this warp's quarter
                 uint4 *stg = reinterpret_cast<uint4 *>(epi_stage + (size_t)q * kEpiStageBytes);
                 const int rl = lane >> 3, ul = lane & 7;        // read phase: row (mod 4) and 16-byte unit of this lane
-                bm_bf16 *ybase = p.y + (size_t)(it.h_row0 + q * 32) * p.D + d0 + 8 * ul;
+                const size_t yrow0 = p.y_tm ? (size_t)(it.tok0 + q * 32) * p.S + (size_t)(it.u - p.G) : (size_t)(it.h_row0 + q * 32);
+                const size_t yrs = p.y_tm ? (size_t)p.S * p.D : (size_t)p.D;        // elements between consecutive chunk rows
+                bm_bf16 *ybase = p.y + yrow0 * p.D + d0 + 8 * ul;
 #pragma unroll 1
                 for (int c = 0; c < 256; c += 64) {
                     uint32_t v[32], w[32];
@@ -760,7 +763,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
                         for (int j = 0; j < 8; ++j) {
                             const int r = 4 * j + rl;
                             if (r < n_q)
-                                *reinterpret_cast<uint4 *>(ybase + (size_t)r * p.D + c) = stg[r * 8 + (ul ^ (r & 7))];
+                                *reinterpret_cast<uint4 *>(ybase + (size_t)r * yrs + c) = stg[r * 8 + (ul ^ (r & 7))];
                         }
                     }
                     __syncwarp();
@@ -1198,6 +1201,10 @@ cudaError_t launch_gemm(const CUtensorMap &a0, const CUtensorMap &a1, const CUte
 
 // [rows, cols] bf16 row-major, box = box_rows x box_cols, no swizzle (rows of a box are contiguous in shared
 // memory); out-of-bounds elements are zero-filled.  Used by the router's slab ring.
+bool make_map_3d_sw128(CUtensorMap *m, const void *base, uint64_t n, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+    return make_map_3d(m, base, n, rows, cols, box_rows);
+}
+
 bool make_map_2d_sw128(CUtensorMap *m, const void *base, uint64_t rows, uint64_t cols, uint32_t box_rows) {
     return make_map_2d(m, base, rows, cols, box_rows);
 }
@@ -1391,7 +1398,7 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
 }
 
 // f_e(x_t) for every expert and token (calibration forward): the prefill GEMM kernels over a
-// dense schedule (G = 0 routed groups, S = E always-on weight sets); y: [E, T, D] bf16.
+// all-shared schedule (G = 0 routed groups, S = E always-on weight sets); y: token-major [T, E, D] bf16.
 cudaError_t launch_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 *W1, const bm_bf16 *W3,
                                   const bm_bf16 *W2, int E, int F, bm_bf16 *y, bm_bf16 *h, cudaStream_t stream) {
     cudaError_t err;
@@ -1399,7 +1406,7 @@ cudaError_t launch_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 
     p.hints = 20;
     p.seg_cap = E + 1;
     p.T = T; p.D = D; p.F = F; p.K = 1; p.G = 0; p.S = E; p.TK = 0;
-    p.h = h; p.y = y; p.x = x;
+    p.h = h; p.y = y; p.x = x; p.y_tm = 1;
     p.ksplit = 1;
     const bool pair = (num_sms() & 1) == 0 && T >= 3 * kChunkRows && opt(OPT_PF_PAIR) != 0;   // as launch_forward_tc
     CUtensorMap m_x, m_w1, m_w3, m_w2, m_h;
@@ -1407,6 +1414,7 @@ cudaError_t launch_expert_outputs(const bm_bf16 *x, int T, int D, const bm_bf16 
         !make_map_3d(&m_w2, W2, E, D, F, pair ? 128 : 256) || !make_map_2d(&m_h, h, (uint64_t)E * T, F, 128))
         return cudaErrorInvalidValue;
     ring_geometry(false, true, T, &p, pair);
+    p.hints = pair ? 21 : 20;          // every chunk of a segment shares its weight tiles (see launch_forward_tc)
     p.kblocks = (D + kBlockK - 1) / kBlockK; p.R = 128; p.n_wtiles = (F + 127) / 128;
     err = pair ? launch_gemm<PF_GEMM1, true>(m_x, m_x, m_w1, m_w3, p, stream) : launch_gemm<PF_GEMM1>(m_x, m_x, m_w1, m_w3, p, stream);
     if (err != cudaSuccess) return err;

@@ -14,6 +14,8 @@ bool make_map_2d_plain(CUtensorMap *m, const void *base, uint64_t rows, uint64_t
 
 // host: 2-D tensor map over a row-major bf16 matrix, box = box_rows x 64 columns, 128-byte swizzle (bm_gemm.cu)
 bool make_map_2d_sw128(CUtensorMap *m, const void *base, uint64_t rows, uint64_t cols, uint32_t box_rows);
+// host: 3-D map over [n, rows, cols] bf16, box = 1 x box_rows x 64, 128-byte swizzle
+bool make_map_3d_sw128(CUtensorMap *m, const void *base, uint64_t n, uint64_t rows, uint64_t cols, uint32_t box_rows);
 
 namespace ptx {
 

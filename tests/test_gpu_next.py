@@ -142,7 +142,8 @@ def test_expert_histogram_and_outputs(T, D, F, E, K, G):
     Y = bm.bm_expert_outputs(L.x.cuda(), Wo[0].cuda(), Wo[1].cuda(), Wo[2].cuda())
     torch.cuda.synchronize()
     ref = oracle.expert_outputs(bf16_bits(L.x), bf16_bits(Wo[0]), bf16_bits(Wo[1]), bf16_bits(Wo[2]))
-    assert_out_close(Y.float().cpu().numpy().astype(np.float64).reshape(E * T, D), ref.reshape(E * T, D))
+    assert tuple(Y.shape) == (T, E, D)                          # token-major
+    assert_out_close(Y.permute(1, 0, 2).float().cpu().numpy().astype(np.float64).reshape(E * T, D), ref.reshape(E * T, D))
 
 
 @pytest.mark.parametrize("E,T,D", [(12, 96, 256), (60, 300, 512), (128, 40, 64), (3, 5, 8)])
@@ -155,7 +156,8 @@ def test_cosine_gram_matches_oracle(E, T, D):
     if E >= 3:
         Y[1] = Y[0]                                                        # identical pair -> cos 1
         Y[2] = -Y[0]                                                       # negated -> cos -1
-    gram, cos = bm.bm_cosine_gram(Y.cuda())
+    Ytm = Y.permute(1, 0, 2).contiguous().cuda()                # the C ABI takes the token-major layout [T, E, D]
+    gram, cos = bm.bm_cosine_gram(Ytm)
     torch.cuda.synchronize()
     g_ref, c_ref = oracle.cosine_matrix(Y.double().numpy())
     gram, cos = gram.cpu().numpy().astype(np.float64), cos.cpu().numpy().astype(np.float64)
@@ -167,7 +169,7 @@ def test_cosine_gram_matches_oracle(E, T, D):
     if E >= 3:
         assert abs(cos[0, 1] - 1) <= 2e-5 and abs(cos[0, 2] + 1) <= 2e-5
     # determinism: partial tiles are summed in a fixed order
-    gram2, _ = bm.bm_cosine_gram(Y.cuda())
+    gram2, _ = bm.bm_cosine_gram(Ytm)
     assert (gram2.cpu().numpy() == gram.astype(np.float32)).all()
 
 
@@ -180,7 +182,8 @@ def test_group_mse_matches_oracle(E, G, T, D):
     gmap = rng.integers(0, G, size=E).astype(np.int32)
     w = rng.integers(0, 50, size=E).astype(np.int32)
     w[gmap == gmap[0]] = 0                                                # one never-selected group (A20)
-    mse, tot = bm.bm_group_mse(Y.cuda(), U.cuda(), torch.as_tensor(w).cuda(), torch.as_tensor(gmap).cuda())
+    mse, tot = bm.bm_group_mse(Y.permute(1, 0, 2).contiguous().cuda(), U.permute(1, 0, 2).contiguous().cuda(),
+                               torch.as_tensor(w).cuda(), torch.as_tensor(gmap).cuda())
     torch.cuda.synchronize()
     m_ref, t_ref, _ = oracle.group_mse(Y.double().numpy(), U.double().numpy(), w, gmap, G)
     mse, tot = mse.cpu().numpy().astype(np.float64), float(tot.cpu()[0])
