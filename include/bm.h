@@ -282,7 +282,12 @@ int bm_moe_forward_path(const bm_bf16 *x, int T, int D, const bm_routing *routin
  *   out_host  HOST [T,D] bf16
  *   x_dev, out_dev   device staging buffers [T,D] bf16 owned by the caller
  * All other arguments as in bm_route / bm_moe_forward (weights, router and group map stay resident on
- * the device).
+ * the device).  Batches of T >= 2 * HOST_CHUNK_T tokens (option, default 2048; 0 = never) are processed in up to 8
+ * token chunks so that the copies of neighbouring chunks overlap the compute of the current one (two internal copy
+ * streams and their events are created on first use, once per device -- the one place where the library owns CUDA
+ * objects).  `out` is the same either way; the routing arrays then hold each chunk's result in the chunk's slice
+ * ([t0*K, (t0+tc)*K) of the [T,K] arrays, row indices relative to the chunk) and counts / offsets those of the LAST
+ * chunk: call bm_route yourself when you need the whole batch's permutation.
  */
 int bm_moe_layer_host(const bm_bf16 *x_host, int T, int D, const bm_bf16 *W_router,
                       const float *router_bias, int E, int K, const int32_t *group_map, int G,
@@ -315,6 +320,7 @@ int bm_device_status(void *workspace, int32_t *host_out, bm_stream_t stream);
  *   GEMV_FUSE (1)           matrix-vector path: fuse the W2 stage with the combine
  *   DC_R1, DC_R2, DC_KS2, DC_RMAX, DC_KS_FORCE (0, 0, 1, 128, 0)   decode tiling overrides (rows per tile, K splits)
  *   DC_STAGES, PF_STAGES (12)   cap on the shared-memory ring depth
+ *   HOST_CHUNK_T (2048)     bm_moe_layer_host: tokens per pipelined chunk; 0 = one piece
  *   ROUTER_FILTER (1)       T >= 512, E <= 256, K <= 8, E >= 4K + 8: tensor-core filter + canonical refinement of the
  *                           candidates; 0 = all E dots; 2 = the filter whenever the kernel supports the shape
  *   DC_KPACK (2)            decode kernels: k-blocks per ring stage

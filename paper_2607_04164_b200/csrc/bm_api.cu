@@ -36,7 +36,7 @@ static const OptDef kOptDefs[OPT_COUNT] = {
     {"GEMV_ROWS", 1}, {"GEMV_MAX_T", 2}, {"GEMV_FUSE", 1}, {"DC_RMAX", 128}, {"DC_KS_FORCE", 0}, {"DC_STAGES", 12},
     {"PF_STAGES", 12}, {"DC_R1", 0}, {"DC_R2", 0}, {"DC_KS2", 1}, {"PF_PAIR", -1}, {"PF_GATHER", 1},
     {"COMBINE_WARPS", 64}, {"PERM_SMALL_WARPS", 0}, {"ROUTER_WE", 0}, {"ROUTER_TP_MIN_T", kSplitRouterMaxT},
-    {"ROUTER_SPLIT_MAX_T", 16}, {"FUSED_COMBINE", -1}, {"PF_G1_BC", -1}, {"PF_G2_BC", -1}, {"PF_G2_BW", -1}, {"PF_G1_HINTS", -1}, {"PF_G2_HINTS", -1}, {"DC_DENSE_MAX_T", kDenseMaxT}, {"DC_PREFETCH_MB", 48}, {"DC_KPACK", 2}, {"ROUTER_FILTER", 1},
+    {"ROUTER_SPLIT_MAX_T", 16}, {"FUSED_COMBINE", -1}, {"PF_G1_BC", -1}, {"PF_G2_BC", -1}, {"PF_G2_BW", -1}, {"PF_G1_HINTS", -1}, {"PF_G2_HINTS", -1}, {"DC_DENSE_MAX_T", kDenseMaxT}, {"DC_PREFETCH_MB", 48}, {"DC_KPACK", 2}, {"ROUTER_FILTER", 1}, {"HOST_CHUNK_T", 2048},
 };
 static int g_opt[OPT_COUNT];
 static bool init_options() {
@@ -380,25 +380,85 @@ int bm_moe_forward(const bm_bf16 *x, int T, int D, const bm_routing *routing, co
                                BM_PATH_AUTO);
 }
 
+// Copy streams and events of bm_moe_layer_host's chunk pipeline, created on first use, one set per device.
+constexpr int kHostMaxChunks = 8;
+struct HostPipe { bool ready = false; cudaStream_t in = nullptr, out = nullptr; cudaEvent_t ev_in[kHostMaxChunks], ev_cmp[kHostMaxChunks], ev_done; };
+static HostPipe g_pipe[kMaxDevices];
+
+static HostPipe *host_pipe() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return nullptr;
+    std::lock_guard<std::mutex> lock(g_dev_mutex);
+    HostPipe &p = g_pipe[dev];
+    if (!p.ready) {
+        if (cudaStreamCreateWithFlags(&p.in, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaStreamCreateWithFlags(&p.out, cudaStreamNonBlocking) != cudaSuccess)
+            return nullptr;
+        for (int i = 0; i < kHostMaxChunks; ++i)
+            if (cudaEventCreateWithFlags(&p.ev_in[i], cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&p.ev_cmp[i], cudaEventDisableTiming) != cudaSuccess)
+                return nullptr;
+        if (cudaEventCreateWithFlags(&p.ev_done, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+        p.ready = true;
+    }
+    return &p;
+}
+
 int bm_moe_layer_host(const bm_bf16 *x_host, int T, int D, const bm_bf16 *W_router, const float *router_bias, int E,
                       int K, const int32_t *group_map, int G, const bm_bf16 *W1, const bm_bf16 *W3,
                       const bm_bf16 *W2, int F, int S, bm_bf16 *out_host, bm_bf16 *x_dev, bm_bf16 *out_dev,
                       bm_routing *routing, void *workspace, size_t workspace_bytes, bm_stream_t stream) {
-    if (T < 0) return BM_ERR_SHAPE;
+    if (T < 0 || K < 1 || D < 8) return BM_ERR_SHAPE;
+    if (!routing) return BM_ERR_NULL;
     if (T > 0 && (!x_host || !out_host || !x_dev || !out_dev)) return BM_ERR_NULL;
     if (device_ok() != 1) return BM_ERR_CUDA;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-    const size_t bytes = (size_t)T * D * sizeof(bm_bf16);
-    if (T > 0 && cudaMemcpyAsync(x_dev, x_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return BM_ERR_CUDA;
-    int rc = bm_route(x_dev, T, D, W_router, router_bias, E, K, group_map, G, routing, workspace, workspace_bytes,
-                      stream);
-    if (rc != BM_OK) return rc;
-    rc = bm_moe_forward(x_dev, T, D, routing, W1, W3, W2, F, S, out_dev, workspace, workspace_bytes, stream);
-    if (rc != BM_OK) return rc;
-    if (T > 0 && cudaMemcpyAsync(out_host, out_dev, bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+    const size_t row_bytes = (size_t)D * sizeof(bm_bf16);
+    // Large batches go through in token chunks (tokens are independent: the layer on a chunk is the layer on its tokens):
+    // the host->device copy of chunk c+1 and the device->host copy of chunk c-1 run on two copy streams while chunk c
+    // computes, so a PCIe-bound step (BJ:configs[2]: 67 MB each way) costs its compute time plus one chunk of copies.
+    const int chunk_t = opt(OPT_HOST_CHUNK_T);
+    int n_chunks = (chunk_t > 0 && T >= 2 * chunk_t) ? (T + chunk_t - 1) / chunk_t : 1;
+    if (n_chunks > kHostMaxChunks) n_chunks = kHostMaxChunks;
+    HostPipe *pipe = n_chunks > 1 ? host_pipe() : nullptr;
+    if (!pipe) n_chunks = 1;
+    if (n_chunks == 1) {
+        if (T > 0 && cudaMemcpyAsync(x_dev, x_host, (size_t)T * row_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return BM_ERR_CUDA;
+        int rc = bm_route(x_dev, T, D, W_router, router_bias, E, K, group_map, G, routing, workspace, workspace_bytes, stream);
+        if (rc != BM_OK) return rc;
+        rc = bm_moe_forward(x_dev, T, D, routing, W1, W3, W2, F, S, out_dev, workspace, workspace_bytes, stream);
+        if (rc != BM_OK) return rc;
+        if (T > 0 && cudaMemcpyAsync(out_host, out_dev, (size_t)T * row_bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+            return BM_ERR_CUDA;
+        return cudaStreamSynchronize(st) == cudaSuccess ? BM_OK : BM_ERR_CUDA;
+    }
+    const int per = ((T + n_chunks - 1) / n_chunks + 127) & ~127;       // tokens per chunk, whole 128-row tiles
+    // the copy streams start after whatever the caller queued on `stream` before this call
+    if (cudaEventRecord(pipe->ev_done, st) != cudaSuccess || cudaStreamWaitEvent(pipe->in, pipe->ev_done, 0) != cudaSuccess ||
+        cudaStreamWaitEvent(pipe->out, pipe->ev_done, 0) != cudaSuccess)
         return BM_ERR_CUDA;
-    if (cudaStreamSynchronize(st) != cudaSuccess) return BM_ERR_CUDA;
-    return BM_OK;
+    const bm_routing whole = *routing;
+    int c = 0;
+    for (int t0 = 0; t0 < T; t0 += per, ++c) {
+        const int tc = T - t0 < per ? T - t0 : per;
+        if (cudaMemcpyAsync(x_dev + (size_t)t0 * D, x_host + (size_t)t0 * D, (size_t)tc * row_bytes, cudaMemcpyHostToDevice, pipe->in) != cudaSuccess ||
+            cudaEventRecord(pipe->ev_in[c], pipe->in) != cudaSuccess || cudaStreamWaitEvent(st, pipe->ev_in[c], 0) != cudaSuccess)
+            return BM_ERR_CUDA;
+        bm_routing r = whole;          // the chunk's slices of the caller's arrays; counts / offsets are reused chunk after chunk
+        r.expert_ids += (size_t)t0 * K; r.group_ids += (size_t)t0 * K; r.gate_w += (size_t)t0 * K; r.n_slots += t0;
+        r.row_token += (size_t)t0 * K; r.row_slot += (size_t)t0 * K; r.slot_row += (size_t)t0 * K;
+        int rc = bm_route(x_dev + (size_t)t0 * D, tc, D, W_router, router_bias, E, K, group_map, G, &r, workspace, workspace_bytes, stream);
+        if (rc != BM_OK) return rc;
+        rc = bm_moe_forward(x_dev + (size_t)t0 * D, tc, D, &r, W1, W3, W2, F, S, out_dev + (size_t)t0 * D, workspace, workspace_bytes, stream);
+        if (rc != BM_OK) return rc;
+        if (cudaEventRecord(pipe->ev_cmp[c], st) != cudaSuccess || cudaStreamWaitEvent(pipe->out, pipe->ev_cmp[c], 0) != cudaSuccess ||
+            cudaMemcpyAsync(out_host + (size_t)t0 * D, out_dev + (size_t)t0 * D, (size_t)tc * row_bytes, cudaMemcpyDeviceToHost, pipe->out) != cudaSuccess)
+            return BM_ERR_CUDA;
+        routing->T = r.T; routing->E = r.E; routing->K = r.K; routing->G = r.G;
+    }
+    if (cudaEventRecord(pipe->ev_done, pipe->out) != cudaSuccess || cudaStreamWaitEvent(st, pipe->ev_done, 0) != cudaSuccess)
+        return BM_ERR_CUDA;
+    return cudaStreamSynchronize(st) == cudaSuccess ? BM_OK : BM_ERR_CUDA;
 }
 
 int bm_device_status(void *workspace, int32_t *host_out, bm_stream_t stream) {

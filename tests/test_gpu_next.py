@@ -303,3 +303,22 @@ def test_tp_moe_forward_under_a_real_nccl_process_group():
             assert_out_close(out.float().cpu().numpy().astype(np.float64), ref)
     finally:
         dist.destroy_process_group()
+
+
+def test_bench_device_layer_tensor_parallel_step_runs_and_matches_oracle():
+    """bench.py's DeviceLayer with tp=(rank, world) (the `--parallel tp` arm): round 1's version raised AttributeError on
+    the first step.  One rank of one: the F shard is the whole F, so the step must reproduce the layer."""
+    import sys, os
+    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    import bench
+    from bm_inputs import CONFIGS
+    import paper_2607_04164_b200 as bm
+    cfg = CONFIGS["tiny"]
+    layer = bench.DeviceLayer(cfg, seed=0, x_seed=0, keep_host_weights=True, tp=(0, 1))
+    layer.step()
+    torch.cuda.synchronize()
+    L = layer.host
+    o = oracle.route(bf16_bits(L.x), bf16_bits(L.W_router), None, cfg.K, L.group_map.numpy(), cfg.G)
+    ref = oracle.moe_forward(bf16_bits(L.x), o, bf16_bits(L.W1), bf16_bits(L.W3), bf16_bits(L.W2), cfg.S)
+    assert_out_close(layer.out.float().cpu().numpy().astype(np.float64), ref)
+    assert bm.bm_device_status(layer.ws) == 0

@@ -420,3 +420,31 @@ def test_layer_host_repeated_calls_with_new_data(own_stream):
         assert_routing_equal(routing_to_numpy(r, T), o)
         assert_out_close(out_pin.float().numpy().astype(np.float64), oracle_forward(L, o))
     assert bm.bm_device_status(ws) == 0
+
+
+def test_layer_host_chunk_pipeline_matches_oracle():
+    """bm_moe_layer_host on a batch large enough for the chunk pipeline (copies of neighbouring chunks overlap compute):
+    `out` must be that of the whole batch; called twice to show that buffers, copy streams and the zero regions are reusable."""
+    import paper_2607_04164_b200 as bm
+    rng = np.random.default_rng(78)
+    T, D, F, E, K, G, S = 3000, 256, 320, 12, 3, 4, 1
+    L = rand_layer(rng, T=T, D=D, F=F, E=E, K=K, G=G, S=S, bias=True)
+    d = to_device(L)
+    ws = bm.alloc_workspace(T, D, F, E, K, G, S)
+    r = bm.Routing(T, K, G)
+    x_pin = L.x.pin_memory()
+    out_pin = torch.empty((T, D), dtype=torch.bfloat16).pin_memory()
+    x_dev = torch.empty((T, D), dtype=torch.bfloat16, device="cuda")
+    out_dev = torch.empty((T, D), dtype=torch.bfloat16, device="cuda")
+    o = oracle_route(L)
+    want = oracle_forward(L, o)
+    with bm.options(HOST_CHUNK_T=512):                             # 6 chunks of 512 tokens (the last one ragged)
+        for _ in range(2):
+            out_pin.fill_(float("nan"))
+            bm.bm_moe_layer_host(x_pin, d.W_router, d.router_bias, K, d.group_map, G, d.W1, d.W3, d.W2, S, out_pin,
+                                 x_dev, out_dev, r, ws)
+            assert_out_close(out_pin.float().numpy().astype(np.float64), want)
+    assert bm.bm_device_status(ws) == 0
+    # the last chunk's slice of the routing arrays holds that chunk's (chunk-relative) routing: expert ids are global facts
+    g = routing_to_numpy(r, T)
+    assert (g.expert_ids == o.expert_ids).all()
