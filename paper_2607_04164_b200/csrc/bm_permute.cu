@@ -37,8 +37,11 @@ permute_small_kernel(const int32_t *__restrict__ group_ids, int T, int K, int G,
                      int32_t *__restrict__ slot_row, int32_t *__restrict__ status) {
     extern __shared__ int s_mem[];
     __shared__ int s_total;
-    grid_dep_wait();
+    // This one-CTA kernel lets its successor start BEFORE it waits for the router: the successor (a GEMM1 kernel) only
+    // sets up barriers and TMEM and asks L2 for weights ahead of its own grid-dependency wait, and that wait still covers
+    // this kernel and, through its wait below, the router.  The weight prefetch then overlaps router + permutation.
     grid_dep_launch();
+    grid_dep_wait();
     permute_block_small(group_ids, T, K, G, per_warp, counts, offsets, row_token, row_slot, slot_row, status, s_mem,
                         &s_total);
 }
