@@ -448,3 +448,34 @@ def test_layer_host_chunk_pipeline_matches_oracle():
     # the last chunk's slice of the routing arrays holds that chunk's (chunk-relative) routing: expert ids are global facts
     g = routing_to_numpy(r, T)
     assert (g.expert_ids == o.expert_ids).all()
+
+
+def test_one_workspace_serves_changing_batch_sizes():
+    """include/bm.h "Workspace": one initialised workspace serves any T <= T_max; its zero regions (accumulator and tickets of
+    the fused combine, anchored at the buffer's end) must be all-zero again after every call whatever T and path the call
+    took.  Batches of different sizes go through the same workspace and routing arrays in a mixed order -- dense decode,
+    gathered decode + finalize pass, fused and two-pass prefill tiles, matrix-vector -- each checked against the oracle."""
+    import paper_2607_04164_b200 as bm
+    rng = np.random.default_rng(321)
+    T_max, D, F, E, K, G, S = 900, 512, 4096, 12, 2, 4, 1        # F = 4096: the prefill tiles take the fused combine
+    L = rand_layer(rng, T=T_max, D=D, F=F, E=E, K=K, G=G, S=S, bias=True, wstd=0.02)
+    d = to_device(L)
+    ws = bm.alloc_workspace(T_max, D, F, E, K, G, S)
+    r = bm.Routing(T_max, K, G)
+    from types import SimpleNamespace
+    for i, T in enumerate([900, 1, 40, 300, 7, 900, 130, 64, 2, 500]):
+        sub = SimpleNamespace(**vars(L)); sub.T = T; sub.x = L.x[:T].contiguous()
+        o = oracle_route(sub)
+        want = oracle_forward(sub, o)
+        xd = d.x[:T].contiguous()
+        out = torch.full((T, D), float("nan"), dtype=torch.bfloat16, device="cuda")
+        with bm.options(FUSED_COMBINE=(0 if i % 4 == 3 else -1)):
+            bm.bm_route(xd, d.W_router, d.router_bias, K, d.group_map, G, r, ws)
+            bm.bm_moe_forward(xd, r, d.W1, d.W3, d.W2, out, ws, S=S)
+        torch.cuda.synchronize()
+        assert bm.bm_device_status(ws) == 0
+        assert_routing_equal(routing_to_numpy(r, T), o)
+        assert_out_close(out.float().cpu().numpy().astype(np.float64), want)
+    # and the regions really are clean: everything behind the front sections reads zero
+    tail = ws[-(T_max * D * 4):]
+    assert int(tail.count_nonzero()) == 0
