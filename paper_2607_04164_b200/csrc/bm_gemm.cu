@@ -14,13 +14,15 @@
 // Pipelines: a 4-stage shared-memory ring (full/empty mbarriers, 48 KB per stage, 128B-swizzled K-major
 // tiles written by TMA) and two TMEM accumulator stages of 256 columns (tmem_full/tmem_empty), so the
 // epilogue of item i overlaps the main loop of item i+1.  Work items are enumerated identically by all
-// roles from a small device-side schedule (non-empty segments and their 128-row chunks) that the prep
-// kernel builds from counts/offsets -- the host never sees the data-dependent counts.
+// roles from a small schedule (non-empty segments and their 128-row chunks) that warp 0 of every CTA builds in
+// shared memory from counts/offsets (build_schedule) -- the host never sees the data-dependent counts.
 //
-// Combine.  A token's <= K group rows live in different tiles.  Prefill: GEMM2 stores y rows (bf16, coalesced
-// 128-byte pieces) and combine_kernel sums a token's rows in slot order with the gate weights -- no
-// atomics, deterministic.  Decode: rows also live in different K-splits and there are few of them, so the
-// partials are added in fp32 with red.global.add into `out_acc` and a last pass rounds to bf16.
+// Combine.  A token's <= K group rows live in different tiles.  Fused form (FC; prefill tiles with F >= 4096, decode up
+// to 64 tokens): the GEMM2 epilogue adds gate_w * y into the fp32 accumulator out_acc with red.global.add (vectorised and
+// row-coalesced on the prefill tiles), takes a ticket, and the arrival that completes an output piece rounds it to bf16
+// and clears accumulator and ticket -- no y rows, no combine / finalize kernel, no zeroing pass.  Two-pass form where the
+// fused epilogue was measured slower: prefill tiles store y rows (bf16, coalesced 128-byte pieces) and combine_kernel sums
+// a token's rows in slot order (deterministic); the decode kernel's reductions are rounded and cleared by finalize_kernel.
 #include <algorithm>
 #include <mutex>
 
@@ -498,7 +500,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
         // Completion is signalled by the hardware: cp.async.mbarrier.arrive.noinc makes the thread's arrival on the
         // stage's gfull barrier happen when its copies have landed, so the thread never waits for its own copies and
         // the whole ring depth stays in flight (a cp.async.wait_group + arrive version kept only 2-3 k-blocks in
-        // flight: 3x slower with CTA pairs).  This replaces the xs pass of the prep kernel: A*D*4 bytes of HBM
+        // flight: 3x slower with CTA pairs).  This replaces the separate gather pass (gather_kernel): A*D*4 bytes of HBM
         // traffic and a launch-wide pass less.
         const int g = (int)threadIdx.x - kThreads;
         const int j = g & 7, rg = g >> 3;
