@@ -76,3 +76,53 @@ def test_argument_errors_are_reported_before_any_device_work():
         r2 = BmRouting(0, 0, 2, 2, *([addr] * 9))
         rc = L.bm_route(p, 4, 64, p, None, 8, 2, p, 2, ctypes.byref(r2), p, 1 << 20, None)
         assert rc == -5, "without a CUDA device the product path must fail loudly, not fall back"
+
+
+def test_options_round_trip_and_unknown_name():
+    import paper_2607_04164_b200 as bm
+    old = bm.get_option("PF_PAIR")
+    with bm.options(PF_PAIR=1, FUSED_COMBINE=0):
+        assert bm.get_option("PF_PAIR") == 1 and bm.get_option("FUSED_COMBINE") == 0
+    assert bm.get_option("PF_PAIR") == old and bm.get_option("FUSED_COMBINE") == -1
+    with pytest.raises(bm.BmError) as ei:
+        bm.set_option("NO_SUCH_OPTION", 1)
+    assert ei.value.code == -2
+    # every option documented in bm.h exists in the library, and the other way round the table has no undocumented name
+    src = open(os.path.join(ROOT, "include", "bm.h")).read()
+    doc = src[src.index(" * Options:"):src.index("int bm_set_option")]
+    names = []
+    for line in doc.splitlines():
+        m = re.match(r" \*   ([A-Z][A-Z0-9_]+(?: \([-0-9]+\))?(?:, [A-Z][A-Z0-9_]+(?: \([-0-9]+\))?)*)", line)
+        if m:
+            names += re.findall(r"[A-Z][A-Z0-9_]+", m.group(1))
+    assert len(names) >= 25
+    for name in names:
+        bm.get_option(name)
+
+
+def test_forward_info_is_a_host_call():
+    """bm_forward_info answers from the host-side sizes alone (no device needed): path and determinism (include/bm.h)."""
+    import paper_2607_04164_b200 as bm
+    assert bm.bm_forward_info(1, 4, 60, 0, 2048, 1408) == (bm.BM_PATH_GEMV, True)
+    assert bm.bm_forward_info(8192, 2, 4, 0, 4096, 14336) == (bm.BM_PATH_PREFILL, True)      # fused, two sources
+    assert bm.bm_forward_info(4096, 6, 16, 2, 2048, 1408) == (bm.BM_PATH_PREFILL, True)      # F < 4096: two-pass, slot order
+    path, det = bm.bm_forward_info(4096, 4, 60, 0, 2048, 4096)
+    assert path == bm.BM_PATH_PREFILL and not det                                             # fused, four sources
+    path, det = bm.bm_forward_info(64, 2, 4, 0, 4096, 14336)
+    assert path == bm.BM_PATH_DECODE and not det                                              # K splits: order varies
+    with pytest.raises(bm.BmError):
+        bm.bm_forward_info(4, 99, 4, 0, 64, 64)
+
+
+def test_workspace_layout_invariants():
+    """bm_workspace_bytes: monotone in T (a workspace for T_max serves every smaller batch), zero for arguments no call
+    accepts, and large enough for the dense decode rows (one H row per active set and token up to 64 tokens)."""
+    import paper_2607_04164_b200 as bm
+    prev = 0
+    for T in (0, 1, 2, 16, 63, 64, 65, 128, 511, 512, 4096, 8192):
+        n = bm.workspace_bytes(T, 2048, 1408, 60, 4, 60, 0)
+        assert n >= prev
+        prev = n
+    assert bm.workspace_bytes(64, 2048, 1408, 60, 4, 60, 0) >= 60 * 64 * 1408 * 2            # dense H rows
+    assert bm.workspace_bytes(64, 256, 512, 8, 2, 4, 17) == 0                                  # S > BM_MAX_S
+    assert bm.BM_MAX_S == 16
