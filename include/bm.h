@@ -188,9 +188,9 @@ int bm_group_mse(const bm_bf16 *Y, const bm_bf16 *U, int T, int D, const int32_t
  * with FFN_u(x) = W2[u] . ( SiLU(W1[u] x) * (W3[u] x) )   (P:42 with united experts P:46; SwiGLU: A3).
  * bf16 operands, fp32 accumulation (tensor cores; CUDA-core FFMA2 on the matrix-vector path), the intermediate h
  * is rounded to bf16 (A12).  The gate-weighted sum is taken in fp32:
- *   - tensor-core paths (decode, prefill): fused into the W2 GEMM's epilogue -- gw * y is added into an fp32
- *     accumulator with vector reductions, the arrival that completes an output piece rounds it to bf16 (north_star
- *     kernel (4)).  fp32 addition is commutative, so the result is bit-deterministic when no token has more than two
+ *   - tensor-core paths (decode, prefill): the W2 GEMM's epilogue adds gw * y into an fp32 accumulator with
+ *     reductions; on the prefill tiles (F >= 4096) the arrival that completes an output piece also rounds it to bf16
+ *     inside the kernel (north_star kernel (4)), on the decode kernel a small finalize pass does.  fp32 addition is commutative, so the result is bit-deterministic when no token has more than two
  *     source rows (K + S <= 2, and no K split on the decode path); with more sources the order of the additions, hence
  *     the last bits before the bf16 rounding, may vary between calls.  bm_forward_info tells which case a call is in.
  *   - matrix-vector path and the two-pass prefill form (F < 4096 by default, or option FUSED_COMBINE = 0): slot order,
@@ -306,7 +306,7 @@ int bm_device_status(void *workspace, int32_t *host_out, bm_stream_t stream);
  *   PDL (1)                 programmatic dependent launch between the kernels of a call
  *   FUSED_COMBINE (-1)      1 = combine fused into the W2 GEMM epilogue, 0 = separate pass (prefill tiles: bf16 y rows +
  *                           slot-order sum, deterministic; decode kernel: finalize pass); -1 = by shape: prefill tiles fused
- *                           from F = 4096 on, decode kernel up to 64 tokens
+ *                           from F = 4096 on, decode kernel never (its finalize pass measured faster)
  *   PF_PAIR (-1)            prefill tiles: 1 / 0 force CTA pairs (cta_group::2) on / off, -1 = by rows per group
  *   PF_GATHER (1)           0 = materialise gathered rows, 1 = gather inside GEMM1 on single-CTA tiles, 2 = also with pairs
  *   PF_G1_BC, PF_G2_BC, PF_G2_BW (-1)   prefill tiles: L2 bands of the item order -- chunk units per band in GEMM1 / GEMM2,

@@ -1264,14 +1264,16 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
     // Combine: fused into the GEMM2 epilogue (fp32 reductions into the zero region + last-arriver rounding) unless
     // option FUSED_COMBINE = 0 asks for the two-pass form on the prefill tiles (bf16 y rows + combine_kernel, slot
     // order: bit-deterministic for any K + S).  The decode kernel always finishes its output itself.
-    // The decode kernel finishes its output itself up to 64 tokens; beyond, its items are so short that the fence and
-    // ticket per item cost more than a separate pass (G = 60, T = 256: 218 us fused, 185 us with the finalize kernel).
+    // Decode kernel: its reductions are rounded and cleared by finalize_kernel.  Finishing inside the kernel (FC: fence +
+    // ticket per item, the last arriver of a piece rounds it) saves that launch but was slower wherever it was measured --
+    // G = 15, T = 16: 58.8 vs 54.9 us; G = 60, T = 16: 98.4 vs 92.7; G = 60, T = 256: 218 vs 190; BJ:configs[1]: equal --
+    // because the items are short and the fence waits for the item's reductions; option FUSED_COMBINE = 1 selects it.
     // Prefill tiles: the fused epilogue (scale, transpose, vector reductions, fence, ticket, finish) takes ~10 us per
     // 128 x 256 tile and hides behind the tile's main loop only when the W2 reduction is long: fused from F = 4096 on
     // (Mixtral: 56 us per tile; also where the outputs are large enough for the fp32 sum to matter against the
     // tolerance), the two-pass form below (Qwen-like F = 1408: 6 us per tile; measured 5-10% faster there).
     const int fc_opt = opt(OPT_FUSED_COMBINE);
-    const bool fused = decode ? (fc_opt < 0 ? a.T <= kDenseMaxT : fc_opt != 0) : (fc_opt < 0 ? a.F >= 4096 : fc_opt != 0);
+    const bool fused = decode ? fc_opt == 1 : (fc_opt < 0 ? a.F >= 4096 : fc_opt != 0);
 
     // CTA pairs (cta_group::2, M = 256 per pair): a pair shares the weight tile, so a CTA stages 32 KB per
     // k-block instead of 48 KB (measured: GEMM1 232 -> 201 us at BJ:configs[3]).  A segment with an odd chunk

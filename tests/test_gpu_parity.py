@@ -361,8 +361,9 @@ VARIANTS = [
     (PATHS["prefill"], {"FUSED_COMBINE": 0, "PF_PAIR": 1}),
     (PATHS["prefill"], {"FUSED_COMBINE": 1}),                  # combine fused into the W2 GEMM epilogue
     (PATHS["prefill"], {"FUSED_COMBINE": 1, "PF_PAIR": 1}),
-    (PATHS["decode"], {"FUSED_COMBINE": 0}),                   # decode kernel + finalize pass
-    (PATHS["decode"], {"FUSED_COMBINE": 1, "DC_DENSE_MAX_T": 0}),   # gathered rows, in-kernel finish
+    (PATHS["decode"], {"FUSED_COMBINE": 1}),                   # decode kernel finishing its output itself (tickets)
+    (PATHS["decode"], {"FUSED_COMBINE": 1, "DC_DENSE_MAX_T": 0}),   # the same on gathered rows
+    (PATHS["decode"], {"DC_DENSE_MAX_T": 0, "DC_KPACK": 1}),   # gathered rows, one k-block per stage, finalize pass
     (0, {"ROUTER_TP_MIN_T": 1, "ROUTER_FILTER": 0}),           # throughput router (all E canonical dots) on any T
     (0, {"ROUTER_TP_MIN_T": 1, "ROUTER_FILTER": 2}),           # tensor-core filter + refinement on any T
     (0, {"ROUTER_SPLIT_MAX_T": 511}),                          # split router (+ fused permutation) on any T < 512
