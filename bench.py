@@ -186,11 +186,12 @@ class DeviceLayer:
 
     def step(self):
         bm, c = self.bm, self.cfg
-        bm.bm_route(self.x, self.W_router, self.bias, c.K, self.gmap, c.G, self.routing, self.ws)
         if self.tp is not None:     # F-sharded weights: fp32 partial, NCCL all-reduce, one rounding
+            bm.bm_route(self.x, self.W_router, self.bias, c.K, self.gmap, c.G, self.routing, self.ws)
             bm.tp_moe_forward(self.x, self.routing, self.W1, self.W3, self.W2, self.out, self.ws, S=c.S, partial=self.partial)
-        else:
-            bm.bm_moe_forward(self.x, self.routing, self.W1, self.W3, self.W2, self.out, self.ws, S=c.S)
+        else:                       # the whole hot path: bm_route + bm_moe_forward (one call; one kernel for single-token decode)
+            bm.bm_moe_layer(self.x, self.W_router, self.bias, c.K, self.gmap, c.G, self.W1, self.W3, self.W2, self.out,
+                            self.routing, self.ws, S=c.S)
 
     def step_host(self):
         bm, c = self.bm, self.cfg
@@ -504,14 +505,15 @@ def run_ours(args):
 # BJ:configs[4]: the brownout sweep (tokens/s and % roofline per point)
 # ---------------------------------------------------------------------------------------------------
 class SweepWeights:
-    """United weights of one G, kept as L distinct copies so that L * weight_bytes >= 512 MB: successive
-    steps read different addresses and no weight byte is served from the 126 MB L2 (SURVEY.md 8(d),
-    "cold weights"; a real model has 24 such layers)."""
+    """United weights of one G, kept as L distinct copies so that successive steps read different addresses and no
+    weight byte is served from the 126 MB L2 ("cold weights"; a real model has 24 such layers,
+    PAPER.md:267).  What must exceed L2 is what a step TOUCHES, not what is allocated: a batch of T tokens touches at most
+    min(G, T*K) weight sets (a single token at G = 60 touches 4 of 60: 69 MB, which one copy would leave L2-resident
+    step after step -- round 1's T = 1 figures at G = 30 and 60 had that flaw), so L * touched bytes >= 512 MB."""
 
-    def __init__(self, cfg, seed=0, min_bytes=512e6):
+    def __init__(self, cfg, seed=0, min_bytes=512e6, copies=None):
         L = make_layer(cfg, seed)
-        one = 3 * cfg.G * cfg.F * cfg.D * 2
-        self.copies = max(1, int(-(-min_bytes // one)))
+        self.copies = copies or self.copies_for(cfg, min_bytes)
         self.W1 = [L.W1.cuda()]
         self.W3 = [L.W3.cuda()]
         self.W2 = [L.W2.cuda()]
@@ -519,6 +521,11 @@ class SweepWeights:
             self.W1.append(self.W1[0].clone()); self.W3.append(self.W3[0].clone()); self.W2.append(self.W2[0].clone())
         self.W_router = L.W_router.cuda()
         self.gmap = L.group_map.cuda()
+
+    @staticmethod
+    def copies_for(cfg, min_bytes=512e6):
+        touched = 3 * (min(cfg.G, cfg.T * cfg.K) + cfg.S) * cfg.F * cfg.D * 2
+        return max(1, int(-(-min_bytes // touched)))
 
 
 class SweepPoint:
@@ -537,8 +544,8 @@ class SweepPoint:
         bm, c, W = self.bm, self.cfg, self.W
         j = self.i % W.copies
         self.i += 1
-        bm.bm_route(self.x, W.W_router, self.bias, c.K, W.gmap, c.G, self.routing, self.ws, stream=stream)
-        bm.bm_moe_forward(self.x, self.routing, W.W1[j], W.W3[j], W.W2[j], self.out, self.ws, S=c.S, stream=stream)
+        bm.bm_moe_layer(self.x, W.W_router, self.bias, c.K, W.gmap, c.G, W.W1[j], W.W3[j], W.W2[j], self.out, self.routing,
+                        self.ws, S=c.S, stream=stream)
 
 
 def time_point(pt, steps, warmup):
@@ -596,11 +603,12 @@ def run_sweep(args):
     sampler = ClockSampler(0)
     with sampler:
         for cfg in pts:
-            if cfg.G not in cache:
+            key = (cfg.G, SweepWeights.copies_for(cfg))
+            if key not in cache:
                 cache.clear()
                 torch.cuda.empty_cache()
-                cache[cfg.G] = SweepWeights(cfg)
-            W = cache[cfg.G]
+                cache[key] = SweepWeights(cfg)
+            W = cache[key]
             pt = SweepPoint(cfg, W)
             steps = 200 if cfg.T <= 256 else (40 if cfg.T <= 4096 else 12)
             steps = max(steps // W.copies * W.copies, W.copies)

@@ -207,6 +207,18 @@ int bm_moe_forward(const bm_bf16 *x, int T, int D, const bm_routing *routing, co
                    size_t workspace_bytes, bm_stream_t stream);
 
 /*
+ * bm_moe_layer -- bm_route followed by bm_moe_forward on device buffers, as one call: out and every routing array are
+ * written exactly as by the two calls.  Having the whole step in one call lets the library run single-token decode
+ * (T <= 2 with T*K <= G, the matrix-vector rule of BM_PATH_AUTO) as ONE persistent kernel -- router dots, selection,
+ * W1/W3 stream, W2 stream + combine separated by two grid-wide barriers (cooperative launch) instead of three
+ * dependent launches; every other shape takes the two calls.  Option LAYER_SMALL = 0 switches the single kernel off.
+ * Arguments as in bm_route / bm_moe_forward (full brownout: no cold mask).
+ */
+int bm_moe_layer(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, const float *router_bias, int E, int K,
+                 const int32_t *group_map, int G, const bm_bf16 *W1, const bm_bf16 *W3, const bm_bf16 *W2, int F, int S,
+                 bm_bf16 *out, bm_routing *routing, void *workspace, size_t workspace_bytes, bm_stream_t stream);
+
+/*
  * Tensor parallelism over F (the paper scales with tensor parallelism).
  * SwiGLU is elementwise over the F hidden features, so with W1, W3 row-sharded and W2 column-sharded over N ranks
  *     FFN_u(x) = sum_r W2_r[u] . ( SiLU(W1_r[u] x) * (W3_r[u] x) ),     W1_r, W3_r [G+S, F/N, D],  W2_r [G+S, D, F/N]
@@ -320,6 +332,7 @@ int bm_device_status(void *workspace, int32_t *host_out, bm_stream_t stream);
  *   GEMV_FUSE (1)           matrix-vector path: fuse the W2 stage with the combine
  *   DC_R1, DC_R2, DC_KS2, DC_RMAX, DC_KS_FORCE (0, 0, 1, 128, 0)   decode tiling overrides (rows per tile, K splits)
  *   DC_STAGES, PF_STAGES (12)   cap on the shared-memory ring depth
+ *   LAYER_SMALL (1)         bm_moe_layer: 1 = one persistent kernel for T <= 2 (single-token decode), 0 = the separate kernels
  *   HOST_CHUNK_T (2048)     bm_moe_layer_host: tokens per pipelined chunk; 0 = one piece
  *   ROUTER_FILTER (1)       T >= 512, E <= 256, K <= 8, E >= 4K + 8: tensor-core filter + canonical refinement of the
  *                           candidates; 0 = all E dots; 2 = the filter whenever the kernel supports the shape

@@ -19,7 +19,7 @@ BM_DEV_BAD_GROUP_MAP, BM_DEV_NONFINITE_LOGIT, BM_DEV_BAD_ROUTING = 1, 2, 4
 BM_MAX_E, BM_MAX_K, BM_MAX_G, BM_MAX_S = 512, 16, 512, 16
 BM_DECODE_MAX_T = 384
 
-EXPORTS = ["bm_expert_outputs_workspace_bytes", "bm_workspace_bytes", "bm_workspace_init", "bm_forward_info", "bm_set_option", "bm_get_option", "bm_route", "bm_route_partial", "bm_unite_weights", "bm_expert_histogram",
+EXPORTS = ["bm_moe_layer", "bm_expert_outputs_workspace_bytes", "bm_workspace_bytes", "bm_workspace_init", "bm_forward_info", "bm_set_option", "bm_get_option", "bm_route", "bm_route_partial", "bm_unite_weights", "bm_expert_histogram",
            "bm_expert_outputs", "bm_gram_workspace_bytes", "bm_cosine_gram", "bm_mse_workspace_bytes", "bm_group_mse",
            "bm_moe_forward", "bm_moe_forward_path", "bm_moe_forward_f32", "bm_round_bf16", "bm_moe_layer_host",
            "bm_device_status", "bm_launch_count", "bm_status_string", "bm_profile_enable", "bm_profile_read", "bm_profile_read_kinds",
@@ -110,6 +110,9 @@ def lib() -> ctypes.CDLL:
         L.bm_salc_cold_mask.argtypes = [c_void_p, c_int, ctypes.c_double, c_void_p]
         L.bm_moe_forward_path.restype = c_int
         L.bm_moe_forward_path.argtypes = L.bm_moe_forward.argtypes + [c_int]
+        L.bm_moe_layer.restype = c_int
+        L.bm_moe_layer.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_int, c_int, c_void_p, c_int,
+                                   c_void_p, c_void_p, c_void_p, c_int, c_int, c_void_p, POINTER(BmRouting), c_void_p, c_size_t, c_void_p]
         L.bm_moe_layer_host.restype = c_int
         L.bm_moe_layer_host.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_int, c_int, c_void_p, c_int,
                                         c_void_p, c_void_p, c_void_p, c_int, c_int, c_void_p, c_void_p, c_void_p,
@@ -432,6 +435,20 @@ def bm_salc_cold_mask(w, threshold):
     if rc != BM_OK:
         raise BmError(rc, "bm_salc_cold_mask")
     return mask
+
+
+def bm_moe_layer(x, W_router, router_bias, K: int, group_map, G: int, W1, W3, W2, out, routing: Routing, workspace,
+                 S: int = 0, stream=None):
+    """bm_route + bm_moe_forward as one call (include/bm.h: bm_moe_layer); single-token decode runs as one kernel."""
+    T, D = x.shape
+    E = W_router.shape[0]
+    _check_route_args(x, W_router, router_bias, group_map, routing, workspace, T, D, E, K, G)
+    _, _, F = _check_forward_args(x, routing, W1, W3, W2, out, torch.bfloat16, workspace, S)
+    rc = lib().bm_moe_layer(_ptr(x), T, D, _ptr(W_router), _ptr(router_bias), E, K, _ptr(group_map), G, _ptr(W1), _ptr(W3),
+                            _ptr(W2), F, S, _ptr(out), ctypes.byref(routing.c), _ptr(workspace), workspace.numel(), _stream(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_moe_layer")
+    return out
 
 
 def bm_moe_layer_host(x_host, W_router, router_bias, K, group_map, G, W1, W3, W2, S, out_host, x_dev, out_dev,

@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libbm.so")
 SOURCES = ["bm_api.cu", "bm_router.cu", "bm_permute.cu", "bm_gemm.cu", "bm_gemv.cu", "bm_simt.cu", "bm_unite.cu", "bm_calib.cu", "bm_salc.cu"]
-HEADERS = ["bm_common.cuh", "bm_ptx.cuh", "bm_permute.cuh", os.path.join("..", "..", "include", "bm.h")]
+HEADERS = ["bm_common.cuh", "bm_ptx.cuh", "bm_permute.cuh", "bm_router.cuh", os.path.join("..", "..", "include", "bm.h")]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     "-Xcompiler", "-fPIC", "--shared", "-cudart", "static",

@@ -36,7 +36,7 @@ static const OptDef kOptDefs[OPT_COUNT] = {
     {"GEMV_ROWS", 1}, {"GEMV_MAX_T", 2}, {"GEMV_FUSE", 1}, {"DC_RMAX", 128}, {"DC_KS_FORCE", 0}, {"DC_STAGES", 12},
     {"PF_STAGES", 12}, {"DC_R1", 0}, {"DC_R2", 0}, {"DC_KS2", 1}, {"PF_PAIR", -1}, {"PF_GATHER", 1},
     {"COMBINE_WARPS", 64}, {"PERM_SMALL_WARPS", 0}, {"ROUTER_WE", 0}, {"ROUTER_TP_MIN_T", kSplitRouterMaxT},
-    {"ROUTER_SPLIT_MAX_T", 16}, {"FUSED_COMBINE", -1}, {"PF_G1_BC", -1}, {"PF_G2_BC", -1}, {"PF_G2_BW", -1}, {"PF_G1_HINTS", -1}, {"PF_G2_HINTS", -1}, {"DC_DENSE_MAX_T", kDenseMaxT}, {"DC_PREFETCH_MB", 48}, {"DC_KPACK", 2}, {"ROUTER_FILTER", 1}, {"HOST_CHUNK_T", 2048},
+    {"ROUTER_SPLIT_MAX_T", 16}, {"FUSED_COMBINE", -1}, {"PF_G1_BC", -1}, {"PF_G2_BC", -1}, {"PF_G2_BW", -1}, {"PF_G1_HINTS", -1}, {"PF_G2_HINTS", -1}, {"DC_DENSE_MAX_T", kDenseMaxT}, {"DC_PREFETCH_MB", 48}, {"DC_KPACK", 2}, {"ROUTER_FILTER", 1}, {"HOST_CHUNK_T", 2048}, {"LAYER_SMALL", 1},
 };
 static int g_opt[OPT_COUNT];
 static bool init_options() {
@@ -380,6 +380,38 @@ int bm_moe_forward(const bm_bf16 *x, int T, int D, const bm_routing *routing, co
                                BM_PATH_AUTO);
 }
 
+int bm_moe_layer(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, const float *router_bias, int E, int K,
+                 const int32_t *group_map, int G, const bm_bf16 *W1, const bm_bf16 *W3, const bm_bf16 *W2, int F, int S,
+                 bm_bf16 *out, bm_routing *routing, void *workspace, size_t workspace_bytes, bm_stream_t stream) {
+    // one or two tokens whose sets expect at most one row (the matrix-vector rule of BM_PATH_AUTO): one persistent kernel
+    if (routing && T >= 1 && T <= 2 && opt(OPT_LAYER_SMALL) != 0 && resolve_auto_path(T, K, G) == BM_PATH_GEMV) {
+        int rc = check_shapes(T, D, F, E, K, G, S, true);
+        if (rc != BM_OK) return rc;
+        if (!x || !W_router || !group_map || !W1 || !W3 || !W2 || !out || !workspace || !routing->expert_ids ||
+            !routing->group_ids || !routing->gate_w || !routing->n_slots || !routing->counts || !routing->offsets ||
+            !routing->row_token || !routing->row_slot || !routing->slot_row)
+            return BM_ERR_NULL;
+        if (!aligned16(x) || !aligned16(W_router) || !aligned16(W1) || !aligned16(W3) || !aligned16(W2) || !aligned16(out) ||
+            !aligned16(workspace))
+            return BM_ERR_ALIGN;
+        const Workspace w = workspace_layout(T, D, F, K, G, S);
+        if (workspace_bytes < w.total) return BM_ERR_WORKSPACE;
+        if (device_ok() != 1) return BM_ERR_CUDA;
+        routing->T = T; routing->E = E; routing->K = K; routing->G = G;
+        uint8_t *ws = static_cast<uint8_t *>(workspace);
+        bool handled = false;
+        const cudaError_t e = launch_layer_small(x, T, D, W_router, router_bias, E, K, group_map, G, W1, W3, W2, F, S, out, *routing,
+                                                 reinterpret_cast<bm_bf16 *>(ws + w.h), reinterpret_cast<float *>(ws + w.route_logits),
+                                                 reinterpret_cast<int32_t *>(ws + w.status), &handled,
+                                                 reinterpret_cast<cudaStream_t>(stream));
+        if (e != cudaSuccess) return BM_ERR_CUDA;
+        if (handled) return BM_OK;
+    }
+    int rc = bm_route(x, T, D, W_router, router_bias, E, K, group_map, G, routing, workspace, workspace_bytes, stream);
+    if (rc != BM_OK) return rc;
+    return bm_moe_forward(x, T, D, routing, W1, W3, W2, F, S, out, workspace, workspace_bytes, stream);
+}
+
 // Copy streams and events of bm_moe_layer_host's chunk pipeline, created on first use, one set per device.
 constexpr int kHostMaxChunks = 8;
 struct HostPipe { bool ready = false; cudaStream_t in = nullptr, out = nullptr; cudaEvent_t ev_in[kHostMaxChunks], ev_cmp[kHostMaxChunks], ev_done; };
@@ -424,9 +456,8 @@ int bm_moe_layer_host(const bm_bf16 *x_host, int T, int D, const bm_bf16 *W_rout
     if (!pipe) n_chunks = 1;
     if (n_chunks == 1) {
         if (T > 0 && cudaMemcpyAsync(x_dev, x_host, (size_t)T * row_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return BM_ERR_CUDA;
-        int rc = bm_route(x_dev, T, D, W_router, router_bias, E, K, group_map, G, routing, workspace, workspace_bytes, stream);
-        if (rc != BM_OK) return rc;
-        rc = bm_moe_forward(x_dev, T, D, routing, W1, W3, W2, F, S, out_dev, workspace, workspace_bytes, stream);
+        int rc = bm_moe_layer(x_dev, T, D, W_router, router_bias, E, K, group_map, G, W1, W3, W2, F, S, out_dev, routing, workspace,
+                              workspace_bytes, stream);
         if (rc != BM_OK) return rc;
         if (T > 0 && cudaMemcpyAsync(out_host, out_dev, (size_t)T * row_bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess)
             return BM_ERR_CUDA;

@@ -121,7 +121,7 @@ enum Opt {
     OPT_PDL, OPT_DECODE_MAX_T, OPT_DECODE_MID_T, OPT_DECODE_ROWS, OPT_DECODE_MID_ROWS, OPT_GEMV_ROWS, OPT_GEMV_MAX_T,
     OPT_GEMV_FUSE, OPT_DC_RMAX, OPT_DC_KS_FORCE, OPT_DC_STAGES, OPT_PF_STAGES, OPT_DC_R1, OPT_DC_R2, OPT_DC_KS2,
     OPT_PF_PAIR, OPT_PF_GATHER, OPT_COMBINE_WARPS, OPT_PERM_SMALL_WARPS, OPT_ROUTER_WE, OPT_ROUTER_TP_MIN_T,
-    OPT_ROUTER_SPLIT_MAX_T, OPT_FUSED_COMBINE, OPT_PF_G1_BC, OPT_PF_G2_BC, OPT_PF_G2_BW, OPT_PF_G1_HINTS, OPT_PF_G2_HINTS, OPT_DC_DENSE_MAX_T, OPT_DC_PREFETCH_MB, OPT_DC_KPACK, OPT_ROUTER_FILTER, OPT_HOST_CHUNK_T, OPT_COUNT
+    OPT_ROUTER_SPLIT_MAX_T, OPT_FUSED_COMBINE, OPT_PF_G1_BC, OPT_PF_G2_BC, OPT_PF_G2_BW, OPT_PF_G1_HINTS, OPT_PF_G2_HINTS, OPT_DC_DENSE_MAX_T, OPT_DC_PREFETCH_MB, OPT_DC_KPACK, OPT_ROUTER_FILTER, OPT_HOST_CHUNK_T, OPT_LAYER_SMALL, OPT_COUNT
 };
 int opt(Opt o);
 
@@ -195,6 +195,10 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
 cudaError_t launch_forward_gemv(const ForwardArgs &a, cudaStream_t stream);
 int decode_ksplit(int T, int D, int F, int K, int G, int S);     // K splits the decode GEMM2 would use
 cudaError_t launch_combine(const ForwardArgs &a, cudaStream_t stream);
+cudaError_t launch_layer_small(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const float *bias, int E, int K,
+                               const int32_t *gmap, int G, const bm_bf16 *W1, const bm_bf16 *W3, const bm_bf16 *W2, int F, int S,
+                               bm_bf16 *out, const bm_routing &r, bm_bf16 *h, float *logits, int32_t *status, bool *handled,
+                               cudaStream_t stream);
 
 // ---------------------------------------------------------------------------------------------
 // Device helpers

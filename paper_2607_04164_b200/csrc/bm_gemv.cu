@@ -22,7 +22,11 @@
 // 8 rows takes several passes over its weights (correct, slower; BM_PATH_AUTO does not send such shapes
 // here).  The W2 stage is normally the fused token-major kernel below (gemv2_combine_kernel); the set-major plain
 // kernel writing bf16 y rows + the prefill path's combine_kernel remain as the fallback for huge K + S or F.
+#include <algorithm>
+
 #include "bm_common.cuh"
+#include "bm_ptx.cuh"
+#include "bm_router.cuh"
 
 namespace bm {
 
@@ -51,7 +55,8 @@ __device__ __forceinline__ void fma2(float &d0, float &d1, float x, float w0, fl
 // The weight stream is software-pipelined: the loads of step s + 1 (a step = U chunks per lane of both rows;
 // the next step may belong to the next unit) are issued before the multiply of step s, from two register
 // buffers, so a warp always has a step of loads in flight -- without it every step paid a full HBM latency
-// (measured: 3 TB/s instead of 6 at T = 16, G = 60).
+// (measured: 3 TB/s instead of 6 at T = 16, G = 60).  Staging the stream through per-lane cp.async rings in shared memory (8 KB
+// per warp in flight instead of 4 KB) was measured too and was slower (single-token layer 26.6 -> 28 us).
 template <int R, bool SWIGLU, typename StageFn>
 __device__ __forceinline__ void warp_units(StageFn stage_rows, const bm_bf16 *__restrict__ base_a, const bm_bf16 *__restrict__ base_b,
                                            size_t stride_q, int n8, int q0, int qb, const uint8_t *s_in, int in_bytes,
@@ -149,18 +154,15 @@ struct GemvArgs {
     int NQ;                     // units per set (F or D/2)
 };
 
+// (body of gemv_kernel; also one phase of layer_small_kernel, where p.offsets / p.row_token point into shared memory)
 template <bool SWIGLU>
-__global__ void __launch_bounds__(kGvThreads, 1)
-gemv_kernel(GemvArgs p, int rows_cap) {
-    extern __shared__ __align__(16) uint8_t gv_smem[];
+__device__ __forceinline__ void gemv_body(const GemvArgs &p, int rows_cap, uint8_t *gv_smem) {
     __shared__ int s_nact;
     const int in_bytes = p.IN * 2, n8 = p.IN / 8;
     uint8_t *s_in = gv_smem;                                              // [rows_cap][IN] bf16
     int *s_set = reinterpret_cast<int *>(gv_smem + (size_t)rows_cap * in_bytes);   // active sets, ascending
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int nsets = p.G + p.S;
-    grid_dep_wait();      // routing arrays, x / h come from predecessors
-    grid_dep_launch();
 
     if (warp == 0) {
         int n = 0;
@@ -238,6 +240,15 @@ gemv_kernel(GemvArgs p, int rows_cap) {
 }
 
 template <bool SWIGLU>
+__global__ void __launch_bounds__(kGvThreads, 1)
+gemv_kernel(GemvArgs p, int rows_cap) {
+    extern __shared__ __align__(16) uint8_t gv_smem[];
+    grid_dep_wait();      // routing arrays, x / h come from predecessors
+    grid_dep_launch();
+    gemv_body<SWIGLU>(p, rows_cap, gv_smem);
+}
+
+template <bool SWIGLU>
 cudaError_t launch_gemv(const GemvArgs &p, int kid, cudaStream_t stream) {
     int rows_cap = kGvRows;
     while (rows_cap > 1 && (size_t)rows_cap * p.IN * 2 > 200 * 1024) rows_cap >>= 1;
@@ -269,9 +280,10 @@ struct Gemv2Args {
     int T, K, G, S, D, F;
 };
 
-__global__ void __launch_bounds__(kGvThreads, 1)
-gemv2_combine_kernel(Gemv2Args p, int max_src, int max_q) {
-    extern __shared__ __align__(16) uint8_t gv_smem[];
+// (body of gemv2_combine_kernel; also one phase of layer_small_kernel.  COHERENT_H: h was written earlier in the SAME
+//  kernel by other CTAs, so it must not be read through the non-coherent path)
+template <bool COHERENT_H, int U = 4>
+__device__ __forceinline__ void gemv2_combine_body(const Gemv2Args &p, int max_src, int max_q, uint8_t *gv_smem) {
     __shared__ int s_u[32], s_row[32];
     __shared__ float s_gw[32];
     const int in_bytes = p.F * 2, n8 = p.F / 8, NQ = p.D / 2;
@@ -279,13 +291,12 @@ gemv2_combine_kernel(Gemv2Args p, int max_src, int max_q) {
     float *s_y = reinterpret_cast<float *>(gv_smem + (size_t)max_src * in_bytes);   // [max_src][2 * max_q]
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const long long TK = (long long)p.T * p.K;
-    grid_dep_wait();      // h comes from the W1/W3 stage, the routing arrays from bm_route
-    grid_dep_launch();
     const long long total = (long long)p.T * NQ;
     const long long per = (total + gridDim.x - 1) / gridDim.x;      // <= max_q by the host's choice
     const long long lo = (long long)blockIdx.x * per;
     const long long hi = lo + per < total ? lo + per : total;
-    constexpr int U = 4;
+    // U = chunks of each row per lane and step.  With F <= 1536 (n8 <= 192) U = 6 makes a unit one step, so a warp -- which
+    // only has one or two units here -- has all of a unit's loads in flight at once
     const int iters = (n8 + 32 * U - 1) / (32 * U);
 
     for (long long pos = lo; pos < hi;) {
@@ -367,8 +378,9 @@ gemv2_combine_kernel(Gemv2Args p, int max_src, int max_q) {
         for (int idx = tid; idx < n_src * n8; idx += kGvThreads) {
             const int r = idx / n8, c = idx - r * n8;
             const int row = s_row[r];
+            const uint4 *hp = reinterpret_cast<const uint4 *>(p.h + (size_t)(row >= 0 ? row : 0) * p.F) + c;
             *reinterpret_cast<uint4 *>(s_in + (size_t)r * in_bytes + (size_t)c * 16) =
-                row >= 0 ? __ldg(reinterpret_cast<const uint4 *>(p.h + (size_t)row * p.F) + c) : make_uint4(0u, 0u, 0u, 0u);
+                row >= 0 ? (COHERENT_H ? __ldcg(hp) : __ldg(hp)) : make_uint4(0u, 0u, 0u, 0u);
         }
         __syncthreads();
         while (v < n_units) {
@@ -399,7 +411,200 @@ gemv2_combine_kernel(Gemv2Args p, int max_src, int max_q) {
     }
 }
 
+__global__ void __launch_bounds__(kGvThreads, 1)
+gemv2_combine_kernel(Gemv2Args p, int max_src, int max_q) {
+    extern __shared__ __align__(16) uint8_t gv_smem[];
+    grid_dep_wait();      // h comes from the W1/W3 stage, the routing arrays from bm_route
+    grid_dep_launch();
+    gemv2_combine_body<false>(p, max_src, max_q, gv_smem);
+}
+
+// -------------------------------------------------------------------------------------------------
+// The whole layer for one or two tokens in ONE persistent kernel (bm_moe_layer, T <= 2, T*K <= G): single-token decode is
+// a chain of four dependent steps -- router logits, selection, W1/W3 stream, W2 stream + combine -- each a few
+// microseconds long, and as three launches every arrow costs a kernel boundary.  Here the arrows are two grid-wide
+// barriers (cooperative launch: all CTAs are resident):
+//   A  canonical router dots (A1), one warp per (token, expert), spread over the grid        -> logits scratch
+//   -- barrier --
+//   B  every CTA selects for itself (R2-R5, R6-R8 on <= 32 items, in shared memory); CTA 0 also writes the routing arrays
+//   C  gemv_body<SWIGLU> with offsets / row_token in shared memory                            -> h
+//   -- barrier --
+//   D  gemv2_combine_body (h read with ld.global.cg: written in this kernel)                  -> out
+// Barrier counters live in the zero-once head of the workspace and are put back to zero by the last CTA to leave.
+// -------------------------------------------------------------------------------------------------
+struct SmallArgs {
+    const bm_bf16 *x, *Wr;
+    const float *bias;
+    const int32_t *gmap;
+    const bm_bf16 *W1, *W3, *W2;
+    bm_bf16 *h, *out;
+    bm_routing r;
+    float *logits;          // [T][E] scratch
+    int32_t *status;        // workspace head: [0] status bits, [1] A, [8], [9], [10] barrier counters
+    int T, D, E, K, G, S, F;
+    int rows_cap, max_src, max_q;
+};
+constexpr int kSmallBar = 8;        // status[8], status[9]: the two grid barriers; status[10]: CTAs that have left
+
+__device__ __forceinline__ void grid_barrier(int32_t *ctr, int n_cta) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicAdd(ctr, 1);
+        uint32_t spins = 0;
+        uint64_t t0 = 0;
+        int v;
+        do {
+            asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory");
+            if (v < n_cta && (++spins & 0x3ffu) == 0) {
+                const uint64_t now = ptx::globaltimer_ns();
+                if (t0 == 0) t0 = now;
+                else if (now - t0 > ptx::kWaitTimeoutNs) __trap();
+            }
+        } while (v < n_cta);
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(kGvThreads, 1)
+layer_small_kernel(SmallArgs a) {
+    extern __shared__ __align__(16) uint8_t gv_smem[];
+    __shared__ int32_t s_eid[2 * BM_MAX_K], s_gid[2 * BM_MAX_K], s_rtok[2 * BM_MAX_K], s_rslot[2 * BM_MAX_K], s_srow[2 * BM_MAX_K];
+    __shared__ int32_t s_ns[2], s_off[BM_MAX_G + 1], s_A;
+    __shared__ float s_gw[2 * BM_MAX_K];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int n_cta = (int)gridDim.x;
+    const int T = a.T, E = a.E, K = a.K, G = a.G, D = a.D;
+
+    // ---- A: router logits in the canonical order (A1), bit for bit as router_kernel ------------------------------
+    for (int i = (int)blockIdx.x + warp * n_cta; i < T * E; i += n_cta * kGvWarps) {
+        const int t = i / E, e = i - t * E;
+        const bm_bf16 *xrow = a.x + (size_t)t * D, *wrow = a.Wr + (size_t)e * D;
+        float p = 0.0f;
+#pragma unroll 8
+        for (int k = lane * 8; k < D; k += 256) {
+            const uint4 xv = __ldg(reinterpret_cast<const uint4 *>(xrow + k));
+            const uint4 wv = __ldg(reinterpret_cast<const uint4 *>(wrow + k));
+            p = __fmaf_rn(bf16_lo(xv.x), bf16_lo(wv.x), p);
+            p = __fmaf_rn(bf16_hi(xv.x), bf16_hi(wv.x), p);
+            p = __fmaf_rn(bf16_lo(xv.y), bf16_lo(wv.y), p);
+            p = __fmaf_rn(bf16_hi(xv.y), bf16_hi(wv.y), p);
+            p = __fmaf_rn(bf16_lo(xv.z), bf16_lo(wv.z), p);
+            p = __fmaf_rn(bf16_hi(xv.z), bf16_hi(wv.z), p);
+            p = __fmaf_rn(bf16_lo(xv.w), bf16_lo(wv.w), p);
+            p = __fmaf_rn(bf16_hi(xv.w), bf16_hi(wv.w), p);
+        }
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) p = __fadd_rn(p, __shfl_xor_sync(kFullMask, p, o));
+        if (lane == 0) {
+            if (a.bias) p = __fadd_rn(p, a.bias[e]);
+            __stcg(a.logits + i, p);
+        }
+    }
+    grid_barrier(a.status + kSmallBar, n_cta);
+
+    // ---- B: selection and the (tiny) permutation, by every CTA for itself ----------------------------------------
+    float *s_l = reinterpret_cast<float *>(gv_smem);
+    for (int i = tid; i < T * E; i += kGvThreads) s_l[i] = __ldcg(a.logits + i);
+    __syncthreads();
+    if (warp < T) select_and_write(s_l + warp * E, warp, lane, E, K, GroupMap{a.gmap, nullptr, G}, s_eid, s_gid, s_gw, s_ns, a.status);
+    __syncthreads();
+    const int items = T * K;                      // <= 32
+    for (int u = tid; u <= G; u += kGvThreads) {
+        int less = 0;
+        for (int j = 0; j < items; ++j) { const int kj = s_gid[j]; less += (kj >= 0 && kj < u) ? 1 : 0; }
+        s_off[u] = less;
+        if (u == G) s_A = less;
+    }
+    if (tid < items) {
+        const int k = s_gid[tid];
+        int row = 0;
+        for (int j = 0; j < items; ++j) { const int kj = s_gid[j]; row += (kj >= 0 && (kj < k || (kj == k && j < tid))) ? 1 : 0; }
+        s_srow[tid] = k >= 0 ? row : -1;
+    }
+    __syncthreads();
+    if (tid < items) { s_rtok[tid] = -1; s_rslot[tid] = -1; }
+    __syncthreads();
+    if (tid < items && s_srow[tid] >= 0) { s_rtok[s_srow[tid]] = tid / K; s_rslot[s_srow[tid]] = tid % K; }
+    __syncthreads();
+    if (blockIdx.x == 0) {                         // the routing arrays of the API (fully written, pads included)
+        if (tid < items) {
+            a.r.expert_ids[tid] = s_eid[tid]; a.r.group_ids[tid] = s_gid[tid]; a.r.gate_w[tid] = s_gw[tid];
+            a.r.row_token[tid] = s_rtok[tid]; a.r.row_slot[tid] = s_rslot[tid]; a.r.slot_row[tid] = s_srow[tid];
+        }
+        if (tid < T) a.r.n_slots[tid] = s_ns[tid];
+        for (int u = tid; u <= G; u += kGvThreads) {
+            a.r.offsets[u] = s_off[u];
+            if (u < G) a.r.counts[u] = s_off[u + 1] - s_off[u];
+        }
+        if (tid == 0) a.status[1] = s_A;
+    }
+
+    // ---- C: W1 / W3 stream ------------------------------------------------------------------------------------------
+    {
+        GemvArgs p{};
+        p.in = a.x; p.Wa = a.W1; p.Wb = a.W3; p.outp = a.h; p.offsets = s_off; p.row_token = s_rtok;
+        p.T = T; p.TK = items; p.G = G; p.S = a.S; p.IN = D; p.OUT = a.F; p.NQ = a.F;
+        gemv_body<true>(p, a.rows_cap, gv_smem);
+    }
+    grid_barrier(a.status + kSmallBar + 1, n_cta);
+
+    // ---- D: W2 stream + gate-weighted combine ------------------------------------------------------------------
+    {
+        Gemv2Args q{};
+        q.h = a.h; q.W2 = a.W2; q.out = a.out; q.out_f32 = nullptr;
+        q.group_ids = s_gid; q.slot_row = s_srow; q.n_slots = s_ns; q.gate_w = s_gw;
+        q.T = T; q.K = K; q.G = G; q.S = a.S; q.D = D; q.F = a.F;
+        if (q.F <= 1536) gemv2_combine_body<true, 6>(q, a.max_src, a.max_q, gv_smem);
+        else gemv2_combine_body<true>(q, a.max_src, a.max_q, gv_smem);
+    }
+    // barrier counters back to zero: the first is free once everybody is past the second; the second (and the exit
+    // counter) once everybody has left it
+    if (tid == 0) {
+        if (blockIdx.x == 0) a.status[kSmallBar] = 0;
+        if (atomicAdd(a.status + kSmallBar + 2, 1) == n_cta - 1) { a.status[kSmallBar + 1] = 0; a.status[kSmallBar + 2] = 0; }
+    }
+}
+
 }  // namespace
+
+// One cooperative launch for the whole layer on T <= 2 tokens; *handled = false when the shape does not fit (the caller
+// then takes the separate kernels).
+cudaError_t launch_layer_small(const bm_bf16 *x, int T, int D, const bm_bf16 *Wr, const float *bias, int E, int K,
+                               const int32_t *gmap, int G, const bm_bf16 *W1, const bm_bf16 *W3, const bm_bf16 *W2, int F, int S,
+                               bm_bf16 *out, const bm_routing &r, bm_bf16 *h, float *logits, int32_t *status, bool *handled,
+                               cudaStream_t stream) {
+    *handled = false;
+    const int sms = num_sms();
+    int rows_cap = 2;                            // a set meets at most T <= 2 rows here
+    while (rows_cap > 1 && (size_t)rows_cap * D * 2 > 200 * 1024) rows_cap >>= 1;
+    const size_t smem1 = (size_t)rows_cap * D * 2 + (size_t)(G + S) * sizeof(int);
+    const int max_src = K + S;
+    const long long total = (long long)T * (D / 2);
+    const int max_q = (int)((total + sms - 1) / sms);
+    const size_t smem2 = (size_t)max_src * F * 2 + (size_t)max_src * max_q * 2 * sizeof(float);
+    const size_t smem = std::max(std::max(smem1, smem2), (size_t)T * E * sizeof(float));
+    if (T < 1 || T > 2 || max_src > 32 || smem > 200 * 1024 || T * E > sms * kGvWarps) return cudaSuccess;
+    if (cudaError_t ea = ensure_dyn_smem(reinterpret_cast<const void *>(layer_small_kernel), smem); ea != cudaSuccess) return ea;
+    SmallArgs a{};
+    a.x = x; a.Wr = Wr; a.bias = bias; a.gmap = gmap; a.W1 = W1; a.W3 = W3; a.W2 = W2; a.h = h; a.out = out; a.r = r;
+    a.logits = logits; a.status = status;
+    a.T = T; a.D = D; a.E = E; a.K = K; a.G = G; a.S = S; a.F = F;
+    a.rows_cap = rows_cap; a.max_src = max_src; a.max_q = max_q;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(sms); cfg.blockDim = dim3(kGvThreads); cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;
+    attr[0].val.cooperative = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    count_launch();
+    profile_begin(BM_KERNEL_GEMM1, stream);
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, layer_small_kernel, a);
+    profile_end(BM_KERNEL_GEMM1, stream);
+    if (e == cudaSuccess) *handled = true;
+    return e;
+}
 
 cudaError_t launch_forward_gemv(const ForwardArgs &a, cudaStream_t stream) {
     GemvArgs p{};

@@ -480,3 +480,43 @@ def test_one_workspace_serves_changing_batch_sizes():
     # and the regions really are clean: everything behind the front sections reads zero
     tail = ws[-(T_max * D * 4):]
     assert int(tail.count_nonzero()) == 0
+
+
+@pytest.mark.parametrize("T,D,F,E,K,G,S", [
+    (1, 2048, 1408, 60, 4, 60, 0),        # BJ:configs[4] single-token decode: the one-kernel layer
+    (1, 2048, 1408, 60, 4, 8, 0),
+    (2, 2048, 1408, 60, 4, 30, 0),
+    (1, 264, 1000, 16, 4, 16, 2),         # shared experts, ragged sizes
+    (2, 512, 320, 200, 8, 97, 1),         # many experts: several router dots per CTA
+    (2, 4096, 14336, 8, 2, 1, 0),         # T*K > G: falls back to the separate kernels
+    (5, 256, 320, 12, 3, 4, 1),           # T > 2: the separate kernels
+])
+def test_moe_layer_single_call(T, D, F, E, K, G, S):
+    """bm_moe_layer = bm_route + bm_moe_forward in one call; for T <= 2 with T*K <= G it is ONE persistent kernel (router dots,
+    selection, W1/W3 stream, W2 stream + combine between two grid barriers).  Routing arrays bit-exact (pads included), out
+    inside the tolerance, repeated calls on one workspace (the barrier counters are put back), same bits as the kernels it replaces."""
+    import paper_2607_04164_b200 as bm
+    rng = np.random.default_rng(T * 101 + G)
+    L = rand_layer(rng, T=T, D=D, F=F, E=E, K=K, G=G, S=S, bias=True, wstd=0.02 if D >= 1024 else 0.05)
+    d = to_device(L)
+    o = oracle_route(L)
+    want = oracle_forward(L, o)
+    ws = bm.alloc_workspace(T, D, F, E, K, G, S)
+    r = bm.Routing(T, K, G)
+    outs = []
+    for small in (1, 1, 0, 1):
+        out = torch.full((T, D), float("nan"), dtype=torch.bfloat16, device="cuda")
+        for arr in (r.expert_ids, r.group_ids, r.row_token, r.row_slot, r.slot_row, r.n_slots, r.counts, r.offsets):
+            arr.fill_(-7)
+        with bm.options(LAYER_SMALL=small):
+            bm.bm_moe_layer(d.x, d.W_router, d.router_bias, K, d.group_map, G, d.W1, d.W3, d.W2, out, r, ws, S=S)
+        torch.cuda.synchronize()
+        assert bm.bm_device_status(ws) == 0
+        assert_routing_equal(routing_to_numpy(r, T), o)
+        assert_out_close(out.float().cpu().numpy().astype(np.float64), want)
+        outs.append(out.clone())
+    head = ws[:4096].view(torch.int32)
+    assert int(head[0]) == 0 and int(head[2:].count_nonzero()) == 0     # status word and every counter back to zero ([1] = A)
+    assert (outs[0] == outs[1]).all() and (outs[0] == outs[3]).all()
+    if bm.bm_forward_info(T, K, G, S, D, F)[1]:
+        assert (outs[0] == outs[2]).all()                        # the same arithmetic as the matrix-vector kernels
