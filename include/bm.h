@@ -3,7 +3,7 @@
  *         SURVEY.md 8(f) rows built on it: partial brownout, united-weight construction, the calibration forward and
  *         the per-rank partial of a tensor-parallel layer.
  *
- * The operation (PAPER.md = /root/reference/PAPER.md, "P:NN" = line NN; readings A1..A20 = DESIGN.md):
+ * The operation (PAPER.md = /root/reference/PAPER.md, "P:NN" = line NN; readings A1..A22 = DESIGN.md):
  *   P:42   MoE layer with E experts and top-K routing:  h_t = sum_{i<=K} g_i(x_t) * FFN_i(x_t),
  *          g_i the gating score.
  *   P:46   united experts / full brownout: every routed expert e is served by the united expert of its
@@ -21,7 +21,7 @@
  *     has completed.  All device pointers must be 16-byte aligned.
  *   - Workspace.  Call bm_workspace_init once after allocating a workspace (it zeroes it).  Two parts of it must be
  *     all-zero whenever a call starts, and every call that completes leaves them all-zero again: the first 4096
- *     bytes (device status word, arrival counters of the small-batch router) and a region anchored at the END of
+ *     bytes (device status word, arrival counters of the small-batch router, grid barriers of the single-token kernel) and a region anchored at the END of
  *     the buffer (fp32 accumulator and tickets of the fused combine; kernels clear what they used).  Hence: pass the
  *     buffer's true size as `workspace_bytes` on every call, use one workspace for one layer shape (D, F, E, K, G, S;
  *     any T <= T_max), and call bm_workspace_init again after a failed launch, after a device status fault
