@@ -71,15 +71,15 @@ enum { BM_DEV_BAD_GROUP_MAP = 1, BM_DEV_NONFINITE_LOGIT = 2, BM_DEV_BAD_ROUTING 
 /* execution path of bm_moe_forward_path */
 enum {
     BM_PATH_AUTO = 0,    /* GEMV if T <= 2 and T*K <= G (a weight set expects at most ~1 row: single-token decode); else DECODE if
-                            T <= 64, or T <= 192 and T*K <= 128*G (one chunk per group), or T <= BM_DECODE_MAX_T and
-                            T*K <= 24*G (few rows per group); else PREFILL */
+                            T <= 64, or T <= 192 (256 where a weight set D*F has >= 64 MB) and T*K <= 128*G (one chunk per
+                            group), or T <= BM_DECODE_MAX_T and T*K <= 44*G (few rows per group); else PREFILL */
     BM_PATH_DECODE = 1,  /* weight-streaming, weights on the MMA M side (small M; HBM-bound)   */
     BM_PATH_PREFILL = 2, /* 128-token x 256-column tcgen05 tiles (large M; tensor-pipe-bound)  */
     BM_PATH_SIMT = 3,    /* plain CUDA-core kernels; a debugging cross-check, never picked by AUTO */
     BM_PATH_GEMV = 4     /* weight-streaming matrix-vector products on the CUDA cores (FFMA2), <= 8 rows of a set per
                             pass over its weights; W2 stage fused with the slot-order combine (deterministic)    */
 };
-enum { BM_DECODE_MAX_T = 384 };
+enum { BM_DECODE_MAX_T = 320 };   /* default of option DECODE_MAX_T: AUTO never picks DECODE beyond it */
 
 /*
  * Routing of one batch: the result of steps R1-R7.  A host struct of device
@@ -211,7 +211,10 @@ int bm_moe_forward(const bm_bf16 *x, int T, int D, const bm_routing *routing, co
  * written exactly as by the two calls.  Having the whole step in one call lets the library run single-token decode
  * (T <= 2 with T*K <= G, the matrix-vector rule of BM_PATH_AUTO) as ONE persistent kernel -- router dots, selection,
  * W1/W3 stream, W2 stream + combine separated by two grid-wide barriers (cooperative launch) instead of three
- * dependent launches; every other shape takes the two calls.  Option LAYER_SMALL = 0 switches the single kernel off.
+ * dependent launches; every other shape takes the two calls' kernels.  Option LAYER_SMALL = 0 switches the single kernel off.
+ * Small decode batches (T <= 64 with G <= T*K) also gain from the single call: their first weight sets are multiplied
+ * while the routing kernels still run (every active set multiplies all T tokens there, so the work needs no routing;
+ * options DC_SPEC_US / DC_SPEC_MIN_ROWS), which bm_moe_forward on its own cannot know to be worth while.
  * Arguments as in bm_route / bm_moe_forward (full brownout: no cold mask).
  */
 int bm_moe_layer(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, const float *router_bias, int E, int K,
@@ -294,13 +297,17 @@ int bm_moe_forward_path(const bm_bf16 *x, int T, int D, const bm_routing *routin
  *   out_host  HOST [T,D] bf16
  *   x_dev, out_dev   device staging buffers [T,D] bf16 owned by the caller
  * All other arguments as in bm_route / bm_moe_forward (weights, router and group map stay resident on
- * the device).  Batches of T >= 2 * HOST_CHUNK_T tokens (option, default 2048; 0 = never) are processed in up to 8
- * token chunks so that the copies of neighbouring chunks overlap the compute of the current one (two internal copy
- * streams and their events are created on first use, once per device -- the one place where the library owns CUDA
- * objects).  `out` is the same either way; the routing arrays then hold each chunk's result in the chunk's slice
- * ([t0*K, (t0+tc)*K) of the [T,K] arrays, row indices relative to the chunk) and counts / offsets those of the LAST
- * chunk: call bm_route yourself when you need the whole batch's permutation.
+ * the device).  Batches of T >= 2 * HOST_CHUNK_T tokens (option; 0 = never) are processed in up to 16 equal token
+ * chunks so that the copies of neighbouring chunks overlap the compute of the current one (two internal copy streams and
+ * their events are created on first use, once per device -- the one place where the library owns CUDA objects).  By
+ * default (HOST_CHUNK_T = -1) a chunk has about 4096 tokens where a token computes at least twice as long as it copies
+ * (F * (K + S) >= 17400, e.g. Mixtral shapes: smaller chunks lose more tile efficiency than their copies hide) and 2048
+ * elsewhere.  bm_host_chunks returns the number of chunks such a call takes and writes the first min(n, cap) chunk sizes
+ * to `sizes` (HOST; no GPU needed).  `out` is the same either way; the routing arrays then hold each chunk's result in
+ * the chunk's slice ([t0*K, (t0+tc)*K) of the [T,K] arrays, row indices relative to the chunk) and counts / offsets those
+ * of the LAST chunk: call bm_route yourself when you need the whole batch's permutation.
  */
+int bm_host_chunks(int T, int F, int K, int S, int *sizes, int cap);
 int bm_moe_layer_host(const bm_bf16 *x_host, int T, int D, const bm_bf16 *W_router,
                       const float *router_bias, int E, int K, const int32_t *group_map, int G,
                       const bm_bf16 *W1, const bm_bf16 *W3, const bm_bf16 *W2, int F, int S,
@@ -325,15 +332,19 @@ int bm_device_status(void *workspace, int32_t *host_out, bm_stream_t stream);
  *                           weight tiles per band in GEMM2; <= 0 = one band (chunk-fastest order, the default)
  *   PF_G1_HINTS, PF_G2_HINTS (-1)       L2 eviction hints of the prefill tiles' TMA loads: 10 * activations + weights with
  *                           0 = evict_first, 1 = normal, 2 = evict_last; -1 = default (21)
- *   DECODE_MAX_T (384), DECODE_MID_T (192), DECODE_ROWS (24), DECODE_MID_ROWS (128), GEMV_MAX_T (2), GEMV_ROWS (1)
+ *   DECODE_MAX_T (320), DECODE_MID_T (192), DECODE_ROWS (44), DECODE_MID_ROWS (128), GEMV_MAX_T (2), GEMV_ROWS (1)
  *                           thresholds of BM_PATH_AUTO
  *   DC_DENSE_MAX_T (64)     decode kernels: up to this many tokens (<= 64) every active set multiplies all T tokens (no gather)
  *   DC_PREFETCH_MB (48)     decode GEMM1: megabytes of W1 / W3 it asks L2 to fetch while it still waits for the routing; 0 = off
  *   GEMV_FUSE (1)           matrix-vector path: fuse the W2 stage with the combine
  *   DC_R1, DC_R2, DC_KS2, DC_RMAX, DC_KS_FORCE (0, 0, 1, 128, 0)   decode tiling overrides (rows per tile, K splits)
  *   DC_STAGES, PF_STAGES (12)   cap on the shared-memory ring depth
+ *   DC_SPEC_US (12), DC_SPEC_MIN_ROWS (1)   bm_moe_layer, dense decode with G <= T*K: GEMM1 multiplies the leading weight sets
+ *                           -- as many as stream from HBM in DC_SPEC_US microseconds -- before it waits for the routing
+ *                           kernels (0 = off), provided T*K >= DC_SPEC_MIN_ROWS * G
+ *   PERM_CLUSTER (1)        permutation of 2048 < T*K <= 65536 items: 1 = one launch (a cluster of eight CTAs), 0 = three kernels
  *   LAYER_SMALL (1)         bm_moe_layer: 1 = one persistent kernel for T <= 2 (single-token decode), 0 = the separate kernels
- *   HOST_CHUNK_T (2048)     bm_moe_layer_host: tokens per pipelined chunk; 0 = one piece
+ *   HOST_CHUNK_T (-1)       bm_moe_layer_host: tokens per pipelined chunk; 0 = one piece; -1 = by shape (4096 or 2048)
  *   ROUTER_FILTER (1)       T >= 512, E <= 256, K <= 8, E >= 4K + 8: tensor-core filter + canonical refinement of the
  *                           candidates; 0 = all E dots; 2 = the filter whenever the kernel supports the shape
  *   DC_KPACK (2)            decode kernels: k-blocks per ring stage

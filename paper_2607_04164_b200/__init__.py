@@ -9,7 +9,7 @@ from .binding import (  # noqa: F401
     BM_PATH_PREFILL, BM_PATH_SIMT, BM_PATH_GEMV, BM_DECODE_MAX_T, BmError, Routing, alloc_workspace, bm_device_status, bm_moe_forward,
     bm_moe_layer_host, bm_moe_layer, bm_route, bm_route_partial, bm_unite_weights, bm_expert_histogram, bm_expert_outputs,
     bm_cosine_gram, bm_group_mse, bm_moe_forward_f32, bm_round_bf16, launch_count, lib, profile_enable, profile_read, profile_read_kinds, status_string,
-    workspace_bytes, KERNELS, Salc, bm_salc_cold_mask, set_option, get_option, options, bm_forward_info, BM_MAX_S,
+    workspace_bytes, KERNELS, Salc, bm_salc_cold_mask, set_option, get_option, options, bm_forward_info, bm_host_chunks, BM_MAX_S,
 )
 from .tp import shard_f, tp_moe_forward  # noqa: F401,E402
 from . import tp  # noqa: F401,E402

@@ -17,9 +17,9 @@ BM_OK = 0
 BM_PATH_AUTO, BM_PATH_DECODE, BM_PATH_PREFILL, BM_PATH_SIMT, BM_PATH_GEMV = 0, 1, 2, 3, 4
 BM_DEV_BAD_GROUP_MAP, BM_DEV_NONFINITE_LOGIT, BM_DEV_BAD_ROUTING = 1, 2, 4
 BM_MAX_E, BM_MAX_K, BM_MAX_G, BM_MAX_S = 512, 16, 512, 16
-BM_DECODE_MAX_T = 384
+BM_DECODE_MAX_T = 320
 
-EXPORTS = ["bm_moe_layer", "bm_expert_outputs_workspace_bytes", "bm_workspace_bytes", "bm_workspace_init", "bm_forward_info", "bm_set_option", "bm_get_option", "bm_route", "bm_route_partial", "bm_unite_weights", "bm_expert_histogram",
+EXPORTS = ["bm_moe_layer", "bm_expert_outputs_workspace_bytes", "bm_workspace_bytes", "bm_workspace_init", "bm_forward_info", "bm_host_chunks", "bm_set_option", "bm_get_option", "bm_route", "bm_route_partial", "bm_unite_weights", "bm_expert_histogram",
            "bm_expert_outputs", "bm_gram_workspace_bytes", "bm_cosine_gram", "bm_mse_workspace_bytes", "bm_group_mse",
            "bm_moe_forward", "bm_moe_forward_path", "bm_moe_forward_f32", "bm_round_bf16", "bm_moe_layer_host",
            "bm_device_status", "bm_launch_count", "bm_status_string", "bm_profile_enable", "bm_profile_read", "bm_profile_read_kinds",
@@ -65,6 +65,8 @@ def lib() -> ctypes.CDLL:
         L.bm_workspace_init.argtypes = [c_void_p, c_size_t, c_void_p]
         L.bm_forward_info.restype = c_int
         L.bm_forward_info.argtypes = [c_int] * 6 + [POINTER(c_int), POINTER(c_int)]
+        L.bm_host_chunks.restype = c_int
+        L.bm_host_chunks.argtypes = [c_int] * 4 + [POINTER(c_int), c_int]
         L.bm_set_option.restype = c_int
         L.bm_set_option.argtypes = [ctypes.c_char_p, c_int]
         L.bm_get_option.restype = c_int
@@ -211,6 +213,15 @@ def bm_forward_info(T: int, K: int, G: int, S: int, D: int, F: int):
     if rc != BM_OK:
         raise BmError(rc, "bm_forward_info")
     return int(pth.value), bool(det.value)
+
+
+def bm_host_chunks(T: int, F: int, K: int, S: int):
+    """Token chunk sizes bm_moe_layer_host processes a batch of T tokens in (include/bm.h: bm_host_chunks)."""
+    sizes = (c_int * 16)()
+    n = lib().bm_host_chunks(T, F, K, S, sizes, 16)
+    if n < 0:
+        raise BmError(n, "bm_host_chunks")
+    return [int(sizes[i]) for i in range(n)]
 
 
 class Routing:

@@ -32,11 +32,11 @@ void profile_end(int kernel, cudaStream_t stream) {
 // ---- options (bm_set_option / bm_get_option) ---------------------------------------------------------------
 struct OptDef { const char *name; int dflt; };
 static const OptDef kOptDefs[OPT_COUNT] = {
-    {"PDL", 1}, {"DECODE_MAX_T", BM_DECODE_MAX_T}, {"DECODE_MID_T", 192}, {"DECODE_ROWS", 24}, {"DECODE_MID_ROWS", 128},
+    {"PDL", 1}, {"DECODE_MAX_T", BM_DECODE_MAX_T}, {"DECODE_MID_T", 192}, {"DECODE_ROWS", 44}, {"DECODE_MID_ROWS", 128},
     {"GEMV_ROWS", 1}, {"GEMV_MAX_T", 2}, {"GEMV_FUSE", 1}, {"DC_RMAX", 128}, {"DC_KS_FORCE", 0}, {"DC_STAGES", 12},
     {"PF_STAGES", 12}, {"DC_R1", 0}, {"DC_R2", 0}, {"DC_KS2", 1}, {"PF_PAIR", -1}, {"PF_GATHER", 1},
     {"COMBINE_WARPS", 64}, {"PERM_SMALL_WARPS", 0}, {"ROUTER_WE", 0}, {"ROUTER_TP_MIN_T", kSplitRouterMaxT},
-    {"ROUTER_SPLIT_MAX_T", 16}, {"FUSED_COMBINE", -1}, {"PF_G1_BC", -1}, {"PF_G2_BC", -1}, {"PF_G2_BW", -1}, {"PF_G1_HINTS", -1}, {"PF_G2_HINTS", -1}, {"DC_DENSE_MAX_T", kDenseMaxT}, {"DC_PREFETCH_MB", 48}, {"DC_KPACK", 2}, {"ROUTER_FILTER", 1}, {"HOST_CHUNK_T", 2048}, {"LAYER_SMALL", 1},
+    {"ROUTER_SPLIT_MAX_T", 16}, {"FUSED_COMBINE", -1}, {"PF_G1_BC", -1}, {"PF_G2_BC", -1}, {"PF_G2_BW", -1}, {"PF_G1_HINTS", -1}, {"PF_G2_HINTS", -1}, {"DC_DENSE_MAX_T", kDenseMaxT}, {"DC_PREFETCH_MB", 48}, {"DC_KPACK", 2}, {"ROUTER_FILTER", 1}, {"HOST_CHUNK_T", -1}, {"LAYER_SMALL", 1}, {"PERM_CLUSTER", 1}, {"DC_SPEC_US", 12}, {"DC_SPEC_MIN_ROWS", 1},
 };
 static int g_opt[OPT_COUNT];
 static bool init_options() {
@@ -280,17 +280,21 @@ int bm_group_mse(const bm_bf16 *Y, const bm_bf16 *U, int T, int D, const int32_t
 }
 
 // BM_PATH_AUTO -> the path a batch of these host-side sizes takes
-static int resolve_auto_path(int T, int K, int G) {
+static int resolve_auto_path(int T, int K, int G, int D, int F) {
 
-    // decode (swap-AB weight streaming) for small batches: always up to 64 tokens; up to BM_DECODE_MID_T = 192
-    // tokens while a group expects at most one 128-row chunk (the weights then stream once); up to
-    // BM_DECODE_MAX_T = 384 tokens while a group expects at most ~24 rows.  Measured decode / prefill path (us):
-    //   D = 2048, F = 1408, E = 60, top-4:  G = 8: T = 128 60 / 70, T = 192 65 / 67, T = 256 70 / 63;
-    //                                       G = 15: T = 128 72 / 80, T = 192 82 / 81, T = 256 95 / 86;
-    //                                       G = 30: T = 192 118 / 122, T = 256 127 / 123;  G = 60: T = 256 185 / 195, T = 320 194 / 206, T = 512 204 / 202
-    //   D = 4096, F = 14336, E = 8, top-2:  G = 4: T = 128 244 / 284, T = 192 283 / 316, T = 256 297 / 299
+    // decode (swap-AB weight streaming) for small batches: always up to 64 tokens; up to DECODE_MID_T = 192 tokens (256
+    // where a weight set has >= 64 MB: long items) while a group expects at most one 128-row chunk (the weights then
+    // stream once); up to DECODE_MAX_T = 320 tokens while a group expects at most ~44 rows.  Measured, forward only,
+    // decode / prefill kernels (us; cold weights):
+    //   D = 2048, F = 1408, E = 60, top-4:
+    //     G = 8:   T = 128 48 / 56,   T = 192 51 / 52,    T = 256 55 / 50,    T = 320 59 / 49
+    //     G = 15:  T = 128 58 / 71,   T = 192 64 / 69,    T = 256 75 / 70,    T = 320 77 / 68
+    //     G = 30:  T = 192 97 / 113,  T = 256 111 / 115,  T = 320 112 / 113,  T = 384 115 / 110
+    //     G = 60:  T = 192 170 / 193, T = 256 194 / 191,  T = 320 195 / 197,  T = 384 202 / 192
+    //   D = 4096, F = 14336, E = 8, top-2, G = 4:  T = 128 240 / 301, T = 192 300 / 375, T = 256 334 / 359, T = 320 423 / 397
     const int max_t = opt(OPT_DECODE_MAX_T);
-    const int mid_t = opt(OPT_DECODE_MID_T);
+    int mid_t = opt(OPT_DECODE_MID_T);
+    if (mid_t == 192 && (long long)D * F * 2 >= (64LL << 20)) mid_t = 256;
     const bool few_rows = (long long)T * K <= (long long)opt(OPT_DECODE_ROWS) * G;
     const bool one_chunk = (long long)T * K <= (long long)opt(OPT_DECODE_MID_ROWS) * G;
     int path = (T <= 64 || (T <= mid_t && one_chunk) || (T <= max_t && few_rows)) ? BM_PATH_DECODE : BM_PATH_PREFILL;
@@ -307,7 +311,7 @@ static int resolve_auto_path(int T, int K, int G) {
 
 static int forward_common(const bm_bf16 *x, int T, int D, const bm_routing *routing, const bm_bf16 *W1,
                           const bm_bf16 *W3, const bm_bf16 *W2, int F, int S, bm_bf16 *out, float *out_f32,
-                          void *workspace, size_t workspace_bytes, bm_stream_t stream, int path) {
+                          void *workspace, size_t workspace_bytes, bm_stream_t stream, int path, bool after_router = false) {
     if (!routing) return BM_ERR_NULL;
     const int K = routing->K, G = routing->G;
     int rc = check_shapes(T, D, F, routing->E, K, G, S, true);
@@ -327,13 +331,14 @@ static int forward_common(const bm_bf16 *x, int T, int D, const bm_routing *rout
     if (workspace_bytes < w.total) return BM_ERR_WORKSPACE;
     if (device_ok() != 1) return BM_ERR_CUDA;
 
-    if (path == BM_PATH_AUTO) path = resolve_auto_path(T, K, G);
+    if (path == BM_PATH_AUTO) path = resolve_auto_path(T, K, G, D, F);
 
     uint8_t *ws = static_cast<uint8_t *>(workspace);
     ForwardArgs a{};
     a.x = x; a.T = T; a.D = D; a.F = F; a.K = K; a.G = G; a.S = S;
     a.r = *routing;
     a.W1 = W1; a.W3 = W3; a.W2 = W2; a.out = out; a.out_f32 = out_f32;
+    a.after_router = after_router;
     a.status = reinterpret_cast<int32_t *>(ws + w.status);
     a.xs = reinterpret_cast<bm_bf16 *>(ws + w.xs);
     a.h = reinterpret_cast<bm_bf16 *>(ws + w.h);
@@ -384,7 +389,7 @@ int bm_moe_layer(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, const 
                  const int32_t *group_map, int G, const bm_bf16 *W1, const bm_bf16 *W3, const bm_bf16 *W2, int F, int S,
                  bm_bf16 *out, bm_routing *routing, void *workspace, size_t workspace_bytes, bm_stream_t stream) {
     // one or two tokens whose sets expect at most one row (the matrix-vector rule of BM_PATH_AUTO): one persistent kernel
-    if (routing && T >= 1 && T <= 2 && opt(OPT_LAYER_SMALL) != 0 && resolve_auto_path(T, K, G) == BM_PATH_GEMV) {
+    if (routing && T >= 1 && T <= 2 && opt(OPT_LAYER_SMALL) != 0 && resolve_auto_path(T, K, G, D, F) == BM_PATH_GEMV) {
         int rc = check_shapes(T, D, F, E, K, G, S, true);
         if (rc != BM_OK) return rc;
         if (!x || !W_router || !group_map || !W1 || !W3 || !W2 || !out || !workspace || !routing->expert_ids ||
@@ -409,11 +414,13 @@ int bm_moe_layer(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, const 
     }
     int rc = bm_route(x, T, D, W_router, router_bias, E, K, group_map, G, routing, workspace, workspace_bytes, stream);
     if (rc != BM_OK) return rc;
-    return bm_moe_forward(x, T, D, routing, W1, W3, W2, F, S, out, workspace, workspace_bytes, stream);
+    if (!out && T > 0) return BM_ERR_NULL;
+    // the forward kernels know that the routing kernels run directly before them (speculative dense decode, bm_gemm.cu)
+    return forward_common(x, T, D, routing, W1, W3, W2, F, S, out, nullptr, workspace, workspace_bytes, stream, BM_PATH_AUTO, true);
 }
 
 // Copy streams and events of bm_moe_layer_host's chunk pipeline, created on first use, one set per device.
-constexpr int kHostMaxChunks = 8;
+constexpr int kHostMaxChunks = 16;
 struct HostPipe { bool ready = false; cudaStream_t in = nullptr, out = nullptr; cudaEvent_t ev_in[kHostMaxChunks], ev_cmp[kHostMaxChunks], ev_done; };
 static HostPipe g_pipe[kMaxDevices];
 
@@ -436,6 +443,36 @@ static HostPipe *host_pipe() {
     return &p;
 }
 
+// Token chunks of bm_moe_layer_host: equal chunks of whole 128-row tiles, about HOST_CHUNK_T tokens each, from two chunks on.
+// The pipeline hides every copy except the first chunk's way in and the last chunk's way out, but a chunk must stay large
+// enough to keep the tiles efficient -- BJ:configs[2]'s layer takes 0.53 us per token at T = 8192, 0.55 at 4096, 0.63 at 2048
+// and 1.03 at 512 (its 1.4 GB of weights stream once per chunk).  Measured there, end to end: one piece 6.12 ms, 2 x 4096
+// 5.21, 4 x 2048 5.36, 8 x 1024 6.34; chunks growing from a small first one towards the middle and shrinking again (512,
+// 1536, 4096, 1536, 512: the exposed copies shrink 4x) 5.54 -- the small chunks cost more than their copies save.  So: 4096
+// tokens where a token computes at least twice as long as it copies (6 D F (K + S) flops at ~1.3 PFLOP/s against 2 D bytes at
+// ~50 GB/s: F (K + S) >= 17400), 2048 elsewhere (Qwen-like shapes: copies as long as compute).  Returns the number of chunks.
+static int host_chunk_plan(int T, int F, int K, int S, int *sizes) {
+    int chunk_t = opt(OPT_HOST_CHUNK_T);
+    if (chunk_t < 0) chunk_t = (long long)F * (K + S) >= 17400 ? 4096 : 2048;
+    sizes[0] = T;
+    if (chunk_t == 0 || T < 2 * chunk_t) return 1;
+    int pieces = (T + chunk_t - 1) / chunk_t;
+    if (pieces > kHostMaxChunks) pieces = kHostMaxChunks;
+    const int per = ((T + pieces - 1) / pieces + 127) & ~127;
+    int n = 0;
+    for (int t0 = 0; t0 < T; t0 += per) sizes[n++] = T - t0 < per ? T - t0 : per;
+    return n;
+}
+
+int bm_host_chunks(int T, int F, int K, int S, int *sizes, int cap) {
+    if (T < 0 || F < 1 || K < 1 || S < 0 || cap < 0) return BM_ERR_SHAPE;
+    if (cap > 0 && !sizes) return BM_ERR_NULL;
+    int plan[kHostMaxChunks];
+    const int n = host_chunk_plan(T, F, K, S, plan);
+    for (int i = 0; i < n && i < cap; ++i) sizes[i] = plan[i];
+    return n;
+}
+
 int bm_moe_layer_host(const bm_bf16 *x_host, int T, int D, const bm_bf16 *W_router, const float *router_bias, int E,
                       int K, const int32_t *group_map, int G, const bm_bf16 *W1, const bm_bf16 *W3,
                       const bm_bf16 *W2, int F, int S, bm_bf16 *out_host, bm_bf16 *x_dev, bm_bf16 *out_dev,
@@ -449,9 +486,8 @@ int bm_moe_layer_host(const bm_bf16 *x_host, int T, int D, const bm_bf16 *W_rout
     // Large batches go through in token chunks (tokens are independent: the layer on a chunk is the layer on its tokens):
     // the host->device copy of chunk c+1 and the device->host copy of chunk c-1 run on two copy streams while chunk c
     // computes, so a PCIe-bound step (BJ:configs[2]: 67 MB each way) costs its compute time plus one chunk of copies.
-    const int chunk_t = opt(OPT_HOST_CHUNK_T);
-    int n_chunks = (chunk_t > 0 && T >= 2 * chunk_t) ? (T + chunk_t - 1) / chunk_t : 1;
-    if (n_chunks > kHostMaxChunks) n_chunks = kHostMaxChunks;
+    int sizes[kHostMaxChunks];
+    int n_chunks = host_chunk_plan(T, F, K, S, sizes);
     HostPipe *pipe = n_chunks > 1 ? host_pipe() : nullptr;
     if (!pipe) n_chunks = 1;
     if (n_chunks == 1) {
@@ -463,15 +499,13 @@ int bm_moe_layer_host(const bm_bf16 *x_host, int T, int D, const bm_bf16 *W_rout
             return BM_ERR_CUDA;
         return cudaStreamSynchronize(st) == cudaSuccess ? BM_OK : BM_ERR_CUDA;
     }
-    const int per = ((T + n_chunks - 1) / n_chunks + 127) & ~127;       // tokens per chunk, whole 128-row tiles
     // the copy streams start after whatever the caller queued on `stream` before this call
     if (cudaEventRecord(pipe->ev_done, st) != cudaSuccess || cudaStreamWaitEvent(pipe->in, pipe->ev_done, 0) != cudaSuccess ||
         cudaStreamWaitEvent(pipe->out, pipe->ev_done, 0) != cudaSuccess)
         return BM_ERR_CUDA;
     const bm_routing whole = *routing;
-    int c = 0;
-    for (int t0 = 0; t0 < T; t0 += per, ++c) {
-        const int tc = T - t0 < per ? T - t0 : per;
+    for (int c = 0, t0 = 0; c < n_chunks; t0 += sizes[c], ++c) {
+        const int tc = sizes[c];
         if (cudaMemcpyAsync(x_dev + (size_t)t0 * D, x_host + (size_t)t0 * D, (size_t)tc * row_bytes, cudaMemcpyHostToDevice, pipe->in) != cudaSuccess ||
             cudaEventRecord(pipe->ev_in[c], pipe->in) != cudaSuccess || cudaStreamWaitEvent(st, pipe->ev_in[c], 0) != cudaSuccess)
             return BM_ERR_CUDA;
@@ -550,7 +584,7 @@ int bm_profile_read(float *total_ms, int *n_records) {
 
 int bm_forward_info(int T, int K, int G, int S, int D, int F, int *path, int *deterministic) {
     if (T < 0 || K < 1 || K > BM_MAX_K || G < 1 || G > BM_MAX_G || S < 0 || S > BM_MAX_S || D < 8 || F < 8) return BM_ERR_SHAPE;
-    const int pth = resolve_auto_path(T, K, G);
+    const int pth = resolve_auto_path(T, K, G, D, F);
     int det = 1;
     if (pth == BM_PATH_PREFILL) {
         const int fc = opt(OPT_FUSED_COMBINE);

@@ -94,6 +94,8 @@ struct GemmParams {
     int32_t *tickets;   // zero region: arrivals per (token, output piece)
     bm_bf16 *y;         // two-pass combine: per-row expert outputs
     int y_tm;           // calibration: y is token-major [T, S, D] (row of shared set j, token t = t * S + j)
+    int dense_u;        // dense decode with G <= T*K: H rows are indexed by the weight set itself (row u * T + t)
+    int spec_sets;      // DC_GEMM1, dense_u: routed sets 0 .. spec_sets-1 are multiplied BEFORE the routing is known
     bm_bf16 *out;       // fused combine: the layer output [T, D] bf16 ...
     float *out_f32;     // ... or, when non-null, the fp32 sums (tensor-parallel partial)
 };
@@ -164,7 +166,7 @@ __device__ __forceinline__ bool get_item(const GemmParams &p, const SchedView &s
     if (p.dense) {
         it.tok0 = chunk * kChunkRows;
         it.perm_row0 = 0;
-        it.h_row0 = s * p.T + it.tok0;
+        it.h_row0 = (p.dense_u ? u : s) * p.T + it.tok0;
         it.act_row0 = (MODE == PF_GEMM1 || MODE == DC_GEMM1) ? it.tok0 : it.h_row0;
     } else if (it.shared) {
         it.tok0 = chunk * kChunkRows;
@@ -199,6 +201,7 @@ __device__ __forceinline__ void build_schedule(const GemmParams &p, int32_t *s_s
                 off = p.offsets[u];
                 if (rows < 0 || off < 0 || off + rows > p.TK) { bad = true; rows = 0; }
                 if (p.dense && rows > 0) rows = p.T;
+                if (u < p.spec_sets) rows = 0;          // done ahead of the routing (DC_GEMM1 only)
             } else {
                 rows = p.T;
             }
@@ -292,6 +295,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
         // GA: a stage is full when the TMA bytes (weights) have landed AND the relay warp (both CTAs' under K2) has signalled that the gathered rows are in place
         for (int i = 0; i < n_stages; ++i) { ptx::mbar_init(&full[i], GA ? 1 + (K2 ? 2 : 1) : 1); ptx::mbar_init(&empty[i], 1); }
         if (GA) for (int i = 0; i < n_stages; ++i) ptx::mbar_init(&gfull[i], kGatherCopyThreads);
+        if (MODE == DC_GEMM1) ptx::mbar_init(&gfull[0], 1);      // "schedule built" (speculative start, below)
         // K2: the leader's tempty collects the 4 epilogue warps of BOTH CTAs
         for (int i = 0; i < kAccStages; ++i) { ptx::mbar_init(&tfull[i], 1); ptx::mbar_init(&tempty[i], K2 ? 8 : 4); }
         ptx::fence_barrier_init();
@@ -355,11 +359,48 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
             ptx::prefetch_l2_bulk(addr, 16384u);
         }
     }
-    grid_dep_wait();
-    if (kGemm1 && warp == 0) build_schedule(p, s_sched, cap, s_hdr);
-    __syncthreads();
-    sv.n_seg = s_hdr[0]; sv.total_chunks = s_hdr[1]; sv.total_pairs = s_hdr[2];
-    if (threadIdx.x == 0) grid_dep_launch();
+    // Speculative start (DC_GEMM1, dense decode inside bm_moe_layer): with T*K >= 2 G tokens x slots nearly every set is
+    // active, and a dense item needs nothing from the routing -- all T tokens times one weight tile.  So the CTAs run the
+    // items of the first spec_sets sets (n_spec items, the same static round-robin) while the router and the permutation
+    // are still at work, and only then wait for them and build the schedule of the remaining active sets.  The router's
+    // latency (~10 us of an idle HBM) disappears behind the weight stream; a set that turns out inactive cost only
+    // bandwidth that nobody else wanted.  Item numbers below n_spec are synthesised by fetch(); the first request beyond
+    // makes the producer warp wait for the routing, build the schedule and release the other warps through an mbarrier.
+    // The dependent grid (GEMM2) is let go only then, so "GEMM1 let GEMM2 start => the routing is complete" still holds.
+    const bool spec = MODE == DC_GEMM1 && p.spec_sets > 0;
+    const int n_spec = spec ? p.spec_sets * p.n_wtiles : 0;
+    uint64_t *sched_bar = gfull;
+    if (!spec) {
+        grid_dep_wait();
+        if (kGemm1 && warp == 0) build_schedule(p, s_sched, cap, s_hdr);
+        __syncthreads();
+        sv.n_seg = s_hdr[0]; sv.total_chunks = s_hdr[1]; sv.total_pairs = s_hdr[2];
+        if (threadIdx.x == 0) grid_dep_launch();
+    }
+    bool sched_seen = !spec;
+    auto fetch = [&](int item, Item &it) -> bool {         // warp-uniform
+        if (MODE == DC_GEMM1 && spec) {
+            if (item < n_spec) {
+                it.u = item / p.n_wtiles; it.wt = item - it.u * p.n_wtiles; it.ks = 0;
+                it.n = p.T; it.act_row0 = 0; it.tok0 = 0; it.perm_row0 = 0; it.h_row0 = it.u * p.T; it.shared = false;
+                return true;
+            }
+            if (!sched_seen) {
+                if (warp == 0) {
+                    grid_dep_wait();
+                    build_schedule(p, s_sched, cap, s_hdr);
+                    if (lane == 0) { grid_dep_launch(); ptx::mbar_arrive(sched_bar); }
+                    __syncwarp();
+                } else {
+                    ptx::mbar_wait(sched_bar, 0);
+                }
+                sv.n_seg = s_hdr[0]; sv.total_chunks = s_hdr[1]; sv.total_pairs = s_hdr[2];
+                sched_seen = true;
+            }
+            item -= n_spec;
+        }
+        return get_item<MODE, K2>(p, sv, item, it, rank);
+    };
 
     // The producer and the MMA issuer run their loops with the WHOLE warp (warp-uniform control flow keeps
     // addresses and descriptors in uniform registers) and elect one lane for the issuing instructions: the
@@ -386,11 +427,11 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
             stage = pre;
             if (stage == n_stages) { stage = 0; phase = 1; }
         } else {
-            have = get_item<MODE, K2>(p, sv, item, it, rank);
+            have = fetch(item, it);
         }
         auto policy = [](int h) { return h == 0 ? ptx::kEvictFirst : (h == 1 ? ptx::kEvictNormal : ptx::kEvictLast); };
         const uint64_t pol_a = policy(p.hints / 10), pol_w = policy(p.hints % 10);
-        for (; have; item += item_stride, have = get_item<MODE, K2>(p, sv, item, it, rank), kb_first = 0) {
+        for (; have; item += item_stride, have = fetch(item, it), kb_first = 0) {
             const CUtensorMap *tm_act = (kGemm1 && (it.shared || p.dense)) ? &tm_act1 : &tm_act0;
             const int wrow0 = it.wt * p.R;
             int kc = (it.ks * nkb + kb_first) * kp * kBlockK;
@@ -450,7 +491,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
         uint32_t acc_phase = 0;
         Item it;
         // K2: only the leader issues MMAs (for both CTAs); the peer's warp 1 just keeps the TMEM allocation
-        for (int item = item0; (!K2 || leader) && get_item<MODE, K2>(p, sv, item, it, rank); item += item_stride) {
+        for (int item = item0; (!K2 || leader) && fetch(item, it); item += item_stride) {
             const uint32_t idesc = kDecode ? ptx::make_idesc_bf16(128, (it.n + 31) & ~31)
                                            : ptx::make_idesc_bf16(K2 ? 256 : 128, 256);
             ptx::mbar_wait(&tempty[acc], acc_phase ^ 1);
@@ -513,7 +554,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
         int stage = 0;
         uint32_t phase = 0;
         Item it;
-        for (int item = item0; get_item<MODE, K2>(p, sv, item, it, rank); item += item_stride) {
+        for (int item = item0; fetch(item, it); item += item_stride) {
             const bm_bf16 *src[8];
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
@@ -546,7 +587,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
         const int rw = warp - 10;
         int n = 0;                       // running k-block number of this CTA
         Item it;
-        for (int item = item0; get_item<MODE, K2>(p, sv, item, it, rank); item += item_stride) {
+        for (int item = item0; fetch(item, it); item += item_stride) {
             for (int kb = 0; kb < nkb; ++kb, ++n) {
                 const int stage = n % n_stages;
                 if (stage % kGatherRelays != rw) continue;
@@ -566,7 +607,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
         int acc = 0;
         uint32_t acc_phase = 0;
         Item it;
-        for (int item = item0; get_item<MODE, K2>(p, sv, item, it, rank); item += item_stride) {
+        for (int item = item0; fetch(item, it); item += item_stride) {
             // FC: token, gate weight and source count of this thread's rows are fetched BEFORE the wait for the
             // accumulator (two dependent global loads hidden behind the item's main loop).
             // PF_GEMM2: row `row` of the chunk (index 0); DC_GEMM2: chunk rows lane, lane + 32, ... (the columns).
@@ -1309,6 +1350,9 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
     GemmParams p{};
     p.hints = 20;            // activations evict_last, weights evict_first (decode: the weights stream once)
     p.dense = dense ? 1 : 0;
+    // G <= T*K: the dense H rows fit when indexed by the weight set itself (h_rows_needed), which lets GEMM1 write them
+    // before it knows which sets are active
+    p.dense_u = dense && (long long)a.G <= (long long)TK ? 1 : 0;
     p.status = a.status;
     p.seg_cap = a.G + a.S + 1;
     p.T = a.T; p.D = a.D; p.F = a.F; p.K = a.K; p.G = a.G; p.S = a.S; p.TK = TK;
@@ -1377,9 +1421,27 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
             unsigned long long per = ((unsigned long long)std::max(opt(OPT_DC_PREFETCH_MB), 0) << 20) / (2ull * (a.G + a.S));
             if (per > set_bytes) per = set_bytes;
             p.w1 = a.W1; p.w3 = a.W3; p.pf_set_bytes = set_bytes; p.pf_bytes = per & ~16383ull;
+            // Speculative start (gemm_kernel): inside bm_moe_layer, as many leading sets as the HBM streams in DC_SPEC_US
+            // microseconds -- about the time the routing kernels take -- at least one.  A speculated set that turns out
+            // inactive costs bandwidth that was idle anyway, as long as the speculated part does not outlast the routing:
+            // D = 2048, F = 1408, E = 60, top-4, T = 16 (us, off / 12 us / 24 us): G = 15 55.3 / 49.3 / 48.9, G = 30 85.8 /
+            // 76.9 / 76.9 and with zipf-2 routing (13 of 30 sets active) 56.6 / 49.9 / 53.0; G = 60, 15 of 60 active: 64.9 /
+            // 60.4.  DC_SPEC_MIN_ROWS (1) asks for that many expected rows per set, T*K >= rows * G, before speculating.
+            // BJ:configs[1] (117 MB per weight matrix) gains nothing: its L2 prefetch already hides the routing kernels.
+            const int spec_us = opt(OPT_DC_SPEC_US);
+            if (p.dense_u && a.after_router && spec_us > 0 && a.G > 0 &&
+                (long long)TK >= (long long)std::max(opt(OPT_DC_SPEC_MIN_ROWS), 1) * a.G) {
+                const unsigned long long budget = (unsigned long long)spec_us * 6400000ull;      // bytes at 6.4 TB/s
+                unsigned long long n = (budget + 2 * set_bytes - 1) / (2 * set_bytes);
+                p.spec_sets = (int)std::min<unsigned long long>(std::max<unsigned long long>(n, 1), (unsigned long long)a.G);
+                // what would be left fills less than one wave of CTAs: take it along instead of waiting for the routing with
+                // most SMs idle (G = 8, T = 16: 39.3 -> 34.5 us)
+                if ((long long)(a.G - p.spec_sets) * p.n_wtiles < sms) p.spec_sets = a.G;
+            }
         }
         if ((err = launch_gemm<DC_GEMM1>(m_xs, m_x, m_w1, m_w3, p, stream)) != cudaSuccess) return err;
         p.ksplit = ks2; p.kblocks = kb2 / ks2; p.R = R2; p.n_wtiles = (a.D + R2 - 1) / R2;
+        p.spec_sets = 0;
         ring_geometry(true, false, a.T, &p);
         err = fused ? launch_gemm<DC_GEMM2, false, false, true>(m_h, m_h, m_w2, m_w2, p, stream)
                     : launch_gemm<DC_GEMM2>(m_h, m_h, m_w2, m_w2, p, stream);

@@ -19,6 +19,7 @@
 //   T*K <= 2048 : one CTA does P1-P3 in a single launch (the decode case).
 #include "bm_common.cuh"
 #include "bm_permute.cuh"
+#include "bm_ptx.cuh"
 
 namespace bm {
 
@@ -130,6 +131,115 @@ permute_scatter_kernel(const int32_t *__restrict__ group_ids, int T, int K, int 
                  slot_row);
 }
 
+// ---- 2048 < T*K <= 65536: one cluster of eight CTAs, one launch -----------------------------------------------
+// The three-kernel path spends most of its 20-26 us (T = 4096 .. 16384, top-4) on two kernel boundaries and on a scan
+// kernel whose single CTA walks the block histograms serially.  Here the eight CTAs of a thread-block cluster split the
+// items 256 ways (32 warps each); a warp keeps its <= 8 rounds of keys in REGISTERS (all loads in flight at once, no
+// second read for the replay), the CTAs publish their per-group counts in shared memory, and after one cluster barrier
+// every CTA reads the other seven through distributed shared memory: counts, offsets and its own bases follow without a
+// trip through global memory.  A second cluster barrier keeps every CTA's counts alive until all peers have read them.
+constexpr int kClSize = 8, kClWarps = 32, kClMaxRounds = 8;
+constexpr long long kPermClusterItems = (long long)kClSize * kClWarps * kClMaxRounds * 32;      // 65536
+
+__device__ __forceinline__ int ld_shared_cluster(uint32_t addr) {
+    int v;
+    asm volatile("ld.shared::cluster.s32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    return v;
+}
+
+__global__ void __launch_bounds__(kClWarps * 32, 1)
+permute_cluster_kernel(const int32_t *__restrict__ group_ids, int T, int K, int G, int per_warp,
+                       int32_t *__restrict__ counts, int32_t *__restrict__ offsets,
+                       int32_t *__restrict__ row_token, int32_t *__restrict__ row_slot,
+                       int32_t *__restrict__ slot_row, int32_t *__restrict__ status) {
+    extern __shared__ int s_mem[];
+    __shared__ int s_total;
+    int *whist = s_mem;                      // [kClWarps][G]: counts, then bases of this CTA's warps
+    int *ctot = whist + kClWarps * G;        // [G] this CTA's counts, read by its peers
+    int *gsum = ctot + G;                    // [G] group totals -> offsets
+    grid_dep_wait();
+    grid_dep_launch();
+    const int rank = (int)ptx::cluster_ctarank();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long items = (long long)T * K;
+    const long long first = ((long long)rank * kClWarps + warp) * per_warp;
+    int keys[kClMaxRounds];
+#pragma unroll
+    for (int r = 0; r < kClMaxRounds; ++r) {
+        const long long i = first + r * 32 + lane;
+        keys[r] = (r * 32 < per_warp && i < items) ? __ldcg(group_ids + i) : -1;
+    }
+    for (int i = threadIdx.x; i < kClWarps * G; i += blockDim.x) whist[i] = 0;
+    __syncthreads();
+    int *whist_w = whist + warp * G;
+#pragma unroll
+    for (int r = 0; r < kClMaxRounds; ++r) {
+        if (r * 32 < per_warp) {                                       // warp-uniform
+            const unsigned peers = __match_any_sync(kFullMask, keys[r]);
+            if (keys[r] >= 0 && lane == __ffs(peers) - 1) whist_w[keys[r]] += __popc(peers);
+            __syncwarp();
+        }
+    }
+    __syncthreads();
+    const int u = threadIdx.x;               // G <= 512 < blockDim.x: one thread per group
+    if (u < G) {
+        int run = 0;
+        for (int w = 0; w < kClWarps; ++w) {                           // whist[w][u] := rows of group u in this CTA's warps before w
+            const int c = whist[w * G + u];
+            whist[w * G + u] = run;
+            run += c;
+        }
+        ctot[u] = run;
+    }
+    ptx::cluster_sync_all();
+    int before = 0;
+    if (u < G) {
+        int tot = 0;
+#pragma unroll
+        for (int c = 0; c < kClSize; ++c) {
+            const int v = ld_shared_cluster(ptx::mapa_u32(&ctot[u], (uint32_t)c));
+            if (c < rank) before += v;
+            tot += v;
+        }
+        gsum[u] = tot;
+        if (rank == 0) counts[u] = tot;
+    }
+    block_exclusive_scan(gsum, G, nullptr, &s_total);
+    if (u < G) {
+        const int base = gsum[u] + before;
+        for (int w = 0; w < kClWarps; ++w) whist[w * G + u] += base;
+        if (rank == 0) offsets[u] = gsum[u];
+    }
+    if (rank == 0 && threadIdx.x == 0) { offsets[G] = s_total; status[1] = s_total; }
+    ptx::cluster_sync_all();                 // peers have read ctot; this CTA's bases are complete
+    const int A = s_total;
+#pragma unroll
+    for (int r = 0; r < kClMaxRounds; ++r) {
+        if (r * 32 < per_warp) {
+            const long long i = first + r * 32 + lane;
+            const int key = keys[r];
+            const unsigned peers = __match_any_sync(kFullMask, key);
+            if (i < items) {
+                if (key >= 0) {
+                    const int row = whist_w[key] + __popc(peers & ((1u << lane) - 1u));
+                    row_token[row] = (int32_t)(i / K);
+                    row_slot[row] = (int32_t)(i % K);
+                    slot_row[i] = row;
+                } else {
+                    slot_row[i] = -1;
+                }
+                if (i >= A) {                   // rows past A stay -1 (A <= items)
+                    row_token[i] = -1;
+                    row_slot[i] = -1;
+                }
+            }
+            __syncwarp();
+            if (key >= 0 && lane == __ffs(peers) - 1) whist_w[key] += __popc(peers);
+            __syncwarp();
+        }
+    }
+}
+
 }  // namespace
 
 cudaError_t launch_permute(int T, int K, int G, const bm_routing &r, int32_t *block_hist, int32_t *status,
@@ -148,6 +258,24 @@ cudaError_t launch_permute(int T, int K, int G, const bm_routing &r, int32_t *bl
         if (cudaError_t ea = ensure_dyn_smem(reinterpret_cast<const void *>(permute_small_kernel), smem); ea != cudaSuccess) return ea;
         return launch_kernel(permute_small_kernel, dim3(1), dim3(nw * 32), smem, stream, (const int32_t *)r.group_ids,
                              T, K, G, per_warp, r.counts, r.offsets, r.row_token, r.row_slot, r.slot_row, status);
+    }
+    if (items <= kPermClusterItems && G <= 512 && opt(OPT_PERM_CLUSTER) != 0) {
+        int per_warp = (int)((items + kClSize * kClWarps - 1) / (kClSize * kClWarps));
+        per_warp = (per_warp + 31) / 32 * 32;
+        const size_t smem = (size_t)(kClWarps + 2) * G * sizeof(int);
+        if (cudaError_t ea = ensure_dyn_smem(reinterpret_cast<const void *>(permute_cluster_kernel), smem); ea != cudaSuccess) return ea;
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(kClSize); cfg.blockDim = dim3(kClWarps * 32); cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+        cudaLaunchAttribute attr[2];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = kClSize; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[1].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = pdl_enabled() ? 2 : 1;
+        count_launch();
+        return cudaLaunchKernelEx(&cfg, permute_cluster_kernel, (const int32_t *)r.group_ids, T, K, G, per_warp, r.counts, r.offsets,
+                                  r.row_token, r.row_slot, r.slot_row, status);
     }
     cudaError_t e = launch_kernel(permute_hist_kernel, dim3(nb), dim3(kWarps * 32), smem_w, stream,
                                   (const int32_t *)r.group_ids, T, K, G, block_hist);

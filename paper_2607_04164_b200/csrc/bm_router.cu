@@ -580,7 +580,10 @@ router_filter_kernel(const __grid_constant__ CUtensorMap tm_x,      // x [T, D],
     __syncthreads();
     ptx::tc_fence_after();
     const uint32_t tmem_base = *tmem_ptr;
-    grid_dep_wait();          // x may come from a predecessor; norms from row_norm_kernel
+    // Only the epilogue needs row_norm_kernel's result.  x and W_router are ready for the producer as soon as this grid runs:
+    // row_norm_kernel let it start only after its own grid-dependency wait had returned, i.e. after everything before this
+    // call had completed -- so the main loop runs beside the norm pass instead of behind it.
+    if (warp >= 2) grid_dep_wait();
     if (threadIdx.x == 0) grid_dep_launch();
 
     if (warp == 0) {

@@ -114,6 +114,30 @@ def test_forward_info_is_a_host_call():
         bm.bm_forward_info(4, 99, 4, 0, 64, 64)
 
 
+def test_host_chunk_plan_is_a_host_call():
+    """bm_host_chunks (include/bm.h, bm_moe_layer_host): chunks cover the batch exactly, at most 16, whole 128-row tiles
+    except the last; about 4096 tokens where compute outweighs the copies, 2048 elsewhere."""
+    import paper_2607_04164_b200 as bm
+    assert bm.bm_host_chunks(8192, 14336, 2, 0) == [4096, 4096]
+    assert bm.bm_host_chunks(8191, 14336, 2, 0) == [8191]                                      # below two chunks: one piece
+    assert bm.bm_host_chunks(16384, 14336, 2, 0) == [4096] * 4
+    assert bm.bm_host_chunks(64, 14336, 2, 0) == [64]
+    assert bm.bm_host_chunks(8192, 1408, 4, 0) == [2048] * 4                                   # copies ~ compute: smaller chunks
+    assert bm.bm_host_chunks(4095, 1408, 4, 4) == [4095]
+    for F, K, S in ((14336, 2, 0), (1408, 4, 4), (4096, 8, 1)):
+        for T in (0, 1, 2047, 4096, 4097, 5632, 8192, 8193, 12345, 16384, 65536, 300000):
+            c = bm.bm_host_chunks(T, F, K, S)
+            assert sum(c) == T and 1 <= len(c) <= 16
+            assert all(v > 0 for v in c) or T == 0
+            assert all(v % 128 == 0 for v in c[:-1]) and len(set(c[:-1])) <= 1 and c[-1] <= c[0]
+    with bm.options(HOST_CHUNK_T=0):
+        assert bm.bm_host_chunks(8192, 14336, 2, 0) == [8192]
+    with bm.options(HOST_CHUNK_T=512):
+        assert bm.bm_host_chunks(3000, 320, 3, 1) == [512] * 5 + [440]
+    with pytest.raises(bm.BmError):
+        bm.bm_host_chunks(-1, 64, 1, 0)
+
+
 def test_workspace_layout_invariants():
     """bm_workspace_bytes: monotone in T (a workspace for T_max serves every smaller batch), zero for arguments no call
     accepts, and large enough for the dense decode rows (one H row per active set and token up to 64 tokens)."""

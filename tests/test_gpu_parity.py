@@ -38,6 +38,9 @@ ROUTE_SHAPES = [
     (300, 64, 200, 16, 97, 0.0),       # many experts, K = BM_MAX_K
     (700, 72, 200, 16, 97, 1.0),       # the same through the staged throughput router: 4 expert passes, ragged slab
     (2500, 128, 512, 3, 512, 0.0),     # E = BM_MAX_E, G = BM_MAX_G
+    (683, 64, 8, 3, 3, 0.0),           # T*K = 2049: the smallest batch of the cluster permutation
+    (16384, 64, 16, 4, 16, 1.0),       # T*K = 65536: its largest (eight rounds of keys per warp)
+    (8193, 64, 9, 8, 5, 0.5),          # T*K = 65544: one item more -> the three-kernel permutation
 ]
 
 
@@ -52,6 +55,11 @@ def test_routing_bit_exact(T, D, E, K, G, s):
         # T >= 512: all E canonical dots (0), the tensor-core filter + refinement by the default rule (1) and forced (2)
         for filt in ((0, 1, 2) if T >= 512 else (1,)):
             with bm.options(ROUTER_FILTER=filt):
+                r, ws, _ = gpu_route(L)
+            assert bm.bm_device_status(ws) == 0
+            assert_routing_equal(routing_to_numpy(r, T), o)
+        if T * K > 2048:                                          # the permutation as three kernels instead of one cluster
+            with bm.options(PERM_CLUSTER=0):
                 r, ws, _ = gpu_route(L)
             assert bm.bm_device_status(ws) == 0
             assert_routing_equal(routing_to_numpy(r, T), o)
@@ -367,6 +375,7 @@ VARIANTS = [
     (0, {"ROUTER_TP_MIN_T": 1, "ROUTER_FILTER": 0}),           # throughput router (all E canonical dots) on any T
     (0, {"ROUTER_TP_MIN_T": 1, "ROUTER_FILTER": 2}),           # tensor-core filter + refinement on any T
     (0, {"ROUTER_SPLIT_MAX_T": 511}),                          # split router (+ fused permutation) on any T < 512
+    (0, {"PERM_CLUSTER": 0}),                                  # three-kernel permutation beyond 2048 items
 ]
 
 
@@ -390,6 +399,45 @@ def test_random_shapes_all_variants(seed):
         assert status == 0, (path, env)
         assert_routing_equal(g, o)
         assert_out_close(out, want)
+
+
+@pytest.mark.parametrize("T,D,F,E,K,G,S,dead", [
+    (16, 2048, 1408, 60, 4, 15, 0, ()),            # BJ:configs[4] small-batch decode: every set active
+    (16, 2048, 1408, 60, 4, 8, 0, (0, 2)),         # the FIRST set (speculated) turns out inactive
+    (64, 1024, 2048, 8, 2, 4, 0, (1,)),            # T = 64: router + permutation kernels ahead of GEMM1
+    (33, 264, 328, 12, 3, 6, 2, (0, 1, 2)),        # shared experts, ragged sizes, half of the sets inactive
+    (7, 512, 320, 16, 4, 14, 0, (13,)),            # T*K = 2 G exactly
+])
+@pytest.mark.parametrize("spec_us", [0, 12, 100000])
+def test_dense_decode_speculative_start(T, D, F, E, K, G, S, dead, spec_us):
+    """bm_moe_layer on dense decode batches (T <= 64, G <= T*K): GEMM1 multiplies its first sets before it waits for the
+    routing kernels (DC_SPEC_US microseconds of weight stream; 0 = off, 100000 = every set).  Sets listed in `dead` get
+    no token (their experts carry a large negative bias), so speculated work on them must leave no trace: routing
+    bit-exact, out inside the tolerance, status clean, the same through repeated calls on one workspace."""
+    import paper_2607_04164_b200 as bm
+    rng = np.random.default_rng(T * 7 + G)
+    L = rand_layer(rng, T=T, D=D, F=F, E=E, K=K, G=G, S=S, bias=True, wstd=0.02 if D >= 1024 else 0.05)
+    gm = L.group_map.numpy()
+    bias = L.router_bias.clone()
+    for e in range(E):
+        if int(gm[e]) in dead:
+            bias[e] = -1.0e4
+    L.router_bias = bias
+    d = to_device(L)
+    o = oracle_route(L)
+    assert all(int(o.counts[u]) == 0 for u in dead) and int((np.asarray(o.counts) > 0).sum()) >= 1
+    want = oracle_forward(L, o)
+    assert bm.bm_forward_info(T, K, G, S, D, F)[0] == bm.BM_PATH_DECODE
+    ws = bm.alloc_workspace(T, D, F, E, K, G, S)
+    r = bm.Routing(T, K, G)
+    with bm.options(DC_SPEC_US=spec_us):
+        for _ in range(3):
+            out = torch.full((T, D), float("nan"), dtype=torch.bfloat16, device="cuda")
+            bm.bm_moe_layer(d.x, d.W_router, d.router_bias, K, d.group_map, G, d.W1, d.W3, d.W2, out, r, ws, S=S)
+            torch.cuda.synchronize()
+            assert bm.bm_device_status(ws) == 0
+            assert_routing_equal(routing_to_numpy(r, T), o)
+            assert_out_close(out.float().cpu().numpy().astype(np.float64), want)
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -423,9 +471,11 @@ def test_layer_host_repeated_calls_with_new_data(own_stream):
     assert bm.bm_device_status(ws) == 0
 
 
-def test_layer_host_chunk_pipeline_matches_oracle():
-    """bm_moe_layer_host on a batch large enough for the chunk pipeline (copies of neighbouring chunks overlap compute):
-    `out` must be that of the whole batch; called twice to show that buffers, copy streams and the zero regions are reusable."""
+@pytest.mark.parametrize("plan", [dict(HOST_CHUNK_T=512), dict(HOST_CHUNK_T=1100)], ids=["512", "1100"])
+def test_layer_host_chunk_pipeline_matches_oracle(plan):
+    """bm_moe_layer_host on a batch large enough for the chunk pipeline (copies of neighbouring chunks overlap compute;
+    chunk sizes: bm_host_chunks): `out` must be that of the whole batch; called twice to show that buffers, copy streams
+    and the zero regions are reusable."""
     import paper_2607_04164_b200 as bm
     rng = np.random.default_rng(78)
     T, D, F, E, K, G, S = 3000, 256, 320, 12, 3, 4, 1
@@ -439,7 +489,9 @@ def test_layer_host_chunk_pipeline_matches_oracle():
     out_dev = torch.empty((T, D), dtype=torch.bfloat16, device="cuda")
     o = oracle_route(L)
     want = oracle_forward(L, o)
-    with bm.options(HOST_CHUNK_T=512):                             # 6 chunks of 512 tokens (the last one ragged)
+    with bm.options(**plan):                                       # equal: 6 chunks of 512 tokens (the last one ragged)
+        chunks = bm.bm_host_chunks(T, F, K, S)
+        assert sum(chunks) == T and len(chunks) >= 2
         for _ in range(2):
             out_pin.fill_(float("nan"))
             bm.bm_moe_layer_host(x_pin, d.W_router, d.router_bias, K, d.group_map, G, d.W1, d.W3, d.W2, S, out_pin,
