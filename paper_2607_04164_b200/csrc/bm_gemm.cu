@@ -1144,7 +1144,9 @@ double decode_time_model(int wrows, int kblocks, int n_seg, int R, int ks, int m
     };
     const long long full = items / sms, rem = items % sms;
     double t = (double)full * wave((double)sms) + (rem ? wave((double)rem) : 0.0);
-    return t * (1.0 + 0.01 * (ks - 1));       // split-K: extra fp32 reds in the epilogue
+    // split-K: every split adds its own fp32 reductions in the epilogue and a k-loop ramp per (shorter) item -- measured at
+    // D = 2048, F = 1408, T = 16, one split / two: G = 60 112.6 / 116.4 us, G = 30 74.4 / 79.1, G = 15 48.8 / 52.8
+    return t * (1.0 + 0.05 * (ks - 1));
 }
 
 void choose_decode_tiling(int wrows, int kblocks, int n_seg, bool allow_split, int mats, int sms, int *R_out,
