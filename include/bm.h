@@ -60,7 +60,8 @@ typedef enum bm_status {
     BM_ERR_ALIGN = -3,     /* a device pointer is not 16-byte aligned */
     BM_ERR_WORKSPACE = -4, /* workspace_bytes < bm_workspace_bytes(...) */
     BM_ERR_CUDA = -5,      /* no sm_100 device, driver entry point missing, or a launch failed */
-    BM_ERR_PATH = -6       /* forced path cannot run this shape (bm_moe_forward_path) */
+    BM_ERR_PATH = -6,      /* forced path cannot run this shape (bm_moe_forward_path) */
+    BM_ERR_LIMIT = -7      /* sizes beyond the fixed scratch of bm_route_static */
 } bm_status;
 
 enum { BM_MAX_E = 512, BM_MAX_K = 16, BM_MAX_G = 512, BM_MAX_S = 16 };
@@ -138,6 +139,29 @@ int bm_route(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, const floa
 int bm_route_partial(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, const float *router_bias, int E,
                      int K, const int32_t *group_map, int G, const int32_t *cold_mask, bm_routing *routing,
                      void *workspace, size_t workspace_bytes, bm_stream_t stream);
+
+/*
+ * bm_route_static -- bm_route without a workspace, for callers that may not allocate device memory (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid cudaMalloc).  The scratch bm_route keeps in the workspace
+ * (status word, arrival counters, permutation histograms, router logits / norms / candidate masks) lives in a
+ * file-scope device array of BM_STATIC_ROUTE_BYTES = 2 MiB inside the library; every GPU that loads the library holds
+ * those 2 MiB until the process exits.  The call allocates and frees nothing and calls no allocating library routine.
+ *   - Arguments and results exactly as bm_route (same kernels, same bits); the caller still passes x, the router, the
+ *     group map and the routing arrays.
+ *   - Limit: T <= BM_STATIC_ROUTE_MAX_T = 8192 (any E, K, G the library accepts then fits the array); beyond it the
+ *     call returns BM_ERR_LIMIT on the host, before anything is enqueued.
+ *   - The array is shared by every call on the device and keeps the last call's contents.  Each call clears the part
+ *     that must start at zero (its first 4096 bytes) on `stream` ahead of its kernels.  Calls that overlap on the GPU
+ *     -- different streams without an ordering between them, or two threads -- RACE on the array: order them.
+ *   - The first call on a device looks up the array's device address (cudaGetSymbolAddress): make one call, e.g. with
+ *     T = 0, outside any stream capture.
+ *   - bm_route_static_status copies the status word of the array (the BM_DEV_* bits the LAST bm_route_static call on
+ *     this device raised) to *host_out (HOST) and SYNCHRONISES `stream`.
+ */
+enum { BM_STATIC_ROUTE_BYTES = 2 * 1024 * 1024, BM_STATIC_ROUTE_MAX_T = 8192 };
+int bm_route_static(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, const float *router_bias, int E, int K,
+                    const int32_t *group_map, int G, bm_routing *routing, bm_stream_t stream);
+int bm_route_static_status(int32_t *host_out, bm_stream_t stream);
 
 /*
  * bm_unite_weights -- united-weight construction.  Cite: "The united expert is

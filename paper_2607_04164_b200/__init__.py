@@ -10,6 +10,7 @@ from .binding import (  # noqa: F401
     bm_moe_layer_host, bm_moe_layer, bm_route, bm_route_partial, bm_unite_weights, bm_expert_histogram, bm_expert_outputs,
     bm_cosine_gram, bm_group_mse, bm_moe_forward_f32, bm_round_bf16, launch_count, lib, profile_enable, profile_read, profile_read_kinds, status_string,
     workspace_bytes, KERNELS, Salc, bm_salc_cold_mask, set_option, get_option, options, bm_forward_info, bm_host_chunks, BM_MAX_S,
+    bm_route_static, bm_route_static_status, BM_ERR_LIMIT, BM_STATIC_ROUTE_BYTES, BM_STATIC_ROUTE_MAX_T,
 )
 from .tp import shard_f, tp_moe_forward  # noqa: F401,E402
 from . import tp  # noqa: F401,E402

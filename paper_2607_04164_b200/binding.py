@@ -18,8 +18,10 @@ BM_PATH_AUTO, BM_PATH_DECODE, BM_PATH_PREFILL, BM_PATH_SIMT, BM_PATH_GEMV = 0, 1
 BM_DEV_BAD_GROUP_MAP, BM_DEV_NONFINITE_LOGIT, BM_DEV_BAD_ROUTING = 1, 2, 4
 BM_MAX_E, BM_MAX_K, BM_MAX_G, BM_MAX_S = 512, 16, 512, 16
 BM_DECODE_MAX_T = 320
+BM_ERR_LIMIT = -7
+BM_STATIC_ROUTE_BYTES, BM_STATIC_ROUTE_MAX_T = 2 * 1024 * 1024, 8192
 
-EXPORTS = ["bm_moe_layer", "bm_expert_outputs_workspace_bytes", "bm_workspace_bytes", "bm_workspace_init", "bm_forward_info", "bm_host_chunks", "bm_set_option", "bm_get_option", "bm_route", "bm_route_partial", "bm_unite_weights", "bm_expert_histogram",
+EXPORTS = ["bm_moe_layer", "bm_expert_outputs_workspace_bytes", "bm_workspace_bytes", "bm_workspace_init", "bm_forward_info", "bm_host_chunks", "bm_set_option", "bm_get_option", "bm_route", "bm_route_static", "bm_route_static_status", "bm_route_partial", "bm_unite_weights", "bm_expert_histogram",
            "bm_expert_outputs", "bm_gram_workspace_bytes", "bm_cosine_gram", "bm_mse_workspace_bytes", "bm_group_mse",
            "bm_moe_forward", "bm_moe_forward_path", "bm_moe_forward_f32", "bm_round_bf16", "bm_moe_layer_host",
            "bm_device_status", "bm_launch_count", "bm_status_string", "bm_profile_enable", "bm_profile_read", "bm_profile_read_kinds",
@@ -74,6 +76,11 @@ def lib() -> ctypes.CDLL:
         L.bm_route.restype = c_int
         L.bm_route.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_int, c_int, c_void_p, c_int,
                                POINTER(BmRouting), c_void_p, c_size_t, c_void_p]
+        L.bm_route_static.restype = c_int
+        L.bm_route_static.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_int, c_int, c_void_p, c_int,
+                                      POINTER(BmRouting), c_void_p]
+        L.bm_route_static_status.restype = c_int
+        L.bm_route_static_status.argtypes = [POINTER(c_int32), c_void_p]
         L.bm_route_partial.restype = c_int
         L.bm_route_partial.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_int, c_int, c_void_p, c_int,
                                        c_void_p, POINTER(BmRouting), c_void_p, c_size_t, c_void_p]
@@ -302,6 +309,35 @@ def bm_route(x, W_router, router_bias, K: int, group_map, G: int, routing: Routi
     if rc != BM_OK:
         raise BmError(rc, "bm_route")
     return routing
+
+
+def bm_route_static(x, W_router, router_bias, K: int, group_map, G: int, routing: Routing, stream=None):
+    """bm_route without a workspace: its scratch is a fixed 2 MiB device array inside the library, nothing is allocated
+    (include/bm.h: bm_route_static).  T <= BM_STATIC_ROUTE_MAX_T, else BmError(BM_ERR_LIMIT); calls that overlap on the
+    GPU race on the shared array."""
+    T, D = x.shape
+    E = W_router.shape[0]
+    _dev("x", x, torch.bfloat16)
+    _dev("W_router", W_router, torch.bfloat16, (E, D))
+    _dev("router_bias", router_bias, torch.float32, (E,), optional=True)
+    _dev("group_map", group_map, torch.int32, (E,))
+    if T > routing.T_max or K != routing.K or G != routing.G:
+        raise ValueError(f"routing arrays were allocated for T <= {routing.T_max}, K = {routing.K}, {routing.G} sets; "
+                         f"got T = {T}, K = {K}, {G} sets")
+    rc = lib().bm_route_static(_ptr(x), T, D, _ptr(W_router), _ptr(router_bias), E, K, _ptr(group_map), G,
+                               ctypes.byref(routing.c), _stream(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_route_static")
+    return routing
+
+
+def bm_route_static_status(stream=None) -> int:
+    """Device status bits of the last bm_route_static call on this device; synchronises the stream."""
+    v = c_int32(0)
+    rc = lib().bm_route_static_status(ctypes.byref(v), _stream(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_route_static_status")
+    return int(v.value)
 
 
 def bm_route_partial(x, W_router, router_bias, K: int, group_map, G: int, cold_mask, routing: Routing, workspace,

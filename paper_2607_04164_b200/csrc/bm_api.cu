@@ -202,6 +202,63 @@ int bm_route_partial(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, co
                         workspace_bytes, stream);
 }
 
+// -------------------------------------------------------------------------------------------------
+// bm_route_static: bm_route for callers that may not allocate (CUDA graph capture, serving loops, harnesses without
+// cudaMalloc).  Its scratch -- the routing part of a workspace: status word and arrival counters, per-block histograms of
+// the permutation, logits / row norms / candidate masks of the router -- is the file-scope device array below, which every
+// GPU that loads the library holds until the process exits.  In host code the array's NAME is a host-side stand-in, not a
+// device address: its device address is looked up once per device with cudaGetSymbolAddress (that device current) and
+// that pointer is what the kernels get.
+// -------------------------------------------------------------------------------------------------
+constexpr size_t kStaticRouteBytes = (size_t)BM_STATIC_ROUTE_BYTES;
+static __device__ __align__(256) unsigned char g_static_route_scratch[kStaticRouteBytes];
+static void *g_static_route_ptr[kMaxDevices];       // device address of the array on device i, nullptr = not looked up yet
+
+static void *static_route_scratch() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return nullptr;
+    std::lock_guard<std::mutex> lock(g_dev_mutex);
+    if (!g_static_route_ptr[dev]) {
+        void *ptr = nullptr;
+        if (cudaGetSymbolAddress(&ptr, g_static_route_scratch) != cudaSuccess || !ptr) {
+            cudaGetLastError();
+            return nullptr;
+        }
+        g_static_route_ptr[dev] = ptr;
+    }
+    return g_static_route_ptr[dev];
+}
+
+int bm_route_static(const bm_bf16 *x, int T, int D, const bm_bf16 *W_router, const float *router_bias, int E, int K,
+                    const int32_t *group_map, int G, bm_routing *routing, bm_stream_t stream) {
+    if (!routing) return BM_ERR_NULL;
+    int rc = check_shapes(T, D, 8, E, K, G, 0, false);
+    if (rc != BM_OK) return rc;
+    // the limit, checked on the host before anything else: the routing scratch of this (T, K, G) must fit the array
+    if (T > BM_STATIC_ROUTE_MAX_T || workspace_layout(T, D, 8, K, G, 0).sched > kStaticRouteBytes) return BM_ERR_LIMIT;
+    if (device_ok() != 1) return BM_ERR_CUDA;
+    void *scratch = static_route_scratch();
+    if (!scratch) return BM_ERR_CUDA;
+    // The array keeps what the last call left.  What a call needs to find zero is the 4096-byte head (status word, arrival
+    // counters): cleared here, on `stream`, ahead of the kernels -- so the status word afterwards holds THIS call's bits.
+    if (T > 0 && cudaMemsetAsync(scratch, 0, kStatusInts * sizeof(int32_t), reinterpret_cast<cudaStream_t>(stream)) != cudaSuccess)
+        return BM_ERR_CUDA;
+    return route_common(x, T, D, W_router, router_bias, E, K, group_map, G, nullptr, false, routing, scratch,
+                        kStaticRouteBytes, stream);
+}
+
+int bm_route_static_status(int32_t *host_out, bm_stream_t stream) {
+    if (!host_out) return BM_ERR_NULL;
+    if (device_ok() != 1) return BM_ERR_CUDA;
+    void *scratch = static_route_scratch();
+    if (!scratch) return BM_ERR_CUDA;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    if (cudaMemcpyAsync(host_out, scratch, sizeof(int32_t), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess)
+        return BM_ERR_CUDA;
+    return BM_OK;
+}
+
 int bm_unite_weights(const bm_bf16 *W, int E, size_t n, const int32_t *group_map, int G, bm_bf16 *out,
                      bm_stream_t stream) {
     if (E < 1 || E > BM_MAX_E || G < 1 || G > BM_MAX_G || n % 8 != 0) return BM_ERR_SHAPE;
@@ -624,6 +681,7 @@ const char *bm_status_string(int code) {
         case BM_ERR_WORKSPACE: return "BM_ERR_WORKSPACE: workspace too small";
         case BM_ERR_CUDA: return "BM_ERR_CUDA: no sm_100 device or a CUDA call failed";
         case BM_ERR_PATH: return "BM_ERR_PATH: the forced path cannot run this shape";
+        case BM_ERR_LIMIT: return "BM_ERR_LIMIT: sizes beyond the fixed scratch of an entry point that allocates nothing";
         default: return "unknown bm_status";
     }
 }
