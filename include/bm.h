@@ -324,7 +324,7 @@ int bm_moe_forward_path(const bm_bf16 *x, int T, int D, const bm_routing *routin
  * the device).  Batches of T >= 2 * HOST_CHUNK_T tokens (option; 0 = never) are processed in up to 16 equal token
  * chunks so that the copies of neighbouring chunks overlap the compute of the current one (two internal copy streams and
  * their events are created on first use, once per device -- the one place where the library owns CUDA objects).  By
- * default (HOST_CHUNK_T = -1) a chunk has about 4096 tokens where a token computes at least twice as long as it copies
+ * default (HOST_CHUNK_T = -1) a chunk has about 2816 tokens where a token computes at least twice as long as it copies
  * (F * (K + S) >= 17400, e.g. Mixtral shapes: smaller chunks lose more tile efficiency than their copies hide) and 2048
  * elsewhere.  bm_host_chunks returns the number of chunks such a call takes and writes the first min(n, cap) chunk sizes
  * to `sizes` (HOST; no GPU needed).  `out` is the same either way; the routing arrays then hold each chunk's result in
@@ -366,9 +366,11 @@ int bm_device_status(void *workspace, int32_t *host_out, bm_stream_t stream);
  *   DC_SPEC_US (12), DC_SPEC_MIN_ROWS (1)   bm_moe_layer, dense decode with G <= T*K: GEMM1 multiplies the leading weight sets
  *                           -- as many as stream from HBM in DC_SPEC_US microseconds -- before it waits for the routing
  *                           kernels (0 = off), provided T*K >= DC_SPEC_MIN_ROWS * G
+ *   PF_SPEC (1)             bm_moe_layer, prefill tiles with S > 0: GEMM1 runs the shared experts' items before it waits for the
+ *                           routing kernels (0 = off)
  *   PERM_CLUSTER (1)        permutation of 2048 < T*K <= 65536 items: 1 = one launch (a cluster of eight CTAs), 0 = three kernels
  *   LAYER_SMALL (1)         bm_moe_layer: 1 = one persistent kernel for T <= 2 (single-token decode), 0 = the separate kernels
- *   HOST_CHUNK_T (-1)       bm_moe_layer_host: tokens per pipelined chunk; 0 = one piece; -1 = by shape (4096 or 2048)
+ *   HOST_CHUNK_T (-1)       bm_moe_layer_host: tokens per pipelined chunk; 0 = one piece; -1 = by shape (2816 or 2048)
  *   ROUTER_FILTER (1)       T >= 512, E <= 256, K <= 8, E >= 4K + 8: tensor-core filter + canonical refinement of the
  *                           candidates; 0 = all E dots; 2 = the filter whenever the kernel supports the shape
  *   DC_KPACK (2)            decode kernels: k-blocks per ring stage

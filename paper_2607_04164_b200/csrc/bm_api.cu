@@ -36,7 +36,7 @@ static const OptDef kOptDefs[OPT_COUNT] = {
     {"GEMV_ROWS", 1}, {"GEMV_MAX_T", 2}, {"GEMV_FUSE", 1}, {"DC_RMAX", 128}, {"DC_KS_FORCE", 0}, {"DC_STAGES", 12},
     {"PF_STAGES", 12}, {"DC_R1", 0}, {"DC_R2", 0}, {"DC_KS2", 1}, {"PF_PAIR", -1}, {"PF_GATHER", 1},
     {"COMBINE_WARPS", 64}, {"PERM_SMALL_WARPS", 0}, {"ROUTER_WE", 0}, {"ROUTER_TP_MIN_T", kSplitRouterMaxT},
-    {"ROUTER_SPLIT_MAX_T", 16}, {"FUSED_COMBINE", -1}, {"PF_G1_BC", -1}, {"PF_G2_BC", -1}, {"PF_G2_BW", -1}, {"PF_G1_HINTS", -1}, {"PF_G2_HINTS", -1}, {"DC_DENSE_MAX_T", kDenseMaxT}, {"DC_PREFETCH_MB", 48}, {"DC_KPACK", 2}, {"ROUTER_FILTER", 1}, {"HOST_CHUNK_T", -1}, {"LAYER_SMALL", 1}, {"PERM_CLUSTER", 1}, {"DC_SPEC_US", 12}, {"DC_SPEC_MIN_ROWS", 1},
+    {"ROUTER_SPLIT_MAX_T", 16}, {"FUSED_COMBINE", -1}, {"PF_G1_BC", -1}, {"PF_G2_BC", -1}, {"PF_G2_BW", -1}, {"PF_G1_HINTS", -1}, {"PF_G2_HINTS", -1}, {"DC_DENSE_MAX_T", kDenseMaxT}, {"DC_PREFETCH_MB", 48}, {"DC_KPACK", 2}, {"ROUTER_FILTER", 1}, {"HOST_CHUNK_T", -1}, {"LAYER_SMALL", 1}, {"PERM_CLUSTER", 1}, {"DC_SPEC_US", 12}, {"DC_SPEC_MIN_ROWS", 1}, {"PF_SPEC", 1},
 };
 static int g_opt[OPT_COUNT];
 static bool init_options() {
@@ -501,16 +501,17 @@ static HostPipe *host_pipe() {
 }
 
 // Token chunks of bm_moe_layer_host: equal chunks of whole 128-row tiles, about HOST_CHUNK_T tokens each, from two chunks on.
-// The pipeline hides every copy except the first chunk's way in and the last chunk's way out, but a chunk must stay large
-// enough to keep the tiles efficient -- BJ:configs[2]'s layer takes 0.53 us per token at T = 8192, 0.55 at 4096, 0.63 at 2048
-// and 1.03 at 512 (its 1.4 GB of weights stream once per chunk).  Measured there, end to end: one piece 6.12 ms, 2 x 4096
-// 5.21, 4 x 2048 5.36, 8 x 1024 6.34; chunks growing from a small first one towards the middle and shrinking again (512,
-// 1536, 4096, 1536, 512: the exposed copies shrink 4x) 5.54 -- the small chunks cost more than their copies save.  So: 4096
-// tokens where a token computes at least twice as long as it copies (6 D F (K + S) flops at ~1.3 PFLOP/s against 2 D bytes at
-// ~50 GB/s: F (K + S) >= 17400), 2048 elsewhere (Qwen-like shapes: copies as long as compute).  Returns the number of chunks.
+// The pipeline hides every copy except the first chunk's way in and the last chunk's way out, but every chunk streams the
+// layer's weights once more -- BJ:configs[2]'s layer takes 0.51 us per token plus ~210 us per call (1.4 GB of weights): 0.53
+// us per token at T = 8192, 0.55 at 4096, 0.63 at 2048, 1.03 at 512.  Measured there, end to end (ms, two boxes): one piece
+// 6.12 / 6.08, 8 x 1024 6.34 / 6.25, 4 x 2048 5.36 / 5.26, 3 x 2816 - / 5.01, 2 x 4096 5.21 / 5.11; chunks growing from a small
+// first one towards the middle and shrinking again (512, 1536, 4096, 1536, 512: the exposed copies shrink 4x) 5.54 -- small
+// chunks cost more than their copies save.  So: 2816 tokens (22 tiles) where a token computes at least twice as long as it
+// copies (6 D F (K + S) flops at ~1.3 PFLOP/s against 2 D bytes at ~50 GB/s: F (K + S) >= 17400), 2048 elsewhere (Qwen-like
+// shapes: copies as long as compute).  Returns the number of chunks.
 static int host_chunk_plan(int T, int F, int K, int S, int *sizes) {
     int chunk_t = opt(OPT_HOST_CHUNK_T);
-    if (chunk_t < 0) chunk_t = (long long)F * (K + S) >= 17400 ? 4096 : 2048;
+    if (chunk_t < 0) chunk_t = (long long)F * (K + S) >= 17400 ? 2816 : 2048;
     sizes[0] = T;
     if (chunk_t == 0 || T < 2 * chunk_t) return 1;
     int pieces = (T + chunk_t - 1) / chunk_t;

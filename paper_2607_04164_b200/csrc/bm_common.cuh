@@ -121,7 +121,7 @@ enum Opt {
     OPT_PDL, OPT_DECODE_MAX_T, OPT_DECODE_MID_T, OPT_DECODE_ROWS, OPT_DECODE_MID_ROWS, OPT_GEMV_ROWS, OPT_GEMV_MAX_T,
     OPT_GEMV_FUSE, OPT_DC_RMAX, OPT_DC_KS_FORCE, OPT_DC_STAGES, OPT_PF_STAGES, OPT_DC_R1, OPT_DC_R2, OPT_DC_KS2,
     OPT_PF_PAIR, OPT_PF_GATHER, OPT_COMBINE_WARPS, OPT_PERM_SMALL_WARPS, OPT_ROUTER_WE, OPT_ROUTER_TP_MIN_T,
-    OPT_ROUTER_SPLIT_MAX_T, OPT_FUSED_COMBINE, OPT_PF_G1_BC, OPT_PF_G2_BC, OPT_PF_G2_BW, OPT_PF_G1_HINTS, OPT_PF_G2_HINTS, OPT_DC_DENSE_MAX_T, OPT_DC_PREFETCH_MB, OPT_DC_KPACK, OPT_ROUTER_FILTER, OPT_HOST_CHUNK_T, OPT_LAYER_SMALL, OPT_PERM_CLUSTER, OPT_DC_SPEC_US, OPT_DC_SPEC_MIN_ROWS, OPT_COUNT
+    OPT_ROUTER_SPLIT_MAX_T, OPT_FUSED_COMBINE, OPT_PF_G1_BC, OPT_PF_G2_BC, OPT_PF_G2_BW, OPT_PF_G1_HINTS, OPT_PF_G2_HINTS, OPT_DC_DENSE_MAX_T, OPT_DC_PREFETCH_MB, OPT_DC_KPACK, OPT_ROUTER_FILTER, OPT_HOST_CHUNK_T, OPT_LAYER_SMALL, OPT_PERM_CLUSTER, OPT_DC_SPEC_US, OPT_DC_SPEC_MIN_ROWS, OPT_PF_SPEC, OPT_COUNT
 };
 int opt(Opt o);
 

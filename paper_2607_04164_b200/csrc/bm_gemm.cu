@@ -47,6 +47,8 @@ constexpr int kChunkRows = 128;
 constexpr int kMaxSeg = BM_MAX_G + kMaxShared;
 constexpr size_t kSmemMax = 232448;         // 227 KB, the per-CTA opt-in limit of sm_100
 constexpr size_t kSmemBars = 512;           // (3*kMaxStages + 2*kAccStages) mbarriers + the TMEM base address
+constexpr int kSchedBarSlot = 3 * kMaxStages + 2 * kAccStages + 1 + 3;   // behind the schedule header (3 ints): "schedule built"
+static_assert((kSchedBarSlot + 1) * 8 <= kSmemBars, "barrier block too small");
 constexpr size_t kEpiStageBytes = 32 * 32 * 4;   // PF_GEMM2: per-epilogue-warp transpose buffer (32 rows x 32 fp32)
 constexpr size_t kSmemEpi = 4 * kEpiStageBytes;
 constexpr size_t kSmemRing = kSmemMax - 1024 /*align slack*/ - kSmemBars;   // minus kSmemEpi for PF_GEMM2
@@ -96,6 +98,7 @@ struct GemmParams {
     int y_tm;           // calibration: y is token-major [T, S, D] (row of shared set j, token t = t * S + j)
     int dense_u;        // dense decode with G <= T*K: H rows are indexed by the weight set itself (row u * T + t)
     int spec_sets;      // DC_GEMM1, dense_u: routed sets 0 .. spec_sets-1 are multiplied BEFORE the routing is known
+    int spec_shared;    // PF_GEMM1: the S shared experts' items (all T tokens, no routing needed) run BEFORE the routing is known
     bm_bf16 *out;       // fused combine: the layer output [T, D] bf16 ...
     float *out_f32;     // ... or, when non-null, the fp32 sums (tensor-parallel partial)
 };
@@ -203,7 +206,7 @@ __device__ __forceinline__ void build_schedule(const GemmParams &p, int32_t *s_s
                 if (p.dense && rows > 0) rows = p.T;
                 if (u < p.spec_sets) rows = 0;          // done ahead of the routing (DC_GEMM1 only)
             } else {
-                rows = p.T;
+                rows = p.spec_shared ? 0 : p.T;         // (PF_GEMM1 only: done ahead of the routing)
             }
         }
         const bool ne = rows > 0;
@@ -295,7 +298,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
         // GA: a stage is full when the TMA bytes (weights) have landed AND the relay warp (both CTAs' under K2) has signalled that the gathered rows are in place
         for (int i = 0; i < n_stages; ++i) { ptx::mbar_init(&full[i], GA ? 1 + (K2 ? 2 : 1) : 1); ptx::mbar_init(&empty[i], 1); }
         if (GA) for (int i = 0; i < n_stages; ++i) ptx::mbar_init(&gfull[i], kGatherCopyThreads);
-        if (MODE == DC_GEMM1) ptx::mbar_init(&gfull[0], 1);      // "schedule built" (speculative start, below)
+        if (kGemm1) ptx::mbar_init(bars + kSchedBarSlot, 1);     // "schedule built" (speculative start, below)
         // K2: the leader's tempty collects the 4 epilogue warps of BOTH CTAs
         for (int i = 0; i < kAccStages; ++i) { ptx::mbar_init(&tfull[i], 1); ptx::mbar_init(&tempty[i], K2 ? 8 : 4); }
         ptx::fence_barrier_init();
@@ -367,9 +370,14 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
     // bandwidth that nobody else wanted.  Item numbers below n_spec are synthesised by fetch(); the first request beyond
     // makes the producer warp wait for the routing, build the schedule and release the other warps through an mbarrier.
     // The dependent grid (GEMM2) is let go only then, so "GEMM1 let GEMM2 start => the routing is complete" still holds.
-    const bool spec = MODE == DC_GEMM1 && p.spec_sets > 0;
-    const int n_spec = spec ? p.spec_sets * p.n_wtiles : 0;
-    uint64_t *sched_bar = gfull;
+    // PF_GEMM1 has the same start for the S shared experts (spec_shared): their items take all T tokens straight from x and
+    // write H rows that no routed item touches, so they run while the router, the permutation and the gather pass are
+    // still at work -- at BJ:configs[3] (two shared experts: 30% of the rows) that hides most of the routing chain.  The
+    // kernels of that chain let their successor start before their own wait, so that this grid is resident early.
+    const bool spec = (MODE == DC_GEMM1 && p.spec_sets > 0) || (MODE == PF_GEMM1 && p.spec_shared != 0);
+    const int pf_units = K2 ? ((p.T + kChunkRows - 1) / kChunkRows + 1) >> 1 : (p.T + kChunkRows - 1) / kChunkRows;
+    const int n_spec = !spec ? 0 : MODE == DC_GEMM1 ? p.spec_sets * p.n_wtiles : p.S * pf_units * p.n_wtiles;
+    uint64_t *sched_bar = bars + kSchedBarSlot;
     if (!spec) {
         grid_dep_wait();
         if (kGemm1 && warp == 0) build_schedule(p, s_sched, cap, s_hdr);
@@ -379,10 +387,25 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
     }
     bool sched_seen = !spec;
     auto fetch = [&](int item, Item &it) -> bool {         // warp-uniform
-        if (MODE == DC_GEMM1 && spec) {
+        if ((MODE == DC_GEMM1 || MODE == PF_GEMM1) && spec) {
             if (item < n_spec) {
-                it.u = item / p.n_wtiles; it.wt = item - it.u * p.n_wtiles; it.ks = 0;
-                it.n = p.T; it.act_row0 = 0; it.tok0 = 0; it.perm_row0 = 0; it.h_row0 = it.u * p.T; it.shared = false;
+                if (MODE == DC_GEMM1) {
+                    it.u = item / p.n_wtiles; it.wt = item - it.u * p.n_wtiles; it.ks = 0;
+                    it.n = p.T; it.act_row0 = 0; it.tok0 = 0; it.perm_row0 = 0; it.h_row0 = it.u * p.T; it.shared = false;
+                } else {
+                    // shared expert j, (chunk unit, weight tile) in get_item's order: unit fastest
+                    const int per_set = pf_units * p.n_wtiles;
+                    const int j = item / per_set, local = item - j * per_set;
+                    it.wt = local / pf_units;
+                    int chunk = local - it.wt * pf_units;
+                    if (K2) chunk = 2 * chunk + (int)rank;
+                    it.n = min(kChunkRows, p.T - chunk * kChunkRows);
+                    if (it.n <= 0) { it.n = 0; chunk = 0; }          // absent half of the last pair: point at real rows
+                    it.u = p.G + j; it.ks = 0; it.shared = true; it.perm_row0 = 0;
+                    it.tok0 = chunk * kChunkRows;
+                    it.h_row0 = p.TK + j * p.T + it.tok0;
+                    it.act_row0 = it.tok0;
+                }
                 return true;
             }
             if (!sched_seen) {
@@ -923,8 +946,8 @@ gemm_kernel(const __grid_constant__ CUtensorMap tm_act0,   // GEMM1: xs [TK, D];
 __global__ void __launch_bounds__(256)
 gather_kernel(const bm_bf16 *__restrict__ x, int T, int D, int K, int G, const int32_t *__restrict__ offsets,
               const int32_t *__restrict__ row_token, bm_bf16 *__restrict__ xs) {
+    grid_dep_launch();     // GEMM1 may be resident (and at work on the shared experts) before this pass has run; it waits for it
     grid_dep_wait();
-    grid_dep_launch();
     const int A = min(max(offsets[G], 0), T * K);
     const int warps = (gridDim.x * blockDim.x) >> 5;
     const int lane = threadIdx.x & 31;
@@ -1389,6 +1412,9 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
         // (with single-CTA tiles a group has at most ~2 chunks: its weights stream once -> evict_first, as on the decode path;
         //  G = 8, T = 256: 69 -> 64 us)
         p.hints = opt(OPT_PF_G1_HINTS) >= 0 ? opt(OPT_PF_G1_HINTS) : (pair ? 21 : 20);
+        // shared experts ahead of the routing (gemm_kernel, "speculative start"): inside bm_moe_layer only -- there the
+        // routing kernels are known to be this launch's predecessors and to let it start early
+        p.spec_shared = a.after_router && a.S > 0 && opt(OPT_PF_SPEC) != 0 ? 1 : 0;
         if (gather_in_gemm)
             err = pair ? launch_gemm<PF_GEMM1, true, true>(m_xs, m_x, m_w1, m_w3, p, stream)
                        : launch_gemm<PF_GEMM1, false, true>(m_xs, m_x, m_w1, m_w3, p, stream);
@@ -1397,6 +1423,7 @@ cudaError_t launch_forward_tc(const ForwardArgs &a, bool decode, cudaStream_t st
                        : launch_gemm<PF_GEMM1>(m_xs, m_x, m_w1, m_w3, p, stream);
         if (err != cudaSuccess) return err;
         p.kblocks = kb2; p.R = 256; p.n_wtiles = (a.D + 255) / 256;
+        p.spec_shared = 0;
         p.band_w = opt(OPT_PF_G2_BW) > 0 ? opt(OPT_PF_G2_BW) : 0;
         p.band_c = opt(OPT_PF_G2_BC) > 0 ? opt(OPT_PF_G2_BC) : 0;
         p.hints = opt(OPT_PF_G2_HINTS) >= 0 ? opt(OPT_PF_G2_HINTS) : (pair ? 21 : 20);

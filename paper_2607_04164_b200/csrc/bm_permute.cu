@@ -52,8 +52,8 @@ __global__ void __launch_bounds__(kWarps * 32)
 permute_hist_kernel(const int32_t *__restrict__ group_ids, int T, int K, int G,
                     int32_t *__restrict__ block_hist) {
     extern __shared__ int s_mem[];
+    grid_dep_launch();     // (not the first kernel of a call: the successor waits for this grid itself)
     grid_dep_wait();
-    grid_dep_launch();
     int *whist = s_mem;                  // [kWarps][G]
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long items = (long long)T * K;
@@ -75,8 +75,8 @@ permute_scan_kernel(int nb, int G, int32_t *__restrict__ block_hist, int32_t *__
     __shared__ int gsum[512];
     __shared__ int tmp[512];
     __shared__ int s_total;
+    grid_dep_launch();     // (not the first kernel of a call: the successor waits for this grid itself)
     grid_dep_wait();
-    grid_dep_launch();
     // block_hist[b][u] := rows of group u in blocks before b (the scatter kernel adds offsets[u]).  Thread u
     // walks the blocks eight at a time: eight independent loads, then the running sums and eight stores --
     // one memory round trip per eight blocks instead of one per block (the first version took 8 us at 12
@@ -108,8 +108,8 @@ permute_scatter_kernel(const int32_t *__restrict__ group_ids, int T, int K, int 
                        int32_t *__restrict__ row_token, int32_t *__restrict__ row_slot,
                        int32_t *__restrict__ slot_row) {
     extern __shared__ int s_mem[];
+    grid_dep_launch();     // (not the first kernel of a call: the successor waits for this grid itself)
     grid_dep_wait();
-    grid_dep_launch();
     int *whist = s_mem;                  // [kWarps][G]
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long items = (long long)T * K;
@@ -138,7 +138,7 @@ permute_scatter_kernel(const int32_t *__restrict__ group_ids, int T, int K, int 
 // second read for the replay), the CTAs publish their per-group counts in shared memory, and after one cluster barrier
 // every CTA reads the other seven through distributed shared memory: counts, offsets and its own bases follow without a
 // trip through global memory.  A second cluster barrier keeps every CTA's counts alive until all peers have read them.
-constexpr int kClSize = 8, kClWarps = 32, kClMaxRounds = 8;
+constexpr int kClSize = 8, kClWarps = 16, kClMaxRounds = 16;
 constexpr long long kPermClusterItems = (long long)kClSize * kClWarps * kClMaxRounds * 32;      // 65536
 
 __device__ __forceinline__ int ld_shared_cluster(uint32_t addr) {
@@ -157,8 +157,8 @@ permute_cluster_kernel(const int32_t *__restrict__ group_ids, int T, int K, int 
     int *whist = s_mem;                      // [kClWarps][G]: counts, then bases of this CTA's warps
     int *ctot = whist + kClWarps * G;        // [G] this CTA's counts, read by its peers
     int *gsum = ctot + G;                    // [G] group totals -> offsets
+    grid_dep_launch();     // (not the first kernel of a call: the successor waits for this grid itself)
     grid_dep_wait();
-    grid_dep_launch();
     const int rank = (int)ptx::cluster_ctarank();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long items = (long long)T * K;

@@ -764,8 +764,10 @@ router_refine_kernel(const bm_bf16 *__restrict__ x, int T, int D, const bm_bf16 
                      int mask_words, int32_t *__restrict__ expert_ids, int32_t *__restrict__ group_ids,
                      float *__restrict__ gate_w, int32_t *__restrict__ n_slots, int32_t *__restrict__ status) {
     extern __shared__ float s_rl[];       // [kWarps][E]
-    grid_dep_wait();
+    // (never the first kernel of a call: its successor may be resident early -- it waits for this grid itself; see
+    //  gemm_kernel's speculative start)
     grid_dep_launch();
+    grid_dep_wait();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     float *l = s_rl + (size_t)warp * E;
     const int n_warps = gridDim.x * kWarps;

@@ -116,11 +116,11 @@ def test_forward_info_is_a_host_call():
 
 def test_host_chunk_plan_is_a_host_call():
     """bm_host_chunks (include/bm.h, bm_moe_layer_host): chunks cover the batch exactly, at most 16, whole 128-row tiles
-    except the last; about 4096 tokens where compute outweighs the copies, 2048 elsewhere."""
+    except the last; about 2816 tokens where compute outweighs the copies, 2048 elsewhere."""
     import paper_2607_04164_b200 as bm
-    assert bm.bm_host_chunks(8192, 14336, 2, 0) == [4096, 4096]
-    assert bm.bm_host_chunks(8191, 14336, 2, 0) == [8191]                                      # below two chunks: one piece
-    assert bm.bm_host_chunks(16384, 14336, 2, 0) == [4096] * 4
+    assert bm.bm_host_chunks(8192, 14336, 2, 0) == [2816, 2816, 2560]
+    assert bm.bm_host_chunks(5631, 14336, 2, 0) == [5631]                                      # below two chunks: one piece
+    assert bm.bm_host_chunks(16384, 14336, 2, 0) == [2816] * 5 + [2304]
     assert bm.bm_host_chunks(64, 14336, 2, 0) == [64]
     assert bm.bm_host_chunks(8192, 1408, 4, 0) == [2048] * 4                                   # copies ~ compute: smaller chunks
     assert bm.bm_host_chunks(4095, 1408, 4, 4) == [4095]

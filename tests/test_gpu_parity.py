@@ -440,6 +440,38 @@ def test_dense_decode_speculative_start(T, D, F, E, K, G, S, dead, spec_us):
             assert_out_close(out.float().cpu().numpy().astype(np.float64), want)
 
 
+@pytest.mark.parametrize("T,D,F,E,K,G,S", [
+    (700, 512, 320, 12, 3, 4, 2),          # CTA pairs (many rows per group), T = 5.5 chunks: the last pair is half empty
+    (900, 264, 1000, 24, 2, 12, 1),        # single-CTA tiles gathering their own rows, ragged D and F
+    (1300, 256, 4096, 8, 2, 4, 3),         # fused combine (F >= 4096), three shared experts
+    (513, 128, 72, 16, 4, 16, 16),         # S = BM_MAX_S: the shared experts are most of the work
+])
+@pytest.mark.parametrize("opts", [dict(PF_SPEC=1), dict(PF_SPEC=0), dict(PF_SPEC=1, PF_PAIR=1, PF_GATHER=0),
+                                  dict(PF_SPEC=1, PF_PAIR=0, PF_GATHER=1), dict(PF_SPEC=1, PF_PAIR=1, PF_GATHER=2)],
+                         ids=["auto", "off", "pairs", "single", "pairs-gather"])
+def test_prefill_shared_experts_ahead_of_the_routing(T, D, F, E, K, G, S, opts):
+    """bm_moe_layer on prefill batches with shared experts: GEMM1 runs the shared experts' items (all tokens, no routing
+    needed) before it waits for the routing kernels (option PF_SPEC).  Same result as without: routing bit-exact, out inside
+    the tolerance, status clean, repeated calls on one workspace."""
+    import paper_2607_04164_b200 as bm
+    rng = np.random.default_rng(T + 31 * S)
+    L = rand_layer(rng, T=T, D=D, F=F, E=E, K=K, G=G, S=S, bias=True, wstd=0.02 if max(D, F) >= 1024 else 0.05)
+    d = to_device(L)
+    o = oracle_route(L)
+    want = oracle_forward(L, o)
+    assert bm.bm_forward_info(T, K, G, S, D, F)[0] == bm.BM_PATH_PREFILL
+    ws = bm.alloc_workspace(T, D, F, E, K, G, S)
+    r = bm.Routing(T, K, G)
+    with bm.options(**opts):
+        for _ in range(3):
+            out = torch.full((T, D), float("nan"), dtype=torch.bfloat16, device="cuda")
+            bm.bm_moe_layer(d.x, d.W_router, d.router_bias, K, d.group_map, G, d.W1, d.W3, d.W2, out, r, ws, S=S)
+            torch.cuda.synchronize()
+            assert bm.bm_device_status(ws) == 0
+            assert_routing_equal(routing_to_numpy(r, T), o)
+            assert_out_close(out.float().cpu().numpy().astype(np.float64), want)
+
+
 # ---------------------------------------------------------------------------------------------------
 # bm_moe_layer_host: the end-to-end call (pinned host x -> host out); the data changes between calls, the
 # buffers do not
