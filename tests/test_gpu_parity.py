@@ -472,6 +472,50 @@ def test_prefill_shared_experts_ahead_of_the_routing(T, D, F, E, K, G, S, opts):
             assert_out_close(out.float().cpu().numpy().astype(np.float64), want)
 
 
+@pytest.mark.parametrize("seed", range(16))
+def test_random_shapes_single_call(seed):
+    """Random shapes through bm_moe_layer -- the call in which GEMM1 may start ahead of the routing kernels (dense decode
+    sets, shared experts on the prefill tiles), the permutation may be one cluster launch and the routing-chain kernels let
+    their successors start early -- with those features on, forced to the maximum, and off; some groups starved of tokens.
+    (A 3000-shape run of the same recipe passed on the round's final tree.)"""
+    import paper_2607_04164_b200 as bm
+    rng = np.random.default_rng(7000 + seed)
+    kind = seed % 4
+    if kind == 0:       # small decode batches: dense GEMM1 + speculative start
+        T = int(rng.integers(3, 65)); E = int(rng.integers(4, 70)); K = int(rng.integers(1, min(E, 8) + 1)); G = int(rng.integers(1, min(E, T * K) + 1))
+    elif kind == 1:     # mid batches: gathered decode / prefill tiles
+        T = int(rng.integers(65, 700)); E = int(rng.integers(2, 70)); K = int(rng.integers(1, min(E, 8) + 1)); G = int(rng.integers(1, E + 1))
+    elif kind == 2:     # prefill tiles with shared experts
+        T = int(rng.integers(400, 2600)); E = int(rng.integers(8, 70)); K = int(rng.integers(1, 7)); G = int(rng.integers(1, E + 1))
+    else:
+        T = int(rng.integers(1, 1500)); E = int(rng.integers(2, 130)); K = int(rng.integers(1, min(E, 16) + 1)); G = int(rng.integers(1, E + 1))
+    D = int(rng.choice([64, 72, 128, 264, 512]))
+    F = int(rng.choice([64, 72, 264, 384, 1000]))
+    S = int(rng.integers(1, 4)) if kind == 2 else int(rng.integers(0, 3))
+    L = rand_layer(rng, T=T, D=D, F=F, E=E, K=K, G=G, S=S, bias=True, wstd=0.02 if max(D, F) >= 512 else 0.05)
+    if seed % 3 == 0 and G > 1:                                    # starve a third of the groups
+        gm = L.group_map.numpy()
+        dead = set(rng.integers(0, G, size=max(1, G // 3)).tolist())
+        if len(dead) < G:
+            for e in range(E):
+                if int(gm[e]) in dead:
+                    L.router_bias[e] = -1.0e4
+    o = oracle_route(L)
+    want = oracle_forward(L, o)
+    d = to_device(L)
+    ws = bm.alloc_workspace(T, D, F, E, K, G, S)
+    r = bm.Routing(T, K, G)
+    for opts in (dict(), dict(DC_SPEC_US=100000), dict(PF_SPEC=0, DC_SPEC_US=0, PERM_CLUSTER=0)):
+        with bm.options(**opts):
+            for _ in range(2):
+                out = torch.full((T, D), float("nan"), dtype=torch.bfloat16, device="cuda")
+                bm.bm_moe_layer(d.x, d.W_router, d.router_bias, K, d.group_map, G, d.W1, d.W3, d.W2, out, r, ws, S=S)
+                torch.cuda.synchronize()
+                assert bm.bm_device_status(ws) == 0, opts
+                assert_routing_equal(routing_to_numpy(r, T), o)
+                assert_out_close(out.float().cpu().numpy().astype(np.float64), want)
+
+
 # ---------------------------------------------------------------------------------------------------
 # bm_moe_layer_host: the end-to-end call (pinned host x -> host out); the data changes between calls, the
 # buffers do not
